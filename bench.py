@@ -1,0 +1,321 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the LEDDS hot path on B200.
+
+A "step" is one pass of the whole hot path: one coupled LBM-DEM step of
+BASELINE.json configs[3] (256^3 D3Q19 BGK lattice, periodic x/y, moving z walls, 20 000 spheres of
+radius 4 placed by seeded RSA, PSM coupling, n_sub = 1).  The headline value is MLUPS from the
+total time per step including DEM and coupling (the paper's own definition).
+Sub-benchmarks (configs[1] LBM-only MLUPS, configs[4] DEM-only particle-updates/s) are reported in
+the same JSON line under "sub".  Multi-GPU (N > 1, torchrun) = independent replicas, no collective
+on the data path ("replicas only").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg4|cfg2|cfg5|small]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "D3Q19 MLUPS of the coupled LBM-DEM step (total time per step incl. DEM and coupling)"
+
+
+def peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"], "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        out = self.p.communicate()[0]
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            c = [v.strip() for v in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------- workloads
+def make_cfg4(small=False):
+    import workloads as W
+    if small:
+        return W.cfg4_shear(seed=4, n=128, n_part=2500, R=4.0)
+    return W.cfg4_shear()
+
+
+def coupled_bytes_per_step(n_cells, n_part, solid_cells):
+    """Algorithmic HBM bytes of the dominant (PSM stream-collide) kernel per launch, DESIGN.md section 6:
+    304 B per cell + 48 B written per (cell, solid) partial."""
+    return 304.0 * n_cells + 48.0 * solid_cells
+
+
+def run_ours(args, rank, world):
+    import torch
+    import torch.distributed as dist
+    import paper_2512_04997_b200 as L
+    from paper_2512_04997_b200 import Coupled, Dem, Lbm
+    import workloads as W
+
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    K, Wm = args.steps, args.warmup
+    peak, peak_src = peaks()
+    launches0 = L.ledds_launch_count()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, k):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(); fn(k); e1.record()
+        barrier()
+        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    out = {}
+    # ------------------------------------------------------------------ main: coupled step, configs[3]
+    small = args.workload == "small"
+    lbm, cpl, pd, x, v, w, R, u = make_cfg4(small)
+    n_cells = int(np.prod(lbm["shape"])); n_part = len(R)
+    g_lbm = Lbm(lbm, None, u)
+    g_dem = Dem(pd, x, v, w, R)
+    g = Coupled(g_lbm, g_dem, cpl, float(R.max()))
+    g.step(Wm)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local) if rank == 0 else None
+    L.ledds_profile(True)
+    l0 = L.ledds_launch_count()
+    ms = timed(g.step, K)
+    launches = L.ledds_launch_count() - l0
+    prof = {name: L.ledds_profile_read(i) for i, name in enumerate(L.KERNEL_GROUPS)}
+    L.ledds_profile(False)
+    clocks = sampler.stop() if sampler else None
+    status = int(g_dem.status[0].item())
+    ms_step = ms / K
+    mlups = world * n_cells / ms_step / 1e3
+    # number of (cell, solid) partials: cells within R + R_c of a sphere centre ~ 4/3 pi (R+Rc)^3 per sphere
+    solid_cells = n_part * 4.0 / 3.0 * np.pi * (float(R.max()) / cpl["dx"] + 0.62035) ** 3
+    k_ms, k_n = prof["lbm"]
+    k_ms_avg = k_ms / max(k_n, 1)
+    bytes_launch = coupled_bytes_per_step(n_cells, n_part, solid_cells)
+    achieved = bytes_launch / (k_ms_avg * 1e-3) / 1e9 if k_ms_avg > 0 else 0.0
+    out.update({
+        "metric": METRIC, "value": round(mlups, 1), "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": round(ms_step, 5), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[3] coupled shear: 256^3 D3Q19 BGK tau=0.6, periodic xy, walls z +-0.05, "
+                               "20000 spheres R=4 (RSA seed 4), PSM coupling, n_sub=1" if not small else
+                               "SMALL stand-in (128^3, 2500 spheres) -- not the headline configuration",
+                   "lattice": list(lbm["shape"]), "particles": n_part, "l2": "inputs exceed L2 (5.1 GB of populations)",
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "coupled_steps_per_s": round(world * 1e3 / ms_step, 2),
+        "particle_updates_per_s": round(world * n_part * cpl["n_sub"] * 1e3 / ms_step, 1),
+        "gpu_launches": int(launches),
+        "status_word": status,
+        "kernel_ms_per_step": {k: round(vv[0] / K, 5) for k, vv in prof.items()},
+        "roofline": {"bound": "hbm", "kernel": "lbm_psm_kernel", "achieved": round(achieved, 1), "peak": peak,
+                     "peak_source": peak_src, "unit": "GB/s", "frac": round(achieved / peak, 4),
+                     "bytes_per_launch": bytes_launch, "kernel_ms": round(k_ms_avg, 5),
+                     "share_of_step": round(k_ms_avg / ms_step, 4), "traffic": args.traffic},
+        "clocks": clocks,
+    })
+
+    # ------------------------------------------------------------------ e2e through the public API with HOST buffers
+    if rank == 0 or world > 1:
+        e2e_steps = max(1, min(K, args.e2e_steps))
+        f_host = torch.empty(19 * n_cells, dtype=torch.float64).pin_memory()
+        f_dev_view = torch.empty(19 * n_cells, dtype=torch.float64, device="cuda")
+        L.ledds_lbm_export(g_lbm.h, g_lbm.f, f_dev_view, None, None)
+        f_host.copy_(f_dev_view); torch.cuda.synchronize()
+        hp = {k: getattr(g_dem, k).cpu().pin_memory() for k in ("x", "v", "w", "a", "alpha", "radius")}
+        res = {k: torch.empty_like(hp[k]).pin_memory() for k in ("x", "v", "w")}
+        fh = torch.empty(n_part, 3, dtype=torch.float64).pin_memory()
+        h2d = f_host.numel() * 8 + sum(t.numel() * 8 for t in hp.values())
+        d2h = sum(t.numel() * 8 for t in res.values()) + fh.numel() * 8
+
+        def e2e(k):
+            for _ in range(k):
+                f_dev_view.copy_(f_host, non_blocking=True)
+                L.ledds_lbm_import(g_lbm.h, g_lbm.f, f_dev_view)
+                for kk in ("x", "v", "w", "a", "alpha"):
+                    getattr(g_dem, kk).copy_(hp[kk], non_blocking=True)
+                g.step(1)
+                for kk in ("x", "v", "w"):
+                    res[kk].copy_(getattr(g_dem, kk), non_blocking=True)
+                fh.copy_(g.f_hyd, non_blocking=True)
+                torch.cuda.current_stream().synchronize()
+        e2e(1)
+        ms_e = timed(e2e, e2e_steps) / e2e_steps
+        out["e2e"] = {"value": round(world * n_cells / ms_e / 1e3, 1), "unit": "MLUPS", "ms_per_step": round(ms_e, 4),
+                      "steps": e2e_steps, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                      "what": "per step: populations + particle state from pinned host -> ledds_coupled_step -> "
+                              "particle state + hydrodynamic forces back to host"}
+        del f_host, f_dev_view
+    del g, g_lbm, g_dem
+    torch.cuda.empty_cache()
+
+    # ------------------------------------------------------------------ sub-benchmarks (rank 0 of a 1-GPU run only)
+    sub = {}
+    if world == 1 and not args.no_sub:
+        # configs[1]: LBM-only 128^3 TGV
+        lb, rho, uu = W.cfg2_tgv(128 if not small else 64)
+        gl = Lbm(lb, rho, uu)
+        gl.step(20); torch.cuda.synchronize()
+        ks = 1000 if not small else 100
+        ms2 = timed(gl.step, ks) / ks
+        nc2 = int(np.prod(lb["shape"]))
+        _, r2, u2 = gl.export(want_moments=True)
+        sub["cfg2_lbm_tgv128"] = {"mlups": round(nc2 / ms2 / 1e3, 1), "ms_per_step": round(ms2, 5), "steps": ks,
+                                   "hbm_gbs": round(304.0 * nc2 / ms2 / 1e6, 1), "hbm_frac": round(304.0 * nc2 / ms2 / 1e6 / peak, 4),
+                                   "note": "638 MB of populations (> 126 MB L2); 304 B/cell"}
+        del gl
+        # configs[4]: DEM-only, 4 M polydisperse spheres (jittered-lattice placement), + supplementary dense state
+        for name, dense in (("cfg5_dem_pour_4M", False), ("cfg5_dense_supplement_4M", True)):
+            pd5, x5, v5, w5, R5 = W.cfg5_pour(n_side=160 if not small else 40, n_part=4_000_000 if not small else 64000, dense=dense)
+            gd = Dem(pd5, x5, v5, w5, R5)
+            gd.step(5); torch.cuda.synchronize()
+            L.ledds_profile(True)
+            kd = 50
+            ms5 = timed(gd.step, kd) / kd
+            pr = {nm: round(L.ledds_profile_read(i)[0] / kd, 5) for i, nm in enumerate(L.KERNEL_GROUPS) if nm.startswith("dem")}
+            L.ledds_profile(False)
+            q = torch.zeros(4, dtype=torch.int32, device="cuda")
+            L.ledds_dem_query(gd.h, gd.history, gd.scratch, None, None, None, None, 0, q, None, None)
+            sub[name] = {"particle_updates_per_s": round(len(R5) * 1e3 / ms5, 1), "ms_per_step": round(ms5, 5), "steps": kd,
+                         "particles": len(R5), "contacts": int(q[0].item()), "kernel_ms_per_step": pr,
+                         "status_word": int(gd.status[0].item())}
+            del gd
+            torch.cuda.empty_cache()
+        out["sub"] = sub
+    out["gpu_launches_total"] = int(L.ledds_launch_count() - launches0)
+    if world > 1:
+        dist.destroy_process_group()
+    return out
+
+
+# ----------------------------------------------------------------------------- oracle legs
+def oracle_sample(n_steps, small):
+    """Time the CPU oracle, as it stands, on the same configs[3] state.  Returns (steps/s, sample text, cores, cells)."""
+    import oracle
+    lbm, cpl, pd, x, v, w, R, u = make_cfg4(small)
+    f0 = oracle.lbm_equilibrium(lbm["shape"], None, u)
+    od = oracle.Dem(pd, x, v, w, R)
+    oc = oracle.Coupled(lbm, cpl, od, f0)
+    oc.step(1)                                                   # untimed first touch
+    t0 = time.perf_counter()
+    oc.step(n_steps)
+    dt = time.perf_counter() - t0
+    cores = len(os.sched_getaffinity(0))
+    return n_steps / dt, int(np.prod(lbm["shape"])), cores, len(R)
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return None
+    K, Wm = args.steps, args.warmup
+    small = (K + Wm) > 12 or args.workload == "small"            # bounded sample: full 256^3 only for short runs
+    import oracle
+    lbm, cpl, pd, x, v, w, R, u = make_cfg4(small)
+    n_cells = int(np.prod(lbm["shape"]))
+    f0 = oracle.lbm_equilibrium(lbm["shape"], None, u)
+    oc = oracle.Coupled(lbm, cpl, oracle.Dem(pd, x, v, w, R), f0)
+    oc.step(Wm)
+    t0 = time.perf_counter()
+    oc.step(K)
+    ms_step = (time.perf_counter() - t0) * 1e3 / K
+    cores = len(os.sched_getaffinity(0))
+    mlups = n_cells / ms_step / 1e3
+    sample = ("each step = one coupled oracle step of the full configs[3] state" if not small else
+              "each step = one coupled oracle step of a 1/8-volume stand-in (128^3, 2500 spheres, same solid fraction "
+              "and parameters); MLUPS is size-independent, steps/s is scaled by 1/8")
+    return {"impl": "reference", "metric": METRIC, "value": round(mlups, 3), "unit": "MLUPS", "n_gpus": world, "steps": K,
+            "warmup": Wm, "ms_per_step": round(ms_step, 3), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[3] coupled shear (CPU oracle, oracle/*.c, gcc -O2 -ffp-contract=off -fopenmp)",
+                       "lattice": list(lbm["shape"]), "particles": len(R)},
+            "cpu_baseline": {"value": round(mlups, 3), "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": round(mlups, 3), "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=["cfg4", "small"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--cpu-steps", type=int, default=2)
+    ap.add_argument("--no-sub", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None, help="ncu dram bytes per launch of the dominant kernel, if known")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", 0)); world = int(os.environ.get("WORLD_SIZE", 1))
+    import __graft_entry__ as ge
+    if rank == 0 or "LOCAL_RANK" not in os.environ:
+        ge.build()
+    if args.impl == "reference":
+        line = run_reference(args, rank, world)
+        if line is not None:
+            print(json.dumps(line), flush=True)
+        return
+    if args.traffic is None:
+        # last ncu --set full capture of the dominant kernel, if one is committed (profiles/)
+        try:
+            args.traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))["lbm_psm_kernel"]["dram_bytes_per_launch"]
+        except Exception:
+            args.traffic = None
+    out = run_ours(args, rank, world)
+    if rank == 0:
+        if world == 1 and not args.no_cpu:
+            sps, cells, cores, npart = oracle_sample(args.cpu_steps, args.workload == "small")
+            out["cpu_baseline"] = {"value": round(sps * cells / 1e6, 3), "unit": "MLUPS", "cores": cores, "kind": "oracle",
+                                   "sample": f"{args.cpu_steps} coupled oracle steps of the same state ({cells} cells, {npart} spheres), "
+                                             "after one untimed step", "steps_per_s": round(sps, 4)}
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,188 @@
+/*
+ * ledds.h -- C ABI of libledds.so: the data-parallel hot path of one coupled
+ * Lattice-Boltzmann / Discrete-Element time step of arxiv 2512.04997 (LEDDS),
+ * hand-written CUDA for sm_100a, fp64, one GPU.
+ *
+ * Conventions (all entry points)
+ *   - Returns int: LEDDS_OK or a negative LEDDS_E* code.  Never throws, never aborts.
+ *   - Every array argument is a DEVICE pointer owned by the caller unless it says "host".
+ *     The library allocates NO device memory; sizes come from the *_workspace_bytes queries.
+ *     Device pointers must be 16-byte aligned (LEDDS_EALIGN otherwise).
+ *   - All work is enqueued on the caller's stream (a cudaStream_t passed as void*; NULL = legacy
+ *     default stream) and the call returns without synchronising.
+ *   - Handles (ledds_lbm, ledds_dem) are small HOST structs that hold parameters and step
+ *     parity only; free them with *_destroy.
+ *   - `status` is a caller-owned device int32[4]; word 0 collects asynchronous fault bits
+ *     (LEDDS_ST_*), to be read by the caller after it synchronises.  Words 1..3 are scratch.
+ *   - Particle arrays are in the caller's (unsorted) particle order; vectors are [n][3].
+ *
+ * Lattice (Eq. 22-28): D3Q19, c_s^2 = 1/3, dx = dt = 1.
+ *   Direction numbering (fixed here; the paper leaves it to "any textbook"):
+ *     q : 0      1   2   3   4   5   6    7    8    9    10   11   12   13   14   15   16   17   18
+ *     cx: 0      1  -1   0   0   0   0    1   -1    1   -1    1   -1    1   -1    0    0    0    0
+ *     cy: 0      0   0   1  -1   0   0    1   -1   -1    1    0    0    0    0    1   -1    1   -1
+ *     cz: 0      0   0   0   0   1  -1    0    0    0    0    1   -1   -1    1    1   -1   -1    1
+ *   opposite(q) = q odd ? q+1 : q-1 (q >= 1); weights 1/3 (q=0), 1/18 (1..6), 1/36 (7..18).
+ *   Canonical population layout: f[q*N + (z*ny + y)*nx + x], N = nx*ny*nz, x fastest.
+ *   Lattice node (x,y,z) sits at integer coordinates; a wall lies half a spacing outside the
+ *   outermost nodes (halfway bounce-back).
+ */
+#ifndef LEDDS_H
+#define LEDDS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LEDDS_OK 0
+#define LEDDS_EINVAL (-1)     /* bad size / parameter / null pointer                     */
+#define LEDDS_EALIGN (-2)     /* device pointer not 16-byte aligned                      */
+#define LEDDS_ECAPACITY (-3)  /* a caller-provided buffer or capacity is too small       */
+#define LEDDS_ECUDA (-4)      /* CUDA launch/runtime error (cudaGetLastError is kept)    */
+
+#define LEDDS_ST_CONTACT_OVERFLOW 1 /* a particle had more than max_contacts contacts    */
+#define LEDDS_ST_SOLID_OVERFLOW 2   /* a fluid cell was cut by more than 2 solids        */
+#define LEDDS_ST_COINCIDENT 4       /* two sphere centres coincide (pair skipped)        */
+#define LEDDS_ST_NONFINITE 8        /* a non-finite force was produced                   */
+
+typedef struct ledds_lbm ledds_lbm;
+typedef struct ledds_dem ledds_dem;
+
+/* ------------------------------------------------------------------------------------ LBM
+ * Fused D3Q19 BGK stream-collide, Eq. (22)-(28), boundaries PAPER.md:254. */
+typedef struct {
+    int nx, ny, nz;          /* lattice size, x fastest                                           */
+    double tau;              /* relaxation time in units of dt, > 0.5 (Eq. 27)                    */
+    int bc[3];               /* per axis: 0 periodic, 1 walls (halfway bounce-back) on both sides */
+    double u_wall[3][2][3];  /* wall velocity [axis][side: 0 low, 1 high][component], lattice units;
+                                velocity-modified bounce-back: f -= 6 t_i rho (c_i . u_wall)      */
+    int layout;              /* 0 = two-lattice (f holds 2 x 19 x N doubles).  1 (AA single array)
+                                is reserved: LEDDS_EINVAL in this version                         */
+    int variant;             /* kernel variant: 0 auto, 1 plain push, 2 row-rotate (aligned stores)*/
+} ledds_lbm_params;
+
+/* f_bytes: size of the population buffer the caller must allocate for this layout. */
+int ledds_lbm_workspace_bytes(const ledds_lbm_params* p, size_t* f_bytes);
+
+/* Creates the handle and sets f to the equilibrium (Eq. 28) of rho[N] (NULL -> 1) and
+ * u[3][N] component-major (NULL -> 0).  f: device, f_bytes large. */
+int ledds_lbm_init(ledds_lbm** h, const ledds_lbm_params* p, double* f, const double* rho, const double* u,
+                   void* stream);
+
+/* Loads a canonical population field f_canonical[19*N] as the current state (parity tests). */
+int ledds_lbm_import(ledds_lbm* h, double* f, const double* f_canonical, void* stream);
+
+/* nsteps collide-and-stream steps (Eq. 23-26) in place in the caller's buffer. */
+int ledds_lbm_step(ledds_lbm* h, double* f, int nsteps, void* stream);
+
+/* Current state in canonical layout and/or its moments (Eq. 22); any output may be NULL.
+ * f_canonical[19*N], rho[N], u[3][N]. */
+int ledds_lbm_export(ledds_lbm* h, const double* f, double* f_canonical, double* rho, double* u, void* stream);
+
+/* Pointer (inside f) of the current canonical 19*N field; host-side query, no device work. */
+const double* ledds_lbm_current(const ledds_lbm* h, const double* f);
+
+int ledds_lbm_destroy(ledds_lbm* h);
+
+/* ------------------------------------------------------------------------------------ DEM
+ * One DEM step for spheres, PAPER.md:63-142 (Eq. 1-15), 158-192 (Eq. 18-21), 431-511:
+ *   drift (18a) + predictor -> cell keys on a uniform grid (spacing >= largest diameter,
+ *   PAPER.md:49, 431) -> stable sort of particles by key -> cell ranges -> contact detection
+ *   (Eq. 2, 6) by walking the 27 neighbour cells -> linear spring-dashpot normal/tangential
+ *   force with Coulomb cap (Eq. 4-13), torque (Eq. 15), tangential history carried per contact
+ *    -> per-particle sums (Eq. 1) without global atomics -> kick (18b-c, 19d).
+ * Damping: gamma = 2 zeta sqrt(k m*), zeta = -ln e / sqrt(pi^2 + ln^2 e) (A.5), m* of (A.9).
+ * A wall is a static infinite particle with a surface velocity; its partner id
+ * is n + 2*axis + side. */
+typedef struct {
+    int n;                         /* particles                                                  */
+    double lo[3], hi[3];           /* box                                                        */
+    int bc[3];                     /* 0 periodic, 1 planar walls at lo/hi                        */
+    double v_wall[3][2][3];        /* wall surface velocity [axis][side][component]              */
+    double cell;                   /* requested grid spacing, >= 2 max radius; the grid has
+                                      floor((hi-lo)/cell) cells per axis (>= 3 on periodic axes) */
+    double dt, g[3], density;      /* step, gravity (already buoyancy-corrected, Eq. 56), rho_p  */
+    double kn, kt, restitution, mu;          /* particle-particle spring-dashpot + Coulomb       */
+    double kn_w, kt_w, restitution_w, mu_w;  /* particle-wall                                    */
+    int max_contacts;              /* history slots per particle, 1..32 (walls included)         */
+} ledds_dem_params;
+
+int ledds_dem_workspace_bytes(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes);
+
+/* Creates the handle, clears history/scratch, evaluates the contacts of the initial state with
+ * delta_t = 0 and returns a(0) = F/m + g, alpha(0) = M/I (I = 2/5 m R^2, Eq. 21a).  x, v, w,
+ * radius: in.  a, alpha: out. */
+int ledds_dem_init(ledds_dem** h, const ledds_dem_params* p, const double* x, const double* v, const double* w,
+                   const double* radius, double* a, double* alpha, void* history, void* scratch, int32_t* status,
+                   void* stream);
+
+/* nsteps DEM steps.  f_ext / m_ext: optional extra force / torque per particle ([n][3], may be NULL). */
+int ledds_dem_step(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha, const double* radius,
+                   const double* f_ext, const double* m_ext, void* history, void* scratch, int32_t* status,
+                   int nsteps, void* stream);
+
+/* Results of the last force evaluation, for parity checks.  Any output may be NULL.
+ *   sorted_idx[n]: particle ids ordered by (cell key, id);  sorted_key[n]: their keys;
+ *   pairs[2*pair_cap]: canonical contact list, i < j, sorted lexicographically (walls as j >= n);
+ *   n_pairs[1]: number of contacts (may exceed pair_cap: then only pair_cap are written);
+ *   pair_dt[3*pair_cap]: delta_t of each listed contact, seen from i;
+ *   force[3n], torque[3n]: contact force / torque per particle (Eq. 1), without gravity. */
+int ledds_dem_query(ledds_dem* h, const void* history, const void* scratch, uint32_t* sorted_idx,
+                    uint32_t* sorted_key, uint32_t* pairs, double* pair_dt, uint32_t pair_cap, uint32_t* n_pairs,
+                    double* force, double* torque, void* stream);
+
+int ledds_dem_destroy(ledds_dem* h);
+
+/* -------------------------------------------------------------------------------- coupling
+ * Partially saturated cells: solid fraction Eq. (39)-(40), weights Eq. (36)-(37),
+ * PSM collision Eq. (32)-(35) fused into the stream-collide pass, hydrodynamic force and torque
+ * Eq. (41)-(42) reduced per particle; order of the step PAPER.md:427, 515-532, sub-stepping
+ * PAPER.md:258. */
+typedef struct {
+    int n_sub;            /* DEM sub-steps per LBM step; LBM dt = n_sub * dem.dt                  */
+    int solid_fraction;   /* 0 = distance-based Eq. (39)-(40); others reserved                    */
+    double dx;            /* lattice spacing in DEM length units                                  */
+    double rho_f;         /* fluid reference density in DEM units (lattice rho = 1)               */
+    double origin[3];     /* DEM coordinates of lattice node (0,0,0)                              */
+} ledds_cpl_params;
+
+int ledds_cpl_workspace_bytes(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_params* c,
+                              const double r_max, size_t* cpl_scratch_bytes);
+
+/* nsteps coupled steps.  f_hyd / m_hyd [n][3]: in = hydrodynamic force / torque of the previous
+ * LBM step (zeros before the first), out = those of this step (DEM units).  The DEM grid
+ * spacing must be >= 2 (r_max + 0.6204 dx) so that the solids cutting a fluid cell are found
+ * in the 2x2x2 grid cells around it.  r_max = largest radius (as passed to the workspace query). */
+int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c, double r_max, double* f,
+                       double* x, double* v, double* w, double* a, double* alpha, const double* radius,
+                       double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
+                       int32_t* status, int nsteps, void* stream);
+
+/* ------------------------------------------------------------------------------ measurement
+ * Optional per-kernel timing with CUDA events recorded on the launching stream around each kernel
+ * group, and a count of the kernels this library has launched.  Host-side state, off by default. */
+#define LEDDS_K_LBM 0          /* stream-collide (plain or PSM) */
+#define LEDDS_K_DEM_KEYS 1     /* drift + predictor + cell keys */
+#define LEDDS_K_DEM_SORT 2     /* histogram + radix passes      */
+#define LEDDS_K_DEM_GATHER 3   /* sorted copies + cell ranges   */
+#define LEDDS_K_DEM_CONTACT 4  /* contact detection + forces    */
+#define LEDDS_K_DEM_KICK 5     /* velocity update               */
+#define LEDDS_K_CPL_REDUCE 6   /* per-particle hydrodynamic sum */
+/* enable != 0: start recording (previous records are dropped); 0: stop and drop. */
+int ledds_profile(int enable);
+/* Sum of the recorded durations [ms] and number of recorded launches of one kernel group;
+ * synchronises on the recorded events.  total_ms / launches: host pointers, may be NULL. */
+int ledds_profile_read(int kernel_id, double* total_ms, int* launches);
+/* Number of CUDA kernels launched by this library since it was loaded. */
+unsigned long long ledds_launch_count(void);
+
+/* Library version string (host). */
+const char* ledds_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LEDDS_H */

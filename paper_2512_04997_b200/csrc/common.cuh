@@ -1,0 +1,115 @@
+// Shared declarations of the CUDA path (sm_100a).  Not used by, and shares nothing with, oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/ledds.h"
+
+#define LEDDS_Q 19
+
+// kernel groups for ledds_profile_read (include/ledds.h LEDDS_K_*)
+#define LEDDS_K_COUNT 7
+void ledds_count_launch(int n);
+void ledds_prof_start(int kernel_id, cudaStream_t st);
+void ledds_prof_stop(int kernel_id, cudaStream_t st);
+
+// after every kernel launch: count it and surface launch errors
+#define LEDDS_CHECK_LAUNCH()                                  \
+    do {                                                      \
+        ledds_count_launch(1);                                \
+        if (cudaPeekAtLastError() != cudaSuccess) return LEDDS_ECUDA; \
+    } while (0)
+
+static inline bool ledds_aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+// ---- D3Q19 tables (numbering of include/ledds.h); constexpr so unrolled loops fold them ----
+__host__ __device__ constexpr int lb_cx(int q)
+{
+    constexpr int t[LEDDS_Q] = {0, 1, -1, 0, 0, 0, 0, 1, -1, 1, -1, 1, -1, 1, -1, 0, 0, 0, 0};
+    return t[q];
+}
+__host__ __device__ constexpr int lb_cy(int q)
+{
+    constexpr int t[LEDDS_Q] = {0, 0, 0, 1, -1, 0, 0, 1, -1, -1, 1, 0, 0, 0, 0, 1, -1, 1, -1};
+    return t[q];
+}
+__host__ __device__ constexpr int lb_cz(int q)
+{
+    constexpr int t[LEDDS_Q] = {0, 0, 0, 0, 0, 1, -1, 0, 0, 0, 0, 1, -1, -1, 1, 1, -1, -1, 1};
+    return t[q];
+}
+__host__ __device__ constexpr int lb_opp(int q) { return q == 0 ? 0 : ((q & 1) ? q + 1 : q - 1); }
+__host__ __device__ constexpr double lb_w(int q) { return q == 0 ? 1.0 / 3.0 : (q <= 6 ? 1.0 / 18.0 : 1.0 / 36.0); }
+
+// Kernel-side view of the lattice parameters (passed by value).
+struct LbmDev {
+    int nx, ny, nz;
+    long long N;
+    double omega;          // dt / tau
+    double tau;
+    int bc[3];
+    double uw[18];         // [axis][side][comp]
+    int any_wall_velocity;
+};
+
+struct ledds_lbm {
+    ledds_lbm_params p;
+    LbmDev d;
+    int parity;            // which half of the two-lattice buffer is current (0 or 1)
+    long long steps;
+};
+
+// Kernel-side DEM parameters.
+struct DemDev {
+    int n;
+    double lo[3], hi[3], L[3];
+    int bc[3];
+    double vw[18];
+    int nc[3];
+    double inv_h[3];
+    unsigned ncell;
+    double dt, g[3], density;
+    double kn, kt, zeta, mu;
+    double kn_w, kt_w, zeta_w, mu_w;
+    int maxc;
+};
+
+// Layout of the caller-owned DEM scratch buffer (byte offsets, all 256-B aligned).
+struct DemScratch {
+    size_t key[2], idx[2];         // ping-pong sort buffers (uint32 [n])
+    size_t hist_digit;             // global digit histograms (uint32 [4][256])
+    size_t tile_state;             // look-back descriptors (uint32 [tiles][256])
+    size_t tile_counter;           // dynamic tile ticket (uint32 [4])
+    size_t cell_start, cell_end;   // uint32 [ncell]
+    size_t xs, vps, wps, rs;       // sorted copies: double [n][3] x3, double [n]
+    size_t vp, wp;                 // predictor velocities in particle order: double [n][3]
+    size_t force, torque;          // contact force / torque per particle: double [n][3]
+    size_t pair_count, pair_off;   // query scratch (uint32 [n+1])
+    size_t total;
+};
+
+struct DemHistory {
+    size_t count[2];               // uint32 [n]
+    size_t id[2];                  // uint32 [n][maxc]
+    size_t dt[2];                  // double [n][maxc][3]
+    size_t total;
+};
+
+struct ledds_dem {
+    ledds_dem_params p;
+    DemDev d;
+    DemScratch s;
+    DemHistory hs;
+    int cur;                       // which history buffer holds the latest contacts
+    int sorted_buf;                // which key/idx ping-pong buffer holds the sorted result
+    int key_bits, passes, tiles;
+    long long steps;
+};
+
+// entry points implemented in dem.cu and used by coupled.cu
+int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const double* w, const double* a,
+                               const double* alpha, const double* radius, void* history, void* scratch,
+                               int32_t* status, double dt_hist, bool drift, cudaStream_t st);
+int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha, const double* radius,
+                   const double* f_ext, const double* m_ext, void* scratch, int32_t* status, cudaStream_t st);

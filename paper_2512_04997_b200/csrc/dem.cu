@@ -1,0 +1,752 @@
+// DEM contact pipeline for spheres on sm_100a (Eq. 1-15, 158-192 Eq. 18-21, 431-511).
+//
+//   dem_drift_key_kernel   Eq. (18a) + predictor, cell key of every particle          (map N_part)
+//   dem_hist_kernel        digit histograms of all radix passes in one sweep          (smem histograms)
+//   dem_onesweep_kernel    one stable 8-bit radix pass: per-warp match ranking, chained scan with
+//                          decoupled look-back across tiles, scatter                    (x passes)
+//   dem_gather_kernel      sorted copies of x, v^p, w^p, R + cell start/end from key changes
+//   dem_contact_kernel     27-cell walk, Eq. (2)/(6) test, spring-dashpot + Coulomb + torque per pair,
+//                          history carried in per-particle slots, per-particle sums in registers
+//   dem_kick_kernel        Eq. (18b-c), (19c-d) for spheres
+//
+// Compiled with -fmad=false: the discrete decisions (cell index, delta_n > 0) must not depend on
+// FMA contraction, and none of these kernels is ALU-bound.  No Thrust/CUB; no global fp atomics.
+#include <math.h>
+
+#include <new>
+
+#include "common.cuh"
+
+#define DEM_PI 3.14159265358979323846
+#define SORT_THREADS 256
+#define SORT_WARPS (SORT_THREADS / 32)
+#define SORT_ITEMS 16
+#define SORT_TILE (SORT_THREADS * SORT_ITEMS)
+#define SORT_RADIX 256
+
+#define ST_FLAG_AGG 0x40000000u
+#define ST_FLAG_PRE 0x80000000u
+#define ST_VALUE_MASK 0x3fffffffu
+
+static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+__device__ __forceinline__ double dem_mass(const DemDev& P, double R) { return P.density * (4.0 / 3.0) * DEM_PI * R * R * R; }
+
+// ------------------------------------------------------------------------------ drift + key
+__device__ __forceinline__ int dem_cell_coord(const DemDev& P, double x, int a)
+{
+    int c = (int)floor((x - P.lo[a]) * P.inv_h[a]);
+    c = c < 0 ? 0 : c;
+    return c > P.nc[a] - 1 ? P.nc[a] - 1 : c;
+}
+
+__global__ void dem_drift_key_kernel(const DemDev P, double* __restrict__ x, const double* __restrict__ v,
+                                     const double* __restrict__ w, const double* __restrict__ a,
+                                     const double* __restrict__ alpha, double* __restrict__ vp,
+                                     double* __restrict__ wp, uint32_t* __restrict__ key, uint32_t* __restrict__ idx,
+                                     int drift)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    double xn[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int q = 3 * i + k;
+        double xv = x[q];
+        const double vv = v[q], wv = w[q];
+        if (drift) {
+            const double av = a[q], alv = alpha[q];
+            xv = xv + P.dt * vv + (0.5 * P.dt * P.dt) * av;                 // Eq. (18a)
+            if (!P.bc[k]) {
+                if (xv >= P.hi[k]) xv -= P.L[k];
+                else if (xv < P.lo[k]) xv += P.L[k];
+            }
+            x[q] = xv;
+            vp[q] = vv + (0.5 * P.dt) * av;                                 // predictor (G11)
+            wp[q] = wv + (0.5 * P.dt) * alv;
+        } else {
+            vp[q] = vv;
+            wp[q] = wv;
+        }
+        xn[k] = xv;
+    }
+    const int cx = dem_cell_coord(P, xn[0], 0), cy = dem_cell_coord(P, xn[1], 1), cz = dem_cell_coord(P, xn[2], 2);
+    key[i] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
+    idx[i] = (uint32_t)i;
+}
+
+// ------------------------------------------------------------------------------ radix sort
+// All digit histograms in one pass over the keys (smem atomics, then one global add per bin).
+__global__ void __launch_bounds__(SORT_THREADS) dem_hist_kernel(const uint32_t* __restrict__ key, int n, int passes,
+                                                               uint32_t* __restrict__ ghist)
+{
+    __shared__ uint32_t h[4][SORT_RADIX];
+    for (int t = threadIdx.x; t < 4 * SORT_RADIX; t += blockDim.x) (&h[0][0])[t] = 0;
+    __syncthreads();
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const uint32_t k = key[i];
+        for (int p = 0; p < passes; ++p) atomicAdd(&h[p][(k >> (8 * p)) & 255u], 1u);
+    }
+    __syncthreads();
+    for (int t = threadIdx.x; t < passes * SORT_RADIX; t += blockDim.x) {
+        const uint32_t c = (&h[0][0])[t];
+        if (c) atomicAdd(&ghist[t], c);
+    }
+}
+
+__device__ __forceinline__ uint32_t ld_volatile(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }
+__device__ __forceinline__ void st_volatile(uint32_t* p, uint32_t v) { *reinterpret_cast<volatile uint32_t*>(p) = v; }
+
+// One stable LSD pass (8-bit digit at `shift`).  Tiles take tickets from an atomic counter so that
+// every tile a block waits on is already resident or done.  Order inside a tile = (warp, item, lane)
+// = ascending input index, which keeps the sort stable.
+__global__ void __launch_bounds__(SORT_THREADS) dem_onesweep_kernel(
+    const uint32_t* __restrict__ key_in, const uint32_t* __restrict__ val_in, uint32_t* __restrict__ key_out,
+    uint32_t* __restrict__ val_out, int n, int shift, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
+    uint32_t* __restrict__ tile_state /*[tiles][256] of this pass*/, uint32_t* __restrict__ ticket)
+{
+    __shared__ uint32_t warp_hist[SORT_WARPS][SORT_RADIX];
+    __shared__ uint32_t bin_base[SORT_RADIX];
+    __shared__ uint32_t s_tile;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    for (int t = tid; t < SORT_WARPS * SORT_RADIX; t += SORT_THREADS) (&warp_hist[0][0])[t] = 0;
+    __syncthreads();
+    const uint32_t tile = s_tile;
+
+    // exclusive prefix of the global digit histogram (thread d owns digit d)
+    uint32_t digit_excl;
+    {
+        const uint32_t c = ghist[tid];
+        uint32_t incl = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        __shared__ uint32_t wsum[SORT_WARPS];
+        if (lane == 31) wsum[warp] = incl;
+        __syncthreads();
+        uint32_t base = 0;
+        for (int w2 = 0; w2 < warp; ++w2) base += wsum[w2];
+        digit_excl = base + incl - c;
+    }
+
+    // load (warp-striped) and rank inside the warp
+    uint32_t k[SORT_ITEMS], v[SORT_ITEMS], r[SORT_ITEMS];
+    const long long base = (long long)tile * SORT_TILE + (long long)warp * (SORT_ITEMS * 32);
+#pragma unroll
+    for (int it = 0; it < SORT_ITEMS; ++it) {
+        const long long i = base + it * 32 + lane;
+        const bool ok = i < n;
+        k[it] = ok ? key_in[i] : 0xffffffffu;
+        v[it] = ok ? val_in[i] : 0u;
+        const uint32_t d = ok ? ((k[it] >> shift) & 255u) : 256u;
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t below = __popc(peers & ((1u << lane) - 1u));
+        uint32_t old = 0;
+        if (ok) old = warp_hist[warp][d];
+        __syncwarp();
+        if (ok && below == 0) warp_hist[warp][d] = old + __popc(peers);
+        __syncwarp();
+        r[it] = old + below;
+    }
+    __syncthreads();
+
+    // per digit: exclusive scan over the warps of this tile, then the chained scan over tiles
+    {
+        const int d = tid;
+        uint32_t run = 0;
+#pragma unroll
+        for (int w2 = 0; w2 < SORT_WARPS; ++w2) {
+            const uint32_t c = warp_hist[w2][d];
+            warp_hist[w2][d] = run;
+            run += c;
+        }
+        uint32_t* my = tile_state + (size_t)tile * SORT_RADIX + d;
+        uint32_t excl = 0;
+        if (tile == 0) {
+            st_volatile(my, ST_FLAG_PRE | run);
+        } else {
+            st_volatile(my, ST_FLAG_AGG | run);
+            for (long long t = (long long)tile - 1; t >= 0; --t) {
+                const uint32_t* p = tile_state + (size_t)t * SORT_RADIX + d;
+                uint32_t s;
+                do { s = ld_volatile(p); } while ((s & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0);
+                excl += s & ST_VALUE_MASK;
+                if (s & ST_FLAG_PRE) break;
+            }
+            st_volatile(my, ST_FLAG_PRE | (excl + run));
+        }
+        bin_base[d] = digit_excl + excl;
+    }
+    __syncthreads();
+
+#pragma unroll
+    for (int it = 0; it < SORT_ITEMS; ++it) {
+        const long long i = base + it * 32 + lane;
+        if (i < n) {
+            const uint32_t d = (k[it] >> shift) & 255u;
+            const uint32_t dst = bin_base[d] + warp_hist[warp][d] + r[it];
+            key_out[dst] = k[it];
+            val_out[dst] = v[it];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------ gather + cell ranges
+__global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
+                                  const double* __restrict__ x, const double* __restrict__ vp,
+                                  const double* __restrict__ wp, const double* __restrict__ radius,
+                                  double* __restrict__ xs, double* __restrict__ vps, double* __restrict__ wps,
+                                  double* __restrict__ rs, uint32_t* __restrict__ cell_start,
+                                  uint32_t* __restrict__ cell_end)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const bool ok = s < P.n;
+    const uint32_t key = ok ? skey[s] : 0xffffffffu;
+    // neighbours' keys inside the warp by shuffle, across warps by one extra load
+    uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
+    uint32_t next = __shfl_down_sync(0xffffffffu, key, 1);
+    if (!ok) return;
+    if (lane == 0) prev = s > 0 ? skey[s - 1] : 0xffffffffu;
+    if (lane == 31 || s == P.n - 1) next = s < P.n - 1 ? skey[s + 1] : 0xffffffffu;
+    if (s == 0 || prev != key) cell_start[key] = (uint32_t)s;
+    if (s == P.n - 1 || next != key) cell_end[key] = (uint32_t)s + 1u;
+    const uint32_t p = sidx[s];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        xs[3 * s + k] = x[3 * p + k];
+        vps[3 * s + k] = vp[3 * p + k];
+        wps[3 * s + k] = wp[3 * p + k];
+    }
+    rs[s] = radius[p];
+}
+
+// ------------------------------------------------------------------------------ contact law
+struct Body { double x[3], v[3], w[3], R; };
+
+__device__ __forceinline__ void cross3(const double* a, const double* b, double* c)
+{
+    c[0] = a[1] * b[2] - a[2] * b[1];
+    c[1] = a[2] * b[0] - a[0] * b[2];
+    c[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+// r_i - r_j with the nearest image on periodic axes
+__device__ __forceinline__ void dem_min_image(const DemDev& P, const double* xi, const double* xj, double* d)
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        d[a] = xi[a] - xj[a];
+        if (!P.bc[a]) {
+            if (d[a] > 0.5 * P.L[a]) d[a] -= P.L[a];
+            else if (d[a] < -0.5 * P.L[a]) d[a] += P.L[a];
+        }
+    }
+}
+
+// Force of one contact in its canonical orientation (i < j, or j = wall), Eq. (4)-(15).
+// en, dn: unit normal from j to i and overlap.  dt3: in = previous delta_t, out = new delta_t.
+// F = force on i; T = e_n x F_t (torque on a body of radius R is -R T, Eq. 15).
+__device__ __forceinline__ void dem_pair_force(const double* en, double dn, const double* vi, const double* wi,
+                                               double Ri, const double* vj, const double* wj, double Rj,
+                                               double mstar, double kn, double kt, double zeta, double mu,
+                                               double dt_hist, double* dt3, double* F, double* T)
+{
+    const double gn = 2.0 * zeta * sqrt(kn * mstar), gt = 2.0 * zeta * sqrt(kt * mstar);
+    double rw[3], rwxe[3], vrel[3], vt[3], Ft[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) rw[a] = Ri * wi[a] + Rj * wj[a];
+    cross3(rw, en, rwxe);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) vrel[a] = (vi[a] - vj[a]) - rwxe[a];                  // Eq. (11)
+    const double vn = vrel[0] * en[0] + vrel[1] * en[1] + vrel[2] * en[2];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) vt[a] = vrel[a] - vn * en[a];                         // Eq. (12)
+    const double fn = kn * dn - gn * vn;                                              // Eq. (10)
+    const double dte = dt3[0] * en[0] + dt3[1] * en[1] + dt3[2] * en[2];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) dt3[a] = (dt3[a] - dte * en[a]) + dt_hist * vt[a];    // Eq. (13)
+#pragma unroll
+    for (int a = 0; a < 3; ++a) Ft[a] = -kt * dt3[a] - gt * vt[a];                    // Eq. (4)
+    const double ft = sqrt(Ft[0] * Ft[0] + Ft[1] * Ft[1] + Ft[2] * Ft[2]), fmax = mu * fabs(fn);
+    if (ft > fmax) {                                                                  // Eq. (5)
+        const double s = fmax / ft;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { Ft[a] *= s; dt3[a] = -(Ft[a] + gt * vt[a]) / kt; }
+    }
+    cross3(en, Ft, T);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) F[a] = fn * en[a] + Ft[a];
+}
+
+// One thread per particle, in sorted order.  History slots: [particle][slot] partner id + delta_t as
+// seen from that particle (the partner stores the negated vector).
+__global__ void __launch_bounds__(128) dem_contact_kernel(
+    const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
+    const double* __restrict__ xs, const double* __restrict__ vps, const double* __restrict__ wps,
+    const double* __restrict__ rs, const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ cell_end,
+    const uint32_t* __restrict__ hcount_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
+    uint32_t* __restrict__ hcount_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
+    double* __restrict__ force, double* __restrict__ torque, int32_t* __restrict__ status, double dt_hist)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.n) return;
+    const uint32_t p = sidx[s];
+    const uint32_t key = skey[s];
+    Body me;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { me.x[a] = xs[3 * s + a]; me.v[a] = vps[3 * s + a]; me.w[a] = wps[3 * s + a]; }
+    me.R = rs[s];
+    const double m_me = dem_mass(P, me.R);
+    const int maxc = P.maxc;
+    const uint32_t nprev = hcount_prev[p];
+    const uint32_t* pid = hid_prev + (size_t)p * maxc;
+    const double* pdt = hdt_prev + (size_t)p * maxc * 3;
+    uint32_t* nid = hid_new + (size_t)p * maxc;
+    double* ndt = hdt_new + (size_t)p * maxc * 3;
+
+    double Fs[3] = {0, 0, 0}, Ms[3] = {0, 0, 0};
+    uint32_t ncont = 0;
+    int st = 0;
+
+    const int c0 = (int)(key % (uint32_t)P.nc[0]);
+    const int c1 = (int)((key / (uint32_t)P.nc[0]) % (uint32_t)P.nc[1]);
+    const int c2 = (int)(key / ((uint32_t)P.nc[0] * (uint32_t)P.nc[1]));
+
+    for (int dz = -1; dz <= 1; ++dz) {
+        int qz = c2 + dz;
+        if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) continue; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
+        for (int dy = -1; dy <= 1; ++dy) {
+            int qy = c1 + dy;
+            if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) continue; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
+            for (int dx = -1; dx <= 1; ++dx) {
+                int qx = c0 + dx;
+                if (qx < 0 || qx >= P.nc[0]) { if (P.bc[0]) continue; qx = qx < 0 ? qx + P.nc[0] : qx - P.nc[0]; }
+                const uint32_t cell = (uint32_t)(qx + P.nc[0] * (qy + P.nc[1] * qz));
+                const uint32_t t0 = cell_start[cell], t1 = cell_end[cell];
+                for (uint32_t t = t0; t < t1; ++t) {
+                    if ((int)t == s) continue;
+                    Body ot;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) ot.x[a] = xs[3 * t + a];
+                    ot.R = rs[t];
+                    const uint32_t q = sidx[t];
+                    const bool me_first = p < q;
+                    const Body& bi = me_first ? me : ot;
+                    const Body& bj = me_first ? ot : me;
+                    double d[3];
+                    dem_min_image(P, bi.x, bj.x, d);
+                    const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+                    const double dn = (bi.R + bj.R) - dist;                            // Eq. (6)
+                    if (!(dn > 0.0)) continue;                                         // Eq. (2), strict
+                    if (dist == 0.0) { st |= LEDDS_ST_COINCIDENT; continue; }
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) { ot.v[a] = vps[3 * t + a]; ot.w[a] = wps[3 * t + a]; }
+                    double en[3] = {d[0] / dist, d[1] / dist, d[2] / dist};            // Eq. (7)
+                    const double mi = dem_mass(P, bi.R), mj = dem_mass(P, bj.R);
+                    const double mstar = mi * mj / (mi + mj);                          // (A.9)
+                    // previous delta_t of this pair, in canonical orientation
+                    double dt3[3] = {0, 0, 0};
+                    for (uint32_t h = 0; h < nprev; ++h)
+                        if (pid[h] == q) {
+                            const double sg = me_first ? 1.0 : -1.0;
+                            dt3[0] = sg * pdt[3 * h]; dt3[1] = sg * pdt[3 * h + 1]; dt3[2] = sg * pdt[3 * h + 2];
+                            break;
+                        }
+                    double F[3], T[3];
+                    dem_pair_force(en, dn, bi.v, bi.w, bi.R, bj.v, bj.w, bj.R, mstar, P.kn, P.kt, P.zeta, P.mu, dt_hist,
+                                   dt3, F, T);
+                    const double sg = me_first ? 1.0 : -1.0;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) { Fs[a] += sg * F[a]; Ms[a] += me.R * (-T[a]); }
+                    if (ncont < (uint32_t)maxc) {
+                        nid[ncont] = q;
+                        ndt[3 * ncont] = sg * dt3[0]; ndt[3 * ncont + 1] = sg * dt3[1]; ndt[3 * ncont + 2] = sg * dt3[2];
+                        ++ncont;
+                    } else st |= LEDDS_ST_CONTACT_OVERFLOW;
+                }
+            }
+        }
+    }
+    // walls: static infinite particles with a surface velocity
+    for (int wl = 0; wl < 6; ++wl) {
+        const int ax = wl >> 1, side = wl & 1;
+        if (!P.bc[ax]) continue;
+        const double dist = side ? P.hi[ax] - me.x[ax] : me.x[ax] - P.lo[ax];
+        const double dn = me.R - dist;
+        if (!(dn > 0.0)) continue;
+        double en[3] = {0, 0, 0};
+        en[ax] = side ? -1.0 : 1.0;
+        const uint32_t q = (uint32_t)P.n + (uint32_t)wl;
+        double dt3[3] = {0, 0, 0};
+        for (uint32_t h = 0; h < nprev; ++h)
+            if (pid[h] == q) { dt3[0] = pdt[3 * h]; dt3[1] = pdt[3 * h + 1]; dt3[2] = pdt[3 * h + 2]; break; }
+        const double vj[3] = {P.vw[wl * 3], P.vw[wl * 3 + 1], P.vw[wl * 3 + 2]}, wj[3] = {0, 0, 0};
+        double F[3], T[3];
+        dem_pair_force(en, dn, me.v, me.w, me.R, vj, wj, 0.0, m_me, P.kn_w, P.kt_w, P.zeta_w, P.mu_w, dt_hist, dt3, F, T);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { Fs[a] += F[a]; Ms[a] += me.R * (-T[a]); }
+        if (ncont < (uint32_t)maxc) {
+            nid[ncont] = q;
+            ndt[3 * ncont] = dt3[0]; ndt[3 * ncont + 1] = dt3[1]; ndt[3 * ncont + 2] = dt3[2];
+            ++ncont;
+        } else st |= LEDDS_ST_CONTACT_OVERFLOW;
+    }
+    hcount_new[p] = ncont;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        force[3 * p + a] = Fs[a];
+        torque[3 * p + a] = Ms[a];
+        if (!isfinite(Fs[a]) || !isfinite(Ms[a])) st |= LEDDS_ST_NONFINITE;
+    }
+    if (st) atomicOr(status, st);
+}
+
+// ------------------------------------------------------------------------------ kick
+__global__ void dem_kick_kernel(const DemDev P, const double* __restrict__ radius, const double* __restrict__ force,
+                                const double* __restrict__ torque, const double* __restrict__ f_ext,
+                                const double* __restrict__ m_ext, double* __restrict__ v, double* __restrict__ w,
+                                double* __restrict__ a, double* __restrict__ alpha, int only_accel)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    const double R = radius[i];
+    const double m = dem_mass(P, R), I = 0.4 * m * R * R;                             // Eq. (21a)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int q = 3 * i + k;
+        const double Fq = force[q] + (f_ext ? f_ext[q] : 0.0), Mq = torque[q] + (m_ext ? m_ext[q] : 0.0);
+        const double an = Fq / m + P.g[k], aln = Mq / I;                              // Eq. (18b), (19c)
+        if (!only_accel) {
+            v[q] = v[q] + (0.5 * P.dt) * (a[q] + an);                                 // Eq. (18c)
+            w[q] = w[q] + (0.5 * P.dt) * (alpha[q] + aln);                            // Eq. (19d)
+        }
+        a[q] = an;
+        alpha[q] = aln;
+    }
+}
+
+// ------------------------------------------------------------------------------ query (parity only)
+__global__ void dem_pair_count_kernel(int n, int maxc, const uint32_t* __restrict__ hcount,
+                                      const uint32_t* __restrict__ hid, uint32_t* __restrict__ cnt)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    uint32_t c = 0;
+    for (uint32_t h = 0; h < hcount[p]; ++h) c += hid[(size_t)p * maxc + h] > (uint32_t)p;
+    cnt[p] = c;
+}
+
+// single-block exclusive scan of cnt[n] into off[n+1]
+__global__ void __launch_bounds__(1024) dem_scan_kernel(int n, const uint32_t* __restrict__ cnt, uint32_t* __restrict__ off)
+{
+    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < n; base += 1024) {
+        const int i = base + tid;
+        const uint32_t c = i < n ? cnt[i] : 0u;
+        uint32_t incl = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) wsum[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            uint32_t s = wsum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, s, o);
+                if (lane >= o) s += t;
+            }
+            wsum[lane] = s;
+        }
+        __syncthreads();
+        const uint32_t before = carry + (warp ? wsum[warp - 1] : 0u) + incl - c;
+        if (i < n) off[i] = before;
+        __syncthreads();
+        if (tid == 1023) carry = before + c;
+        __syncthreads();
+    }
+    if (tid == 0) off[n] = carry;
+}
+
+__global__ void dem_pair_write_kernel(int n, int maxc, const uint32_t* __restrict__ hcount,
+                                      const uint32_t* __restrict__ hid, const double* __restrict__ hdt,
+                                      const uint32_t* __restrict__ off, uint32_t cap, uint32_t* __restrict__ pairs,
+                                      double* __restrict__ pair_dt, uint32_t* __restrict__ n_pairs)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p == 0 && n_pairs) *n_pairs = off[n];
+    if (p >= n) return;
+    uint32_t ids[32], slot[32];
+    int c = 0;
+    for (uint32_t h = 0; h < hcount[p]; ++h) {
+        const uint32_t q = hid[(size_t)p * maxc + h];
+        if (q <= (uint32_t)p) continue;
+        int k = c++;
+        while (k > 0 && ids[k - 1] > q) { ids[k] = ids[k - 1]; slot[k] = slot[k - 1]; --k; }   // insertion sort
+        ids[k] = q; slot[k] = h;
+    }
+    for (int k = 0; k < c; ++k) {
+        const uint32_t o = off[p] + k;
+        if (o >= cap) break;
+        if (pairs) { pairs[2 * o] = (uint32_t)p; pairs[2 * o + 1] = ids[k]; }
+        if (pair_dt)
+            for (int a = 0; a < 3; ++a) pair_dt[3 * o + a] = hdt[((size_t)p * maxc + slot[k]) * 3 + a];
+    }
+}
+
+// ------------------------------------------------------------------------------ host API
+static double dem_zeta_host(double eps)
+{
+    if (eps >= 1.0) return 0.0;
+    const double l = log(eps);
+    return -l / sqrt(l * l + DEM_PI * DEM_PI);                                        // -beta of (A.5)
+}
+
+static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
+{
+    if (!p || p->n < 1 || p->max_contacts < 1 || p->max_contacts > 32) return LEDDS_EINVAL;
+    if (!(p->cell > 0.0) || !(p->dt >= 0.0) || !(p->density > 0.0)) return LEDDS_EINVAL;
+    if (!(p->kn > 0.0) || !(p->kt > 0.0) || !(p->kn_w > 0.0) || !(p->kt_w > 0.0)) return LEDDS_EINVAL;
+    if (!(p->restitution > 0.0) || !(p->restitution_w > 0.0) || p->mu < 0.0 || p->mu_w < 0.0) return LEDDS_EINVAL;
+    h->p = *p;
+    DemDev& d = h->d;
+    d.n = p->n;
+    double ncell = 1.0;
+    for (int a = 0; a < 3; ++a) {
+        if (!(p->hi[a] > p->lo[a]) || (p->bc[a] != 0 && p->bc[a] != 1)) return LEDDS_EINVAL;
+        d.lo[a] = p->lo[a]; d.hi[a] = p->hi[a]; d.L[a] = p->hi[a] - p->lo[a]; d.bc[a] = p->bc[a];
+        int nc = (int)floor(d.L[a] / p->cell);
+        if (nc < 1) nc = 1;
+        if (!p->bc[a] && nc < 3) return LEDDS_EINVAL;          // a periodic axis needs >= 3 cells (27-cell walk)
+        d.nc[a] = nc;
+        d.inv_h[a] = (double)nc / d.L[a];
+        d.g[a] = p->g[a];
+        ncell *= nc;
+        for (int s = 0; s < 2; ++s)
+            for (int c = 0; c < 3; ++c) d.vw[(a * 2 + s) * 3 + c] = p->v_wall[a][s][c];
+    }
+    if (ncell > 4.0e9) return LEDDS_EINVAL;
+    d.ncell = (unsigned)ncell;
+    d.dt = p->dt; d.density = p->density;
+    d.kn = p->kn; d.kt = p->kt; d.zeta = dem_zeta_host(p->restitution); d.mu = p->mu;
+    d.kn_w = p->kn_w; d.kt_w = p->kt_w; d.zeta_w = dem_zeta_host(p->restitution_w); d.mu_w = p->mu_w;
+    d.maxc = p->max_contacts;
+    int bits = 1;
+    while (bits < 32 && (1ull << bits) < (unsigned long long)d.ncell) ++bits;
+    h->key_bits = bits;
+    h->passes = (bits + 7) / 8;
+    h->tiles = (p->n + SORT_TILE - 1) / SORT_TILE;
+
+    const size_t n = (size_t)p->n;
+    size_t o = 0;
+    DemScratch& s = h->s;
+    auto take = [&](size_t bytes) { const size_t at = o; o += align_up(bytes); return at; };
+    // zeroed before every sort: histograms, tickets, tile states (kept contiguous)
+    s.hist_digit = take(4 * SORT_RADIX * 4);
+    s.tile_counter = take(4 * 4);
+    s.tile_state = take((size_t)4 * h->tiles * SORT_RADIX * 4);
+    // zeroed before every range build
+    s.cell_start = take((size_t)d.ncell * 4);
+    s.cell_end = take((size_t)d.ncell * 4);
+    for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
+    s.xs = take(n * 24); s.vps = take(n * 24); s.wps = take(n * 24); s.rs = take(n * 8);
+    s.vp = take(n * 24); s.wp = take(n * 24);
+    s.force = take(n * 24); s.torque = take(n * 24);
+    s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4);
+    s.total = o;
+
+    DemHistory& hs = h->hs;
+    o = 0;
+    for (int b = 0; b < 2; ++b) {
+        hs.count[b] = take(n * 4);
+        hs.id[b] = take(n * d.maxc * 4);
+        hs.dt[b] = take(n * d.maxc * 24);
+    }
+    hs.total = o;
+    h->cur = 0;
+    h->sorted_buf = 0;
+    h->steps = 0;
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_dem_workspace_bytes(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes)
+{
+    ledds_dem tmp;
+    const int rc = dem_setup(p, &tmp);
+    if (rc) return rc;
+    if (scratch_bytes) *scratch_bytes = tmp.s.total;
+    if (history_bytes) *history_bytes = tmp.hs.total;
+    return LEDDS_OK;
+}
+
+template <typename T>
+static T* at(void* base, size_t off) { return reinterpret_cast<T*>(static_cast<char*>(base) + off); }
+template <typename T>
+static const T* at(const void* base, size_t off) { return reinterpret_cast<const T*>(static_cast<const char*>(base) + off); }
+
+// drift (optional) -> keys -> sort -> gather/ranges -> contacts.  Leaves force/torque in scratch.
+int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const double* w, const double* a,
+                               const double* alpha, const double* radius, void* history, void* scratch,
+                               int32_t* status, double dt_hist, bool drift, cudaStream_t st)
+{
+    const DemDev& d = h->d;
+    const DemScratch& s = h->s;
+    const int n = d.n, tb = 128, nb = (n + tb - 1) / tb;
+    // clear sort bookkeeping + cell ranges (one contiguous region)
+    if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
+    ledds_prof_start(LEDDS_K_DEM_KEYS, st);
+    dem_drift_key_kernel<<<nb, tb, 0, st>>>(d, x, v, w, a, alpha, at<double>(scratch, s.vp), at<double>(scratch, s.wp),
+                                            at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
+    ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
+    LEDDS_CHECK_LAUNCH();
+    ledds_prof_start(LEDDS_K_DEM_SORT, st);
+    int hb = (n + SORT_THREADS * 8 - 1) / (SORT_THREADS * 8);
+    if (hb > 148 * 8) hb = 148 * 8;
+    dem_hist_kernel<<<hb, SORT_THREADS, 0, st>>>(at<uint32_t>(scratch, s.key[0]), n, h->passes,
+                                                 at<uint32_t>(scratch, s.hist_digit));
+    LEDDS_CHECK_LAUNCH();
+    for (int p = 0; p < h->passes; ++p) {
+        const int in = p & 1, out = in ^ 1;
+        dem_onesweep_kernel<<<h->tiles, SORT_THREADS, 0, st>>>(
+            at<uint32_t>(scratch, s.key[in]), at<uint32_t>(scratch, s.idx[in]), at<uint32_t>(scratch, s.key[out]),
+            at<uint32_t>(scratch, s.idx[out]), n, 8 * p, at<uint32_t>(scratch, s.hist_digit) + p * SORT_RADIX,
+            at<uint32_t>(scratch, s.tile_state) + (size_t)p * h->tiles * SORT_RADIX,
+            at<uint32_t>(scratch, s.tile_counter) + p);
+        LEDDS_CHECK_LAUNCH();
+    }
+    ledds_prof_stop(LEDDS_K_DEM_SORT, st);
+    h->sorted_buf = h->passes & 1;
+    const uint32_t* skey = at<uint32_t>(scratch, s.key[h->sorted_buf]);
+    const uint32_t* sidx = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
+    ledds_prof_start(LEDDS_K_DEM_GATHER, st);
+    dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sidx, x, at<double>(scratch, s.vp), at<double>(scratch, s.wp), radius,
+                                         at<double>(scratch, s.xs), at<double>(scratch, s.vps), at<double>(scratch, s.wps),
+                                         at<double>(scratch, s.rs), at<uint32_t>(scratch, s.cell_start),
+                                         at<uint32_t>(scratch, s.cell_end));
+    ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
+    LEDDS_CHECK_LAUNCH();
+    const DemHistory& hs = h->hs;
+    const int prev = h->cur, nw = 1 - h->cur;
+    ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
+    dem_contact_kernel<<<nb, tb, 0, st>>>(
+        d, skey, sidx, at<double>(scratch, s.xs), at<double>(scratch, s.vps), at<double>(scratch, s.wps),
+        at<double>(scratch, s.rs), at<uint32_t>(scratch, s.cell_start), at<uint32_t>(scratch, s.cell_end),
+        at<uint32_t>(history, hs.count[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
+        at<uint32_t>(history, hs.count[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]),
+        at<double>(scratch, s.force), at<double>(scratch, s.torque), status, dt_hist);
+    ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
+    LEDDS_CHECK_LAUNCH();
+    h->cur = nw;
+    return LEDDS_OK;
+}
+
+int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha, const double* radius,
+                   const double* f_ext, const double* m_ext, void* scratch, int32_t* status, cudaStream_t st)
+{
+    (void)status;
+    const int n = h->d.n, tb = 128, nb = (n + tb - 1) / tb;
+    ledds_prof_start(LEDDS_K_DEM_KICK, st);
+    dem_kick_kernel<<<nb, tb, 0, st>>>(h->d, radius, at<double>(scratch, h->s.force), at<double>(scratch, h->s.torque),
+                                       f_ext, m_ext, v, w, a, alpha, 0);
+    ledds_prof_stop(LEDDS_K_DEM_KICK, st);
+    LEDDS_CHECK_LAUNCH();
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const double* x, const double* v,
+                              const double* w, const double* radius, double* a, double* alpha, void* history,
+                              void* scratch, int32_t* status, void* stream)
+{
+    if (!out || !x || !v || !w || !radius || !a || !alpha || !history || !scratch || !status) return LEDDS_EINVAL;
+    const void* ptrs[] = {x, v, w, radius, a, alpha, history, scratch, status};
+    for (const void* q : ptrs)
+        if (!ledds_aligned16(q)) return LEDDS_EALIGN;
+    ledds_dem* h = new (std::nothrow) ledds_dem();
+    if (!h) return LEDDS_EINVAL;
+    int rc = dem_setup(p, h);
+    if (rc) { delete h; return rc; }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemsetAsync(history, 0, h->hs.total, st) != cudaSuccess || cudaMemsetAsync(status, 0, 16, st) != cudaSuccess) {
+        delete h;
+        return LEDDS_ECUDA;
+    }
+    // forces of the initial state: no drift, delta_t stays 0 (dt_hist = 0)
+    rc = ledds_dem_advance_contacts(h, const_cast<double*>(x), v, w, a, alpha, radius, history, scratch, status, 0.0, false, st);
+    if (rc) { delete h; return rc; }
+    const int tb = 128, nb = (h->d.n + tb - 1) / tb;
+    dem_kick_kernel<<<nb, tb, 0, st>>>(h->d, radius, at<double>(scratch, h->s.force), at<double>(scratch, h->s.torque),
+                                       nullptr, nullptr, nullptr, nullptr, a, alpha, 1);
+    ledds_count_launch(1);
+    if (cudaPeekAtLastError() != cudaSuccess) { delete h; return LEDDS_ECUDA; }
+    *out = h;
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_dem_step(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha,
+                              const double* radius, const double* f_ext, const double* m_ext, void* history,
+                              void* scratch, int32_t* status, int nsteps, void* stream)
+{
+    if (!h || !x || !v || !w || !a || !alpha || !radius || !history || !scratch || !status || nsteps < 0) return LEDDS_EINVAL;
+    const void* ptrs[] = {x, v, w, a, alpha, radius, f_ext, m_ext, history, scratch, status};
+    for (const void* q : ptrs)
+        if (!ledds_aligned16(q)) return LEDDS_EALIGN;
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int s = 0; s < nsteps; ++s) {
+        int rc = ledds_dem_advance_contacts(h, x, v, w, a, alpha, radius, history, scratch, status, h->d.dt, true, st);
+        if (rc) return rc;
+        rc = ledds_dem_kick(h, v, w, a, alpha, radius, f_ext, m_ext, scratch, status, st);
+        if (rc) return rc;
+        h->steps++;
+    }
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* scratch, uint32_t* sorted_idx,
+                               uint32_t* sorted_key, uint32_t* pairs, double* pair_dt, uint32_t pair_cap,
+                               uint32_t* n_pairs, double* force, double* torque, void* stream)
+{
+    if (!h || !history || !scratch) return LEDDS_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n = (size_t)h->d.n;
+    const DemScratch& s = h->s;
+    auto copy = [&](void* dst, const void* src, size_t bytes) {
+        return !dst || cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st) == cudaSuccess;
+    };
+    if (!copy(sorted_idx, at<char>(scratch, s.idx[h->sorted_buf]), n * 4) ||
+        !copy(sorted_key, at<char>(scratch, s.key[h->sorted_buf]), n * 4) ||
+        !copy(force, at<char>(scratch, s.force), n * 24) || !copy(torque, at<char>(scratch, s.torque), n * 24))
+        return LEDDS_ECUDA;
+    if (pairs || pair_dt || n_pairs) {
+        const DemHistory& hs = h->hs;
+        const int tb = 128, nb = ((int)n + tb - 1) / tb;
+        // scratch is logically const for the caller; the two query arrays are ours to overwrite
+        uint32_t* cnt = const_cast<uint32_t*>(at<uint32_t>(scratch, s.pair_count));
+        uint32_t* off = const_cast<uint32_t*>(at<uint32_t>(scratch, s.pair_off));
+        dem_pair_count_kernel<<<nb, tb, 0, st>>>((int)n, h->d.maxc, at<uint32_t>(history, hs.count[h->cur]),
+                                                 at<uint32_t>(history, hs.id[h->cur]), cnt);
+        dem_scan_kernel<<<1, 1024, 0, st>>>((int)n, cnt, off);
+        dem_pair_write_kernel<<<nb, tb, 0, st>>>((int)n, h->d.maxc, at<uint32_t>(history, hs.count[h->cur]),
+                                                 at<uint32_t>(history, hs.id[h->cur]), at<double>(history, hs.dt[h->cur]),
+                                                 off, pair_cap, pairs, pair_dt, n_pairs);
+        ledds_count_launch(2);
+        LEDDS_CHECK_LAUNCH();
+    }
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_dem_destroy(ledds_dem* h)
+{
+    delete h;
+    return LEDDS_OK;
+}

@@ -1,0 +1,295 @@
+// D3Q19 BGK fused stream-collide for sm_100a (Eq. 22-28; boundaries PAPER.md:254).
+//
+// State = pre-collision populations in canonical layout f[q][z][y][x] (x fastest), two lattices.
+// One pass reads 19 doubles and writes 19 doubles per cell: 304 B/cell of algorithmic traffic.
+//   variant 1 "push":       one cell per thread, aligned coalesced loads, stores shifted by c_q.
+//   variant 2 "row-rotate": two cells per thread (16-B loads and stores); the +-1 shift along x is
+//                           done inside the row with warp shuffles (+ one smem word per warp and
+//                           direction), so every global store is aligned and full-sector too.
+#include <new>
+
+#include "lbm_kernels.cuh"
+
+// ------------------------------------------------------------------------------------ helpers
+__global__ void lbm_init_eq_kernel(double* __restrict__ f, const double* __restrict__ rho,
+                                   const double* __restrict__ u, long long N)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= N) return;
+    const double r = rho ? rho[c] : 1.0;
+    const double ux = u ? u[c] : 0.0, uy = u ? u[N + c] : 0.0, uz = u ? u[2 * N + c] : 0.0;
+    double fe[LEDDS_Q];
+    lb_equilibrium(fe, r, ux, uy, uz);
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) f[(long long)q * N + c] = fe[q];
+}
+
+__global__ void lbm_export_kernel(const double* __restrict__ f, double* __restrict__ fc, double* __restrict__ rho,
+                                  double* __restrict__ u, long long N)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= N) return;
+    double v[LEDDS_Q];
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) v[q] = f[(long long)q * N + c];
+    if (fc) {
+#pragma unroll
+        for (int q = 0; q < LEDDS_Q; ++q) fc[(long long)q * N + c] = v[q];
+    }
+    if (rho || u) {
+        double r, ux, uy, uz;
+        lb_moments(v, r, ux, uy, uz);
+        if (rho) rho[c] = r;
+        if (u) { u[c] = ux; u[N + c] = uy; u[2 * N + c] = uz; }
+    }
+}
+
+// ------------------------------------------------------------------------------------ variant 1
+__global__ void __launch_bounds__(128) lbm_push_kernel(const double* __restrict__ fin, double* __restrict__ fout,
+                                                       const LbmDev P)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y, z = blockIdx.z;
+    if (x >= P.nx) return;
+    const long long cell = ((long long)z * P.ny + y) * P.nx + x;
+    double f[LEDDS_Q];
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (long long)q * P.N + cell);
+    double rho, ux, uy, uz;
+    lb_moments(f, rho, ux, uy, uz);
+    lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
+    lb_push_store(fout, P, x, y, z, f, rho);
+}
+
+// ------------------------------------------------------------------------------------ variant 2
+// blockDim = (nx/2, RY); thread (j, r) owns cells x = 2j, 2j+1 of row y = blockIdx.x*RY + r, z = blockIdx.y.
+// nx/2 is a multiple of 32, so a warp never straddles rows.
+#define LEDDS_ROT_MAX_THREADS 256
+
+__device__ __forceinline__ void st2(double* p, double a, double b)
+{
+    *reinterpret_cast<double2*>(p) = make_double2(a, b);
+}
+
+__global__ void __launch_bounds__(LEDDS_ROT_MAX_THREADS) lbm_rowrot_kernel(const double* __restrict__ fin,
+                                                                         double* __restrict__ fout, const LbmDev P)
+{
+    // edge[k][warp]: value crossing a warp boundary for the k-th direction with cx != 0
+    __shared__ double edge[10][LEDDS_ROT_MAX_THREADS / 32];
+    const int j = threadIdx.x, lane = threadIdx.x & 31;
+    const int wrow = threadIdx.x >> 5;                         // warp index inside the row
+    const int wpr = blockDim.x >> 5;                           // warps per row
+    const int wblk = threadIdx.y * wpr + wrow;                 // warp index inside the block
+    const int y = blockIdx.x * blockDim.y + threadIdx.y, z = blockIdx.y;
+    const int x0 = 2 * j;
+    const long long row = ((long long)z * P.ny + y) * P.nx;
+
+    double fa[LEDDS_Q], fb[LEDDS_Q];
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) {
+        const double2 v = __ldg(reinterpret_cast<const double2*>(fin + (long long)q * P.N + row) + j);
+        fa[q] = v.x; fb[q] = v.y;
+    }
+    double rhoa, rhob, ux, uy, uz;
+    lb_moments(fa, rhoa, ux, uy, uz);
+    lb_collide_bgk(fa, P.omega, rhoa, ux, uy, uz);
+    lb_moments(fb, rhob, ux, uy, uz);
+    lb_collide_bgk(fb, P.omega, rhob, ux, uy, uz);
+
+    // publish warp-edge values of the 10 x-moving directions
+    {
+        int k = 0;
+#pragma unroll
+        for (int q = 1; q < LEDDS_Q; ++q) {
+            if (lb_cx(q) == 1) { if (lane == 31) edge[k][wblk] = fb[q]; ++k; }
+            else if (lb_cx(q) == -1) { if (lane == 0) edge[k][wblk] = fa[q]; ++k; }
+        }
+    }
+    __syncthreads();
+
+    const bool xwall = P.bc[0] != 0;
+    const bool first = (j == 0), last = (j == (int)blockDim.x - 1);
+    int k = 0;
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) {
+        const int cx = lb_cx(q), cy = lb_cy(q), cz = lb_cz(q);
+        // row-level part of the link: target row and whether the whole row bounces off a y/z wall
+        bool rowb = false;
+        double cuw_row = 0.0;
+        const int ty = lb_axis_target<1>(P, q, cy, y, P.ny, rowb, cuw_row);
+        const int tz = lb_axis_target<2>(P, q, cz, z, P.nz, rowb, cuw_row);
+        const long long trow = ((long long)tz * P.ny + ty) * P.nx;
+        double* const dst = fout + (long long)q * P.N + trow;                 // streamed target (slot q)
+        double* const own = fout + (long long)lb_opp(q) * P.N + row;          // bounce target (slot opp q)
+        const double w6 = 6.0 * lb_w(q);
+
+        if (cx == 0) {
+            if (rowb) st2(own + x0, fa[q] - w6 * rhoa * cuw_row, fb[q] - w6 * rhob * cuw_row);
+            else st2(dst + x0, fa[q], fb[q]);
+            continue;
+        }
+        // x-wall crossing of the two edge cells of the row
+        double cuw_x = 0.0;
+        if (xwall && P.any_wall_velocity) {
+            const double* uw = P.uw + (cx > 0 ? 1 : 0) * 3;                   // axis 0, side hi for cx=+1
+            cuw_x = lb_cdot(q, uw[0], uw[1], uw[2]);
+        }
+        if (cx == 1) {
+            double lo = __shfl_up_sync(0xffffffffu, fb[q], 1);
+            if (lane == 0) lo = edge[k][threadIdx.y * wpr + (wrow == 0 ? wpr - 1 : wrow - 1)];
+            if (rowb) {
+                const double cb = cuw_row + ((xwall && last) ? cuw_x : 0.0);
+                st2(own + x0, fa[q] - w6 * rhoa * cuw_row, fb[q] - w6 * rhob * cb);
+            } else {
+                if (xwall && first) dst[x0 + 1] = fa[q];                      // x = 0 has no source
+                else st2(dst + x0, lo, fa[q]);
+                if (xwall && last) own[x0 + 1] = fb[q] - w6 * rhob * cuw_x;    // link leaves through x = nx-1/2
+            }
+        } else {
+            double hi = __shfl_down_sync(0xffffffffu, fa[q], 1);
+            if (lane == 31) hi = edge[k][threadIdx.y * wpr + (wrow == wpr - 1 ? 0 : wrow + 1)];
+            if (rowb) {
+                const double ca = cuw_row + ((xwall && first) ? cuw_x : 0.0);
+                st2(own + x0, fa[q] - w6 * rhoa * ca, fb[q] - w6 * rhob * cuw_row);
+            } else {
+                if (xwall && last) dst[x0] = fb[q];                           // x = nx-1 has no source
+                else st2(dst + x0, fb[q], hi);
+                if (xwall && first) own[x0] = fa[q] - w6 * rhoa * cuw_x;       // link leaves through x = -1/2
+            }
+        }
+        ++k;
+    }
+}
+
+// ------------------------------------------------------------------------------------ host API
+static int lbm_validate(const ledds_lbm_params* p)
+{
+    if (!p) return LEDDS_EINVAL;
+    if (p->nx < 1 || p->ny < 1 || p->nz < 1) return LEDDS_EINVAL;
+    if ((long long)p->nx * p->ny * p->nz > (1ll << 31)) return LEDDS_EINVAL;
+    if (!(p->tau > 0.5)) return LEDDS_EINVAL;
+    if (p->layout != 0) return LEDDS_EINVAL;
+    if (p->variant < 0 || p->variant > 2) return LEDDS_EINVAL;
+    for (int a = 0; a < 3; ++a)
+        if (p->bc[a] != 0 && p->bc[a] != 1) return LEDDS_EINVAL;
+    // a periodic axis of length 1 would stream a population onto itself: allowed (it is a no-op wrap)
+    return LEDDS_OK;
+}
+
+static bool lbm_rowrot_ok(const ledds_lbm_params* p) { return p->nx % 64 == 0 && p->nx / 2 <= LEDDS_ROT_MAX_THREADS; }
+
+extern "C" int ledds_lbm_workspace_bytes(const ledds_lbm_params* p, size_t* f_bytes)
+{
+    const int rc = lbm_validate(p);
+    if (rc) return rc;
+    if (!f_bytes) return LEDDS_EINVAL;
+    *f_bytes = (size_t)2 * LEDDS_Q * p->nx * p->ny * p->nz * sizeof(double);
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_lbm_init(ledds_lbm** out, const ledds_lbm_params* p, double* f, const double* rho,
+                              const double* u, void* stream)
+{
+    const int rc = lbm_validate(p);
+    if (rc) return rc;
+    if (!out || !f) return LEDDS_EINVAL;
+    if (!ledds_aligned16(f) || !ledds_aligned16(rho) || !ledds_aligned16(u)) return LEDDS_EALIGN;
+    if (p->variant == 2 && !lbm_rowrot_ok(p)) return LEDDS_EINVAL;
+    ledds_lbm* h = new (std::nothrow) ledds_lbm();
+    if (!h) return LEDDS_EINVAL;
+    h->p = *p;
+    LbmDev& d = h->d;
+    d.nx = p->nx; d.ny = p->ny; d.nz = p->nz;
+    d.N = (long long)p->nx * p->ny * p->nz;
+    d.tau = p->tau;
+    d.omega = 1.0 / p->tau;
+    d.any_wall_velocity = 0;
+    for (int a = 0; a < 3; ++a) {
+        d.bc[a] = p->bc[a];
+        for (int s = 0; s < 2; ++s)
+            for (int c = 0; c < 3; ++c) {
+                d.uw[(a * 2 + s) * 3 + c] = p->u_wall[a][s][c];
+                if (p->bc[a] && p->u_wall[a][s][c] != 0.0) d.any_wall_velocity = 1;
+            }
+    }
+    h->parity = 0;
+    h->steps = 0;
+    const int tb = 256;
+    lbm_init_eq_kernel<<<(unsigned)((d.N + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(f, rho, u, d.N);
+    ledds_count_launch(1);
+    if (cudaPeekAtLastError() != cudaSuccess) { delete h; return LEDDS_ECUDA; }
+    *out = h;
+    return LEDDS_OK;
+}
+
+extern "C" const double* ledds_lbm_current(const ledds_lbm* h, const double* f)
+{
+    return (h && f) ? f + (size_t)h->parity * LEDDS_Q * h->d.N : nullptr;
+}
+
+extern "C" int ledds_lbm_import(ledds_lbm* h, double* f, const double* fc, void* stream)
+{
+    if (!h || !f || !fc) return LEDDS_EINVAL;
+    if (!ledds_aligned16(f) || !ledds_aligned16(fc)) return LEDDS_EALIGN;
+    double* cur = f + (size_t)h->parity * LEDDS_Q * h->d.N;
+    if (cudaMemcpyAsync(cur, fc, sizeof(double) * LEDDS_Q * h->d.N, cudaMemcpyDeviceToDevice, (cudaStream_t)stream) !=
+        cudaSuccess)
+        return LEDDS_ECUDA;
+    return LEDDS_OK;
+}
+
+// one stream-collide launch src -> dst (used by ledds_lbm_step; coupled.cu has its own PSM launch)
+static int lbm_launch(const ledds_lbm* h, const double* src, double* dst, cudaStream_t st)
+{
+    const LbmDev& d = h->d;
+    int variant = h->p.variant;
+    if (variant == 0) variant = 1;   // measured on B200: the plain push kernel already runs at the HBM copy rate
+    if (variant != 2 && (d.ny > 65535 || d.nz > 65535)) return LEDDS_EINVAL;
+    ledds_prof_start(LEDDS_K_LBM, st);
+    if (variant == 2) {
+        const int tx = d.nx / 2;
+        int ry = 1;
+        while (ry < 8 && tx * ry * 2 <= LEDDS_ROT_MAX_THREADS && d.ny % (ry * 2) == 0) ry *= 2;
+        dim3 block(tx, ry), grid(d.ny / ry, d.nz);
+        lbm_rowrot_kernel<<<grid, block, 0, st>>>(src, dst, d);
+    } else {
+        dim3 block(128), grid((d.nx + 127) / 128, d.ny, d.nz);
+        lbm_push_kernel<<<grid, block, 0, st>>>(src, dst, d);
+    }
+    ledds_prof_stop(LEDDS_K_LBM, st);
+    LEDDS_CHECK_LAUNCH();
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_lbm_step(ledds_lbm* h, double* f, int nsteps, void* stream)
+{
+    if (!h || !f || nsteps < 0) return LEDDS_EINVAL;
+    if (!ledds_aligned16(f)) return LEDDS_EALIGN;
+    const size_t half = (size_t)LEDDS_Q * h->d.N;
+    for (int s = 0; s < nsteps; ++s) {
+        const int rc = lbm_launch(h, f + h->parity * half, f + (1 - h->parity) * half, (cudaStream_t)stream);
+        if (rc) return rc;
+        h->parity ^= 1;
+        h->steps++;
+    }
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_lbm_export(ledds_lbm* h, const double* f, double* fc, double* rho, double* u, void* stream)
+{
+    if (!h || !f) return LEDDS_EINVAL;
+    if (!ledds_aligned16(f) || !ledds_aligned16(fc) || !ledds_aligned16(rho) || !ledds_aligned16(u)) return LEDDS_EALIGN;
+    const int tb = 256;
+    lbm_export_kernel<<<(unsigned)((h->d.N + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(
+        f + (size_t)h->parity * LEDDS_Q * h->d.N, fc, rho, u, h->d.N);
+    LEDDS_CHECK_LAUNCH();
+    return LEDDS_OK;
+}
+
+extern "C" int ledds_lbm_destroy(ledds_lbm* h)
+{
+    delete h;
+    return LEDDS_OK;
+}
+
+extern "C" const char* ledds_version(void) { return "ledds-b200 0.1 (sm_100a, fp64)"; }

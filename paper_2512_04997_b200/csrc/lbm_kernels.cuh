@@ -1,0 +1,93 @@
+// Device-side building blocks of the D3Q19 stream-collide kernels (Eq. 22-28).
+#pragma once
+#include "common.cuh"
+
+// Eq. (22a), (22b): density and velocity of one cell.
+__device__ __forceinline__ void lb_moments(const double (&f)[LEDDS_Q], double& rho, double& ux, double& uy, double& uz)
+{
+    double r = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) {
+        r += f[q];
+        if (lb_cx(q) == 1) jx += f[q]; else if (lb_cx(q) == -1) jx -= f[q];
+        if (lb_cy(q) == 1) jy += f[q]; else if (lb_cy(q) == -1) jy -= f[q];
+        if (lb_cz(q) == 1) jz += f[q]; else if (lb_cz(q) == -1) jz -= f[q];
+    }
+    const double inv = 1.0 / r;
+    rho = r; ux = jx * inv; uy = jy * inv; uz = jz * inv;
+}
+
+// c_q . u with the zero components folded away at compile time.
+__device__ __forceinline__ double lb_cdot(int q, double ux, double uy, double uz)
+{
+    double s = 0.0;
+    if (lb_cx(q) == 1) s += ux; else if (lb_cx(q) == -1) s -= ux;
+    if (lb_cy(q) == 1) s += uy; else if (lb_cy(q) == -1) s -= uy;
+    if (lb_cz(q) == 1) s += uz; else if (lb_cz(q) == -1) s -= uz;
+    return s;
+}
+
+// Eq. (28) with c_s^2 = 1/3 for all 19 directions.
+__device__ __forceinline__ void lb_equilibrium(double (&fe)[LEDDS_Q], double rho, double ux, double uy, double uz)
+{
+    const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
+    fe[0] = lb_w(0) * rho * k;
+#pragma unroll
+    for (int q = 1; q < LEDDS_Q; q += 2) {            // q and q+1 are opposites
+        const double cu = lb_cdot(q, ux, uy, uz);
+        const double wr = lb_w(q) * rho;
+        const double even = wr * (k + 4.5 * cu * cu), odd = wr * 3.0 * cu;
+        fe[q] = even + odd;
+        fe[q + 1] = even - odd;
+    }
+}
+
+// Eq. (24), (26): f* = f - omega (f - feq), in place.
+__device__ __forceinline__ void lb_collide_bgk(double (&f)[LEDDS_Q], double omega, double rho, double ux, double uy, double uz)
+{
+    double fe[LEDDS_Q];
+    lb_equilibrium(fe, rho, ux, uy, uz);
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) f[q] = f[q] - omega * (f[q] - fe[q]);
+}
+
+// Where does the link q that starts at coordinate `r` on one axis end?  Returns the target
+// coordinate (wrapped on a periodic axis); sets `bounced` and adds c_q . u_wall of the crossed
+// wall when the axis is walled (halfway bounce-back).
+template <int AXIS>
+__device__ __forceinline__ int lb_axis_target(const LbmDev& P, int q, int c, int r, int n, bool& bounced, double& cuw)
+{
+    if (c == 0) return r;
+    int t = r + c;
+    if (t < 0 || t >= n) {
+        if (P.bc[AXIS]) {
+            bounced = true;
+            if (P.any_wall_velocity) {
+                const double* uw = P.uw + (AXIS * 2 + (t < 0 ? 0 : 1)) * 3;
+                cuw += lb_cdot(q, uw[0], uw[1], uw[2]);
+            }
+        } else {
+            t = t < 0 ? t + n : t - n;
+        }
+    }
+    return t;
+}
+
+// Eq. (25) as a push of all 19 post-collision populations of cell (x,y,z), with boundaries.
+__device__ __forceinline__ void lb_push_store(double* __restrict__ fout, const LbmDev& P, int x, int y, int z,
+                                              const double (&fs)[LEDDS_Q], double rho)
+{
+    const long long cell = ((long long)z * P.ny + y) * P.nx + x;
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) {
+        bool bounced = false;
+        double cuw = 0.0;
+        const int tx = lb_axis_target<0>(P, q, lb_cx(q), x, P.nx, bounced, cuw);
+        const int ty = lb_axis_target<1>(P, q, lb_cy(q), y, P.ny, bounced, cuw);
+        const int tz = lb_axis_target<2>(P, q, lb_cz(q), z, P.nz, bounced, cuw);
+        if (bounced)
+            fout[(long long)lb_opp(q) * P.N + cell] = fs[q] - 6.0 * lb_w(q) * rho * cuw;
+        else
+            fout[(long long)q * P.N + ((long long)tz * P.ny + ty) * P.nx + tx] = fs[q];
+    }
+}

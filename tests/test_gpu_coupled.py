@@ -1,0 +1,110 @@
+"""GPU parity: coupled PSM step (ledds_coupled_step) vs the CPU oracle."""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def both(lbm, cpl, pd, x, v, w, R, u=None):
+    import oracle
+    from paper_2512_04997_b200 import Coupled, Dem, Lbm
+    f0 = oracle.lbm_equilibrium(lbm["shape"], None, u)
+    od = oracle.Dem(pd, x, v, w, R)
+    o = oracle.Coupled(lbm, cpl, od, f0)
+    gl = Lbm(lbm, None, u)
+    gd = Dem(pd, x, v, w, R)
+    g = Coupled(gl, gd, cpl, float(np.max(R)))
+    return o, g
+
+
+def compare(o, g, tol_f=1e-12, tol_F=1e-10):
+    """Populations 1e-12 of max |f|.  Forces: the momentum exchange of Eq. 41 is a sum of differences
+    of O(1) populations, so its rounding floor is ~1e-17 per term whatever the size of the force:
+    tolerance = tol_F * max|F| + FLOOR (lattice units, set-ups here have dx = rho_f = Dt = 1), and
+    likewise for the velocities integrated from it."""
+    FLOOR = 1e-13
+    f = g.lbm.export()
+    assert np.abs(f - o.f).max() <= tol_f * np.abs(o.f).max()
+    F, M = g.f_hyd.cpu().numpy(), g.m_hyd.cpu().numpy()
+    Rm = float(o.dem.R.max())
+    assert np.abs(F - o.F_sf).max() <= tol_F * np.abs(o.F_sf).max() + FLOOR
+    assert np.abs(M - o.M_sf).max() <= tol_F * np.abs(o.M_sf).max() + FLOOR * Rm
+    s = g.dem.state()
+    L = max(o.lbm["shape"])
+    assert np.abs(s["x"] - o.dem.x).max() <= 1e-9 * L
+    assert np.abs(s["v"] - o.dem.v).max() <= 1e-9 * np.abs(o.dem.v).max() + FLOOR
+    assert np.abs(s["w"] - o.dem.w).max() <= 1e-9 * np.abs(o.dem.w).max() + FLOOR
+    assert int(g.dem.status[0].item()) == o.status
+
+
+def test_single_sphere_settling_small():
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(32, 32, 64), R=5.0, z0=40.0, g=1e-3)
+    o, g = both(lbm, cpl, pd, x, v, w, R)
+    o.step(1); g.step(1)
+    compare(o, g)
+    o.step(9); g.step(9)
+    compare(o, g)
+    assert o.F_sf[0, 2] > 0 and o.dem.v[0, 2] < 0
+
+
+def test_zero_reach_particle_is_plain_lbm_bit_exact():
+    # no solid in any cell -> the coupled kernel is the plain stream-collide, bit for bit
+    from paper_2512_04997_b200 import Lbm
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(64, 16, 16), R=3.0, z0=8.0, g=0.0)
+    pd = dict(pd); pd["lo"] = (-0.5, -0.5, -100.5); pd["bc"] = (1, 1, 1)
+    x = np.array([[8.0, 8.0, -50.0]])                          # far below the lattice
+    lbm = dict(lbm); cpl = dict(cpl)
+    rho, u = W.random_flow(lbm["shape"], 4)
+    import oracle
+    from paper_2512_04997_b200 import Coupled, Dem
+    gl = Lbm(dict(lbm, variant=1), rho, u)
+    gd = Dem(pd, x, v, w, R)
+    g = Coupled(gl, gd, cpl, 3.0)
+    g.step(5)
+    plain = Lbm(dict(lbm, variant=1), rho, u)
+    plain.step(5)
+    assert np.array_equal(gl.export(), plain.export())
+    assert np.all(g.f_hyd.cpu().numpy() == 0)
+
+
+def test_shear_suspension_small_with_contacts_and_periodic_wrap():
+    # config-4 shaped: periodic x,y, moving z walls, spheres placed by RSA, some across the periodic seam
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=2, n=64, n_part=60, R=4.0)
+    x[0] = (0.2, 30.0, 20.0); x[1] = (63.3, 10.0, 40.0)          # straddle the x seam (kept apart from others below)
+    keep = np.ones(len(x), bool)
+    for i in (0, 1):
+        d = x - x[i]; d[:, :2] -= 64 * np.round(d[:, :2] / 64)
+        close = (np.linalg.norm(d, axis=1) < 2 * 4.0); close[i] = False
+        keep &= ~close
+    x, v, w, R = x[keep], v[keep], w[keep], R[keep]
+    pd = dict(pd); pd["n"] = len(x)
+    # give two spheres an overlap so the DEM contact path is active inside the coupled step
+    x[3] = x[2] + np.array([7.5, 0.0, 0.0]); x[3, 0] %= 64
+    o, g = both(lbm, cpl, pd, x, v, w, R, u)
+    o.step(1); g.step(1)
+    compare(o, g)
+    o.step(4); g.step(4)
+    compare(o, g)
+    assert np.abs(o.F_sf).max() > 0
+
+
+def test_substepping():
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(32, 32, 48), R=4.0, z0=5.0, g=2e-3)
+    cpl = dict(cpl, n_sub=4); pd = dict(pd, dt=0.25)
+    o, g = both(lbm, cpl, pd, x, v, w, R)
+    o.step(6); g.step(6)
+    compare(o, g)
+
+
+def test_three_solids_in_a_cell_are_flagged():
+    import paper_2512_04997_b200 as L
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(32, 32, 32), R=3.0, z0=16.0, g=0.0)
+    pd = dict(pd, n=3, kn=1e-9, kn_w=1e-9, kt=1e-9, kt_w=1e-9)
+    x = np.array([[15.0, 16.0, 16.0], [17.0, 16.0, 16.0], [16.0, 17.5, 16.0]])
+    z = np.zeros((3, 3))
+    o, g = both(lbm, cpl, pd, x, z, z, np.full(3, 3.0))
+    o.step(1); g.step(1)
+    assert o.status & 2 and int(g.dem.status[0].item()) & L.ST_SOLID_OVERFLOW
+    compare(o, g)

@@ -1,0 +1,107 @@
+"""GPU parity: CUDA DEM pipeline (through the C ABI) vs the CPU oracle.
+north_star: cell ordering and contact pair list bit-exact; per-particle forces after one step
+within 1e-12 relative; trajectories over 10 steps within 1e-9."""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def both(pd, x, v, w, R):
+    import oracle
+    from paper_2512_04997_b200 import Dem
+    return oracle.Dem(pd, x, v, w, R), Dem(pd, x, v, w, R)
+
+
+def check_state(o, g, steps_done, box):
+    q = g.query()
+    assert q["status"] == 0
+    assert np.array_equal(q["key"], o.key[o.idx]) and np.array_equal(q["idx"], o.idx)
+    assert np.array_equal(q["pairs"], o.pairs), (len(q["pairs"]), len(o.pairs))
+    fs = max(np.abs(o.F).max(), 1e-300)
+    assert np.abs(q["F"] - o.F).max() <= 1e-12 * fs
+    assert np.abs(q["M"] - o.M).max() <= 1e-12 * max(np.abs(o.M).max(), 1e-300)
+    if len(o.pairs):
+        assert np.abs(q["pair_dt"] - o.dt_hist).max() <= 1e-12 * max(np.abs(o.dt_hist).max(), 1e-300)
+    s = g.state()
+    assert np.abs(s["x"] - o.x).max() <= 1e-9 * box
+    assert np.abs(s["v"] - o.v).max() <= 1e-9 * max(np.abs(o.v).max(), 1e-300)
+    assert np.abs(s["w"] - o.w).max() <= 1e-9 * max(np.abs(o.w).max(), 1e-300)
+
+
+@pytest.mark.parametrize("seed,bc,n", [(1, (1, 1, 1), 3000), (2, (0, 0, 0), 4000), (3, (0, 1, 0), 1777), (4, (1, 0, 1), 33)])
+def test_random_overlapping_cloud(seed, bc, n):
+    # dense random polydisperse cloud: many contacts, friction, rotation, periodic wrap, walls
+    pd, x, v, w, R = W.dem_random(seed, n, box=(14.0, 11.0, 9.0), bc=bc)
+    pd["max_contacts"] = 32
+    o, g = both(pd, x, v, w, R)
+    check_state(o, g, 0, 14.0)                                 # forces of the initial state, a(0)
+    assert np.abs(g.state()["a"] - o.a).max() <= 1e-12 * np.abs(o.a).max()
+    o.step(); g.step()
+    check_state(o, g, 1, 14.0)                                 # forces after one step: 1e-12
+    for _ in range(9):
+        o.step(); g.step()
+    check_state(o, g, 10, 14.0)                                # trajectories over 10 steps: 1e-9
+
+
+def test_config1_gas_full():
+    # BASELINE configs[0] at full size: 2048 spheres, 10 steps, then 200 more with ordering still exact
+    pd, x, v, w, R = W.cfg1_gas()
+    o, g = both(pd, x, v, w, R)
+    o.step(10); g.step(10)
+    check_state(o, g, 10, pd["hi"][0])
+
+
+def test_multi_tile_sort_and_ragged_tail():
+    # 70 001 particles: 18 sort tiles with a ragged last tile, 3 radix passes (grid has > 65536 cells)
+    n_side = 42
+    pd, x, v, w, R = W.cfg5_pour(seed=9, n_side=n_side, n_part=70001, dense=True)
+    o, g = both(pd, x, v, w, R)
+    check_state(o, g, 0, pd["hi"][2])
+    assert len(o.pairs) > 50000
+    o.step(2); g.step(2)
+    check_state(o, g, 2, pd["hi"][2])
+
+
+def test_edge_cases_single_particle_and_no_contacts():
+    pd = W.dem_defaults(1, (0, 0, 0), (4, 4, 4), (1, 1, 1), cell=1.0, dt=1e-3, g=(0, 0, -9.81), density=1000.0, kn=1e5,
+                        restitution=0.5, mu=0.3)
+    o, g = both(pd, [[2, 2, 0.45]], [[0.1, 0, 0]], [[0, 0, 0]], [0.5])
+    o.step(20); g.step(20)
+    check_state(o, g, 20, 4.0)
+    assert o.pairs.tolist() == [[0, 5]]
+    # no contact at all
+    pd, x, v, w, R = W.cfg5_pour(seed=3, n_side=10, n_part=1000, dense=False)
+    o, g = both(pd, x, v, w, R)
+    o.step(3); g.step(3)
+    check_state(o, g, 3, pd["hi"][2])
+    assert len(o.pairs) == 0
+
+
+def test_contact_slot_overflow_is_flagged():
+    import paper_2512_04997_b200 as L
+    from paper_2512_04997_b200 import Dem
+    pd, x, v, w, R = W.dem_random(5, 400, box=(3.0, 3.0, 3.0))
+    pd["max_contacts"] = 2
+    g = Dem(pd, x, v, w, R)
+    assert int(g.status[0].item()) & L.ST_CONTACT_OVERFLOW
+
+
+def test_history_persists_and_is_dropped():
+    # oblique wall impact: tangential history accumulates during the contact, gone afterwards
+    pd = W.dem_defaults(1, (0, 0, 0), (10, 1, 1), (1, 1, 1), cell=0.2, dt=2e-5, g=(0, 0, 0), density=2000.0, kn=1e6,
+                        restitution=1.0, mu=0.3)
+    o, g = both(pd, [[1.0, 0.5, 0.05 + 1e-6]], [[2.0, 0, -1.0]], [[0, 0, 0]], [0.05])
+    seen = 0
+    for _ in range(200):
+        o.step(); g.step()
+        q = g.query()
+        assert np.array_equal(q["pairs"], o.pairs)
+        if len(o.pairs):
+            seen += 1
+            assert np.abs(q["pair_dt"] - o.dt_hist).max() <= 1e-12 * np.abs(o.dt_hist).max()
+    assert seen > 10 and len(o.pairs) == 0
+    s = g.state()
+    assert np.abs(s["w"] - o.w).max() <= 1e-9 * np.abs(o.w).max() and abs(o.w[0, 1]) > 1.0
