@@ -10,7 +10,7 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 # dem.cu: no FMA contraction (cell index and delta_n > 0 must not depend on it); lbm/coupled keep FMA
 UNITS = [("lbm.cu", []), ("dem.cu", ["-fmad=false"]), ("coupled.cu", []), ("prof.cu", [])]
-HEADERS = ["common.cuh", "lbm_kernels.cuh", os.path.join("..", "..", "include", "ledds.h")]
+HEADERS = ["common.cuh", "lbm_kernels.cuh", "psm_kernels.cuh", os.path.join("..", "..", "include", "ledds.h")]
 
 
 def _newer(target, deps):

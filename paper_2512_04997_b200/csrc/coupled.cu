@@ -10,179 +10,141 @@
 //                      no sort over N_fluid as in PAPER.md:525-530).
 #include <math.h>
 
-#include "lbm_kernels.cuh"
+#include "psm_kernels.cuh"
 
-struct CplDev {
-    int n;
-    double rc;                 // Eq. (40) in lattice units
-    double inv_dx, vscale, wscale, origin[3];
-    double fscale, mscale;     // lattice -> DEM units for force / torque
-    // DEM grid seen from lattice indices: grid coordinate = r * gs + g0, search half-width dg
-    int nc[3], gbc[3];
-    double gs[3], g0[3], dg[3];
-    int H, S;                  // box of partials per solid: S^3 entries of 6 doubles
-    const uint32_t* cell_start; const uint32_t* cell_end; const uint32_t* sidx;
-    const double* xs; const double* vps; const double* wps; const double* rs;
-    double* boxes;
-    int32_t* status;
-};
-
-// delta_sc of Eq. (40) > 0, evaluated with explicitly rounded operations so that the collide kernel
-// and the reduce kernel take the same decision for the same (cell, solid).
-__device__ __forceinline__ double cpl_dist(const double* d)
+// Cold path: the block's shared candidate list overflowed (never at resolved-particle densities), so the
+// thread searches the 2x2x2 DEM grid cells around its own cell in global memory.
+__device__ __noinline__ void psm_cell_global_search(const LbmDev& P, const CplDev& C, const int* r, double (&f)[LEDDS_Q],
+                                                    double rho, double ux, double uy, double uz)
 {
-    return __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2])));
-}
-__device__ __forceinline__ double cpl_dsc(double Rk, double rc, double dist) { return __dsub_rn(__dadd_rn(Rk, rc), dist); }
-
-// lattice node image nearest to the solid: integer offset di = r - floor(xk), wrapped on periodic axes
-__device__ __forceinline__ int cpl_offset(int r, int fk, int n, int periodic)
-{
-    int di = r - fk;
-    if (periodic) {
-        if (2 * di > n) di -= n;
-        else if (2 * di < -n) di += n;
-    }
-    return di;
-}
-
-__global__ void __launch_bounds__(128) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
-                                                      const LbmDev P, const CplDev C)
-{
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y, z = blockIdx.z;
-    if (x >= P.nx) return;
-    const long long cell = ((long long)z * P.ny + y) * P.nx + x;
-    double f[LEDDS_Q];
-#pragma unroll
-    for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (long long)q * P.N + cell);
-
-    // ---- which solids cut this cell (two lowest ids with beta > 0) ----
-    const int r[3] = {x, y, z};
-    const int nl[3] = {P.nx, P.ny, P.nz};
     int clo[3], chi[3];
-#pragma unroll
     for (int a = 0; a < 3; ++a) {
         const double g = r[a] * C.gs[a] + C.g0[a];
-        clo[a] = (int)floor(g - C.dg[a]);
-        chi[a] = (int)floor(g + C.dg[a]);
+        clo[a] = (int)floor(g - C.dg[a]); chi[a] = (int)floor(g + C.dg[a]);
         if (C.gbc[a]) { clo[a] = max(clo[a], 0); chi[a] = min(chi[a], C.nc[a] - 1); }
     }
-    uint32_t id0 = 0xffffffffu, id1 = 0xffffffffu, t0 = 0, t1 = 0;
-    int extra = 0;
-    for (int gz = clo[2]; gz <= chi[2]; ++gz) {
-        const int wz = C.gbc[2] ? gz : (gz % C.nc[2] + C.nc[2]) % C.nc[2];
-        for (int gy = clo[1]; gy <= chi[1]; ++gy) {
-            const int wy = C.gbc[1] ? gy : (gy % C.nc[1] + C.nc[1]) % C.nc[1];
-            for (int gx = clo[0]; gx <= chi[0]; ++gx) {
-                const int wx = C.gbc[0] ? gx : (gx % C.nc[0] + C.nc[0]) % C.nc[0];
-                const uint32_t gc = (uint32_t)(wx + C.nc[0] * (wy + C.nc[1] * wz));
-                const uint32_t b = C.cell_start[gc], e = C.cell_end[gc];
-                for (uint32_t t = b; t < e; ++t) {
-                    double d[3];
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) {
-                        const double xk = (C.xs[3 * t + a] - C.origin[a]) * C.inv_dx;
-                        const int fk = (int)floor(xk);
-                        d[a] = (double)(fk + cpl_offset(r[a], fk, nl[a], !P.bc[a])) - xk;
+    uint32_t id0 = 0xffffffffu, id1 = 0xffffffffu;
+    int c0 = 0, c1 = 0;
+    bool dropped = false;
+    PsmCand far0, far1;
+    for (int pass = 0; pass < 2; ++pass) {                       // pass 0: select; pass 1: zero the dropped ones
+        if (pass == 1 && !dropped) break;
+        for (int gz = clo[2]; gz <= chi[2]; ++gz)
+            for (int gy = clo[1]; gy <= chi[1]; ++gy)
+                for (int gx = clo[0]; gx <= chi[0]; ++gx) {
+                    const int wz = C.gbc[2] ? gz : (gz % C.nc[2] + C.nc[2]) % C.nc[2];
+                    const int wy = C.gbc[1] ? gy : (gy % C.nc[1] + C.nc[1]) % C.nc[1];
+                    const int wx = C.gbc[0] ? gx : (gx % C.nc[0] + C.nc[0]) % C.nc[0];
+                    const uint32_t gc = (uint32_t)(wx + C.nc[0] * (wy + C.nc[1] * wz));
+                    for (uint32_t t = C.cell_start[gc]; t < C.cell_end[gc]; ++t) {
+                        PsmCand pc;
+                        psm_load_cand(C, t, pc);
+                        if (pass == 1) { if (pc.id != id0 && pc.id != id1) psm_zero_dropped(P, C, r, pc); continue; }
+                        double d[3]; int loc[3];
+                        psm_rel(P, C, r, pc, d, loc);
+                        if (!(cpl_dsc(pc.Rk, C.rc, cpl_dist(d)) > 0.0)) continue;
+                        const uint32_t o0 = id0, o1 = id1;
+                        dropped |= psm_select(pc.id, 0, id0, id1, c0, c1);
+                        if (id0 != o0) { far1 = far0; far0 = pc; } else if (id1 != o1) far1 = pc;
                     }
-                    if (!(cpl_dsc(C.rs[t] * C.inv_dx, C.rc, cpl_dist(d)) > 0.0)) continue;
-                    const uint32_t id = C.sidx[t];
-                    if (id == id0 || id == id1) continue;                  // same solid seen through a wrapped cell
-                    if (id < id0) { if (id1 != 0xffffffffu) ++extra; id1 = id0; t1 = t0; id0 = id; t0 = t; }
-                    else if (id < id1) { if (id1 != 0xffffffffu) ++extra; id1 = id; t1 = t; }
-                    else ++extra;
                 }
+    }
+    if (id0 == 0xffffffffu) { lb_collide_bgk(f, P.omega, rho, ux, uy, uz); return; }
+    if (dropped) atomicOr(C.status, LEDDS_ST_SOLID_OVERFLOW);
+    psm_cell(P, C, r, f, rho, ux, uy, uz, far0, far1, id1 == 0xffffffffu ? 1 : 2);
+}
+
+// One thread per cell, one block per 128-cell row segment.  The block first collects, together, the solids
+// that can reach its row segment (walking the DEM grid cells around it) into shared memory; a row with no
+// candidate runs the plain BGK path.
+__global__ void __launch_bounds__(PSM_BLOCK, 4) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
+                                                               const __grid_constant__ LbmDev P,
+                                                               const __grid_constant__ CplDev C)
+{
+    __shared__ PsmCand cand[PSM_MAXC];
+    __shared__ int s_n;
+    const int tid = threadIdx.x;
+    const int x_first = blockIdx.x * PSM_BLOCK;
+    const int x = x_first + tid, y = blockIdx.y, z = blockIdx.z;
+    const bool active = x < P.nx;
+    const long long cell = ((long long)z * P.ny + y) * P.nx + (active ? x : 0);
+    double f[LEDDS_Q];
+    if (active) {
+#pragma unroll
+        for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (long long)q * P.N + cell);
+    }
+    if (tid == 0) s_n = 0;
+    __syncthreads();
+    {
+        const int x_last = min(x_first + PSM_BLOCK - 1, P.nx - 1);
+        const int rlo[3] = {x_first, y, z}, rhi[3] = {x_last, y, z};
+        int clo[3], cnt[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            int lo = (int)floor(rlo[a] * C.gs[a] + C.g0[a] - C.dg[a]);
+            int hi = (int)floor(rhi[a] * C.gs[a] + C.g0[a] + C.dg[a]);
+            if (C.gbc[a]) { lo = max(lo, 0); hi = min(hi, C.nc[a] - 1); }
+            else if (hi - lo + 1 > C.nc[a]) hi = lo + C.nc[a] - 1;                    // whole periodic axis: once
+            clo[a] = lo; cnt[a] = max(hi - lo + 1, 0);
+        }
+        const int total = cnt[0] * cnt[1] * cnt[2];
+        for (int c = tid; c < total; c += PSM_BLOCK) {
+            int g[3] = {clo[0] + c % cnt[0], clo[1] + (c / cnt[0]) % cnt[1], clo[2] + c / (cnt[0] * cnt[1])};
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                if (!C.gbc[a]) g[a] = (g[a] % C.nc[a] + C.nc[a]) % C.nc[a];
+            const uint32_t gc = (uint32_t)(g[0] + C.nc[0] * (g[1] + C.nc[1] * g[2]));
+            const uint32_t b = C.cell_start[gc], e = C.cell_end[gc];
+            for (uint32_t t = b; t < e; ++t) {
+                PsmCand pc;
+                psm_load_cand(C, t, pc);
+                // distance of the row (y, z fixed) from the sphere centre, nearest images
+                const double dy = (double)(pc.fk[1] + cpl_offset(y, pc.fk[1], P.ny, !P.bc[1])) - pc.xk[1];
+                const double dz = (double)(pc.fk[2] + cpl_offset(z, pc.fk[2], P.nz, !P.bc[2])) - pc.xk[2];
+                const double reach = pc.Rk + C.rc;
+                if (dy * dy + dz * dz > reach * reach * (1.0 + 1e-12)) continue;
+                const int slot = atomicAdd(&s_n, 1);
+                if (slot < PSM_MAXC) cand[slot] = pc;
             }
         }
     }
-
+    __syncthreads();
+    if (!active) return;
+    const int ncand = s_n;
+    const int r[3] = {x, y, z};
     double rho, ux, uy, uz;
     lb_moments(f, rho, ux, uy, uz);
-    if (id0 == 0xffffffffu) {
-        lb_collide_bgk(f, P.omega, rho, ux, uy, uz);                         // plain collide-and-stream
+    if (ncand == 0) {
+        lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
+    } else if (ncand > PSM_MAXC) {
+        // the out-of-line cold path gets a copy, so that f itself never has its address taken (it would
+        // otherwise live in local memory for the whole kernel)
+        double tmp[LEDDS_Q];
+#pragma unroll
+        for (int q = 0; q < LEDDS_Q; ++q) tmp[q] = f[q];
+        psm_cell_global_search(P, C, r, tmp, rho, ux, uy, uz);
+#pragma unroll
+        for (int q = 0; q < LEDDS_Q; ++q) f[q] = tmp[q];
     } else {
-        if (extra) {
-            // more than two solids (PAPER.md:515 allows two): flag it and give every dropped solid a
-            // zero partial so that its reduction never reads a stale entry
-            atomicOr(C.status, LEDDS_ST_SOLID_OVERFLOW);
-            for (int gz = clo[2]; gz <= chi[2]; ++gz)
-                for (int gy = clo[1]; gy <= chi[1]; ++gy)
-                    for (int gx = clo[0]; gx <= chi[0]; ++gx) {
-                        const int wz = C.gbc[2] ? gz : (gz % C.nc[2] + C.nc[2]) % C.nc[2];
-                        const int wy = C.gbc[1] ? gy : (gy % C.nc[1] + C.nc[1]) % C.nc[1];
-                        const int wx = C.gbc[0] ? gx : (gx % C.nc[0] + C.nc[0]) % C.nc[0];
-                        const uint32_t gc = (uint32_t)(wx + C.nc[0] * (wy + C.nc[1] * wz));
-                        for (uint32_t t = C.cell_start[gc]; t < C.cell_end[gc]; ++t) {
-                            const uint32_t id = C.sidx[t];
-                            if (id == id0 || id == id1) continue;
-                            double d[3];
-                            int loc[3];
-                            for (int a = 0; a < 3; ++a) {
-                                const double xk = (C.xs[3 * t + a] - C.origin[a]) * C.inv_dx;
-                                const int fk = (int)floor(xk);
-                                const int di = cpl_offset(r[a], fk, nl[a], !P.bc[a]);
-                                d[a] = (double)(fk + di) - xk;
-                                loc[a] = di + C.H;
-                            }
-                            if (!(cpl_dsc(C.rs[t] * C.inv_dx, C.rc, cpl_dist(d)) > 0.0)) continue;
-                            double* e = C.boxes + (((long long)id * C.S + loc[2]) * C.S + loc[1]) * C.S * 6 + (long long)loc[0] * 6;
-                            for (int c = 0; c < 6; ++c) e[c] = 0.0;
-                        }
-                    }
+        uint32_t id0 = 0xffffffffu, id1 = 0xffffffffu;
+        int c0 = 0, c1 = 0;
+        bool dropped = false;
+        for (int ci = 0; ci < ncand; ++ci) {
+            const PsmCand& pc = cand[ci];
+            double d[3]; int loc[3];
+            psm_rel(P, C, r, pc, d, loc);
+            if (!(cpl_dsc(pc.Rk, C.rc, cpl_dist(d)) > 0.0)) continue;
+            dropped |= psm_select(pc.id, ci, id0, id1, c0, c1);
         }
-        double fe[LEDDS_Q], solid[LEDDS_Q];
-        lb_equilibrium(fe, rho, ux, uy, uz);
-#pragma unroll
-        for (int q = 0; q < LEDDS_Q; ++q) solid[q] = 0.0;
-        double Bsum = 0.0;
-        const int ns = id1 == 0xffffffffu ? 1 : 2;
-        for (int s = 0; s < ns; ++s) {
-            const uint32_t t = s ? t1 : t0, id = s ? id1 : id0;
-            double d[3], xk[3];
-            int loc[3];
-#pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                xk[a] = (C.xs[3 * t + a] - C.origin[a]) * C.inv_dx;
-                const int fk = (int)floor(xk[a]);
-                const int di = cpl_offset(r[a], fk, nl[a], !P.bc[a]);
-                d[a] = (double)(fk + di) - xk[a];
-                loc[a] = di + C.H;
+        if (id0 == 0xffffffffu) {
+            lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
+        } else {
+            psm_cell(P, C, r, f, rho, ux, uy, uz, cand[c0], cand[c1], id1 == 0xffffffffu ? 1 : 2);
+            if (dropped) {
+                atomicOr(C.status, LEDDS_ST_SOLID_OVERFLOW);
+                for (int ci = 0; ci < ncand; ++ci)
+                    if (cand[ci].id != id0 && cand[ci].id != id1) psm_zero_dropped(P, C, r, cand[ci]);
             }
-            const double Rk = C.rs[t] * C.inv_dx;
-            const double dsc = cpl_dsc(Rk, C.rc, cpl_dist(d));
-            const double beta = dsc >= 2.0 * C.rc ? 1.0 : dsc / (2.0 * C.rc);           // Eq. (39)
-            const double B = beta * (P.tau - 0.5) / ((1.0 - beta) + (P.tau - 0.5));     // Eq. (36)
-            const double vk[3] = {C.vps[3 * t] * C.vscale, C.vps[3 * t + 1] * C.vscale, C.vps[3 * t + 2] * C.vscale};
-            const double wk[3] = {C.wps[3 * t] * C.wscale, C.wps[3 * t + 1] * C.wscale, C.wps[3 * t + 2] * C.wscale};
-            const double ukx = vk[0] + (wk[1] * d[2] - wk[2] * d[1]);                   // Eq. (35)
-            const double uky = vk[1] + (wk[2] * d[0] - wk[0] * d[2]);
-            const double ukz = vk[2] + (wk[0] * d[1] - wk[1] * d[0]);
-            double fk_eq[LEDDS_Q];
-            lb_equilibrium(fk_eq, rho, ukx, uky, ukz);
-            double sx = 0.0, sy = 0.0, sz = 0.0;
-#pragma unroll
-            for (int q = 0; q < LEDDS_Q; ++q) {
-                const int o = lb_opp(q);
-                const double Os = (f[o] - fe[o]) - (f[q] - fk_eq[q]);                   // Eq. (34)
-                if (lb_cx(q) == 1) sx += Os; else if (lb_cx(q) == -1) sx -= Os;
-                if (lb_cy(q) == 1) sy += Os; else if (lb_cy(q) == -1) sy -= Os;
-                if (lb_cz(q) == 1) sz += Os; else if (lb_cz(q) == -1) sz -= Os;
-                solid[q] += B * Os;
-            }
-            Bsum += B;
-            const double dF[3] = {-B * sx, -B * sy, -B * sz};                           // Eq. (41), lattice units
-            double* e = C.boxes + (((long long)id * C.S + loc[2]) * C.S + loc[1]) * C.S * 6 + (long long)loc[0] * 6;
-            e[0] = dF[0]; e[1] = dF[1]; e[2] = dF[2];
-            e[3] = d[1] * dF[2] - d[2] * dF[1];                                         // Eq. (42)
-            e[4] = d[2] * dF[0] - d[0] * dF[2];
-            e[5] = d[0] * dF[1] - d[1] * dF[0];
-        }
-        const double Btot = Bsum < 1.0 ? Bsum : 1.0;                                    // Eq. (37)
-#pragma unroll
-        for (int q = 0; q < LEDDS_Q; ++q) {
-            const double bgk = -P.omega * (f[q] - fe[q]);
-            f[q] = f[q] + ((1.0 - Btot) * bgk + solid[q]);                              // Eq. (32)-(33)
         }
     }
     lb_push_store(fout, P, x, y, z, f, rho);
