@@ -149,13 +149,20 @@ typedef struct {
     double origin[3];     /* DEM coordinates of lattice node (0,0,0)                              */
 } ledds_cpl_params;
 
+/* Size of the coupling scratch: one uint32 pair per fluid cell (the solids cutting it) + per solid
+ * (2H+2)^2 row partials of Eq. (41)-(42), H = ceil(r_max/dx + 0.6204).  r_max = largest radius. */
 int ledds_cpl_workspace_bytes(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_params* c,
                               const double r_max, size_t* cpl_scratch_bytes);
 
+/* Prepares cpl_scratch (all cell slots empty, no row partial current).  Call once before the first
+ * ledds_coupled_step on this scratch, with the same lbm / dem / c / r_max. */
+int ledds_cpl_init(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_params* c, double r_max,
+                   void* cpl_scratch, void* stream);
+
 /* nsteps coupled steps.  f_hyd / m_hyd [n][3]: in = hydrodynamic force / torque of the previous
- * LBM step (zeros before the first), out = those of this step (DEM units).  The DEM grid
- * spacing must be >= 2 (r_max + 0.6204 dx) so that the solids cutting a fluid cell are found
- * in the 2x2x2 grid cells around it.  r_max = largest radius (as passed to the workspace query). */
+ * LBM step (zeros before the first), out = those of this step (DEM units).  The lattice and the DEM
+ * box must have the same topology (bc); a periodic lattice axis must be at least 2 (2H+2) long
+ * (unique nearest image); 2H+2 <= 128.  LEDDS_EINVAL otherwise. */
 int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c, double r_max, double* f,
                        double* x, double* v, double* w, double* a, double* alpha, const double* radius,
                        double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
@@ -171,6 +178,7 @@ int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c
 #define LEDDS_K_DEM_CONTACT 4  /* contact detection + forces    */
 #define LEDDS_K_DEM_KICK 5     /* velocity update               */
 #define LEDDS_K_CPL_REDUCE 6   /* per-particle hydrodynamic sum */
+#define LEDDS_K_CPL_RASTER 7   /* solids -> per-cell slots      */
 /* enable != 0: start recording (previous records are dropped); 0: stop and drop. */
 int ledds_profile(int enable);
 /* Sum of the recorded durations [ms] and number of recorded launches of one kernel group;

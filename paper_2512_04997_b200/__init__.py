@@ -21,7 +21,7 @@ LEDDS_OK, LEDDS_EINVAL, LEDDS_EALIGN, LEDDS_ECAPACITY, LEDDS_ECUDA = 0, -1, -2, 
 ST_CONTACT_OVERFLOW, ST_SOLID_OVERFLOW, ST_COINCIDENT, ST_NONFINITE = 1, 2, 4, 8
 EXPORTS = ["ledds_lbm_workspace_bytes", "ledds_lbm_init", "ledds_lbm_import", "ledds_lbm_step", "ledds_lbm_export",
            "ledds_lbm_current", "ledds_lbm_destroy", "ledds_dem_workspace_bytes", "ledds_dem_init", "ledds_dem_step",
-           "ledds_dem_query", "ledds_dem_destroy", "ledds_cpl_workspace_bytes", "ledds_coupled_step", "ledds_version",
+           "ledds_dem_query", "ledds_dem_destroy", "ledds_cpl_workspace_bytes", "ledds_cpl_init", "ledds_coupled_step", "ledds_version",
            "ledds_profile", "ledds_profile_read", "ledds_launch_count"]
 
 
@@ -71,8 +71,8 @@ for _n in EXPORTS:
 _lib.ledds_version.restype = C.c_char_p
 _lib.ledds_lbm_current.restype = C.c_void_p
 _lib.ledds_launch_count.restype = C.c_ulonglong
-K_LBM, K_DEM_KEYS, K_DEM_SORT, K_DEM_GATHER, K_DEM_CONTACT, K_DEM_KICK, K_CPL_REDUCE = range(7)
-KERNEL_GROUPS = ["lbm", "dem_keys", "dem_sort", "dem_gather", "dem_contact", "dem_kick", "cpl_reduce"]
+K_LBM, K_DEM_KEYS, K_DEM_SORT, K_DEM_GATHER, K_DEM_CONTACT, K_DEM_KICK, K_CPL_REDUCE, K_CPL_RASTER = range(8)
+KERNEL_GROUPS = ["lbm", "dem_keys", "dem_sort", "dem_gather", "dem_contact", "dem_kick", "cpl_reduce", "cpl_raster"]
 
 
 def lbm_params(d) -> LbmParams:
@@ -197,6 +197,10 @@ def ledds_cpl_workspace_bytes(lbm, dem, c: CplParams, r_max: float) -> int:
     n = C.c_size_t(0)
     _check(_lib.ledds_cpl_workspace_bytes(lbm, dem, C.byref(c), C.c_double(r_max), C.byref(n)), "ledds_cpl_workspace_bytes")
     return n.value
+
+
+def ledds_cpl_init(lbm, dem, c: CplParams, r_max: float, cpl_scratch):
+    _check(_lib.ledds_cpl_init(lbm, dem, C.byref(c), C.c_double(r_max), _p(cpl_scratch), _stream()), "ledds_cpl_init")
 
 
 def ledds_coupled_step(lbm, dem, c: CplParams, r_max, f, x, v, w, a, alpha, radius, f_hyd, m_hyd, history, scratch,

@@ -1,30 +1,33 @@
-// Device code of the PSM stream-collide kernel (Eq. 32-42).  Included by coupled.cu.
+// Device code of the PSM coupling kernels (Eq. 32-42).  Included by coupled.cu.
 #pragma once
 #include "lbm_kernels.cuh"
 
 #define PSM_BLOCK 128
-#define PSM_MAXC 64
+#define PSM_EMPTY 0xffffffffu
 
+// Layout of the caller-owned coupling scratch (ledds_cpl_workspace_bytes):
+//   slots[N]                      uint2 per fluid cell: the (<= 2, lowest) ids of the solids cutting it,
+//                                 PSM_EMPTY when free.  Written by cpl_raster_kernel, consumed and reset
+//                                 by lbm_psm_kernel, so it is all-empty between steps.
+//   stamps[n][S][S][nseg]         uint32: LBM step that wrote the row partial
+//   rows  [n][S][S][nseg][6]      double: sum over one lattice row segment of the (cell, solid) terms of
+//                                 Eq. (41)-(42); S = 2H+2 rows per axis around floor(x_k)
 struct CplDev {
     int n;
     double rc;                 // Eq. (40) in lattice units
     double inv_dx, vscale, wscale, origin[3];
     double fscale, mscale;     // lattice -> DEM units for force / torque
-    // DEM grid seen from lattice indices: grid coordinate = r * gs + g0, search half-width dg
-    int nc[3], gbc[3];
-    double gs[3], g0[3], dg[3];
-    int H, S;                  // box of partials per solid: S^3 entries of 6 doubles
-    const uint32_t* cell_start; const uint32_t* cell_end; const uint32_t* sidx;
-    const double* xs; const double* vps; const double* wps; const double* rs;
-    double* boxes;
+    int H, S, nseg, nbx;       // box half-width, box width, row segments per row, blocks along x
+    uint32_t stamp;            // id of this LBM step (never 0)
+    const double* x; const double* vp; const double* wp; const double* radius;   // particle order
+    uint2* slots;
+    uint32_t* stamps;
+    double* rows;
     int32_t* status;
 };
 
-// A solid that may cut cells of the row segment a block works on (lattice units).
-struct PsmCand { double xk[3], Rk; int fk[3]; uint32_t id, t; };
-
-// delta_sc of Eq. (40) > 0, evaluated with explicitly rounded operations so that the collide kernel
-// and the reduce kernel take the same decision for the same (cell, solid).
+// delta_sc of Eq. (40) > 0, evaluated with explicitly rounded operations so that the raster kernel and
+// the collide kernel take the same decision for the same (cell, solid) whatever the compiler contracts.
 __device__ __forceinline__ double cpl_dist(const double* d)
 {
     return __dsqrt_rn(__dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2])));
@@ -40,6 +43,27 @@ __device__ __forceinline__ int cpl_offset(int r, int fk, int n, int periodic)
         else if (2 * di < -n) di += n;
     }
     return di;
+}
+
+__device__ __forceinline__ int cpl_floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
+
+// Ordinal of the PSM_BLOCK-wide block that holds unwrapped lattice coordinate p (periodic images
+// of the row follow each other), used to number the row segments of one solid.
+__device__ __forceinline__ int cpl_block_ordinal(int p, int nx, int nbx)
+{
+    const int per = cpl_floordiv(p, nx);
+    return per * nbx + (p - per * nx) / PSM_BLOCK;
+}
+
+// lattice-unit position of solid k: x_k, floor(x_k), R_k
+__device__ __forceinline__ void cpl_solid(const CplDev& C, uint32_t k, double* xk, int* fk, double& Rk)
+{
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        xk[a] = (C.x[3 * k + a] - C.origin[a]) * C.inv_dx;
+        fk[a] = (int)floor(xk[a]);
+    }
+    Rk = C.radius[k] * C.inv_dx;
 }
 
 // PSM collision of one cell cut by one or two solids (B[1] = 0 when there is one), Eq. (32)-(37), and the
@@ -91,88 +115,54 @@ __device__ __forceinline__ void psm_collide(double (&f)[LEDDS_Q], double omega, 
     }
 }
 
-// lattice-unit state of the solid at sorted position t
-__device__ __forceinline__ void psm_load_cand(const CplDev& C, uint32_t t, PsmCand& c)
-{
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        c.xk[a] = (C.xs[3 * t + a] - C.origin[a]) * C.inv_dx;
-        c.fk[a] = (int)floor(c.xk[a]);
-    }
-    c.Rk = C.rs[t] * C.inv_dx;
-    c.id = C.sidx[t];
-    c.t = t;
-}
+// What a cell contributes to one solid: force and torque terms of Eq. (41)-(42) in lattice units, and
+// where the row partial they are summed into lives.
+struct PsmRecord {
+    double v[6];
+    int row;        // (id * S + lz) * S + ly
+    int xu;         // unwrapped x coordinate of this cell as seen from the solid (fk + di)
+    int x0;         // unwrapped x coordinate of the first cell of the solid's box (fk - H)
+};
 
-// r_j - r_k (nearest image) and the index of cell r inside the solid's box of partials
-__device__ __forceinline__ void psm_rel(const LbmDev& P, const CplDev& C, const int* r, const PsmCand& c, double* d, int* loc)
+// Collision of a cell cut by the solids id[0] (and id[1] unless PSM_EMPTY), Eq. (32)-(37), (39)-(40).
+__device__ __forceinline__ void psm_cell(const LbmDev& P, const CplDev& C, const int* r, double (&f)[LEDDS_Q], double rho,
+                                         double ux, double uy, double uz, const uint32_t (&id)[2], PsmRecord (&rec)[2])
 {
     const int nl[3] = {P.nx, P.ny, P.nz};
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        const int di = cpl_offset(r[a], c.fk[a], nl[a], !P.bc[a]);
-        d[a] = (double)(c.fk[a] + di) - c.xk[a];
-        loc[a] = di + C.H;
-    }
-}
-
-__device__ __forceinline__ double* psm_entry(const CplDev& C, uint32_t id, const int* loc)
-{
-    return C.boxes + ((((long long)id * C.S + loc[2]) * C.S + loc[1]) * C.S + loc[0]) * 6;
-}
-
-// keep the two lowest ids (G24); returns true when a solid had to be dropped
-__device__ __forceinline__ bool psm_select(uint32_t id, int ci, uint32_t& id0, uint32_t& id1, int& c0, int& c1)
-{
-    if (id == id0 || id == id1) return false;
-    if (id < id0) { const bool drop = id1 != 0xffffffffu; id1 = id0; c1 = c0; id0 = id; c0 = ci; return drop; }
-    if (id < id1) { const bool drop = id1 != 0xffffffffu; id1 = id; c1 = ci; return drop; }
-    return true;
-}
-
-// Collision of a cell cut by ns (1 or 2) solids + the partials of Eq. (41)-(42) into the solids' boxes.
-__device__ __forceinline__ void psm_cell(const LbmDev& P, const CplDev& C, const int* r, double (&f)[LEDDS_Q], double rho,
-                                         double ux, double uy, double uz, const PsmCand& p0, const PsmCand& p1, int ns)
-{
     double B[2] = {0.0, 0.0}, uk[2][3] = {{0, 0, 0}, {0, 0, 0}}, d[2][3], soc[2][3];
-    double* entry[2] = {nullptr, nullptr};
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
-        if (s >= ns) continue;
-        const PsmCand& pc = s ? p1 : p0;
-        int loc[3];
-        psm_rel(P, C, r, pc, d[s], loc);
-        const double dsc = cpl_dsc(pc.Rk, C.rc, cpl_dist(d[s]));
-        const double beta = dsc >= 2.0 * C.rc ? 1.0 : dsc / (2.0 * C.rc);             // Eq. (39)
+        if (id[s] == PSM_EMPTY) continue;
+        const uint32_t k = id[s];
+        double xk[3], Rk;
+        int fk[3], loc[3];
+        cpl_solid(C, k, xk, fk, Rk);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const int di = cpl_offset(r[a], fk[a], nl[a], !P.bc[a]);
+            d[s][a] = (double)(fk[a] + di) - xk[a];                                   // r_j - r_k, nearest image
+            loc[a] = di + C.H;
+        }
+        rec[s].row = ((int)k * C.S + loc[2]) * C.S + loc[1];
+        rec[s].xu = fk[0] + loc[0] - C.H;
+        rec[s].x0 = fk[0] - C.H;
+        const double dsc = cpl_dsc(Rk, C.rc, cpl_dist(d[s]));
+        const double beta = dsc >= 2.0 * C.rc ? 1.0 : (dsc > 0.0 ? dsc / (2.0 * C.rc) : 0.0);   // Eq. (39)
         B[s] = beta * (P.tau - 0.5) / ((1.0 - beta) + (P.tau - 0.5));                 // Eq. (36)
-        const uint32_t t = pc.t;
-        const double vk[3] = {C.vps[3 * t] * C.vscale, C.vps[3 * t + 1] * C.vscale, C.vps[3 * t + 2] * C.vscale};
-        const double wk[3] = {C.wps[3 * t] * C.wscale, C.wps[3 * t + 1] * C.wscale, C.wps[3 * t + 2] * C.wscale};
+        const double vk[3] = {C.vp[3 * k] * C.vscale, C.vp[3 * k + 1] * C.vscale, C.vp[3 * k + 2] * C.vscale};
+        const double wk[3] = {C.wp[3 * k] * C.wscale, C.wp[3 * k + 1] * C.wscale, C.wp[3 * k + 2] * C.wscale};
         uk[s][0] = vk[0] + (wk[1] * d[s][2] - wk[2] * d[s][1]);                       // Eq. (35)
         uk[s][1] = vk[1] + (wk[2] * d[s][0] - wk[0] * d[s][2]);
         uk[s][2] = vk[2] + (wk[0] * d[s][1] - wk[1] * d[s][0]);
-        entry[s] = psm_entry(C, pc.id, loc);
     }
     psm_collide(f, P.omega, rho, ux, uy, uz, B, uk, soc);
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
-        if (s >= ns) continue;
+        if (id[s] == PSM_EMPTY) continue;
         const double dF[3] = {-B[s] * soc[s][0], -B[s] * soc[s][1], -B[s] * soc[s][2]};       // Eq. (41), lattice units
-        double* e = entry[s];
-        e[0] = dF[0]; e[1] = dF[1]; e[2] = dF[2];
-        e[3] = d[s][1] * dF[2] - d[s][2] * dF[1];                                     // Eq. (42)
-        e[4] = d[s][2] * dF[0] - d[s][0] * dF[2];
-        e[5] = d[s][0] * dF[1] - d[s][1] * dF[0];
+        rec[s].v[0] = dF[0]; rec[s].v[1] = dF[1]; rec[s].v[2] = dF[2];
+        rec[s].v[3] = d[s][1] * dF[2] - d[s][2] * dF[1];                              // Eq. (42)
+        rec[s].v[4] = d[s][2] * dF[0] - d[s][0] * dF[2];
+        rec[s].v[5] = d[s][0] * dF[1] - d[s][1] * dF[0];
     }
-}
-
-// A dropped solid (more than two in a cell, PAPER.md:515 allows two) gets a zero partial so that its
-// reduction never reads a stale entry.
-__device__ __forceinline__ void psm_zero_dropped(const LbmDev& P, const CplDev& C, const int* r, const PsmCand& pc)
-{
-    double dd[3]; int loc[3];
-    psm_rel(P, C, r, pc, dd, loc);
-    if (!(cpl_dsc(pc.Rk, C.rc, cpl_dist(dd)) > 0.0)) return;
-    double* e = psm_entry(C, pc.id, loc);
-    for (int c = 0; c < 6; ++c) e[c] = 0.0;
 }

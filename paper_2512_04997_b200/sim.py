@@ -108,7 +108,8 @@ class Coupled:
         self.c = L.cpl_params(cpl)
         self.r_max = float(r_max)
         nb = L.ledds_cpl_workspace_bytes(lbm.h, dem.h, self.c, self.r_max)
-        self.cpl_scratch = torch.zeros(max(nb, 16), dtype=torch.uint8, device="cuda")
+        self.cpl_scratch = torch.empty(max(nb, 16), dtype=torch.uint8, device="cuda")
+        L.ledds_cpl_init(lbm.h, dem.h, self.c, self.r_max, self.cpl_scratch)
         self.f_hyd = torch.zeros(dem.n, 3, dtype=torch.float64, device="cuda")
         self.m_hyd = torch.zeros(dem.n, 3, dtype=torch.float64, device="cuda")
 
