@@ -74,20 +74,39 @@ __device__ __forceinline__ int lb_axis_target(const LbmDev& P, int q, int c, int
 }
 
 // Eq. (25) as a push of all 19 post-collision populations of cell (x,y,z), with boundaries.
+// The neighbour coordinates and "this link leaves through a wall" flags are worked out once per axis
+// (y and z are uniform over the block), so a direction costs a predicate, an address and a store.
 __device__ __forceinline__ void lb_push_store(double* __restrict__ fout, const LbmDev& P, int x, int y, int z,
                                               const double (&fs)[LEDDS_Q], double rho)
 {
+    // t[a][0] / t[a][1]: target coordinate for c = -1 / +1; w[a][0] / w[a][1]: link crosses the low / high wall
+    int tx[2] = {x - 1, x + 1}, ty[2] = {y - 1, y + 1}, tz[2] = {z - 1, z + 1};
+    bool wx[2] = {false, false}, wy[2] = {false, false}, wz[2] = {false, false};
+    if (x == 0) { if (P.bc[0]) wx[0] = true; else tx[0] = P.nx - 1; }
+    if (x == P.nx - 1) { if (P.bc[0]) wx[1] = true; else tx[1] = 0; }
+    if (y == 0) { if (P.bc[1]) wy[0] = true; else ty[0] = P.ny - 1; }
+    if (y == P.ny - 1) { if (P.bc[1]) wy[1] = true; else ty[1] = 0; }
+    if (z == 0) { if (P.bc[2]) wz[0] = true; else tz[0] = P.nz - 1; }
+    if (z == P.nz - 1) { if (P.bc[2]) wz[1] = true; else tz[1] = 0; }
     const long long cell = ((long long)z * P.ny + y) * P.nx + x;
 #pragma unroll
     for (int q = 0; q < LEDDS_Q; ++q) {
+        const int cx = lb_cx(q), cy = lb_cy(q), cz = lb_cz(q);
         bool bounced = false;
-        double cuw = 0.0;
-        const int tx = lb_axis_target<0>(P, q, lb_cx(q), x, P.nx, bounced, cuw);
-        const int ty = lb_axis_target<1>(P, q, lb_cy(q), y, P.ny, bounced, cuw);
-        const int tz = lb_axis_target<2>(P, q, lb_cz(q), z, P.nz, bounced, cuw);
-        if (bounced)
+        if (cx != 0) bounced = bounced || wx[cx > 0];
+        if (cy != 0) bounced = bounced || wy[cy > 0];
+        if (cz != 0) bounced = bounced || wz[cz > 0];
+        if (!bounced) {
+            const int ax = cx == 0 ? x : tx[cx > 0], ay = cy == 0 ? y : ty[cy > 0], az = cz == 0 ? z : tz[cz > 0];
+            fout[(long long)q * P.N + ((long long)az * P.ny + ay) * P.nx + ax] = fs[q];
+        } else {
+            double cuw = 0.0;                                   // c_q . u_wall summed over the crossed walls (G19)
+            if (P.any_wall_velocity) {
+                if (cx != 0 && wx[cx > 0]) { const double* uw = P.uw + (0 + (cx > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
+                if (cy != 0 && wy[cy > 0]) { const double* uw = P.uw + (2 + (cy > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
+                if (cz != 0 && wz[cz > 0]) { const double* uw = P.uw + (4 + (cz > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
+            }
             fout[(long long)lb_opp(q) * P.N + cell] = fs[q] - 6.0 * lb_w(q) * rho * cuw;
-        else
-            fout[(long long)q * P.N + ((long long)tz * P.ny + ty) * P.nx + tx] = fs[q];
+        }
     }
 }
