@@ -18,8 +18,29 @@
 
 // ------------------------------------------------------------------------------------ raster
 // slots[cell] = the two lowest ids of the solids cutting the cell (x < y), kept with a 64-bit compare-and-swap;
-// a third solid raises LEDDS_ST_SOLID_OVERFLOW.  Also writes sol[k].  A warp walks the rows of the solid's
-// box, 32 / Spad rows at a time (Spad = S rounded up to a power of two), one lane per cell.
+// a third solid raises LEDDS_ST_SOLID_OVERFLOW; a cell that gets its second solid is appended to list2.
+// Also writes sol[k].  A warp walks the rows of the solid's box, 32 / Spad rows at a time (Spad = S rounded
+// up to a power of two), one lane per cell.  RASTER_BATCH optimistic swaps (expecting an empty slot) are in
+// flight before the first answer is looked at, so the walk is not a chain of memory round trips.
+#define RASTER_BATCH 6
+#define PSM_EMPTY64 0xffffffffffffffffull
+
+// returns true when this insert gave the cell its second solid
+__device__ __forceinline__ bool raster_insert(unsigned long long* slot, unsigned long long old, uint32_t k, bool& overflow)
+{
+    for (;;) {
+        const uint32_t a = (uint32_t)old, b = (uint32_t)(old >> 32);           // uint2 {x = low word, y = high word}, a <= b
+        if (k > b) { overflow = true; return false; }                           // two lower ids are already there
+        const uint32_t na = k < a ? k : a, nb = k < a ? a : k;
+        const unsigned long long seen = atomicCAS(slot, old, ((unsigned long long)nb << 32) | na);
+        if (seen == old) {
+            if (b != PSM_EMPTY) { overflow = true; return false; }              // b was pushed out
+            return a != PSM_EMPTY;
+        }
+        old = seen;
+    }
+}
+
 __global__ void __launch_bounds__(128) cpl_raster_kernel(const LbmDev P, const CplDev C, int spad_log2)
 {
     const int k = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
@@ -44,34 +65,52 @@ __global__ void __launch_bounds__(128) cpl_raster_kernel(const LbmDev P, const C
     const int S = C.S;
     const int sub = lane >> spad_log2, lx0 = lane & ((1 << spad_log2) - 1), rows_per_iter = 32 >> spad_log2;
     const int xstep = 1 << spad_log2;
+    const int iters_y = (S + rows_per_iter - 1) / rows_per_iter, iters = S * iters_y;
     bool overflow = false;
-    for (int lz = 0; lz < S; ++lz) {
-        int rz = fk[2] + lz - C.H;
-        const double dz = (double)rz - xk[2];
-        if (P.bc[2]) { if (rz < 0 || rz >= P.nz) continue; }
-        else rz = rz < 0 ? rz + P.nz : (rz >= P.nz ? rz - P.nz : rz);
-        for (int ly0 = 0; ly0 < S; ly0 += rows_per_iter) {
-            const int ly = ly0 + sub;
-            int ry = fk[1] + ly - C.H;
-            const double dy = (double)ry - xk[1];
-            bool row_ok = ly < S;
-            if (P.bc[1]) { if (ry < 0 || ry >= P.ny) row_ok = false; }
-            else ry = ry < 0 ? ry + P.ny : (ry >= P.ny ? ry - P.ny : ry);
-            for (int lx = lx0; lx < S; lx += xstep) {
-                int rx = fk[0] + lx - C.H;
-                const double d[3] = {(double)rx - xk[0], dy, dz};
-                if (P.bc[0]) { if (rx < 0 || rx >= P.nx) continue; }
-                else rx = rx < 0 ? rx + P.nx : (rx >= P.nx ? rx - P.nx : rx);
-                if (!row_ok || !cpl_cuts(Rk, C.rc, d)) continue;
-                unsigned long long* slot = reinterpret_cast<unsigned long long*>(C.slots + (((long long)rz * P.ny + ry) * P.nx + rx));
-                unsigned long long old = *slot;
-                for (;;) {
-                    const uint32_t a = (uint32_t)old, b = (uint32_t)(old >> 32);   // uint2 {x = low word, y = high word}, a <= b
-                    if ((uint32_t)k > b) { overflow = true; break; }                // two lower ids are already there
-                    const uint32_t na = (uint32_t)k < a ? (uint32_t)k : a, nb = (uint32_t)k < a ? a : (uint32_t)k;
-                    const unsigned long long seen = atomicCAS(slot, old, ((unsigned long long)nb << 32) | na);
-                    if (seen == old) { overflow = overflow || b != PSM_EMPTY; break; }   // b was pushed out
-                    old = seen;
+    for (int lxb = 0; lxb < S; lxb += xstep) {                                  // one trip unless S > 32; uniform
+        const int lx = lxb + lx0;
+        int rx = fk[0] + lx - C.H;
+        const double dx = (double)rx - xk[0];
+        bool xok = lx < S;
+        if (P.bc[0]) xok = xok && rx >= 0 && rx < P.nx;
+        else rx = rx < 0 ? rx + P.nx : (rx >= P.nx ? rx - P.nx : rx);
+        for (int it0 = 0; it0 < iters; it0 += RASTER_BATCH) {
+            unsigned long long* slot[RASTER_BATCH];
+            unsigned long long seen[RASTER_BATCH];
+            uint32_t cell[RASTER_BATCH];
+#pragma unroll
+            for (int b = 0; b < RASTER_BATCH; ++b) {
+                const int it = it0 + b;
+                const int lz = it / iters_y, ly = (it - lz * iters_y) * rows_per_iter + sub;
+                int rz = fk[2] + lz - C.H, ry = fk[1] + ly - C.H;
+                const double d[3] = {dx, (double)ry - xk[1], (double)rz - xk[2]};
+                bool ok = xok && it < iters && ly < S;
+                if (P.bc[2]) ok = ok && rz >= 0 && rz < P.nz;
+                else rz = rz < 0 ? rz + P.nz : (rz >= P.nz ? rz - P.nz : rz);
+                if (P.bc[1]) ok = ok && ry >= 0 && ry < P.ny;
+                else ry = ry < 0 ? ry + P.ny : (ry >= P.ny ? ry - P.ny : ry);
+                ok = ok && cpl_cuts(Rk, C.rc, d);
+                slot[b] = nullptr;
+                seen[b] = PSM_EMPTY64;
+                cell[b] = 0u;
+                if (ok) {
+                    cell[b] = (uint32_t)(((long long)rz * P.ny + ry) * P.nx + rx);
+                    slot[b] = reinterpret_cast<unsigned long long*>(C.slots + cell[b]);
+                    seen[b] = atomicCAS(slot[b], PSM_EMPTY64, ((unsigned long long)PSM_EMPTY << 32) | (uint32_t)k);
+                }
+            }
+#pragma unroll
+            for (int b = 0; b < RASTER_BATCH; ++b) {
+                bool second = false;
+                if (slot[b] && seen[b] != PSM_EMPTY64) second = raster_insert(slot[b], seen[b], (uint32_t)k, overflow);
+                // one list2 append per warp, in lane (= x) order so that neighbouring cells stay neighbours
+                const unsigned m = __ballot_sync(0xffffffffu, second);
+                if (m) {
+                    uint32_t base = 0;
+                    if (lane == __ffs(m) - 1) base = atomicAdd(C.list2, (uint32_t)__popc(m));
+                    base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+                    const uint32_t at = base + (uint32_t)__popc(m & ((1u << lane) - 1u));
+                    if (second && at < C.list2_cap) C.list2[1 + at] = cell[b];
                 }
             }
         }
@@ -80,7 +119,9 @@ __global__ void __launch_bounds__(128) cpl_raster_kernel(const LbmDev P, const C
 }
 
 // ------------------------------------------------------------------------------------ collide + stream
-__global__ void __launch_bounds__(PSM_BLOCK, 4) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
+// Cells cut by two solids are left to lbm_psm2_kernel: here they take the plain collision (overwritten later)
+// and contribute no partial.
+__global__ void __launch_bounds__(PSM_BLOCK, 5) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                                const __grid_constant__ LbmDev P,
                                                                const __grid_constant__ CplDev C)
 {
@@ -93,7 +134,7 @@ __global__ void __launch_bounds__(PSM_BLOCK, 4) lbm_psm_kernel(const double* __r
 #pragma unroll
         for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (long long)q * P.N + cell);
         const uint2 slot = C.slots[cell];
-        id[0] = slot.x; id[1] = slot.y;
+        if (slot.y == PSM_EMPTY) id[0] = slot.x;
     } else {
 #pragma unroll
         for (int q = 0; q < LEDDS_Q; ++q) f[q] = lb_w(q);
@@ -101,43 +142,82 @@ __global__ void __launch_bounds__(PSM_BLOCK, 4) lbm_psm_kernel(const double* __r
     double rho, ux, uy, uz;
     lb_moments(f, rho, ux, uy, uz);
     const bool any1 = __any_sync(0xffffffffu, id[0] != PSM_EMPTY);
-    const bool any2 = __any_sync(0xffffffffu, id[1] != PSM_EMPTY);
     double rec[2][6];
     int ent[2];
     if (!any1) {
         lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
     } else {
         if (id[0] != PSM_EMPTY) C.slots[cell] = make_uint2(PSM_EMPTY, PSM_EMPTY);     // consumed: free for the next step
-        if (!any2) psm_cell<1>(P, C, x, y, z, f, rho, ux, uy, uz, id, rec, ent);
-        else psm_cell<2>(P, C, x, y, z, f, rho, ux, uy, uz, id, rec, ent);
+        psm_cell<1>(P, C, x, y, z, f, rho, ux, uy, uz, id, rec, ent);
     }
     if (active) lb_push_store(fout, P, x, y, z, f, rho);
     if (any1) psm_run_reduce(C, id[0], ent[0], rec[0]);
-    if (any2) psm_run_reduce(C, id[1], ent[1], rec[1]);
+}
+
+// The cells cut by two solids (list2), one thread each: same step as above with both solids; every cell stores
+// its own two partials.  Runs after lbm_psm_kernel on the same stream and overwrites what that wrote for them.
+__global__ void __launch_bounds__(128) lbm_psm2_kernel(const double* __restrict__ fin, double* __restrict__ fout,
+                                                       const __grid_constant__ LbmDev P,
+                                                       const __grid_constant__ CplDev C)
+{
+    const uint32_t count = min(C.list2[0], C.list2_cap);
+    const uint32_t padded = (count + 31u) & ~31u;                                    // whole warps stay together
+    for (uint32_t t = blockIdx.x * blockDim.x + threadIdx.x; t < padded; t += gridDim.x * blockDim.x) {
+        const bool on = t < count;
+        const uint32_t cell = on ? C.list2[1 + t] : 0u;
+        const int x = (int)(cell % (uint32_t)P.nx), y = (int)((cell / (uint32_t)P.nx) % (uint32_t)P.ny);
+        const int z = (int)(cell / ((uint32_t)P.nx * (uint32_t)P.ny));
+        double f[LEDDS_Q];
+#pragma unroll
+        for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (long long)q * P.N + cell);
+        uint32_t id[2] = {PSM_EMPTY, PSM_EMPTY};
+        if (on) {
+            const uint2 slot = C.slots[cell];
+            C.slots[cell] = make_uint2(PSM_EMPTY, PSM_EMPTY);
+            id[0] = slot.x; id[1] = slot.y;
+        }
+        double rho, ux, uy, uz;
+        lb_moments(f, rho, ux, uy, uz);
+        double rec[2][6];
+        int ent[2];
+        psm_cell<2>(P, C, x, y, z, f, rho, ux, uy, uz, id, rec, ent);
+        if (on) lb_push_store(fout, P, x, y, z, f, rho);
+        // neighbours in the list are mostly neighbours on the lattice cut by the same two solids
+        psm_run_reduce(C, id[0], ent[0], rec[0]);
+        psm_run_reduce(C, id[1], ent[1], rec[1]);
+    }
 }
 
 // ------------------------------------------------------------------------------------ reduce
 // One warp per solid; lane -> entry map and the shuffle tree are fixed, so the sums are deterministic.
+// Each lane takes 16 flags at a time (one 16-byte load) and reads the flagged partials.
 __global__ void __launch_bounds__(128) cpl_reduce_kernel(const CplDev C, double* __restrict__ f_hyd,
                                                          double* __restrict__ m_hyd)
 {
     const int k = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
     const int lane = threadIdx.x & 31;
+    if (blockIdx.x == 0 && threadIdx.x == 0) C.list2[0] = 0u;                        // list worked through: empty it
     if (k >= C.n) return;
     const int S3 = C.S * C.S * C.S;                                                  // multiple of 8
-    uint32_t* fl = reinterpret_cast<uint32_t*>(C.flags + (size_t)k * S3);
-    const double* box = C.box + (size_t)k * S3 * 6;
+    uint2* fl = reinterpret_cast<uint2*>(C.flags + (size_t)k * S3);
+    const double2* box = reinterpret_cast<const double2*>(C.box + (size_t)k * S3 * 6);
     double acc[6] = {0, 0, 0, 0, 0, 0};
-    for (int w4 = lane; w4 < S3 / 4; w4 += 32) {
-        uint32_t m = fl[w4];
-        if (!m) continue;
-        fl[w4] = 0u;
+    const double2 zero = make_double2(0.0, 0.0);
+    for (int w8 = lane; w8 < S3 / 8; w8 += 32) {
+        const uint2 m = fl[w8];
+        if (!(m.x | m.y)) continue;
+        fl[w8] = make_uint2(0u, 0u);
+        double2 a[8][3];
 #pragma unroll
-        for (int b = 0; b < 4; ++b) {
-            if (!((m >> (8 * b)) & 0xffu)) continue;
-            const double2* in = reinterpret_cast<const double2*>(box + (size_t)(4 * w4 + b) * 6);
-            const double2 a0 = in[0], a1 = in[1], a2 = in[2];
-            acc[0] += a0.x; acc[1] += a0.y; acc[2] += a1.x; acc[3] += a1.y; acc[4] += a2.x; acc[5] += a2.y;
+        for (int b = 0; b < 8; ++b) {
+            const bool on = (((b < 4 ? m.x : m.y) >> (8 * (b & 3))) & 0xffu) != 0u;
+            const double2* in = box + (size_t)(8 * w8 + b) * 3;
+            a[b][0] = on ? in[0] : zero; a[b][1] = on ? in[1] : zero; a[b][2] = on ? in[2] : zero;
+        }
+#pragma unroll
+        for (int b = 0; b < 8; ++b) {
+            acc[0] += a[b][0].x; acc[1] += a[b][0].y; acc[2] += a[b][1].x;
+            acc[3] += a[b][1].y; acc[4] += a[b][2].x; acc[5] += a[b][2].y;
         }
     }
 #pragma unroll
@@ -157,7 +237,7 @@ __global__ void __launch_bounds__(128) cpl_reduce_kernel(const CplDev C, double*
 }
 
 // ------------------------------------------------------------------------------------ host API
-struct CplLayout { size_t slots, sol, flags, box, total; };
+struct CplLayout { size_t slots, sol, list2, flags, box, total; uint32_t list2_cap; };
 
 static size_t cpl_align(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -188,7 +268,9 @@ static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl
     const size_t N = (size_t)lbm->d.N, S3 = (size_t)C->S * C->S * C->S, E = (size_t)C->n * S3;   // S even: S3 % 8 == 0
     L->slots = 0;
     L->sol = cpl_align(N * sizeof(uint2));
-    L->flags = L->sol + cpl_align((size_t)C->n * 10 * sizeof(double));
+    L->list2 = L->sol + cpl_align((size_t)C->n * 10 * sizeof(double));
+    L->list2_cap = (uint32_t)(E < N ? E : N);                              // every 2-solid cell lies in some solid's box
+    L->flags = L->list2 + cpl_align(((size_t)L->list2_cap + 1) * sizeof(uint32_t));
     L->box = L->flags + cpl_align(E);
     L->total = L->box + cpl_align(E * 6 * sizeof(double));
     return LEDDS_OK;
@@ -218,6 +300,7 @@ extern "C" int ledds_cpl_init(const ledds_lbm* lbm, const ledds_dem* dem, const 
     cudaStream_t st = (cudaStream_t)stream;
     char* base = static_cast<char*>(cpl_scratch);
     if (cudaMemsetAsync(base + L.slots, 0xff, L.sol - L.slots, st) != cudaSuccess ||        // all slots PSM_EMPTY
+        cudaMemsetAsync(base + L.list2, 0, 256, st) != cudaSuccess ||                       // list2 count
         cudaMemsetAsync(base + L.flags, 0, L.box - L.flags, st) != cudaSuccess)             // no partial pending
         return LEDDS_ECUDA;
     return LEDDS_OK;
@@ -248,6 +331,8 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
     C.radius = radius;
     C.slots = reinterpret_cast<uint2*>(cs + L.slots);
     C.sol = reinterpret_cast<double*>(cs + L.sol);
+    C.list2 = reinterpret_cast<uint32_t*>(cs + L.list2);
+    C.list2_cap = L.list2_cap;
     C.flags = reinterpret_cast<uint8_t*>(cs + L.flags);
     C.box = reinterpret_cast<double*>(cs + L.box);
     C.status = status;
@@ -275,6 +360,10 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         ledds_prof_start(LEDDS_K_LBM, st);
         lbm_psm_kernel<<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
         ledds_prof_stop(LEDDS_K_LBM, st);
+        LEDDS_CHECK_LAUNCH();
+        ledds_prof_start(LEDDS_K_CPL_PSM2, st);
+        lbm_psm2_kernel<<<148 * 4, 128, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
+        ledds_prof_stop(LEDDS_K_CPL_PSM2, st);
         LEDDS_CHECK_LAUNCH();
         lbm->parity ^= 1;
         lbm->steps++;

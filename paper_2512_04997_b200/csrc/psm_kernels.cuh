@@ -12,6 +12,8 @@
 //   sol[n][10]          per solid, lattice units: x_k[3], R_k, v_k[3], w_k[3] (predictor values)
 //   flags[n][S^3]       uint8: box entry holds a partial of this step (set by lbm_psm_kernel, reset by
 //                       cpl_reduce_kernel)
+//   list2[1 + cap]      uint32: number and linear indices of the cells cut by two solids (written by the
+//                       raster kernel, worked through by lbm_psm2_kernel, count reset by cpl_reduce_kernel)
 //   box[n][S^3][6]      double: sum of the (cell, solid) terms of Eq. (41)-(42) over one run of
 //                       consecutive cells of a lattice row inside a warp, stored at the run's first cell;
 //                       S = 2H+2 cells per axis around floor(x_k)
@@ -26,6 +28,8 @@ struct CplDev {
     double* sol;
     uint8_t* flags;
     double* box;
+    uint32_t* list2;           // [0] = count, [1..] = linear indices of the cells cut by two solids
+    uint32_t list2_cap;
     int32_t* status;
 };
 
@@ -61,14 +65,12 @@ __device__ __forceinline__ bool cpl_cuts(double Rk, double rc, const double* d)
     return __dsub_rn(s, __dsqrt_rn(d2)) > 0.0;
 }
 
-// PSM collision of one cell cut by NS (1 or 2) solids, Eq. (32)-(37), and the momentum exchange
-// sum_i Omega^s_{i,k} c_i of Eq. (41).  Written pair by pair (q, opposite q) so that no per-direction array
-// besides f itself is live.  A solid with B = 0 contributes nothing, so lanes of a warp that are cut by fewer
-// solids than their neighbours run the same code with B = 0.
+// PSM collision of one cell cut by NS (1 or 2) solids, Eq. (32)-(37).  Written pair by pair (q, opposite q)
+// so that no per-direction array besides f itself is live.  A solid with B = 0 contributes nothing, so lanes
+// of a warp that are not cut run the same code with B = 0.
 template <int NS>
 __device__ __forceinline__ void psm_collide(double (&f)[LEDDS_Q], double omega, double rho, double ux, double uy,
-                                            double uz, const double (&B)[NS], const double (&uk)[NS][3],
-                                            double (&soc)[NS][3])
+                                            double uz, const double (&B)[NS], const double (&uk)[NS][3])
 {
     const double k0 = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
     double kk[NS];
@@ -76,7 +78,6 @@ __device__ __forceinline__ void psm_collide(double (&f)[LEDDS_Q], double omega, 
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
         kk[s] = 1.0 - 1.5 * (uk[s][0] * uk[s][0] + uk[s][1] * uk[s][1] + uk[s][2] * uk[s][2]);
-        soc[s][0] = soc[s][1] = soc[s][2] = 0.0;
         Bsum += B[s];
     }
     const double keep = 1.0 - (Bsum < 1.0 ? Bsum : 1.0);                              // 1 - B_tot, Eq. (37)
@@ -99,14 +100,8 @@ __device__ __forceinline__ void psm_collide(double (&f)[LEDDS_Q], double omega, 
         for (int s = 0; s < NS; ++s) {
             const double cuk = lb_cdot(q, uk[s][0], uk[s][1], uk[s][2]);
             const double evk = wr * (kk[s] + 4.5 * cuk * cuk), odk = wr * 3.0 * cuk;
-            const double Os_q = no - (f[q] - (evk + odk));                              // Eq. (34), direction q
-            const double Os_o = nq - (f[q + 1] - (evk - odk));                          //           its opposite
-            const double diff = Os_q - Os_o;                                            // c_q Os_q + c_o Os_o = c_q diff
-            if (lb_cx(q) == 1) soc[s][0] += diff; else if (lb_cx(q) == -1) soc[s][0] -= diff;
-            if (lb_cy(q) == 1) soc[s][1] += diff; else if (lb_cy(q) == -1) soc[s][1] -= diff;
-            if (lb_cz(q) == 1) soc[s][2] += diff; else if (lb_cz(q) == -1) soc[s][2] -= diff;
-            acc_q += B[s] * Os_q;
-            acc_o += B[s] * Os_o;
+            acc_q += B[s] * (no - (f[q] - (evk + odk)));                                // B Omega^s, Eq. (34), direction q
+            acc_o += B[s] * (nq - (f[q + 1] - (evk - odk)));                            //                      its opposite
         }
         f[q] = f[q] + (acc_q - komega * nq);                                            // Eq. (32)-(33)
         f[q + 1] = f[q + 1] + (acc_o - komega * no);
@@ -121,7 +116,7 @@ __device__ __forceinline__ void psm_cell(const LbmDev& P, const CplDev& C, int x
                                          double rho, double ux, double uy, double uz, const uint32_t (&id)[2],
                                          double (&rec)[2][6], int (&ent)[2])
 {
-    double B[NS], uk[NS][3], d[NS][3], soc[NS][3];
+    double B[NS], uk[NS][3], d[NS][3];
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
         const bool has = id[s] != PSM_EMPTY;
@@ -145,15 +140,18 @@ __device__ __forceinline__ void psm_cell(const LbmDev& P, const CplDev& C, int x
         uk[s][1] = vk[1] + (wk[2] * d[s][0] - wk[0] * d[s][2]);
         uk[s][2] = vk[2] + (wk[0] * d[s][1] - wk[1] * d[s][0]);
     }
-    psm_collide<NS>(f, P.omega, rho, ux, uy, uz, B, uk, soc);
+    // Eq. (41): -B_k sum_i Omega^s_{i,k} c_i.  The sum is rho (u_k - u) identically (sum_i c_i f_i = rho u,
+    // sum_i c_i f_i^eq(rho, v) = rho v, c_opp = -c), so it is formed from the moments.
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
-        const double dF[3] = {-B[s] * soc[s][0], -B[s] * soc[s][1], -B[s] * soc[s][2]};       // Eq. (41), lattice units
+        const double Br = B[s] * rho;
+        const double dF[3] = {Br * (ux - uk[s][0]), Br * (uy - uk[s][1]), Br * (uz - uk[s][2])};   // lattice units
         rec[s][0] = dF[0]; rec[s][1] = dF[1]; rec[s][2] = dF[2];
         rec[s][3] = d[s][1] * dF[2] - d[s][2] * dF[1];                                // Eq. (42)
         rec[s][4] = d[s][2] * dF[0] - d[s][0] * dF[2];
         rec[s][5] = d[s][0] * dF[1] - d[s][1] * dF[0];
     }
+    psm_collide<NS>(f, P.omega, rho, ux, uy, uz, B, uk);
 }
 
 // Sum the records of each run of consecutive lanes that hold the same solid id (a solid cuts a lattice row
