@@ -179,7 +179,6 @@ int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c
 #define LEDDS_K_DEM_KICK 5     /* velocity update               */
 #define LEDDS_K_CPL_REDUCE 6   /* per-particle hydrodynamic sum */
 #define LEDDS_K_CPL_RASTER 7   /* solids -> per-cell slots      */
-#define LEDDS_K_CPL_PSM2 8     /* cells cut by two solids       */
 /* enable != 0: start recording (previous records are dropped); 0: stop and drop. */
 int ledds_profile(int enable);
 /* Sum of the recorded durations [ms] and number of recorded launches of one kernel group;

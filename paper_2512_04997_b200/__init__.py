@@ -71,8 +71,8 @@ for _n in EXPORTS:
 _lib.ledds_version.restype = C.c_char_p
 _lib.ledds_lbm_current.restype = C.c_void_p
 _lib.ledds_launch_count.restype = C.c_ulonglong
-K_LBM, K_DEM_KEYS, K_DEM_SORT, K_DEM_GATHER, K_DEM_CONTACT, K_DEM_KICK, K_CPL_REDUCE, K_CPL_RASTER, K_CPL_PSM2 = range(9)
-KERNEL_GROUPS = ["lbm", "dem_keys", "dem_sort", "dem_gather", "dem_contact", "dem_kick", "cpl_reduce", "cpl_raster", "cpl_psm2"]
+K_LBM, K_DEM_KEYS, K_DEM_SORT, K_DEM_GATHER, K_DEM_CONTACT, K_DEM_KICK, K_CPL_REDUCE, K_CPL_RASTER = range(8)
+KERNEL_GROUPS = ["lbm", "dem_keys", "dem_sort", "dem_gather", "dem_contact", "dem_kick", "cpl_reduce", "cpl_raster"]
 
 
 def lbm_params(d) -> LbmParams:

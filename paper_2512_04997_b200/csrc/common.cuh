@@ -9,7 +9,7 @@
 #define LEDDS_Q 19
 
 // kernel groups for ledds_profile_read (include/ledds.h LEDDS_K_*)
-#define LEDDS_K_COUNT 9
+#define LEDDS_K_COUNT 8
 void ledds_count_launch(int n);
 void ledds_prof_start(int kernel_id, cudaStream_t st);
 void ledds_prof_stop(int kernel_id, cudaStream_t st);

@@ -12,8 +12,6 @@
 //   sol[n][10]          per solid, lattice units: x_k[3], R_k, v_k[3], w_k[3] (predictor values)
 //   flags[n][S^3]       uint8: box entry holds a partial of this step (set by lbm_psm_kernel, reset by
 //                       cpl_reduce_kernel)
-//   list2[1 + cap]      uint32: number and linear indices of the cells cut by two solids (written by the
-//                       raster kernel, worked through by lbm_psm2_kernel, count reset by cpl_reduce_kernel)
 //   box[n][S^3][6]      double: sum of the (cell, solid) terms of Eq. (41)-(42) over one run of
 //                       consecutive cells of a lattice row inside a warp, stored at the run's first cell;
 //                       S = 2H+2 cells per axis around floor(x_k)
@@ -28,8 +26,6 @@ struct CplDev {
     double* sol;
     uint8_t* flags;
     double* box;
-    uint32_t* list2;           // [0] = count, [1..] = linear indices of the cells cut by two solids
-    uint32_t list2_cap;
     int32_t* status;
 };
 
@@ -65,28 +61,63 @@ __device__ __forceinline__ bool cpl_cuts(double Rk, double rc, const double* d)
     return __dsub_rn(s, __dsqrt_rn(d2)) > 0.0;
 }
 
-// PSM collision of one cell cut by NS (1 or 2) solids, Eq. (32)-(37).  Written pair by pair (q, opposite q)
-// so that no per-direction array besides f itself is live.  A solid with B = 0 contributes nothing, so lanes
-// of a warp that are not cut run the same code with B = 0.
-template <int NS>
+// What one solid does to one cell: weight B (Eq. 36, 39-40), solid velocity at the cell (Eq. 35), the terms
+// of Eq. (41)-(42) in lattice units (rec) and the index of the cell in the solid's box (ent).
+// id = PSM_EMPTY: no solid here: B = 0, rec = 0, ent = -1 (the lane still runs the code of its warp).
+__device__ __forceinline__ void psm_solid_terms(const LbmDev& P, const CplDev& C, int x, int y, int z, uint32_t id,
+                                                double rho, double ux, double uy, double uz, double& B,
+                                                double (&uk)[3], double (&rec)[6], int& ent)
+{
+    const bool has = id != PSM_EMPTY;
+    const uint32_t k = has ? id : 0u;
+    const double2* sp = reinterpret_cast<const double2*>(C.sol + (size_t)k * 10);
+    const double2 a0 = __ldg(sp), a1 = __ldg(sp + 1), a2 = __ldg(sp + 2), a3 = __ldg(sp + 3), a4 = __ldg(sp + 4);
+    const double xk[3] = {a0.x, a0.y, a1.x}, Rk = a1.y;
+    const double vk[3] = {a2.x, a2.y, a3.x}, wk[3] = {a3.y, a4.x, a4.y};
+    const int fk[3] = {(int)floor(xk[0]), (int)floor(xk[1]), (int)floor(xk[2])};
+    const int di[3] = {cpl_offset(x, fk[0], P.nx, !P.bc[0]), cpl_offset(y, fk[1], P.ny, !P.bc[1]),
+                       cpl_offset(z, fk[2], P.nz, !P.bc[2])};
+    double d[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) d[a] = (double)(fk[a] + di[a]) - xk[a];              // r_j - r_k, nearest image
+    ent = has ? ((di[2] + C.H) * C.S + (di[1] + C.H)) * C.S + (di[0] + C.H) : -1;
+    const double dsc = cpl_dsc(Rk, C.rc, cpl_dist(d));
+    double beta = dsc * C.inv_2rc;                                                   // Eq. (39)-(40)
+    beta = beta > 1.0 ? 1.0 : beta;
+    beta = (has && beta > 0.0) ? beta : 0.0;
+    B = beta * (P.tau - 0.5) / ((1.0 - beta) + (P.tau - 0.5));                        // Eq. (36)
+    uk[0] = vk[0] + (wk[1] * d[2] - wk[2] * d[1]);                                   // Eq. (35)
+    uk[1] = vk[1] + (wk[2] * d[0] - wk[0] * d[2]);
+    uk[2] = vk[2] + (wk[0] * d[1] - wk[1] * d[0]);
+    // Eq. (41): -B_k sum_i Omega^s_{i,k} c_i.  The sum is rho (u_k - u) identically (sum_i c_i f_i = rho u,
+    // sum_i c_i f_i^eq(rho, v) = rho v, c_opp = -c), so it is formed from the moments (DESIGN.md section 7).
+    const double Br = B * rho;
+    const double dF[3] = {Br * (ux - uk[0]), Br * (uy - uk[1]), Br * (uz - uk[2])};  // lattice units
+    rec[0] = dF[0]; rec[1] = dF[1]; rec[2] = dF[2];
+    rec[3] = d[1] * dF[2] - d[2] * dF[1];                                            // Eq. (42)
+    rec[4] = d[2] * dF[0] - d[0] * dF[2];
+    rec[5] = d[0] * dF[1] - d[1] * dF[0];
+}
+
+// Second solid of a cell, parked in shared memory while the collision runs (one column per thread):
+// rows 0..4 = B, 1 - 1.5 u_k^2, u_k[3].
+#define PSM_S2_ROWS 5
+
+// PSM collision, Eq. (32)-(37), of a cell cut by the solid (B0, uk0) and, when the warp-uniform flag `two` is
+// set, by the second one parked in s2 (B = 0 there for the lanes that have none).  Written pair by pair
+// (q, opposite q) so that no per-direction array besides f itself is live.
 __device__ __forceinline__ void psm_collide(double (&f)[LEDDS_Q], double omega, double rho, double ux, double uy,
-                                            double uz, const double (&B)[NS], const double (&uk)[NS][3])
+                                            double uz, double B0, const double (&uk0)[3], bool two, const double* s2)
 {
     const double k0 = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
-    double kk[NS];
-    double Bsum = 0.0;
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        kk[s] = 1.0 - 1.5 * (uk[s][0] * uk[s][0] + uk[s][1] * uk[s][1] + uk[s][2] * uk[s][2]);
-        Bsum += B[s];
-    }
+    const double kk0 = 1.0 - 1.5 * (uk0[0] * uk0[0] + uk0[1] * uk0[1] + uk0[2] * uk0[2]);
+    const double Bsum = B0 + (two ? s2[0] : 0.0);
     const double keep = 1.0 - (Bsum < 1.0 ? Bsum : 1.0);                              // 1 - B_tot, Eq. (37)
     const double komega = keep * omega;
     {   // rest population: its own opposite, Omega^s = feq(rho,u_k) - feq(rho,u)
         const double wr = lb_w(0) * rho, fe = wr * k0;
-        double acc = 0.0;
-#pragma unroll
-        for (int s = 0; s < NS; ++s) acc += B[s] * (wr * kk[s] - fe);
+        double acc = B0 * (wr * kk0 - fe);
+        if (two) acc += s2[0] * (wr * s2[PSM_BLOCK] - fe);
         f[0] = f[0] + (acc - komega * (f[0] - fe));
     }
 #pragma unroll
@@ -95,63 +126,20 @@ __device__ __forceinline__ void psm_collide(double (&f)[LEDDS_Q], double omega, 
         const double cu = lb_cdot(q, ux, uy, uz);
         const double ev = wr * (k0 + 4.5 * cu * cu), od = wr * 3.0 * cu;
         const double nq = f[q] - (ev + od), no = f[q + 1] - (ev - od);                   // f - feq(rho,u), Eq. (28)
-        double acc_q = 0.0, acc_o = 0.0;
-#pragma unroll
-        for (int s = 0; s < NS; ++s) {
-            const double cuk = lb_cdot(q, uk[s][0], uk[s][1], uk[s][2]);
-            const double evk = wr * (kk[s] + 4.5 * cuk * cuk), odk = wr * 3.0 * cuk;
-            acc_q += B[s] * (no - (f[q] - (evk + odk)));                                // B Omega^s, Eq. (34), direction q
-            acc_o += B[s] * (nq - (f[q + 1] - (evk - odk)));                            //                      its opposite
+        const double cuk = lb_cdot(q, uk0[0], uk0[1], uk0[2]);
+        const double evk = wr * (kk0 + 4.5 * cuk * cuk), odk = wr * 3.0 * cuk;
+        double acc_q = B0 * (no - (f[q] - (evk + odk)));                                // B Omega^s, Eq. (34), direction q
+        double acc_o = B0 * (nq - (f[q + 1] - (evk - odk)));                            //                      its opposite
+        if (two) {
+            const double B1 = s2[0], kk1 = s2[PSM_BLOCK];
+            const double cu1 = lb_cdot(q, s2[2 * PSM_BLOCK], s2[3 * PSM_BLOCK], s2[4 * PSM_BLOCK]);
+            const double ev1 = wr * (kk1 + 4.5 * cu1 * cu1), od1 = wr * 3.0 * cu1;
+            acc_q += B1 * (no - (f[q] - (ev1 + od1)));
+            acc_o += B1 * (nq - (f[q + 1] - (ev1 - od1)));
         }
         f[q] = f[q] + (acc_q - komega * nq);                                            // Eq. (32)-(33)
         f[q + 1] = f[q + 1] + (acc_o - komega * no);
     }
-}
-
-// Collision of a cell of a warp in which some cell is cut by a solid.  id[s] = PSM_EMPTY: no solid s here
-// (B = 0).  Outputs per solid the terms of Eq. (41)-(42) in lattice units (rec) and the index of this cell
-// in the solid's box (ent, -1 when there is no solid s).
-template <int NS>
-__device__ __forceinline__ void psm_cell(const LbmDev& P, const CplDev& C, int x, int y, int z, double (&f)[LEDDS_Q],
-                                         double rho, double ux, double uy, double uz, const uint32_t (&id)[2],
-                                         double (&rec)[2][6], int (&ent)[2])
-{
-    double B[NS], uk[NS][3], d[NS][3];
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        const bool has = id[s] != PSM_EMPTY;
-        const uint32_t k = has ? id[s] : 0u;
-        const double2* sp = reinterpret_cast<const double2*>(C.sol + (size_t)k * 10);
-        const double2 a0 = __ldg(sp), a1 = __ldg(sp + 1), a2 = __ldg(sp + 2), a3 = __ldg(sp + 3), a4 = __ldg(sp + 4);
-        const double xk[3] = {a0.x, a0.y, a1.x}, Rk = a1.y;
-        const double vk[3] = {a2.x, a2.y, a3.x}, wk[3] = {a3.y, a4.x, a4.y};
-        const int fk[3] = {(int)floor(xk[0]), (int)floor(xk[1]), (int)floor(xk[2])};
-        const int di[3] = {cpl_offset(x, fk[0], P.nx, !P.bc[0]), cpl_offset(y, fk[1], P.ny, !P.bc[1]),
-                           cpl_offset(z, fk[2], P.nz, !P.bc[2])};
-#pragma unroll
-        for (int a = 0; a < 3; ++a) d[s][a] = (double)(fk[a] + di[a]) - xk[a];        // r_j - r_k, nearest image
-        ent[s] = has ? ((di[2] + C.H) * C.S + (di[1] + C.H)) * C.S + (di[0] + C.H) : -1;
-        const double dsc = cpl_dsc(Rk, C.rc, cpl_dist(d[s]));
-        double beta = dsc * C.inv_2rc;                                                // Eq. (39)-(40)
-        beta = beta > 1.0 ? 1.0 : beta;
-        beta = (has && beta > 0.0) ? beta : 0.0;
-        B[s] = beta * (P.tau - 0.5) / ((1.0 - beta) + (P.tau - 0.5));                 // Eq. (36)
-        uk[s][0] = vk[0] + (wk[1] * d[s][2] - wk[2] * d[s][1]);                       // Eq. (35)
-        uk[s][1] = vk[1] + (wk[2] * d[s][0] - wk[0] * d[s][2]);
-        uk[s][2] = vk[2] + (wk[0] * d[s][1] - wk[1] * d[s][0]);
-    }
-    // Eq. (41): -B_k sum_i Omega^s_{i,k} c_i.  The sum is rho (u_k - u) identically (sum_i c_i f_i = rho u,
-    // sum_i c_i f_i^eq(rho, v) = rho v, c_opp = -c), so it is formed from the moments (DESIGN.md section 7).
-#pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        const double Br = B[s] * rho;
-        const double dF[3] = {Br * (ux - uk[s][0]), Br * (uy - uk[s][1]), Br * (uz - uk[s][2])};   // lattice units
-        rec[s][0] = dF[0]; rec[s][1] = dF[1]; rec[s][2] = dF[2];
-        rec[s][3] = d[s][1] * dF[2] - d[s][2] * dF[1];                                // Eq. (42)
-        rec[s][4] = d[s][2] * dF[0] - d[s][0] * dF[2];
-        rec[s][5] = d[s][0] * dF[1] - d[s][1] * dF[0];
-    }
-    psm_collide<NS>(f, P.omega, rho, ux, uy, uz, B, uk);
 }
 
 // Sum the records of each run of consecutive lanes that hold the same solid id (a solid cuts a lattice row
