@@ -93,6 +93,7 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
 }
 
 // ------------------------------------------------------------------------------------ collide + stream
+template <typename I>
 __global__ void __launch_bounds__(PSM_BLOCK, 5) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                                const __grid_constant__ LbmDev P,
                                                                const __grid_constant__ CplDev C)
@@ -100,17 +101,13 @@ __global__ void __launch_bounds__(PSM_BLOCK, 5) lbm_psm_kernel(const double* __r
     __shared__ double s2[PSM_S2_ROWS][PSM_BLOCK];
     const int x = blockIdx.x * PSM_BLOCK + threadIdx.x, y = blockIdx.y, z = blockIdx.z;
     const bool active = x < P.nx;
-    const long long cell = ((long long)z * P.ny + y) * P.nx + (active ? x : 0);
-    uint32_t id0 = PSM_EMPTY, id1 = PSM_EMPTY;
+    const I cell = ((I)z * (I)P.ny + (I)y) * (I)P.nx + (I)(active ? x : 0);    // a lane past the row reads cell 0, stores nothing
     double f[LEDDS_Q];
+    lb_load<I>(fin, (I)P.N, cell, f);
+    uint32_t id0 = PSM_EMPTY, id1 = PSM_EMPTY;
     if (active) {
-#pragma unroll
-        for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (long long)q * P.N + cell);
         const uint2 slot = C.slots[cell];
         id0 = slot.x; id1 = slot.y;
-    } else {
-#pragma unroll
-        for (int q = 0; q < LEDDS_Q; ++q) f[q] = lb_w(q);
     }
     double rho, ux, uy, uz;
     lb_moments(f, rho, ux, uy, uz);
@@ -135,7 +132,7 @@ __global__ void __launch_bounds__(PSM_BLOCK, 5) lbm_psm_kernel(const double* __r
         psm_run_reduce(C, id0, ent, rec);
         psm_collide(f, P.omega, rho, ux, uy, uz, B0, uk0, two, mine);
     }
-    if (active) lb_push_store(fout, P, x, y, z, f, rho);
+    if (active) lb_push_store<I>(fout, P, x, y, z, f, rho);
 }
 
 // ------------------------------------------------------------------------------------ reduce
@@ -302,7 +299,8 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         LEDDS_CHECK_LAUNCH();
         dim3 block(PSM_BLOCK), grid((d.nx + PSM_BLOCK - 1) / PSM_BLOCK, d.ny, d.nz);
         ledds_prof_start(LEDDS_K_LBM, st);
-        lbm_psm_kernel<<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
+        if (lb_fits_u32(d.N)) lbm_psm_kernel<unsigned><<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
+        else lbm_psm_kernel<long long><<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
         ledds_prof_stop(LEDDS_K_LBM, st);
         LEDDS_CHECK_LAUNCH();
         lbm->parity ^= 1;

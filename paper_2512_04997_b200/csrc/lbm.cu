@@ -45,20 +45,20 @@ __global__ void lbm_export_kernel(const double* __restrict__ f, double* __restri
 }
 
 // ------------------------------------------------------------------------------------ variant 1
+template <typename I>
 __global__ void __launch_bounds__(128) lbm_push_kernel(const double* __restrict__ fin, double* __restrict__ fout,
-                                                       const LbmDev P)
+                                                       const __grid_constant__ LbmDev P)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y, z = blockIdx.z;
     if (x >= P.nx) return;
-    const long long cell = ((long long)z * P.ny + y) * P.nx + x;
+    const I cell = ((I)z * (I)P.ny + (I)y) * (I)P.nx + (I)x;
     double f[LEDDS_Q];
-#pragma unroll
-    for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (long long)q * P.N + cell);
+    lb_load<I>(fin, (I)P.N, cell, f);
     double rho, ux, uy, uz;
     lb_moments(f, rho, ux, uy, uz);
     lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
-    lb_push_store(fout, P, x, y, z, f, rho);
+    lb_push_store<I>(fout, P, x, y, z, f, rho);
 }
 
 // ------------------------------------------------------------------------------------ variant 2
@@ -254,7 +254,8 @@ static int lbm_launch(const ledds_lbm* h, const double* src, double* dst, cudaSt
         lbm_rowrot_kernel<<<grid, block, 0, st>>>(src, dst, d);
     } else {
         dim3 block(128), grid((d.nx + 127) / 128, d.ny, d.nz);
-        lbm_push_kernel<<<grid, block, 0, st>>>(src, dst, d);
+        if (lb_fits_u32(d.N)) lbm_push_kernel<unsigned><<<grid, block, 0, st>>>(src, dst, d);
+        else lbm_push_kernel<long long><<<grid, block, 0, st>>>(src, dst, d);
     }
     ledds_prof_stop(LEDDS_K_LBM, st);
     LEDDS_CHECK_LAUNCH();

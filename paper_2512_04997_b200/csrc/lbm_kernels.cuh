@@ -73,22 +73,40 @@ __device__ __forceinline__ int lb_axis_target(const LbmDev& P, int q, int c, int
     return t;
 }
 
+// Index type of the population arrays: unsigned 32-bit when 19 N < 2^32 (one IMAD.WIDE per access), else 64-bit.
+static inline bool lb_fits_u32(long long N) { return (unsigned long long)N * LEDDS_Q < 0xffffffffull; }
+
+// The 19 pre-collision populations of cell `cell`.
+template <typename I>
+__device__ __forceinline__ void lb_load(const double* __restrict__ fin, I N, I cell, double (&f)[LEDDS_Q])
+{
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (I)((I)q * N + cell));
+}
+
 // Eq. (25) as a push of all 19 post-collision populations of cell (x,y,z), with boundaries.
-// The neighbour coordinates and "this link leaves through a wall" flags are worked out once per axis
-// (y and z are uniform over the block), so a direction costs a predicate, an address and a store.
+// The neighbour coordinates and "this link leaves through a wall" flags are worked out once per axis and
+// the nine row offsets once per block (y and z are uniform over the block), so a direction costs a
+// predicate, an index and a store.
+template <typename I>
 __device__ __forceinline__ void lb_push_store(double* __restrict__ fout, const LbmDev& P, int x, int y, int z,
                                               const double (&fs)[LEDDS_Q], double rho)
 {
-    // t[a][0] / t[a][1]: target coordinate for c = -1 / +1; w[a][0] / w[a][1]: link crosses the low / high wall
-    int tx[2] = {x - 1, x + 1}, ty[2] = {y - 1, y + 1}, tz[2] = {z - 1, z + 1};
+    // t?[0] / t?[2]: target coordinate for c = -1 / +1; w?[0] / w?[1]: link crosses the low / high wall
+    int tx[3] = {x - 1, x, x + 1}, ty[3] = {y - 1, y, y + 1}, tz[3] = {z - 1, z, z + 1};
     bool wx[2] = {false, false}, wy[2] = {false, false}, wz[2] = {false, false};
     if (x == 0) { if (P.bc[0]) wx[0] = true; else tx[0] = P.nx - 1; }
-    if (x == P.nx - 1) { if (P.bc[0]) wx[1] = true; else tx[1] = 0; }
+    if (x == P.nx - 1) { if (P.bc[0]) wx[1] = true; else tx[2] = 0; }
     if (y == 0) { if (P.bc[1]) wy[0] = true; else ty[0] = P.ny - 1; }
-    if (y == P.ny - 1) { if (P.bc[1]) wy[1] = true; else ty[1] = 0; }
+    if (y == P.ny - 1) { if (P.bc[1]) wy[1] = true; else ty[2] = 0; }
     if (z == 0) { if (P.bc[2]) wz[0] = true; else tz[0] = P.nz - 1; }
-    if (z == P.nz - 1) { if (P.bc[2]) wz[1] = true; else tz[1] = 0; }
-    const long long cell = ((long long)z * P.ny + y) * P.nx + x;
+    if (z == P.nz - 1) { if (P.bc[2]) wz[1] = true; else tz[2] = 0; }
+    const I N = (I)P.N;
+    I rb[3][3];                                                   // row offsets [cz + 1][cy + 1]
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) rb[a][b] = ((I)tz[a] * (I)P.ny + (I)ty[b]) * (I)P.nx;
 #pragma unroll
     for (int q = 0; q < LEDDS_Q; ++q) {
         const int cx = lb_cx(q), cy = lb_cy(q), cz = lb_cz(q);
@@ -97,8 +115,7 @@ __device__ __forceinline__ void lb_push_store(double* __restrict__ fout, const L
         if (cy != 0) bounced = bounced || wy[cy > 0];
         if (cz != 0) bounced = bounced || wz[cz > 0];
         if (!bounced) {
-            const int ax = cx == 0 ? x : tx[cx > 0], ay = cy == 0 ? y : ty[cy > 0], az = cz == 0 ? z : tz[cz > 0];
-            fout[(long long)q * P.N + ((long long)az * P.ny + ay) * P.nx + ax] = fs[q];
+            fout[(I)((I)q * N + rb[cz + 1][cy + 1] + (I)tx[cx + 1])] = fs[q];
         } else {
             double cuw = 0.0;                                   // c_q . u_wall summed over the crossed walls (G19)
             if (P.any_wall_velocity) {
@@ -106,7 +123,7 @@ __device__ __forceinline__ void lb_push_store(double* __restrict__ fout, const L
                 if (cy != 0 && wy[cy > 0]) { const double* uw = P.uw + (2 + (cy > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
                 if (cz != 0 && wz[cz > 0]) { const double* uw = P.uw + (4 + (cz > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
             }
-            fout[(long long)lb_opp(q) * P.N + cell] = fs[q] - 6.0 * lb_w(q) * rho * cuw;
+            fout[(I)((I)lb_opp(q) * N + rb[1][1] + (I)x)] = fs[q] - 6.0 * lb_w(q) * rho * cuw;
         }
     }
 }
