@@ -20,12 +20,12 @@
 // ------------------------------------------------------------------------------------ raster
 #define PSM_EMPTY64 0xffffffffffffffffull
 
-// Enter solid k in a slot {x = low word, y = high word, x <= y}: keep the two lowest ids; a third one raises
-// the overflow flag.
-__device__ __forceinline__ void raster_insert(unsigned long long* slot, uint32_t k, bool& overflow)
+// Enter solid k in a slot {x = low word, y = high word, x <= y} that was seen to hold `old` (not free): keep
+// the two lowest ids; a third one raises the overflow flag.
+#define RASTER_BATCH 6
+__device__ __forceinline__ void raster_insert(unsigned long long* slot, unsigned long long old, uint32_t k, bool& overflow)
 {
-    unsigned long long old = atomicCAS(slot, PSM_EMPTY64, ((unsigned long long)PSM_EMPTY << 32) | k);   // usual case: free
-    while (old != PSM_EMPTY64) {
+    for (;;) {
         const uint32_t a = (uint32_t)old, b = (uint32_t)(old >> 32);
         if (k > b) { overflow = true; return; }                                 // two lower ids are already there
         const uint32_t na = k < a ? k : a, nb = k < a ? a : k;
@@ -82,19 +82,65 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
     while (xa > lo && cuts(xa - 1)) --xa;
     while (xb < hi && cuts(xb + 1)) ++xb;
     bool overflow = false;
-    const long long row = ((long long)rz * P.ny + ry) * P.nx;
-    for (int xi = xa; xi <= xb; ++xi) {
-        int rx = xi;
-        if (P.bc[0]) { if (rx < 0 || rx >= P.nx) continue; }
-        else rx = rx < 0 ? rx + P.nx : (rx >= P.nx ? rx - P.nx : rx);
-        raster_insert(reinterpret_cast<unsigned long long*>(C.slots + row + rx), (uint32_t)k, overflow);
+    unsigned long long* const row = reinterpret_cast<unsigned long long*>(C.slots + ((long long)rz * P.ny + ry) * P.nx);
+    const unsigned long long mine = ((unsigned long long)PSM_EMPTY << 32) | (uint32_t)k;
+    // RASTER_BATCH optimistic swaps (a free slot is the usual case) are in flight before the first answer is
+    // looked at, so the run is not a chain of memory round trips
+    for (int x0 = xa; x0 <= xb; x0 += RASTER_BATCH) {
+        unsigned long long* slot[RASTER_BATCH];
+        unsigned long long seen[RASTER_BATCH];
+#pragma unroll
+        for (int b = 0; b < RASTER_BATCH; ++b) {
+            int rx = x0 + b;
+            bool ok = rx <= xb;
+            if (P.bc[0]) ok = ok && rx >= 0 && rx < P.nx;
+            else rx = rx < 0 ? rx + P.nx : (rx >= P.nx ? rx - P.nx : rx);
+            slot[b] = ok ? row + rx : nullptr;
+            seen[b] = ok ? atomicCAS(row + rx, PSM_EMPTY64, mine) : PSM_EMPTY64;
+        }
+#pragma unroll
+        for (int b = 0; b < RASTER_BATCH; ++b)
+            if (seen[b] != PSM_EMPTY64) raster_insert(slot[b], seen[b], (uint32_t)k, overflow);
     }
     if (overflow) atomicOr(C.status, LEDDS_ST_SOLID_OVERFLOW);
 }
 
 // ------------------------------------------------------------------------------------ collide + stream
+// One cell: f = its 19 pre-collision populations, (id0, id1) = its slot.  Collides (BGK or PSM), streams, and
+// takes part in the warp's run reductions.  All 32 lanes of a warp call this together.
 template <typename I>
-__global__ void __launch_bounds__(PSM_BLOCK, 5) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
+__device__ __forceinline__ void psm_cell_step(double (&f)[LEDDS_Q], uint32_t id0, uint32_t id1, bool active, I cell, int x,
+                                              int y, int z, double* __restrict__ fout, const LbmDev& P, const CplDev& C,
+                                              double* s2col)
+{
+    double rho, ux, uy, uz;
+    lb_moments(f, rho, ux, uy, uz);
+    if (!__any_sync(0xffffffffu, id0 != PSM_EMPTY)) {
+        lb_collide_bgk(f, P.omega, rho, ux, uy, uz);                                  // PAPER.md:297
+    } else {
+        if (id0 != PSM_EMPTY) C.slots[cell] = make_uint2(PSM_EMPTY, PSM_EMPTY);       // consumed: free for the next step
+        const bool two = __any_sync(0xffffffffu, id1 != PSM_EMPTY);
+        if (two) {                                                                    // warp-uniform, rarer
+            double B1, uk1[3], rec[6];
+            int ent;
+            psm_solid_terms(P, C, x, y, z, id1, rho, ux, uy, uz, B1, uk1, rec, ent);
+            s2col[0] = B1;
+            s2col[PSM_BLOCK] = 1.0 - 1.5 * (uk1[0] * uk1[0] + uk1[1] * uk1[1] + uk1[2] * uk1[2]);
+            s2col[2 * PSM_BLOCK] = uk1[0]; s2col[3 * PSM_BLOCK] = uk1[1]; s2col[4 * PSM_BLOCK] = uk1[2];
+            psm_run_reduce(C, id1, ent, rec);
+        }
+        double B0, uk0[3], rec[6];
+        int ent;
+        psm_solid_terms(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
+        psm_run_reduce(C, id0, ent, rec);
+        psm_collide(f, P.omega, rho, ux, uy, uz, B0, uk0, two, s2col);
+    }
+    if (active) lb_push_store<I>(fout, P, x, y, z, f, rho);
+}
+
+// One block per 128-cell row segment, populations loaded straight into registers.
+template <typename I>
+__global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                                const __grid_constant__ LbmDev P,
                                                                const __grid_constant__ CplDev C)
 {
@@ -109,30 +155,7 @@ __global__ void __launch_bounds__(PSM_BLOCK, 5) lbm_psm_kernel(const double* __r
         const uint2 slot = C.slots[cell];
         id0 = slot.x; id1 = slot.y;
     }
-    double rho, ux, uy, uz;
-    lb_moments(f, rho, ux, uy, uz);
-    if (!__any_sync(0xffffffffu, id0 != PSM_EMPTY)) {
-        lb_collide_bgk(f, P.omega, rho, ux, uy, uz);                                  // PAPER.md:297
-    } else {
-        if (id0 != PSM_EMPTY) C.slots[cell] = make_uint2(PSM_EMPTY, PSM_EMPTY);       // consumed: free for the next step
-        const bool two = __any_sync(0xffffffffu, id1 != PSM_EMPTY);
-        double* mine = &s2[0][threadIdx.x];
-        if (two) {                                                                    // warp-uniform, rarer
-            double B1, uk1[3], rec[6];
-            int ent;
-            psm_solid_terms(P, C, x, y, z, id1, rho, ux, uy, uz, B1, uk1, rec, ent);
-            mine[0] = B1;
-            mine[PSM_BLOCK] = 1.0 - 1.5 * (uk1[0] * uk1[0] + uk1[1] * uk1[1] + uk1[2] * uk1[2]);
-            mine[2 * PSM_BLOCK] = uk1[0]; mine[3 * PSM_BLOCK] = uk1[1]; mine[4 * PSM_BLOCK] = uk1[2];
-            psm_run_reduce(C, id1, ent, rec);
-        }
-        double B0, uk0[3], rec[6];
-        int ent;
-        psm_solid_terms(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
-        psm_run_reduce(C, id0, ent, rec);
-        psm_collide(f, P.omega, rho, ux, uy, uz, B0, uk0, two, mine);
-    }
-    if (active) lb_push_store<I>(fout, P, x, y, z, f, rho);
+    psm_cell_step<I>(f, id0, id1, active, cell, x, y, z, fout, P, C, &s2[0][threadIdx.x]);
 }
 
 // ------------------------------------------------------------------------------------ reduce

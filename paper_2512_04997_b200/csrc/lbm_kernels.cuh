@@ -2,16 +2,21 @@
 #pragma once
 #include "common.cuh"
 
-// Eq. (22a), (22b): density and velocity of one cell.
+// Eq. (22a), (22b): density and velocity of one cell.  Opposite directions are paired (q, q+1), so the sums
+// are short trees rather than 19-long dependent chains.
 __device__ __forceinline__ void lb_moments(const double (&f)[LEDDS_Q], double& rho, double& ux, double& uy, double& uz)
 {
-    double r = 0.0, jx = 0.0, jy = 0.0, jz = 0.0;
+    double s[9], d[9];
 #pragma unroll
-    for (int q = 0; q < LEDDS_Q; ++q) {
-        r += f[q];
-        if (lb_cx(q) == 1) jx += f[q]; else if (lb_cx(q) == -1) jx -= f[q];
-        if (lb_cy(q) == 1) jy += f[q]; else if (lb_cy(q) == -1) jy -= f[q];
-        if (lb_cz(q) == 1) jz += f[q]; else if (lb_cz(q) == -1) jz -= f[q];
+    for (int p = 0; p < 9; ++p) { s[p] = f[2 * p + 1] + f[2 * p + 2]; d[p] = f[2 * p + 1] - f[2 * p + 2]; }
+    const double r = (f[0] + s[0]) + ((s[1] + s[2]) + (s[3] + s[4])) + ((s[5] + s[6]) + (s[7] + s[8]));
+    double jx = 0.0, jy = 0.0, jz = 0.0;
+#pragma unroll
+    for (int p = 0; p < 9; ++p) {                         // d[p] = f_q - f_opp(q) carries c_q
+        const int q = 2 * p + 1;
+        if (lb_cx(q) == 1) jx += d[p]; else if (lb_cx(q) == -1) jx -= d[p];
+        if (lb_cy(q) == 1) jy += d[p]; else if (lb_cy(q) == -1) jy -= d[p];
+        if (lb_cz(q) == 1) jz += d[p]; else if (lb_cz(q) == -1) jz -= d[p];
     }
     const double inv = 1.0 / r;
     rho = r; ux = jx * inv; uy = jy * inv; uz = jz * inv;

@@ -3,6 +3,9 @@
 #include "lbm_kernels.cuh"
 
 #define PSM_BLOCK 128
+#ifndef PSM_MIN_BLOCKS
+#define PSM_MIN_BLOCKS 5      // resident blocks per SM the collide kernel is compiled for (<= 102 registers)
+#endif
 #define PSM_EMPTY 0xffffffffu
 
 // Layout of the caller-owned coupling scratch (ledds_cpl_workspace_bytes):
@@ -152,9 +155,11 @@ __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int
     const uint32_t prev = __shfl_up_sync(full, id, 1);
     const unsigned starts = __ballot_sync(full, lane == 0 || prev != id);          // bit l: lane l begins a run
     const unsigned above = lane == 31 ? 0u : (starts >> (lane + 1));
-    const int len = above ? __ffs(above) : 32 - lane;                               // lanes from here to the end of my run
+    const int len = id == PSM_EMPTY ? 1 : (above ? __ffs(above) : 32 - lane);       // lanes from here to the end of my run
+    const int maxlen = __reduce_max_sync(full, len);                                // runs are ~2 (R + r_c) cells long
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
+        if (o >= maxlen) break;
 #pragma unroll
         for (int c = 0; c < 6; ++c) {
             const double t = __shfl_down_sync(full, v[c], o);
