@@ -20,20 +20,7 @@
 // ------------------------------------------------------------------------------------ raster
 #define PSM_EMPTY64 0xffffffffffffffffull
 
-// Enter solid k in a slot {x = low word, y = high word, x <= y} that was seen to hold `old` (not free): keep
-// the two lowest ids; a third one raises the overflow flag.
 #define RASTER_BATCH 6
-__device__ __forceinline__ void raster_insert(unsigned long long* slot, unsigned long long old, uint32_t k, bool& overflow)
-{
-    for (;;) {
-        const uint32_t a = (uint32_t)old, b = (uint32_t)(old >> 32);
-        if (k > b) { overflow = true; return; }                                 // two lower ids are already there
-        const uint32_t na = k < a ? k : a, nb = k < a ? a : k;
-        const unsigned long long seen = atomicCAS(slot, old, ((unsigned long long)nb << 32) | na);
-        if (seen == old) { if (b != PSM_EMPTY) overflow = true; return; }       // b was pushed out
-        old = seen;
-    }
-}
 
 // sol[k] = the solid in lattice units (one thread per solid)
 __global__ void cpl_solid_kernel(const CplDev C)
@@ -50,7 +37,12 @@ __global__ void cpl_solid_kernel(const CplDev C)
     o[3] = C.radius[k] * C.inv_dx;
 }
 
-// thread t -> solid k = t / S^2, row (ly, lz) = t % S^2 of its box
+// thread t -> solid k = t / S^2, row (ly, lz) = t % S^2 of its box.
+// ROUND 0: slots[cell].x = min id over the solids cutting the cell (reductions without a return value: nothing
+//          waits on them).
+// ROUND 1: a solid that did not win a cell enters slots[cell].y the same way; the value found there tells a
+//          third solid apart (LEDDS_ST_SOLID_OVERFLOW).  Together: the two lowest ids.
+template <int ROUND>
 __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const CplDev C)
 {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -82,25 +74,28 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
     while (xa > lo && cuts(xa - 1)) --xa;
     while (xb < hi && cuts(xb + 1)) ++xb;
     bool overflow = false;
-    unsigned long long* const row = reinterpret_cast<unsigned long long*>(C.slots + ((long long)rz * P.ny + ry) * P.nx);
-    const unsigned long long mine = ((unsigned long long)PSM_EMPTY << 32) | (uint32_t)k;
-    // RASTER_BATCH optimistic swaps (a free slot is the usual case) are in flight before the first answer is
-    // looked at, so the run is not a chain of memory round trips
+    uint2* const row = C.slots + ((long long)rz * P.ny + ry) * P.nx;
     for (int x0 = xa; x0 <= xb; x0 += RASTER_BATCH) {
-        unsigned long long* slot[RASTER_BATCH];
-        unsigned long long seen[RASTER_BATCH];
+        uint32_t first[RASTER_BATCH];
+        int rxs[RASTER_BATCH];
 #pragma unroll
-        for (int b = 0; b < RASTER_BATCH; ++b) {
+        for (int b = 0; b < RASTER_BATCH; ++b) {                                   // independent accesses, issued together
             int rx = x0 + b;
             bool ok = rx <= xb;
             if (P.bc[0]) ok = ok && rx >= 0 && rx < P.nx;
             else rx = rx < 0 ? rx + P.nx : (rx >= P.nx ? rx - P.nx : rx);
-            slot[b] = ok ? row + rx : nullptr;
-            seen[b] = ok ? atomicCAS(row + rx, PSM_EMPTY64, mine) : PSM_EMPTY64;
+            rxs[b] = ok ? rx : -1;
+            first[b] = (uint32_t)k;
+            if (ok) {
+                if (ROUND == 0) atomicMin(&row[rx].x, (uint32_t)k);
+                else first[b] = __ldcg(&row[rx].x);
+            }
         }
+        if (ROUND == 1) {
 #pragma unroll
-        for (int b = 0; b < RASTER_BATCH; ++b)
-            if (seen[b] != PSM_EMPTY64) raster_insert(slot[b], seen[b], (uint32_t)k, overflow);
+            for (int b = 0; b < RASTER_BATCH; ++b)
+                if (first[b] != (uint32_t)k && atomicMin(&row[rxs[b]].y, (uint32_t)k) != PSM_EMPTY) overflow = true;
+        }
     }
     if (overflow) atomicOr(C.status, LEDDS_ST_SOLID_OVERFLOW);
 }
@@ -160,33 +155,36 @@ __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(cons
 
 // ------------------------------------------------------------------------------------ reduce
 // One warp per solid; lane -> entry map and the shuffle tree are fixed, so the sums are deterministic.
-// Each lane takes 16 flags at a time (one 16-byte load) and reads the flagged partials.
+// A lane takes one word of 32 flags at a time and reads the flagged partials, four at a time.
 __global__ void __launch_bounds__(128) cpl_reduce_kernel(const CplDev C, double* __restrict__ f_hyd,
                                                          double* __restrict__ m_hyd)
 {
     const int k = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
     const int lane = threadIdx.x & 31;
     if (k >= C.n) return;
-    const int S3 = C.S * C.S * C.S;                                                  // multiple of 8
-    uint2* fl = reinterpret_cast<uint2*>(C.flags + (size_t)k * S3);
-    const double2* box = reinterpret_cast<const double2*>(C.box + (size_t)k * S3 * 6);
+    uint32_t* fl = C.flags + (size_t)k * C.W;
+    const double2* box = reinterpret_cast<const double2*>(C.box + (size_t)k * (size_t)(C.S * C.S * C.S) * 8);
     double acc[6] = {0, 0, 0, 0, 0, 0};
     const double2 zero = make_double2(0.0, 0.0);
-    for (int w8 = lane; w8 < S3 / 8; w8 += 32) {
-        const uint2 m = fl[w8];
-        if (!(m.x | m.y)) continue;
-        fl[w8] = make_uint2(0u, 0u);
-        double2 a[8][3];
+    for (int w = lane; w < C.W; w += 32) {
+        uint32_t m = fl[w];
+        if (!m) continue;
+        fl[w] = 0u;
+        while (m) {
+            double2 a[4][3];
 #pragma unroll
-        for (int b = 0; b < 8; ++b) {
-            const bool on = (((b < 4 ? m.x : m.y) >> (8 * (b & 3))) & 0xffu) != 0u;
-            const double2* in = box + (size_t)(8 * w8 + b) * 3;
-            a[b][0] = on ? in[0] : zero; a[b][1] = on ? in[1] : zero; a[b][2] = on ? in[2] : zero;
-        }
+            for (int b = 0; b < 4; ++b) {                                         // ascending bit order: fixed
+                const bool on = m != 0u;
+                const int bit = on ? __ffs(m) - 1 : 0;
+                m &= m - 1u;
+                const double2* in = box + (size_t)(32 * w + bit) * 4;
+                a[b][0] = on ? in[0] : zero; a[b][1] = on ? in[1] : zero; a[b][2] = on ? in[2] : zero;
+            }
 #pragma unroll
-        for (int b = 0; b < 8; ++b) {
-            acc[0] += a[b][0].x; acc[1] += a[b][0].y; acc[2] += a[b][1].x;
-            acc[3] += a[b][1].y; acc[4] += a[b][2].x; acc[5] += a[b][2].y;
+            for (int b = 0; b < 4; ++b) {
+                acc[0] += a[b][0].x; acc[1] += a[b][0].y; acc[2] += a[b][1].x;
+                acc[3] += a[b][1].y; acc[4] += a[b][2].x; acc[5] += a[b][2].y;
+            }
         }
     }
 #pragma unroll
@@ -238,8 +236,9 @@ static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl
     L->slots = 0;
     L->sol = cpl_align(N * sizeof(uint2));
     L->flags = L->sol + cpl_align((size_t)C->n * 10 * sizeof(double));
-    L->box = L->flags + cpl_align(E);
-    L->total = L->box + cpl_align(E * 6 * sizeof(double));
+    C->W = (int)((S3 + 31) / 32);
+    L->box = L->flags + cpl_align((size_t)C->n * C->W * sizeof(uint32_t));
+    L->total = L->box + cpl_align(E * 8 * sizeof(double));
     return LEDDS_OK;
 }
 
@@ -297,7 +296,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
     C.radius = radius;
     C.slots = reinterpret_cast<uint2*>(cs + L.slots);
     C.sol = reinterpret_cast<double*>(cs + L.sol);
-    C.flags = reinterpret_cast<uint8_t*>(cs + L.flags);
+    C.flags = reinterpret_cast<uint32_t*>(cs + L.flags);
     C.box = reinterpret_cast<double*>(cs + L.box);
     C.status = status;
     const LbmDev& d = lbm->d;
@@ -317,7 +316,9 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         ledds_prof_start(LEDDS_K_CPL_RASTER, st);
         cpl_solid_kernel<<<(C.n + 127) / 128, 128, 0, st>>>(C);
         ledds_count_launch(1);
-        cpl_raster_kernel<<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
+        cpl_raster_kernel<0><<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
+        cpl_raster_kernel<1><<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
+        ledds_count_launch(1);
         ledds_prof_stop(LEDDS_K_CPL_RASTER, st);
         LEDDS_CHECK_LAUNCH();
         dim3 block(PSM_BLOCK), grid((d.nx + PSM_BLOCK - 1) / PSM_BLOCK, d.ny, d.nz);

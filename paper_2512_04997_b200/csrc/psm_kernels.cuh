@@ -13,9 +13,9 @@
 //                       when free.  Written by cpl_raster_kernel, consumed and reset by lbm_psm_kernel,
 //                       so it is all-empty between steps.
 //   sol[n][10]          per solid, lattice units: x_k[3], R_k, v_k[3], w_k[3] (predictor values)
-//   flags[n][S^3]       uint8: box entry holds a partial of this step (set by lbm_psm_kernel, reset by
-//                       cpl_reduce_kernel)
-//   box[n][S^3][6]      double: sum of the (cell, solid) terms of Eq. (41)-(42) over one run of
+//   flags[n][W]         uint32 bit sets, W = ceil(S^3 / 32): box entry holds a partial of this step (bit set
+//                       by lbm_psm_kernel with a reduction, word reset by cpl_reduce_kernel)
+//   box[n][S^3][8]      double (6 used; 64-byte entries = one DRAM access each): sum of the (cell, solid) terms of Eq. (41)-(42) over one run of
 //                       consecutive cells of a lattice row inside a warp, stored at the run's first cell;
 //                       S = 2H+2 cells per axis around floor(x_k)
 struct CplDev {
@@ -23,11 +23,11 @@ struct CplDev {
     double rc, inv_2rc;        // Eq. (40) in lattice units
     double inv_dx, vscale, wscale, origin[3];
     double fscale, mscale;     // lattice -> DEM units for force / torque
-    int H, S;                  // box half-width, box width
+    int H, S, W;               // box half-width, box width, flag words per solid
     const double* x; const double* vp; const double* wp; const double* radius;   // particle order, DEM units
     uint2* slots;
     double* sol;
-    uint8_t* flags;
+    uint32_t* flags;
     double* box;
     int32_t* status;
 };
@@ -168,10 +168,10 @@ __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int
     }
     if (id != PSM_EMPTY && ((starts >> lane) & 1u)) {
         const size_t e = (size_t)id * (size_t)(C.S * C.S * C.S) + (size_t)ent;
-        double2* out = reinterpret_cast<double2*>(C.box + e * 6);
+        double2* out = reinterpret_cast<double2*>(C.box + e * 8);
         out[0] = make_double2(v[0], v[1]);
         out[1] = make_double2(v[2], v[3]);
         out[2] = make_double2(v[4], v[5]);
-        C.flags[e] = 1;
+        atomicOr(C.flags + (size_t)id * C.W + (ent >> 5), 1u << (ent & 31));
     }
 }
