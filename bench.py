@@ -77,10 +77,31 @@ def make_cfg4(small=False):
     return W.cfg4_shear()
 
 
-def coupled_bytes_per_step(n_cells, n_part, solid_cells):
-    """Algorithmic HBM bytes of the dominant (PSM stream-collide) kernel per launch, DESIGN.md section 6:
-    304 B per cell + 48 B written per (cell, solid) partial."""
-    return 304.0 * n_cells + 48.0 * solid_cells
+# ncu --set full capture of one lbm_psm_kernel launch at configs[3] (profiles/r1_ncu_summary.md):
+# dram__bytes_read.sum + dram__bytes_write.sum
+PSM_KERNEL_DRAM_BYTES = 5.48e9
+
+
+def coupled_bytes_per_step(n_cells):
+    """Algorithmic HBM bytes of the dominant (PSM stream-collide) kernel per launch, DESIGN.md section 7:
+    19 populations read + 19 written (304 B) + the 8-byte solid slot read, per cell."""
+    return 312.0 * n_cells
+
+
+def max_over_ranks(ms, world, device="cuda"):
+    """Elapsed time of the slowest rank (replicas run independently; the job is as slow as the slowest)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_mlups(n_cells, ms_step, world):
+    """Cells updated per second by all replicas together, in 1e6."""
+    return world * n_cells / ms_step / 1e3
 
 
 def run_ours(args, rank, world):
@@ -108,10 +129,7 @@ def run_ours(args, rank, world):
         barrier()
         e0.record(); fn(k); e1.record()
         barrier()
-        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item())
+        return max_over_ranks(e0.elapsed_time(e1), world)
 
     out = {}
     # ------------------------------------------------------------------ main: coupled step, configs[3]
@@ -133,12 +151,10 @@ def run_ours(args, rank, world):
     clocks = sampler.stop() if sampler else None
     status = int(g_dem.status[0].item())
     ms_step = ms / K
-    mlups = world * n_cells / ms_step / 1e3
-    # number of (cell, solid) partials: cells within R + R_c of a sphere centre ~ 4/3 pi (R+Rc)^3 per sphere
-    solid_cells = n_part * 4.0 / 3.0 * np.pi * (float(R.max()) / cpl["dx"] + 0.62035) ** 3
+    mlups = whole_job_mlups(n_cells, ms_step, world)
     k_ms, k_n = prof["lbm"]
     k_ms_avg = k_ms / max(k_n, 1)
-    bytes_launch = coupled_bytes_per_step(n_cells, n_part, solid_cells)
+    bytes_launch = coupled_bytes_per_step(n_cells)
     achieved = bytes_launch / (k_ms_avg * 1e-3) / 1e9 if k_ms_avg > 0 else 0.0
     out.update({
         "metric": METRIC, "value": round(mlups, 1), "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": Wm,
@@ -302,11 +318,7 @@ def main():
             print(json.dumps(line), flush=True)
         return
     if args.traffic is None:
-        # last ncu --set full capture of the dominant kernel, if one is committed (profiles/)
-        try:
-            args.traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))["lbm_psm_kernel"]["dram_bytes_per_launch"]
-        except Exception:
-            args.traffic = None
+        args.traffic = PSM_KERNEL_DRAM_BYTES if args.workload == "cfg4" else None
     out = run_ours(args, rank, world)
     if rank == 0:
         if world == 1 and not args.no_cpu:
