@@ -82,7 +82,7 @@ struct DemScratch {
     size_t tile_state;             // look-back descriptors (uint32 [tiles][256])
     size_t tile_counter;           // dynamic tile ticket (uint32 [4])
     size_t cell_start, cell_end;   // uint32 [ncell]
-    size_t xs, vps, wps, rs;       // sorted copies: double [n][3] x3, double [n]
+    size_t xr, xr_s;               // (x, y, z, R) per particle, 32 B: particle order / sorted order
     size_t vp, wp;                 // predictor velocities in particle order: double [n][3]
     size_t force, torque;          // contact force / torque per particle: double [n][3]
     size_t pair_count, pair_off;   // query scratch (uint32 [n+1])

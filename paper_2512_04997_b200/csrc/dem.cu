@@ -42,9 +42,9 @@ __device__ __forceinline__ int dem_cell_coord(const DemDev& P, double x, int a)
 
 __global__ void dem_drift_key_kernel(const DemDev P, double* __restrict__ x, const double* __restrict__ v,
                                      const double* __restrict__ w, const double* __restrict__ a,
-                                     const double* __restrict__ alpha, double* __restrict__ vp,
-                                     double* __restrict__ wp, uint32_t* __restrict__ key, uint32_t* __restrict__ idx,
-                                     int drift)
+                                     const double* __restrict__ alpha, const double* __restrict__ radius,
+                                     double* __restrict__ vp, double* __restrict__ wp, double4* __restrict__ xr,
+                                     uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
@@ -73,6 +73,7 @@ __global__ void dem_drift_key_kernel(const DemDev P, double* __restrict__ x, con
     const int cx = dem_cell_coord(P, xn[0], 0), cy = dem_cell_coord(P, xn[1], 1), cz = dem_cell_coord(P, xn[2], 2);
     key[i] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
     idx[i] = (uint32_t)i;
+    xr[i] = make_double4(xn[0], xn[1], xn[2], radius[i]);          // one 32-byte sector per particle for the gather
 }
 
 // ------------------------------------------------------------------------------ radix sort
@@ -197,11 +198,8 @@ __global__ void __launch_bounds__(SORT_THREADS) dem_onesweep_kernel(
 
 // ------------------------------------------------------------------------------ gather + cell ranges
 __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
-                                  const double* __restrict__ x, const double* __restrict__ vp,
-                                  const double* __restrict__ wp, const double* __restrict__ radius,
-                                  double* __restrict__ xs, double* __restrict__ vps, double* __restrict__ wps,
-                                  double* __restrict__ rs, uint32_t* __restrict__ cell_start,
-                                  uint32_t* __restrict__ cell_end)
+                                  const double4* __restrict__ xr, double4* __restrict__ xr_s,
+                                  uint32_t* __restrict__ cell_start, uint32_t* __restrict__ cell_end)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -215,14 +213,9 @@ __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ s
     if (lane == 31 || s == P.n - 1) next = s < P.n - 1 ? skey[s + 1] : 0xffffffffu;
     if (s == 0 || prev != key) cell_start[key] = (uint32_t)s;
     if (s == P.n - 1 || next != key) cell_end[key] = (uint32_t)s + 1u;
-    const uint32_t p = sidx[s];
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        xs[3 * s + k] = x[3 * p + k];
-        vps[3 * s + k] = vp[3 * p + k];
-        wps[3 * s + k] = wp[3 * p + k];
-    }
-    rs[s] = radius[p];
+    const double2* src = reinterpret_cast<const double2*>(xr + sidx[s]);
+    const double2 a = __ldg(src), b = __ldg(src + 1);
+    xr_s[s] = make_double4(a.x, a.y, b.x, b.y);
 }
 
 // ------------------------------------------------------------------------------ contact law
@@ -283,94 +276,130 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
     for (int a = 0; a < 3; ++a) F[a] = fn * en[a] + Ft[a];
 }
 
-// One thread per particle, in sorted order.  History slots: [particle][slot] partner id + delta_t as
-// seen from that particle (the partner stores the negated vector).
-__global__ void __launch_bounds__(128) dem_contact_kernel(
+// One thread per particle, in sorted order, two phases so that the lanes of a warp stay together:
+//   1. detect: walk the 9 runs of x-adjacent neighbour cells (they are contiguous in the sorted order), test
+//      Eq. (2)/(6) on the packed (x, R) records with squared distances (the square root only when the decision
+//      is within rounding), and note the partners' sorted positions in a per-thread shared-memory list;
+//   2. evaluate: all lanes work through their k-th contact together: Eq. (7), (10)-(13), (5), (15), history.
+// History slots: [particle][slot] partner id + delta_t as seen from that particle (the partner stores the
+// negated vector).  Per-particle sums stay in registers: no atomics.
+#define CONTACT_BLOCK 128
+
+__device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, const double4& b)
+{
+    const double xa[3] = {a.x, a.y, a.z}, xb[3] = {b.x, b.y, b.z};
+    double d[3];
+    dem_min_image(P, xa, xb, d);
+    const double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    const double sr = a.w + b.w, s2 = sr * sr;
+    if (d2 > s2 * (1.0 + 1e-14)) return false;
+    if (d2 < s2 * (1.0 - 1e-14)) return true;
+    return sr - sqrt(d2) > 0.0;                                                       // Eq. (2), (6), strict (G7)
+}
+
+__global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
     const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
-    const double* __restrict__ xs, const double* __restrict__ vps, const double* __restrict__ wps,
-    const double* __restrict__ rs, const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ cell_end,
+    const double4* __restrict__ xr_s, const double* __restrict__ vp, const double* __restrict__ wp,
+    const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ cell_end,
     const uint32_t* __restrict__ hcount_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
     uint32_t* __restrict__ hcount_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
     double* __restrict__ force, double* __restrict__ torque, int32_t* __restrict__ status, double dt_hist)
 {
+    extern __shared__ uint32_t s_list[];                       // [maxc][CONTACT_BLOCK] sorted positions of the partners
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
-    const uint32_t p = sidx[s];
-    const uint32_t key = skey[s];
-    Body me;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { me.x[a] = xs[3 * s + a]; me.v[a] = vps[3 * s + a]; me.w[a] = wps[3 * s + a]; }
-    me.R = rs[s];
-    const double m_me = dem_mass(P, me.R);
     const int maxc = P.maxc;
-    const uint32_t nprev = hcount_prev[p];
-    const uint32_t* pid = hid_prev + (size_t)p * maxc;
-    const double* pdt = hdt_prev + (size_t)p * maxc * 3;
-    uint32_t* nid = hid_new + (size_t)p * maxc;
-    double* ndt = hdt_new + (size_t)p * maxc * 3;
-
-    double Fs[3] = {0, 0, 0}, Ms[3] = {0, 0, 0};
-    uint32_t ncont = 0;
+    const uint32_t key = skey[s];
+    const double4 mine = xr_s[s];
     int st = 0;
+    int ncand = 0;
 
     const int c0 = (int)(key % (uint32_t)P.nc[0]);
     const int c1 = (int)((key / (uint32_t)P.nc[0]) % (uint32_t)P.nc[1]);
     const int c2 = (int)(key / ((uint32_t)P.nc[0] * (uint32_t)P.nc[1]));
 
+    // ---- phase 1: detect
     for (int dz = -1; dz <= 1; ++dz) {
         int qz = c2 + dz;
         if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) continue; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
         for (int dy = -1; dy <= 1; ++dy) {
             int qy = c1 + dy;
             if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) continue; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
-            for (int dx = -1; dx <= 1; ++dx) {
-                int qx = c0 + dx;
-                if (qx < 0 || qx >= P.nc[0]) { if (P.bc[0]) continue; qx = qx < 0 ? qx + P.nc[0] : qx - P.nc[0]; }
-                const uint32_t cell = (uint32_t)(qx + P.nc[0] * (qy + P.nc[1] * qz));
-                const uint32_t t0 = cell_start[cell], t1 = cell_end[cell];
+            const uint32_t rowc = (uint32_t)P.nc[0] * (uint32_t)(qy + P.nc[1] * qz);
+            // run 0: the cells c0-1 .. c0+1 that lie inside the row; run 1: the one wrapped cell of a periodic row
+            const int lo = max(c0 - 1, 0), hi = min(c0 + 1, P.nc[0] - 1);
+            const int wrapped = P.bc[0] ? -1 : (c0 == 0 ? P.nc[0] - 1 : (c0 == P.nc[0] - 1 ? 0 : -1));
+            for (int run = 0; run < 2; ++run) {
+                uint32_t t0 = 0, t1 = 0;
+                if (run == 0) {
+                    bool any = false;
+                    for (int c = lo; c <= hi; ++c) {
+                        const uint32_t a = cell_start[rowc + c], b = cell_end[rowc + c];
+                        if (b > a) { if (!any) t0 = a; t1 = b; any = true; }
+                    }
+                } else {
+                    if (wrapped < 0 || (wrapped >= lo && wrapped <= hi)) break;
+                    t0 = cell_start[rowc + wrapped]; t1 = cell_end[rowc + wrapped];
+                }
                 for (uint32_t t = t0; t < t1; ++t) {
                     if ((int)t == s) continue;
-                    Body ot;
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) ot.x[a] = xs[3 * t + a];
-                    ot.R = rs[t];
-                    const uint32_t q = sidx[t];
-                    const bool me_first = p < q;
-                    const Body& bi = me_first ? me : ot;
-                    const Body& bj = me_first ? ot : me;
-                    double d[3];
-                    dem_min_image(P, bi.x, bj.x, d);
-                    const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-                    const double dn = (bi.R + bj.R) - dist;                            // Eq. (6)
-                    if (!(dn > 0.0)) continue;                                         // Eq. (2), strict
-                    if (dist == 0.0) { st |= LEDDS_ST_COINCIDENT; continue; }
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) { ot.v[a] = vps[3 * t + a]; ot.w[a] = wps[3 * t + a]; }
-                    double en[3] = {d[0] / dist, d[1] / dist, d[2] / dist};            // Eq. (7)
-                    const double mi = dem_mass(P, bi.R), mj = dem_mass(P, bj.R);
-                    const double mstar = mi * mj / (mi + mj);                          // (A.9)
-                    // previous delta_t of this pair, in canonical orientation
-                    double dt3[3] = {0, 0, 0};
-                    for (uint32_t h = 0; h < nprev; ++h)
-                        if (pid[h] == q) {
-                            const double sg = me_first ? 1.0 : -1.0;
-                            dt3[0] = sg * pdt[3 * h]; dt3[1] = sg * pdt[3 * h + 1]; dt3[2] = sg * pdt[3 * h + 2];
-                            break;
-                        }
-                    double F[3], T[3];
-                    dem_pair_force(en, dn, bi.v, bi.w, bi.R, bj.v, bj.w, bj.R, mstar, P.kn, P.kt, P.zeta, P.mu, dt_hist,
-                                   dt3, F, T);
-                    const double sg = me_first ? 1.0 : -1.0;
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) { Fs[a] += sg * F[a]; Ms[a] += me.R * (-T[a]); }
-                    if (ncont < (uint32_t)maxc) {
-                        nid[ncont] = q;
-                        ndt[3 * ncont] = sg * dt3[0]; ndt[3 * ncont + 1] = sg * dt3[1]; ndt[3 * ncont + 2] = sg * dt3[2];
-                        ++ncont;
-                    } else st |= LEDDS_ST_CONTACT_OVERFLOW;
+                    if (!dem_touch(P, mine, xr_s[t])) continue;
+                    if (ncand < maxc) s_list[ncand * CONTACT_BLOCK + threadIdx.x] = t;
+                    else st |= LEDDS_ST_CONTACT_OVERFLOW;
+                    ncand += ncand < maxc;
                 }
             }
         }
+    }
+
+    // ---- phase 2: evaluate
+    const uint32_t p = sidx[s];
+    Body me;
+    me.x[0] = mine.x; me.x[1] = mine.y; me.x[2] = mine.z; me.R = mine.w;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { me.v[a] = vp[3 * p + a]; me.w[a] = wp[3 * p + a]; }
+    const double m_me = dem_mass(P, me.R);
+    const uint32_t nprev = hcount_prev[p];
+    const uint32_t* pid = hid_prev + (size_t)p * maxc;
+    const double* pdt = hdt_prev + (size_t)p * maxc * 3;
+    uint32_t* nid = hid_new + (size_t)p * maxc;
+    double* ndt = hdt_new + (size_t)p * maxc * 3;
+    double Fs[3] = {0, 0, 0}, Ms[3] = {0, 0, 0};
+    uint32_t ncont = 0;
+
+    for (int c = 0; c < ncand; ++c) {
+        const uint32_t t = s_list[c * CONTACT_BLOCK + threadIdx.x];
+        const double4 o4 = xr_s[t];
+        const uint32_t q = sidx[t];
+        Body ot;
+        ot.x[0] = o4.x; ot.x[1] = o4.y; ot.x[2] = o4.z; ot.R = o4.w;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { ot.v[a] = vp[3 * q + a]; ot.w[a] = wp[3 * q + a]; }
+        const bool me_first = p < q;                                                   // canonical orientation i < j
+        const Body& bi = me_first ? me : ot;
+        const Body& bj = me_first ? ot : me;
+        double d[3];
+        dem_min_image(P, bi.x, bj.x, d);
+        const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        const double dn = (bi.R + bj.R) - dist;                                        // Eq. (6)
+        if (dist == 0.0) { st |= LEDDS_ST_COINCIDENT; continue; }
+        double en[3] = {d[0] / dist, d[1] / dist, d[2] / dist};                        // Eq. (7)
+        const double mi = dem_mass(P, bi.R), mj = dem_mass(P, bj.R);
+        const double mstar = mi * mj / (mi + mj);                                      // (A.9)
+        const double sg = me_first ? 1.0 : -1.0;
+        double dt3[3] = {0, 0, 0};                                                     // previous delta_t, canonical
+        for (uint32_t h = 0; h < nprev; ++h)
+            if (pid[h] == q) {
+                dt3[0] = sg * pdt[3 * h]; dt3[1] = sg * pdt[3 * h + 1]; dt3[2] = sg * pdt[3 * h + 2];
+                break;
+            }
+        double F[3], T[3];
+        dem_pair_force(en, dn, bi.v, bi.w, bi.R, bj.v, bj.w, bj.R, mstar, P.kn, P.kt, P.zeta, P.mu, dt_hist, dt3, F, T);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { Fs[a] += sg * F[a]; Ms[a] += me.R * (-T[a]); }
+        nid[ncont] = q;
+        ndt[3 * ncont] = sg * dt3[0]; ndt[3 * ncont + 1] = sg * dt3[1]; ndt[3 * ncont + 2] = sg * dt3[2];
+        ++ncont;
     }
     // walls: static infinite particles with a surface velocity
     for (int wl = 0; wl < 6; ++wl) {
@@ -560,7 +589,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     s.cell_start = take((size_t)d.ncell * 4);
     s.cell_end = take((size_t)d.ncell * 4);
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
-    s.xs = take(n * 24); s.vps = take(n * 24); s.wps = take(n * 24); s.rs = take(n * 8);
+    s.xr = take(n * 32); s.xr_s = take(n * 32);
     s.vp = take(n * 24); s.wp = take(n * 24);
     s.force = take(n * 24); s.torque = take(n * 24);
     s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4);
@@ -606,7 +635,8 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     // clear sort bookkeeping + cell ranges (one contiguous region)
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
     ledds_prof_start(LEDDS_K_DEM_KEYS, st);
-    dem_drift_key_kernel<<<nb, tb, 0, st>>>(d, x, v, w, a, alpha, at<double>(scratch, s.vp), at<double>(scratch, s.wp),
+    dem_drift_key_kernel<<<nb, tb, 0, st>>>(d, x, v, w, a, alpha, radius, at<double>(scratch, s.vp),
+                                            at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
                                             at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
     ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
     LEDDS_CHECK_LAUNCH();
@@ -630,18 +660,16 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     const uint32_t* skey = at<uint32_t>(scratch, s.key[h->sorted_buf]);
     const uint32_t* sidx = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
     ledds_prof_start(LEDDS_K_DEM_GATHER, st);
-    dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sidx, x, at<double>(scratch, s.vp), at<double>(scratch, s.wp), radius,
-                                         at<double>(scratch, s.xs), at<double>(scratch, s.vps), at<double>(scratch, s.wps),
-                                         at<double>(scratch, s.rs), at<uint32_t>(scratch, s.cell_start),
-                                         at<uint32_t>(scratch, s.cell_end));
+    dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr), at<double4>(scratch, s.xr_s),
+                                         at<uint32_t>(scratch, s.cell_start), at<uint32_t>(scratch, s.cell_end));
     ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
     LEDDS_CHECK_LAUNCH();
     const DemHistory& hs = h->hs;
     const int prev = h->cur, nw = 1 - h->cur;
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
-    dem_contact_kernel<<<nb, tb, 0, st>>>(
-        d, skey, sidx, at<double>(scratch, s.xs), at<double>(scratch, s.vps), at<double>(scratch, s.wps),
-        at<double>(scratch, s.rs), at<uint32_t>(scratch, s.cell_start), at<uint32_t>(scratch, s.cell_end),
+    dem_contact_kernel<<<nb, CONTACT_BLOCK, (size_t)d.maxc * CONTACT_BLOCK * sizeof(uint32_t), st>>>(
+        d, skey, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
+        at<uint32_t>(scratch, s.cell_start), at<uint32_t>(scratch, s.cell_end),
         at<uint32_t>(history, hs.count[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
         at<uint32_t>(history, hs.count[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]),
         at<double>(scratch, s.force), at<double>(scratch, s.torque), status, dt_hist);
