@@ -27,6 +27,7 @@
 #define ST_FLAG_AGG 0x40000000u
 #define ST_FLAG_PRE 0x80000000u
 #define ST_VALUE_MASK 0x3fffffffu
+#define LOOKBACK 8
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -108,6 +109,9 @@ __global__ void __launch_bounds__(SORT_THREADS) dem_onesweep_kernel(
 {
     __shared__ uint32_t warp_hist[SORT_WARPS][SORT_RADIX];
     __shared__ uint32_t bin_base[SORT_RADIX];
+    __shared__ uint32_t tile_start[SORT_RADIX];
+    __shared__ uint32_t wsum2[SORT_WARPS];
+    __shared__ uint32_t stage_key[SORT_TILE], stage_val[SORT_TILE];
     __shared__ uint32_t s_tile;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
@@ -138,11 +142,15 @@ __global__ void __launch_bounds__(SORT_THREADS) dem_onesweep_kernel(
     uint32_t k[SORT_ITEMS], v[SORT_ITEMS], r[SORT_ITEMS];
     const long long base = (long long)tile * SORT_TILE + (long long)warp * (SORT_ITEMS * 32);
 #pragma unroll
-    for (int it = 0; it < SORT_ITEMS; ++it) {
+    for (int it = 0; it < SORT_ITEMS; ++it) {                   // all loads first: 2 x SORT_ITEMS independent requests
         const long long i = base + it * 32 + lane;
         const bool ok = i < n;
         k[it] = ok ? key_in[i] : 0xffffffffu;
         v[it] = ok ? val_in[i] : 0u;
+    }
+#pragma unroll
+    for (int it = 0; it < SORT_ITEMS; ++it) {
+        const bool ok = base + it * 32 + lane < n;
         const uint32_t d = ok ? ((k[it] >> shift) & 255u) : 256u;
         const uint32_t peers = __match_any_sync(0xffffffffu, d);
         const uint32_t below = __popc(peers & ((1u << lane) - 1u));
@@ -171,28 +179,60 @@ __global__ void __launch_bounds__(SORT_THREADS) dem_onesweep_kernel(
             st_volatile(my, ST_FLAG_PRE | run);
         } else {
             st_volatile(my, ST_FLAG_AGG | run);
-            for (long long t = (long long)tile - 1; t >= 0; --t) {
-                const uint32_t* p = tile_state + (size_t)t * SORT_RADIX + d;
-                uint32_t s;
-                do { s = ld_volatile(p); } while ((s & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0);
-                excl += s & ST_VALUE_MASK;
-                if (s & ST_FLAG_PRE) break;
+            // look back over the predecessors' descriptors, LOOKBACK of them per round trip
+            long long t = (long long)tile - 1;
+            bool done = false;
+            while (!done) {
+                uint32_t sv[LOOKBACK];
+#pragma unroll
+                for (int b = 0; b < LOOKBACK; ++b)
+                    sv[b] = t - b >= 0 ? ld_volatile(tile_state + (size_t)(t - b) * SORT_RADIX + d) : ST_FLAG_PRE;
+#pragma unroll
+                for (int b = 0; b < LOOKBACK; ++b) {
+                    if (done) break;
+                    uint32_t sb = sv[b];
+                    while ((sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0) sb = ld_volatile(tile_state + (size_t)(t - b) * SORT_RADIX + d);
+                    excl += sb & ST_VALUE_MASK;
+                    if (sb & ST_FLAG_PRE) done = true;
+                }
+                t -= LOOKBACK;
             }
             st_volatile(my, ST_FLAG_PRE | (excl + run));
         }
-        bin_base[d] = digit_excl + excl;
+        // where digit d starts inside this tile once the tile is ordered by digit (block-wide exclusive scan of run)
+        uint32_t incl = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t u = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += u;
+        }
+        if (lane == 31) wsum2[warp] = incl;
+        __syncthreads();
+        uint32_t before = 0;
+        for (int w2 = 0; w2 < warp; ++w2) before += wsum2[w2];
+        tile_start[d] = before + incl - run;
+        bin_base[d] = digit_excl + excl - (before + incl - run);    // global position = bin_base[d] + position in the tile
     }
     __syncthreads();
 
+    // order the tile by digit in shared memory, so that the global writes of a digit are contiguous
 #pragma unroll
     for (int it = 0; it < SORT_ITEMS; ++it) {
-        const long long i = base + it * 32 + lane;
-        if (i < n) {
+        if (base + it * 32 + lane < n) {
             const uint32_t d = (k[it] >> shift) & 255u;
-            const uint32_t dst = bin_base[d] + warp_hist[warp][d] + r[it];
-            key_out[dst] = k[it];
-            val_out[dst] = v[it];
+            const uint32_t lp = tile_start[d] + warp_hist[warp][d] + r[it];
+            stage_key[lp] = k[it];
+            stage_val[lp] = v[it];
         }
+    }
+    __syncthreads();
+    const long long tile_first = (long long)tile * SORT_TILE;
+    const int count = (int)min((long long)SORT_TILE, (long long)n - tile_first);
+    for (int i = tid; i < count; i += SORT_THREADS) {
+        const uint32_t kk = stage_key[i];
+        const uint32_t dst = bin_base[(kk >> shift) & 255u] + (uint32_t)i;
+        key_out[dst] = kk;
+        val_out[dst] = stage_val[i];
     }
 }
 
@@ -356,6 +396,17 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
     const uint32_t p = sidx[s];
     Body me;
     me.x[0] = mine.x; me.x[1] = mine.y; me.x[2] = mine.z; me.R = mine.w;
+    bool near_wall = false;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+        if (P.bc[a] && (me.x[a] - P.lo[a] < me.R || P.hi[a] - me.x[a] < me.R)) near_wall = true;
+    if (ncand == 0 && !near_wall) {                             // the usual case in a dilute state: nothing touches
+        hcount_new[p] = 0u;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { force[3 * p + a] = 0.0; torque[3 * p + a] = 0.0; }
+        if (st) atomicOr(status, st);
+        return;
+    }
 #pragma unroll
     for (int a = 0; a < 3; ++a) { me.v[a] = vp[3 * p + a]; me.w[a] = wp[3 * p + a]; }
     const double m_me = dem_mass(P, me.R);
