@@ -84,13 +84,12 @@ struct DemScratch {
     size_t cell_start, cell_end;   // uint32 [ncell]
     size_t xr, xr_s;               // (x, y, z, R) per particle, 32 B: particle order / sorted order
     size_t vp, wp;                 // predictor velocities in particle order: double [n][3]
-    size_t force, torque;          // contact force / torque per particle: double [n][3]
     size_t pair_count, pair_off;   // query scratch (uint32 [n+1])
     size_t total;
 };
 
 struct DemHistory {
-    size_t count[2];               // uint32 [n]
+    size_t ft[2];                  // per particle, 64 B: contact force[3], torque[3], number of contacts, pad
     size_t id[2];                  // uint32 [n][maxc]
     size_t dt[2];                  // double [n][maxc][3]
     size_t total;
@@ -112,4 +111,4 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
                                const double* alpha, const double* radius, void* history, void* scratch,
                                int32_t* status, double dt_hist, bool drift, cudaStream_t st);
 int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha, const double* radius,
-                   const double* f_ext, const double* m_ext, void* scratch, int32_t* status, cudaStream_t st);
+                   const double* f_ext, const double* m_ext, const void* history, int32_t* status, cudaStream_t st);

@@ -308,7 +308,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
             rc = ledds_dem_advance_contacts(dem, x, v, w, a, alpha, radius, history, scratch, status, dem->d.dt, true, st);
             if (rc) return rc;
             if (sub < c->n_sub - 1) {                                        // F_sf of the previous LBM step is held
-                rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, scratch, status, st);
+                rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);
                 if (rc) return rc;
                 dem->steps++;
             }
@@ -333,7 +333,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         cpl_reduce_kernel<<<warp_blocks, 128, 0, st>>>(C, f_hyd, m_hyd);
         ledds_prof_stop(LEDDS_K_CPL_REDUCE, st);
         LEDDS_CHECK_LAUNCH();
-        rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, scratch, status, st);
+        rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);
         if (rc) return rc;
         dem->steps++;
     }

@@ -325,6 +325,16 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // negated vector).  Per-particle sums stay in registers: no atomics.
 #define CONTACT_BLOCK 128
 
+// one full 64-byte record per particle: contact force, torque, number of contacts (exact in a double), pad
+__device__ __forceinline__ void dem_store_ft(double* __restrict__ ft, uint32_t p, const double* F, const double* M, uint32_t count)
+{
+    double2* o = reinterpret_cast<double2*>(ft + 8 * (size_t)p);
+    o[0] = make_double2(F[0], F[1]);
+    o[1] = make_double2(F[2], M[0]);
+    o[2] = make_double2(M[1], M[2]);
+    o[3] = make_double2((double)count, 0.0);
+}
+
 __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, const double4& b)
 {
     const double xa[3] = {a.x, a.y, a.z}, xb[3] = {b.x, b.y, b.z};
@@ -341,9 +351,9 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
     const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
     const double4* __restrict__ xr_s, const double* __restrict__ vp, const double* __restrict__ wp,
     const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ cell_end,
-    const uint32_t* __restrict__ hcount_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
-    uint32_t* __restrict__ hcount_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
-    double* __restrict__ force, double* __restrict__ torque, int32_t* __restrict__ status, double dt_hist)
+    const double* __restrict__ ft_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
+    double* __restrict__ ft_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
+    int32_t* __restrict__ status, double dt_hist)
 {
     extern __shared__ uint32_t s_list[];                       // [maxc][CONTACT_BLOCK] sorted positions of the partners
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -400,17 +410,16 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
 #pragma unroll
     for (int a = 0; a < 3; ++a)
         if (P.bc[a] && (me.x[a] - P.lo[a] < me.R || P.hi[a] - me.x[a] < me.R)) near_wall = true;
+    const double Fs0[3] = {0.0, 0.0, 0.0};
     if (ncand == 0 && !near_wall) {                             // the usual case in a dilute state: nothing touches
-        hcount_new[p] = 0u;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { force[3 * p + a] = 0.0; torque[3 * p + a] = 0.0; }
+        dem_store_ft(ft_new, p, Fs0, Fs0, 0u);
         if (st) atomicOr(status, st);
         return;
     }
 #pragma unroll
     for (int a = 0; a < 3; ++a) { me.v[a] = vp[3 * p + a]; me.w[a] = wp[3 * p + a]; }
     const double m_me = dem_mass(P, me.R);
-    const uint32_t nprev = hcount_prev[p];
+    const uint32_t nprev = (uint32_t)ft_prev[8 * (size_t)p + 6];
     const uint32_t* pid = hid_prev + (size_t)p * maxc;
     const double* pdt = hdt_prev + (size_t)p * maxc * 3;
     uint32_t* nid = hid_new + (size_t)p * maxc;
@@ -476,19 +485,16 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
             ++ncont;
         } else st |= LEDDS_ST_CONTACT_OVERFLOW;
     }
-    hcount_new[p] = ncont;
 #pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        force[3 * p + a] = Fs[a];
-        torque[3 * p + a] = Ms[a];
+    for (int a = 0; a < 3; ++a)
         if (!isfinite(Fs[a]) || !isfinite(Ms[a])) st |= LEDDS_ST_NONFINITE;
-    }
+    dem_store_ft(ft_new, p, Fs, Ms, ncont);
     if (st) atomicOr(status, st);
 }
 
 // ------------------------------------------------------------------------------ kick
-__global__ void dem_kick_kernel(const DemDev P, const double* __restrict__ radius, const double* __restrict__ force,
-                                const double* __restrict__ torque, const double* __restrict__ f_ext,
+__global__ void dem_kick_kernel(const DemDev P, const double* __restrict__ radius, const double* __restrict__ ft,
+                                const double* __restrict__ f_ext,
                                 const double* __restrict__ m_ext, double* __restrict__ v, double* __restrict__ w,
                                 double* __restrict__ a, double* __restrict__ alpha, int only_accel)
 {
@@ -499,7 +505,7 @@ __global__ void dem_kick_kernel(const DemDev P, const double* __restrict__ radiu
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         const int q = 3 * i + k;
-        const double Fq = force[q] + (f_ext ? f_ext[q] : 0.0), Mq = torque[q] + (m_ext ? m_ext[q] : 0.0);
+        const double Fq = ft[8 * (size_t)i + k] + (f_ext ? f_ext[q] : 0.0), Mq = ft[8 * (size_t)i + 3 + k] + (m_ext ? m_ext[q] : 0.0);
         const double an = Fq / m + P.g[k], aln = Mq / I;                              // Eq. (18b), (19c)
         if (!only_accel) {
             v[q] = v[q] + (0.5 * P.dt) * (a[q] + an);                                 // Eq. (18c)
@@ -511,14 +517,25 @@ __global__ void dem_kick_kernel(const DemDev P, const double* __restrict__ radiu
 }
 
 // ------------------------------------------------------------------------------ query (parity only)
-__global__ void dem_pair_count_kernel(int n, int maxc, const uint32_t* __restrict__ hcount,
+__global__ void dem_pair_count_kernel(int n, int maxc, const double* __restrict__ ft,
                                       const uint32_t* __restrict__ hid, uint32_t* __restrict__ cnt)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
     uint32_t c = 0;
-    for (uint32_t h = 0; h < hcount[p]; ++h) c += hid[(size_t)p * maxc + h] > (uint32_t)p;
+    const uint32_t hc = (uint32_t)ft[8 * (size_t)p + 6];
+    for (uint32_t h = 0; h < hc; ++h) c += hid[(size_t)p * maxc + h] > (uint32_t)p;
     cnt[p] = c;
+}
+
+__global__ void dem_unpack_ft_kernel(int n, const double* __restrict__ ft, double* __restrict__ force, double* __restrict__ torque)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    for (int a = 0; a < 3; ++a) {
+        if (force) force[3 * p + a] = ft[8 * (size_t)p + a];
+        if (torque) torque[3 * p + a] = ft[8 * (size_t)p + 3 + a];
+    }
 }
 
 // single-block exclusive scan of cnt[n] into off[n+1]
@@ -559,7 +576,7 @@ __global__ void __launch_bounds__(1024) dem_scan_kernel(int n, const uint32_t* _
     if (tid == 0) off[n] = carry;
 }
 
-__global__ void dem_pair_write_kernel(int n, int maxc, const uint32_t* __restrict__ hcount,
+__global__ void dem_pair_write_kernel(int n, int maxc, const double* __restrict__ ft,
                                       const uint32_t* __restrict__ hid, const double* __restrict__ hdt,
                                       const uint32_t* __restrict__ off, uint32_t cap, uint32_t* __restrict__ pairs,
                                       double* __restrict__ pair_dt, uint32_t* __restrict__ n_pairs)
@@ -569,7 +586,8 @@ __global__ void dem_pair_write_kernel(int n, int maxc, const uint32_t* __restric
     if (p >= n) return;
     uint32_t ids[32], slot[32];
     int c = 0;
-    for (uint32_t h = 0; h < hcount[p]; ++h) {
+    const uint32_t hc = (uint32_t)ft[8 * (size_t)p + 6];
+    for (uint32_t h = 0; h < hc; ++h) {
         const uint32_t q = hid[(size_t)p * maxc + h];
         if (q <= (uint32_t)p) continue;
         int k = c++;
@@ -642,14 +660,13 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
     s.xr = take(n * 32); s.xr_s = take(n * 32);
     s.vp = take(n * 24); s.wp = take(n * 24);
-    s.force = take(n * 24); s.torque = take(n * 24);
     s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4);
     s.total = o;
 
     DemHistory& hs = h->hs;
     o = 0;
     for (int b = 0; b < 2; ++b) {
-        hs.count[b] = take(n * 4);
+        hs.ft[b] = take(n * 64);
         hs.id[b] = take(n * d.maxc * 4);
         hs.dt[b] = take(n * d.maxc * 24);
     }
@@ -721,9 +738,8 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     dem_contact_kernel<<<nb, CONTACT_BLOCK, (size_t)d.maxc * CONTACT_BLOCK * sizeof(uint32_t), st>>>(
         d, skey, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
         at<uint32_t>(scratch, s.cell_start), at<uint32_t>(scratch, s.cell_end),
-        at<uint32_t>(history, hs.count[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
-        at<uint32_t>(history, hs.count[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]),
-        at<double>(scratch, s.force), at<double>(scratch, s.torque), status, dt_hist);
+        at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
+        at<double>(history, hs.ft[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]), status, dt_hist);
     ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
     LEDDS_CHECK_LAUNCH();
     h->cur = nw;
@@ -731,13 +747,12 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
 }
 
 int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha, const double* radius,
-                   const double* f_ext, const double* m_ext, void* scratch, int32_t* status, cudaStream_t st)
+                   const double* f_ext, const double* m_ext, const void* history, int32_t* status, cudaStream_t st)
 {
     (void)status;
     const int n = h->d.n, tb = 128, nb = (n + tb - 1) / tb;
     ledds_prof_start(LEDDS_K_DEM_KICK, st);
-    dem_kick_kernel<<<nb, tb, 0, st>>>(h->d, radius, at<double>(scratch, h->s.force), at<double>(scratch, h->s.torque),
-                                       f_ext, m_ext, v, w, a, alpha, 0);
+    dem_kick_kernel<<<nb, tb, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), f_ext, m_ext, v, w, a, alpha, 0);
     ledds_prof_stop(LEDDS_K_DEM_KICK, st);
     LEDDS_CHECK_LAUNCH();
     return LEDDS_OK;
@@ -764,8 +779,8 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
     rc = ledds_dem_advance_contacts(h, const_cast<double*>(x), v, w, a, alpha, radius, history, scratch, status, 0.0, false, st);
     if (rc) { delete h; return rc; }
     const int tb = 128, nb = (h->d.n + tb - 1) / tb;
-    dem_kick_kernel<<<nb, tb, 0, st>>>(h->d, radius, at<double>(scratch, h->s.force), at<double>(scratch, h->s.torque),
-                                       nullptr, nullptr, nullptr, nullptr, a, alpha, 1);
+    dem_kick_kernel<<<nb, tb, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), nullptr, nullptr, nullptr,
+                                       nullptr, a, alpha, 1);
     ledds_count_launch(1);
     if (cudaPeekAtLastError() != cudaSuccess) { delete h; return LEDDS_ECUDA; }
     *out = h;
@@ -784,7 +799,7 @@ extern "C" int ledds_dem_step(ledds_dem* h, double* x, double* v, double* w, dou
     for (int s = 0; s < nsteps; ++s) {
         int rc = ledds_dem_advance_contacts(h, x, v, w, a, alpha, radius, history, scratch, status, h->d.dt, true, st);
         if (rc) return rc;
-        rc = ledds_dem_kick(h, v, w, a, alpha, radius, f_ext, m_ext, scratch, status, st);
+        rc = ledds_dem_kick(h, v, w, a, alpha, radius, f_ext, m_ext, history, status, st);
         if (rc) return rc;
         h->steps++;
     }
@@ -803,19 +818,22 @@ extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* sc
         return !dst || cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st) == cudaSuccess;
     };
     if (!copy(sorted_idx, at<char>(scratch, s.idx[h->sorted_buf]), n * 4) ||
-        !copy(sorted_key, at<char>(scratch, s.key[h->sorted_buf]), n * 4) ||
-        !copy(force, at<char>(scratch, s.force), n * 24) || !copy(torque, at<char>(scratch, s.torque), n * 24))
+        !copy(sorted_key, at<char>(scratch, s.key[h->sorted_buf]), n * 4))
         return LEDDS_ECUDA;
+    if (force || torque) {
+        dem_unpack_ft_kernel<<<((int)n + 127) / 128, 128, 0, st>>>((int)n, at<double>(history, h->hs.ft[h->cur]), force, torque);
+        LEDDS_CHECK_LAUNCH();
+    }
     if (pairs || pair_dt || n_pairs) {
         const DemHistory& hs = h->hs;
         const int tb = 128, nb = ((int)n + tb - 1) / tb;
         // scratch is logically const for the caller; the two query arrays are ours to overwrite
         uint32_t* cnt = const_cast<uint32_t*>(at<uint32_t>(scratch, s.pair_count));
         uint32_t* off = const_cast<uint32_t*>(at<uint32_t>(scratch, s.pair_off));
-        dem_pair_count_kernel<<<nb, tb, 0, st>>>((int)n, h->d.maxc, at<uint32_t>(history, hs.count[h->cur]),
+        dem_pair_count_kernel<<<nb, tb, 0, st>>>((int)n, h->d.maxc, at<double>(history, hs.ft[h->cur]),
                                                  at<uint32_t>(history, hs.id[h->cur]), cnt);
         dem_scan_kernel<<<1, 1024, 0, st>>>((int)n, cnt, off);
-        dem_pair_write_kernel<<<nb, tb, 0, st>>>((int)n, h->d.maxc, at<uint32_t>(history, hs.count[h->cur]),
+        dem_pair_write_kernel<<<nb, tb, 0, st>>>((int)n, h->d.maxc, at<double>(history, hs.ft[h->cur]),
                                                  at<uint32_t>(history, hs.id[h->cur]), at<double>(history, hs.dt[h->cur]),
                                                  off, pair_cap, pairs, pair_dt, n_pairs);
         ledds_count_launch(2);
