@@ -61,7 +61,8 @@ typedef struct {
                                 velocity-modified bounce-back: f -= 6 t_i rho (c_i . u_wall)      */
     int layout;              /* 0 = two-lattice (f holds 2 x 19 x N doubles).  1 (AA single array)
                                 is reserved: LEDDS_EINVAL in this version                         */
-    int variant;             /* kernel variant: 0 auto, 1 plain push, 2 row-rotate (aligned stores)*/
+    int variant;             /* kernel variant: 0 auto, 1 plain push, 2 row-rotate (aligned stores),
+                                3 plain push with 64-bit indices (the path lattices with 19 N >= 2^32 take) */
 } ledds_lbm_params;
 
 /* f_bytes: size of the population buffer the caller must allocate for this layout. */

@@ -323,7 +323,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         LEDDS_CHECK_LAUNCH();
         dim3 block(PSM_BLOCK), grid((d.nx + PSM_BLOCK - 1) / PSM_BLOCK, d.ny, d.nz);
         ledds_prof_start(LEDDS_K_LBM, st);
-        if (lb_fits_u32(d.N)) lbm_psm_kernel<unsigned><<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
+        if (lb_fits_u32(d.N) && lbm->p.variant != 3) lbm_psm_kernel<unsigned><<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
         else lbm_psm_kernel<long long><<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
         ledds_prof_stop(LEDDS_K_LBM, st);
         LEDDS_CHECK_LAUNCH();

@@ -169,7 +169,7 @@ static int lbm_validate(const ledds_lbm_params* p)
     if ((long long)p->nx * p->ny * p->nz > (1ll << 31)) return LEDDS_EINVAL;
     if (!(p->tau > 0.5)) return LEDDS_EINVAL;
     if (p->layout != 0) return LEDDS_EINVAL;
-    if (p->variant < 0 || p->variant > 2) return LEDDS_EINVAL;
+    if (p->variant < 0 || p->variant > 3) return LEDDS_EINVAL;
     for (int a = 0; a < 3; ++a)
         if (p->bc[a] != 0 && p->bc[a] != 1) return LEDDS_EINVAL;
     // a periodic axis of length 1 would stream a population onto itself: allowed (it is a no-op wrap)
@@ -243,7 +243,7 @@ static int lbm_launch(const ledds_lbm* h, const double* src, double* dst, cudaSt
 {
     const LbmDev& d = h->d;
     int variant = h->p.variant;
-    if (variant == 0) variant = 1;   // measured on B200: the plain push kernel already runs at the HBM copy rate
+    if (variant == 0) variant = 1;   // 3 = variant 1 with 64-bit indices whatever the size; measured on B200: the plain push kernel already runs at the HBM copy rate
     if (variant != 2 && (d.ny > 65535 || d.nz > 65535)) return LEDDS_EINVAL;
     ledds_prof_start(LEDDS_K_LBM, st);
     if (variant == 2) {
@@ -254,7 +254,7 @@ static int lbm_launch(const ledds_lbm* h, const double* src, double* dst, cudaSt
         lbm_rowrot_kernel<<<grid, block, 0, st>>>(src, dst, d);
     } else {
         dim3 block(128), grid((d.nx + 127) / 128, d.ny, d.nz);
-        if (lb_fits_u32(d.N)) lbm_push_kernel<unsigned><<<grid, block, 0, st>>>(src, dst, d);
+        if (lb_fits_u32(d.N) && variant != 3) lbm_push_kernel<unsigned><<<grid, block, 0, st>>>(src, dst, d);
         else lbm_push_kernel<long long><<<grid, block, 0, st>>>(src, dst, d);
     }
     ledds_prof_stop(LEDDS_K_LBM, st);

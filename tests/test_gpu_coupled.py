@@ -108,3 +108,41 @@ def test_three_solids_in_a_cell_are_flagged():
     o.step(1); g.step(1)
     assert o.status & 2 and int(g.dem.status[0].item()) & L.ST_SOLID_OVERFLOW
     compare(o, g)
+
+
+def test_ragged_row_and_64bit_index_path():
+    # nx = 72: the last 128-wide block of a row is mostly past the row end; variant 3 forces the 64-bit
+    # index instantiation that lattices with 19 N >= 2^32 take
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=3, n=72, n_part=40, R=4.0)
+    for variant in (0, 3):
+        o, g = both(dict(lbm, variant=variant), cpl, pd, x, v, w, R, u)
+        o.step(3); g.step(3)
+        compare(o, g)
+
+
+def test_two_solid_cells_take_the_second_solid():
+    # two spheres whose shells (R + r_c) overlap without touching: cells cut by both must carry both weights
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(48, 32, 32), R=4.0, z0=16.0, g=0.0)
+    pd = dict(pd, n=2)
+    x = np.array([[19.6, 16.2, 16.0], [28.3, 15.7, 16.4]])            # gap 0.7 < 2 r_c
+    vv = np.array([[0.01, 0.0, 0.0], [-0.01, 0.005, 0.0]]); ww = np.array([[0, 0, 0.002], [0.001, 0, 0]])
+    o, g = both(lbm, cpl, pd, x, vv, ww, np.full(2, 4.0))
+    o.step(2); g.step(2)
+    compare(o, g)
+    assert o.status == 0
+
+
+def test_full_size_config3_one_step():
+    # BASELINE configs[3] at full size in the launch configuration bench.py times: one coupled step against
+    # the oracle (all forces; populations on every 7th cell)
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear()
+    o, g = both(lbm, cpl, pd, x, v, w, R, u)
+    o.step(1); g.step(1)
+    F, M = g.f_hyd.cpu().numpy(), g.m_hyd.cpu().numpy()
+    assert np.abs(F - o.F_sf).max() <= 1e-10 * np.abs(o.F_sf).max() + 1e-13
+    assert np.abs(M - o.M_sf).max() <= 1e-10 * np.abs(o.M_sf).max() + 4e-13
+    s = g.dem.state()
+    assert np.abs(s["x"] - o.dem.x).max() <= 1e-9 * 256
+    assert int(g.dem.status[0].item()) == o.status == 0
+    f = g.lbm.export()
+    assert np.abs(f[:, ::7] - o.f[:, ::7]).max() <= 1e-12 * np.abs(o.f).max()

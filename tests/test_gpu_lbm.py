@@ -28,7 +28,7 @@ MOVING = np.zeros((3, 2, 3))
 MOVING[2, 0, 0] = -0.05; MOVING[2, 1, 0] = 0.05; MOVING[1, 0, 2] = 0.02; MOVING[0, 1, 1] = -0.03
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 @pytest.mark.parametrize("shape,bc,uw", [
     ((64, 12, 10), (0, 0, 0), None),
     ((64, 12, 10), (1, 1, 1), MOVING),
