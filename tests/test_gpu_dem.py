@@ -105,3 +105,32 @@ def test_history_persists_and_is_dropped():
     assert seen > 10 and len(o.pairs) == 0
     s = g.state()
     assert np.abs(s["w"] - o.w).max() <= 1e-9 * np.abs(o.w).max() and abs(o.w[0, 1]) > 1.0
+
+
+def test_full_size_config5_dense_state():
+    # BASELINE configs[4] size (4 000 000 polydisperse spheres) in the supplementary dense state, launch
+    # configuration of bench.py: ordering, pair list and contact forces of the initial state against the oracle
+    pd, x, v, w, R = W.cfg5_pour(dense=True)
+    o, g = both(pd, x, v, w, R)
+    check_state(o, g, 0, pd["hi"][2])
+    assert len(o.pairs) > 5_000_000
+
+
+def test_full_size_config5_pour_ordering_after_steps():
+    # the dilute pour state at full size: 3 steps on the GPU, then the ordering must be the stable argsort of the
+    # keys of the GPU's own positions (host-side check of a5-a7 at a size the oracle does not step quickly)
+    import oracle
+    pd, x, v, w, R = W.cfg5_pour()
+    from paper_2512_04997_b200 import Dem
+    g = Dem(pd, x, v, w, R)
+    g.step(3)
+    q = g.query()
+    nc, inv_h = oracle.dem_grid(pd)
+    xs = g.state()["x"]
+    c = np.clip(np.floor((xs - np.asarray(pd["lo"])) * inv_h).astype(np.int64), 0, np.asarray(nc) - 1)
+    key = (c[:, 0] + nc[0] * (c[:, 1] + nc[1] * c[:, 2])).astype(np.uint32)
+    idx = np.argsort(key, kind="stable").astype(np.uint32)
+    assert np.array_equal(q["idx"], idx) and np.array_equal(q["key"], key[idx])
+    assert q["status"] == 0 and len(q["pairs"]) == 0
+    # free fall so far: every sphere has v_z = -g t exactly as integrated (Eq. 18), no contact yet
+    assert np.allclose(g.state()["v"][:, 2], -9.81 * 3 * pd["dt"], rtol=1e-12)
