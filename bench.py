@@ -88,6 +88,15 @@ def coupled_bytes_per_step(n_cells):
     return 312.0 * n_cells
 
 
+def dem_bytes_per_particle(passes):
+    """Algorithmic HBM bytes per particle of each DEM kernel group."""
+    return {"dem_keys": 128 + 116,                 # x v w a alpha R read; x vp wp (x,R) key id written
+            "dem_sort": 4 + 16 * passes,           # histogram read + (key, id) read and written per pass
+            "dem_gather": 8 + 32 + 32,             # (key, id), one packed record read, one written
+            "dem_contact": 8 + 32 + 64,            # (key, id), own record, force/torque/count record written
+            "dem_kick": 8 + 64 + 96 + 96}          # R, record, v w a alpha read; v w a alpha written
+
+
 def max_over_ranks(ms, world, device="cuda"):
     """Elapsed time of the slowest rank (replicas run independently; the job is as slow as the slowest)."""
     if world <= 1:
@@ -238,8 +247,18 @@ def run_ours(args, rank, world):
             L.ledds_profile(False)
             q = torch.zeros(4, dtype=torch.int32, device="cuda")
             L.ledds_dem_query(gd.h, gd.history, gd.scratch, None, None, None, None, 0, q, None, None)
+            ncell = 1
+            for a in range(3):
+                ncell *= max(1, int((pd5["hi"][a] - pd5["lo"][a]) / pd5["cell"]))
+            bpp = dem_bytes_per_particle((max(1, int(np.ceil(np.log2(ncell)))) + 7) // 8)
+            gbs = {nm: round(bpp[nm] * len(R5) / (pr[nm] * 1e-3) / 1e9, 1) for nm in pr if pr[nm] > 0}
+            total_bytes = sum(bpp.values()) * len(R5)
             sub[name] = {"particle_updates_per_s": round(len(R5) * 1e3 / ms5, 1), "ms_per_step": round(ms5, 5), "steps": kd,
                          "particles": len(R5), "contacts": int(q[0].item()), "kernel_ms_per_step": pr,
+                         "algorithmic_bytes_per_particle": bpp, "kernel_hbm_gbs": gbs,
+                         "pipeline_hbm_gbs": round(total_bytes / (ms5 * 1e-3) / 1e9, 1),
+                         "pipeline_hbm_frac": round(total_bytes / (ms5 * 1e-3) / 1e9 / peak, 4),
+                         "note": "contacts add 28 B read + written per live contact end and the partner's state",
                          "status_word": int(gd.status[0].item())}
             del gd
             torch.cuda.empty_cache()

@@ -41,36 +41,46 @@ __device__ __forceinline__ int dem_cell_coord(const DemDev& P, double x, int a)
     return c > P.nc[a] - 1 ? P.nc[a] - 1 : c;
 }
 
-__global__ void dem_drift_key_kernel(const DemDev P, double* __restrict__ x, const double* __restrict__ v,
-                                     const double* __restrict__ w, const double* __restrict__ a,
-                                     const double* __restrict__ alpha, const double* __restrict__ radius,
-                                     double* __restrict__ vp, double* __restrict__ wp, double4* __restrict__ xr,
-                                     uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift)
+// Block = DRIFT_BLOCK particles.  The [n][3] arrays are walked as flat arrays (element e = 3 i + k), so every
+// load and store is fully coalesced; the new positions pass through shared memory to form the key and the
+// packed record per particle.
+#define DRIFT_BLOCK 128
+__global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
+    const DemDev P, double* __restrict__ x, const double* __restrict__ v, const double* __restrict__ w,
+    const double* __restrict__ a, const double* __restrict__ alpha, const double* __restrict__ radius,
+    double* __restrict__ vp, double* __restrict__ wp, double4* __restrict__ xr, uint32_t* __restrict__ key,
+    uint32_t* __restrict__ idx, int drift)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.n) return;
-    double xn[3];
+    __shared__ double sx[3 * DRIFT_BLOCK];
+    const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * P.n;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        const int q = 3 * i + k;
-        double xv = x[q];
-        const double vv = v[q], wv = w[q];
+    for (int j = 0; j < 3; ++j) {
+        const int le = threadIdx.x + j * DRIFT_BLOCK;
+        const long long e = e0 + le;
+        if (e >= ne) break;
+        const int k = le % 3;                                                 // e0 is a multiple of 3
+        double xv = x[e];
+        const double vv = v[e], wv = w[e];
         if (drift) {
-            const double av = a[q], alv = alpha[q];
-            xv = xv + P.dt * vv + (0.5 * P.dt * P.dt) * av;                 // Eq. (18a)
+            const double av = a[e], alv = alpha[e];
+            xv = xv + P.dt * vv + (0.5 * P.dt * P.dt) * av;                   // Eq. (18a)
             if (!P.bc[k]) {
                 if (xv >= P.hi[k]) xv -= P.L[k];
                 else if (xv < P.lo[k]) xv += P.L[k];
             }
-            x[q] = xv;
-            vp[q] = vv + (0.5 * P.dt) * av;                                 // predictor (G11)
-            wp[q] = wv + (0.5 * P.dt) * alv;
+            x[e] = xv;
+            vp[e] = vv + (0.5 * P.dt) * av;                                   // predictor (G11)
+            wp[e] = wv + (0.5 * P.dt) * alv;
         } else {
-            vp[q] = vv;
-            wp[q] = wv;
+            vp[e] = vv;
+            wp[e] = wv;
         }
-        xn[k] = xv;
+        sx[le] = xv;
     }
+    __syncthreads();
+    const int i = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
+    if (i >= P.n) return;
+    const double xn[3] = {sx[3 * threadIdx.x], sx[3 * threadIdx.x + 1], sx[3 * threadIdx.x + 2]};
     const int cx = dem_cell_coord(P, xn[0], 0), cy = dem_cell_coord(P, xn[1], 1), cz = dem_cell_coord(P, xn[2], 2);
     key[i] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
     idx[i] = (uint32_t)i;
@@ -239,7 +249,7 @@ __global__ void __launch_bounds__(SORT_THREADS) dem_onesweep_kernel(
 // ------------------------------------------------------------------------------ gather + cell ranges
 __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
                                   const double4* __restrict__ xr, double4* __restrict__ xr_s,
-                                  uint32_t* __restrict__ cell_start, uint32_t* __restrict__ cell_end)
+                                  uint2* __restrict__ cell_range)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -251,8 +261,8 @@ __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ s
     if (!ok) return;
     if (lane == 0) prev = s > 0 ? skey[s - 1] : 0xffffffffu;
     if (lane == 31 || s == P.n - 1) next = s < P.n - 1 ? skey[s + 1] : 0xffffffffu;
-    if (s == 0 || prev != key) cell_start[key] = (uint32_t)s;
-    if (s == P.n - 1 || next != key) cell_end[key] = (uint32_t)s + 1u;
+    if (s == 0 || prev != key) cell_range[key].x = (uint32_t)s;                    // [x, y) = the particles of the cell
+    if (s == P.n - 1 || next != key) cell_range[key].y = (uint32_t)s + 1u;
     const double2* src = reinterpret_cast<const double2*>(xr + sidx[s]);
     const double2 a = __ldg(src), b = __ldg(src + 1);
     xr_s[s] = make_double4(a.x, a.y, b.x, b.y);
@@ -335,11 +345,13 @@ __device__ __forceinline__ void dem_store_ft(double* __restrict__ ft, uint32_t p
     o[3] = make_double2((double)count, 0.0);
 }
 
+// PERIODIC = false: no axis is periodic, the nearest image is the particle itself
+template <bool PERIODIC>
 __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, const double4& b)
 {
     const double xa[3] = {a.x, a.y, a.z}, xb[3] = {b.x, b.y, b.z};
-    double d[3];
-    dem_min_image(P, xa, xb, d);
+    double d[3] = {xa[0] - xb[0], xa[1] - xb[1], xa[2] - xb[2]};
+    if (PERIODIC) dem_min_image(P, xa, xb, d);
     const double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
     const double sr = a.w + b.w, s2 = sr * sr;
     if (d2 > s2 * (1.0 + 1e-14)) return false;
@@ -347,10 +359,11 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
     return sr - sqrt(d2) > 0.0;                                                       // Eq. (2), (6), strict (G7)
 }
 
+template <bool PERIODIC>
 __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
     const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
     const double4* __restrict__ xr_s, const double* __restrict__ vp, const double* __restrict__ wp,
-    const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ cell_end,
+    const uint2* __restrict__ cell_range,
     const double* __restrict__ ft_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
     double* __restrict__ ft_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
     int32_t* __restrict__ status, double dt_hist)
@@ -384,16 +397,17 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
                 if (run == 0) {
                     bool any = false;
                     for (int c = lo; c <= hi; ++c) {
-                        const uint32_t a = cell_start[rowc + c], b = cell_end[rowc + c];
-                        if (b > a) { if (!any) t0 = a; t1 = b; any = true; }
+                        const uint2 r = cell_range[rowc + c];
+                        if (r.y > r.x) { if (!any) t0 = r.x; t1 = r.y; any = true; }
                     }
                 } else {
                     if (wrapped < 0 || (wrapped >= lo && wrapped <= hi)) break;
-                    t0 = cell_start[rowc + wrapped]; t1 = cell_end[rowc + wrapped];
+                    const uint2 r = cell_range[rowc + wrapped];
+                    t0 = r.x; t1 = r.y;
                 }
                 for (uint32_t t = t0; t < t1; ++t) {
                     if ((int)t == s) continue;
-                    if (!dem_touch(P, mine, xr_s[t])) continue;
+                    if (!dem_touch<PERIODIC>(P, mine, xr_s[t])) continue;
                     if (ncand < maxc) s_list[ncand * CONTACT_BLOCK + threadIdx.x] = t;
                     else st |= LEDDS_ST_CONTACT_OVERFLOW;
                     ncand += ncand < maxc;
@@ -493,27 +507,24 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
 }
 
 // ------------------------------------------------------------------------------ kick
+// One thread per vector component (element e = 3 i + k of the flat [n][3] arrays): coalesced.
 __global__ void dem_kick_kernel(const DemDev P, const double* __restrict__ radius, const double* __restrict__ ft,
-                                const double* __restrict__ f_ext,
-                                const double* __restrict__ m_ext, double* __restrict__ v, double* __restrict__ w,
-                                double* __restrict__ a, double* __restrict__ alpha, int only_accel)
+                                const double* __restrict__ f_ext, const double* __restrict__ m_ext, double* __restrict__ v,
+                                double* __restrict__ w, double* __restrict__ a, double* __restrict__ alpha, int only_accel)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.n) return;
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= 3ll * P.n) return;
+    const int i = (int)(e / 3), k = (int)(e - 3ll * i);
     const double R = radius[i];
     const double m = dem_mass(P, R), I = 0.4 * m * R * R;                             // Eq. (21a)
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        const int q = 3 * i + k;
-        const double Fq = ft[8 * (size_t)i + k] + (f_ext ? f_ext[q] : 0.0), Mq = ft[8 * (size_t)i + 3 + k] + (m_ext ? m_ext[q] : 0.0);
-        const double an = Fq / m + P.g[k], aln = Mq / I;                              // Eq. (18b), (19c)
-        if (!only_accel) {
-            v[q] = v[q] + (0.5 * P.dt) * (a[q] + an);                                 // Eq. (18c)
-            w[q] = w[q] + (0.5 * P.dt) * (alpha[q] + aln);                            // Eq. (19d)
-        }
-        a[q] = an;
-        alpha[q] = aln;
+    const double Fq = ft[8 * (size_t)i + k] + (f_ext ? f_ext[e] : 0.0), Mq = ft[8 * (size_t)i + 3 + k] + (m_ext ? m_ext[e] : 0.0);
+    const double an = Fq / m + P.g[k], aln = Mq / I;                                  // Eq. (18b), (19c)
+    if (!only_accel) {
+        v[e] = v[e] + (0.5 * P.dt) * (a[e] + an);                                     // Eq. (18c)
+        w[e] = w[e] + (0.5 * P.dt) * (alpha[e] + aln);                                // Eq. (19d)
     }
+    a[e] = an;
+    alpha[e] = aln;
 }
 
 // ------------------------------------------------------------------------------ query (parity only)
@@ -655,8 +666,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     s.tile_counter = take(4 * 4);
     s.tile_state = take((size_t)4 * h->tiles * SORT_RADIX * 4);
     // zeroed before every range build
-    s.cell_start = take((size_t)d.ncell * 4);
-    s.cell_end = take((size_t)d.ncell * 4);
+    s.cell_range = take((size_t)d.ncell * 8);
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
     s.xr = take(n * 32); s.xr_s = take(n * 32);
     s.vp = take(n * 24); s.wp = take(n * 24);
@@ -703,7 +713,7 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     // clear sort bookkeeping + cell ranges (one contiguous region)
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
     ledds_prof_start(LEDDS_K_DEM_KEYS, st);
-    dem_drift_key_kernel<<<nb, tb, 0, st>>>(d, x, v, w, a, alpha, radius, at<double>(scratch, s.vp),
+    dem_drift_key_kernel<<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(d, x, v, w, a, alpha, radius, at<double>(scratch, s.vp),
                                             at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
                                             at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
     ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
@@ -729,17 +739,25 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     const uint32_t* sidx = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
     ledds_prof_start(LEDDS_K_DEM_GATHER, st);
     dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr), at<double4>(scratch, s.xr_s),
-                                         at<uint32_t>(scratch, s.cell_start), at<uint32_t>(scratch, s.cell_end));
+                                         at<uint2>(scratch, s.cell_range));
     ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
     LEDDS_CHECK_LAUNCH();
     const DemHistory& hs = h->hs;
     const int prev = h->cur, nw = 1 - h->cur;
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
-    dem_contact_kernel<<<nb, CONTACT_BLOCK, (size_t)d.maxc * CONTACT_BLOCK * sizeof(uint32_t), st>>>(
+    {
+        const size_t smem = (size_t)d.maxc * CONTACT_BLOCK * sizeof(uint32_t);
+        if (d.bc[0] && d.bc[1] && d.bc[2]) dem_contact_kernel<false><<<nb, CONTACT_BLOCK, smem, st>>>(
         d, skey, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
-        at<uint32_t>(scratch, s.cell_start), at<uint32_t>(scratch, s.cell_end),
+        at<uint2>(scratch, s.cell_range),
         at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
         at<double>(history, hs.ft[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]), status, dt_hist);
+        else dem_contact_kernel<true><<<nb, CONTACT_BLOCK, smem, st>>>(
+        d, skey, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
+        at<uint2>(scratch, s.cell_range),
+        at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
+        at<double>(history, hs.ft[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]), status, dt_hist);
+    }
     ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
     LEDDS_CHECK_LAUNCH();
     h->cur = nw;
@@ -750,9 +768,9 @@ int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha,
                    const double* f_ext, const double* m_ext, const void* history, int32_t* status, cudaStream_t st)
 {
     (void)status;
-    const int n = h->d.n, tb = 128, nb = (n + tb - 1) / tb;
+    const int n = h->d.n;
     ledds_prof_start(LEDDS_K_DEM_KICK, st);
-    dem_kick_kernel<<<nb, tb, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), f_ext, m_ext, v, w, a, alpha, 0);
+    dem_kick_kernel<<<(unsigned)((3ll * n + 255) / 256), 256, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), f_ext, m_ext, v, w, a, alpha, 0);
     ledds_prof_stop(LEDDS_K_DEM_KICK, st);
     LEDDS_CHECK_LAUNCH();
     return LEDDS_OK;
@@ -778,9 +796,8 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
     // forces of the initial state: no drift, delta_t stays 0 (dt_hist = 0)
     rc = ledds_dem_advance_contacts(h, const_cast<double*>(x), v, w, a, alpha, radius, history, scratch, status, 0.0, false, st);
     if (rc) { delete h; return rc; }
-    const int tb = 128, nb = (h->d.n + tb - 1) / tb;
-    dem_kick_kernel<<<nb, tb, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), nullptr, nullptr, nullptr,
-                                       nullptr, a, alpha, 1);
+    dem_kick_kernel<<<(unsigned)((3ll * h->d.n + 255) / 256), 256, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), nullptr,
+                                                                            nullptr, nullptr, nullptr, a, alpha, 1);
     ledds_count_launch(1);
     if (cudaPeekAtLastError() != cudaSuccess) { delete h; return LEDDS_ECUDA; }
     *out = h;
