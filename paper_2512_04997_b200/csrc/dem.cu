@@ -20,7 +20,9 @@
 #define DEM_PI 3.14159265358979323846
 #define SORT_THREADS 256
 #define SORT_WARPS (SORT_THREADS / 32)
+#ifndef SORT_ITEMS
 #define SORT_ITEMS 16
+#endif
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define SORT_RADIX 256
 
