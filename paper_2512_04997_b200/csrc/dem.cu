@@ -384,37 +384,50 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
     const int c2 = (int)(key / ((uint32_t)P.nc[0] * (uint32_t)P.nc[1]));
 
     // ---- phase 1: detect
-    for (int dz = -1; dz <= 1; ++dz) {
-        int qz = c2 + dz;
-        if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) continue; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
-        for (int dy = -1; dy <= 1; ++dy) {
-            int qy = c1 + dy;
+    auto note = [&](uint32_t t) {
+        if (ncand < maxc) s_list[ncand * CONTACT_BLOCK + threadIdx.x] = t;
+        else st |= LEDDS_ST_CONTACT_OVERFLOW;
+        ncand += ncand < maxc;
+    };
+    // the 9 runs [t0, t1) of x-adjacent cells (c0-1 .. c0+1 inside the row): all 27 range loads are independent
+    // and issued together; an empty cell holds (0, 0), so "first start, last end" needs no special case
+    uint32_t t0[9], t1[9];
+#pragma unroll
+    for (int j = 0; j < 9; ++j) {
+        int qz = c2 + (j / 3 - 1), qy = c1 + (j % 3 - 1);
+        bool ok = true;
+        if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) ok = false; else qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
+        if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) ok = false; else qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
+        const uint2 none = make_uint2(0u, 0u);
+        uint2 r0 = none, r1 = none, r2 = none;
+        if (ok) {
+            const uint2* row = cell_range + (size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + c0;
+            r1 = row[0];
+            if (c0 > 0) r0 = row[-1];
+            if (c0 < P.nc[0] - 1) r2 = row[1];
+        }
+        const bool e0 = r0.y > r0.x, e1 = r1.y > r1.x, e2 = r2.y > r2.x;
+        t0[j] = e0 ? r0.x : (e1 ? r1.x : r2.x);
+        t1[j] = e2 ? r2.y : (e1 ? r1.y : r0.y);
+    }
+#pragma unroll
+    for (int j = 0; j < 9; ++j) {
+        for (uint32_t t = t0[j]; t < t1[j]; t += 2) {                              // two candidates in flight
+            const bool two = t + 1 < t1[j];
+            const double4 ca = xr_s[t], cb = xr_s[two ? t + 1 : t];
+            if ((int)t != s && dem_touch<PERIODIC>(P, mine, ca)) note(t);
+            if (two && (int)(t + 1) != s && dem_touch<PERIODIC>(P, mine, cb)) note(t + 1);
+        }
+    }
+    if (PERIODIC && !P.bc[0] && (c0 == 0 || c0 == P.nc[0] - 1)) {                  // the wrapped cell of a periodic row
+        const int wc = c0 == 0 ? P.nc[0] - 1 : 0;
+        for (int j = 0; j < 9; ++j) {
+            int qz = c2 + (j / 3 - 1), qy = c1 + (j % 3 - 1);
+            if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) continue; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
             if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) continue; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
-            const uint32_t rowc = (uint32_t)P.nc[0] * (uint32_t)(qy + P.nc[1] * qz);
-            // run 0: the cells c0-1 .. c0+1 that lie inside the row; run 1: the one wrapped cell of a periodic row
-            const int lo = max(c0 - 1, 0), hi = min(c0 + 1, P.nc[0] - 1);
-            const int wrapped = P.bc[0] ? -1 : (c0 == 0 ? P.nc[0] - 1 : (c0 == P.nc[0] - 1 ? 0 : -1));
-            for (int run = 0; run < 2; ++run) {
-                uint32_t t0 = 0, t1 = 0;
-                if (run == 0) {
-                    bool any = false;
-                    for (int c = lo; c <= hi; ++c) {
-                        const uint2 r = cell_range[rowc + c];
-                        if (r.y > r.x) { if (!any) t0 = r.x; t1 = r.y; any = true; }
-                    }
-                } else {
-                    if (wrapped < 0 || (wrapped >= lo && wrapped <= hi)) break;
-                    const uint2 r = cell_range[rowc + wrapped];
-                    t0 = r.x; t1 = r.y;
-                }
-                for (uint32_t t = t0; t < t1; ++t) {
-                    if ((int)t == s) continue;
-                    if (!dem_touch<PERIODIC>(P, mine, xr_s[t])) continue;
-                    if (ncand < maxc) s_list[ncand * CONTACT_BLOCK + threadIdx.x] = t;
-                    else st |= LEDDS_ST_CONTACT_OVERFLOW;
-                    ncand += ncand < maxc;
-                }
-            }
+            const uint2 r = cell_range[(size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + wc];
+            for (uint32_t t = r.x; t < r.y; ++t)
+                if ((int)t != s && dem_touch<PERIODIC>(P, mine, xr_s[t])) note(t);
         }
     }
 
