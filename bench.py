@@ -235,6 +235,41 @@ def run_ours(args, rank, world):
                                    "hbm_gbs": round(304.0 * nc2 / ms2 / 1e6, 1), "hbm_frac": round(304.0 * nc2 / ms2 / 1e6 / peak, 4),
                                    "note": "638 MB of populations (> 126 MB L2); 304 B/cell"}
         del gl
+        # configs[0] and configs[2]: small, launch-latency-bound workloads, timed plainly and replayed from a CUDA
+        # graph (the library only enqueues on the caller's stream, so its calls can be captured)
+        def graph_time(step_fn, per_graph, replays):
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                step_fn(per_graph)                                  # warm-up on the capture stream
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr):
+                step_fn(per_graph)
+            gr.replay(); torch.cuda.synchronize()
+            return timed(lambda k: [gr.replay() for _ in range(k)], replays) / (replays * per_graph)
+        pd1, x1, v1, w1, R1 = W.cfg1_gas()
+        g1 = Dem(pd1, x1, v1, w1, R1)
+        g1.step(50); torch.cuda.synchronize()
+        ms1 = timed(g1.step, 1000) / 1000
+        ms1g = graph_time(g1.step, 20, 50)
+        sub["cfg1_dem_gas_2048"] = {"steps_per_s": round(1e3 / ms1, 1), "particle_updates_per_s": round(len(R1) * 1e3 / ms1, 1),
+                                     "cuda_graph_steps_per_s": round(1e3 / ms1g, 1),
+                                     "cuda_graph_particle_updates_per_s": round(len(R1) * 1e3 / ms1g, 1),
+                                     "status_word": int(g1.status[0].item()), "note": "launch-latency bound: 7 launches + 1 memset per step"}
+        del g1
+        lb3, cp3, pd3, x3, v3, w3, R3 = W.cfg3_settling()
+        gl3 = Lbm(lb3); gd3 = Dem(pd3, x3, v3, w3, R3); g3 = Coupled(gl3, gd3, cp3, float(R3.max()))
+        g3.step(20); torch.cuda.synchronize()
+        ms3 = timed(g3.step, 500) / 500
+        ms3g = graph_time(g3.step, 20, 25)                          # an even number of steps per graph keeps the lattice parity
+        nc3 = int(np.prod(lb3["shape"]))
+        sub["cfg3_settling_64x64x256"] = {"coupled_steps_per_s": round(1e3 / ms3, 1), "mlups": round(nc3 / ms3 / 1e3, 1),
+                                           "cuda_graph_coupled_steps_per_s": round(1e3 / ms3g, 1),
+                                           "cuda_graph_mlups": round(nc3 / ms3g / 1e3, 1), "status_word": int(gd3.status[0].item()),
+                                           "note": "159 MB per lattice: close to L2 size, so MLUPS may exceed the HBM bound"}
+        del g3, gl3, gd3
         # configs[4]: DEM-only, 4 M polydisperse spheres (jittered-lattice placement), + supplementary dense state
         for name, dense in (("cfg5_dem_pour_4M", False), ("cfg5_dense_supplement_4M", True)):
             pd5, x5, v5, w5, R5 = W.cfg5_pour(n_side=160 if not small else 40, n_part=4_000_000 if not small else 64000, dense=dense)
