@@ -38,11 +38,11 @@ __global__ void cpl_solid_kernel(const CplDev C)
 }
 
 // thread t -> solid k = t / S^2, row (ly, lz) = t % S^2 of its box.
-// ROUND 0: slots[cell].x = min id over the solids cutting the cell (reductions without a return value: nothing
-//          waits on them).
-// ROUND 1: a solid that did not win a cell enters slots[cell].y the same way; the value found there tells a
-//          third solid apart (LEDDS_ST_SOLID_OVERFLOW).  Together: the two lowest ids.
-template <int ROUND>
+// Every cut cell gets slots[cell].x = min(x, k).  The value that was there tells who lost the cell: the
+// newcomer if a lower id was already in, else the id it displaced; the loser is entered into slots[cell].y
+// the same way.  Every solid but the lowest is a loser exactly once, so y ends as the second lowest id
+// whatever the order of arrival (the two lowest ids), and a second loser is a third solid
+// (LEDDS_ST_SOLID_OVERFLOW).  Only cells shared by two solids pay the second atomic.
 __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const CplDev C)
 {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -76,26 +76,20 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
     bool overflow = false;
     uint2* const row = C.slots + ((long long)rz * P.ny + ry) * P.nx;
     for (int x0 = xa; x0 <= xb; x0 += RASTER_BATCH) {
-        uint32_t first[RASTER_BATCH];
+        uint32_t was[RASTER_BATCH];
         int rxs[RASTER_BATCH];
 #pragma unroll
-        for (int b = 0; b < RASTER_BATCH; ++b) {                                   // independent accesses, issued together
+        for (int b = 0; b < RASTER_BATCH; ++b) {                                   // independent atomics, issued together
             int rx = x0 + b;
             bool ok = rx <= xb;
             if (P.bc[0]) ok = ok && rx >= 0 && rx < P.nx;
             else rx = rx < 0 ? rx + P.nx : (rx >= P.nx ? rx - P.nx : rx);
-            rxs[b] = ok ? rx : -1;
-            first[b] = (uint32_t)k;
-            if (ok) {
-                if (ROUND == 0) atomicMin(&row[rx].x, (uint32_t)k);
-                else first[b] = __ldcg(&row[rx].x);
-            }
+            rxs[b] = rx;
+            was[b] = ok ? atomicMin(&row[rx].x, (uint32_t)k) : PSM_EMPTY;
         }
-        if (ROUND == 1) {
 #pragma unroll
-            for (int b = 0; b < RASTER_BATCH; ++b)
-                if (first[b] != (uint32_t)k && atomicMin(&row[rxs[b]].y, (uint32_t)k) != PSM_EMPTY) overflow = true;
-        }
+        for (int b = 0; b < RASTER_BATCH; ++b)
+            if (was[b] != PSM_EMPTY && atomicMin(&row[rxs[b]].y, max(was[b], (uint32_t)k)) != PSM_EMPTY) overflow = true;
     }
     if (overflow) atomicOr(C.status, LEDDS_ST_SOLID_OVERFLOW);
 }
@@ -316,9 +310,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         ledds_prof_start(LEDDS_K_CPL_RASTER, st);
         cpl_solid_kernel<<<(C.n + 127) / 128, 128, 0, st>>>(C);
         ledds_count_launch(1);
-        cpl_raster_kernel<0><<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
-        cpl_raster_kernel<1><<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
-        ledds_count_launch(1);
+        cpl_raster_kernel<<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
         ledds_prof_stop(LEDDS_K_CPL_RASTER, st);
         LEDDS_CHECK_LAUNCH();
         dim3 block(PSM_BLOCK), grid((d.nx + PSM_BLOCK - 1) / PSM_BLOCK, d.ny, d.nz);
