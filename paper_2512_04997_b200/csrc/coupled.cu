@@ -9,10 +9,10 @@
 //                      the plain BGK path; otherwise all its lanes run the PSM collision Eq. (32)-(37) (B = 0
 //                      where there is no solid; the rarer second solid of a cell is parked in shared memory),
 //                      stream with boundaries, and the (cell, solid) terms of Eq. (41)-(42) are summed over
-//                      runs of consecutive lanes by warp shuffles in a fixed order; the first lane of a run
-//                      stores one partial.
-//   cpl_reduce_kernel  one warp per solid: fixed-order sum of its partials -> F_sf, M_sf.  No floating point
-//                      atomics and no sort over N_fluid (as PAPER.md:525-530 needs).
+//                      runs of consecutive lanes by warp shuffles; the first lane of a run adds the sum to the
+//                      solid's 2^-83 fixed-point accumulators with integer reductions.
+//   cpl_finish_kernel  fixed point -> F_sf, M_sf.  No floating point atomics and no sort over N_fluid (as
+//                      PAPER.md:525-530 needs); the integer sums are exact and order-independent.
 #include <math.h>
 
 #include "psm_kernels.cuh"
@@ -95,110 +95,86 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
 }
 
 // ------------------------------------------------------------------------------------ collide + stream
-// One cell: f = its 19 pre-collision populations, (id0, id1) = its slot.  Collides (BGK or PSM), streams, and
-// takes part in the warp's run reductions.  All 32 lanes of a warp call this together.
-template <typename I>
-__device__ __forceinline__ void psm_cell_step(double (&f)[LEDDS_Q], uint32_t id0, uint32_t id1, bool active, I cell, int x,
-                                              int y, int z, double* __restrict__ fout, const LbmDev& P, const CplDev& C,
-                                              double* s2col)
-{
-    double rho, ux, uy, uz;
-    lb_moments(f, rho, ux, uy, uz);
-    if (!__any_sync(0xffffffffu, id0 != PSM_EMPTY)) {
-        lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
-    } else {
-        if (id0 != PSM_EMPTY) C.slots[cell] = make_uint2(PSM_EMPTY, PSM_EMPTY);       // consumed: free for the next step
-        const bool two = __any_sync(0xffffffffu, id1 != PSM_EMPTY);
-        if (two) {                                                                    // warp-uniform, rarer
-            double B1, uk1[3], rec[6];
-            int ent;
-            psm_solid_terms(P, C, x, y, z, id1, rho, ux, uy, uz, B1, uk1, rec, ent);
-            s2col[0] = B1;
-            s2col[PSM_BLOCK] = 1.0 - 1.5 * (uk1[0] * uk1[0] + uk1[1] * uk1[1] + uk1[2] * uk1[2]);
-            s2col[2 * PSM_BLOCK] = uk1[0]; s2col[3 * PSM_BLOCK] = uk1[1]; s2col[4 * PSM_BLOCK] = uk1[2];
-            psm_run_reduce(C, id1, ent, rec);
-        }
-        double B0, uk0[3], rec[6];
-        int ent;
-        psm_solid_terms(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
-        psm_run_reduce(C, id0, ent, rec);
-        psm_collide(f, P.omega, rho, ux, uy, uz, B0, uk0, two, s2col);
-    }
-    if (active) lb_push_store<I>(fout, P, x, y, z, f, rho);
-}
-
-// One block per 128-cell row segment, populations loaded straight into registers.
+// One block per 128-cell row segment.  The 19 populations of a cell go from global memory straight into the
+// thread's column of shared memory with asynchronous copies (no registers tied up while they are in flight);
+// the moments are summed from there and the collision runs pair by pair, each pair pushed as soon as it is
+// collided.  The kernel needs <= 64 registers, so 8 blocks (32 warps) are resident per SM.
 template <typename I>
 __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                                const __grid_constant__ LbmDev P,
                                                                const __grid_constant__ CplDev C)
 {
+    __shared__ double sfull[LEDDS_Q][PSM_BLOCK];
     __shared__ double s2[PSM_S2_ROWS][PSM_BLOCK];
     const int x = blockIdx.x * PSM_BLOCK + threadIdx.x, y = blockIdx.y, z = blockIdx.z;
     const bool active = x < P.nx;
     const I cell = ((I)z * (I)P.ny + (I)y) * (I)P.nx + (I)(active ? x : 0);    // a lane past the row reads cell 0, stores nothing
-    double f[LEDDS_Q];
-    lb_load<I>(fin, (I)P.N, cell, f);
+    double* sf = &sfull[0][threadIdx.x];
+    {
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(sf);
+#pragma unroll
+        for (int q = 0; q < LEDDS_Q; ++q)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + (uint32_t)(q * PSM_BLOCK * sizeof(double))),
+                         "l"(fin + (I)((I)q * (I)P.N + cell))
+                         : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    }
     uint32_t id0 = PSM_EMPTY, id1 = PSM_EMPTY;
     if (active) {
         const uint2 slot = C.slots[cell];
         id0 = slot.x; id1 = slot.y;
     }
-    psm_cell_step<I>(f, id0, id1, active, cell, x, y, z, fout, P, C, &s2[0][threadIdx.x]);
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    double rho, ux, uy, uz;
+    {
+        double f[LEDDS_Q];
+#pragma unroll
+        for (int q = 0; q < LEDDS_Q; ++q) f[q] = sf[q * PSM_BLOCK];
+        lb_moments(f, rho, ux, uy, uz);
+    }
+    const LbPush<I> push(P, x, y, z);
+    if (!__any_sync(0xffffffffu, id0 != PSM_EMPTY)) {
+        bgk_collide_stream<I>(sf, P.omega, rho, ux, uy, uz, push, fout, P, active);
+        return;
+    }
+    if (id0 != PSM_EMPTY) C.slots[cell] = make_uint2(PSM_EMPTY, PSM_EMPTY);           // consumed: free for the next step
+    const bool two = __any_sync(0xffffffffu, id1 != PSM_EMPTY);
+    double* s2col = &s2[0][threadIdx.x];
+    if (two) {                                                                        // warp-uniform, rarer
+        double B1, uk1[3], rec[6];
+        int ent;
+        psm_solid_terms(P, C, x, y, z, id1, rho, ux, uy, uz, B1, uk1, rec, ent);
+        s2col[0] = B1;
+        s2col[PSM_BLOCK] = 1.0 - 1.5 * (uk1[0] * uk1[0] + uk1[1] * uk1[1] + uk1[2] * uk1[2]);
+        s2col[2 * PSM_BLOCK] = uk1[0]; s2col[3 * PSM_BLOCK] = uk1[1]; s2col[4 * PSM_BLOCK] = uk1[2];
+        psm_run_reduce(C, id1, ent, rec);
+    }
+    double B0, uk0[3];
+    {
+        double rec[6];
+        int ent;
+        psm_solid_terms(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
+        psm_run_reduce(C, id0, ent, rec);
+    }
+    psm_collide_stream<I>(sf, P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
 }
 
-// ------------------------------------------------------------------------------------ reduce
-// One warp per solid; lane -> entry map and the shuffle tree are fixed, so the sums are deterministic.
-// A lane takes one word of 32 flags at a time and reads the flagged partials, four at a time.
-__global__ void __launch_bounds__(128) cpl_reduce_kernel(const CplDev C, double* __restrict__ f_hyd,
-                                                         double* __restrict__ m_hyd)
+// ------------------------------------------------------------------------------------ finish
+// One thread per (solid, component): fixed point -> double, lattice -> DEM units, accumulator reset.
+__global__ void cpl_finish_kernel(const CplDev C, double* __restrict__ f_hyd, double* __restrict__ m_hyd)
 {
-    const int k = (int)((blockIdx.x * (unsigned)blockDim.x + threadIdx.x) >> 5);
-    const int lane = threadIdx.x & 31;
-    if (k >= C.n) return;
-    uint32_t* fl = C.flags + (size_t)k * C.W;
-    const double2* box = reinterpret_cast<const double2*>(C.box + (size_t)k * (size_t)(C.S * C.S * C.S) * 8);
-    double acc[6] = {0, 0, 0, 0, 0, 0};
-    const double2 zero = make_double2(0.0, 0.0);
-    for (int w = lane; w < C.W; w += 32) {
-        uint32_t m = fl[w];
-        if (!m) continue;
-        fl[w] = 0u;
-        while (m) {
-            double2 a[4][3];
-#pragma unroll
-            for (int b = 0; b < 4; ++b) {                                         // ascending bit order: fixed
-                const bool on = m != 0u;
-                const int bit = on ? __ffs(m) - 1 : 0;
-                m &= m - 1u;
-                const double2* in = box + (size_t)(32 * w + bit) * 4;
-                a[b][0] = on ? in[0] : zero; a[b][1] = on ? in[1] : zero; a[b][2] = on ? in[2] : zero;
-            }
-#pragma unroll
-            for (int b = 0; b < 4; ++b) {
-                acc[0] += a[b][0].x; acc[1] += a[b][0].y; acc[2] += a[b][1].x;
-                acc[3] += a[b][1].y; acc[4] += a[b][2].x; acc[5] += a[b][2].y;
-            }
-        }
-    }
-#pragma unroll
-    for (int c = 0; c < 6; ++c) {
-        double v = acc[c];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-        acc[c] = v;
-    }
-    if (lane == 0) {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            f_hyd[3 * k + c] = acc[c] * C.fscale;
-            m_hyd[3 * k + c] = acc[3 + c] * C.mscale;
-        }
-    }
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= 6 * C.n) return;
+    const int k = t / 6, c = t - 6 * k;
+    unsigned long long* a = C.acc + (size_t)t * 2;
+    const double v = (double)(long long)a[0] * (1.0 / PSM_FIX_HI) + (double)(long long)a[1] * (1.0 / PSM_FIX_HI / PSM_FIX_LO);
+    a[0] = 0ull; a[1] = 0ull;
+    if (c < 3) f_hyd[3 * k + c] = v * C.fscale;
+    else m_hyd[3 * k + c - 3] = v * C.mscale;
 }
 
 // ------------------------------------------------------------------------------------ host API
-struct CplLayout { size_t slots, sol, flags, box, total; };
+struct CplLayout { size_t slots, sol, acc, total; };
 
 static size_t cpl_align(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -226,13 +202,11 @@ static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl
         if (dem->d.bc[a] != lbm->d.bc[a]) return LEDDS_EINVAL;              // same topology on both grids
         if (!lbm->d.bc[a] && nl[a] < 2 * C->S) return LEDDS_EINVAL;         // unambiguous nearest image (G33)
     }
-    const size_t N = (size_t)lbm->d.N, S3 = (size_t)C->S * C->S * C->S, E = (size_t)C->n * S3;   // S even: S3 % 8 == 0
+    const size_t N = (size_t)lbm->d.N;
     L->slots = 0;
     L->sol = cpl_align(N * sizeof(uint2));
-    L->flags = L->sol + cpl_align((size_t)C->n * 10 * sizeof(double));
-    C->W = (int)((S3 + 31) / 32);
-    L->box = L->flags + cpl_align((size_t)C->n * C->W * sizeof(uint32_t));
-    L->total = L->box + cpl_align(E * 8 * sizeof(double));
+    L->acc = L->sol + cpl_align((size_t)C->n * 10 * sizeof(double));
+    L->total = L->acc + cpl_align((size_t)C->n * 12 * sizeof(unsigned long long));
     return LEDDS_OK;
 }
 
@@ -260,7 +234,7 @@ extern "C" int ledds_cpl_init(const ledds_lbm* lbm, const ledds_dem* dem, const 
     cudaStream_t st = (cudaStream_t)stream;
     char* base = static_cast<char*>(cpl_scratch);
     if (cudaMemsetAsync(base + L.slots, 0xff, L.sol - L.slots, st) != cudaSuccess ||        // all slots PSM_EMPTY
-        cudaMemsetAsync(base + L.flags, 0, L.box - L.flags, st) != cudaSuccess)             // no partial pending
+        cudaMemsetAsync(base + L.acc, 0, L.total - L.acc, st) != cudaSuccess)               // accumulators at zero
         return LEDDS_ECUDA;
     return LEDDS_OK;
 }
@@ -290,13 +264,11 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
     C.radius = radius;
     C.slots = reinterpret_cast<uint2*>(cs + L.slots);
     C.sol = reinterpret_cast<double*>(cs + L.sol);
-    C.flags = reinterpret_cast<uint32_t*>(cs + L.flags);
-    C.box = reinterpret_cast<double*>(cs + L.box);
+    C.acc = reinterpret_cast<unsigned long long*>(cs + L.acc);
     C.status = status;
     const LbmDev& d = lbm->d;
     const size_t half = (size_t)LEDDS_Q * d.N;
     if (d.ny > 65535 || d.nz > 65535) return LEDDS_EINVAL;
-    const unsigned warp_blocks = (unsigned)(((long long)C.n * 32 + 127) / 128);
     for (int step = 0; step < nsteps; ++step) {
         for (int sub = 0; sub < c->n_sub; ++sub) {
             rc = ledds_dem_advance_contacts(dem, x, v, w, a, alpha, radius, history, scratch, status, dem->d.dt, true, st);
@@ -322,7 +294,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         lbm->parity ^= 1;
         lbm->steps++;
         ledds_prof_start(LEDDS_K_CPL_REDUCE, st);
-        cpl_reduce_kernel<<<warp_blocks, 128, 0, st>>>(C, f_hyd, m_hyd);
+        cpl_finish_kernel<<<(6 * C.n + 127) / 128, 128, 0, st>>>(C, f_hyd, m_hyd);
         ledds_prof_stop(LEDDS_K_CPL_REDUCE, st);
         LEDDS_CHECK_LAUNCH();
         rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);

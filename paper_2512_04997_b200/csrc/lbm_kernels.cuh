@@ -89,46 +89,61 @@ __device__ __forceinline__ void lb_load(const double* __restrict__ fin, I N, I c
     for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (I)((I)q * N + cell));
 }
 
-// Eq. (25) as a push of all 19 post-collision populations of cell (x,y,z), with boundaries.
+// Eq. (25) as a push of the post-collision populations of cell (x,y,z), with boundaries.
 // The neighbour coordinates and "this link leaves through a wall" flags are worked out once per axis and
 // the nine row offsets once per block (y and z are uniform over the block), so a direction costs a
 // predicate, an index and a store.
 template <typename I>
-__device__ __forceinline__ void lb_push_store(double* __restrict__ fout, const LbmDev& P, int x, int y, int z,
-                                              const double (&fs)[LEDDS_Q], double rho)
-{
-    // t?[0] / t?[2]: target coordinate for c = -1 / +1; w?[0] / w?[1]: link crosses the low / high wall
-    int tx[3] = {x - 1, x, x + 1}, ty[3] = {y - 1, y, y + 1}, tz[3] = {z - 1, z, z + 1};
-    bool wx[2] = {false, false}, wy[2] = {false, false}, wz[2] = {false, false};
-    if (x == 0) { if (P.bc[0]) wx[0] = true; else tx[0] = P.nx - 1; }
-    if (x == P.nx - 1) { if (P.bc[0]) wx[1] = true; else tx[2] = 0; }
-    if (y == 0) { if (P.bc[1]) wy[0] = true; else ty[0] = P.ny - 1; }
-    if (y == P.ny - 1) { if (P.bc[1]) wy[1] = true; else ty[2] = 0; }
-    if (z == 0) { if (P.bc[2]) wz[0] = true; else tz[0] = P.nz - 1; }
-    if (z == P.nz - 1) { if (P.bc[2]) wz[1] = true; else tz[2] = 0; }
-    const I N = (I)P.N;
-    I rb[3][3];                                                   // row offsets [cz + 1][cy + 1]
+struct LbPush {
+    int x, tx[3];                 // tx[0] / tx[2]: target x for c_x = -1 / +1
+    bool wx[2], wy[2], wz[2];     // link crosses the low / high wall of the axis
+    I N, rb[3][3];                // row offsets [c_z + 1][c_y + 1]
+
+    __device__ __forceinline__ LbPush(const LbmDev& P, int x_, int y, int z) : x(x_), N((I)P.N)
+    {
+        int ty[3] = {y - 1, y, y + 1}, tz[3] = {z - 1, z, z + 1};
+        tx[0] = x - 1; tx[1] = x; tx[2] = x + 1;
+        wx[0] = wx[1] = wy[0] = wy[1] = wz[0] = wz[1] = false;
+        if (x == 0) { if (P.bc[0]) wx[0] = true; else tx[0] = P.nx - 1; }
+        if (x == P.nx - 1) { if (P.bc[0]) wx[1] = true; else tx[2] = 0; }
+        if (y == 0) { if (P.bc[1]) wy[0] = true; else ty[0] = P.ny - 1; }
+        if (y == P.ny - 1) { if (P.bc[1]) wy[1] = true; else ty[2] = 0; }
+        if (z == 0) { if (P.bc[2]) wz[0] = true; else tz[0] = P.nz - 1; }
+        if (z == P.nz - 1) { if (P.bc[2]) wz[1] = true; else tz[2] = 0; }
 #pragma unroll
-    for (int a = 0; a < 3; ++a)
+        for (int a = 0; a < 3; ++a)
 #pragma unroll
-        for (int b = 0; b < 3; ++b) rb[a][b] = ((I)tz[a] * (I)P.ny + (I)ty[b]) * (I)P.nx;
-#pragma unroll
-    for (int q = 0; q < LEDDS_Q; ++q) {
+            for (int b = 0; b < 3; ++b) rb[a][b] = ((I)tz[a] * (I)P.ny + (I)ty[b]) * (I)P.nx;
+    }
+
+    // post-collision population v of direction q (a compile-time constant after unrolling); rho = the cell's
+    // pre-collision density (moving-wall term, G19)
+    __device__ __forceinline__ void put(double* __restrict__ fout, const LbmDev& P, int q, double v, double rho) const
+    {
         const int cx = lb_cx(q), cy = lb_cy(q), cz = lb_cz(q);
         bool bounced = false;
         if (cx != 0) bounced = bounced || wx[cx > 0];
         if (cy != 0) bounced = bounced || wy[cy > 0];
         if (cz != 0) bounced = bounced || wz[cz > 0];
         if (!bounced) {
-            fout[(I)((I)q * N + rb[cz + 1][cy + 1] + (I)tx[cx + 1])] = fs[q];
+            fout[(I)((I)q * N + rb[cz + 1][cy + 1] + (I)tx[cx + 1])] = v;
         } else {
-            double cuw = 0.0;                                   // c_q . u_wall summed over the crossed walls (G19)
+            double cuw = 0.0;                                   // c_q . u_wall summed over the crossed walls
             if (P.any_wall_velocity) {
                 if (cx != 0 && wx[cx > 0]) { const double* uw = P.uw + (0 + (cx > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
                 if (cy != 0 && wy[cy > 0]) { const double* uw = P.uw + (2 + (cy > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
                 if (cz != 0 && wz[cz > 0]) { const double* uw = P.uw + (4 + (cz > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
             }
-            fout[(I)((I)lb_opp(q) * N + rb[1][1] + (I)x)] = fs[q] - 6.0 * lb_w(q) * rho * cuw;
+            fout[(I)((I)lb_opp(q) * N + rb[1][1] + (I)x)] = v - 6.0 * lb_w(q) * rho * cuw;
         }
     }
+};
+
+template <typename I>
+__device__ __forceinline__ void lb_push_store(double* __restrict__ fout, const LbmDev& P, int x, int y, int z,
+                                              const double (&fs)[LEDDS_Q], double rho)
+{
+    const LbPush<I> push(P, x, y, z);
+#pragma unroll
+    for (int q = 0; q < LEDDS_Q; ++q) push.put(fout, P, q, fs[q], rho);
 }

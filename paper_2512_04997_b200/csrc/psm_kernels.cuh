@@ -13,22 +13,20 @@
 //                       when free.  Written by cpl_raster_kernel, consumed and reset by lbm_psm_kernel,
 //                       so it is all-empty between steps.
 //   sol[n][10]          per solid, lattice units: x_k[3], R_k, v_k[3], w_k[3] (predictor values)
-//   flags[n][W]         uint32 bit sets, W = ceil(S^3 / 32): box entry holds a partial of this step (bit set
-//                       by lbm_psm_kernel with a reduction, word reset by cpl_reduce_kernel)
-//   box[n][S^3][8]      double (6 used; 64-byte entries = one DRAM access each): sum of the (cell, solid) terms of Eq. (41)-(42) over one run of
-//                       consecutive cells of a lattice row inside a warp, stored at the run's first cell;
-//                       S = 2H+2 cells per axis around floor(x_k)
+//   acc[n][6][2]        uint64: per solid and component of (F, M), the exact sum of the (cell, solid) terms of
+//                       Eq. (41)-(42) in 2^-83 fixed point (two limbs: units of 2^-30 and of 2^-83).  Integer
+//                       additions commute, so the sum does not depend on the order in which blocks finish;
+//                       cpl_finish_kernel converts and resets it.
 struct CplDev {
     int n;
     double rc, inv_2rc;        // Eq. (40) in lattice units
     double inv_dx, vscale, wscale, origin[3];
     double fscale, mscale;     // lattice -> DEM units for force / torque
-    int H, S, W;               // box half-width, box width, flag words per solid
+    int H, S;                  // half-width and width of the solid's bounding box in cells (raster)
     const double* x; const double* vp; const double* wp; const double* radius;   // particle order, DEM units
     uint2* slots;
     double* sol;
-    uint32_t* flags;
-    double* box;
+    unsigned long long* acc;
     int32_t* status;
 };
 
@@ -146,10 +144,14 @@ __device__ __forceinline__ void psm_collide(double (&f)[LEDDS_Q], double omega, 
 }
 
 // Sum the records of each run of consecutive lanes that hold the same solid id (a solid cuts a lattice row
-// in consecutive cells) with a fixed shuffle tree, and let the first lane of the run write the sum into the
-// solid's box at its own cell.  All 32 lanes call this; id = PSM_EMPTY marks a lane without a record.
+// in consecutive cells) with a shuffle tree, and let the first lane of the run add the sum to the solid's
+// fixed-point accumulators (12 integer reductions, no return value).  All 32 lanes call this; id = PSM_EMPTY
+// marks a lane without a record.  ent is unused here (kept for the callers' bookkeeping).
+#define PSM_FIX_HI 1073741824.0                /* 2^30 */
+#define PSM_FIX_LO 9007199254740992.0          /* 2^53 */
 __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int ent, double (&v)[6])
 {
+    (void)ent;
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const uint32_t prev = __shfl_up_sync(full, id, 1);
@@ -167,11 +169,85 @@ __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int
         }
     }
     if (id != PSM_EMPTY && ((starts >> lane) & 1u)) {
-        const size_t e = (size_t)id * (size_t)(C.S * C.S * C.S) + (size_t)ent;
-        double2* out = reinterpret_cast<double2*>(C.box + e * 8);
-        out[0] = make_double2(v[0], v[1]);
-        out[1] = make_double2(v[2], v[3]);
-        out[2] = make_double2(v[4], v[5]);
-        atomicOr(C.flags + (size_t)id * C.W + (ent >> 5), 1u << (ent & 31));
+        unsigned long long* a = C.acc + (size_t)id * 12;
+        bool finite = true;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) finite = finite && fabs(v[c]) < 4.0e9;
+        if (!finite) { atomicOr(C.status, LEDDS_ST_NONFINITE); return; }
+#pragma unroll
+        for (int c = 0; c < 6; ++c) {
+            const double s = v[c] * PSM_FIX_HI, h = rint(s), l = rint((s - h) * PSM_FIX_LO);   // s - h is exact
+            atomicAdd(a + 2 * c, (unsigned long long)(long long)h);
+            atomicAdd(a + 2 * c + 1, (unsigned long long)(long long)l);
+        }
+    }
+}
+
+// ---- streaming forms: the populations of the cell sit in shared memory (column `sf`, stride PSM_BLOCK), are
+// collided pair by pair and pushed right away, so that only one pair is live in registers at a time.
+
+// BGK, same expressions as lb_collide_bgk / lb_equilibrium
+template <typename I>
+__device__ __forceinline__ void bgk_collide_stream(const double* sf, double omega, double rho, double ux, double uy, double uz,
+                                                   const LbPush<I>& push, double* __restrict__ fout, const LbmDev& P, bool active)
+{
+    const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
+    {
+        const double f0 = sf[0], fe = lb_w(0) * rho * k;
+        if (active) push.put(fout, P, 0, f0 - omega * (f0 - fe), rho);
+    }
+#pragma unroll
+    for (int q = 1; q < LEDDS_Q; q += 2) {
+        const double a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
+        const double cu = lb_cdot(q, ux, uy, uz);
+        const double wr = lb_w(q) * rho;
+        const double even = wr * (k + 4.5 * cu * cu), odd = wr * 3.0 * cu;
+        const double fa = even + odd, fb = even - odd;
+        if (active) {
+            push.put(fout, P, q, a - omega * (a - fa), rho);
+            push.put(fout, P, q + 1, b - omega * (b - fb), rho);
+        }
+    }
+}
+
+// PSM, same expressions as psm_collide
+template <typename I>
+__device__ __forceinline__ void psm_collide_stream(const double* sf, double omega, double rho, double ux, double uy, double uz,
+                                                   double B0, const double (&uk0)[3], bool two, const double* s2,
+                                                   const LbPush<I>& push, double* __restrict__ fout, const LbmDev& P, bool active)
+{
+    const double k0 = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
+    const double kk0 = 1.0 - 1.5 * (uk0[0] * uk0[0] + uk0[1] * uk0[1] + uk0[2] * uk0[2]);
+    const double Bsum = B0 + (two ? s2[0] : 0.0);
+    const double keep = 1.0 - (Bsum < 1.0 ? Bsum : 1.0);                              // 1 - B_tot, Eq. (37)
+    const double komega = keep * omega;
+    {   // rest population: its own opposite, Omega^s = feq(rho,u_k) - feq(rho,u)
+        const double f0 = sf[0], wr = lb_w(0) * rho, fe = wr * k0;
+        double acc = B0 * (wr * kk0 - fe);
+        if (two) acc += s2[0] * (wr * s2[PSM_BLOCK] - fe);
+        if (active) push.put(fout, P, 0, f0 + (acc - komega * (f0 - fe)), rho);
+    }
+#pragma unroll
+    for (int q = 1; q < LEDDS_Q; q += 2) {
+        const double a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
+        const double wr = lb_w(q) * rho;
+        const double cu = lb_cdot(q, ux, uy, uz);
+        const double ev = wr * (k0 + 4.5 * cu * cu), od = wr * 3.0 * cu;
+        const double nq = a - (ev + od), no = b - (ev - od);                            // f - feq(rho,u), Eq. (28)
+        const double cuk = lb_cdot(q, uk0[0], uk0[1], uk0[2]);
+        const double evk = wr * (kk0 + 4.5 * cuk * cuk), odk = wr * 3.0 * cuk;
+        double acc_q = B0 * (no - (a - (evk + odk)));                                   // B Omega^s, Eq. (34), direction q
+        double acc_o = B0 * (nq - (b - (evk - odk)));                                   //                      its opposite
+        if (two) {
+            const double B1 = s2[0], kk1 = s2[PSM_BLOCK];
+            const double cu1 = lb_cdot(q, s2[2 * PSM_BLOCK], s2[3 * PSM_BLOCK], s2[4 * PSM_BLOCK]);
+            const double ev1 = wr * (kk1 + 4.5 * cu1 * cu1), od1 = wr * 3.0 * cu1;
+            acc_q += B1 * (no - (a - (ev1 + od1)));
+            acc_o += B1 * (nq - (b - (ev1 - od1)));
+        }
+        if (active) {
+            push.put(fout, P, q, a + (acc_q - komega * nq), rho);                       // Eq. (32)-(33)
+            push.put(fout, P, q + 1, b + (acc_o - komega * no), rho);
+        }
     }
 }
