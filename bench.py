@@ -79,7 +79,7 @@ def make_cfg4(small=False):
 
 # ncu --set full capture of one lbm_psm_kernel launch at configs[3] (profiles/r1_ncu_summary.md):
 # dram__bytes_read.sum + dram__bytes_write.sum
-PSM_KERNEL_DRAM_BYTES = 5.448e9
+PSM_KERNEL_DRAM_BYTES = 5.283e9
 
 
 def coupled_bytes_per_step(n_cells):

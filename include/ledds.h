@@ -150,12 +150,13 @@ typedef struct {
     double origin[3];     /* DEM coordinates of lattice node (0,0,0)                              */
 } ledds_cpl_params;
 
-/* Size of the coupling scratch: one uint32 pair per fluid cell (the solids cutting it) + per solid
- * (2H+2)^2 row partials of Eq. (41)-(42), H = ceil(r_max/dx + 0.6204).  r_max = largest radius. */
+/* Size of the coupling scratch: one uint32 pair per fluid cell (the solids cutting it), 80 B per solid
+ * (its state in lattice units) and 96 B per solid (fixed-point accumulators of Eq. (41)-(42)).
+ * r_max = largest radius. */
 int ledds_cpl_workspace_bytes(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_params* c,
                               const double r_max, size_t* cpl_scratch_bytes);
 
-/* Prepares cpl_scratch (all cell slots empty, no row partial current).  Call once before the first
+/* Prepares cpl_scratch (all cell slots empty, accumulators at zero).  Call once before the first
  * ledds_coupled_step on this scratch, with the same lbm / dem / c / r_max. */
 int ledds_cpl_init(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_params* c, double r_max,
                    void* cpl_scratch, void* stream);
@@ -163,7 +164,8 @@ int ledds_cpl_init(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_p
 /* nsteps coupled steps.  f_hyd / m_hyd [n][3]: in = hydrodynamic force / torque of the previous
  * LBM step (zeros before the first), out = those of this step (DEM units).  The lattice and the DEM
  * box must have the same topology (bc); a periodic lattice axis must be at least 2 (2H+2) long
- * (unique nearest image); 2H+2 <= 128.  LEDDS_EINVAL otherwise. */
+ * (unique nearest image), H = ceil(r_max/dx + 0.6204).  LEDDS_EINVAL otherwise.  f_hyd / m_hyd are exact
+ * sums (2^-83 fixed point) of the per-cell terms, so they do not depend on the order of execution. */
 int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c, double r_max, double* f,
                        double* x, double* v, double* w, double* a, double* alpha, const double* radius,
                        double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
@@ -178,7 +180,7 @@ int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c
 #define LEDDS_K_DEM_GATHER 3   /* sorted copies + cell ranges   */
 #define LEDDS_K_DEM_CONTACT 4  /* contact detection + forces    */
 #define LEDDS_K_DEM_KICK 5     /* velocity update               */
-#define LEDDS_K_CPL_REDUCE 6   /* per-particle hydrodynamic sum */
+#define LEDDS_K_CPL_REDUCE 6   /* fixed point -> F_sf, M_sf      */
 #define LEDDS_K_CPL_RASTER 7   /* solids -> per-cell slots      */
 /* enable != 0: start recording (previous records are dropped); 0: stop and drop. */
 int ledds_profile(int enable);
