@@ -99,7 +99,8 @@ int ledds_lbm_destroy(ledds_lbm* h);
  * A wall is a static infinite particle with a surface velocity; its partner id
  * is n + 2*axis + side. */
 typedef struct {
-    int n;                         /* particles                                                  */
+    int n;                         /* particles, >= 0 (n = 0: every DEM call is a no-op and the
+                                      array arguments may be NULL)                               */
     double lo[3], hi[3];           /* box                                                        */
     int bc[3];                     /* 0 periodic, 1 planar walls at lo/hi                        */
     double v_wall[3][2][3];        /* wall surface velocity [axis][side][component]              */

@@ -244,9 +244,9 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
                                   double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
                                   int32_t* status, int nsteps, void* stream)
 {
-    if (!f || !x || !v || !w || !a || !alpha || !radius || !f_hyd || !m_hyd || !history || !scratch || !cpl_scratch ||
-        !status || nsteps < 0)
-        return LEDDS_EINVAL;
+    if (!lbm || !dem || !f || !cpl_scratch || !status || nsteps < 0) return LEDDS_EINVAL;
+    if (dem->d.n != 0 && (!x || !v || !w || !a || !alpha || !radius || !f_hyd || !m_hyd || !history || !scratch))
+        return LEDDS_EINVAL;                                                 // an empty particle system needs none of them
     const void* ptrs[] = {f, x, v, w, a, alpha, radius, f_hyd, m_hyd, history, scratch, cpl_scratch, status};
     for (const void* q : ptrs)
         if (!ledds_aligned16(q)) return LEDDS_EALIGN;
@@ -280,9 +280,11 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
             }
         }
         ledds_prof_start(LEDDS_K_CPL_RASTER, st);
-        cpl_solid_kernel<<<(C.n + 127) / 128, 128, 0, st>>>(C);
-        ledds_count_launch(1);
-        cpl_raster_kernel<<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
+        if (C.n > 0) {
+            cpl_solid_kernel<<<(C.n + 127) / 128, 128, 0, st>>>(C);
+            ledds_count_launch(1);
+            cpl_raster_kernel<<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
+        }
         ledds_prof_stop(LEDDS_K_CPL_RASTER, st);
         LEDDS_CHECK_LAUNCH();
         dim3 block(PSM_BLOCK), grid((d.nx + PSM_BLOCK - 1) / PSM_BLOCK, d.ny, d.nz);
@@ -294,7 +296,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         lbm->parity ^= 1;
         lbm->steps++;
         ledds_prof_start(LEDDS_K_CPL_REDUCE, st);
-        cpl_finish_kernel<<<(6 * C.n + 127) / 128, 128, 0, st>>>(C, f_hyd, m_hyd);
+        if (C.n > 0) cpl_finish_kernel<<<(6 * C.n + 127) / 128, 128, 0, st>>>(C, f_hyd, m_hyd);
         ledds_prof_stop(LEDDS_K_CPL_REDUCE, st);
         LEDDS_CHECK_LAUNCH();
         rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);

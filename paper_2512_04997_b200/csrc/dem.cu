@@ -639,7 +639,7 @@ static double dem_zeta_host(double eps)
 
 static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
 {
-    if (!p || p->n < 1 || p->max_contacts < 1 || p->max_contacts > 32) return LEDDS_EINVAL;
+    if (!p || p->n < 0 || p->max_contacts < 1 || p->max_contacts > 32) return LEDDS_EINVAL;   // n = 0: a valid, empty system
     if (!(p->cell > 0.0) || !(p->dt >= 0.0) || !(p->density > 0.0)) return LEDDS_EINVAL;
     if (!(p->kn > 0.0) || !(p->kt > 0.0) || !(p->kn_w > 0.0) || !(p->kt_w > 0.0)) return LEDDS_EINVAL;
     if (!(p->restitution > 0.0) || !(p->restitution_w > 0.0) || p->mu < 0.0 || p->mu_w < 0.0) return LEDDS_EINVAL;
@@ -725,6 +725,7 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     const DemDev& d = h->d;
     const DemScratch& s = h->s;
     const int n = d.n, tb = 128, nb = (n + tb - 1) / tb;
+    if (n == 0) { h->cur = 1 - h->cur; return LEDDS_OK; }
     // clear sort bookkeeping + cell ranges (one contiguous region)
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
     ledds_prof_start(LEDDS_K_DEM_KEYS, st);
@@ -784,6 +785,7 @@ int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha,
 {
     (void)status;
     const int n = h->d.n;
+    if (n == 0) return LEDDS_OK;
     ledds_prof_start(LEDDS_K_DEM_KICK, st);
     dem_kick_kernel<<<(unsigned)((3ll * n + 255) / 256), 256, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), f_ext, m_ext, v, w, a, alpha, 0);
     ledds_prof_stop(LEDDS_K_DEM_KICK, st);
@@ -795,7 +797,8 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
                               const double* w, const double* radius, double* a, double* alpha, void* history,
                               void* scratch, int32_t* status, void* stream)
 {
-    if (!out || !x || !v || !w || !radius || !a || !alpha || !history || !scratch || !status) return LEDDS_EINVAL;
+    if (!out || !p || !status) return LEDDS_EINVAL;
+    if (p->n != 0 && (!x || !v || !w || !radius || !a || !alpha || !history || !scratch)) return LEDDS_EINVAL;
     const void* ptrs[] = {x, v, w, radius, a, alpha, history, scratch, status};
     for (const void* q : ptrs)
         if (!ledds_aligned16(q)) return LEDDS_EALIGN;
@@ -804,13 +807,15 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
     int rc = dem_setup(p, h);
     if (rc) { delete h; return rc; }
     cudaStream_t st = (cudaStream_t)stream;
-    if (cudaMemsetAsync(history, 0, h->hs.total, st) != cudaSuccess || cudaMemsetAsync(status, 0, 16, st) != cudaSuccess) {
+    if ((h->hs.total && cudaMemsetAsync(history, 0, h->hs.total, st) != cudaSuccess) ||
+        cudaMemsetAsync(status, 0, 16, st) != cudaSuccess) {
         delete h;
         return LEDDS_ECUDA;
     }
     // forces of the initial state: no drift, delta_t stays 0 (dt_hist = 0)
     rc = ledds_dem_advance_contacts(h, const_cast<double*>(x), v, w, a, alpha, radius, history, scratch, status, 0.0, false, st);
     if (rc) { delete h; return rc; }
+    if (h->d.n == 0) { *out = h; return LEDDS_OK; }
     dem_kick_kernel<<<(unsigned)((3ll * h->d.n + 255) / 256), 256, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), nullptr,
                                                                             nullptr, nullptr, nullptr, a, alpha, 1);
     ledds_count_launch(1);
@@ -823,7 +828,9 @@ extern "C" int ledds_dem_step(ledds_dem* h, double* x, double* v, double* w, dou
                               const double* radius, const double* f_ext, const double* m_ext, void* history,
                               void* scratch, int32_t* status, int nsteps, void* stream)
 {
-    if (!h || !x || !v || !w || !a || !alpha || !radius || !history || !scratch || !status || nsteps < 0) return LEDDS_EINVAL;
+    if (!h || !status || nsteps < 0) return LEDDS_EINVAL;
+    if (h->d.n == 0) return LEDDS_OK;
+    if (!x || !v || !w || !a || !alpha || !radius || !history || !scratch) return LEDDS_EINVAL;
     const void* ptrs[] = {x, v, w, a, alpha, radius, f_ext, m_ext, history, scratch, status};
     for (const void* q : ptrs)
         if (!ledds_aligned16(q)) return LEDDS_EALIGN;
@@ -842,9 +849,14 @@ extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* sc
                                uint32_t* sorted_key, uint32_t* pairs, double* pair_dt, uint32_t pair_cap,
                                uint32_t* n_pairs, double* force, double* torque, void* stream)
 {
-    if (!h || !history || !scratch) return LEDDS_EINVAL;
+    if (!h) return LEDDS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t n = (size_t)h->d.n;
+    if (n == 0) {
+        if (n_pairs && cudaMemsetAsync(n_pairs, 0, sizeof(uint32_t), st) != cudaSuccess) return LEDDS_ECUDA;
+        return LEDDS_OK;
+    }
+    if (!history || !scratch) return LEDDS_EINVAL;
     const DemScratch& s = h->s;
     auto copy = [&](void* dst, const void* src, size_t bytes) {
         return !dst || cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st) == cudaSuccess;

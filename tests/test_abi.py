@@ -64,3 +64,9 @@ def test_parameter_validation_without_gpu():
     d["max_contacts"] = 64
     with pytest.raises(L.LeddsError):
         L.ledds_dem_workspace_bytes(L.dem_params(d))
+    d.update(max_contacts=16, bc=(1, 1, 1), n=0)               # an empty system is valid and needs no history
+    sb0, hb0 = L.ledds_dem_workspace_bytes(L.dem_params(d))
+    assert hb0 == 0 and sb0 > 0
+    d["n"] = -1
+    with pytest.raises(L.LeddsError):
+        L.ledds_dem_workspace_bytes(L.dem_params(d))

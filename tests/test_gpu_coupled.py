@@ -146,3 +146,37 @@ def test_full_size_config3_one_step():
     assert int(g.dem.status[0].item()) == o.status == 0
     f = g.lbm.export()
     assert np.abs(f[:, ::7] - o.f[:, ::7]).max() <= 1e-12 * np.abs(o.f).max()
+
+
+def test_empty_particle_system_is_plain_lbm():
+    # n = 0 is a valid input: the coupled step is then the plain stream-collide, bit for bit, and DEM calls are no-ops
+    import oracle
+    from paper_2512_04997_b200 import Coupled, Dem, Lbm
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(48, 12, 10), R=3.0, z0=5.0, g=0.0)
+    pd = dict(pd, n=0)
+    e3, e1 = np.zeros((0, 3)), np.zeros(0)
+    rho, u = W.random_flow(lbm["shape"], 9)
+    gl = Lbm(dict(lbm, variant=1), rho, u)
+    gd = Dem(pd, e3, e3, e3, e1)
+    g = Coupled(gl, gd, cpl, 3.0)
+    g.step(4)
+    gd.step(3)
+    q = gd.query()
+    assert len(q["pairs"]) == 0 and q["status"] == 0
+    plain = Lbm(dict(lbm, variant=1), rho, u)
+    plain.step(4)
+    assert np.array_equal(gl.export(), plain.export())
+    ref = oracle.lbm_run(lbm["shape"], oracle.lbm_equilibrium(lbm["shape"], rho, u), lbm["tau"], 4, bc=lbm["bc"])
+    assert np.abs(gl.export() - ref).max() <= 1e-13 * np.abs(ref).max()
+
+
+def test_hydrodynamic_force_is_bit_reproducible():
+    # the per-solid sums are exact integer sums: two runs of the same problem agree bit for bit
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=5, n=64, n_part=120, R=4.0)
+    out = []
+    for _ in range(2):
+        o, g = both(lbm, cpl, pd, x, v, w, R, u)
+        g.step(6)
+        out.append((g.f_hyd.cpu().numpy().copy(), g.m_hyd.cpu().numpy().copy(), g.lbm.export()))
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+    assert np.array_equal(out[0][2], out[1][2])
