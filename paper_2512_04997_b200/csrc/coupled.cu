@@ -99,16 +99,17 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
 // thread's column of shared memory with asynchronous copies (no registers tied up while they are in flight);
 // the moments are summed from there and the collision runs pair by pair, each pair pushed as soon as it is
 // collided.  The kernel needs <= 64 registers, so 8 blocks (32 warps) are resident per SM.
-template <typename I>
+template <typename I, int BX>
 __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                                const __grid_constant__ LbmDev P,
                                                                const __grid_constant__ CplDev C)
 {
     __shared__ double sfull[LEDDS_Q][PSM_BLOCK];
     __shared__ double s2[PSM_S2_ROWS][PSM_BLOCK];
-    const int x = blockIdx.x * PSM_BLOCK + threadIdx.x, y = blockIdx.y, z = blockIdx.z;
-    const bool active = x < P.nx;
-    const I cell = ((I)z * (I)P.ny + (I)y) * (I)P.nx + (I)(active ? x : 0);    // a lane past the row reads cell 0, stores nothing
+    const int x = blockIdx.x * BX + (int)(threadIdx.x % BX);
+    const int y = blockIdx.y * (PSM_BLOCK / BX) + (int)(threadIdx.x / BX), z = blockIdx.z;   // a warp lies inside one row
+    const bool active = x < P.nx && y < P.ny;
+    const I cell = active ? ((I)z * (I)P.ny + (I)y) * (I)P.nx + (I)x : (I)0;   // a lane past the lattice reads cell 0, stores nothing
     double* sf = &sfull[0][threadIdx.x];
     {
         const uint32_t dst = (uint32_t)__cvta_generic_to_shared(sf);
@@ -157,6 +158,16 @@ __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(cons
         psm_run_reduce(C, id0, ent, rec);
     }
     psm_collide_stream<I>(sf, P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
+}
+
+template <typename I>
+static void psm_launch(const double* src, double* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
+{
+    const int bx = lb_block_x(d.nx), rows = PSM_BLOCK / bx;
+    const dim3 block(PSM_BLOCK), grid((d.nx + bx - 1) / bx, (d.ny + rows - 1) / rows, d.nz);
+    if (bx == 128) lbm_psm_kernel<I, 128><<<grid, block, 0, st>>>(src, dst, d, C);
+    else if (bx == 64) lbm_psm_kernel<I, 64><<<grid, block, 0, st>>>(src, dst, d, C);
+    else lbm_psm_kernel<I, 32><<<grid, block, 0, st>>>(src, dst, d, C);
 }
 
 // ------------------------------------------------------------------------------------ finish
@@ -287,10 +298,9 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         }
         ledds_prof_stop(LEDDS_K_CPL_RASTER, st);
         LEDDS_CHECK_LAUNCH();
-        dim3 block(PSM_BLOCK), grid((d.nx + PSM_BLOCK - 1) / PSM_BLOCK, d.ny, d.nz);
         ledds_prof_start(LEDDS_K_LBM, st);
-        if (lb_fits_u32(d.N) && lbm->p.variant != 3) lbm_psm_kernel<unsigned><<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
-        else lbm_psm_kernel<long long><<<grid, block, 0, st>>>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C);
+        if (lb_fits_u32(d.N) && lbm->p.variant != 3) psm_launch<unsigned>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C, st);
+        else psm_launch<long long>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C, st);
         ledds_prof_stop(LEDDS_K_LBM, st);
         LEDDS_CHECK_LAUNCH();
         lbm->parity ^= 1;

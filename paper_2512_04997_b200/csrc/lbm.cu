@@ -45,13 +45,15 @@ __global__ void lbm_export_kernel(const double* __restrict__ f, double* __restri
 }
 
 // ------------------------------------------------------------------------------------ variant 1
-template <typename I>
+// Block = 128 threads = BX cells along x times 128 / BX rows along y (BX = 128 unless the lattice is narrower,
+// so that narrow lattices do not run half-empty blocks); a warp always lies inside one row.
+template <typename I, int BX>
 __global__ void __launch_bounds__(128) lbm_push_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                        const __grid_constant__ LbmDev P)
 {
-    const int x = blockIdx.x * blockDim.x + threadIdx.x;
-    const int y = blockIdx.y, z = blockIdx.z;
-    if (x >= P.nx) return;
+    const int x = blockIdx.x * BX + (int)(threadIdx.x % BX);
+    const int y = blockIdx.y * (128 / BX) + (int)(threadIdx.x / BX), z = blockIdx.z;
+    if (x >= P.nx || y >= P.ny) return;
     const I cell = ((I)z * (I)P.ny + (I)y) * (I)P.nx + (I)x;
     double f[LEDDS_Q];
     lb_load<I>(fin, (I)P.N, cell, f);
@@ -59,6 +61,16 @@ __global__ void __launch_bounds__(128) lbm_push_kernel(const double* __restrict_
     lb_moments(f, rho, ux, uy, uz);
     lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
     lb_push_store<I>(fout, P, x, y, z, f, rho);
+}
+
+template <typename I>
+static void lbm_push_launch(const double* src, double* dst, const LbmDev& d, cudaStream_t st)
+{
+    const int bx = lb_block_x(d.nx), rows = 128 / bx;
+    const dim3 block(128), grid((d.nx + bx - 1) / bx, (d.ny + rows - 1) / rows, d.nz);
+    if (bx == 128) lbm_push_kernel<I, 128><<<grid, block, 0, st>>>(src, dst, d);
+    else if (bx == 64) lbm_push_kernel<I, 64><<<grid, block, 0, st>>>(src, dst, d);
+    else lbm_push_kernel<I, 32><<<grid, block, 0, st>>>(src, dst, d);
 }
 
 // ------------------------------------------------------------------------------------ variant 2
@@ -253,9 +265,8 @@ static int lbm_launch(const ledds_lbm* h, const double* src, double* dst, cudaSt
         dim3 block(tx, ry), grid(d.ny / ry, d.nz);
         lbm_rowrot_kernel<<<grid, block, 0, st>>>(src, dst, d);
     } else {
-        dim3 block(128), grid((d.nx + 127) / 128, d.ny, d.nz);
-        if (lb_fits_u32(d.N) && variant != 3) lbm_push_kernel<unsigned><<<grid, block, 0, st>>>(src, dst, d);
-        else lbm_push_kernel<long long><<<grid, block, 0, st>>>(src, dst, d);
+        if (lb_fits_u32(d.N) && variant != 3) lbm_push_launch<unsigned>(src, dst, d, st);
+        else lbm_push_launch<long long>(src, dst, d, st);
     }
     ledds_prof_stop(LEDDS_K_LBM, st);
     LEDDS_CHECK_LAUNCH();

@@ -78,6 +78,9 @@ __device__ __forceinline__ int lb_axis_target(const LbmDev& P, int q, int c, int
     return t;
 }
 
+// cells along x covered by one 128-thread block (the rest of the block goes along y)
+static inline int lb_block_x(int nx) { return nx > 64 ? 128 : (nx > 32 ? 64 : 32); }
+
 // Index type of the population arrays: unsigned 32-bit when 19 N < 2^32 (one IMAD.WIDE per access), else 64-bit.
 static inline bool lb_fits_u32(long long N) { return (unsigned long long)N * LEDDS_Q < 0xffffffffull; }
 
