@@ -83,6 +83,7 @@ struct DemScratch {
     size_t tile_counter;           // dynamic tile ticket (uint32 [4])
     size_t cell_range;             // uint2 [ncell]: [start, end) of the cell in the sorted order, 0,0 when empty
     size_t xr, xr_s;               // (x, y, z, R) per particle, 32 B: particle order / sorted order
+    size_t ncand, cand;            // contacts found per sorted position: uint32 [n], uint32 [maxc][n]
     size_t vp, wp;                 // predictor velocities in particle order: double [n][3]
     size_t pair_count, pair_off;   // query scratch (uint32 [n+1])
     size_t total;

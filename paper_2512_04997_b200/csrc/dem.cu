@@ -361,16 +361,13 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
     return sr - sqrt(d2) > 0.0;                                                       // Eq. (2), (6), strict (G7)
 }
 
+// cand[c][s] (c < ncand[s]) = sorted positions of the particles touching the particle at sorted position s
 template <bool PERIODIC>
-__global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
-    const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
-    const double4* __restrict__ xr_s, const double* __restrict__ vp, const double* __restrict__ wp,
-    const uint2* __restrict__ cell_range,
-    const double* __restrict__ ft_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
-    double* __restrict__ ft_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
-    int32_t* __restrict__ status, double dt_hist)
+__global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
+    const DemDev P, const uint32_t* __restrict__ skey, const double4* __restrict__ xr_s,
+    const uint2* __restrict__ cell_range, uint32_t* __restrict__ ncand_g, uint32_t* __restrict__ cand_g,
+    int32_t* __restrict__ status)
 {
-    extern __shared__ uint32_t s_list[];                       // [maxc][CONTACT_BLOCK] sorted positions of the partners
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
     const int maxc = P.maxc;
@@ -385,7 +382,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
 
     // ---- phase 1: detect
     auto note = [&](uint32_t t) {
-        if (ncand < maxc) s_list[ncand * CONTACT_BLOCK + threadIdx.x] = t;
+        if (ncand < maxc) cand_g[(size_t)ncand * P.n + s] = t;
         else st |= LEDDS_ST_CONTACT_OVERFLOW;
         ncand += ncand < maxc;
     };
@@ -431,7 +428,24 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
         }
     }
 
-    // ---- phase 2: evaluate
+    ncand_g[s] = (uint32_t)ncand;
+    if (st) atomicOr(status, st);
+}
+
+// ---- phase 2: evaluate
+__global__ void __launch_bounds__(CONTACT_BLOCK) dem_force_kernel(
+    const DemDev P, const uint32_t* __restrict__ sidx, const double4* __restrict__ xr_s, const double* __restrict__ vp,
+    const double* __restrict__ wp, const uint32_t* __restrict__ ncand_g, const uint32_t* __restrict__ cand_g,
+    const double* __restrict__ ft_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
+    double* __restrict__ ft_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
+    int32_t* __restrict__ status, double dt_hist)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.n) return;
+    const int maxc = P.maxc;
+    const double4 mine = xr_s[s];
+    const int ncand = (int)ncand_g[s];
+    int st = 0;
     const uint32_t p = sidx[s];
     Body me;
     me.x[0] = mine.x; me.x[1] = mine.y; me.x[2] = mine.z; me.R = mine.w;
@@ -457,7 +471,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_contact_kernel(
     uint32_t ncont = 0;
 
     for (int c = 0; c < ncand; ++c) {
-        const uint32_t t = s_list[c * CONTACT_BLOCK + threadIdx.x];
+        const uint32_t t = cand_g[(size_t)c * P.n + s];
         const double4 o4 = xr_s[t];
         const uint32_t q = sidx[t];
         Body ot;
@@ -684,6 +698,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     s.cell_range = take((size_t)d.ncell * 8);
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
     s.xr = take(n * 32); s.xr_s = take(n * 32);
+    s.ncand = take(n * 4); s.cand = take(n * d.maxc * 4);
     s.vp = take(n * 24); s.wp = take(n * 24);
     s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4);
     s.total = o;
@@ -761,19 +776,18 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     const DemHistory& hs = h->hs;
     const int prev = h->cur, nw = 1 - h->cur;
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
-    {
-        const size_t smem = (size_t)d.maxc * CONTACT_BLOCK * sizeof(uint32_t);
-        if (d.bc[0] && d.bc[1] && d.bc[2]) dem_contact_kernel<false><<<nb, CONTACT_BLOCK, smem, st>>>(
-        d, skey, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
-        at<uint2>(scratch, s.cell_range),
+    if (d.bc[0] && d.bc[1] && d.bc[2])
+        dem_detect_kernel<false><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
+                                                               at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand), status);
+    else
+        dem_detect_kernel<true><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
+                                                              at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand), status);
+    ledds_count_launch(1);
+    dem_force_kernel<<<nb, CONTACT_BLOCK, 0, st>>>(
+        d, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
+        at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
         at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
         at<double>(history, hs.ft[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]), status, dt_hist);
-        else dem_contact_kernel<true><<<nb, CONTACT_BLOCK, smem, st>>>(
-        d, skey, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
-        at<uint2>(scratch, s.cell_range),
-        at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
-        at<double>(history, hs.ft[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]), status, dt_hist);
-    }
     ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
     LEDDS_CHECK_LAUNCH();
     h->cur = nw;
