@@ -179,6 +179,7 @@ def run_ours(args, rank, world):
         "gpu_launches": int(launches),
         "status_word": status,
         "kernel_ms_per_step": {k: round(vv[0] / K, 5) for k, vv in prof.items()},
+        "kernel_ms_note": "dem_sort/gather/contact run on a side stream beside cpl_raster and lbm: their event spans overlap those",
         "roofline": {"bound": "hbm", "kernel": "lbm_psm_kernel", "achieved": round(achieved, 1), "peak": peak,
                      "peak_source": peak_src, "unit": "GB/s", "frac": round(achieved / peak, 4),
                      "bytes_per_launch": bytes_launch, "kernel_ms": round(k_ms_avg, 5),

@@ -8,8 +8,10 @@
  *   - Every array argument is a DEVICE pointer owned by the caller unless it says "host".
  *     The library allocates NO device memory; sizes come from the *_workspace_bytes queries.
  *     Device pointers must be 16-byte aligned (LEDDS_EALIGN otherwise).
- *   - All work is enqueued on the caller's stream (a cudaStream_t passed as void*; NULL = legacy
- *     default stream) and the call returns without synchronising.
+ *   - All work is ordered on the caller's stream (a cudaStream_t passed as void*; NULL = legacy
+ *     default stream) and the call returns without synchronising.  ledds_coupled_step runs the
+ *     contact pipeline of the DEM step beside the lattice kernels on an internal stream that is
+ *     forked from and joined back into the caller's stream with events (capturable in a CUDA graph).
  *   - Handles (ledds_lbm, ledds_dem) are small HOST structs that hold parameters and step
  *     parity only; free them with *_destroy.
  *   - `status` is a caller-owned device int32[4]; word 0 collects asynchronous fault bits

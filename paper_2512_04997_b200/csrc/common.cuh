@@ -105,11 +105,14 @@ struct ledds_dem {
     int sorted_buf;                // which key/idx ping-pong buffer holds the sorted result
     int key_bits, passes, tiles;
     long long steps;
+    // fork/join of the contact pipeline beside the lattice kernels of a coupled step (host resources, lazily made)
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 // entry points implemented in dem.cu and used by coupled.cu
 int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const double* w, const double* a,
                                const double* alpha, const double* radius, void* history, void* scratch,
-                               int32_t* status, double dt_hist, bool drift, cudaStream_t st);
+                               int32_t* status, double dt_hist, bool drift, cudaStream_t st, bool fork = false);
 int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha, const double* radius,
                    const double* f_ext, const double* m_ext, const void* history, int32_t* status, cudaStream_t st);

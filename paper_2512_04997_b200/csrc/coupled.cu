@@ -282,7 +282,9 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
     if (d.ny > 65535 || d.nz > 65535) return LEDDS_EINVAL;
     for (int step = 0; step < nsteps; ++step) {
         for (int sub = 0; sub < c->n_sub; ++sub) {
-            rc = ledds_dem_advance_contacts(dem, x, v, w, a, alpha, radius, history, scratch, status, dem->d.dt, true, st);
+            // the contact pipeline of the last sub-step runs beside the lattice kernels: only the kick needs both
+            const bool fork = sub == c->n_sub - 1 && dem->d.n > 0;
+            rc = ledds_dem_advance_contacts(dem, x, v, w, a, alpha, radius, history, scratch, status, dem->d.dt, true, st, fork);
             if (rc) return rc;
             if (sub < c->n_sub - 1) {                                        // F_sf of the previous LBM step is held
                 rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);
@@ -309,6 +311,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         if (C.n > 0) cpl_finish_kernel<<<(6 * C.n + 127) / 128, 128, 0, st>>>(C, f_hyd, m_hyd);
         ledds_prof_stop(LEDDS_K_CPL_REDUCE, st);
         LEDDS_CHECK_LAUNCH();
+        if (dem->d.n > 0 && cudaStreamWaitEvent(st, dem->ev_join, 0) != cudaSuccess) return LEDDS_ECUDA;   // join
         rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);
         if (rc) return rc;
         dem->steps++;

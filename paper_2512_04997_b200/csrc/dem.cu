@@ -735,8 +735,10 @@ static const T* at(const void* base, size_t off) { return reinterpret_cast<const
 // drift (optional) -> keys -> sort -> gather/ranges -> contacts.  Leaves force/torque in scratch.
 int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const double* w, const double* a,
                                const double* alpha, const double* radius, void* history, void* scratch,
-                               int32_t* status, double dt_hist, bool drift, cudaStream_t st)
+                               int32_t* status, double dt_hist, bool drift, cudaStream_t st, bool fork)
 {
+    // fork = true: everything after the drift/key kernel is enqueued on the handle's side stream (ordered after
+    // that kernel by an event); the caller joins by waiting on h->ev_join before it needs the contact forces.
     const DemDev& d = h->d;
     const DemScratch& s = h->s;
     const int n = d.n, tb = 128, nb = (n + tb - 1) / tb;
@@ -749,6 +751,15 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
                                             at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
     ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
     LEDDS_CHECK_LAUNCH();
+    if (fork) {
+        if (!h->side && (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
+                         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess))
+            return LEDDS_ECUDA;
+        if (cudaEventRecord(h->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(h->side, h->ev_fork, 0) != cudaSuccess)
+            return LEDDS_ECUDA;
+        st = h->side;
+    }
     ledds_prof_start(LEDDS_K_DEM_SORT, st);
     int hb = (n + SORT_THREADS * 8 - 1) / (SORT_THREADS * 8);
     if (hb > 148 * 8) hb = 148 * 8;
@@ -791,6 +802,7 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
     LEDDS_CHECK_LAUNCH();
     h->cur = nw;
+    if (fork && cudaEventRecord(h->ev_join, st) != cudaSuccess) return LEDDS_ECUDA;
     return LEDDS_OK;
 }
 
@@ -902,6 +914,11 @@ extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* sc
 
 extern "C" int ledds_dem_destroy(ledds_dem* h)
 {
+    if (h && h->side) {
+        cudaStreamDestroy(h->side);
+        cudaEventDestroy(h->ev_fork);
+        cudaEventDestroy(h->ev_join);
+    }
     delete h;
     return LEDDS_OK;
 }
