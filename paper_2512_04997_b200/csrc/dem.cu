@@ -336,6 +336,7 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // History slots: [particle][slot] partner id + delta_t as seen from that particle (the partner stores the
 // negated vector).  Per-particle sums stay in registers: no atomics.
 #define CONTACT_BLOCK 128
+#define DEM_IDLE 0xffffffffu   // ncand value of a particle the detect kernel has already finished
 
 // one full 64-byte record per particle: contact force, torque, number of contacts (exact in a double), pad
 __device__ __forceinline__ void dem_store_ft(double* __restrict__ ft, uint32_t p, const double* F, const double* M, uint32_t count)
@@ -364,9 +365,9 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
 // cand[c][s] (c < ncand[s]) = sorted positions of the particles touching the particle at sorted position s
 template <bool PERIODIC>
 __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
-    const DemDev P, const uint32_t* __restrict__ skey, const double4* __restrict__ xr_s,
-    const uint2* __restrict__ cell_range, uint32_t* __restrict__ ncand_g, uint32_t* __restrict__ cand_g,
-    int32_t* __restrict__ status)
+    const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
+    const double4* __restrict__ xr_s, const uint2* __restrict__ cell_range, uint32_t* __restrict__ ncand_g,
+    uint32_t* __restrict__ cand_g, double* __restrict__ ft_new, int32_t* __restrict__ status)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
@@ -428,7 +429,20 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
         }
     }
 
-    ncand_g[s] = (uint32_t)ncand;
+    // a particle that touches nothing and has no wall in reach is finished here (the usual case in a dilute
+    // state): zero record written, DEM_IDLE tells the force kernel to skip it
+    bool near_wall = false;
+    const double xm[3] = {mine.x, mine.y, mine.z};
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+        if (P.bc[a] && (xm[a] - P.lo[a] < mine.w || P.hi[a] - xm[a] < mine.w)) near_wall = true;
+    if (ncand == 0 && !near_wall) {
+        const double zero[3] = {0.0, 0.0, 0.0};
+        dem_store_ft(ft_new, sidx[s], zero, zero, 0u);
+        ncand_g[s] = DEM_IDLE;
+    } else {
+        ncand_g[s] = (uint32_t)ncand;
+    }
     if (st) atomicOr(status, st);
 }
 
@@ -443,22 +457,13 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_force_kernel(
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
     const int maxc = P.maxc;
+    if (ncand_g[s] == DEM_IDLE) return;
     const double4 mine = xr_s[s];
     const int ncand = (int)ncand_g[s];
     int st = 0;
     const uint32_t p = sidx[s];
     Body me;
     me.x[0] = mine.x; me.x[1] = mine.y; me.x[2] = mine.z; me.R = mine.w;
-    bool near_wall = false;
-#pragma unroll
-    for (int a = 0; a < 3; ++a)
-        if (P.bc[a] && (me.x[a] - P.lo[a] < me.R || P.hi[a] - me.x[a] < me.R)) near_wall = true;
-    const double Fs0[3] = {0.0, 0.0, 0.0};
-    if (ncand == 0 && !near_wall) {                             // the usual case in a dilute state: nothing touches
-        dem_store_ft(ft_new, p, Fs0, Fs0, 0u);
-        if (st) atomicOr(status, st);
-        return;
-    }
 #pragma unroll
     for (int a = 0; a < 3; ++a) { me.v[a] = vp[3 * p + a]; me.w[a] = wp[3 * p + a]; }
     const double m_me = dem_mass(P, me.R);
@@ -788,11 +793,13 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     const int prev = h->cur, nw = 1 - h->cur;
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
     if (d.bc[0] && d.bc[1] && d.bc[2])
-        dem_detect_kernel<false><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
-                                                               at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand), status);
+        dem_detect_kernel<false><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
+                                                               at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
+                                                               at<double>(history, hs.ft[nw]), status);
     else
-        dem_detect_kernel<true><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
-                                                              at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand), status);
+        dem_detect_kernel<true><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
+                                                              at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
+                                                              at<double>(history, hs.ft[nw]), status);
     ledds_count_launch(1);
     dem_force_kernel<<<nb, CONTACT_BLOCK, 0, st>>>(
         d, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
