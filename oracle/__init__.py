@@ -54,7 +54,8 @@ _feq = _sig("orc_feq", C.c_double, C.c_int, C.c_double, C.c_double, C.c_double, 
 _lattice = _sig("orc_lbm_lattice", None, _ip, _ip, _ip, _ip, _dp)
 _lbm_eq = _sig("orc_lbm_equilibrium", None, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, _dp)
 _lbm_mom = _sig("orc_lbm_moments", None, C.c_int, C.c_int, C.c_int, _dp, _dp, _dp)
-_lbm_run = _sig("orc_lbm_run", None, C.c_int, C.c_int, C.c_int, C.c_double, _ip, _dp, _dp, _dp, C.c_int)
+_lbm_run = _sig("orc_lbm_run", None, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _ip, _dp, _dp, _dp, C.c_int)
+_trt_om = _sig("orc_trt_omega_minus", C.c_double, C.c_double)
 _zeta = _sig("orc_dem_zeta", C.c_double, C.c_double)
 _grid = _sig("orc_dem_grid", None, C.POINTER(DemParams), _ip, _dp)
 _keys = _sig("orc_dem_keys", None, C.POINTER(DemParams), _dp, _up)
@@ -65,7 +66,7 @@ _forces = _sig("orc_dem_forces", None, C.POINTER(DemParams), _dp, _dp, _dp, _dp,
                C.c_double, _dp, _dp, _dp, _ip)
 _advance = _sig("orc_dem_advance", None, C.POINTER(DemParams), _dp, _dp, _dp, _dp, _dp, _dp, _dp)
 _kick = _sig("orc_dem_kick", None, C.POINTER(DemParams), _dp, _dp, _dp, C.c_void_p, C.c_void_p, _dp, _dp, _dp, _dp)
-_psm_step = _sig("orc_psm_step", None, C.c_int, C.c_int, C.c_int, C.c_double, _ip, _dp, C.c_int, _dp, _dp, _dp, _dp,
+_psm_step = _sig("orc_psm_step", None, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _ip, _dp, C.c_int, _dp, _dp, _dp, _dp,
                  _dp, _dp, _dp, _dp, _ip, _ip)
 _psm_beta = _sig("orc_psm_beta", C.c_double, C.c_double, C.c_double)
 _psm_B = _sig("orc_psm_B", C.c_double, C.c_double, C.c_double)
@@ -110,14 +111,25 @@ def lbm_moments(shape, f):
     return rho, u
 
 
-def lbm_run(shape, f, tau, nsteps, bc=(0, 0, 0), u_wall=None, omega=None):
-    """nsteps BGK collide-and-stream steps (Eq. 22-28); returns the new f [19, N]."""
+def trt_omega_minus(omega_plus):
+    """Eq. (31)"""
+    return _trt_om(omega_plus)
+
+
+def lbm_run(shape, f, tau, nsteps, bc=(0, 0, 0), u_wall=None, omega=None, omega_minus=None, trt=False):
+    """nsteps collide-and-stream steps (Eq. 22-28); returns the new f [19, N].
+    BGK unless trt (then omega_minus of Eq. 31) or an explicit omega_minus is given (TRT, Eq. 29-30)."""
     nx, ny, nz = shape
     f = _f64(f).copy()
     tmp = np.empty_like(f)
     uw = np.zeros(18) if u_wall is None else _f64(u_wall).ravel()
     om = (1.0 / tau) if omega is None else omega
-    _lbm_run(nx, ny, nz, om, np.asarray(bc, np.int32), uw, f, tmp, nsteps)
+    om_m = -1.0
+    if omega_minus is not None:
+        om_m = omega_minus
+    elif trt:
+        om_m = trt_omega_minus(om)
+    _lbm_run(nx, ny, nz, om, om_m, np.asarray(bc, np.int32), uw, f, tmp, nsteps)
     return f
 
 
@@ -216,7 +228,7 @@ def psm_beta_sum(shape, bc, xk, Rk):
     return _psm_beta_sum(shape[0], shape[1], shape[2], np.asarray(bc, np.int32), _f64(xk), Rk)
 
 
-def psm_step(shape, f, tau, bc, u_wall, xk, vk, wk, Rk):
+def psm_step(shape, f, tau, bc, u_wall, xk, vk, wk, Rk, trt=False):
     """One PSM collide-and-stream step in lattice units (Eq. 32-42).
     Returns f_new [19,N], F [np,3], M [np,3], status."""
     nx, ny, nz = shape
@@ -228,7 +240,7 @@ def psm_step(shape, f, tau, bc, u_wall, xk, vk, wk, Rk):
     status = np.zeros(1, np.int32)
     uw = np.zeros(18) if u_wall is None else _f64(u_wall).ravel()
     pad = lambda a, k: _f64(a).reshape(-1) if n else np.zeros(k)
-    _psm_step(nx, ny, nz, tau, np.asarray(bc, np.int32), uw, n, pad(xk, 3), pad(vk, 3), pad(wk, 3), pad(Rk, 1),
+    _psm_step(nx, ny, nz, tau, trt_omega_minus(1.0 / tau) if trt else -1.0, np.asarray(bc, np.int32), uw, n, pad(xk, 3), pad(vk, 3), pad(wk, 3), pad(Rk, 1),
               f, f_out, F, M, slots, status)
     return f_out, F[:n], M[:n], int(status[0])
 
@@ -263,7 +275,8 @@ class Coupled:
             vk = d.vp * (Dt / dx)
             wk = d.wp * Dt
             Rk = d.R / dx
-            self.f, F, M, st = psm_step(lbm["shape"], self.f, lbm["tau"], lbm["bc"], lbm.get("u_wall"), xk, vk, wk, Rk)
+            self.f, F, M, st = psm_step(lbm["shape"], self.f, lbm["tau"], lbm["bc"], lbm.get("u_wall"), xk, vk, wk, Rk,
+                                        trt=bool(lbm.get("collision", 0)))
             self.status |= st
             self.F_sf = F * (rho_f * dx ** 4 / Dt ** 2)
             self.M_sf = M * (rho_f * dx ** 5 / Dt ** 2)

@@ -11,6 +11,7 @@
  *   moments        PAPER.md:200-202  Eq. (22a), (22b)
  *   collide/stream PAPER.md:206-216  Eq. (23)-(25)
  *   BGK            PAPER.md:222      Eq. (26), relaxation time Eq. (27)
+ *   TRT            PAPER.md:236-246  Eq. (29)-(31)
  *   equilibrium    PAPER.md:230      Eq. (28), c_s^2 = 1/3 (reading G17)
  *   boundaries     PAPER.md:254      "standard and velocity-modified bounce-back"
  *                                    (reading G19: halfway, link-wise)
@@ -27,7 +28,8 @@
  *
  * Pins (tests/test_oracle_lbm.py): Taylor-Green decay, exact mass
  * conservation, pure streaming is a permutation, uniform equilibrium is a
- * fixed point, Couette profile, lattice isotropy sums.
+ * fixed point, Couette profile, lattice isotropy sums; TRT: equals BGK for
+ * tau^- = tau^+, (tau^+ - 1/2)(tau^- - 1/2) = 3/16, decay rate set by tau^+ alone.
  */
 #include <math.h>
 #include <stddef.h>
@@ -114,9 +116,25 @@ void orc_stream_one(int nx, int ny, int nz, const int *bc, const double *u_wall,
         f_out[(size_t)i * N + ((size_t)t[2] * ny + t[1]) * nx + t[0]] = fs;
 }
 
-/* One BGK collide-and-stream step, Eq. (22)-(28); omega = dt/tau.
+/* Eq. (31): dt/tau^- for the TRT model, given dt/tau^+ (the "magic" combination
+ * (tau^+ - 1/2)(tau^- - 1/2) = 3/16). */
+double orc_trt_omega_minus(double omega_plus) { return 8.0 * (2.0 - omega_plus) / (8.0 - omega_plus); }
+
+/* Collision term Omega_i of one cell.  omega_minus < 0: BGK, Eq. (26).  Otherwise TRT, Eq. (29)-(30),
+ * written out as printed: f^+- = 0.5 (f_i +- f_ibar), same for the equilibria. */
+double orc_collision(int i, const double *f, double rho, double ux, double uy, double uz, double omega, double omega_minus)
+{
+    double fe = orc_feq(i, rho, ux, uy, uz);
+    if (omega_minus < 0.0) return -omega * (f[i] - fe);
+    double feo = orc_feq(OPP[i], rho, ux, uy, uz);
+    double fp = 0.5 * (f[i] + f[OPP[i]]), fm = 0.5 * (f[i] - f[OPP[i]]);
+    double ep = 0.5 * (fe + feo), em = 0.5 * (fe - feo);
+    return -omega * (fp - ep) - omega_minus * (fm - em);
+}
+
+/* One collide-and-stream step, Eq. (22)-(28); omega = dt/tau (tau^+ for TRT), omega_minus < 0 selects BGK.
  * omega = 0 gives pure streaming (used by the permutation pin). */
-void orc_lbm_step(int nx, int ny, int nz, double omega, const int *bc, const double *u_wall,
+void orc_lbm_step(int nx, int ny, int nz, double omega, double omega_minus, const int *bc, const double *u_wall,
                   const double *f_in, double *f_out)
 {
     size_t N = (size_t)nx * ny * nz;
@@ -132,20 +150,21 @@ void orc_lbm_step(int nx, int ny, int nz, double omega, const int *bc, const dou
                 }
                 double ux = jx / rho, uy = jy / rho, uz = jz / rho;
                 for (int i = 0; i < Q; ++i) {
-                    double fs = f[i] - omega * (f[i] - orc_feq(i, rho, ux, uy, uz));
+                    double fs = omega_minus < 0.0 ? f[i] - omega * (f[i] - orc_feq(i, rho, ux, uy, uz))
+                                                  : f[i] + orc_collision(i, f, rho, ux, uy, uz, omega, omega_minus);
                     orc_stream_one(nx, ny, nz, bc, u_wall, x, y, z, i, fs, rho, f_out);
                 }
             }
 }
 
 /* nsteps steps, ping-pong between f and tmp; result always ends in f. */
-void orc_lbm_run(int nx, int ny, int nz, double omega, const int *bc, const double *u_wall,
+void orc_lbm_run(int nx, int ny, int nz, double omega, double omega_minus, const int *bc, const double *u_wall,
                  double *f, double *tmp, int nsteps)
 {
     size_t N = (size_t)nx * ny * nz;
     double *a = f, *b = tmp;
     for (int s = 0; s < nsteps; ++s) {
-        orc_lbm_step(nx, ny, nz, omega, bc, u_wall, a, b);
+        orc_lbm_step(nx, ny, nz, omega, omega_minus, bc, u_wall, a, b);
         double *sw = a; a = b; b = sw;
     }
     if (a != f) memcpy(f, a, sizeof(double) * Q * N);

@@ -5,7 +5,7 @@
  * coupling of PAPER.md (arxiv 2512.04997) section 2.4 on top of the BGK
  * collide-and-stream of oracle/lbm.c.  Shares nothing with the CUDA path.
  *
- *   PSM collision        PAPER.md:270-275  Eq. (32), (33) (BGK in place of TRT, G20)
+ *   PSM collision        PAPER.md:270-275  Eq. (32), (33) with Omega_i = BGK (configs, G20) or TRT (Eq. 30)
  *   solid operator       PAPER.md:281      Eq. (34), overbar restored (reading G21)
  *   solid velocity       PAPER.md:285      Eq. (35), sign/index reading G22
  *   weighting            PAPER.md:289-295  Eq. (36), (37); only B_tot truncated (G23)
@@ -100,7 +100,10 @@ static double solid_terms(const int *n, const int *bc, double tau, const int *r,
  * velocity wk, radius Rk, all in lattice units.  Outputs: f_out, and the
  * hydrodynamic force F[3np] and torque M[3np] on every sphere (lattice units).
  * slots is scratch of 2*N ints.  status |= 2 when a third solid was dropped. */
-void orc_psm_step(int nx, int ny, int nz, double tau, const int *bc, const double *u_wall,
+double orc_collision(int i, const double *f, double rho, double ux, double uy, double uz, double omega, double omega_minus);
+
+/* omega_minus < 0: BGK; else the TRT model of Eq. (29)-(31) as Omega_i in Eq. (33) */
+void orc_psm_step(int nx, int ny, int nz, double tau, double omega_minus, const int *bc, const double *u_wall,
                   int np, const double *xk, const double *vk, const double *wk, const double *Rk,
                   const double *f_in, double *f_out, double *F, double *M, int *slots, int *status)
 {
@@ -156,7 +159,8 @@ void orc_psm_step(int nx, int ny, int nz, double tau, const int *bc, const doubl
                 }
                 double Btot = Bsum < 1.0 ? Bsum : 1.0;                       /* Eq. (37) */
                 for (int i = 0; i < Q; ++i) {
-                    double bgk = -omega * (f[i] - orc_feq(i, rho, u[0], u[1], u[2]));
+                    double bgk = omega_minus < 0.0 ? -omega * (f[i] - orc_feq(i, rho, u[0], u[1], u[2]))
+                                                   : orc_collision(i, f, rho, u[0], u[1], u[2], omega, omega_minus);
                     fs[i] = f[i] + ((1.0 - Btot) * bgk + solid[i]);          /* Eq. (32)-(33) */
                     orc_stream_one(nx, ny, nz, bc, u_wall, x, y, z, i, fs[i], rho, f_out);
                 }

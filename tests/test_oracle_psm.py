@@ -47,7 +47,8 @@ def test_no_particle_is_plain_lbm_bit_for_bit(bc):
     assert np.array_equal(a2, b2) and np.all(F == 0)
 
 
-def test_momentum_budget_periodic():
+@pytest.mark.parametrize("trt", [False, True])
+def test_momentum_budget_periodic(trt):
     # G26: in a periodic box the fluid momentum changes by exactly minus the force on the solids
     # (lattice units): sum f' c - sum f c = - sum_k F_k.  Also mass is conserved (sum_i Omega^s = 0).
     shape = (16, 14, 12)
@@ -57,7 +58,7 @@ def test_momentum_budget_periodic():
     vk = np.array([[0.02, 0.0, -0.01], [-0.01, 0.01, 0.0], [0.0, 0.0, 0.03]])
     wk = np.array([[0.0, 0.002, 0.0], [0.001, 0.0, 0.0], [0.0, 0.0, -0.003]])
     Rk = np.array([3.0, 3.2, 2.5])
-    f1, F, M, st = oracle.psm_step(shape, f, 0.6, (0, 0, 0), None, xk, vk, wk, Rk)
+    f1, F, M, st = oracle.psm_step(shape, f, 0.6, (0, 0, 0), None, xk, vk, wk, Rk, trt=trt)   # Eq. 33 with BGK or TRT
     assert st == 0
     assert abs(f1.sum() - f.sum()) < 1e-12 * f.sum()
     assert np.abs(F).min() > 1e-5
