@@ -54,7 +54,7 @@ typedef struct ledds_lbm ledds_lbm;
 typedef struct ledds_dem ledds_dem;
 
 /* ------------------------------------------------------------------------------------ LBM
- * Fused D3Q19 BGK stream-collide, Eq. (22)-(28), boundaries PAPER.md:254. */
+ * Fused D3Q19 stream-collide (BGK or TRT), Eq. (22)-(31), boundaries PAPER.md:254. */
 typedef struct {
     int nx, ny, nz;          /* lattice size, x fastest                                           */
     double tau;              /* relaxation time in units of dt, > 0.5 (Eq. 27)                    */
@@ -65,6 +65,8 @@ typedef struct {
                                 is reserved: LEDDS_EINVAL in this version                         */
     int variant;             /* kernel variant: 0 auto, 1 plain push, 2 row-rotate (aligned stores),
                                 3 plain push with 64-bit indices (the path lattices with 19 N >= 2^32 take) */
+    int collision;           /* 0 = BGK, Eq. (26).  1 = TRT, Eq. (29)-(30) with tau^+ = tau and tau^- of
+                                Eq. (31); also the Omega_i of the PSM collision Eq. (33)  */
 } ledds_lbm_params;
 
 /* f_bytes: size of the population buffer the caller must allocate for this layout. */

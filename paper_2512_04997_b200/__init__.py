@@ -27,7 +27,7 @@ EXPORTS = ["ledds_lbm_workspace_bytes", "ledds_lbm_init", "ledds_lbm_import", "l
 
 class LbmParams(C.Structure):
     _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("tau", C.c_double), ("bc", C.c_int * 3),
-                ("u_wall", C.c_double * 18), ("layout", C.c_int), ("variant", C.c_int)]
+                ("u_wall", C.c_double * 18), ("layout", C.c_int), ("variant", C.c_int), ("collision", C.c_int)]
 
 
 class DemParams(C.Structure):
@@ -76,7 +76,7 @@ KERNEL_GROUPS = ["lbm", "dem_keys", "dem_sort", "dem_gather", "dem_contact", "de
 
 
 def lbm_params(d) -> LbmParams:
-    """dict(shape, tau, bc, u_wall[, variant]) -> ledds_lbm_params"""
+    """dict(shape, tau, bc, u_wall[, variant, collision]) -> ledds_lbm_params"""
     p = LbmParams()
     p.nx, p.ny, p.nz = (int(v) for v in d["shape"])
     p.tau = float(d["tau"])
@@ -85,6 +85,7 @@ def lbm_params(d) -> LbmParams:
     p.u_wall[:] = [0.0] * 18 if uw is None else [float(v) for v in list(uw.reshape(-1) if hasattr(uw, "reshape") else uw)]
     p.layout = 0
     p.variant = int(d.get("variant", 0))
+    p.collision = int(d.get("collision", 0))
     return p
 
 

@@ -46,7 +46,9 @@ __host__ __device__ constexpr double lb_w(int q) { return q == 0 ? 1.0 / 3.0 : (
 struct LbmDev {
     int nx, ny, nz;
     long long N;
-    double omega;          // dt / tau
+    double omega;          // dt / tau (tau^+ for TRT)
+    double omega_minus;    // dt / tau^-, Eq. (31)
+    int trt;               // collision model: 0 BGK, 1 TRT
     double tau;
     int bc[3];
     double uw[18];         // [axis][side][comp]

@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
 // thread's column of shared memory with asynchronous copies (no registers tied up while they are in flight);
 // the moments are summed from there and the collision runs pair by pair, each pair pushed as soon as it is
 // collided.  The kernel needs <= 64 registers, so 8 blocks (32 warps) are resident per SM.
-template <typename I, int BX>
+template <typename I, int BX, bool TRT>
 __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                                const __grid_constant__ LbmDev P,
                                                                const __grid_constant__ CplDev C)
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(cons
     }
     const LbPush<I> push(P, x, y, z);
     if (!__any_sync(0xffffffffu, id0 != PSM_EMPTY)) {
-        bgk_collide_stream<I>(sf, P.omega, rho, ux, uy, uz, push, fout, P, active);
+        bgk_collide_stream<I, TRT>(sf, P.omega, rho, ux, uy, uz, push, fout, P, active);
         return;
     }
     if (id0 != PSM_EMPTY) C.slots[cell] = make_uint2(PSM_EMPTY, PSM_EMPTY);           // consumed: free for the next step
@@ -157,17 +157,17 @@ __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(cons
         psm_solid_terms(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
         psm_run_reduce(C, id0, ent, rec);
     }
-    psm_collide_stream<I>(sf, P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
+    psm_collide_stream<I, TRT>(sf, P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
 }
 
-template <typename I>
+template <typename I, bool TRT>
 static void psm_launch(const double* src, double* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
 {
     const int bx = lb_block_x(d.nx), rows = PSM_BLOCK / bx;
     const dim3 block(PSM_BLOCK), grid((d.nx + bx - 1) / bx, (d.ny + rows - 1) / rows, d.nz);
-    if (bx == 128) lbm_psm_kernel<I, 128><<<grid, block, 0, st>>>(src, dst, d, C);
-    else if (bx == 64) lbm_psm_kernel<I, 64><<<grid, block, 0, st>>>(src, dst, d, C);
-    else lbm_psm_kernel<I, 32><<<grid, block, 0, st>>>(src, dst, d, C);
+    if (bx == 128) lbm_psm_kernel<I, 128, TRT><<<grid, block, 0, st>>>(src, dst, d, C);
+    else if (bx == 64) lbm_psm_kernel<I, 64, TRT><<<grid, block, 0, st>>>(src, dst, d, C);
+    else lbm_psm_kernel<I, 32, TRT><<<grid, block, 0, st>>>(src, dst, d, C);
 }
 
 // ------------------------------------------------------------------------------------ finish
@@ -301,8 +301,15 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         ledds_prof_stop(LEDDS_K_CPL_RASTER, st);
         LEDDS_CHECK_LAUNCH();
         ledds_prof_start(LEDDS_K_LBM, st);
-        if (lb_fits_u32(d.N) && lbm->p.variant != 3) psm_launch<unsigned>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C, st);
-        else psm_launch<long long>(f + lbm->parity * half, f + (1 - lbm->parity) * half, d, C, st);
+        {
+            const double* src = f + lbm->parity * half;
+            double* dst = f + (1 - lbm->parity) * half;
+            const bool u32 = lb_fits_u32(d.N) && lbm->p.variant != 3;
+            if (u32 && !d.trt) psm_launch<unsigned, false>(src, dst, d, C, st);
+            else if (u32) psm_launch<unsigned, true>(src, dst, d, C, st);
+            else if (!d.trt) psm_launch<long long, false>(src, dst, d, C, st);
+            else psm_launch<long long, true>(src, dst, d, C, st);
+        }
         ledds_prof_stop(LEDDS_K_LBM, st);
         LEDDS_CHECK_LAUNCH();
         lbm->parity ^= 1;

@@ -47,7 +47,7 @@ __global__ void lbm_export_kernel(const double* __restrict__ f, double* __restri
 // ------------------------------------------------------------------------------------ variant 1
 // Block = 128 threads = BX cells along x times 128 / BX rows along y (BX = 128 unless the lattice is narrower,
 // so that narrow lattices do not run half-empty blocks); a warp always lies inside one row.
-template <typename I, int BX>
+template <typename I, int BX, bool TRT>
 __global__ void __launch_bounds__(128) lbm_push_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                        const __grid_constant__ LbmDev P)
 {
@@ -59,18 +59,18 @@ __global__ void __launch_bounds__(128) lbm_push_kernel(const double* __restrict_
     lb_load<I>(fin, (I)P.N, cell, f);
     double rho, ux, uy, uz;
     lb_moments(f, rho, ux, uy, uz);
-    lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
+    lb_collide<TRT>(f, P, rho, ux, uy, uz);
     lb_push_store<I>(fout, P, x, y, z, f, rho);
 }
 
-template <typename I>
+template <typename I, bool TRT>
 static void lbm_push_launch(const double* src, double* dst, const LbmDev& d, cudaStream_t st)
 {
     const int bx = lb_block_x(d.nx), rows = 128 / bx;
     const dim3 block(128), grid((d.nx + bx - 1) / bx, (d.ny + rows - 1) / rows, d.nz);
-    if (bx == 128) lbm_push_kernel<I, 128><<<grid, block, 0, st>>>(src, dst, d);
-    else if (bx == 64) lbm_push_kernel<I, 64><<<grid, block, 0, st>>>(src, dst, d);
-    else lbm_push_kernel<I, 32><<<grid, block, 0, st>>>(src, dst, d);
+    if (bx == 128) lbm_push_kernel<I, 128, TRT><<<grid, block, 0, st>>>(src, dst, d);
+    else if (bx == 64) lbm_push_kernel<I, 64, TRT><<<grid, block, 0, st>>>(src, dst, d);
+    else lbm_push_kernel<I, 32, TRT><<<grid, block, 0, st>>>(src, dst, d);
 }
 
 // ------------------------------------------------------------------------------------ variant 2
@@ -83,6 +83,7 @@ __device__ __forceinline__ void st2(double* p, double a, double b)
     *reinterpret_cast<double2*>(p) = make_double2(a, b);
 }
 
+template <bool TRT>
 __global__ void __launch_bounds__(LEDDS_ROT_MAX_THREADS) lbm_rowrot_kernel(const double* __restrict__ fin,
                                                                          double* __restrict__ fout, const LbmDev P)
 {
@@ -104,9 +105,9 @@ __global__ void __launch_bounds__(LEDDS_ROT_MAX_THREADS) lbm_rowrot_kernel(const
     }
     double rhoa, rhob, ux, uy, uz;
     lb_moments(fa, rhoa, ux, uy, uz);
-    lb_collide_bgk(fa, P.omega, rhoa, ux, uy, uz);
+    lb_collide<TRT>(fa, P, rhoa, ux, uy, uz);
     lb_moments(fb, rhob, ux, uy, uz);
-    lb_collide_bgk(fb, P.omega, rhob, ux, uy, uz);
+    lb_collide<TRT>(fb, P, rhob, ux, uy, uz);
 
     // publish warp-edge values of the 10 x-moving directions
     {
@@ -182,6 +183,7 @@ static int lbm_validate(const ledds_lbm_params* p)
     if (!(p->tau > 0.5)) return LEDDS_EINVAL;
     if (p->layout != 0) return LEDDS_EINVAL;
     if (p->variant < 0 || p->variant > 3) return LEDDS_EINVAL;
+    if (p->collision != 0 && p->collision != 1) return LEDDS_EINVAL;
     for (int a = 0; a < 3; ++a)
         if (p->bc[a] != 0 && p->bc[a] != 1) return LEDDS_EINVAL;
     // a periodic axis of length 1 would stream a population onto itself: allowed (it is a no-op wrap)
@@ -215,6 +217,8 @@ extern "C" int ledds_lbm_init(ledds_lbm** out, const ledds_lbm_params* p, double
     d.N = (long long)p->nx * p->ny * p->nz;
     d.tau = p->tau;
     d.omega = 1.0 / p->tau;
+    d.omega_minus = 8.0 * (2.0 - d.omega) / (8.0 - d.omega);                  // Eq. (31)
+    d.trt = p->collision;
     d.any_wall_velocity = 0;
     for (int a = 0; a < 3; ++a) {
         d.bc[a] = p->bc[a];
@@ -263,10 +267,14 @@ static int lbm_launch(const ledds_lbm* h, const double* src, double* dst, cudaSt
         int ry = 1;
         while (ry < 8 && tx * ry * 2 <= LEDDS_ROT_MAX_THREADS && d.ny % (ry * 2) == 0) ry *= 2;
         dim3 block(tx, ry), grid(d.ny / ry, d.nz);
-        lbm_rowrot_kernel<<<grid, block, 0, st>>>(src, dst, d);
+        if (d.trt) lbm_rowrot_kernel<true><<<grid, block, 0, st>>>(src, dst, d);
+        else lbm_rowrot_kernel<false><<<grid, block, 0, st>>>(src, dst, d);
     } else {
-        if (lb_fits_u32(d.N) && variant != 3) lbm_push_launch<unsigned>(src, dst, d, st);
-        else lbm_push_launch<long long>(src, dst, d, st);
+        const bool u32 = lb_fits_u32(d.N) && variant != 3;
+        if (u32 && !d.trt) lbm_push_launch<unsigned, false>(src, dst, d, st);
+        else if (u32) lbm_push_launch<unsigned, true>(src, dst, d, st);
+        else if (!d.trt) lbm_push_launch<long long, false>(src, dst, d, st);
+        else lbm_push_launch<long long, true>(src, dst, d, st);
     }
     ledds_prof_stop(LEDDS_K_LBM, st);
     LEDDS_CHECK_LAUNCH();

@@ -56,6 +56,32 @@ __device__ __forceinline__ void lb_collide_bgk(double (&f)[LEDDS_Q], double omeg
     for (int q = 0; q < LEDDS_Q; ++q) f[q] = f[q] - omega * (f[q] - fe[q]);
 }
 
+// Eq. (29)-(30): TRT.  f+- = (f_q +- f_qbar)/2 relax with dt/tau+ and dt/tau- towards the even and odd parts
+// of the equilibrium; the rest population has no odd part.
+__device__ __forceinline__ void lb_collide_trt(double (&f)[LEDDS_Q], double omega_p, double omega_m, double rho, double ux,
+                                               double uy, double uz)
+{
+    const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
+    f[0] = f[0] - omega_p * (f[0] - lb_w(0) * rho * k);
+#pragma unroll
+    for (int q = 1; q < LEDDS_Q; q += 2) {
+        const double cu = lb_cdot(q, ux, uy, uz);
+        const double wr = lb_w(q) * rho;
+        const double even = wr * (k + 4.5 * cu * cu), odd = wr * 3.0 * cu;
+        const double rp = omega_p * (0.5 * (f[q] + f[q + 1]) - even), rm = omega_m * (0.5 * (f[q] - f[q + 1]) - odd);
+        f[q] = f[q] - (rp + rm);
+        f[q + 1] = f[q + 1] - (rp - rm);
+    }
+}
+
+// the collision model is a compile-time choice: each kernel is instantiated for BGK and for TRT
+template <bool TRT>
+__device__ __forceinline__ void lb_collide(double (&f)[LEDDS_Q], const LbmDev& P, double rho, double ux, double uy, double uz)
+{
+    if (TRT) lb_collide_trt(f, P.omega, P.omega_minus, rho, ux, uy, uz);
+    else lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
+}
+
 // Where does the link q that starts at coordinate `r` on one axis end?  Returns the target
 // coordinate (wrapped on a periodic axis); sets `bounced` and adds c_q . u_wall of the crossed
 // wall when the axis is walled (halfway bounce-back).

@@ -104,45 +104,6 @@ __device__ __forceinline__ void psm_solid_terms(const LbmDev& P, const CplDev& C
 // rows 0..4 = B, 1 - 1.5 u_k^2, u_k[3].
 #define PSM_S2_ROWS 5
 
-// PSM collision, Eq. (32)-(37), of a cell cut by the solid (B0, uk0) and, when the warp-uniform flag `two` is
-// set, by the second one parked in s2 (B = 0 there for the lanes that have none).  Written pair by pair
-// (q, opposite q) so that no per-direction array besides f itself is live.
-__device__ __forceinline__ void psm_collide(double (&f)[LEDDS_Q], double omega, double rho, double ux, double uy,
-                                            double uz, double B0, const double (&uk0)[3], bool two, const double* s2)
-{
-    const double k0 = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
-    const double kk0 = 1.0 - 1.5 * (uk0[0] * uk0[0] + uk0[1] * uk0[1] + uk0[2] * uk0[2]);
-    const double Bsum = B0 + (two ? s2[0] : 0.0);
-    const double keep = 1.0 - (Bsum < 1.0 ? Bsum : 1.0);                              // 1 - B_tot, Eq. (37)
-    const double komega = keep * omega;
-    {   // rest population: its own opposite, Omega^s = feq(rho,u_k) - feq(rho,u)
-        const double wr = lb_w(0) * rho, fe = wr * k0;
-        double acc = B0 * (wr * kk0 - fe);
-        if (two) acc += s2[0] * (wr * s2[PSM_BLOCK] - fe);
-        f[0] = f[0] + (acc - komega * (f[0] - fe));
-    }
-#pragma unroll
-    for (int q = 1; q < LEDDS_Q; q += 2) {
-        const double wr = lb_w(q) * rho;
-        const double cu = lb_cdot(q, ux, uy, uz);
-        const double ev = wr * (k0 + 4.5 * cu * cu), od = wr * 3.0 * cu;
-        const double nq = f[q] - (ev + od), no = f[q + 1] - (ev - od);                   // f - feq(rho,u), Eq. (28)
-        const double cuk = lb_cdot(q, uk0[0], uk0[1], uk0[2]);
-        const double evk = wr * (kk0 + 4.5 * cuk * cuk), odk = wr * 3.0 * cuk;
-        double acc_q = B0 * (no - (f[q] - (evk + odk)));                                // B Omega^s, Eq. (34), direction q
-        double acc_o = B0 * (nq - (f[q + 1] - (evk - odk)));                            //                      its opposite
-        if (two) {
-            const double B1 = s2[0], kk1 = s2[PSM_BLOCK];
-            const double cu1 = lb_cdot(q, s2[2 * PSM_BLOCK], s2[3 * PSM_BLOCK], s2[4 * PSM_BLOCK]);
-            const double ev1 = wr * (kk1 + 4.5 * cu1 * cu1), od1 = wr * 3.0 * cu1;
-            acc_q += B1 * (no - (f[q] - (ev1 + od1)));
-            acc_o += B1 * (nq - (f[q + 1] - (ev1 - od1)));
-        }
-        f[q] = f[q] + (acc_q - komega * nq);                                            // Eq. (32)-(33)
-        f[q + 1] = f[q + 1] + (acc_o - komega * no);
-    }
-}
-
 // Sum the records of each run of consecutive lanes that hold the same solid id (a solid cuts a lattice row
 // in consecutive cells) with a shuffle tree, and let the first lane of the run add the sum to the solid's
 // fixed-point accumulators (12 integer reductions, no return value).  All 32 lanes call this; id = PSM_EMPTY
@@ -186,11 +147,31 @@ __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int
 // ---- streaming forms: the populations of the cell sit in shared memory (column `sf`, stride PSM_BLOCK), are
 // collided pair by pair and pushed right away, so that only one pair is live in registers at a time.
 
-// BGK, same expressions as lb_collide_bgk / lb_equilibrium
-template <typename I>
+// BGK or TRT without solids, same expressions as lb_collide_bgk / lb_collide_trt
+template <typename I, bool TRT>
 __device__ __forceinline__ void bgk_collide_stream(const double* sf, double omega, double rho, double ux, double uy, double uz,
                                                    const LbPush<I>& push, double* __restrict__ fout, const LbmDev& P, bool active)
 {
+    if (TRT) {
+        const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
+        {
+            const double f0 = sf[0];
+            if (active) push.put(fout, P, 0, f0 - omega * (f0 - lb_w(0) * rho * k), rho);
+        }
+#pragma unroll
+        for (int q = 1; q < LEDDS_Q; q += 2) {
+            const double a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
+            const double cu = lb_cdot(q, ux, uy, uz);
+            const double wr = lb_w(q) * rho;
+            const double even = wr * (k + 4.5 * cu * cu), odd = wr * 3.0 * cu;
+            const double rp = omega * (0.5 * (a + b) - even), rm = P.omega_minus * (0.5 * (a - b) - odd);
+            if (active) {
+                push.put(fout, P, q, a - (rp + rm), rho);
+                push.put(fout, P, q + 1, b - (rp - rm), rho);
+            }
+        }
+        return;
+    }
     const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
     {
         const double f0 = sf[0], fe = lb_w(0) * rho * k;
@@ -210,8 +191,9 @@ __device__ __forceinline__ void bgk_collide_stream(const double* sf, double omeg
     }
 }
 
-// PSM, same expressions as psm_collide
-template <typename I>
+// PSM collision, Eq. (32)-(37), of a cell cut by the solid (B0, uk0) and, when the warp-uniform flag `two` is
+// set, by the second one parked in s2 (B = 0 there for the lanes that have none)
+template <typename I, bool TRT>
 __device__ __forceinline__ void psm_collide_stream(const double* sf, double omega, double rho, double ux, double uy, double uz,
                                                    double B0, const double (&uk0)[3], bool two, const double* s2,
                                                    const LbPush<I>& push, double* __restrict__ fout, const LbmDev& P, bool active)
@@ -245,9 +227,14 @@ __device__ __forceinline__ void psm_collide_stream(const double* sf, double omeg
             acc_q += B1 * (no - (a - (ev1 + od1)));
             acc_o += B1 * (nq - (b - (ev1 - od1)));
         }
+        double oq = komega * nq, oo = komega * no;                                      // -(1 - B_tot) Omega_i, BGK
+        if (TRT) {                                                                      //                        TRT, Eq. (30)
+            const double rp = komega * (0.5 * (a + b) - ev), rm = keep * P.omega_minus * (0.5 * (a - b) - od);
+            oq = rp + rm; oo = rp - rm;
+        }
         if (active) {
-            push.put(fout, P, q, a + (acc_q - komega * nq), rho);                       // Eq. (32)-(33)
-            push.put(fout, P, q + 1, b + (acc_o - komega * no), rho);
+            push.put(fout, P, q, a + (acc_q - oq), rho);                                // Eq. (32)-(33)
+            push.put(fout, P, q + 1, b + (acc_o - oo), rho);
         }
     }
 }

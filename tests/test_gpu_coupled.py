@@ -180,3 +180,14 @@ def test_hydrodynamic_force_is_bit_reproducible():
         out.append((g.f_hyd.cpu().numpy().copy(), g.m_hyd.cpu().numpy().copy(), g.lbm.export()))
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
     assert np.array_equal(out[0][2], out[1][2])
+
+
+def test_trt_coupled_step():
+    # Eq. (33) with the TRT operator of Eq. (30) as Omega_i (the model of the paper's results), moving walls,
+    # contacts, two-solid cells
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=7, n=64, n_part=90, R=4.0)
+    o, g = both(dict(lbm, collision=1), cpl, pd, x, v, w, R, u)
+    o.step(1); g.step(1)
+    compare(o, g)
+    o.step(5); g.step(5)
+    compare(o, g)

@@ -9,18 +9,18 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-12
 
 
-def run_pair(shape, tau, bc, u_wall, steps, variant, seed=0, flow="random"):
+def run_pair(shape, tau, bc, u_wall, steps, variant, seed=0, flow="random", collision=0):
     import oracle
     from paper_2512_04997_b200 import Lbm
     rho, u = W.random_flow(shape, seed) if flow == "random" else W.tgv(shape, 0.02, 1.0, "xy")
-    lbm = dict(shape=shape, tau=tau, bc=bc, u_wall=u_wall, variant=variant)
+    lbm = dict(shape=shape, tau=tau, bc=bc, u_wall=u_wall, variant=variant, collision=collision)
     g = Lbm(lbm, rho, u)
     f0 = g.export()
     ref0 = oracle.lbm_equilibrium(shape, rho, u)
     assert np.abs(f0 - ref0).max() <= 1e-15                    # init (Eq. 28) agrees
     g.step(steps)
     f = g.export()
-    ref = oracle.lbm_run(shape, ref0, tau, steps, bc=bc, u_wall=u_wall)
+    ref = oracle.lbm_run(shape, ref0, tau, steps, bc=bc, u_wall=u_wall, trt=bool(collision))
     return f, ref
 
 
@@ -38,6 +38,16 @@ MOVING[2, 0, 0] = -0.05; MOVING[2, 1, 0] = 0.05; MOVING[1, 0, 2] = 0.02; MOVING[
 ])
 def test_populations_after_100_steps(variant, shape, bc, uw):
     f, ref = run_pair(shape, 0.6, bc, uw, 100, variant)
+    assert np.abs(f - ref).max() <= TOL * np.abs(ref).max()
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("shape,bc,uw", [((64, 12, 10), (0, 0, 0), None), ((64, 9, 10), (1, 0, 1), MOVING), ((37, 6, 5), (0, 1, 0), MOVING)])
+def test_trt_populations_after_100_steps(variant, shape, bc, uw):
+    # PAPER.md:236-246, Eq. (29)-(31): the collision model the paper's results use
+    if variant == 2 and shape[0] % 64:
+        pytest.skip("row-rotate needs nx % 64 == 0")
+    f, ref = run_pair(shape, 0.56, bc, uw, 100, variant, collision=1)
     assert np.abs(f - ref).max() <= TOL * np.abs(ref).max()
 
 
