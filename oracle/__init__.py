@@ -66,12 +66,13 @@ _forces = _sig("orc_dem_forces", None, C.POINTER(DemParams), _dp, _dp, _dp, _dp,
                C.c_double, _dp, _dp, _dp, _ip)
 _advance = _sig("orc_dem_advance", None, C.POINTER(DemParams), _dp, _dp, _dp, _dp, _dp, _dp, _dp)
 _kick = _sig("orc_dem_kick", None, C.POINTER(DemParams), _dp, _dp, _dp, C.c_void_p, C.c_void_p, _dp, _dp, _dp, _dp)
-_psm_step = _sig("orc_psm_step", None, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, _ip, _dp, C.c_int, _dp, _dp, _dp, _dp,
+_psm_step = _sig("orc_psm_step", None, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int, _ip, _dp, C.c_int, _dp, _dp, _dp, _dp,
                  _dp, _dp, _dp, _dp, _ip, _ip)
 _psm_beta = _sig("orc_psm_beta", C.c_double, C.c_double, C.c_double)
 _psm_B = _sig("orc_psm_B", C.c_double, C.c_double, C.c_double)
 _psm_rc = _sig("orc_psm_rc", C.c_double)
-_psm_beta_sum = _sig("orc_psm_beta_sum", C.c_double, C.c_int, C.c_int, C.c_int, _ip, _dp, C.c_double)
+_psm_beta_sum = _sig("orc_psm_beta_sum", C.c_double, C.c_int, C.c_int, C.c_int, _ip, _dp, C.c_double, C.c_int)
+_psm_beta_subdiv = _sig("orc_psm_beta_subdiv", C.c_double, _dp, C.c_double, C.c_int)
 
 
 def _ptr(a):
@@ -224,11 +225,16 @@ def psm_B(beta, tau):
     return _psm_B(beta, tau)
 
 
-def psm_beta_sum(shape, bc, xk, Rk):
-    return _psm_beta_sum(shape[0], shape[1], shape[2], np.asarray(bc, np.int32), _f64(xk), Rk)
+def psm_beta_sum(shape, bc, xk, Rk, subdiv=0):
+    return _psm_beta_sum(shape[0], shape[1], shape[2], np.asarray(bc, np.int32), _f64(xk), Rk, int(subdiv))
 
 
-def psm_step(shape, f, tau, bc, u_wall, xk, vk, wk, Rk, trt=False):
+def psm_beta_subdiv(d, Rk, ns=10):
+    """Eq. (38): d = r_j - r_k (cell centre minus sphere centre), ns points per direction."""
+    return _psm_beta_subdiv(_f64(d), Rk, int(ns))
+
+
+def psm_step(shape, f, tau, bc, u_wall, xk, vk, wk, Rk, trt=False, subdiv=0):
     """One PSM collide-and-stream step in lattice units (Eq. 32-42).
     Returns f_new [19,N], F [np,3], M [np,3], status."""
     nx, ny, nz = shape
@@ -240,7 +246,7 @@ def psm_step(shape, f, tau, bc, u_wall, xk, vk, wk, Rk, trt=False):
     status = np.zeros(1, np.int32)
     uw = np.zeros(18) if u_wall is None else _f64(u_wall).ravel()
     pad = lambda a, k: _f64(a).reshape(-1) if n else np.zeros(k)
-    _psm_step(nx, ny, nz, tau, trt_omega_minus(1.0 / tau) if trt else -1.0, np.asarray(bc, np.int32), uw, n, pad(xk, 3), pad(vk, 3), pad(wk, 3), pad(Rk, 1),
+    _psm_step(nx, ny, nz, tau, trt_omega_minus(1.0 / tau) if trt else -1.0, int(subdiv), np.asarray(bc, np.int32), uw, n, pad(xk, 3), pad(vk, 3), pad(wk, 3), pad(Rk, 1),
               f, f_out, F, M, slots, status)
     return f_out, F[:n], M[:n], int(status[0])
 
@@ -276,7 +282,7 @@ class Coupled:
             wk = d.wp * Dt
             Rk = d.R / dx
             self.f, F, M, st = psm_step(lbm["shape"], self.f, lbm["tau"], lbm["bc"], lbm.get("u_wall"), xk, vk, wk, Rk,
-                                        trt=bool(lbm.get("collision", 0)))
+                                        trt=bool(lbm.get("collision", 0)), subdiv=10 if cpl.get("solid_fraction", 0) else 0)
             self.status |= st
             self.F_sf = F * (rho_f * dx ** 4 / Dt ** 2)
             self.M_sf = M * (rho_f * dx ** 5 / Dt ** 2)

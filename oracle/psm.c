@@ -9,7 +9,7 @@
  *   solid operator       PAPER.md:281      Eq. (34), overbar restored (reading G21)
  *   solid velocity       PAPER.md:285      Eq. (35), sign/index reading G22
  *   weighting            PAPER.md:289-295  Eq. (36), (37); only B_tot truncated (G23)
- *   solid fraction       PAPER.md:307-310  Eq. (39), (40) distance-based
+ *   solid fraction       PAPER.md:307-310  Eq. (39), (40) distance-based; Eq. (38) subdivision
  *   force / torque       PAPER.md:320-322  Eq. (41), (42), pre-collision f (G26)
  *   n_s <= 2 per cell    PAPER.md:515      the two lowest ids with beta > 0 (G24)
  *
@@ -56,6 +56,36 @@ double orc_psm_beta(double Rk, double dist)
     return dsc / (2.0 * Rc);
 }
 
+/* Eq. (38), subdivision method: fraction of the ns^3 points s_i = r_j + ((a + 1/2)/ns - 1/2) (a = 0..ns-1 per
+ * axis, "spread evenly inside the cell") that lie inside the sphere.  d = r_j - r_k. */
+double orc_psm_beta_subdiv(const double *d, double Rk, int ns)
+{
+    int count = 0;
+    double R2 = Rk * Rk;
+    for (int c = 0; c < ns; ++c) {
+        double sz = d[2] + (((double)c + 0.5) / (double)ns - 0.5);
+        for (int b = 0; b < ns; ++b) {
+            double sy = d[1] + (((double)b + 0.5) / (double)ns - 0.5);
+            for (int a = 0; a < ns; ++a) {
+                double sx = d[0] + (((double)a + 0.5) / (double)ns - 0.5);
+                if (sx * sx + sy * sy + sz * sz < R2) ++count;
+            }
+        }
+    }
+    return (double)count / (double)(ns * ns * ns);
+}
+
+/* solid fraction of the cell whose centre is at d = r_j - r_k: subdiv = 0 distance-based (Eq. 39-40),
+ * subdiv = ns > 0 subdivision with ns points per direction (Eq. 38) */
+static double beta_of(const double *d, double Rk, int subdiv)
+{
+    if (subdiv > 0) return orc_psm_beta_subdiv(d, Rk, subdiv);
+    return orc_psm_beta(Rk, sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]));
+}
+
+/* how far from the sphere centre a cell centre can be and still have beta > 0 */
+static double reach_of(double Rk, int subdiv) { return subdiv > 0 ? Rk + 0.8661 : Rk + orc_psm_rc(); }
+
 /* Eq. (36) */
 double orc_psm_B(double beta, double tau) { return beta * (tau - 0.5) / ((1.0 - beta) + (tau - 0.5)); }
 
@@ -75,11 +105,10 @@ static void node_minus_centre(const int *n, const int *bc, const int *r, const d
  * optionally adding B_k Omega^s_{i,k} to fs[].  f = pre-collision populations. */
 static double solid_terms(const int *n, const int *bc, double tau, const int *r, const double *f,
                           double rho, const double *u, const double *xk, const double *vk, const double *wk,
-                          double Rk, double *d, double *sumOc, double *fs)
+                          double Rk, int subdiv, double *d, double *sumOc, double *fs)
 {
     node_minus_centre(n, bc, r, xk, d);
-    double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-    double beta = orc_psm_beta(Rk, dist);
+    double beta = beta_of(d, Rk, subdiv);
     double B = orc_psm_B(beta, tau);
     /* Eq. (35): u_k = v_k + w_k x (r_j - r_k) */
     double uk[3] = {vk[0] + (wk[1] * d[2] - wk[2] * d[1]),
@@ -103,19 +132,19 @@ static double solid_terms(const int *n, const int *bc, double tau, const int *r,
 double orc_collision(int i, const double *f, double rho, double ux, double uy, double uz, double omega, double omega_minus);
 
 /* omega_minus < 0: BGK; else the TRT model of Eq. (29)-(31) as Omega_i in Eq. (33) */
-void orc_psm_step(int nx, int ny, int nz, double tau, double omega_minus, const int *bc, const double *u_wall,
+void orc_psm_step(int nx, int ny, int nz, double tau, double omega_minus, int subdiv, const int *bc, const double *u_wall,
                   int np, const double *xk, const double *vk, const double *wk, const double *Rk,
                   const double *f_in, double *f_out, double *F, double *M, int *slots, int *status)
 {
     size_t N = (size_t)nx * ny * nz;
     int n[3] = {nx, ny, nz};
-    double Rc = orc_psm_rc(), omega = 1.0 / tau;
+    double omega = 1.0 / tau;
     tables();
     for (size_t c = 0; c < 2 * N; ++c) slots[c] = -1;
 
     /* (1) which solids cut which cell: ascending id, so a full cell keeps the two lowest */
     for (int k = 0; k < np; ++k) {
-        double reach = Rk[k] + Rc;
+        double reach = reach_of(Rk[k], subdiv);
         int lo[3], hi[3];
         for (int a = 0; a < 3; ++a) { lo[a] = (int)ceil(xk[3 * k + a] - reach); hi[a] = (int)floor(xk[3 * k + a] + reach); }
         for (int z = lo[2]; z <= hi[2]; ++z)
@@ -127,7 +156,7 @@ void orc_psm_step(int nx, int ny, int nz, double tau, double omega_minus, const 
                     if (!ok) continue;
                     double d[3];
                     node_minus_centre(n, bc, r, xk + 3 * k, d);
-                    if (orc_psm_beta(Rk[k], sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2])) <= 0.0) continue;
+                    if (beta_of(d, Rk[k], subdiv) <= 0.0) continue;
                     size_t c = ((size_t)r[2] * ny + r[1]) * nx + r[0];
                     if (slots[2 * c] < 0) slots[2 * c] = k;
                     else if (slots[2 * c] == k) {}
@@ -155,7 +184,7 @@ void orc_psm_step(int nx, int ny, int nz, double tau, double omega_minus, const 
                     int k = slots[2 * c + s];
                     if (k < 0) continue;
                     double d[3], soc[3];
-                    Bsum += solid_terms(n, bc, tau, r, f, rho, u, xk + 3 * k, vk + 3 * k, wk + 3 * k, Rk[k], d, soc, solid);
+                    Bsum += solid_terms(n, bc, tau, r, f, rho, u, xk + 3 * k, vk + 3 * k, wk + 3 * k, Rk[k], subdiv, d, soc, solid);
                 }
                 double Btot = Bsum < 1.0 ? Bsum : 1.0;                       /* Eq. (37) */
                 for (int i = 0; i < Q; ++i) {
@@ -169,7 +198,7 @@ void orc_psm_step(int nx, int ny, int nz, double tau, double omega_minus, const 
     /* (3) Eq. (41), (42): per-particle sums over the cells the solid occupies */
 #pragma omp parallel for schedule(dynamic, 16)
     for (int k = 0; k < np; ++k) {
-        double reach = Rk[k] + Rc, Fk[3] = {0, 0, 0}, Mk[3] = {0, 0, 0};
+        double reach = reach_of(Rk[k], subdiv), Fk[3] = {0, 0, 0}, Mk[3] = {0, 0, 0};
         int lo[3], hi[3];
         for (int a = 0; a < 3; ++a) { lo[a] = (int)ceil(xk[3 * k + a] - reach); hi[a] = (int)floor(xk[3 * k + a] + reach); }
         for (int z = lo[2]; z <= hi[2]; ++z)
@@ -187,7 +216,7 @@ void orc_psm_step(int nx, int ny, int nz, double tau, double omega_minus, const 
                         rho += f[i]; j[0] += f[i] * cx[i]; j[1] += f[i] * cy[i]; j[2] += f[i] * cz[i];
                     }
                     double u[3] = {j[0] / rho, j[1] / rho, j[2] / rho}, d[3], soc[3];
-                    double B = solid_terms(n, bc, tau, r, f, rho, u, xk + 3 * k, vk + 3 * k, wk + 3 * k, Rk[k], d, soc, NULL);
+                    double B = solid_terms(n, bc, tau, r, f, rho, u, xk + 3 * k, vk + 3 * k, wk + 3 * k, Rk[k], subdiv, d, soc, NULL);
                     double dF[3] = {-B * soc[0], -B * soc[1], -B * soc[2]};  /* Eq. (41) */
                     Fk[0] += dF[0]; Fk[1] += dF[1]; Fk[2] += dF[2];
                     Mk[0] += d[1] * dF[2] - d[2] * dF[1];                     /* Eq. (42) */
@@ -199,7 +228,7 @@ void orc_psm_step(int nx, int ny, int nz, double tau, double omega_minus, const 
 }
 
 /* per-cell total solid fraction sum_k beta_k (diagnostic for the volume pin) */
-double orc_psm_beta_sum(int nx, int ny, int nz, const int *bc, const double *xk, double Rk)
+double orc_psm_beta_sum(int nx, int ny, int nz, const int *bc, const double *xk, double Rk, int subdiv)
 {
     int n[3] = {nx, ny, nz};
     double s = 0.0;
@@ -209,7 +238,7 @@ double orc_psm_beta_sum(int nx, int ny, int nz, const int *bc, const double *xk,
                 int r[3] = {x, y, z};
                 double d[3];
                 node_minus_centre(n, bc, r, xk, d);
-                s += orc_psm_beta(Rk, sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]));
+                s += beta_of(d, Rk, subdiv);
             }
     return s;
 }
