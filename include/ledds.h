@@ -149,7 +149,8 @@ int ledds_dem_destroy(ledds_dem* h);
  * PAPER.md:258. */
 typedef struct {
     int n_sub;            /* DEM sub-steps per LBM step; LBM dt = n_sub * dem.dt                  */
-    int solid_fraction;   /* 0 = distance-based Eq. (39)-(40); others reserved                    */
+    int solid_fraction;   /* 0 = distance-based Eq. (39)-(40); 1 = subdivision Eq. (38), 10^3 points per
+                             cell: + 8 B x (2H+2)^3 of scratch per solid             */
     double dx;            /* lattice spacing in DEM length units                                  */
     double rho_f;         /* fluid reference density in DEM units (lattice rho = 1)               */
     double origin[3];     /* DEM coordinates of lattice node (0,0,0)                              */

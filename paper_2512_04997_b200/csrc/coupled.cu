@@ -43,6 +43,7 @@ __global__ void cpl_solid_kernel(const CplDev C)
 // the same way.  Every solid but the lowest is a loser exactly once, so y ends as the second lowest id
 // whatever the order of arrival (the two lowest ids), and a second loser is a third solid
 // (LEDDS_ST_SOLID_OVERFLOW).  Only cells shared by two solids pay the second atomic.
+template <bool SUBDIV>
 __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const CplDev C)
 {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -59,20 +60,34 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
     else ry = ry < 0 ? ry + P.ny : (ry >= P.ny ? ry - P.ny : ry);
     if (P.bc[2]) { if (rz < 0 || rz >= P.nz) return; }
     else rz = rz < 0 ? rz + P.nz : (rz >= P.nz ? rz - P.nz : rz);
-    // the cut cells of the row are the run [xa, xb] around x_k (the squared distance grows with |dx| also in
-    // floating point): estimate its ends, then settle them with the exact test
-    const double s = Rk + C.rc, h2 = s * s - (d[1] * d[1] + d[2] * d[2]);
-    if (h2 < -1e-9 * s * s) return;
-    const double w = sqrt(h2 > 0.0 ? h2 : 0.0);
     const int lo = fk[0] - C.H, hi = fk[0] + C.H + 1;                          // the box
-    int xa = max(lo, (int)ceil(xk[0] - w)), xb = min(hi, (int)floor(xk[0] + w));
+    int xa, xb;
     auto cuts = [&](int xi) { d[0] = (double)xi - xk[0]; return cpl_cuts(Rk, C.rc, d); };
-    if (xa > xb) { xa = xb = min(hi, max(lo, (int)floor(xk[0] + 0.5))); if (!cuts(xa)) return; }
-    while (xa <= xb && !cuts(xa)) ++xa;
-    while (xb >= xa && !cuts(xb)) --xb;
-    if (xa > xb) return;
-    while (xa > lo && cuts(xa - 1)) --xa;
-    while (xb < hi && cuts(xb + 1)) ++xb;
+    if (SUBDIV) {
+        // Eq. (38): beta of every cell of the row, kept in the solid's box; the cut cells (beta > 0) are a run
+        double* brow = C.betabox + ((size_t)k * S2 + r) * S;
+        xa = hi + 1; xb = lo - 1;
+        for (int xi = lo; xi <= hi; ++xi) {
+            d[0] = (double)xi - xk[0];
+            const double beta = cpl_beta_subdiv(d, Rk);
+            brow[xi - lo] = beta;
+            if (beta > 0.0) { xa = min(xa, xi); xb = max(xb, xi); }
+        }
+        if (xa > xb) return;
+    } else {
+        // the cut cells of the row are the run [xa, xb] around x_k (the squared distance grows with |dx| also in
+        // floating point): estimate its ends, then settle them with the exact test
+        const double s = Rk + C.rc, h2 = s * s - (d[1] * d[1] + d[2] * d[2]);
+        if (h2 < -1e-9 * s * s) return;
+        const double w = sqrt(h2 > 0.0 ? h2 : 0.0);
+        xa = max(lo, (int)ceil(xk[0] - w)); xb = min(hi, (int)floor(xk[0] + w));
+        if (xa > xb) { xa = xb = min(hi, max(lo, (int)floor(xk[0] + 0.5))); if (!cuts(xa)) return; }
+        while (xa <= xb && !cuts(xa)) ++xa;
+        while (xb >= xa && !cuts(xb)) --xb;
+        if (xa > xb) return;
+        while (xa > lo && cuts(xa - 1)) --xa;
+        while (xb < hi && cuts(xb + 1)) ++xb;
+    }
     bool overflow = false;
     uint2* const row = C.slots + ((long long)rz * P.ny + ry) * P.nx;
     for (int x0 = xa; x0 <= xb; x0 += RASTER_BATCH) {
@@ -99,7 +114,7 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
 // thread's column of shared memory with asynchronous copies (no registers tied up while they are in flight);
 // the moments are summed from there and the collision runs pair by pair, each pair pushed as soon as it is
 // collided.  The kernel needs <= 64 registers, so 8 blocks (32 warps) are resident per SM.
-template <typename I, int BX, bool TRT>
+template <typename I, int BX, bool TRT, bool SUBDIV>
 __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
                                                                const __grid_constant__ LbmDev P,
                                                                const __grid_constant__ CplDev C)
@@ -144,7 +159,7 @@ __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(cons
     if (two) {                                                                        // warp-uniform, rarer
         double B1, uk1[3], rec[6];
         int ent;
-        psm_solid_terms(P, C, x, y, z, id1, rho, ux, uy, uz, B1, uk1, rec, ent);
+        psm_solid_terms<SUBDIV>(P, C, x, y, z, id1, rho, ux, uy, uz, B1, uk1, rec, ent);
         s2col[0] = B1;
         s2col[PSM_BLOCK] = 1.0 - 1.5 * (uk1[0] * uk1[0] + uk1[1] * uk1[1] + uk1[2] * uk1[2]);
         s2col[2 * PSM_BLOCK] = uk1[0]; s2col[3 * PSM_BLOCK] = uk1[1]; s2col[4 * PSM_BLOCK] = uk1[2];
@@ -154,20 +169,27 @@ __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(cons
     {
         double rec[6];
         int ent;
-        psm_solid_terms(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
+        psm_solid_terms<SUBDIV>(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
         psm_run_reduce(C, id0, ent, rec);
     }
     psm_collide_stream<I, TRT>(sf, P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
 }
 
-template <typename I, bool TRT>
-static void psm_launch(const double* src, double* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
+template <typename I, bool TRT, bool SUBDIV>
+static void psm_launch2(const double* src, double* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
 {
     const int bx = lb_block_x(d.nx), rows = PSM_BLOCK / bx;
     const dim3 block(PSM_BLOCK), grid((d.nx + bx - 1) / bx, (d.ny + rows - 1) / rows, d.nz);
-    if (bx == 128) lbm_psm_kernel<I, 128, TRT><<<grid, block, 0, st>>>(src, dst, d, C);
-    else if (bx == 64) lbm_psm_kernel<I, 64, TRT><<<grid, block, 0, st>>>(src, dst, d, C);
-    else lbm_psm_kernel<I, 32, TRT><<<grid, block, 0, st>>>(src, dst, d, C);
+    if (bx == 128) lbm_psm_kernel<I, 128, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
+    else if (bx == 64) lbm_psm_kernel<I, 64, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
+    else lbm_psm_kernel<I, 32, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
+}
+
+template <typename I, bool TRT>
+static void psm_launch(const double* src, double* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
+{
+    if (C.subdiv) psm_launch2<I, TRT, true>(src, dst, d, C, st);
+    else psm_launch2<I, TRT, false>(src, dst, d, C, st);
 }
 
 // ------------------------------------------------------------------------------------ finish
@@ -185,14 +207,14 @@ __global__ void cpl_finish_kernel(const CplDev C, double* __restrict__ f_hyd, do
 }
 
 // ------------------------------------------------------------------------------------ host API
-struct CplLayout { size_t slots, sol, acc, total; };
+struct CplLayout { size_t slots, sol, acc, betabox, total; };
 
 static size_t cpl_align(size_t v) { return (v + 255) & ~(size_t)255; }
 
 static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_params* c, double r_max, CplDev* C,
                      CplLayout* L)
 {
-    if (!lbm || !dem || !c || c->n_sub < 1 || c->solid_fraction != 0 || !(c->dx > 0.0) || !(c->rho_f > 0.0) || !(r_max > 0.0))
+    if (!lbm || !dem || !c || c->n_sub < 1 || (c->solid_fraction != 0 && c->solid_fraction != 1) || !(c->dx > 0.0) || !(c->rho_f > 0.0) || !(r_max > 0.0))
         return LEDDS_EINVAL;
     const double rc = cbrt(3.0 / (4.0 * 3.14159265358979323846));           // Eq. (40), dx = 1
     const double Dt = c->n_sub * dem->d.dt;
@@ -205,7 +227,9 @@ static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl
     C->fscale = c->rho_f * pow(c->dx, 4) / (Dt * Dt);
     C->mscale = c->rho_f * pow(c->dx, 5) / (Dt * Dt);
     const int nl[3] = {lbm->d.nx, lbm->d.ny, lbm->d.nz};
-    C->H = (int)ceil(r_max / c->dx + rc);
+    C->subdiv = c->solid_fraction ? PSM_NSUB : 0;
+    // a cell is cut when its centre is closer than R + r_c (Eq. 40) / when one of its sample points is inside (Eq. 38)
+    C->H = (int)ceil(r_max / c->dx + (C->subdiv ? 0.8661 : rc));
     C->S = 2 * C->H + 2;
     if (C->S > 256) return LEDDS_EINVAL;
     for (int a = 0; a < 3; ++a) {
@@ -217,7 +241,8 @@ static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl
     L->slots = 0;
     L->sol = cpl_align(N * sizeof(uint2));
     L->acc = L->sol + cpl_align((size_t)C->n * 10 * sizeof(double));
-    L->total = L->acc + cpl_align((size_t)C->n * 12 * sizeof(unsigned long long));
+    L->betabox = L->acc + cpl_align((size_t)C->n * 12 * sizeof(unsigned long long));
+    L->total = L->betabox + (C->subdiv ? cpl_align((size_t)C->n * C->S * C->S * C->S * sizeof(double)) : 0);
     return LEDDS_OK;
 }
 
@@ -245,7 +270,7 @@ extern "C" int ledds_cpl_init(const ledds_lbm* lbm, const ledds_dem* dem, const 
     cudaStream_t st = (cudaStream_t)stream;
     char* base = static_cast<char*>(cpl_scratch);
     if (cudaMemsetAsync(base + L.slots, 0xff, L.sol - L.slots, st) != cudaSuccess ||        // all slots PSM_EMPTY
-        cudaMemsetAsync(base + L.acc, 0, L.total - L.acc, st) != cudaSuccess)               // accumulators at zero
+        cudaMemsetAsync(base + L.acc, 0, L.betabox - L.acc, st) != cudaSuccess)             // accumulators at zero
         return LEDDS_ECUDA;
     return LEDDS_OK;
 }
@@ -276,6 +301,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
     C.slots = reinterpret_cast<uint2*>(cs + L.slots);
     C.sol = reinterpret_cast<double*>(cs + L.sol);
     C.acc = reinterpret_cast<unsigned long long*>(cs + L.acc);
+    C.betabox = C.subdiv ? reinterpret_cast<double*>(cs + L.betabox) : nullptr;
     C.status = status;
     const LbmDev& d = lbm->d;
     const size_t half = (size_t)LEDDS_Q * d.N;
@@ -296,7 +322,9 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         if (C.n > 0) {
             cpl_solid_kernel<<<(C.n + 127) / 128, 128, 0, st>>>(C);
             ledds_count_launch(1);
-            cpl_raster_kernel<<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(d, C);
+            const unsigned rb = (unsigned)(((long long)C.n * C.S * C.S + 255) / 256);
+            if (C.subdiv) cpl_raster_kernel<true><<<rb, 256, 0, st>>>(d, C);
+            else cpl_raster_kernel<false><<<rb, 256, 0, st>>>(d, C);
         }
         ledds_prof_stop(LEDDS_K_CPL_RASTER, st);
         LEDDS_CHECK_LAUNCH();

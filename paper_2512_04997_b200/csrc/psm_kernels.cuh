@@ -13,6 +13,8 @@
 //                       when free.  Written by cpl_raster_kernel, consumed and reset by lbm_psm_kernel,
 //                       so it is all-empty between steps.
 //   sol[n][10]          per solid, lattice units: x_k[3], R_k, v_k[3], w_k[3] (predictor values)
+//   betabox[n][S^3]     double: solid fraction of Eq. (38) per (solid, cell of its bounding box); only allocated
+//                       and used with the subdivision method (written by the raster, read by the collide kernel)
 //   acc[n][6][2]        uint64: per solid and component of (F, M), the exact sum of the (cell, solid) terms of
 //                       Eq. (41)-(42) in 2^-83 fixed point (two limbs: units of 2^-30 and of 2^-83).  Integer
 //                       additions commute, so the sum does not depend on the order in which blocks finish;
@@ -23,6 +25,8 @@ struct CplDev {
     double inv_dx, vscale, wscale, origin[3];
     double fscale, mscale;     // lattice -> DEM units for force / torque
     int H, S;                  // half-width and width of the solid's bounding box in cells (raster)
+    int subdiv;                // 0: distance-based solid fraction Eq. (39)-(40); else points per direction of Eq. (38)
+    double* betabox;           // [n][S^3] solid fraction per (solid, cell of its box), subdivision method only
     const double* x; const double* vp; const double* wp; const double* radius;   // particle order, DEM units
     uint2* slots;
     double* sol;
@@ -62,9 +66,42 @@ __device__ __forceinline__ bool cpl_cuts(double Rk, double rc, const double* d)
     return __dsub_rn(s, __dsqrt_rn(d2)) > 0.0;
 }
 
+// Eq. (38), subdivision method with PSM_NSUB points per direction at r_j + ((a + 1/2)/NSUB - 1/2); d = r_j - r_k.
+// Each point is tested as the oracle tests it (explicitly rounded operations), so the count is the same; cells
+// whose farthest point is inside / nearest point is outside need no count (rounding is monotone).
+#define PSM_NSUB 10
+__device__ __forceinline__ double cpl_beta_subdiv(const double* d, double Rk)
+{
+    const double R2 = __dmul_rn(Rk, Rk);
+    double s2[3][PSM_NSUB], lo2[3], hi2[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        lo2[a] = 1.0e300; hi2[a] = 0.0;
+#pragma unroll
+        for (int i = 0; i < PSM_NSUB; ++i) {
+            const double off = __dsub_rn(__ddiv_rn((double)i + 0.5, (double)PSM_NSUB), 0.5);
+            const double sv = __dadd_rn(d[a], off);
+            s2[a][i] = __dmul_rn(sv, sv);
+            lo2[a] = fmin(lo2[a], s2[a][i]);
+            hi2[a] = fmax(hi2[a], s2[a][i]);
+        }
+    }
+    if (__dadd_rn(__dadd_rn(hi2[0], hi2[1]), hi2[2]) < R2) return 1.0;
+    if (!(__dadd_rn(__dadd_rn(lo2[0], lo2[1]), lo2[2]) < R2)) return 0.0;
+    int count = 0;
+    for (int c = 0; c < PSM_NSUB; ++c)
+        for (int b = 0; b < PSM_NSUB; ++b) {
+#pragma unroll
+            for (int a = 0; a < PSM_NSUB; ++a)
+                count += __dadd_rn(__dadd_rn(s2[0][a], s2[1][b]), s2[2][c]) < R2;
+        }
+    return (double)count / (double)(PSM_NSUB * PSM_NSUB * PSM_NSUB);
+}
+
 // What one solid does to one cell: weight B (Eq. 36, 39-40), solid velocity at the cell (Eq. 35), the terms
 // of Eq. (41)-(42) in lattice units (rec) and the index of the cell in the solid's box (ent).
 // id = PSM_EMPTY: no solid here: B = 0, rec = 0, ent = -1 (the lane still runs the code of its warp).
+template <bool SUBDIV>
 __device__ __forceinline__ void psm_solid_terms(const LbmDev& P, const CplDev& C, int x, int y, int z, uint32_t id,
                                                 double rho, double ux, double uy, double uz, double& B,
                                                 double (&uk)[3], double (&rec)[6], int& ent)
@@ -82,10 +119,15 @@ __device__ __forceinline__ void psm_solid_terms(const LbmDev& P, const CplDev& C
 #pragma unroll
     for (int a = 0; a < 3; ++a) d[a] = (double)(fk[a] + di[a]) - xk[a];              // r_j - r_k, nearest image
     ent = has ? ((di[2] + C.H) * C.S + (di[1] + C.H)) * C.S + (di[0] + C.H) : -1;
-    const double dsc = cpl_dsc(Rk, C.rc, cpl_dist(d));
-    double beta = dsc * C.inv_2rc;                                                   // Eq. (39)-(40)
-    beta = beta > 1.0 ? 1.0 : beta;
-    beta = (has && beta > 0.0) ? beta : 0.0;
+    double beta;
+    if (SUBDIV) {
+        beta = has ? C.betabox[(size_t)k * (size_t)(C.S * C.S * C.S) + (size_t)ent] : 0.0;   // Eq. (38), from the raster
+    } else {
+        const double dsc = cpl_dsc(Rk, C.rc, cpl_dist(d));
+        beta = dsc * C.inv_2rc;                                                      // Eq. (39)-(40)
+        beta = beta > 1.0 ? 1.0 : beta;
+        beta = (has && beta > 0.0) ? beta : 0.0;
+    }
     B = beta * (P.tau - 0.5) / ((1.0 - beta) + (P.tau - 0.5));                        // Eq. (36)
     uk[0] = vk[0] + (wk[1] * d[2] - wk[2] * d[1]);                                   // Eq. (35)
     uk[1] = vk[1] + (wk[2] * d[0] - wk[0] * d[2]);

@@ -191,3 +191,24 @@ def test_trt_coupled_step():
     compare(o, g)
     o.step(5); g.step(5)
     compare(o, g)
+
+
+@pytest.mark.parametrize("collision", [0, 1])
+def test_subdivision_solid_fraction(collision):
+    # Eq. (38), 10^3 points per cell (the paper's validation setting), with BGK and with TRT: the counts are
+    # integers, so the weights must agree exactly and the step to the usual tolerances
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=8, n=64, n_part=70, R=4.0)
+    cpl = dict(cpl, solid_fraction=1)
+    o, g = both(dict(lbm, collision=collision), cpl, pd, x, v, w, R, u)
+    o.step(1); g.step(1)
+    compare(o, g)
+    o.step(3); g.step(3)
+    compare(o, g)
+    assert np.abs(o.F_sf).max() > 0
+
+
+def test_subdivision_single_sphere_walls():
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(32, 32, 48), R=5.3, z0=30.0, g=1e-3)
+    o, g = both(lbm, dict(cpl, solid_fraction=1), pd, x, v, w, R)
+    o.step(6); g.step(6)
+    compare(o, g)
