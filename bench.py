@@ -243,6 +243,23 @@ def run_ours(args, rank, world):
         sub["cfg2_lbm_tgv128_trt"] = {"mlups": round(nc2 / ms2t / 1e3, 1), "ms_per_step": round(ms2t, 5), "steps": ks,
                                        "hbm_gbs": round(304.0 * nc2 / ms2t / 1e6, 1), "hbm_frac": round(304.0 * nc2 / ms2t / 1e6 / peak, 4)}
         del gt
+        # the paper's own validation combination on the headline workload: TRT collision (Eq. 29-31) + subdivision
+        # solid fraction (Eq. 38, 10^3 points per cell)
+        if not args.sub_large_only:
+            lbv, cpv, pdv, xv, vv, wv, Rv, uv = make_cfg4(small)
+            glv = Lbm(dict(lbv, collision=1), None, uv); gdv = Dem(pdv, xv, vv, wv, Rv)
+            gv = Coupled(glv, gdv, dict(cpv, solid_fraction=1), float(Rv.max()))
+            gv.step(3); torch.cuda.synchronize()
+            L.ledds_profile(True)
+            msv = timed(gv.step, 10) / 10
+            prv = {nm: round(L.ledds_profile_read(i)[0] / 10, 5) for i, nm in enumerate(L.KERNEL_GROUPS) if nm in ("lbm", "cpl_raster", "cpl_reduce")}
+            L.ledds_profile(False)
+            ncv = int(np.prod(lbv["shape"]))
+            sub["cfg4_trt_subdivision"] = {"mlups": round(ncv / msv / 1e3, 1), "ms_per_step": round(msv, 5), "steps": 10,
+                                           "kernel_ms_per_step": prv, "status_word": int(gdv.status[0].item()),
+                                           "note": "TRT + Eq. 38 with 1000 points per cell: the raster counts points for every boundary cell"}
+            del gv, glv, gdv
+            torch.cuda.empty_cache()
         # configs[0] and configs[2]: small, launch-latency-bound workloads, timed plainly and replayed from a CUDA
         # graph (the library only enqueues on the caller's stream, so its calls can be captured)
         small_cfgs = not args.sub_large_only

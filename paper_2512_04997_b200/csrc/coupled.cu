@@ -37,6 +37,58 @@ __global__ void cpl_solid_kernel(const CplDev C)
     o[3] = C.radius[k] * C.inv_dx;
 }
 
+// Eq. (38) in two kernels: every (solid, cell of its bounding box) is classified from its nearest and farthest
+// sample point (all inside: 1, all outside: 0); the cells the surface crosses go to a list, and the second kernel
+// counts their 10^3 points with one thread per listed cell, so that its warps hold only cells that need it.
+__device__ __forceinline__ void cpl_box_cell(const CplDev& C, long long t, double* d, double& Rk)
+{
+    const int S = C.S, S3 = S * S * S;
+    const int k = (int)(t / S3);
+    const int e = (int)(t - (long long)k * S3), lz = e / (S * S), ly = (e / S) % S, lx = e % S;
+    const double* o = C.sol + (size_t)k * 10;
+    d[0] = (double)((int)floor(o[0]) + lx - C.H) - o[0];
+    d[1] = (double)((int)floor(o[1]) + ly - C.H) - o[1];
+    d[2] = (double)((int)floor(o[2]) + lz - C.H) - o[2];
+    Rk = o[3];
+}
+
+__global__ void __launch_bounds__(256) cpl_beta_classify_kernel(const CplDev C)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool in = t < (long long)C.n * C.S * C.S * C.S;
+    double beta = 0.0;
+    if (in) {
+        double d[3], Rk;
+        cpl_box_cell(C, t, d, Rk);
+        SubdivPoints p;
+        cpl_subdiv_points(d, Rk, p);
+        beta = cpl_beta_classify(p);
+        C.betabox[t] = beta;
+    }
+    const bool todo = in && beta < 0.0;
+    const unsigned m = __ballot_sync(0xffffffffu, todo);                            // one list append per warp
+    if (m) {
+        const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+        uint32_t base = 0;
+        if (lane == leader) base = atomicAdd(C.blist, (uint32_t)__popc(m));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (todo) C.blist[1 + base + __popc(m & ((1u << lane) - 1u))] = (uint32_t)t;
+    }
+}
+
+__global__ void __launch_bounds__(256, 3) cpl_beta_count_kernel(const CplDev C)
+{
+    const uint32_t count = C.blist[0];
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < count; i += gridDim.x * blockDim.x) {
+        const long long t = C.blist[1 + i];
+        double d[3], Rk;
+        cpl_box_cell(C, t, d, Rk);
+        SubdivPoints p;
+        cpl_subdiv_points(d, Rk, p);
+        C.betabox[t] = cpl_beta_count(p);
+    }
+}
+
 // thread t -> solid k = t / S^2, row (ly, lz) = t % S^2 of its box.
 // Every cut cell gets slots[cell].x = min(x, k).  The value that was there tells who lost the cell: the
 // newcomer if a lower id was already in, else the id it displaced; the loser is entered into slots[cell].y
@@ -65,14 +117,10 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
     auto cuts = [&](int xi) { d[0] = (double)xi - xk[0]; return cpl_cuts(Rk, C.rc, d); };
     if (SUBDIV) {
         // Eq. (38): beta of every cell of the row, kept in the solid's box; the cut cells (beta > 0) are a run
-        double* brow = C.betabox + ((size_t)k * S2 + r) * S;
+        const double* brow = C.betabox + ((size_t)k * S2 + r) * S;
         xa = hi + 1; xb = lo - 1;
-        for (int xi = lo; xi <= hi; ++xi) {
-            d[0] = (double)xi - xk[0];
-            const double beta = cpl_beta_subdiv(d, Rk);
-            brow[xi - lo] = beta;
-            if (beta > 0.0) { xa = min(xa, xi); xb = max(xb, xi); }
-        }
+        for (int xi = lo; xi <= hi; ++xi)                                       // written by cpl_beta_kernel
+            if (brow[xi - lo] > 0.0) { xa = min(xa, xi); xb = max(xb, xi); }
         if (xa > xb) return;
     } else {
         // the cut cells of the row are the run [xa, xb] around x_k (the squared distance grows with |dx| also in
@@ -197,6 +245,7 @@ static void psm_launch(const double* src, double* dst, const LbmDev& d, const Cp
 __global__ void cpl_finish_kernel(const CplDev C, double* __restrict__ f_hyd, double* __restrict__ m_hyd)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t == 0) C.blist[0] = 0u;                                                     // the subdivision list is worked through
     if (t >= 6 * C.n) return;
     const int k = t / 6, c = t - 6 * k;
     unsigned long long* a = C.acc + (size_t)t * 2;
@@ -207,7 +256,7 @@ __global__ void cpl_finish_kernel(const CplDev C, double* __restrict__ f_hyd, do
 }
 
 // ------------------------------------------------------------------------------------ host API
-struct CplLayout { size_t slots, sol, acc, betabox, total; };
+struct CplLayout { size_t slots, sol, acc, blist, betabox, total; };
 
 static size_t cpl_align(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -241,8 +290,11 @@ static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl
     L->slots = 0;
     L->sol = cpl_align(N * sizeof(uint2));
     L->acc = L->sol + cpl_align((size_t)C->n * 10 * sizeof(double));
-    L->betabox = L->acc + cpl_align((size_t)C->n * 12 * sizeof(unsigned long long));
-    L->total = L->betabox + (C->subdiv ? cpl_align((size_t)C->n * C->S * C->S * C->S * sizeof(double)) : 0);
+    const size_t box = (size_t)C->n * C->S * C->S * C->S;
+    if (C->subdiv && box >= 0xffffffffull) return LEDDS_EINVAL;
+    L->blist = L->acc + cpl_align((size_t)C->n * 12 * sizeof(unsigned long long));      // zeroed with acc at init
+    L->betabox = L->blist + (C->subdiv ? cpl_align((box + 1) * sizeof(uint32_t)) : 256);
+    L->total = L->betabox + (C->subdiv ? cpl_align(box * sizeof(double)) : 0);
     return LEDDS_OK;
 }
 
@@ -270,7 +322,7 @@ extern "C" int ledds_cpl_init(const ledds_lbm* lbm, const ledds_dem* dem, const 
     cudaStream_t st = (cudaStream_t)stream;
     char* base = static_cast<char*>(cpl_scratch);
     if (cudaMemsetAsync(base + L.slots, 0xff, L.sol - L.slots, st) != cudaSuccess ||        // all slots PSM_EMPTY
-        cudaMemsetAsync(base + L.acc, 0, L.betabox - L.acc, st) != cudaSuccess)             // accumulators at zero
+        cudaMemsetAsync(base + L.acc, 0, L.blist + 256 - L.acc, st) != cudaSuccess)         // accumulators, list count
         return LEDDS_ECUDA;
     return LEDDS_OK;
 }
@@ -302,6 +354,7 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
     C.sol = reinterpret_cast<double*>(cs + L.sol);
     C.acc = reinterpret_cast<unsigned long long*>(cs + L.acc);
     C.betabox = C.subdiv ? reinterpret_cast<double*>(cs + L.betabox) : nullptr;
+    C.blist = reinterpret_cast<uint32_t*>(cs + L.blist);
     C.status = status;
     const LbmDev& d = lbm->d;
     const size_t half = (size_t)LEDDS_Q * d.N;
@@ -323,7 +376,12 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
             cpl_solid_kernel<<<(C.n + 127) / 128, 128, 0, st>>>(C);
             ledds_count_launch(1);
             const unsigned rb = (unsigned)(((long long)C.n * C.S * C.S + 255) / 256);
-            if (C.subdiv) cpl_raster_kernel<true><<<rb, 256, 0, st>>>(d, C);
+            if (C.subdiv) {
+                cpl_beta_classify_kernel<<<(unsigned)(((long long)C.n * C.S * C.S * C.S + 255) / 256), 256, 0, st>>>(C);
+                cpl_beta_count_kernel<<<148 * 6, 256, 0, st>>>(C);
+                ledds_count_launch(2);
+                cpl_raster_kernel<true><<<rb, 256, 0, st>>>(d, C);
+            }
             else cpl_raster_kernel<false><<<rb, 256, 0, st>>>(d, C);
         }
         ledds_prof_stop(LEDDS_K_CPL_RASTER, st);

@@ -27,6 +27,7 @@ struct CplDev {
     int H, S;                  // half-width and width of the solid's bounding box in cells (raster)
     int subdiv;                // 0: distance-based solid fraction Eq. (39)-(40); else points per direction of Eq. (38)
     double* betabox;           // [n][S^3] solid fraction per (solid, cell of its box), subdivision method only
+    uint32_t* blist;           // [0] = count, [1..]: box-cell indices k S^3 + e whose points have to be counted
     const double* x; const double* vp; const double* wp; const double* radius;   // particle order, DEM units
     uint2* slots;
     double* sol;
@@ -70,30 +71,43 @@ __device__ __forceinline__ bool cpl_cuts(double Rk, double rc, const double* d)
 // Each point is tested as the oracle tests it (explicitly rounded operations), so the count is the same; cells
 // whose farthest point is inside / nearest point is outside need no count (rounding is monotone).
 #define PSM_NSUB 10
-__device__ __forceinline__ double cpl_beta_subdiv(const double* d, double Rk)
+struct SubdivPoints { double s2[3][PSM_NSUB], lo2[3], hi2[3], R2; };
+
+__device__ __forceinline__ void cpl_subdiv_points(const double* d, double Rk, SubdivPoints& p)
 {
-    const double R2 = __dmul_rn(Rk, Rk);
-    double s2[3][PSM_NSUB], lo2[3], hi2[3];
+    p.R2 = __dmul_rn(Rk, Rk);
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        lo2[a] = 1.0e300; hi2[a] = 0.0;
+        p.lo2[a] = 1.0e300; p.hi2[a] = 0.0;
 #pragma unroll
         for (int i = 0; i < PSM_NSUB; ++i) {
-            const double off = __dsub_rn(__ddiv_rn((double)i + 0.5, (double)PSM_NSUB), 0.5);
+            const double off = ((double)i + 0.5) / (double)PSM_NSUB - 0.5;           // folded at compile time (IEEE, as the oracle's)
             const double sv = __dadd_rn(d[a], off);
-            s2[a][i] = __dmul_rn(sv, sv);
-            lo2[a] = fmin(lo2[a], s2[a][i]);
-            hi2[a] = fmax(hi2[a], s2[a][i]);
+            p.s2[a][i] = __dmul_rn(sv, sv);
+            p.lo2[a] = fmin(p.lo2[a], p.s2[a][i]);
+            p.hi2[a] = fmax(p.hi2[a], p.s2[a][i]);
         }
     }
-    if (__dadd_rn(__dadd_rn(hi2[0], hi2[1]), hi2[2]) < R2) return 1.0;
-    if (!(__dadd_rn(__dadd_rn(lo2[0], lo2[1]), lo2[2]) < R2)) return 0.0;
+}
+
+// 1 / 0 when every / no point is inside, -1 when the points have to be counted
+__device__ __forceinline__ double cpl_beta_classify(const SubdivPoints& p)
+{
+    if (__dadd_rn(__dadd_rn(p.hi2[0], p.hi2[1]), p.hi2[2]) < p.R2) return 1.0;
+    if (!(__dadd_rn(__dadd_rn(p.lo2[0], p.lo2[1]), p.lo2[2]) < p.R2)) return 0.0;
+    return -1.0;
+}
+
+__device__ __forceinline__ double cpl_beta_count(const SubdivPoints& p)
+{
     int count = 0;
-    for (int c = 0; c < PSM_NSUB; ++c)
-        for (int b = 0; b < PSM_NSUB; ++b) {
 #pragma unroll
-            for (int a = 0; a < PSM_NSUB; ++a)
-                count += __dadd_rn(__dadd_rn(s2[0][a], s2[1][b]), s2[2][c]) < R2;
+    for (int a = 0; a < PSM_NSUB; ++a)
+#pragma unroll
+        for (int b = 0; b < PSM_NSUB; ++b) {
+            const double sxy = __dadd_rn(p.s2[0][a], p.s2[1][b]);                   // (sx^2 + sy^2) + sz^2, as the oracle sums
+#pragma unroll
+            for (int c = 0; c < PSM_NSUB; ++c) count += __dadd_rn(sxy, p.s2[2][c]) < p.R2;
         }
     return (double)count / (double)(PSM_NSUB * PSM_NSUB * PSM_NSUB);
 }
