@@ -27,7 +27,8 @@ class DemParams(C.Structure):
                 ("v_wall", C.c_double * 18), ("cell", C.c_double), ("dt", C.c_double), ("g", C.c_double * 3),
                 ("density", C.c_double), ("kn", C.c_double), ("kt", C.c_double), ("restitution", C.c_double),
                 ("mu", C.c_double), ("kn_w", C.c_double), ("kt_w", C.c_double), ("restitution_w", C.c_double),
-                ("mu_w", C.c_double)]
+                ("mu_w", C.c_double), ("model", C.c_int), ("young", C.c_double), ("poisson", C.c_double),
+                ("young_w", C.c_double), ("poisson_w", C.c_double)]
 
 
 def dem_params(d: dict) -> DemParams:
@@ -40,6 +41,9 @@ def dem_params(d: dict) -> DemParams:
     p.kn = d["kn"]; p.kt = d["kt"]; p.restitution = d["restitution"]; p.mu = d["mu"]
     p.kn_w = d.get("kn_w", d["kn"]); p.kt_w = d.get("kt_w", d["kt"])
     p.restitution_w = d.get("restitution_w", d["restitution"]); p.mu_w = d.get("mu_w", d["mu"])
+    p.model = int(d.get("model", 0))
+    p.young = d.get("young", 0.0); p.poisson = d.get("poisson", 0.0)
+    p.young_w = d.get("young_w", p.young); p.poisson_w = d.get("poisson_w", p.poisson)
     return p
 
 

@@ -19,6 +19,7 @@
  *                                                with a surface velocity (G13)
  *   damping             PAPER.md:982-1001        beta of (A.5), m* of (A.9); linear
  *                                                spring reading G5
+ *   Hertz-Mindlin       PAPER.md:968-1001        (A.1)-(A.8), model = 1
  *   integration         PAPER.md:158-167, 188    Eq. (18a-c), (19d), (21a) (G11)
  *   pair list           PAPER.md:447-453, 492    unique pairs i<j sorted
  *                                                lexicographically
@@ -47,6 +48,8 @@ typedef struct {
     double dt, g[3], density;
     double kn, kt, restitution, mu;
     double kn_w, kt_w, restitution_w, mu_w;
+    int model;               /* 0 linear spring-dashpot (configs, G4); 1 Hertz-Mindlin coefficients (A.1)-(A.8) */
+    double young, poisson, young_w, poisson_w;   /* material of the spheres / of the walls */
 } orc_dem_params;
 
 #define PI 3.14159265358979323846
@@ -279,7 +282,24 @@ void orc_dem_forces(const orc_dem_params *p, const double *x, const double *v, c
             for (int a = 0; a < 3; ++a) vj[a] = p->v_wall[wl * 3 + a];
             kn = p->kn_w; kt = p->kt_w; z = zeta_w; mu = p->mu_w;
         }
-        double gn = 2.0 * z * sqrt(kn * mstar), gt = 2.0 * z * sqrt(kt * mstar);   /* reading G5 */
+        double gn, gt;
+        if (p->model == 1) {
+            /* Hertz-Mindlin coefficients of the pair.  (A.6) Y*, (A.7) G*, (A.8) R* (a wall is
+             * a sphere of infinite radius: R* = R_i), (A.1) k_n, k_t, (A.3)-(A.4) S_n, S_t, (A.2) gamma with
+             * beta of (A.5) = -zeta. */
+            double Ei = p->young, ni = p->poisson, Ej = wall ? p->young_w : p->young, nj = wall ? p->poisson_w : p->poisson;
+            double Ystar = 1.0 / ((1.0 - ni * ni) / Ei + (1.0 - nj * nj) / Ej);
+            double Gstar = 1.0 / (2.0 * (2.0 - ni) * (1.0 + ni) / Ei + 2.0 * (2.0 - nj) * (1.0 + nj) / Ej);
+            double Rstar = wall ? Ri : Ri * Rj / (Ri + Rj);
+            double sq = sqrt(Rstar * dn);
+            kn = (4.0 / 3.0) * Ystar * sq;
+            kt = 8.0 * Gstar * sq;
+            double Sn = 2.0 * Ystar * sq, St = 8.0 * Gstar * sq;
+            gn = 2.0 * sqrt(5.0 / 6.0) * z * sqrt(Sn * mstar);
+            gt = 2.0 * sqrt(5.0 / 6.0) * z * sqrt(St * mstar);
+        } else {
+            gn = 2.0 * z * sqrt(kn * mstar); gt = 2.0 * z * sqrt(kt * mstar);     /* reading G5 */
+        }
         /* Eq. (11): v_rel = (v_i - v_j) - (R_i w_i + R_j w_j) x e_n */
         double rw[3], rwxe[3], vrel[3];
         for (int a = 0; a < 3; ++a) rw[a] = Ri * w[3 * i + a] + Rj * wj[a];
