@@ -215,3 +215,68 @@ def test_history_is_dropped_when_contact_ends_and_restarts_from_zero():
             seen = True
             break
     assert seen
+
+
+# ---------------------------------------------------------------- Hertz-Mindlin coefficients (A.1-A.8)
+def hertz_pair(eps, E=1.0e7, nu=0.3, v0=0.1, R=0.5e-3, rho=2500.0, dt_frac=200.0):
+    """Two equal spheres head-on with the Hertz-Mindlin model.  Textbook Hertz impact [Landau-Lifshitz par. 9]:
+    delta_max = (15 m* v^2 / (16 Y* sqrt(R*)))^(2/5), t_c = 2.9432 delta_max / v (v = approach speed)."""
+    m = rho * 4.0 / 3.0 * np.pi * R ** 3
+    Ystar, Rstar, mstar, vrel = E / (2.0 * (1.0 - nu * nu)), R / 2.0, m / 2.0, 2.0 * v0
+    dmax = (15.0 * mstar * vrel ** 2 / (16.0 * Ystar * np.sqrt(Rstar))) ** 0.4
+    tc = 2.9432 * dmax / vrel
+    gap = 1e-3 * R
+    x = np.array([[-R - gap / 2, 0.0, 0.0], [R + gap / 2, 0.0, 0.0]])
+    v = np.array([[v0, 0, 0], [-v0, 0, 0]], float)
+    pd = W.dem_defaults(2, (-1, -1, -1), (1, 1, 1), (1, 1, 1), cell=0.5, dt=tc / dt_frac, g=(0, 0, 0), density=rho,
+                        kn=1.0, restitution=eps, mu=0.0, model=1, young=E, poisson=nu)
+    return pd, x, v, np.zeros((2, 3)), np.full(2, R), dict(m=m, Ystar=Ystar, Rstar=Rstar, dmax=dmax, tc=tc)
+
+
+def test_hertz_elastic_impact_overlap_and_duration():
+    pd, x, v, w, R, c = hertz_pair(1.0)
+    d = oracle.Dem(pd, x, v, w, R, pairs_mode="brute")
+    deepest, steps_in_contact = 0.0, 0
+    for _ in range(2000):
+        d.step()
+        if len(d.pairs):
+            steps_in_contact += 1
+            deepest = max(deepest, 2 * R[0] - (d.x[1, 0] - d.x[0, 0]))
+        elif steps_in_contact:
+            break
+    assert abs(deepest / c["dmax"] - 1.0) < 2e-3
+    assert abs(steps_in_contact * pd["dt"] / c["tc"] - 1.0) < 0.01
+    assert abs((d.v[1, 0] - d.v[0, 0]) / 0.2 - 1.0) < 1e-3                  # elastic: speeds are restored
+
+
+@pytest.mark.parametrize("eps", [0.5, 0.8])
+def test_hertz_restitution_equals_epsilon(eps):
+    # (A.2) with beta of (A.5) and S_n of (A.3) is built so that the restitution coefficient of a Hertzian
+    # contact is epsilon whatever the impact speed
+    for v0 in (0.05, 0.2):
+        pd, x, v, w, R, c = hertz_pair(eps, v0=v0, dt_frac=400.0)
+        d = oracle.Dem(pd, x, v, w, R, pairs_mode="brute")
+        run_until_separated(d)
+        assert abs((d.v[1, 0] - d.v[0, 0]) / (2 * v0) / eps - 1.0) < 0.01, (eps, v0)
+
+
+def test_hertz_normal_force_is_the_hertz_law_and_mindlin_ratio():
+    # static pair with overlap delta: F_n = 4/3 Y* sqrt(R*) delta^(3/2) (Hertz); one step of pure sliding by
+    # dt v_t gives F_t = -k_t delta_t with k_t / (dF_n/d delta) = 2 (1 - nu) / (2 - nu) (Mindlin)
+    E, nu, R, delta = 5.0e6, 0.25, 1.0e-3, 2.0e-6
+    Ystar, Rstar = E / (2 * (1 - nu * nu)), R / 2
+    x = np.array([[0.0, 0, 0], [2 * R - delta, 0, 0]])
+    z = np.zeros((2, 3))
+    pd = W.dem_defaults(2, (-1, -1, -1), (1, 1, 1), (1, 1, 1), cell=0.5, dt=1e-9, g=(0, 0, 0), density=2500.0,
+                        kn=1.0, restitution=1.0, mu=1e9, model=1, young=E, poisson=nu)
+    d = oracle.Dem(pd, x, z, z, np.full(2, R), pairs_mode="brute")
+    Fn = -d.F[0, 0]
+    assert abs(Fn / (4.0 / 3.0 * Ystar * np.sqrt(Rstar) * delta ** 1.5) - 1.0) < 1e-12
+    vt = 1.0e-3
+    d2 = oracle.Dem(pd, x, np.array([[0, vt, 0], [0, 0, 0.0]]), z, np.full(2, R), pairs_mode="brute")
+    d2.step()                                                  # delta_t = dt v_t (x moves by 1e-12 only)
+    en = (d2.x[0] - d2.x[1]) / np.linalg.norm(d2.x[0] - d2.x[1])      # the normal has turned by 5e-10: take F_n e_n out
+    Ft_y = d2.F[0, 1] - (d2.F[0] @ en) * en[1]
+    kt = -Ft_y / (pd["dt"] * vt)
+    Sn = 2.0 * Ystar * np.sqrt(Rstar * delta)                  # d F_n / d delta of the Hertz law
+    assert abs(kt / Sn / (2 * (1 - nu) / (2 - nu)) - 1.0) < 1e-5
