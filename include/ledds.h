@@ -114,6 +114,11 @@ typedef struct {
     double kn, kt, restitution, mu;          /* particle-particle spring-dashpot + Coulomb       */
     double kn_w, kt_w, restitution_w, mu_w;  /* particle-wall                                    */
     int max_contacts;              /* history slots per particle, 1..32 (walls included)         */
+    int model;                     /* 0 = linear spring-dashpot with the k, restitution above;
+                                      1 = Hertz-Mindlin coefficients per contact from the materials,
+                                      PAPER.md:968-1001 (A.1)-(A.8); kn, kt are then ignored          */
+    double young, poisson;         /* Young's modulus and Poisson ratio of the spheres (model 1)  */
+    double young_w, poisson_w;     /* ... of the walls                                            */
 } ledds_dem_params;
 
 int ledds_dem_workspace_bytes(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes);

@@ -35,7 +35,8 @@ class DemParams(C.Structure):
                 ("v_wall", C.c_double * 18), ("cell", C.c_double), ("dt", C.c_double), ("g", C.c_double * 3),
                 ("density", C.c_double), ("kn", C.c_double), ("kt", C.c_double), ("restitution", C.c_double),
                 ("mu", C.c_double), ("kn_w", C.c_double), ("kt_w", C.c_double), ("restitution_w", C.c_double),
-                ("mu_w", C.c_double), ("max_contacts", C.c_int)]
+                ("mu_w", C.c_double), ("max_contacts", C.c_int), ("model", C.c_int), ("young", C.c_double),
+                ("poisson", C.c_double), ("young_w", C.c_double), ("poisson_w", C.c_double)]
 
 
 class CplParams(C.Structure):
@@ -100,6 +101,9 @@ def dem_params(d) -> DemParams:
     p.kn_w = d.get("kn_w", d["kn"]); p.kt_w = d.get("kt_w", d["kt"])
     p.restitution_w = d.get("restitution_w", d["restitution"]); p.mu_w = d.get("mu_w", d["mu"])
     p.max_contacts = int(d.get("max_contacts", 16))
+    p.model = int(d.get("model", 0))
+    p.young = float(d.get("young", 0.0)); p.poisson = float(d.get("poisson", 0.0))
+    p.young_w = float(d.get("young_w", p.young)); p.poisson_w = float(d.get("poisson_w", p.poisson))
     return p
 
 

@@ -74,6 +74,7 @@ struct DemDev {
     double dt, g[3], density;
     double kn, kt, zeta, mu;
     double kn_w, kt_w, zeta_w, mu_w;
+    double Ystar, Gstar, Ystar_w, Gstar_w;   // Hertz-Mindlin (A.6), (A.7): sphere-sphere / sphere-wall
     int maxc;
 };
 

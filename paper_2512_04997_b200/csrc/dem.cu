@@ -298,10 +298,9 @@ __device__ __forceinline__ void dem_min_image(const DemDev& P, const double* xi,
 // F = force on i; T = e_n x F_t (torque on a body of radius R is -R T, Eq. 15).
 __device__ __forceinline__ void dem_pair_force(const double* en, double dn, const double* vi, const double* wi,
                                                double Ri, const double* vj, const double* wj, double Rj,
-                                               double mstar, double kn, double kt, double zeta, double mu,
+                                               double kn, double kt, double gn, double gt, double mu,
                                                double dt_hist, double* dt3, double* F, double* T)
 {
-    const double gn = 2.0 * zeta * sqrt(kn * mstar), gt = 2.0 * zeta * sqrt(kt * mstar);
     double rw[3], rwxe[3], vrel[3], vt[3], Ft[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) rw[a] = Ri * wi[a] + Rj * wj[a];
@@ -337,6 +336,27 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // negated vector).  Per-particle sums stay in registers: no atomics.
 #define CONTACT_BLOCK 128
 #define DEM_IDLE 0xffffffffu   // ncand value of a particle the detect kernel has already finished
+
+// Stiffness and damping of one contact.  HERTZ = false: the linear spring-dashpot of the configs, gamma =
+// 2 zeta sqrt(k m*) (G5).  HERTZ = true: Hertz-Mindlin: (A.1) k_n = 4/3 Y* sqrt(R* d_n),
+// k_t = 8 G* sqrt(R* d_n); (A.3)-(A.4) S_n = 2 Y* sqrt(R* d_n), S_t = 8 G* sqrt(R* d_n); (A.2) gamma =
+// 2 sqrt(5/6) zeta sqrt(S m*), zeta = -beta of (A.5).  Y*, G* of (A.6)-(A.7) come from the host (one material).
+template <bool HERTZ>
+__device__ __forceinline__ void dem_coefficients(double kn0, double kt0, double Ystar, double Gstar, double zeta, double mstar,
+                                                 double Rstar, double dn, double& kn, double& kt, double& gn, double& gt)
+{
+    if (HERTZ) {
+        const double sq = sqrt(Rstar * dn);
+        kn = (4.0 / 3.0) * Ystar * sq;
+        kt = 8.0 * Gstar * sq;
+        const double Sn = 2.0 * Ystar * sq, St = 8.0 * Gstar * sq;
+        gn = 2.0 * sqrt(5.0 / 6.0) * zeta * sqrt(Sn * mstar);
+        gt = 2.0 * sqrt(5.0 / 6.0) * zeta * sqrt(St * mstar);
+    } else {
+        kn = kn0; kt = kt0;
+        gn = 2.0 * zeta * sqrt(kn * mstar); gt = 2.0 * zeta * sqrt(kt * mstar);
+    }
+}
 
 // one full 64-byte record per particle: contact force, torque, number of contacts (exact in a double), pad
 __device__ __forceinline__ void dem_store_ft(double* __restrict__ ft, uint32_t p, const double* F, const double* M, uint32_t count)
@@ -447,6 +467,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
 }
 
 // ---- phase 2: evaluate
+template <bool HERTZ>
 __global__ void __launch_bounds__(CONTACT_BLOCK) dem_force_kernel(
     const DemDev P, const uint32_t* __restrict__ sidx, const double4* __restrict__ xr_s, const double* __restrict__ vp,
     const double* __restrict__ wp, const uint32_t* __restrict__ ncand_g, const uint32_t* __restrict__ cand_g,
@@ -502,7 +523,9 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_force_kernel(
                 break;
             }
         double F[3], T[3];
-        dem_pair_force(en, dn, bi.v, bi.w, bi.R, bj.v, bj.w, bj.R, mstar, P.kn, P.kt, P.zeta, P.mu, dt_hist, dt3, F, T);
+        double kn, kt, gn, gt;
+        dem_coefficients<HERTZ>(P.kn, P.kt, P.Ystar, P.Gstar, P.zeta, mstar, bi.R * bj.R / (bi.R + bj.R), dn, kn, kt, gn, gt);
+        dem_pair_force(en, dn, bi.v, bi.w, bi.R, bj.v, bj.w, bj.R, kn, kt, gn, gt, P.mu, dt_hist, dt3, F, T);
 #pragma unroll
         for (int a = 0; a < 3; ++a) { Fs[a] += sg * F[a]; Ms[a] += me.R * (-T[a]); }
         nid[ncont] = q;
@@ -524,7 +547,9 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_force_kernel(
             if (pid[h] == q) { dt3[0] = pdt[3 * h]; dt3[1] = pdt[3 * h + 1]; dt3[2] = pdt[3 * h + 2]; break; }
         const double vj[3] = {P.vw[wl * 3], P.vw[wl * 3 + 1], P.vw[wl * 3 + 2]}, wj[3] = {0, 0, 0};
         double F[3], T[3];
-        dem_pair_force(en, dn, me.v, me.w, me.R, vj, wj, 0.0, m_me, P.kn_w, P.kt_w, P.zeta_w, P.mu_w, dt_hist, dt3, F, T);
+        double kn, kt, gn, gt;                                                        // the wall: R* = R_i, m* = m_i
+        dem_coefficients<HERTZ>(P.kn_w, P.kt_w, P.Ystar_w, P.Gstar_w, P.zeta_w, m_me, me.R, dn, kn, kt, gn, gt);
+        dem_pair_force(en, dn, me.v, me.w, me.R, vj, wj, 0.0, kn, kt, gn, gt, P.mu_w, dt_hist, dt3, F, T);
 #pragma unroll
         for (int a = 0; a < 3; ++a) { Fs[a] += F[a]; Ms[a] += me.R * (-T[a]); }
         if (ncont < (uint32_t)maxc) {
@@ -660,7 +685,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
 {
     if (!p || p->n < 0 || p->max_contacts < 1 || p->max_contacts > 32) return LEDDS_EINVAL;   // n = 0: a valid, empty system
     if (!(p->cell > 0.0) || !(p->dt >= 0.0) || !(p->density > 0.0)) return LEDDS_EINVAL;
-    if (!(p->kn > 0.0) || !(p->kt > 0.0) || !(p->kn_w > 0.0) || !(p->kt_w > 0.0)) return LEDDS_EINVAL;
+    if (p->model == 0 && (!(p->kn > 0.0) || !(p->kt > 0.0) || !(p->kn_w > 0.0) || !(p->kt_w > 0.0))) return LEDDS_EINVAL;
     if (!(p->restitution > 0.0) || !(p->restitution_w > 0.0) || p->mu < 0.0 || p->mu_w < 0.0) return LEDDS_EINVAL;
     h->p = *p;
     DemDev& d = h->d;
@@ -685,6 +710,16 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     d.kn = p->kn; d.kt = p->kt; d.zeta = dem_zeta_host(p->restitution); d.mu = p->mu;
     d.kn_w = p->kn_w; d.kt_w = p->kt_w; d.zeta_w = dem_zeta_host(p->restitution_w); d.mu_w = p->mu_w;
     d.maxc = p->max_contacts;
+    d.Ystar = d.Gstar = d.Ystar_w = d.Gstar_w = 0.0;
+    if (p->model != 0 && p->model != 1) return LEDDS_EINVAL;
+    if (p->model == 1) {                                                              // (A.6), (A.7)
+        const double Ei = p->young, ni = p->poisson, Ew = p->young_w, nw = p->poisson_w;
+        if (!(Ei > 0.0) || !(Ew > 0.0) || !(ni > -1.0 && ni < 0.5 + 1e-12) || !(nw > -1.0 && nw < 0.5 + 1e-12)) return LEDDS_EINVAL;
+        d.Ystar = 1.0 / ((1.0 - ni * ni) / Ei + (1.0 - ni * ni) / Ei);
+        d.Gstar = 1.0 / (2.0 * (2.0 - ni) * (1.0 + ni) / Ei + 2.0 * (2.0 - ni) * (1.0 + ni) / Ei);
+        d.Ystar_w = 1.0 / ((1.0 - ni * ni) / Ei + (1.0 - nw * nw) / Ew);
+        d.Gstar_w = 1.0 / (2.0 * (2.0 - ni) * (1.0 + ni) / Ei + 2.0 * (2.0 - nw) * (1.0 + nw) / Ew);
+    }
     int bits = 1;
     while (bits < 32 && (1ull << bits) < (unsigned long long)d.ncell) ++bits;
     h->key_bits = bits;
@@ -801,7 +836,7 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
                                                               at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
                                                               at<double>(history, hs.ft[nw]), status);
     ledds_count_launch(1);
-    dem_force_kernel<<<nb, CONTACT_BLOCK, 0, st>>>(
+    (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<nb, CONTACT_BLOCK, 0, st>>>(
         d, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
         at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
         at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),

@@ -134,3 +134,18 @@ def test_full_size_config5_pour_ordering_after_steps():
     assert q["status"] == 0 and len(q["pairs"]) == 0
     # free fall so far: every sphere has v_z = -g t exactly as integrated (Eq. 18), no contact yet
     assert np.allclose(g.state()["v"][:, 2], -9.81 * 3 * pd["dt"], rtol=1e-12)
+
+
+@pytest.mark.parametrize("seed,bc,n", [(11, (1, 1, 1), 2500), (12, (0, 1, 0), 1500)])
+def test_hertz_mindlin_cloud(seed, bc, n):
+    # PAPER.md:968-1001 (A.1)-(A.8): stiffness and damping per contact from Young's modulus, Poisson ratio and the
+    # overlap; walls of another material; polydisperse radii, friction, rotation, periodic wrap
+    pd, x, v, w, R = W.dem_random(seed, n, box=(14.0, 11.0, 9.0), bc=bc)
+    pd.update(max_contacts=32, model=1, young=2.0e6, poisson=0.3, young_w=7.0e6, poisson_w=0.22, dt=2e-5)
+    o, g = both(pd, x, v, w, R)
+    check_state(o, g, 0, 14.0)
+    o.step(); g.step()
+    check_state(o, g, 1, 14.0)
+    for _ in range(9):
+        o.step(); g.step()
+    check_state(o, g, 10, 14.0)
