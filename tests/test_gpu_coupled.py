@@ -212,3 +212,13 @@ def test_subdivision_single_sphere_walls():
     o, g = both(lbm, dict(cpl, solid_fraction=1), pd, x, v, w, R)
     o.step(6); g.step(6)
     compare(o, g)
+
+
+def test_paper_bed_workload_small():
+    # SURVEY 8(f) rank 3 in small: the generator of the paper's performance workload (TRT, 10 DEM sub-steps per
+    # LBM step, periodic x y, walls z) on a 96 x 48 x 64 lattice with spheres of 12 cells diameter at phi = 0.3
+    lbm, cpl, pd, x, v, w, R = W.paper_bed(0.30, shape=(96, 48, 64), D=12.0)
+    assert len(R) > 30
+    o, g = both(lbm, cpl, pd, x, v, w, R)
+    o.step(2); g.step(2)
+    compare(o, g)

@@ -231,3 +231,47 @@ def dem_random(seed, n, box=(10.0, 10.0, 10.0), bc=(1, 1, 1), rmin=0.4, rmax=0.6
     pd = dem_defaults(n, (0, 0, 0), box, bc, cell=2 * rmax, dt=1e-4, g=(0, 0, -9.81), density=1000.0, kn=1e5,
                       restitution=0.8, mu=0.4)
     return pd, x, v, w, radius
+
+
+def paper_bed(phi, shape=(500, 200, 800), D=20.0, seed=6, n_sub=10):
+    """the paper's performance workload: a 500 x 200 x 800 lattice,
+    spheres of diameter 20 cells at solid fraction phi (0 / 0.15 / 0.30 / 0.45 -> 0 / 2 866 / 5 731 / 8 596 spheres
+    in the paper), density ratio 1.1, 10 DEM sub-steps per LBM step, TRT collision.  The paper's inlet / outlet
+    are not part of the hot path: here the box is periodic in x, y with walls in z, fluid at rest, gravity on
+    the spheres.  Placement: seeded jittered simple-cubic lattice at the spacing that gives phi (RSA cannot
+    reach 0.45), filled from the bottom."""
+    nx, ny, nz = shape
+    R = 0.5 * D
+    lbm = dict(shape=shape, tau=0.6, bc=(0, 0, 1), u_wall=np.zeros(18), collision=1)
+    cpl = dict(n_sub=n_sub, dx=1.0, rho_f=1.0, origin=(0.0, 0.0, 0.0))
+    lo, hi = (-0.5, -0.5, -0.5), (nx - 0.5, ny - 0.5, nz - 0.5)
+    vol = (4.0 / 3.0) * PI * R ** 3
+    n_part = int(round(phi * nx * ny * nz / vol))
+    g = _rng(seed)
+    if n_part > 0:
+        # lattice spacing for the target fraction, snapped so that whole cells fit the periodic directions
+        s = (vol / phi) ** (1.0 / 3.0)
+        best = None
+        for mx in (int(nx // s), int(nx // s) + 1):
+            for my in (int(ny // s), int(ny // s) + 1):
+                sx, sy = nx / mx, ny / my
+                sz = vol / (phi * sx * sy)
+                if best is None or min(sx, sy, sz) > best[0]:
+                    best = (min(sx, sy, sz), mx, my, sx, sy, sz)
+        _, mx, my, sx, sy, sz = best
+        mz = int((nz - 1.0) // sz)
+        n_part = min(n_part, mx * my * mz)
+        sites = np.arange(mx * my * mz)[:n_part]
+        i, j, k = sites % mx, (sites // mx) % my, sites // (mx * my)
+        x = np.stack([(i + 0.5) * sx - 0.5, (j + 0.5) * sy - 0.5, (k + 0.5) * sz], -1)
+        slack = 0.5 * (min(sx, sy, sz) - 2.0 * R)
+        assert slack > 0.0, "spheres would overlap at this fraction"
+        x = x + g.uniform(-0.4 * slack, 0.4 * slack, (n_part, 3))
+        x = x[g.permutation(n_part)]
+    else:
+        x = np.zeros((0, 3))
+    m = 1.1 * vol
+    kn = 0.5 * m * (PI / (50.0 / n_sub)) ** 2               # contact lasts ~50 DEM steps (dt = 1/n_sub)
+    pd = dem_defaults(n_part, lo, hi, (0, 0, 1), cell=2 * R + 1.3, dt=1.0 / n_sub, g=(0, 0, -(1.0 - 1.0 / 1.1) * 1e-5),
+                      density=1.1, kn=kn, restitution=0.9, mu=0.3)
+    return lbm, cpl, pd, x, np.zeros((n_part, 3)), np.zeros((n_part, 3)), np.full(n_part, R)
