@@ -90,11 +90,11 @@ def coupled_bytes_per_step(n_cells):
 
 def dem_bytes_per_particle(passes):
     """Algorithmic HBM bytes per particle of each DEM kernel group."""
-    return {"dem_keys": 128 + 116,                 # x v w a alpha R read; x vp wp (x,R) key id written
+    return {"dem_keys": 192 + 208,                 # kick of the previous step + drift + keys in one pass: record, R, x v w a
+                                                   # alpha read; v w a alpha x vp wp (x,R) key id written
             "dem_sort": 4 + 16 * passes,           # histogram read + (key, id) read and written per pass
             "dem_gather": 8 + 32 + 32,             # (key, id), one packed record read, one written
-            "dem_contact": 8 + 32 + 64,            # (key, id), own record, force/torque/count record written
-            "dem_kick": 8 + 64 + 96 + 96}          # R, record, v w a alpha read; v w a alpha written
+            "dem_contact": 8 + 32 + 64}            # (key, id), own record, force/torque/count record written
 
 
 def max_over_ranks(ms, world, device="cuda"):
@@ -336,7 +336,7 @@ def run_ours(args, rank, world):
             for a in range(3):
                 ncell *= max(1, int((pd5["hi"][a] - pd5["lo"][a]) / pd5["cell"]))
             bpp = dem_bytes_per_particle((max(1, int(np.ceil(np.log2(ncell)))) + 7) // 8)
-            gbs = {nm: round(bpp[nm] * len(R5) / (pr[nm] * 1e-3) / 1e9, 1) for nm in pr if pr[nm] > 0}
+            gbs = {nm: round(bpp[nm] * len(R5) / (pr[nm] * 1e-3) / 1e9, 1) for nm in bpp if pr.get(nm, 0) > 0}
             total_bytes = sum(bpp.values()) * len(R5)
             sub[name] = {"particle_updates_per_s": round(len(R5) * 1e3 / ms5, 1), "ms_per_step": round(ms5, 5), "steps": kd,
                          "particles": len(R5), "contacts": int(q[0].item()), "kernel_ms_per_step": pr,

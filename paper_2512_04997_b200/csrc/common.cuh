@@ -114,8 +114,9 @@ struct ledds_dem {
 };
 
 // entry points implemented in dem.cu and used by coupled.cu
-int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const double* w, const double* a,
-                               const double* alpha, const double* radius, void* history, void* scratch,
-                               int32_t* status, double dt_hist, bool drift, cudaStream_t st, bool fork = false);
+struct DemKick { const double* f_ext; const double* m_ext; };   // external force / torque of a kick, [n][3] or NULL
+int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha,
+                               const double* radius, void* history, void* scratch, int32_t* status, double dt_hist,
+                               bool drift, cudaStream_t st, bool fork = false, const DemKick* kick = nullptr);
 int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha, const double* radius,
                    const double* f_ext, const double* m_ext, const void* history, int32_t* status, cudaStream_t st);

@@ -359,17 +359,20 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
     const LbmDev& d = lbm->d;
     const size_t half = (size_t)LEDDS_Q * d.N;
     if (d.ny > 65535 || d.nz > 65535) return LEDDS_EINVAL;
+    // A kick (with F_sf, M_sf as they stand when it runs) rides on the drift kernel of the next DEM (sub-)step:
+    // between sub-steps the values of the previous LBM step are held, and the kick that closes an LBM step
+    // rides on the first drift of the next one; only the last step of the call kicks on its own.
+    const DemKick hyd = {f_hyd, m_hyd};
+    bool pending = false;
     for (int step = 0; step < nsteps; ++step) {
         for (int sub = 0; sub < c->n_sub; ++sub) {
             // the contact pipeline of the last sub-step runs beside the lattice kernels: only the kick needs both
             const bool fork = sub == c->n_sub - 1 && dem->d.n > 0;
-            rc = ledds_dem_advance_contacts(dem, x, v, w, a, alpha, radius, history, scratch, status, dem->d.dt, true, st, fork);
+            rc = ledds_dem_advance_contacts(dem, x, v, w, a, alpha, radius, history, scratch, status, dem->d.dt, true, st, fork,
+                                            pending ? &hyd : nullptr);
             if (rc) return rc;
-            if (sub < c->n_sub - 1) {                                        // F_sf of the previous LBM step is held
-                rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);
-                if (rc) return rc;
-                dem->steps++;
-            }
+            pending = sub < c->n_sub - 1;                                    // F_sf of the previous LBM step is held
+            if (pending) dem->steps++;
         }
         ledds_prof_start(LEDDS_K_CPL_RASTER, st);
         if (C.n > 0) {
@@ -405,9 +408,12 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         ledds_prof_stop(LEDDS_K_CPL_REDUCE, st);
         LEDDS_CHECK_LAUNCH();
         if (dem->d.n > 0 && cudaStreamWaitEvent(st, dem->ev_join, 0) != cudaSuccess) return LEDDS_ECUDA;   // join
-        rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);
-        if (rc) return rc;
         dem->steps++;
+        pending = step < nsteps - 1;
+        if (!pending) {
+            rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);
+            if (rc) return rc;
+        }
     }
     return LEDDS_OK;
 }

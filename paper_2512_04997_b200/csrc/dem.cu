@@ -46,12 +46,16 @@ __device__ __forceinline__ int dem_cell_coord(const DemDev& P, double x, int a)
 // Block = DRIFT_BLOCK particles.  The [n][3] arrays are walked as flat arrays (element e = 3 i + k), so every
 // load and store is fully coalesced; the new positions pass through shared memory to form the key and the
 // packed record per particle.
+// KICK = true: the kick of the previous step (Eq. 18b-c, 19c-d with the contact record ft and the external
+// force / torque) is applied first, in the same pass: between two steps of one call the state is read and
+// written once instead of twice.
 #define DRIFT_BLOCK 128
+template <bool KICK>
 __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
-    const DemDev P, double* __restrict__ x, const double* __restrict__ v, const double* __restrict__ w,
-    const double* __restrict__ a, const double* __restrict__ alpha, const double* __restrict__ radius,
-    double* __restrict__ vp, double* __restrict__ wp, double4* __restrict__ xr, uint32_t* __restrict__ key,
-    uint32_t* __restrict__ idx, int drift)
+    const DemDev P, double* __restrict__ x, double* __restrict__ v, double* __restrict__ w, double* __restrict__ a,
+    double* __restrict__ alpha, const double* __restrict__ radius, const double* __restrict__ ft,
+    const double* __restrict__ f_ext, const double* __restrict__ m_ext, double* __restrict__ vp,
+    double* __restrict__ wp, double4* __restrict__ xr, uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift)
 {
     __shared__ double sx[3 * DRIFT_BLOCK];
     const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * P.n;
@@ -62,9 +66,19 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
         if (e >= ne) break;
         const int k = le % 3;                                                 // e0 is a multiple of 3
         double xv = x[e];
-        const double vv = v[e], wv = w[e];
+        double vv = v[e], wv = w[e], av = a[e], alv = alpha[e];
+        if (KICK) {                                                           // same expressions as dem_kick_kernel
+            const int i = (int)(e / 3);
+            const double R = radius[i];
+            const double m = dem_mass(P, R), I = 0.4 * m * R * R;             // Eq. (21a)
+            const double Fq = ft[8 * (size_t)i + k] + (f_ext ? f_ext[e] : 0.0), Mq = ft[8 * (size_t)i + 3 + k] + (m_ext ? m_ext[e] : 0.0);
+            const double an = Fq / m + P.g[k], aln = Mq / I;                  // Eq. (18b), (19c)
+            vv = vv + (0.5 * P.dt) * (av + an);                               // Eq. (18c)
+            wv = wv + (0.5 * P.dt) * (alv + aln);                             // Eq. (19d)
+            av = an; alv = aln;
+            v[e] = vv; w[e] = wv; a[e] = av; alpha[e] = alv;
+        }
         if (drift) {
-            const double av = a[e], alv = alpha[e];
             xv = xv + P.dt * vv + (0.5 * P.dt * P.dt) * av;                   // Eq. (18a)
             if (!P.bc[k]) {
                 if (xv >= P.hi[k]) xv -= P.L[k];
@@ -773,10 +787,12 @@ template <typename T>
 static const T* at(const void* base, size_t off) { return reinterpret_cast<const T*>(static_cast<const char*>(base) + off); }
 
 // drift (optional) -> keys -> sort -> gather/ranges -> contacts.  Leaves force/torque in scratch.
-int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const double* w, const double* a,
-                               const double* alpha, const double* radius, void* history, void* scratch,
-                               int32_t* status, double dt_hist, bool drift, cudaStream_t st, bool fork)
+int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha,
+                               const double* radius, void* history, void* scratch, int32_t* status, double dt_hist,
+                               bool drift, cudaStream_t st, bool fork, const DemKick* kick)
 {
+    // kick != nullptr: the kick that closes the previous step (with the contact forces still in ft[cur] and the
+    // external force / torque of *kick) is fused into the drift kernel of this one.
     // fork = true: everything after the drift/key kernel is enqueued on the handle's side stream (ordered after
     // that kernel by an event); the caller joins by waiting on h->ev_join before it needs the contact forces.
     const DemDev& d = h->d;
@@ -786,9 +802,18 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, const double* v, const d
     // clear sort bookkeeping + cell ranges (one contiguous region)
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
     ledds_prof_start(LEDDS_K_DEM_KEYS, st);
-    dem_drift_key_kernel<<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(d, x, v, w, a, alpha, radius, at<double>(scratch, s.vp),
-                                            at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
-                                            at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
+    {
+        const dim3 grid((n + DRIFT_BLOCK - 1) / DRIFT_BLOCK);
+        const double* ft = at<double>(history, h->hs.ft[h->cur]);
+        if (kick)
+            dem_drift_key_kernel<true><<<grid, DRIFT_BLOCK, 0, st>>>(d, x, v, w, a, alpha, radius, ft, kick->f_ext, kick->m_ext,
+                                                                      at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
+                                                                      at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
+        else
+            dem_drift_key_kernel<false><<<grid, DRIFT_BLOCK, 0, st>>>(d, x, v, w, a, alpha, radius, ft, nullptr, nullptr,
+                                                                       at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
+                                                                       at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
+    }
     ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
     LEDDS_CHECK_LAUNCH();
     if (fork) {
@@ -881,7 +906,8 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
         return LEDDS_ECUDA;
     }
     // forces of the initial state: no drift, delta_t stays 0 (dt_hist = 0)
-    rc = ledds_dem_advance_contacts(h, const_cast<double*>(x), v, w, a, alpha, radius, history, scratch, status, 0.0, false, st);
+    rc = ledds_dem_advance_contacts(h, const_cast<double*>(x), const_cast<double*>(v), const_cast<double*>(w), a, alpha, radius, history,
+                                    scratch, status, 0.0, false, st, false, nullptr);
     if (rc) { delete h; return rc; }
     if (h->d.n == 0) { *out = h; return LEDDS_OK; }
     dem_kick_kernel<<<(unsigned)((3ll * h->d.n + 255) / 256), 256, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), nullptr,
@@ -903,13 +929,15 @@ extern "C" int ledds_dem_step(ledds_dem* h, double* x, double* v, double* w, dou
     for (const void* q : ptrs)
         if (!ledds_aligned16(q)) return LEDDS_EALIGN;
     cudaStream_t st = (cudaStream_t)stream;
+    const DemKick kick = {f_ext, m_ext};
     for (int s = 0; s < nsteps; ++s) {
-        int rc = ledds_dem_advance_contacts(h, x, v, w, a, alpha, radius, history, scratch, status, h->d.dt, true, st);
-        if (rc) return rc;
-        rc = ledds_dem_kick(h, v, w, a, alpha, radius, f_ext, m_ext, history, status, st);
+        // the kick of step s - 1 rides on the drift of step s; only the last step of the call kicks on its own
+        int rc = ledds_dem_advance_contacts(h, x, v, w, a, alpha, radius, history, scratch, status, h->d.dt, true, st, false,
+                                            s > 0 ? &kick : nullptr);
         if (rc) return rc;
         h->steps++;
     }
+    if (nsteps > 0) return ledds_dem_kick(h, v, w, a, alpha, radius, f_ext, m_ext, history, status, st);
     return LEDDS_OK;
 }
 
