@@ -5,11 +5,13 @@ A "step" is one pass of the whole hot path: one couple
 BASELINE.json configs[3] (256^3 D3Q19 BGK lattice, periodic x/y, moving z walls, 20 000 spheres of
 radius 4 placed by seeded RSA, PSM coupling, n_sub = 1).  The headline value is MLUPS from the
 total time per step including DEM and coupling (the paper's own definition).
-Sub-benchmarks (configs[1] LBM-only MLUPS, configs[4] DEM-only particle-updates/s) are reported in
-the same JSON line under "sub".  Multi-GPU (N > 1, torchrun) = independent replicas, no collective
+Sub-benchmarks are reported in the same JSON line under "sub": configs[1] LBM-only MLUPS (BGK and TRT),
+configs[0] and configs[2] (latency-bound; plain and from a CUDA graph), configs[4] DEM-only
+particle-updates/s with GB/s per kernel, configs[3] with TRT + subdivision solid fraction, and the paper's
+own 500x200x800 performance workload at four solid fractions.  Multi-GPU (N > 1, torchrun) = independent replicas, no collective
 on the data path ("replicas only").
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg4|cfg2|cfg5|small]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg4|small] [--no-sub]
 """
 import argparse
 import json
