@@ -18,7 +18,6 @@
 #include "psm_kernels.cuh"
 
 // ------------------------------------------------------------------------------------ raster
-#define PSM_EMPTY64 0xffffffffffffffffull
 
 #define RASTER_BATCH 6
 

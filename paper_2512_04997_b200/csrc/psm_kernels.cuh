@@ -54,8 +54,6 @@ __device__ __forceinline__ int cpl_offset(int r, int fk, int n, int periodic)
     return di;
 }
 
-__device__ __forceinline__ int cpl_floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
-
 // delta_sc > 0 (Eq. 39-40) decided exactly as cpl_dsc(...) > 0 would, but without the square root unless
 // the squared distance is within rounding of (R_k + r_c)^2.
 __device__ __forceinline__ bool cpl_cuts(double Rk, double rc, const double* d)
