@@ -178,7 +178,13 @@ __global__ void __launch_bounds__(SORT_THREADS) dem_onesweep_kernel(
     for (int it = 0; it < SORT_ITEMS; ++it) {
         const bool ok = base + it * 32 + lane < n;
         const uint32_t d = ok ? ((k[it] >> shift) & 255u) : 256u;
-        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        uint32_t peers = 0xffffffffu;                               // lanes with the same digit: 9 ballots, one per bit
+#pragma unroll
+        for (int b = 0; b < 9; ++b) {
+            const bool bit = (d >> b) & 1u;
+            const uint32_t bal = __ballot_sync(0xffffffffu, bit);
+            peers &= bit ? bal : ~bal;
+        }
         const uint32_t below = __popc(peers & ((1u << lane) - 1u));
         uint32_t old = 0;
         if (ok) old = warp_hist[warp][d];
