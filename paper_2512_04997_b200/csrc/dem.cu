@@ -21,7 +21,10 @@
 #define SORT_THREADS 256
 #define SORT_WARPS (SORT_THREADS / 32)
 #ifndef SORT_ITEMS
-#define SORT_ITEMS 16
+#define SORT_ITEMS 12
+#endif
+#ifndef SORT_MIN_BLOCKS
+#define SORT_MIN_BLOCKS 4
 #endif
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define SORT_RADIX 256
@@ -128,7 +131,7 @@ __device__ __forceinline__ void st_volatile(uint32_t* p, uint32_t v) { *reinterp
 // One stable LSD pass (8-bit digit at `shift`).  Tiles take tickets from an atomic counter so that
 // every tile a block waits on is already resident or done.  Order inside a tile = (warp, item, lane)
 // = ascending input index, which keeps the sort stable.
-__global__ void __launch_bounds__(SORT_THREADS) dem_onesweep_kernel(
+__global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS) dem_onesweep_kernel(
     const uint32_t* __restrict__ key_in, const uint32_t* __restrict__ val_in, uint32_t* __restrict__ key_out,
     uint32_t* __restrict__ val_out, int n, int shift, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
     uint32_t* __restrict__ tile_state /*[tiles][256] of this pass*/, uint32_t* __restrict__ ticket)
