@@ -92,6 +92,19 @@ const double* ledds_lbm_current(const ledds_lbm* h, const double* f);
 
 int ledds_lbm_destroy(ledds_lbm* h);
 
+/* Single-precision variant of the plain LBM calls above (the paper runs most of its validations and one
+ * of its two performance curves in fp32).  Same operation, layout (two lattices of
+ * 19 x N floats), boundaries and collision models; all arithmetic in fp32; rho, u and f_canonical are float
+ * arrays.  variant 2 (row-rotate) does not exist in fp32: LEDDS_EINVAL.  A handle made by
+ * ledds_lbm_init_f32 is accepted by the _f32 calls and ledds_lbm_destroy only, a handle made by
+ * ledds_lbm_init by the fp64 calls only (LEDDS_EINVAL otherwise).  The coupled step is fp64 in this version. */
+int ledds_lbm_workspace_bytes_f32(const ledds_lbm_params* p, size_t* f_bytes);
+int ledds_lbm_init_f32(ledds_lbm** h, const ledds_lbm_params* p, float* f, const float* rho, const float* u,
+                       void* stream);
+int ledds_lbm_import_f32(ledds_lbm* h, float* f, const float* f_canonical, void* stream);
+int ledds_lbm_step_f32(ledds_lbm* h, float* f, int nsteps, void* stream);
+int ledds_lbm_export_f32(ledds_lbm* h, const float* f, float* f_canonical, float* rho, float* u, void* stream);
+
 /* ------------------------------------------------------------------------------------ DEM
  * One DEM step for spheres, PAPER.md:63-142 (Eq. 1-15), 158-192 (Eq. 18-21), 431-511:
  *   drift (18a) + predictor -> cell keys on a uniform grid (spacing >= largest diameter,

@@ -20,7 +20,8 @@ _lib = C.CDLL(_LIB_PATH)
 LEDDS_OK, LEDDS_EINVAL, LEDDS_EALIGN, LEDDS_ECAPACITY, LEDDS_ECUDA = 0, -1, -2, -3, -4
 ST_CONTACT_OVERFLOW, ST_SOLID_OVERFLOW, ST_COINCIDENT, ST_NONFINITE = 1, 2, 4, 8
 EXPORTS = ["ledds_lbm_workspace_bytes", "ledds_lbm_init", "ledds_lbm_import", "ledds_lbm_step", "ledds_lbm_export",
-           "ledds_lbm_current", "ledds_lbm_destroy", "ledds_dem_workspace_bytes", "ledds_dem_init", "ledds_dem_step",
+           "ledds_lbm_current", "ledds_lbm_destroy", "ledds_lbm_workspace_bytes_f32", "ledds_lbm_init_f32",
+           "ledds_lbm_import_f32", "ledds_lbm_step_f32", "ledds_lbm_export_f32", "ledds_dem_workspace_bytes", "ledds_dem_init", "ledds_dem_step",
            "ledds_dem_query", "ledds_dem_destroy", "ledds_cpl_workspace_bytes", "ledds_cpl_init", "ledds_coupled_step", "ledds_version",
            "ledds_profile", "ledds_profile_read", "ledds_launch_count"]
 
@@ -166,6 +167,31 @@ def ledds_lbm_export(h, f, f_canonical=None, rho=None, u=None):
 
 def ledds_lbm_destroy(h):
     _lib.ledds_lbm_destroy(h)
+
+
+# fp32 set: same calls on float buffers (include/ledds.h)
+def ledds_lbm_workspace_bytes_f32(p: LbmParams) -> int:
+    n = C.c_size_t(0)
+    _check(_lib.ledds_lbm_workspace_bytes_f32(C.byref(p), C.byref(n)), "ledds_lbm_workspace_bytes_f32")
+    return n.value
+
+
+def ledds_lbm_init_f32(p: LbmParams, f, rho=None, u=None):
+    h = C.c_void_p(0)
+    _check(_lib.ledds_lbm_init_f32(C.byref(h), C.byref(p), _p(f), _p(rho), _p(u), _stream()), "ledds_lbm_init_f32")
+    return h
+
+
+def ledds_lbm_import_f32(h, f, f_canonical):
+    _check(_lib.ledds_lbm_import_f32(h, _p(f), _p(f_canonical), _stream()), "ledds_lbm_import_f32")
+
+
+def ledds_lbm_step_f32(h, f, nsteps=1):
+    _check(_lib.ledds_lbm_step_f32(h, _p(f), C.c_int(nsteps), _stream()), "ledds_lbm_step_f32")
+
+
+def ledds_lbm_export_f32(h, f, f_canonical=None, rho=None, u=None):
+    _check(_lib.ledds_lbm_export_f32(h, _p(f), _p(f_canonical), _p(rho), _p(u), _stream()), "ledds_lbm_export_f32")
 
 
 # ------------------------------------------------------------------------------------ DEM

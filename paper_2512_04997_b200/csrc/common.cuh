@@ -60,6 +60,7 @@ struct ledds_lbm {
     LbmDev d;
     int parity;            // which half of the two-lattice buffer is current (0 or 1)
     long long steps;
+    bool f32;              // populations are float (ledds_lbm_*_f32 calls); the coupled step takes fp64 handles only
 };
 
 // Kernel-side DEM parameters.

@@ -262,7 +262,7 @@ static size_t cpl_align(size_t v) { return (v + 255) & ~(size_t)255; }
 static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_params* c, double r_max, CplDev* C,
                      CplLayout* L)
 {
-    if (!lbm || !dem || !c || c->n_sub < 1 || (c->solid_fraction != 0 && c->solid_fraction != 1) || !(c->dx > 0.0) || !(c->rho_f > 0.0) || !(r_max > 0.0))
+    if (!lbm || lbm->f32 || !dem || !c || c->n_sub < 1 || (c->solid_fraction != 0 && c->solid_fraction != 1) || !(c->dx > 0.0) || !(c->rho_f > 0.0) || !(r_max > 0.0))
         return LEDDS_EINVAL;
     const double rc = cbrt(3.0 / (4.0 * 3.14159265358979323846));           // Eq. (40), dx = 1
     const double Dt = c->n_sub * dem->d.dt;

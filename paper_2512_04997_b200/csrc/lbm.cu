@@ -11,25 +11,26 @@
 #include "lbm_kernels.cuh"
 
 // ------------------------------------------------------------------------------------ helpers
-__global__ void lbm_init_eq_kernel(double* __restrict__ f, const double* __restrict__ rho,
-                                   const double* __restrict__ u, long long N)
+template <typename T>
+__global__ void lbm_init_eq_kernel(T* __restrict__ f, const T* __restrict__ rho, const T* __restrict__ u, long long N)
 {
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= N) return;
-    const double r = rho ? rho[c] : 1.0;
-    const double ux = u ? u[c] : 0.0, uy = u ? u[N + c] : 0.0, uz = u ? u[2 * N + c] : 0.0;
-    double fe[LEDDS_Q];
+    const T r = rho ? rho[c] : T(1);
+    const T ux = u ? u[c] : T(0), uy = u ? u[N + c] : T(0), uz = u ? u[2 * N + c] : T(0);
+    T fe[LEDDS_Q];
     lb_equilibrium(fe, r, ux, uy, uz);
 #pragma unroll
     for (int q = 0; q < LEDDS_Q; ++q) f[(long long)q * N + c] = fe[q];
 }
 
-__global__ void lbm_export_kernel(const double* __restrict__ f, double* __restrict__ fc, double* __restrict__ rho,
-                                  double* __restrict__ u, long long N)
+template <typename T>
+__global__ void lbm_export_kernel(const T* __restrict__ f, T* __restrict__ fc, T* __restrict__ rho, T* __restrict__ u,
+                                  long long N)
 {
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= N) return;
-    double v[LEDDS_Q];
+    T v[LEDDS_Q];
 #pragma unroll
     for (int q = 0; q < LEDDS_Q; ++q) v[q] = f[(long long)q * N + c];
     if (fc) {
@@ -37,7 +38,7 @@ __global__ void lbm_export_kernel(const double* __restrict__ f, double* __restri
         for (int q = 0; q < LEDDS_Q; ++q) fc[(long long)q * N + c] = v[q];
     }
     if (rho || u) {
-        double r, ux, uy, uz;
+        T r, ux, uy, uz;
         lb_moments(v, r, ux, uy, uz);
         if (rho) rho[c] = r;
         if (u) { u[c] = ux; u[N + c] = uy; u[2 * N + c] = uz; }
@@ -47,30 +48,30 @@ __global__ void lbm_export_kernel(const double* __restrict__ f, double* __restri
 // ------------------------------------------------------------------------------------ variant 1
 // Block = 128 threads = BX cells along x times 128 / BX rows along y (BX = 128 unless the lattice is narrower,
 // so that narrow lattices do not run half-empty blocks); a warp always lies inside one row.
-template <typename I, int BX, bool TRT>
-__global__ void __launch_bounds__(128) lbm_push_kernel(const double* __restrict__ fin, double* __restrict__ fout,
+template <typename T, typename I, int BX, bool TRT>
+__global__ void __launch_bounds__(128) lbm_push_kernel(const T* __restrict__ fin, T* __restrict__ fout,
                                                        const __grid_constant__ LbmDev P)
 {
     const int x = blockIdx.x * BX + (int)(threadIdx.x % BX);
     const int y = blockIdx.y * (128 / BX) + (int)(threadIdx.x / BX), z = blockIdx.z;
     if (x >= P.nx || y >= P.ny) return;
     const I cell = ((I)z * (I)P.ny + (I)y) * (I)P.nx + (I)x;
-    double f[LEDDS_Q];
+    T f[LEDDS_Q];
     lb_load<I>(fin, (I)P.N, cell, f);
-    double rho, ux, uy, uz;
+    T rho, ux, uy, uz;
     lb_moments(f, rho, ux, uy, uz);
     lb_collide<TRT>(f, P, rho, ux, uy, uz);
     lb_push_store<I>(fout, P, x, y, z, f, rho);
 }
 
-template <typename I, bool TRT>
-static void lbm_push_launch(const double* src, double* dst, const LbmDev& d, cudaStream_t st)
+template <typename T, typename I, bool TRT>
+static void lbm_push_launch(const T* src, T* dst, const LbmDev& d, cudaStream_t st)
 {
     const int bx = lb_block_x(d.nx), rows = 128 / bx;
     const dim3 block(128), grid((d.nx + bx - 1) / bx, (d.ny + rows - 1) / rows, d.nz);
-    if (bx == 128) lbm_push_kernel<I, 128, TRT><<<grid, block, 0, st>>>(src, dst, d);
-    else if (bx == 64) lbm_push_kernel<I, 64, TRT><<<grid, block, 0, st>>>(src, dst, d);
-    else lbm_push_kernel<I, 32, TRT><<<grid, block, 0, st>>>(src, dst, d);
+    if (bx == 128) lbm_push_kernel<T, I, 128, TRT><<<grid, block, 0, st>>>(src, dst, d);
+    else if (bx == 64) lbm_push_kernel<T, I, 64, TRT><<<grid, block, 0, st>>>(src, dst, d);
+    else lbm_push_kernel<T, I, 32, TRT><<<grid, block, 0, st>>>(src, dst, d);
 }
 
 // ------------------------------------------------------------------------------------ variant 2
@@ -192,26 +193,30 @@ static int lbm_validate(const ledds_lbm_params* p)
 
 static bool lbm_rowrot_ok(const ledds_lbm_params* p) { return p->nx % 64 == 0 && p->nx / 2 <= LEDDS_ROT_MAX_THREADS; }
 
-extern "C" int ledds_lbm_workspace_bytes(const ledds_lbm_params* p, size_t* f_bytes)
+// ---- the calls are written once for both precisions; T = float is the _f32 set of entry points
+template <typename T>
+static int lbm_workspace_bytes_t(const ledds_lbm_params* p, size_t* f_bytes)
 {
     const int rc = lbm_validate(p);
     if (rc) return rc;
     if (!f_bytes) return LEDDS_EINVAL;
-    *f_bytes = (size_t)2 * LEDDS_Q * p->nx * p->ny * p->nz * sizeof(double);
+    if (sizeof(T) == 4 && p->variant == 2) return LEDDS_EINVAL;
+    *f_bytes = (size_t)2 * LEDDS_Q * p->nx * p->ny * p->nz * sizeof(T);
     return LEDDS_OK;
 }
 
-extern "C" int ledds_lbm_init(ledds_lbm** out, const ledds_lbm_params* p, double* f, const double* rho,
-                              const double* u, void* stream)
+template <typename T>
+static int lbm_init_t(ledds_lbm** out, const ledds_lbm_params* p, T* f, const T* rho, const T* u, void* stream)
 {
     const int rc = lbm_validate(p);
     if (rc) return rc;
     if (!out || !f) return LEDDS_EINVAL;
     if (!ledds_aligned16(f) || !ledds_aligned16(rho) || !ledds_aligned16(u)) return LEDDS_EALIGN;
-    if (p->variant == 2 && !lbm_rowrot_ok(p)) return LEDDS_EINVAL;
+    if (p->variant == 2 && (sizeof(T) == 4 || !lbm_rowrot_ok(p))) return LEDDS_EINVAL;
     ledds_lbm* h = new (std::nothrow) ledds_lbm();
     if (!h) return LEDDS_EINVAL;
     h->p = *p;
+    h->f32 = sizeof(T) == 4;
     LbmDev& d = h->d;
     d.nx = p->nx; d.ny = p->ny; d.nz = p->nz;
     d.N = (long long)p->nx * p->ny * p->nz;
@@ -231,63 +236,81 @@ extern "C" int ledds_lbm_init(ledds_lbm** out, const ledds_lbm_params* p, double
     h->parity = 0;
     h->steps = 0;
     const int tb = 256;
-    lbm_init_eq_kernel<<<(unsigned)((d.N + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(f, rho, u, d.N);
+    lbm_init_eq_kernel<T><<<(unsigned)((d.N + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(f, rho, u, d.N);
     ledds_count_launch(1);
     if (cudaPeekAtLastError() != cudaSuccess) { delete h; return LEDDS_ECUDA; }
     *out = h;
     return LEDDS_OK;
 }
 
-extern "C" const double* ledds_lbm_current(const ledds_lbm* h, const double* f)
-{
-    return (h && f) ? f + (size_t)h->parity * LEDDS_Q * h->d.N : nullptr;
-}
+template <typename T>
+static bool lbm_handle_is(const ledds_lbm* h) { return h && h->f32 == (sizeof(T) == 4); }
 
-extern "C" int ledds_lbm_import(ledds_lbm* h, double* f, const double* fc, void* stream)
+template <typename T>
+static int lbm_import_t(ledds_lbm* h, T* f, const T* fc, void* stream)
 {
-    if (!h || !f || !fc) return LEDDS_EINVAL;
+    if (!lbm_handle_is<T>(h) || !f || !fc) return LEDDS_EINVAL;
     if (!ledds_aligned16(f) || !ledds_aligned16(fc)) return LEDDS_EALIGN;
-    double* cur = f + (size_t)h->parity * LEDDS_Q * h->d.N;
-    if (cudaMemcpyAsync(cur, fc, sizeof(double) * LEDDS_Q * h->d.N, cudaMemcpyDeviceToDevice, (cudaStream_t)stream) !=
-        cudaSuccess)
+    T* cur = f + (size_t)h->parity * LEDDS_Q * h->d.N;
+    if (cudaMemcpyAsync(cur, fc, sizeof(T) * LEDDS_Q * h->d.N, cudaMemcpyDeviceToDevice, (cudaStream_t)stream) != cudaSuccess)
         return LEDDS_ECUDA;
     return LEDDS_OK;
 }
 
 // one stream-collide launch src -> dst (used by ledds_lbm_step; coupled.cu has its own PSM launch)
-static int lbm_launch(const ledds_lbm* h, const double* src, double* dst, cudaStream_t st)
+template <typename T>
+static int lbm_launch(const ledds_lbm* h, const T* src, T* dst, cudaStream_t st);
+
+template <typename T>
+static int lbm_launch_push(const ledds_lbm* h, const T* src, T* dst, cudaStream_t st)
 {
     const LbmDev& d = h->d;
-    int variant = h->p.variant;
-    if (variant == 0) variant = 1;   // 3 = variant 1 with 64-bit indices whatever the size; measured on B200: the plain push kernel already runs at the HBM copy rate
-    if (variant != 2 && (d.ny > 65535 || d.nz > 65535)) return LEDDS_EINVAL;
+    if (d.ny > 65535 || d.nz > 65535) return LEDDS_EINVAL;
+    const bool u32 = lb_fits_u32(d.N) && h->p.variant != 3;   // 3 = 64-bit indices whatever the size
     ledds_prof_start(LEDDS_K_LBM, st);
-    if (variant == 2) {
+    if (u32 && !d.trt) lbm_push_launch<T, unsigned, false>(src, dst, d, st);
+    else if (u32) lbm_push_launch<T, unsigned, true>(src, dst, d, st);
+    else if (!d.trt) lbm_push_launch<T, long long, false>(src, dst, d, st);
+    else lbm_push_launch<T, long long, true>(src, dst, d, st);
+    ledds_prof_stop(LEDDS_K_LBM, st);
+    LEDDS_CHECK_LAUNCH();
+    return LEDDS_OK;
+}
+
+template <>
+int lbm_launch<float>(const ledds_lbm* h, const float* src, float* dst, cudaStream_t st)
+{
+    return lbm_launch_push<float>(h, src, dst, st);
+}
+
+template <>
+int lbm_launch<double>(const ledds_lbm* h, const double* src, double* dst, cudaStream_t st)
+{
+    const LbmDev& d = h->d;
+    // variant 0 (auto) = 1: measured on B200, the plain push kernel already runs at the HBM copy rate
+    if (h->p.variant != 2) return lbm_launch_push<double>(h, src, dst, st);
+    ledds_prof_start(LEDDS_K_LBM, st);
+    {
         const int tx = d.nx / 2;
         int ry = 1;
         while (ry < 8 && tx * ry * 2 <= LEDDS_ROT_MAX_THREADS && d.ny % (ry * 2) == 0) ry *= 2;
         dim3 block(tx, ry), grid(d.ny / ry, d.nz);
         if (d.trt) lbm_rowrot_kernel<true><<<grid, block, 0, st>>>(src, dst, d);
         else lbm_rowrot_kernel<false><<<grid, block, 0, st>>>(src, dst, d);
-    } else {
-        const bool u32 = lb_fits_u32(d.N) && variant != 3;
-        if (u32 && !d.trt) lbm_push_launch<unsigned, false>(src, dst, d, st);
-        else if (u32) lbm_push_launch<unsigned, true>(src, dst, d, st);
-        else if (!d.trt) lbm_push_launch<long long, false>(src, dst, d, st);
-        else lbm_push_launch<long long, true>(src, dst, d, st);
     }
     ledds_prof_stop(LEDDS_K_LBM, st);
     LEDDS_CHECK_LAUNCH();
     return LEDDS_OK;
 }
 
-extern "C" int ledds_lbm_step(ledds_lbm* h, double* f, int nsteps, void* stream)
+template <typename T>
+static int lbm_step_t(ledds_lbm* h, T* f, int nsteps, void* stream)
 {
-    if (!h || !f || nsteps < 0) return LEDDS_EINVAL;
+    if (!lbm_handle_is<T>(h) || !f || nsteps < 0) return LEDDS_EINVAL;
     if (!ledds_aligned16(f)) return LEDDS_EALIGN;
     const size_t half = (size_t)LEDDS_Q * h->d.N;
     for (int s = 0; s < nsteps; ++s) {
-        const int rc = lbm_launch(h, f + h->parity * half, f + (1 - h->parity) * half, (cudaStream_t)stream);
+        const int rc = lbm_launch<T>(h, f + h->parity * half, f + (1 - h->parity) * half, (cudaStream_t)stream);
         if (rc) return rc;
         h->parity ^= 1;
         h->steps++;
@@ -295,15 +318,50 @@ extern "C" int ledds_lbm_step(ledds_lbm* h, double* f, int nsteps, void* stream)
     return LEDDS_OK;
 }
 
-extern "C" int ledds_lbm_export(ledds_lbm* h, const double* f, double* fc, double* rho, double* u, void* stream)
+template <typename T>
+static int lbm_export_t(ledds_lbm* h, const T* f, T* fc, T* rho, T* u, void* stream)
 {
-    if (!h || !f) return LEDDS_EINVAL;
+    if (!lbm_handle_is<T>(h) || !f) return LEDDS_EINVAL;
     if (!ledds_aligned16(f) || !ledds_aligned16(fc) || !ledds_aligned16(rho) || !ledds_aligned16(u)) return LEDDS_EALIGN;
     const int tb = 256;
-    lbm_export_kernel<<<(unsigned)((h->d.N + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(
+    lbm_export_kernel<T><<<(unsigned)((h->d.N + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(
         f + (size_t)h->parity * LEDDS_Q * h->d.N, fc, rho, u, h->d.N);
     LEDDS_CHECK_LAUNCH();
     return LEDDS_OK;
+}
+
+extern "C" int ledds_lbm_workspace_bytes(const ledds_lbm_params* p, size_t* f_bytes) { return lbm_workspace_bytes_t<double>(p, f_bytes); }
+extern "C" int ledds_lbm_workspace_bytes_f32(const ledds_lbm_params* p, size_t* f_bytes) { return lbm_workspace_bytes_t<float>(p, f_bytes); }
+
+extern "C" int ledds_lbm_init(ledds_lbm** out, const ledds_lbm_params* p, double* f, const double* rho, const double* u,
+                              void* stream)
+{
+    return lbm_init_t<double>(out, p, f, rho, u, stream);
+}
+extern "C" int ledds_lbm_init_f32(ledds_lbm** out, const ledds_lbm_params* p, float* f, const float* rho, const float* u,
+                                  void* stream)
+{
+    return lbm_init_t<float>(out, p, f, rho, u, stream);
+}
+
+extern "C" const double* ledds_lbm_current(const ledds_lbm* h, const double* f)
+{
+    return (lbm_handle_is<double>(h) && f) ? f + (size_t)h->parity * LEDDS_Q * h->d.N : nullptr;
+}
+
+extern "C" int ledds_lbm_import(ledds_lbm* h, double* f, const double* fc, void* stream) { return lbm_import_t<double>(h, f, fc, stream); }
+extern "C" int ledds_lbm_import_f32(ledds_lbm* h, float* f, const float* fc, void* stream) { return lbm_import_t<float>(h, f, fc, stream); }
+
+extern "C" int ledds_lbm_step(ledds_lbm* h, double* f, int nsteps, void* stream) { return lbm_step_t<double>(h, f, nsteps, stream); }
+extern "C" int ledds_lbm_step_f32(ledds_lbm* h, float* f, int nsteps, void* stream) { return lbm_step_t<float>(h, f, nsteps, stream); }
+
+extern "C" int ledds_lbm_export(ledds_lbm* h, const double* f, double* fc, double* rho, double* u, void* stream)
+{
+    return lbm_export_t<double>(h, f, fc, rho, u, stream);
+}
+extern "C" int ledds_lbm_export_f32(ledds_lbm* h, const float* f, float* fc, float* rho, float* u, void* stream)
+{
+    return lbm_export_t<float>(h, f, fc, rho, u, stream);
 }
 
 extern "C" int ledds_lbm_destroy(ledds_lbm* h)
@@ -312,4 +370,4 @@ extern "C" int ledds_lbm_destroy(ledds_lbm* h)
     return LEDDS_OK;
 }
 
-extern "C" const char* ledds_version(void) { return "ledds-b200 0.1 (sm_100a, fp64)"; }
+extern "C" const char* ledds_version(void) { return "ledds-b200 0.2 (sm_100a, fp64; plain LBM also fp32)"; }

@@ -4,13 +4,14 @@
 
 // Eq. (22a), (22b): density and velocity of one cell.  Opposite directions are paired (q, q+1), so the sums
 // are short trees rather than 19-long dependent chains.
-__device__ __forceinline__ void lb_moments(const double (&f)[LEDDS_Q], double& rho, double& ux, double& uy, double& uz)
+template <typename T>
+__device__ __forceinline__ void lb_moments(const T (&f)[LEDDS_Q], T& rho, T& ux, T& uy, T& uz)
 {
-    double s[9], d[9];
+    T s[9], d[9];
 #pragma unroll
     for (int p = 0; p < 9; ++p) { s[p] = f[2 * p + 1] + f[2 * p + 2]; d[p] = f[2 * p + 1] - f[2 * p + 2]; }
-    const double r = (f[0] + s[0]) + ((s[1] + s[2]) + (s[3] + s[4])) + ((s[5] + s[6]) + (s[7] + s[8]));
-    double jx = 0.0, jy = 0.0, jz = 0.0;
+    const T r = (f[0] + s[0]) + ((s[1] + s[2]) + (s[3] + s[4])) + ((s[5] + s[6]) + (s[7] + s[8]));
+    T jx = T(0), jy = T(0), jz = T(0);
 #pragma unroll
     for (int p = 0; p < 9; ++p) {                         // d[p] = f_q - f_opp(q) carries c_q
         const int q = 2 * p + 1;
@@ -18,14 +19,15 @@ __device__ __forceinline__ void lb_moments(const double (&f)[LEDDS_Q], double& r
         if (lb_cy(q) == 1) jy += d[p]; else if (lb_cy(q) == -1) jy -= d[p];
         if (lb_cz(q) == 1) jz += d[p]; else if (lb_cz(q) == -1) jz -= d[p];
     }
-    const double inv = 1.0 / r;
+    const T inv = T(1) / r;
     rho = r; ux = jx * inv; uy = jy * inv; uz = jz * inv;
 }
 
 // c_q . u with the zero components folded away at compile time.
-__device__ __forceinline__ double lb_cdot(int q, double ux, double uy, double uz)
+template <typename T>
+__device__ __forceinline__ T lb_cdot(int q, T ux, T uy, T uz)
 {
-    double s = 0.0;
+    T s = T(0);
     if (lb_cx(q) == 1) s += ux; else if (lb_cx(q) == -1) s -= ux;
     if (lb_cy(q) == 1) s += uy; else if (lb_cy(q) == -1) s -= uy;
     if (lb_cz(q) == 1) s += uz; else if (lb_cz(q) == -1) s -= uz;
@@ -33,24 +35,26 @@ __device__ __forceinline__ double lb_cdot(int q, double ux, double uy, double uz
 }
 
 // Eq. (28) with c_s^2 = 1/3 for all 19 directions.
-__device__ __forceinline__ void lb_equilibrium(double (&fe)[LEDDS_Q], double rho, double ux, double uy, double uz)
+template <typename T>
+__device__ __forceinline__ void lb_equilibrium(T (&fe)[LEDDS_Q], T rho, T ux, T uy, T uz)
 {
-    const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
-    fe[0] = lb_w(0) * rho * k;
+    const T k = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+    fe[0] = T(lb_w(0)) * rho * k;
 #pragma unroll
     for (int q = 1; q < LEDDS_Q; q += 2) {            // q and q+1 are opposites
-        const double cu = lb_cdot(q, ux, uy, uz);
-        const double wr = lb_w(q) * rho;
-        const double even = wr * (k + 4.5 * cu * cu), odd = wr * 3.0 * cu;
+        const T cu = lb_cdot(q, ux, uy, uz);
+        const T wr = T(lb_w(q)) * rho;
+        const T even = wr * (k + T(4.5) * cu * cu), odd = wr * T(3) * cu;
         fe[q] = even + odd;
         fe[q + 1] = even - odd;
     }
 }
 
 // Eq. (24), (26): f* = f - omega (f - feq), in place.
-__device__ __forceinline__ void lb_collide_bgk(double (&f)[LEDDS_Q], double omega, double rho, double ux, double uy, double uz)
+template <typename T>
+__device__ __forceinline__ void lb_collide_bgk(T (&f)[LEDDS_Q], T omega, T rho, T ux, T uy, T uz)
 {
-    double fe[LEDDS_Q];
+    T fe[LEDDS_Q];
     lb_equilibrium(fe, rho, ux, uy, uz);
 #pragma unroll
     for (int q = 0; q < LEDDS_Q; ++q) f[q] = f[q] - omega * (f[q] - fe[q]);
@@ -58,35 +62,36 @@ __device__ __forceinline__ void lb_collide_bgk(double (&f)[LEDDS_Q], double omeg
 
 // Eq. (29)-(30): TRT.  f+- = (f_q +- f_qbar)/2 relax with dt/tau+ and dt/tau- towards the even and odd parts
 // of the equilibrium; the rest population has no odd part.
-__device__ __forceinline__ void lb_collide_trt(double (&f)[LEDDS_Q], double omega_p, double omega_m, double rho, double ux,
-                                               double uy, double uz)
+template <typename T>
+__device__ __forceinline__ void lb_collide_trt(T (&f)[LEDDS_Q], T omega_p, T omega_m, T rho, T ux,
+                                               T uy, T uz)
 {
-    const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
-    f[0] = f[0] - omega_p * (f[0] - lb_w(0) * rho * k);
+    const T k = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+    f[0] = f[0] - omega_p * (f[0] - T(lb_w(0)) * rho * k);
 #pragma unroll
     for (int q = 1; q < LEDDS_Q; q += 2) {
-        const double cu = lb_cdot(q, ux, uy, uz);
-        const double wr = lb_w(q) * rho;
-        const double even = wr * (k + 4.5 * cu * cu), odd = wr * 3.0 * cu;
-        const double rp = omega_p * (0.5 * (f[q] + f[q + 1]) - even), rm = omega_m * (0.5 * (f[q] - f[q + 1]) - odd);
+        const T cu = lb_cdot(q, ux, uy, uz);
+        const T wr = T(lb_w(q)) * rho;
+        const T even = wr * (k + T(4.5) * cu * cu), odd = wr * T(3) * cu;
+        const T rp = omega_p * (T(0.5) * (f[q] + f[q + 1]) - even), rm = omega_m * (T(0.5) * (f[q] - f[q + 1]) - odd);
         f[q] = f[q] - (rp + rm);
         f[q + 1] = f[q + 1] - (rp - rm);
     }
 }
 
 // the collision model is a compile-time choice: each kernel is instantiated for BGK and for TRT
-template <bool TRT>
-__device__ __forceinline__ void lb_collide(double (&f)[LEDDS_Q], const LbmDev& P, double rho, double ux, double uy, double uz)
+template <bool TRT, typename T>
+__device__ __forceinline__ void lb_collide(T (&f)[LEDDS_Q], const LbmDev& P, T rho, T ux, T uy, T uz)
 {
-    if (TRT) lb_collide_trt(f, P.omega, P.omega_minus, rho, ux, uy, uz);
-    else lb_collide_bgk(f, P.omega, rho, ux, uy, uz);
+    if (TRT) lb_collide_trt(f, (T)P.omega, (T)P.omega_minus, rho, ux, uy, uz);
+    else lb_collide_bgk(f, (T)P.omega, rho, ux, uy, uz);
 }
 
 // Where does the link q that starts at coordinate `r` on one axis end?  Returns the target
 // coordinate (wrapped on a periodic axis); sets `bounced` and adds c_q . u_wall of the crossed
 // wall when the axis is walled (halfway bounce-back).
-template <int AXIS>
-__device__ __forceinline__ int lb_axis_target(const LbmDev& P, int q, int c, int r, int n, bool& bounced, double& cuw)
+template <int AXIS, typename T>
+__device__ __forceinline__ int lb_axis_target(const LbmDev& P, int q, int c, int r, int n, bool& bounced, T& cuw)
 {
     if (c == 0) return r;
     int t = r + c;
@@ -95,7 +100,7 @@ __device__ __forceinline__ int lb_axis_target(const LbmDev& P, int q, int c, int
             bounced = true;
             if (P.any_wall_velocity) {
                 const double* uw = P.uw + (AXIS * 2 + (t < 0 ? 0 : 1)) * 3;
-                cuw += lb_cdot(q, uw[0], uw[1], uw[2]);
+                cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]);
             }
         } else {
             t = t < 0 ? t + n : t - n;
@@ -111,8 +116,8 @@ static inline int lb_block_x(int nx) { return nx > 64 ? 128 : (nx > 32 ? 64 : 32
 static inline bool lb_fits_u32(long long N) { return (unsigned long long)N * LEDDS_Q < 0xffffffffull; }
 
 // The 19 pre-collision populations of cell `cell`.
-template <typename I>
-__device__ __forceinline__ void lb_load(const double* __restrict__ fin, I N, I cell, double (&f)[LEDDS_Q])
+template <typename I, typename T>
+__device__ __forceinline__ void lb_load(const T* __restrict__ fin, I N, I cell, T (&f)[LEDDS_Q])
 {
 #pragma unroll
     for (int q = 0; q < LEDDS_Q; ++q) f[q] = __ldg(fin + (I)((I)q * N + cell));
@@ -147,7 +152,8 @@ struct LbPush {
 
     // post-collision population v of direction q (a compile-time constant after unrolling); rho = the cell's
     // pre-collision density (moving-wall term, G19)
-    __device__ __forceinline__ void put(double* __restrict__ fout, const LbmDev& P, int q, double v, double rho) const
+    template <typename T>
+    __device__ __forceinline__ void put(T* __restrict__ fout, const LbmDev& P, int q, T v, T rho) const
     {
         const int cx = lb_cx(q), cy = lb_cy(q), cz = lb_cz(q);
         bool bounced = false;
@@ -157,20 +163,20 @@ struct LbPush {
         if (!bounced) {
             fout[(I)((I)q * N + rb[cz + 1][cy + 1] + (I)tx[cx + 1])] = v;
         } else {
-            double cuw = 0.0;                                   // c_q . u_wall summed over the crossed walls
+            T cuw = T(0);                                   // c_q . u_wall summed over the crossed walls
             if (P.any_wall_velocity) {
-                if (cx != 0 && wx[cx > 0]) { const double* uw = P.uw + (0 + (cx > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
-                if (cy != 0 && wy[cy > 0]) { const double* uw = P.uw + (2 + (cy > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
-                if (cz != 0 && wz[cz > 0]) { const double* uw = P.uw + (4 + (cz > 0)) * 3; cuw += lb_cdot(q, uw[0], uw[1], uw[2]); }
+                if (cx != 0 && wx[cx > 0]) { const double* uw = P.uw + (0 + (cx > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
+                if (cy != 0 && wy[cy > 0]) { const double* uw = P.uw + (2 + (cy > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
+                if (cz != 0 && wz[cz > 0]) { const double* uw = P.uw + (4 + (cz > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
             }
-            fout[(I)((I)lb_opp(q) * N + rb[1][1] + (I)x)] = v - 6.0 * lb_w(q) * rho * cuw;
+            fout[(I)((I)lb_opp(q) * N + rb[1][1] + (I)x)] = v - T(6.0 * lb_w(q)) * rho * cuw;
         }
     }
 };
 
-template <typename I>
-__device__ __forceinline__ void lb_push_store(double* __restrict__ fout, const LbmDev& P, int x, int y, int z,
-                                              const double (&fs)[LEDDS_Q], double rho)
+template <typename I, typename T>
+__device__ __forceinline__ void lb_push_store(T* __restrict__ fout, const LbmDev& P, int x, int y, int z,
+                                              const T (&fs)[LEDDS_Q], T rho)
 {
     const LbPush<I> push(P, x, y, z);
 #pragma unroll

@@ -16,28 +16,36 @@ def _dev(a, dtype=torch.float64):
 
 
 class Lbm:
-    """D3Q19 BGK lattice on the GPU (ledds_lbm_*)."""
+    """D3Q19 lattice on the GPU (ledds_lbm_*; precision="f32" -> the ledds_lbm_*_f32 calls on float buffers)."""
 
-    def __init__(self, lbm: dict, rho=None, u=None, f_canonical=None):
+    def __init__(self, lbm: dict, rho=None, u=None, f_canonical=None, precision="f64"):
         self.p = L.lbm_params(lbm)
         self.shape = tuple(lbm["shape"])
         self.N = self.shape[0] * self.shape[1] * self.shape[2]
-        self.f = torch.empty(L.ledds_lbm_workspace_bytes(self.p) // 8, dtype=torch.float64, device="cuda")
-        rho_d = None if rho is None else _dev(rho).reshape(-1)
-        u_d = None if u is None else _dev(u).reshape(-1)
-        self.h = L.ledds_lbm_init(self.p, self.f, rho_d, u_d)
+        f32 = self.f32 = precision == "f32"
+        if precision not in ("f64", "f32"):
+            raise ValueError(precision)
+        self.dtype = torch.float32 if f32 else torch.float64
+        self._bytes, self._init, self._import, self._step, self._export = (
+            (L.ledds_lbm_workspace_bytes_f32, L.ledds_lbm_init_f32, L.ledds_lbm_import_f32, L.ledds_lbm_step_f32,
+             L.ledds_lbm_export_f32) if f32 else
+            (L.ledds_lbm_workspace_bytes, L.ledds_lbm_init, L.ledds_lbm_import, L.ledds_lbm_step, L.ledds_lbm_export))
+        self.f = torch.empty(self._bytes(self.p) // (4 if f32 else 8), dtype=self.dtype, device="cuda")
+        rho_d = None if rho is None else _dev(rho, self.dtype).reshape(-1)
+        u_d = None if u is None else _dev(u, self.dtype).reshape(-1)
+        self.h = self._init(self.p, self.f, rho_d, u_d)
         if f_canonical is not None:
-            L.ledds_lbm_import(self.h, self.f, _dev(f_canonical).reshape(-1))
+            self._import(self.h, self.f, _dev(f_canonical, self.dtype).reshape(-1))
         torch.cuda.current_stream().synchronize()     # rho_d / u_d may be freed after this
 
     def step(self, nsteps=1):
-        L.ledds_lbm_step(self.h, self.f, nsteps)
+        self._step(self.h, self.f, nsteps)
 
     def export(self, want_f=True, want_moments=False):
-        fc = torch.empty(19 * self.N, dtype=torch.float64, device="cuda") if want_f else None
-        rho = torch.empty(self.N, dtype=torch.float64, device="cuda") if want_moments else None
-        u = torch.empty(3 * self.N, dtype=torch.float64, device="cuda") if want_moments else None
-        L.ledds_lbm_export(self.h, self.f, fc, rho, u)
+        fc = torch.empty(19 * self.N, dtype=self.dtype, device="cuda") if want_f else None
+        rho = torch.empty(self.N, dtype=self.dtype, device="cuda") if want_moments else None
+        u = torch.empty(3 * self.N, dtype=self.dtype, device="cuda") if want_moments else None
+        self._export(self.h, self.f, fc, rho, u)
         out = []
         if want_f:
             out.append(fc.cpu().numpy().reshape(19, self.N))

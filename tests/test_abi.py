@@ -16,7 +16,7 @@ def _lib():
 def test_every_declared_symbol_is_exported():
     hdr = open(os.path.join(ROOT, "include", "ledds.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = sorted(set(re.findall(r"\b(ledds_[a-z_]+)\s*\(", hdr)))
+    names = sorted(set(re.findall(r"\b(ledds_[a-z0-9_]+)\s*\(", hdr)))
     assert len(names) >= 15
     lib = _lib()
     for n in names:
@@ -27,7 +27,7 @@ def test_binding_names_match_header():
     import paper_2512_04997_b200 as L
     hdr = open(os.path.join(ROOT, "include", "ledds.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"\b(ledds_[a-z_]+)\s*\(", hdr))
+    names = set(re.findall(r"\b(ledds_[a-z0-9_]+)\s*\(", hdr))
     assert names == set(L.EXPORTS)
     for n in names - {"ledds_lbm_current"}:
         assert callable(getattr(L, n)), n
@@ -51,6 +51,11 @@ def test_parameter_validation_without_gpu():
     import pytest
     p = L.lbm_params(dict(shape=(8, 8, 8), tau=0.6, bc=(0, 0, 0), u_wall=None))
     assert L.ledds_lbm_workspace_bytes(p) == 2 * 19 * 512 * 8
+    assert L.ledds_lbm_workspace_bytes_f32(p) == 2 * 19 * 512 * 4
+    p.variant = 2
+    with pytest.raises(L.LeddsError):
+        L.ledds_lbm_workspace_bytes_f32(p)                     # no fp32 row-rotate kernel
+    p.variant = 0
     p.tau = 0.5
     with pytest.raises(L.LeddsError):
         L.ledds_lbm_workspace_bytes(p)

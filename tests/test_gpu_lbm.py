@@ -103,3 +103,85 @@ def test_import_roundtrip_and_errors():
         Lbm(dict(shape=(37, 4, 4), tau=0.9, bc=(0, 0, 0), u_wall=None, variant=2))
     with pytest.raises(L.LeddsError):
         L.ledds_lbm_step(g.h, g.f[1:], 1)                    # misaligned pointer -> LEDDS_EALIGN
+
+
+# ------------------------------------------------------------------------------------ fp32 variant
+# the paper's single-precision runs.  The oracle stays fp64; the bound on the difference
+# is the rounding of the fp32 arithmetic: every step adds at most ~8 roundings of size
+# 2^-24 max|f| to a population (tree sums of Eq. 22, Eq. 28, Eq. 26), so after `steps` steps
+# |f32 - f64| <= 8 * steps * 2^-24 * max|f|; the observed difference is ~sqrt(steps) of that.
+EPS32 = 2.0 ** -24
+
+
+def run_pair_f32(shape, tau, bc, u_wall, steps, variant, collision=0, seed=0):
+    import oracle
+    from paper_2512_04997_b200 import Lbm
+    rho, u = W.random_flow(shape, seed)
+    rho, u = rho.astype(np.float32), u.astype(np.float32)     # both sides start from the same fp32 fields
+    lbm = dict(shape=shape, tau=tau, bc=bc, u_wall=u_wall, variant=variant, collision=collision)
+    g = Lbm(lbm, rho, u, precision="f32")
+    f0 = g.export()
+    assert f0.dtype == np.float32
+    ref0 = oracle.lbm_equilibrium(shape, rho.astype(np.float64), u.astype(np.float64))
+    assert np.abs(f0 - ref0).max() <= 4 * EPS32 * np.abs(ref0).max()
+    g.step(steps)
+    f = g.export()
+    ref = oracle.lbm_run(shape, ref0, tau, steps, bc=bc, u_wall=u_wall, trt=bool(collision))
+    return f.astype(np.float64), ref
+
+
+@pytest.mark.parametrize("variant,collision", [(1, 0), (3, 0), (1, 1)])
+@pytest.mark.parametrize("shape,bc,uw", [
+    ((64, 12, 10), (0, 0, 0), None),
+    ((64, 12, 10), (1, 1, 1), MOVING),
+    ((130, 6, 5), (0, 0, 1), MOVING),
+    ((37, 7, 9), (1, 0, 0), MOVING),
+])
+def test_f32_populations_after_100_steps(variant, collision, shape, bc, uw):
+    f, ref = run_pair_f32(shape, 0.6, bc, uw, 100, variant, collision)
+    err = np.abs(f - ref).max() / np.abs(ref).max()
+    assert err <= 8 * 100 * EPS32
+    assert np.sqrt(np.mean((f - ref) ** 2)) <= 8 * 10 * EPS32 * np.abs(ref).max()    # random-walk growth
+
+
+def test_f32_tgv_decay_and_mass():
+    from paper_2512_04997_b200 import Lbm
+    shape = (64, 64, 64)
+    rho, u = W.tgv(shape, 0.02, 1.0, "xy")
+    g = Lbm(dict(shape=shape, tau=0.6, bc=(0, 0, 0), u_wall=None), rho, u, precision="f32")
+    f0 = g.export().astype(np.float64)
+    g.step(100); _, r1, u1 = g.export(want_moments=True)
+    g.step(400); f2, r2, u2 = g.export(want_moments=True)
+    assert abs(f2.astype(np.float64).sum() - f0.sum()) <= 500 * EPS32 * f0.sum()
+    rate = 4.0 * (0.1 / 3.0) * (2 * np.pi / 64) ** 2
+    e1, e2 = (u1.astype(np.float64) ** 2).sum(), (u2.astype(np.float64) ** 2).sum()
+    assert abs(np.log(e1 / e2) / 400 / rate - 1.0) < 0.01
+
+
+def test_f32_full_size_config2_against_oracle():
+    import oracle
+    from paper_2512_04997_b200 import Lbm
+    lbm, rho, u = W.cfg2_tgv(128)
+    rho, u = rho.astype(np.float32), u.astype(np.float32)
+    g = Lbm(lbm, rho, u, precision="f32")
+    g.step(10)
+    f = g.export().astype(np.float64)
+    ref = oracle.lbm_run(lbm["shape"], oracle.lbm_equilibrium(lbm["shape"], rho.astype(np.float64), u.astype(np.float64)),
+                         lbm["tau"], 10)
+    assert np.abs(f - ref).max() <= 8 * 10 * EPS32 * np.abs(ref).max()
+
+
+def test_f32_handles_and_fp64_calls_do_not_mix():
+    import paper_2512_04997_b200 as L
+    from paper_2512_04997_b200 import Lbm
+    lbm = dict(shape=(64, 4, 4), tau=0.9, bc=(0, 0, 0), u_wall=None)
+    g32, g64 = Lbm(lbm, precision="f32"), Lbm(lbm)
+    with pytest.raises(L.LeddsError):
+        L.ledds_lbm_step(g32.h, g64.f, 1)
+    with pytest.raises(L.LeddsError):
+        L.ledds_lbm_step_f32(g64.h, g32.f, 1)
+    with pytest.raises(L.LeddsError):
+        Lbm(dict(lbm, variant=2), precision="f32")           # no row-rotate kernel in fp32
+    f0 = (np.random.default_rng(1).random((19, 64 * 16)) + 0.5).astype(np.float32)
+    g = Lbm(lbm, f_canonical=f0, precision="f32")
+    assert np.array_equal(g.export(), f0)
