@@ -245,6 +245,22 @@ def run_ours(args, rank, world):
         sub["cfg2_lbm_tgv128_trt"] = {"mlups": round(nc2 / ms2t / 1e3, 1), "ms_per_step": round(ms2t, 5), "steps": ks,
                                        "hbm_gbs": round(304.0 * nc2 / ms2t / 1e6, 1), "hbm_frac": round(304.0 * nc2 / ms2t / 1e6 / peak, 4)}
         del gt
+        # fp32 variant of the plain LBM path (152 B/cell), at 128^3 and at the headline lattice size
+        if not args.sub_large_only:
+            for nn in ((128, 256) if not small else (64,)):
+                lbf, rhof, uuf = W.cfg2_tgv(nn)
+                ncf = int(np.prod(lbf["shape"]))
+                for prec, bpc in (("f32", 152.0), ("f64", 304.0)):
+                    if prec == "f64" and nn == 128:
+                        continue                                         # that is cfg2_lbm_tgv128 above
+                    gf = Lbm(lbf, rhof, uuf, precision=prec)
+                    gf.step(20); torch.cuda.synchronize()
+                    kf = 400 if not small else 100
+                    msf = timed(gf.step, kf) / kf
+                    sub[f"lbm_tgv{nn}_{prec}"] = {"mlups": round(ncf / msf / 1e3, 1), "ms_per_step": round(msf, 5), "steps": kf,
+                                                  "hbm_gbs": round(bpc * ncf / msf / 1e6, 1),
+                                                  "hbm_frac": round(bpc * ncf / msf / 1e6 / peak, 4), "dtype": prec}
+                    del gf
         # the paper's own validation combination on the headline workload: TRT collision (Eq. 29-31) + subdivision
         # solid fraction (Eq. 38, 10^3 points per cell)
         if not args.sub_large_only:
