@@ -97,7 +97,8 @@ int ledds_lbm_destroy(ledds_lbm* h);
  * 19 x N floats), boundaries and collision models; all arithmetic in fp32; rho, u and f_canonical are float
  * arrays.  variant 2 (row-rotate) does not exist in fp32: LEDDS_EINVAL.  A handle made by
  * ledds_lbm_init_f32 is accepted by the _f32 calls and ledds_lbm_destroy only, a handle made by
- * ledds_lbm_init by the fp64 calls only (LEDDS_EINVAL otherwise).  The coupled step is fp64 in this version. */
+ * ledds_lbm_init by the fp64 calls only (LEDDS_EINVAL otherwise).  ledds_coupled_step_f32 below takes the
+ * fp32 handle. */
 int ledds_lbm_workspace_bytes_f32(const ledds_lbm_params* p, size_t* f_bytes);
 int ledds_lbm_init_f32(ledds_lbm** h, const ledds_lbm_params* p, float* f, const float* rho, const float* u,
                        void* stream);
@@ -194,6 +195,17 @@ int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c
                        double* x, double* v, double* w, double* a, double* alpha, const double* radius,
                        double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
                        int32_t* status, int nsteps, void* stream);
+
+/* The coupled step on an fp32 lattice (handle from ledds_lbm_init_f32, f = 2 x 19 x N floats): the populations,
+ * their moments (Eq. 22) and the collision (Eq. 26 / 29-30, 32-37) are single precision; the geometry of the
+ * solids (Eq. 35, 39-40, 38), the sums of Eq. (41)-(42) and the whole DEM step stay double, so the cells a
+ * solid cuts, the contact list and the order-independence of f_hyd / m_hyd are those of the fp64 call.  All other
+ * arguments, the scratch buffers (ledds_cpl_workspace_bytes / ledds_cpl_init take either kind of handle) and the
+ * error behaviour are as for ledds_coupled_step; LEDDS_EINVAL when the handle's precision does not match. */
+int ledds_coupled_step_f32(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c, double r_max, float* f,
+                           double* x, double* v, double* w, double* a, double* alpha, const double* radius,
+                           double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
+                           int32_t* status, int nsteps, void* stream);
 
 /* ------------------------------------------------------------------------------ measurement
  * Optional per-kernel timing with CUDA events recorded on the launching stream around each kernel

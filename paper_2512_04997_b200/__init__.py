@@ -22,7 +22,8 @@ ST_CONTACT_OVERFLOW, ST_SOLID_OVERFLOW, ST_COINCIDENT, ST_NONFINITE = 1, 2, 4, 8
 EXPORTS = ["ledds_lbm_workspace_bytes", "ledds_lbm_init", "ledds_lbm_import", "ledds_lbm_step", "ledds_lbm_export",
            "ledds_lbm_current", "ledds_lbm_destroy", "ledds_lbm_workspace_bytes_f32", "ledds_lbm_init_f32",
            "ledds_lbm_import_f32", "ledds_lbm_step_f32", "ledds_lbm_export_f32", "ledds_dem_workspace_bytes", "ledds_dem_init", "ledds_dem_step",
-           "ledds_dem_query", "ledds_dem_destroy", "ledds_cpl_workspace_bytes", "ledds_cpl_init", "ledds_coupled_step", "ledds_version",
+           "ledds_dem_query", "ledds_dem_destroy", "ledds_cpl_workspace_bytes", "ledds_cpl_init", "ledds_coupled_step",
+           "ledds_coupled_step_f32", "ledds_version",
            "ledds_profile", "ledds_profile_read", "ledds_launch_count"]
 
 
@@ -239,6 +240,13 @@ def ledds_coupled_step(lbm, dem, c: CplParams, r_max, f, x, v, w, a, alpha, radi
     _check(_lib.ledds_coupled_step(lbm, dem, C.byref(c), C.c_double(r_max), _p(f), _p(x), _p(v), _p(w), _p(a), _p(alpha),
                                    _p(radius), _p(f_hyd), _p(m_hyd), _p(history), _p(scratch), _p(cpl_scratch),
                                    _p(status), C.c_int(nsteps), _stream()), "ledds_coupled_step")
+
+
+def ledds_coupled_step_f32(lbm, dem, c: CplParams, r_max, f, x, v, w, a, alpha, radius, f_hyd, m_hyd, history, scratch,
+                           cpl_scratch, status, nsteps=1):
+    _check(_lib.ledds_coupled_step_f32(lbm, dem, C.byref(c), C.c_double(r_max), _p(f), _p(x), _p(v), _p(w), _p(a), _p(alpha),
+                                       _p(radius), _p(f_hyd), _p(m_hyd), _p(history), _p(scratch), _p(cpl_scratch),
+                                       _p(status), C.c_int(nsteps), _stream()), "ledds_coupled_step_f32")
 
 
 from .sim import Lbm, Dem, Coupled  # noqa: E402  (buffer-owning convenience wrappers; no arithmetic)

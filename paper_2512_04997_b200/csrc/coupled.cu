@@ -161,24 +161,28 @@ __global__ void __launch_bounds__(256) cpl_raster_kernel(const LbmDev P, const C
 // thread's column of shared memory with asynchronous copies (no registers tied up while they are in flight);
 // the moments are summed from there and the collision runs pair by pair, each pair pushed as soon as it is
 // collided.  The kernel needs <= 64 registers, so 8 blocks (32 warps) are resident per SM.
-template <typename I, int BX, bool TRT, bool SUBDIV>
-__global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(const double* __restrict__ fin, double* __restrict__ fout,
+// T = population type: double on the path of the configs; float = the fp32 variant (ledds_coupled_step_f32), where
+// the populations, their moments, the collision and the per-cell terms of the solids (Eq. 35-36, 39-42) are single
+// precision; which cells a solid cuts is decided by the raster (in double) and the sums of Eq. (41)-(42) over the
+// cells are accumulated in double / fixed point as for T = double.
+template <typename T, typename I, int BX, bool TRT, bool SUBDIV>
+__global__ void __launch_bounds__(PSM_BLOCK, sizeof(T) == 4 ? PSM_MIN_BLOCKS_F32 : PSM_MIN_BLOCKS) lbm_psm_kernel(const T* __restrict__ fin, T* __restrict__ fout,
                                                                const __grid_constant__ LbmDev P,
                                                                const __grid_constant__ CplDev C)
 {
-    __shared__ double sfull[LEDDS_Q][PSM_BLOCK];
-    __shared__ double s2[PSM_S2_ROWS][PSM_BLOCK];
+    __shared__ T sfull[LEDDS_Q][PSM_BLOCK];
+    __shared__ T s2[PSM_S2_ROWS][PSM_BLOCK];
     const int x = blockIdx.x * BX + (int)(threadIdx.x % BX);
     const int y = blockIdx.y * (PSM_BLOCK / BX) + (int)(threadIdx.x / BX), z = blockIdx.z;   // a warp lies inside one row
     const bool active = x < P.nx && y < P.ny;
     const I cell = active ? ((I)z * (I)P.ny + (I)y) * (I)P.nx + (I)x : (I)0;   // a lane past the lattice reads cell 0, stores nothing
-    double* sf = &sfull[0][threadIdx.x];
+    T* sf = &sfull[0][threadIdx.x];
     {
         const uint32_t dst = (uint32_t)__cvta_generic_to_shared(sf);
 #pragma unroll
         for (int q = 0; q < LEDDS_Q; ++q)
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + (uint32_t)(q * PSM_BLOCK * sizeof(double))),
-                         "l"(fin + (I)((I)q * (I)P.N + cell))
+            asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(dst + (uint32_t)(q * PSM_BLOCK * sizeof(T))),
+                         "l"(fin + (I)((I)q * (I)P.N + cell)), "n"((int)sizeof(T))
                          : "memory");
         asm volatile("cp.async.commit_group;" ::: "memory");
     }
@@ -188,55 +192,56 @@ __global__ void __launch_bounds__(PSM_BLOCK, PSM_MIN_BLOCKS) lbm_psm_kernel(cons
         id0 = slot.x; id1 = slot.y;
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
-    double rho, ux, uy, uz;
+    T rho, ux, uy, uz;
     {
-        double f[LEDDS_Q];
+        T f[LEDDS_Q];
 #pragma unroll
         for (int q = 0; q < LEDDS_Q; ++q) f[q] = sf[q * PSM_BLOCK];
         lb_moments(f, rho, ux, uy, uz);
     }
     const LbPush<I> push(P, x, y, z);
     if (!__any_sync(0xffffffffu, id0 != PSM_EMPTY)) {
-        bgk_collide_stream<I, TRT>(sf, P.omega, rho, ux, uy, uz, push, fout, P, active);
+        bgk_collide_stream<I, TRT>(sf, (T)P.omega, rho, ux, uy, uz, push, fout, P, active);
         return;
     }
     if (id0 != PSM_EMPTY) C.slots[cell] = make_uint2(PSM_EMPTY, PSM_EMPTY);           // consumed: free for the next step
     const bool two = __any_sync(0xffffffffu, id1 != PSM_EMPTY);
-    double* s2col = &s2[0][threadIdx.x];
+    T* s2col = &s2[0][threadIdx.x];
     if (two) {                                                                        // warp-uniform, rarer
-        double B1, uk1[3], rec[6];
+        T B1, uk1[3];
+        double rec[6];
         int ent;
         psm_solid_terms<SUBDIV>(P, C, x, y, z, id1, rho, ux, uy, uz, B1, uk1, rec, ent);
         s2col[0] = B1;
-        s2col[PSM_BLOCK] = 1.0 - 1.5 * (uk1[0] * uk1[0] + uk1[1] * uk1[1] + uk1[2] * uk1[2]);
+        s2col[PSM_BLOCK] = T(1) - T(1.5) * (uk1[0] * uk1[0] + uk1[1] * uk1[1] + uk1[2] * uk1[2]);
         s2col[2 * PSM_BLOCK] = uk1[0]; s2col[3 * PSM_BLOCK] = uk1[1]; s2col[4 * PSM_BLOCK] = uk1[2];
         psm_run_reduce(C, id1, ent, rec);
     }
-    double B0, uk0[3];
+    T B0, uk0[3];
     {
         double rec[6];
         int ent;
         psm_solid_terms<SUBDIV>(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
         psm_run_reduce(C, id0, ent, rec);
     }
-    psm_collide_stream<I, TRT>(sf, P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
+    psm_collide_stream<I, TRT>(sf, (T)P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
 }
 
-template <typename I, bool TRT, bool SUBDIV>
-static void psm_launch2(const double* src, double* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
+template <typename T, typename I, bool TRT, bool SUBDIV>
+static void psm_launch2(const T* src, T* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
 {
     const int bx = lb_block_x(d.nx), rows = PSM_BLOCK / bx;
     const dim3 block(PSM_BLOCK), grid((d.nx + bx - 1) / bx, (d.ny + rows - 1) / rows, d.nz);
-    if (bx == 128) lbm_psm_kernel<I, 128, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
-    else if (bx == 64) lbm_psm_kernel<I, 64, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
-    else lbm_psm_kernel<I, 32, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
+    if (bx == 128) lbm_psm_kernel<T, I, 128, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
+    else if (bx == 64) lbm_psm_kernel<T, I, 64, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
+    else lbm_psm_kernel<T, I, 32, TRT, SUBDIV><<<grid, block, 0, st>>>(src, dst, d, C);
 }
 
-template <typename I, bool TRT>
-static void psm_launch(const double* src, double* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
+template <typename T, typename I, bool TRT>
+static void psm_launch(const T* src, T* dst, const LbmDev& d, const CplDev& C, cudaStream_t st)
 {
-    if (C.subdiv) psm_launch2<I, TRT, true>(src, dst, d, C, st);
-    else psm_launch2<I, TRT, false>(src, dst, d, C, st);
+    if (C.subdiv) psm_launch2<T, I, TRT, true>(src, dst, d, C, st);
+    else psm_launch2<T, I, TRT, false>(src, dst, d, C, st);
 }
 
 // ------------------------------------------------------------------------------------ finish
@@ -262,7 +267,7 @@ static size_t cpl_align(size_t v) { return (v + 255) & ~(size_t)255; }
 static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl_params* c, double r_max, CplDev* C,
                      CplLayout* L)
 {
-    if (!lbm || lbm->f32 || !dem || !c || c->n_sub < 1 || (c->solid_fraction != 0 && c->solid_fraction != 1) || !(c->dx > 0.0) || !(c->rho_f > 0.0) || !(r_max > 0.0))
+    if (!lbm || !dem || !c || c->n_sub < 1 || (c->solid_fraction != 0 && c->solid_fraction != 1) || !(c->dx > 0.0) || !(c->rho_f > 0.0) || !(r_max > 0.0))
         return LEDDS_EINVAL;
     const double rc = cbrt(3.0 / (4.0 * 3.14159265358979323846));           // Eq. (40), dx = 1
     const double Dt = c->n_sub * dem->d.dt;
@@ -326,12 +331,13 @@ extern "C" int ledds_cpl_init(const ledds_lbm* lbm, const ledds_dem* dem, const 
     return LEDDS_OK;
 }
 
-extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c, double r_max, double* f,
-                                  double* x, double* v, double* w, double* a, double* alpha, const double* radius,
-                                  double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
-                                  int32_t* status, int nsteps, void* stream)
+template <typename T>
+static int coupled_step_t(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c, double r_max, T* f, double* x, double* v,
+                          double* w, double* a, double* alpha, const double* radius, double* f_hyd, double* m_hyd,
+                          void* history, void* scratch, void* cpl_scratch, int32_t* status, int nsteps, void* stream)
 {
     if (!lbm || !dem || !f || !cpl_scratch || !status || nsteps < 0) return LEDDS_EINVAL;
+    if (lbm->f32 != (sizeof(T) == 4)) return LEDDS_EINVAL;                    // the handle fixes the population type
     if (dem->d.n != 0 && (!x || !v || !w || !a || !alpha || !radius || !f_hyd || !m_hyd || !history || !scratch))
         return LEDDS_EINVAL;                                                 // an empty particle system needs none of them
     const void* ptrs[] = {f, x, v, w, a, alpha, radius, f_hyd, m_hyd, history, scratch, cpl_scratch, status};
@@ -390,13 +396,13 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         LEDDS_CHECK_LAUNCH();
         ledds_prof_start(LEDDS_K_LBM, st);
         {
-            const double* src = f + lbm->parity * half;
-            double* dst = f + (1 - lbm->parity) * half;
+            const T* src = f + lbm->parity * half;
+            T* dst = f + (1 - lbm->parity) * half;
             const bool u32 = lb_fits_u32(d.N) && lbm->p.variant != 3;
-            if (u32 && !d.trt) psm_launch<unsigned, false>(src, dst, d, C, st);
-            else if (u32) psm_launch<unsigned, true>(src, dst, d, C, st);
-            else if (!d.trt) psm_launch<long long, false>(src, dst, d, C, st);
-            else psm_launch<long long, true>(src, dst, d, C, st);
+            if (u32 && !d.trt) psm_launch<T, unsigned, false>(src, dst, d, C, st);
+            else if (u32) psm_launch<T, unsigned, true>(src, dst, d, C, st);
+            else if (!d.trt) psm_launch<T, long long, false>(src, dst, d, C, st);
+            else psm_launch<T, long long, true>(src, dst, d, C, st);
         }
         ledds_prof_stop(LEDDS_K_LBM, st);
         LEDDS_CHECK_LAUNCH();
@@ -415,4 +421,22 @@ extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cp
         }
     }
     return LEDDS_OK;
+}
+
+extern "C" int ledds_coupled_step(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c, double r_max, double* f,
+                                  double* x, double* v, double* w, double* a, double* alpha, const double* radius,
+                                  double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
+                                  int32_t* status, int nsteps, void* stream)
+{
+    return coupled_step_t<double>(lbm, dem, c, r_max, f, x, v, w, a, alpha, radius, f_hyd, m_hyd, history, scratch, cpl_scratch,
+                                  status, nsteps, stream);
+}
+
+extern "C" int ledds_coupled_step_f32(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params* c, double r_max, float* f,
+                                      double* x, double* v, double* w, double* a, double* alpha, const double* radius,
+                                      double* f_hyd, double* m_hyd, void* history, void* scratch, void* cpl_scratch,
+                                      int32_t* status, int nsteps, void* stream)
+{
+    return coupled_step_t<float>(lbm, dem, c, r_max, f, x, v, w, a, alpha, radius, f_hyd, m_hyd, history, scratch, cpl_scratch,
+                                 status, nsteps, stream);
 }

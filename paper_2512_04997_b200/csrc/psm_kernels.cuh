@@ -6,6 +6,9 @@
 #ifndef PSM_MIN_BLOCKS
 #define PSM_MIN_BLOCKS 5      // resident blocks per SM the collide kernel is compiled for (<= 102 registers)
 #endif
+#ifndef PSM_MIN_BLOCKS_F32
+#define PSM_MIN_BLOCKS_F32 8  // the same for float populations (<= 64 registers)
+#endif
 #define PSM_EMPTY 0xffffffffu
 
 // Layout of the caller-owned coupling scratch (ledds_cpl_workspace_bytes):
@@ -113,41 +116,49 @@ __device__ __forceinline__ double cpl_beta_count(const SubdivPoints& p)
 // What one solid does to one cell: weight B (Eq. 36, 39-40), solid velocity at the cell (Eq. 35), the terms
 // of Eq. (41)-(42) in lattice units (rec) and the index of the cell in the solid's box (ent).
 // id = PSM_EMPTY: no solid here: B = 0, rec = 0, ent = -1 (the lane still runs the code of its warp).
-template <bool SUBDIV>
+// R = arithmetic type of the cell's terms: double, or float for the fp32 lattice (there the offsets d = r_j - r_k are
+// still formed in double from the same floor(x_k) as the raster's, so `ent` addresses the same box cell).
+template <bool SUBDIV, typename R>
 __device__ __forceinline__ void psm_solid_terms(const LbmDev& P, const CplDev& C, int x, int y, int z, uint32_t id,
-                                                double rho, double ux, double uy, double uz, double& B,
-                                                double (&uk)[3], double (&rec)[6], int& ent)
+                                                R rho, R ux, R uy, R uz, R& B, R (&uk)[3], double (&rec)[6], int& ent)
 {
     const bool has = id != PSM_EMPTY;
     const uint32_t k = has ? id : 0u;
     const double2* sp = reinterpret_cast<const double2*>(C.sol + (size_t)k * 10);
     const double2 a0 = __ldg(sp), a1 = __ldg(sp + 1), a2 = __ldg(sp + 2), a3 = __ldg(sp + 3), a4 = __ldg(sp + 4);
     const double xk[3] = {a0.x, a0.y, a1.x}, Rk = a1.y;
-    const double vk[3] = {a2.x, a2.y, a3.x}, wk[3] = {a3.y, a4.x, a4.y};
+    const R vk[3] = {(R)a2.x, (R)a2.y, (R)a3.x}, wk[3] = {(R)a3.y, (R)a4.x, (R)a4.y};
     const int fk[3] = {(int)floor(xk[0]), (int)floor(xk[1]), (int)floor(xk[2])};
     const int di[3] = {cpl_offset(x, fk[0], P.nx, !P.bc[0]), cpl_offset(y, fk[1], P.ny, !P.bc[1]),
                        cpl_offset(z, fk[2], P.nz, !P.bc[2])};
-    double d[3];
+    double dd[3];
 #pragma unroll
-    for (int a = 0; a < 3; ++a) d[a] = (double)(fk[a] + di[a]) - xk[a];              // r_j - r_k, nearest image
+    for (int a = 0; a < 3; ++a) dd[a] = (double)(fk[a] + di[a]) - xk[a];             // r_j - r_k, nearest image
+    const R d[3] = {(R)dd[0], (R)dd[1], (R)dd[2]};
     ent = has ? ((di[2] + C.H) * C.S + (di[1] + C.H)) * C.S + (di[0] + C.H) : -1;
-    double beta;
+    R beta;
     if (SUBDIV) {
-        beta = has ? C.betabox[(size_t)k * (size_t)(C.S * C.S * C.S) + (size_t)ent] : 0.0;   // Eq. (38), from the raster
+        beta = has ? (R)C.betabox[(size_t)k * (size_t)(C.S * C.S * C.S) + (size_t)ent] : R(0);   // Eq. (38), from the raster
     } else {
-        const double dsc = cpl_dsc(Rk, C.rc, cpl_dist(d));
-        beta = dsc * C.inv_2rc;                                                      // Eq. (39)-(40)
-        beta = beta > 1.0 ? 1.0 : beta;
-        beta = (has && beta > 0.0) ? beta : 0.0;
+        if constexpr (sizeof(R) == 8) {
+            const double dsc = cpl_dsc(Rk, C.rc, cpl_dist(dd));
+            beta = dsc * C.inv_2rc;                                                  // Eq. (39)-(40)
+        } else {
+            const float dist = __fsqrt_rn(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            beta = (((float)Rk + (float)C.rc) - dist) * (float)C.inv_2rc;
+        }
+        beta = beta > R(1) ? R(1) : beta;
+        beta = (has && beta > R(0)) ? beta : R(0);
     }
-    B = beta * (P.tau - 0.5) / ((1.0 - beta) + (P.tau - 0.5));                        // Eq. (36)
+    const R tm = (R)(P.tau - 0.5);
+    B = beta * tm / ((R(1) - beta) + tm);                                            // Eq. (36)
     uk[0] = vk[0] + (wk[1] * d[2] - wk[2] * d[1]);                                   // Eq. (35)
     uk[1] = vk[1] + (wk[2] * d[0] - wk[0] * d[2]);
     uk[2] = vk[2] + (wk[0] * d[1] - wk[1] * d[0]);
     // Eq. (41): -B_k sum_i Omega^s_{i,k} c_i.  The sum is rho (u_k - u) identically (sum_i c_i f_i = rho u,
     // sum_i c_i f_i^eq(rho, v) = rho v, c_opp = -c), so it is formed from the moments.
-    const double Br = B * rho;
-    const double dF[3] = {Br * (ux - uk[0]), Br * (uy - uk[1]), Br * (uz - uk[2])};  // lattice units
+    const R Br = B * rho;
+    const R dF[3] = {Br * (ux - uk[0]), Br * (uy - uk[1]), Br * (uz - uk[2])};       // lattice units
     rec[0] = dF[0]; rec[1] = dF[1]; rec[2] = dF[2];
     rec[3] = d[1] * dF[2] - d[2] * dF[1];                                            // Eq. (42)
     rec[4] = d[2] * dF[0] - d[0] * dF[2];
@@ -202,23 +213,23 @@ __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int
 // collided pair by pair and pushed right away, so that only one pair is live in registers at a time.
 
 // BGK or TRT without solids, same expressions as lb_collide_bgk / lb_collide_trt
-template <typename I, bool TRT>
-__device__ __forceinline__ void bgk_collide_stream(const double* sf, double omega, double rho, double ux, double uy, double uz,
-                                                   const LbPush<I>& push, double* __restrict__ fout, const LbmDev& P, bool active)
+template <typename I, bool TRT, typename T>
+__device__ __forceinline__ void bgk_collide_stream(const T* sf, T omega, T rho, T ux, T uy, T uz,
+                                                   const LbPush<I>& push, T* __restrict__ fout, const LbmDev& P, bool active)
 {
     if (TRT) {
-        const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
+        const T k = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
         {
-            const double f0 = sf[0];
-            if (active) push.put(fout, P, 0, f0 - omega * (f0 - lb_w(0) * rho * k), rho);
+            const T f0 = sf[0];
+            if (active) push.put(fout, P, 0, f0 - omega * (f0 - T(lb_w(0)) * rho * k), rho);
         }
 #pragma unroll
         for (int q = 1; q < LEDDS_Q; q += 2) {
-            const double a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
-            const double cu = lb_cdot(q, ux, uy, uz);
-            const double wr = lb_w(q) * rho;
-            const double even = wr * (k + 4.5 * cu * cu), odd = wr * 3.0 * cu;
-            const double rp = omega * (0.5 * (a + b) - even), rm = P.omega_minus * (0.5 * (a - b) - odd);
+            const T a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
+            const T cu = lb_cdot(q, ux, uy, uz);
+            const T wr = T(lb_w(q)) * rho;
+            const T even = wr * (k + T(4.5) * cu * cu), odd = wr * T(3) * cu;
+            const T rp = omega * (T(0.5) * (a + b) - even), rm = (T)P.omega_minus * (T(0.5) * (a - b) - odd);
             if (active) {
                 push.put(fout, P, q, a - (rp + rm), rho);
                 push.put(fout, P, q + 1, b - (rp - rm), rho);
@@ -226,18 +237,18 @@ __device__ __forceinline__ void bgk_collide_stream(const double* sf, double omeg
         }
         return;
     }
-    const double k = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
+    const T k = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
     {
-        const double f0 = sf[0], fe = lb_w(0) * rho * k;
+        const T f0 = sf[0], fe = T(lb_w(0)) * rho * k;
         if (active) push.put(fout, P, 0, f0 - omega * (f0 - fe), rho);
     }
 #pragma unroll
     for (int q = 1; q < LEDDS_Q; q += 2) {
-        const double a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
-        const double cu = lb_cdot(q, ux, uy, uz);
-        const double wr = lb_w(q) * rho;
-        const double even = wr * (k + 4.5 * cu * cu), odd = wr * 3.0 * cu;
-        const double fa = even + odd, fb = even - odd;
+        const T a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
+        const T cu = lb_cdot(q, ux, uy, uz);
+        const T wr = T(lb_w(q)) * rho;
+        const T even = wr * (k + T(4.5) * cu * cu), odd = wr * T(3) * cu;
+        const T fa = even + odd, fb = even - odd;
         if (active) {
             push.put(fout, P, q, a - omega * (a - fa), rho);
             push.put(fout, P, q + 1, b - omega * (b - fb), rho);
@@ -247,43 +258,43 @@ __device__ __forceinline__ void bgk_collide_stream(const double* sf, double omeg
 
 // PSM collision, Eq. (32)-(37), of a cell cut by the solid (B0, uk0) and, when the warp-uniform flag `two` is
 // set, by the second one parked in s2 (B = 0 there for the lanes that have none)
-template <typename I, bool TRT>
-__device__ __forceinline__ void psm_collide_stream(const double* sf, double omega, double rho, double ux, double uy, double uz,
-                                                   double B0, const double (&uk0)[3], bool two, const double* s2,
-                                                   const LbPush<I>& push, double* __restrict__ fout, const LbmDev& P, bool active)
+template <typename I, bool TRT, typename T>
+__device__ __forceinline__ void psm_collide_stream(const T* sf, T omega, T rho, T ux, T uy, T uz,
+                                                   T B0, const T (&uk0)[3], bool two, const T* s2,
+                                                   const LbPush<I>& push, T* __restrict__ fout, const LbmDev& P, bool active)
 {
-    const double k0 = 1.0 - 1.5 * (ux * ux + uy * uy + uz * uz);
-    const double kk0 = 1.0 - 1.5 * (uk0[0] * uk0[0] + uk0[1] * uk0[1] + uk0[2] * uk0[2]);
-    const double Bsum = B0 + (two ? s2[0] : 0.0);
-    const double keep = 1.0 - (Bsum < 1.0 ? Bsum : 1.0);                              // 1 - B_tot, Eq. (37)
-    const double komega = keep * omega;
+    const T k0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+    const T kk0 = T(1) - T(1.5) * (uk0[0] * uk0[0] + uk0[1] * uk0[1] + uk0[2] * uk0[2]);
+    const T Bsum = B0 + (two ? s2[0] : T(0));
+    const T keep = T(1) - (Bsum < T(1) ? Bsum : T(1));                              // 1 - B_tot, Eq. (37)
+    const T komega = keep * omega;
     {   // rest population: its own opposite, Omega^s = feq(rho,u_k) - feq(rho,u)
-        const double f0 = sf[0], wr = lb_w(0) * rho, fe = wr * k0;
-        double acc = B0 * (wr * kk0 - fe);
+        const T f0 = sf[0], wr = T(lb_w(0)) * rho, fe = wr * k0;
+        T acc = B0 * (wr * kk0 - fe);
         if (two) acc += s2[0] * (wr * s2[PSM_BLOCK] - fe);
         if (active) push.put(fout, P, 0, f0 + (acc - komega * (f0 - fe)), rho);
     }
 #pragma unroll
     for (int q = 1; q < LEDDS_Q; q += 2) {
-        const double a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
-        const double wr = lb_w(q) * rho;
-        const double cu = lb_cdot(q, ux, uy, uz);
-        const double ev = wr * (k0 + 4.5 * cu * cu), od = wr * 3.0 * cu;
-        const double nq = a - (ev + od), no = b - (ev - od);                            // f - feq(rho,u), Eq. (28)
-        const double cuk = lb_cdot(q, uk0[0], uk0[1], uk0[2]);
-        const double evk = wr * (kk0 + 4.5 * cuk * cuk), odk = wr * 3.0 * cuk;
-        double acc_q = B0 * (no - (a - (evk + odk)));                                   // B Omega^s, Eq. (34), direction q
-        double acc_o = B0 * (nq - (b - (evk - odk)));                                   //                      its opposite
+        const T a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
+        const T wr = T(lb_w(q)) * rho;
+        const T cu = lb_cdot(q, ux, uy, uz);
+        const T ev = wr * (k0 + T(4.5) * cu * cu), od = wr * T(3) * cu;
+        const T nq = a - (ev + od), no = b - (ev - od);                            // f - feq(rho,u), Eq. (28)
+        const T cuk = lb_cdot(q, uk0[0], uk0[1], uk0[2]);
+        const T evk = wr * (kk0 + T(4.5) * cuk * cuk), odk = wr * T(3) * cuk;
+        T acc_q = B0 * (no - (a - (evk + odk)));                                   // B Omega^s, Eq. (34), direction q
+        T acc_o = B0 * (nq - (b - (evk - odk)));                                   //                      its opposite
         if (two) {
-            const double B1 = s2[0], kk1 = s2[PSM_BLOCK];
-            const double cu1 = lb_cdot(q, s2[2 * PSM_BLOCK], s2[3 * PSM_BLOCK], s2[4 * PSM_BLOCK]);
-            const double ev1 = wr * (kk1 + 4.5 * cu1 * cu1), od1 = wr * 3.0 * cu1;
+            const T B1 = s2[0], kk1 = s2[PSM_BLOCK];
+            const T cu1 = lb_cdot(q, s2[2 * PSM_BLOCK], s2[3 * PSM_BLOCK], s2[4 * PSM_BLOCK]);
+            const T ev1 = wr * (kk1 + T(4.5) * cu1 * cu1), od1 = wr * T(3) * cu1;
             acc_q += B1 * (no - (a - (ev1 + od1)));
             acc_o += B1 * (nq - (b - (ev1 - od1)));
         }
-        double oq = komega * nq, oo = komega * no;                                      // -(1 - B_tot) Omega_i, BGK
+        T oq = komega * nq, oo = komega * no;                                      // -(1 - B_tot) Omega_i, BGK
         if (TRT) {                                                                      //                        TRT, Eq. (30)
-            const double rp = komega * (0.5 * (a + b) - ev), rm = keep * P.omega_minus * (0.5 * (a - b) - od);
+            const T rp = komega * (T(0.5) * (a + b) - ev), rm = keep * (T)P.omega_minus * (T(0.5) * (a - b) - od);
             oq = rp + rm; oo = rp - rm;
         }
         if (active) {

@@ -109,7 +109,7 @@ class Dem:
 
 
 class Coupled:
-    """Coupled LBM-DEM step on the GPU (ledds_coupled_step)."""
+    """Coupled LBM-DEM step on the GPU (ledds_coupled_step; ledds_coupled_step_f32 when the lattice is fp32)."""
 
     def __init__(self, lbm: Lbm, dem: Dem, cpl: dict, r_max: float):
         self.lbm, self.dem = lbm, dem
@@ -123,5 +123,6 @@ class Coupled:
 
     def step(self, nsteps=1):
         d = self.dem
-        L.ledds_coupled_step(self.lbm.h, d.h, self.c, self.r_max, self.lbm.f, d.x, d.v, d.w, d.a, d.alpha, d.radius,
-                             self.f_hyd, self.m_hyd, d.history, d.scratch, self.cpl_scratch, d.status, nsteps)
+        call = L.ledds_coupled_step_f32 if self.lbm.f32 else L.ledds_coupled_step
+        call(self.lbm.h, d.h, self.c, self.r_max, self.lbm.f, d.x, d.v, d.w, d.a, d.alpha, d.radius,
+             self.f_hyd, self.m_hyd, d.history, d.scratch, self.cpl_scratch, d.status, nsteps)

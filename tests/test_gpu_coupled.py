@@ -222,3 +222,76 @@ def test_paper_bed_workload_small():
     o, g = both(lbm, cpl, pd, x, v, w, R)
     o.step(2); g.step(2)
     compare(o, g)
+
+
+# ------------------------------------------------------------------------------------ fp32 lattice
+# ledds_coupled_step_f32: populations, moments and collision in fp32; solid geometry, force sums and DEM in fp64.
+# Bounds: populations as for the plain fp32 lattice, 8 * steps * 2^-24 * max|f|.  A cell's
+# term of Eq. (41) is B rho (u - u_k) with rho u = sum_i c_i f_i, ten populations per axis, so a solid's force
+# differs from the fp64 one by at most (cells it cuts) * 10 * that bound per component, and its torque by
+# (R + r_c + 1) times as much; the observed differences are far smaller (the errors of the cells do not add up
+# coherently), and the test also asserts them against 1e-3 of the largest force.
+EPS32 = 2.0 ** -24
+
+
+def both_f32(lbm, cpl, pd, x, v, w, R, u=None):
+    import oracle
+    from paper_2512_04997_b200 import Coupled, Dem, Lbm
+    u32 = None if u is None else u.astype(np.float32)
+    f0 = oracle.lbm_equilibrium(lbm["shape"], None, None if u is None else u32.astype(np.float64))
+    o = oracle.Coupled(lbm, cpl, oracle.Dem(pd, x, v, w, R), f0)
+    g = Coupled(Lbm(lbm, None, u32, precision="f32"), Dem(pd, x, v, w, R), cpl, float(np.max(R)))
+    return o, g
+
+
+def compare_f32(o, g, steps, cpl):
+    f = g.lbm.export().astype(np.float64)
+    pop = 8 * steps * EPS32 * np.abs(o.f).max()
+    assert np.abs(f - o.f).max() <= pop
+    Rm = float(o.dem.R.max())
+    reach = Rm / cpl["dx"] + 1.0
+    cells = (2 * reach + 1) ** 3
+    F, M = g.f_hyd.cpu().numpy(), g.m_hyd.cpu().numpy()
+    # lattice units -> DEM units: force rho_f dx^4 / Dt^2, torque one more dx (set-ups here have all three = 1)
+    dF, dM = np.abs(F - o.F_sf).max(), np.abs(M - o.M_sf).max()
+    assert dF <= cells * 10 * pop and dM <= cells * 10 * pop * (reach + 1)
+    assert dF <= 1e-3 * np.abs(o.F_sf).max() + 1e-7 and dM <= 1e-3 * np.abs(o.M_sf).max() + 1e-7 * Rm
+    s = g.dem.state()
+    assert np.abs(s["x"] - o.dem.x).max() <= 1e-5 * max(o.lbm["shape"])
+    assert int(g.dem.status[0].item()) == o.status
+    return dF / (np.abs(o.F_sf).max() + 1e-300), np.abs(f - o.f).max() / np.abs(o.f).max()
+
+
+@pytest.mark.parametrize("collision", [0, 1])
+def test_f32_single_sphere_settling(collision):
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(32, 32, 64), R=5.0, z0=40.0, g=1e-3)
+    lbm = dict(lbm, collision=collision)
+    o, g = both_f32(lbm, cpl, pd, x, v, w, R)
+    o.step(10); g.step(10)
+    compare_f32(o, g, 10, cpl)
+
+
+def test_f32_shear_suspension_with_two_solid_cells_and_wrap():
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=2, n=64, n_part=60, R=4.0)
+    o, g = both_f32(lbm, cpl, pd, x, v, w, R, u)
+    o.step(5); g.step(5)
+    compare_f32(o, g, 5, cpl)
+
+
+def test_f32_ragged_64bit_and_subdivision():
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=3, n=72, n_part=40, R=4.0)
+    lbm = dict(lbm, variant=3, collision=1)
+    cpl = dict(cpl, solid_fraction=1)
+    o, g = both_f32(lbm, cpl, pd, x, v, w, R, u)
+    o.step(3); g.step(3)
+    compare_f32(o, g, 3, cpl)
+
+
+def test_f32_handle_is_rejected_by_the_fp64_call():
+    import paper_2512_04997_b200 as L
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(32, 32, 32), R=3.0, z0=16.0, g=0.0)
+    o, g = both_f32(lbm, cpl, pd, x, v, w, R)
+    d = g.dem
+    with pytest.raises(L.LeddsError):
+        L.ledds_coupled_step(g.lbm.h, d.h, g.c, g.r_max, g.lbm.f, d.x, d.v, d.w, d.a, d.alpha, d.radius, g.f_hyd, g.m_hyd,
+                             d.history, d.scratch, g.cpl_scratch, d.status, 1)
