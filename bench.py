@@ -278,6 +278,19 @@ def run_ours(args, rank, world):
                                            "note": "TRT + Eq. 38 with 1000 points per cell: the raster counts points for every boundary cell"}
             del gv, glv, gdv
             torch.cuda.empty_cache()
+            # the headline workload on an fp32 lattice (ledds_coupled_step_f32): 160 B per cell
+            glf = Lbm(lbv, None, uv.astype(np.float32), precision="f32"); gdf = Dem(pdv, xv, vv, wv, Rv)
+            gf4 = Coupled(glf, gdf, cpv, float(Rv.max()))
+            gf4.step(3); torch.cuda.synchronize()
+            L.ledds_profile(True)
+            msf4 = timed(gf4.step, 20) / 20
+            prf = {nm: round(L.ledds_profile_read(i)[0] / 20, 5) for i, nm in enumerate(L.KERNEL_GROUPS) if nm in ("lbm", "cpl_raster", "cpl_reduce")}
+            L.ledds_profile(False)
+            sub["cfg4_f32_lattice"] = {"mlups": round(ncv / msf4 / 1e3, 1), "ms_per_step": round(msf4, 5), "steps": 20, "dtype": "f32 lattice, f64 solids and DEM",
+                                       "kernel_ms_per_step": prf, "hbm_gbs": round(160.0 * ncv / prf["lbm"] / 1e6, 1),
+                                       "hbm_frac": round(160.0 * ncv / prf["lbm"] / 1e6 / peak, 4), "status_word": int(gdf.status[0].item())}
+            del gf4, glf, gdf
+            torch.cuda.empty_cache()
         # the paper's own performance workload: 500 x 200 x 800 cells, spheres of
         # 20 cells diameter at solid fraction 0 ... 0.45, 10 DEM sub-steps per LBM step, TRT, distance-based fraction
         if not args.sub_large_only and not small:

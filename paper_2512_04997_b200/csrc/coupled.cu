@@ -208,8 +208,7 @@ __global__ void __launch_bounds__(PSM_BLOCK, sizeof(T) == 4 ? PSM_MIN_BLOCKS_F32
     const bool two = __any_sync(0xffffffffu, id1 != PSM_EMPTY);
     T* s2col = &s2[0][threadIdx.x];
     if (two) {                                                                        // warp-uniform, rarer
-        T B1, uk1[3];
-        double rec[6];
+        T B1, uk1[3], rec[6];
         int ent;
         psm_solid_terms<SUBDIV>(P, C, x, y, z, id1, rho, ux, uy, uz, B1, uk1, rec, ent);
         s2col[0] = B1;
@@ -219,7 +218,7 @@ __global__ void __launch_bounds__(PSM_BLOCK, sizeof(T) == 4 ? PSM_MIN_BLOCKS_F32
     }
     T B0, uk0[3];
     {
-        double rec[6];
+        T rec[6];
         int ent;
         psm_solid_terms<SUBDIV>(P, C, x, y, z, id0, rho, ux, uy, uz, B0, uk0, rec, ent);
         psm_run_reduce(C, id0, ent, rec);

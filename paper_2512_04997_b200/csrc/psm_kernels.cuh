@@ -120,7 +120,7 @@ __device__ __forceinline__ double cpl_beta_count(const SubdivPoints& p)
 // still formed in double from the same floor(x_k) as the raster's, so `ent` addresses the same box cell).
 template <bool SUBDIV, typename R>
 __device__ __forceinline__ void psm_solid_terms(const LbmDev& P, const CplDev& C, int x, int y, int z, uint32_t id,
-                                                R rho, R ux, R uy, R uz, R& B, R (&uk)[3], double (&rec)[6], int& ent)
+                                                R rho, R ux, R uy, R uz, R& B, R (&uk)[3], R (&rec)[6], int& ent)
 {
     const bool has = id != PSM_EMPTY;
     const uint32_t k = has ? id : 0u;
@@ -175,7 +175,8 @@ __device__ __forceinline__ void psm_solid_terms(const LbmDev& P, const CplDev& C
 // marks a lane without a record.  ent is unused here (kept for the callers' bookkeeping).
 #define PSM_FIX_HI 1073741824.0                /* 2^30 */
 #define PSM_FIX_LO 9007199254740992.0          /* 2^53 */
-__device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int ent, double (&v)[6])
+template <typename R>
+__device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int ent, R (&v)[6])
 {
     (void)ent;
     const unsigned full = 0xffffffffu;
@@ -190,7 +191,7 @@ __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int
         if (o >= maxlen) break;
 #pragma unroll
         for (int c = 0; c < 6; ++c) {
-            const double t = __shfl_down_sync(full, v[c], o);
+            const R t = __shfl_down_sync(full, v[c], o);
             if (o < len) v[c] += t;
         }
     }
@@ -198,11 +199,11 @@ __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int
         unsigned long long* a = C.acc + (size_t)id * 12;
         bool finite = true;
 #pragma unroll
-        for (int c = 0; c < 6; ++c) finite = finite && fabs(v[c]) < 4.0e9;
+        for (int c = 0; c < 6; ++c) finite = finite && fabs((double)v[c]) < 4.0e9;
         if (!finite) { atomicOr(C.status, LEDDS_ST_NONFINITE); return; }
 #pragma unroll
         for (int c = 0; c < 6; ++c) {
-            const double s = v[c] * PSM_FIX_HI, h = rint(s), l = rint((s - h) * PSM_FIX_LO);   // s - h is exact
+            const double s = (double)v[c] * PSM_FIX_HI, h = rint(s), l = rint((s - h) * PSM_FIX_LO);   // s - h is exact
             atomicAdd(a + 2 * c, (unsigned long long)(long long)h);
             atomicAdd(a + 2 * c + 1, (unsigned long long)(long long)l);
         }
