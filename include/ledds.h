@@ -1,7 +1,7 @@
 /*
  * ledds.h -- C ABI of libledds.so: the data-parallel hot path of one coupled
  * Lattice-Boltzmann / Discrete-Element time step of arxiv 2512.04997 (LEDDS),
- * hand-written CUDA for sm_100a, fp64, one GPU.
+ * hand-written CUDA for sm_100a, fp64 (optionally an fp32 lattice), one GPU.
  *
  * Conventions (all entry points)
  *   - Returns int: LEDDS_OK or a negative LEDDS_E* code.  Never throws, never aborts.

@@ -370,4 +370,4 @@ extern "C" int ledds_lbm_destroy(ledds_lbm* h)
     return LEDDS_OK;
 }
 
-extern "C" const char* ledds_version(void) { return "ledds-b200 0.2 (sm_100a, fp64; plain LBM also fp32)"; }
+extern "C" const char* ledds_version(void) { return "ledds-b200 0.2 (sm_100a, fp64; fp32 lattice optional)"; }
