@@ -295,3 +295,11 @@ def test_f32_handle_is_rejected_by_the_fp64_call():
     with pytest.raises(L.LeddsError):
         L.ledds_coupled_step(g.lbm.h, d.h, g.c, g.r_max, g.lbm.f, d.x, d.v, d.w, d.a, d.alpha, d.radius, g.f_hyd, g.m_hyd,
                              d.history, d.scratch, g.cpl_scratch, d.status, 1)
+
+
+def test_f32_full_size_config3_one_step():
+    # the configuration bench.py times as sub.cfg4_f32_lattice: 256^3, 20 000 spheres, one coupled step
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear()
+    o, g = both_f32(lbm, cpl, pd, x, v, w, R, u)
+    o.step(1); g.step(1)
+    compare_f32(o, g, 1, cpl)
