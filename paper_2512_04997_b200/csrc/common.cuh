@@ -89,6 +89,7 @@ struct DemScratch {
     size_t xr, xr_s;               // (x, y, z, R) per particle, 32 B: particle order / sorted order
     size_t ncand, cand;            // contacts found per sorted position: uint32 [n], uint32 [maxc][n]
     size_t vp, wp;                 // predictor velocities in particle order: double [n][3]
+    size_t vw_s;                   // (v^p, w^p) of the particles in contact, sorted order: double [n][6]
     size_t pair_count, pair_off;   // query scratch (uint32 [n+1])
     size_t total;
 };

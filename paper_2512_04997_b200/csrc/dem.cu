@@ -358,6 +358,9 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // History slots: [particle][slot] partner id + delta_t as seen from that particle (the partner stores the
 // negated vector).  Per-particle sums stay in registers: no atomics.
 #define CONTACT_BLOCK 128
+#ifndef FORCE_MIN_BLOCKS
+#define FORCE_MIN_BLOCKS 1
+#endif
 #define DEM_IDLE 0xffffffffu   // ncand value of a particle the detect kernel has already finished
 
 // Stiffness and damping of one contact.  HERTZ = false: the linear spring-dashpot of the configs, gamma =
@@ -409,7 +412,8 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
 template <bool PERIODIC>
 __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
     const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
-    const double4* __restrict__ xr_s, const uint2* __restrict__ cell_range, uint32_t* __restrict__ ncand_g,
+    const double4* __restrict__ xr_s, const uint2* __restrict__ cell_range, const double* __restrict__ vp,
+    const double* __restrict__ wp, double2* __restrict__ vw_s, uint32_t* __restrict__ ncand_g,
     uint32_t* __restrict__ cand_g, double* __restrict__ ft_new, int32_t* __restrict__ status)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -484,6 +488,13 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
         dem_store_ft(ft_new, sidx[s], zero, zero, 0u);
         ncand_g[s] = DEM_IDLE;
     } else {
+        // predictor velocities of the particles that take part in a contact, in sorted order: the force kernel
+        // reads its own and its partners' (v^p, w^p) from neighbouring records instead of by particle id
+        const size_t p3 = 3 * (size_t)sidx[s];
+        double2* o = vw_s + 3 * (size_t)s;
+        o[0] = make_double2(vp[p3], vp[p3 + 1]);
+        o[1] = make_double2(vp[p3 + 2], wp[p3]);
+        o[2] = make_double2(wp[p3 + 1], wp[p3 + 2]);
         ncand_g[s] = (uint32_t)ncand;
     }
     if (st) atomicOr(status, st);
@@ -491,9 +502,9 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
 
 // ---- phase 2: evaluate
 template <bool HERTZ>
-__global__ void __launch_bounds__(CONTACT_BLOCK) dem_force_kernel(
-    const DemDev P, const uint32_t* __restrict__ sidx, const double4* __restrict__ xr_s, const double* __restrict__ vp,
-    const double* __restrict__ wp, const uint32_t* __restrict__ ncand_g, const uint32_t* __restrict__ cand_g,
+__global__ void __launch_bounds__(CONTACT_BLOCK, FORCE_MIN_BLOCKS) dem_force_kernel(
+    const DemDev P, const uint32_t* __restrict__ sidx, const double4* __restrict__ xr_s,
+    const double2* __restrict__ vw_s, const uint32_t* __restrict__ ncand_g, const uint32_t* __restrict__ cand_g,
     const double* __restrict__ ft_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
     double* __restrict__ ft_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
     int32_t* __restrict__ status, double dt_hist)
@@ -508,8 +519,11 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_force_kernel(
     const uint32_t p = sidx[s];
     Body me;
     me.x[0] = mine.x; me.x[1] = mine.y; me.x[2] = mine.z; me.R = mine.w;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) { me.v[a] = vp[3 * p + a]; me.w[a] = wp[3 * p + a]; }
+    {
+        const double2* r = vw_s + 3 * (size_t)s;
+        const double2 a = r[0], b = r[1], c = r[2];
+        me.v[0] = a.x; me.v[1] = a.y; me.v[2] = b.x; me.w[0] = b.y; me.w[1] = c.x; me.w[2] = c.y;
+    }
     const double m_me = dem_mass(P, me.R);
     const uint32_t nprev = (uint32_t)ft_prev[8 * (size_t)p + 6];
     const uint32_t* pid = hid_prev + (size_t)p * maxc;
@@ -525,8 +539,11 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_force_kernel(
         const uint32_t q = sidx[t];
         Body ot;
         ot.x[0] = o4.x; ot.x[1] = o4.y; ot.x[2] = o4.z; ot.R = o4.w;
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { ot.v[a] = vp[3 * q + a]; ot.w[a] = wp[3 * q + a]; }
+        {
+            const double2* r = vw_s + 3 * (size_t)t;
+            const double2 a = r[0], b = r[1], c = r[2];
+            ot.v[0] = a.x; ot.v[1] = a.y; ot.v[2] = b.x; ot.w[0] = b.y; ot.w[1] = c.x; ot.w[2] = c.y;
+        }
         const bool me_first = p < q;                                                   // canonical orientation i < j
         const Body& bi = me_first ? me : ot;
         const Body& bj = me_first ? ot : me;
@@ -762,7 +779,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
     s.xr = take(n * 32); s.xr_s = take(n * 32);
     s.ncand = take(n * 4); s.cand = take(n * d.maxc * 4);
-    s.vp = take(n * 24); s.wp = take(n * 24);
+    s.vp = take(n * 24); s.wp = take(n * 24); s.vw_s = take(n * 48);
     s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4);
     s.total = o;
 
@@ -863,15 +880,17 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, do
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
     if (d.bc[0] && d.bc[1] && d.bc[2])
         dem_detect_kernel<false><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
+                                                               at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double2>(scratch, s.vw_s),
                                                                at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
                                                                at<double>(history, hs.ft[nw]), status);
     else
         dem_detect_kernel<true><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
+                                                              at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double2>(scratch, s.vw_s),
                                                               at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
                                                               at<double>(history, hs.ft[nw]), status);
     ledds_count_launch(1);
     (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<nb, CONTACT_BLOCK, 0, st>>>(
-        d, sidx, at<double4>(scratch, s.xr_s), at<double>(scratch, s.vp), at<double>(scratch, s.wp),
+        d, sidx, at<double4>(scratch, s.xr_s), at<double2>(scratch, s.vw_s),
         at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
         at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
         at<double>(history, hs.ft[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]), status, dt_hist);
