@@ -95,9 +95,9 @@ struct DemScratch {
 };
 
 struct DemHistory {
-    size_t ft[2];                  // per particle, 64 B: contact force[3], torque[3], number of contacts, pad
-    size_t id[2];                  // uint32 [n][maxc]
-    size_t dt[2];                  // double [n][maxc][3]
+    size_t ft[2];                  // per particle, 64 B: contact force[3], torque[3], number of contacts, history row
+    size_t id[2];                  // uint32 [n][maxc], rows in the sorted order of the step that wrote them
+    size_t dt[2];                  // double [n][maxc][3], same rows
     size_t total;
 };
 

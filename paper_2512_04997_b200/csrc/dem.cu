@@ -384,14 +384,18 @@ __device__ __forceinline__ void dem_coefficients(double kn0, double kt0, double 
     }
 }
 
-// one full 64-byte record per particle: contact force, torque, number of contacts (exact in a double), pad
-__device__ __forceinline__ void dem_store_ft(double* __restrict__ ft, uint32_t p, const double* F, const double* M, uint32_t count)
+// one full 64-byte record per particle: contact force, torque, number of contacts and the row of the history
+// arrays that holds them (both exact in a double).  The history rows of a step are in that step's SORTED order
+// (row = sorted position): neighbouring threads write neighbouring rows, and because a particle's sorted
+// position changes little from one step to the next they also read nearly neighbouring rows.
+__device__ __forceinline__ void dem_store_ft(double* __restrict__ ft, uint32_t p, const double* F, const double* M, uint32_t count,
+                                             uint32_t row)
 {
     double2* o = reinterpret_cast<double2*>(ft + 8 * (size_t)p);
     o[0] = make_double2(F[0], F[1]);
     o[1] = make_double2(F[2], M[0]);
     o[2] = make_double2(M[1], M[2]);
-    o[3] = make_double2((double)count, 0.0);
+    o[3] = make_double2((double)count, (double)row);
 }
 
 // PERIODIC = false: no axis is periodic, the nearest image is the particle itself
@@ -485,7 +489,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
         if (P.bc[a] && (xm[a] - P.lo[a] < mine.w || P.hi[a] - xm[a] < mine.w)) near_wall = true;
     if (ncand == 0 && !near_wall) {
         const double zero[3] = {0.0, 0.0, 0.0};
-        dem_store_ft(ft_new, sidx[s], zero, zero, 0u);
+        dem_store_ft(ft_new, sidx[s], zero, zero, 0u, 0u);
         ncand_g[s] = DEM_IDLE;
     } else {
         // predictor velocities of the particles that take part in a contact, in sorted order: the force kernel
@@ -525,11 +529,13 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, FORCE_MIN_BLOCKS) dem_force_ker
         me.v[0] = a.x; me.v[1] = a.y; me.v[2] = b.x; me.w[0] = b.y; me.w[1] = c.x; me.w[2] = c.y;
     }
     const double m_me = dem_mass(P, me.R);
-    const uint32_t nprev = (uint32_t)ft_prev[8 * (size_t)p + 6];
-    const uint32_t* pid = hid_prev + (size_t)p * maxc;
-    const double* pdt = hdt_prev + (size_t)p * maxc * 3;
-    uint32_t* nid = hid_new + (size_t)p * maxc;
-    double* ndt = hdt_new + (size_t)p * maxc * 3;
+    const double2 cr = *reinterpret_cast<const double2*>(ft_prev + 8 * (size_t)p + 6);   // (contacts, row) of the last step
+    const uint32_t nprev = (uint32_t)cr.x;
+    const size_t prow = (size_t)cr.y;
+    const uint32_t* pid = hid_prev + prow * maxc;
+    const double* pdt = hdt_prev + prow * maxc * 3;
+    uint32_t* nid = hid_new + (size_t)s * maxc;
+    double* ndt = hdt_new + (size_t)s * maxc * 3;
     double Fs[3] = {0, 0, 0}, Ms[3] = {0, 0, 0};
     uint32_t ncont = 0;
 
@@ -601,7 +607,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, FORCE_MIN_BLOCKS) dem_force_ker
 #pragma unroll
     for (int a = 0; a < 3; ++a)
         if (!isfinite(Fs[a]) || !isfinite(Ms[a])) st |= LEDDS_ST_NONFINITE;
-    dem_store_ft(ft_new, p, Fs, Ms, ncont);
+    dem_store_ft(ft_new, p, Fs, Ms, ncont, (uint32_t)s);
     if (st) atomicOr(status, st);
 }
 
@@ -634,7 +640,8 @@ __global__ void dem_pair_count_kernel(int n, int maxc, const double* __restrict_
     if (p >= n) return;
     uint32_t c = 0;
     const uint32_t hc = (uint32_t)ft[8 * (size_t)p + 6];
-    for (uint32_t h = 0; h < hc; ++h) c += hid[(size_t)p * maxc + h] > (uint32_t)p;
+    const size_t row = (size_t)ft[8 * (size_t)p + 7];
+    for (uint32_t h = 0; h < hc; ++h) c += hid[row * maxc + h] > (uint32_t)p;
     cnt[p] = c;
 }
 
@@ -697,8 +704,9 @@ __global__ void dem_pair_write_kernel(int n, int maxc, const double* __restrict_
     uint32_t ids[32], slot[32];
     int c = 0;
     const uint32_t hc = (uint32_t)ft[8 * (size_t)p + 6];
+    const size_t row = (size_t)ft[8 * (size_t)p + 7];
     for (uint32_t h = 0; h < hc; ++h) {
-        const uint32_t q = hid[(size_t)p * maxc + h];
+        const uint32_t q = hid[row * maxc + h];
         if (q <= (uint32_t)p) continue;
         int k = c++;
         while (k > 0 && ids[k - 1] > q) { ids[k] = ids[k - 1]; slot[k] = slot[k - 1]; --k; }   // insertion sort
@@ -709,7 +717,7 @@ __global__ void dem_pair_write_kernel(int n, int maxc, const double* __restrict_
         if (o >= cap) break;
         if (pairs) { pairs[2 * o] = (uint32_t)p; pairs[2 * o + 1] = ids[k]; }
         if (pair_dt)
-            for (int a = 0; a < 3; ++a) pair_dt[3 * o + a] = hdt[((size_t)p * maxc + slot[k]) * 3 + a];
+            for (int a = 0; a < 3; ++a) pair_dt[3 * o + a] = hdt[(row * maxc + slot[k]) * 3 + a];
     }
 }
 
