@@ -95,8 +95,8 @@ def dem_bytes_per_particle(passes):
     return {"dem_keys": 192 + 208,                 # kick of the previous step + drift + keys in one pass: record, R, x v w a
                                                    # alpha read; v w a alpha x vp wp (x,R) key id written
             "dem_sort": 4 + 16 * passes,           # histogram read + (key, id) read and written per pass
-            "dem_gather": 8 + 32 + 32,             # (key, id), one packed record read, one written
-            "dem_contact": 8 + 32 + 64}            # (key, id), own record, force/torque/count record written
+            "dem_gather": 8 + 32 + 32 + 16,        # (key, id), one packed record read, one written + its fp32 copy
+            "dem_contact": 8 + 32 + 16 + 64}       # (key, id), own record (+ fp32 copy), force/torque/count record written
 
 
 def max_over_ranks(ms, world, device="cuda"):

@@ -67,6 +67,7 @@ struct ledds_lbm {
 struct DemDev {
     int n;
     double lo[3], hi[3], L[3];
+    float Lf[3], fmargin;          // single-precision first look of the detect kernel: (float)L, 2^-19 max L
     int bc[3];
     double vw[18];
     int nc[3];
@@ -87,6 +88,7 @@ struct DemScratch {
     size_t tile_counter;           // dynamic tile ticket (uint32 [4])
     size_t cell_range;             // uint2 [ncell]: [start, end) of the cell in the sorted order, 0,0 when empty
     size_t xr, xr_s;               // (x, y, z, R) per particle, 32 B: particle order / sorted order
+    size_t xf_s;                   // (x - lo, R) in single precision, sorted order, 16 B (first look only)
     size_t ncand, cand;            // contacts found per sorted position: uint32 [n], uint32 [maxc][n]
     size_t vp, wp;                 // predictor velocities in particle order: double [n][3]
     size_t vw_s;                   // (v^p, w^p) of the particles in contact, sorted order: double [n][6]

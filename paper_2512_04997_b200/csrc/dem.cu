@@ -274,7 +274,7 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS) dem_onesweep_ke
 // ------------------------------------------------------------------------------ gather + cell ranges
 __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
                                   const double4* __restrict__ xr, double4* __restrict__ xr_s,
-                                  uint2* __restrict__ cell_range)
+                                  float4* __restrict__ xf_s, uint2* __restrict__ cell_range)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -291,6 +291,12 @@ __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ s
     const double2* src = reinterpret_cast<const double2*>(xr + sidx[s]);
     const double2 a = __ldg(src), b = __ldg(src + 1);
     xr_s[s] = make_double4(a.x, a.y, b.x, b.y);
+    // single-precision copy (x - lo, R) for the detect kernel's first look at a candidate (dem_near).  A particle
+    // further than 2 L from the box corner (or not finite) gets NaN: it passes every first look.
+    const double rx = a.x - P.lo[0], ry = a.y - P.lo[1], rz = b.x - P.lo[2];
+    const bool sane = fabs(rx) <= 2.0 * P.L[0] && fabs(ry) <= 2.0 * P.L[1] && fabs(rz) <= 2.0 * P.L[2];
+    const float qnan = __int_as_float(0x7fc00000);
+    xf_s[s] = sane ? make_float4((float)rx, (float)ry, (float)rz, (float)b.y) : make_float4(qnan, qnan, qnan, qnan);
 }
 
 // ------------------------------------------------------------------------------ contact law
@@ -358,6 +364,9 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // History slots: [particle][slot] partner id + delta_t as seen from that particle (the partner stores the
 // negated vector).  Per-particle sums stay in registers: no atomics.
 #define CONTACT_BLOCK 128
+#ifndef DETECT_MIN_BLOCKS
+#define DETECT_MIN_BLOCKS 8
+#endif
 #ifndef FORCE_MIN_BLOCKS
 #define FORCE_MIN_BLOCKS 1
 #endif
@@ -398,6 +407,27 @@ __device__ __forceinline__ void dem_store_ft(double* __restrict__ ft, uint32_t p
     o[3] = make_double2((double)count, (double)row);
 }
 
+// First look at a candidate on the 16-byte single-precision records: false only when the pair is certainly apart.
+// Stored coordinates are within 2 L of the origin, so each is off by <= L 2^-23, a difference by <= L 2^-22 (+ the
+// rounding of L itself on a wrapped axis) and the distance by < 5e-7 L; fmargin = 2^-19 max L = 1.9e-6 L covers
+// that four times over and the factor 1.00001 the roundings of the squares.  NaN records compare as "maybe".
+template <bool PERIODIC>
+__device__ __forceinline__ bool dem_near(const DemDev& P, const float4& a, const float4& b)
+{
+    float d[3] = {a.x - b.x, a.y - b.y, a.z - b.z};
+    if (PERIODIC) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+            if (!P.bc[k]) {
+                if (d[k] > 0.5f * P.Lf[k]) d[k] -= P.Lf[k];
+                else if (d[k] < -0.5f * P.Lf[k]) d[k] += P.Lf[k];
+            }
+    }
+    const float d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    const float lim = (a.w + b.w) + P.fmargin;
+    return !(d2 > lim * lim * 1.00001f);
+}
+
 // PERIODIC = false: no axis is periodic, the nearest image is the particle itself
 template <bool PERIODIC>
 __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, const double4& b)
@@ -414,10 +444,10 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
 
 // cand[c][s] (c < ncand[s]) = sorted positions of the particles touching the particle at sorted position s
 template <bool PERIODIC>
-__global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
+__global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_kernel(
     const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
-    const double4* __restrict__ xr_s, const uint2* __restrict__ cell_range, const double* __restrict__ vp,
-    const double* __restrict__ wp, double2* __restrict__ vw_s, uint32_t* __restrict__ ncand_g,
+    const double4* __restrict__ xr_s, const float4* __restrict__ xf_s, const uint2* __restrict__ cell_range,
+    const double* __restrict__ vp, const double* __restrict__ wp, double2* __restrict__ vw_s, uint32_t* __restrict__ ncand_g,
     uint32_t* __restrict__ cand_g, double* __restrict__ ft_new, int32_t* __restrict__ status)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -425,6 +455,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
     const int maxc = P.maxc;
     const uint32_t key = skey[s];
     const double4 mine = xr_s[s];
+    const float4 minef = xf_s[s];
     int st = 0;
     int ncand = 0;
 
@@ -463,9 +494,9 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
     for (int j = 0; j < 9; ++j) {
         for (uint32_t t = t0[j]; t < t1[j]; t += 2) {                              // two candidates in flight
             const bool two = t + 1 < t1[j];
-            const double4 ca = xr_s[t], cb = xr_s[two ? t + 1 : t];
-            if ((int)t != s && dem_touch<PERIODIC>(P, mine, ca)) note(t);
-            if (two && (int)(t + 1) != s && dem_touch<PERIODIC>(P, mine, cb)) note(t + 1);
+            const float4 fa = xf_s[t], fb = xf_s[two ? t + 1 : t];                 // first look in single precision,
+            if ((int)t != s && dem_near<PERIODIC>(P, minef, fa) && dem_touch<PERIODIC>(P, mine, xr_s[t])) note(t);   // Eq. (2) in double
+            if (two && (int)(t + 1) != s && dem_near<PERIODIC>(P, minef, fb) && dem_touch<PERIODIC>(P, mine, xr_s[t + 1])) note(t + 1);
         }
     }
     if (PERIODIC && !P.bc[0] && (c0 == 0 || c0 == P.nc[0] - 1)) {                  // the wrapped cell of a periodic row
@@ -476,7 +507,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
             if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) continue; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
             const uint2 r = cell_range[(size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + wc];
             for (uint32_t t = r.x; t < r.y; ++t)
-                if ((int)t != s && dem_touch<PERIODIC>(P, mine, xr_s[t])) note(t);
+                if ((int)t != s && dem_near<PERIODIC>(P, minef, xf_s[t]) && dem_touch<PERIODIC>(P, mine, xr_s[t])) note(t);
         }
     }
 
@@ -742,6 +773,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     for (int a = 0; a < 3; ++a) {
         if (!(p->hi[a] > p->lo[a]) || (p->bc[a] != 0 && p->bc[a] != 1)) return LEDDS_EINVAL;
         d.lo[a] = p->lo[a]; d.hi[a] = p->hi[a]; d.L[a] = p->hi[a] - p->lo[a]; d.bc[a] = p->bc[a];
+        d.Lf[a] = (float)d.L[a];
         int nc = (int)floor(d.L[a] / p->cell);
         if (nc < 1) nc = 1;
         if (!p->bc[a] && nc < 3) return LEDDS_EINVAL;          // a periodic axis needs >= 3 cells (27-cell walk)
@@ -754,6 +786,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     }
     if (ncell > 4.0e9) return LEDDS_EINVAL;
     d.ncell = (unsigned)ncell;
+    d.fmargin = (float)(fmax(d.L[0], fmax(d.L[1], d.L[2])) / 524288.0);              // 2^-19 max L (dem_near)
     d.dt = p->dt; d.density = p->density;
     d.kn = p->kn; d.kt = p->kt; d.zeta = dem_zeta_host(p->restitution); d.mu = p->mu;
     d.kn_w = p->kn_w; d.kt_w = p->kt_w; d.zeta_w = dem_zeta_host(p->restitution_w); d.mu_w = p->mu_w;
@@ -785,7 +818,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     // zeroed before every range build
     s.cell_range = take((size_t)d.ncell * 8);
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
-    s.xr = take(n * 32); s.xr_s = take(n * 32);
+    s.xr = take(n * 32); s.xr_s = take(n * 32); s.xf_s = take(n * 16);
     s.ncand = take(n * 4); s.cand = take(n * d.maxc * 4);
     s.vp = take(n * 24); s.wp = take(n * 24); s.vw_s = take(n * 48);
     s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4);
@@ -880,19 +913,19 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, do
     const uint32_t* sidx = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
     ledds_prof_start(LEDDS_K_DEM_GATHER, st);
     dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr), at<double4>(scratch, s.xr_s),
-                                         at<uint2>(scratch, s.cell_range));
+                                         at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range));
     ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
     LEDDS_CHECK_LAUNCH();
     const DemHistory& hs = h->hs;
     const int prev = h->cur, nw = 1 - h->cur;
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
     if (d.bc[0] && d.bc[1] && d.bc[2])
-        dem_detect_kernel<false><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
+        dem_detect_kernel<false><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range),
                                                                at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double2>(scratch, s.vw_s),
                                                                at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
                                                                at<double>(history, hs.ft[nw]), status);
     else
-        dem_detect_kernel<true><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<uint2>(scratch, s.cell_range),
+        dem_detect_kernel<true><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range),
                                                               at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double2>(scratch, s.vw_s),
                                                               at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
                                                               at<double>(history, hs.ft[nw]), status);

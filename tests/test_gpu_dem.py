@@ -149,3 +149,36 @@ def test_hertz_mindlin_cloud(seed, bc, n):
     for _ in range(9):
         o.step(); g.step()
     check_state(o, g, 10, 14.0)
+
+
+@pytest.mark.parametrize("bc", [(1, 1, 1), (0, 0, 0)])
+def test_first_look_in_single_precision_never_hides_a_contact(bc):
+    # The detect kernel looks at a candidate first on single-precision records (dem_near) and only then decides
+    # Eq. (2) in double.  Here single precision cannot tell the pairs apart: a 300^3 box of unit cells with
+    # spheres of radius ~1e-3 (coordinate rounding 300 * 2^-24 = 1.8 % of a radius) whose partner sits at
+    # (R_i + R_j)(1 +- 1e-12 ... 1e-4), some of them across a periodic face; one particle far outside the box
+    # (NaN record).  The pair list must still equal the oracle's (which is pinned to the O(N^2) list).
+    g = np.random.Generator(np.random.PCG64(77))
+    npair = 1500
+    L = 300.0
+    R = g.uniform(0.8e-3, 1.2e-3, 2 * npair + 1)
+    a = g.uniform(1.0, L - 1.0, (npair, 3))
+    a[:200, 0] = g.uniform(0.0, 2.0e-4, 200)                   # next to the x = 0 face: the partner wraps or meets the wall
+    e = g.normal(size=(npair, 3)); e /= np.linalg.norm(e, axis=1)[:, None]
+    e[:200, 0] = -np.abs(e[:200, 0])
+    gap = np.where(g.random(npair) < 0.5, -1.0, 1.0) * 10.0 ** g.uniform(-12, -4, npair)
+    b = a + e * ((R[:npair] + R[npair:2 * npair]) * (1.0 + gap))[:, None]
+    x = np.concatenate([a, b, [[L + 450.0, 10.0, 10.0]]])      # the last one has left the box
+    if bc == (0, 0, 0):
+        x[:-1] = np.mod(x[:-1], L)
+    else:
+        x[:-1] = np.clip(x[:-1], 0.0, L)
+    pd = W.dem_defaults(len(R), (0, 0, 0), (L, L, L), bc, cell=1.0, dt=1e-7, g=(0, 0, 0), density=1000.0, kn=1e2,
+                        restitution=0.8, mu=0.4)
+    v = np.zeros_like(x); w = np.zeros_like(x)
+    o, gp = both(pd, x, v, w, R)
+    q = gp.query()
+    assert np.array_equal(q["idx"], o.idx)
+    assert np.array_equal(q["pairs"], o.pairs), (len(q["pairs"]), len(o.pairs))
+    touching = int((o.pairs[:, 1] < len(R)).sum())
+    assert 400 < touching < npair - 400                        # both outcomes are well represented
