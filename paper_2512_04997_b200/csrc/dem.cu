@@ -493,10 +493,14 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
 #pragma unroll
     for (int j = 0; j < 9; ++j) {
         for (uint32_t t = t0[j]; t < t1[j]; t += 2) {                              // two candidates in flight
-            const bool two = t + 1 < t1[j];
-            const float4 fa = xf_s[t], fb = xf_s[two ? t + 1 : t];                 // first look in single precision,
-            if ((int)t != s && dem_near<PERIODIC>(P, minef, fa) && dem_touch<PERIODIC>(P, mine, xr_s[t])) note(t);   // Eq. (2) in double
-            if (two && (int)(t + 1) != s && dem_near<PERIODIC>(P, minef, fb) && dem_touch<PERIODIC>(P, mine, xr_s[t + 1])) note(t + 1);
+            const uint32_t tb = min(t + 1u, t1[j] - 1u);                           // odd tail: the same candidate again
+            const float4 fa = xf_s[t], fb = xf_s[tb];                              // first look in single precision (no branch),
+            const bool na = dem_near<PERIODIC>(P, minef, fa) & ((int)t != s);
+            const bool nb = dem_near<PERIODIC>(P, minef, fb) & ((int)tb != s) & (tb != t);
+            if (na | nb) {                                                         // Eq. (2) in double for the few that pass
+                if (na && dem_touch<PERIODIC>(P, mine, xr_s[t])) note(t);
+                if (nb && dem_touch<PERIODIC>(P, mine, xr_s[tb])) note(tb);
+            }
         }
     }
     if (PERIODIC && !P.bc[0] && (c0 == 0 || c0 == P.nc[0] - 1)) {                  // the wrapped cell of a periodic row
