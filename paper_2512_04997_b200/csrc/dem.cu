@@ -364,6 +364,9 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // History slots: [particle][slot] partner id + delta_t as seen from that particle (the partner stores the
 // negated vector).  Per-particle sums stay in registers: no atomics.
 #define CONTACT_BLOCK 128
+#ifndef DETECT_NB
+#define DETECT_NB 3
+#endif
 #ifndef DETECT_MIN_BLOCKS
 #define DETECT_MIN_BLOCKS 8
 #endif
@@ -492,14 +495,24 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
     }
 #pragma unroll
     for (int j = 0; j < 9; ++j) {
-        for (uint32_t t = t0[j]; t < t1[j]; t += 2) {                              // two candidates in flight
-            const uint32_t tb = min(t + 1u, t1[j] - 1u);                           // odd tail: the same candidate again
-            const float4 fa = xf_s[t], fb = xf_s[tb];                              // first look in single precision (no branch),
-            const bool na = dem_near<PERIODIC>(P, minef, fa) & ((int)t != s);
-            const bool nb = dem_near<PERIODIC>(P, minef, fb) & ((int)tb != s) & (tb != t);
-            if (na | nb) {                                                         // Eq. (2) in double for the few that pass
-                if (na && dem_touch<PERIODIC>(P, mine, xr_s[t])) note(t);
-                if (nb && dem_touch<PERIODIC>(P, mine, xr_s[tb])) note(tb);
+        for (uint32_t t = t0[j]; t < t1[j]; t += DETECT_NB) {                      // DETECT_NB candidates in flight
+            uint32_t tt[DETECT_NB];
+            float4 fc[DETECT_NB];
+            bool nn[DETECT_NB], any = false;
+#pragma unroll
+            for (int b = 0; b < DETECT_NB; ++b) {
+                tt[b] = min(t + (uint32_t)b, t1[j] - 1u);                          // past the end: the last candidate again
+                fc[b] = xf_s[tt[b]];                                               // first look in single precision (no branch),
+            }
+#pragma unroll
+            for (int b = 0; b < DETECT_NB; ++b) {
+                nn[b] = dem_near<PERIODIC>(P, minef, fc[b]) & ((int)tt[b] != s) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
+                any |= nn[b];
+            }
+            if (any) {                                                             // Eq. (2) in double for the few that pass
+#pragma unroll
+                for (int b = 0; b < DETECT_NB; ++b)
+                    if (nn[b] && dem_touch<PERIODIC>(P, mine, xr_s[tt[b]])) note(tt[b]);
             }
         }
     }
