@@ -363,7 +363,9 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 //   2. evaluate: all lanes work through their k-th contact together: Eq. (7), (10)-(13), (5), (15), history.
 // History slots: [particle][slot] partner id + delta_t as seen from that particle (the partner stores the
 // negated vector).  Per-particle sums stay in registers: no atomics.
+#ifndef CONTACT_BLOCK
 #define CONTACT_BLOCK 128
+#endif
 #ifndef DETECT_NB
 #define DETECT_NB 3
 #endif
@@ -937,17 +939,17 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, do
     const int prev = h->cur, nw = 1 - h->cur;
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
     if (d.bc[0] && d.bc[1] && d.bc[2])
-        dem_detect_kernel<false><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range),
+        dem_detect_kernel<false><<<(n + CONTACT_BLOCK - 1) / CONTACT_BLOCK, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range),
                                                                at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double2>(scratch, s.vw_s),
                                                                at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
                                                                at<double>(history, hs.ft[nw]), status);
     else
-        dem_detect_kernel<true><<<nb, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range),
+        dem_detect_kernel<true><<<(n + CONTACT_BLOCK - 1) / CONTACT_BLOCK, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range),
                                                               at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double2>(scratch, s.vw_s),
                                                               at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
                                                               at<double>(history, hs.ft[nw]), status);
     ledds_count_launch(1);
-    (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<nb, CONTACT_BLOCK, 0, st>>>(
+    (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<(n + CONTACT_BLOCK - 1) / CONTACT_BLOCK, CONTACT_BLOCK, 0, st>>>(
         d, sidx, at<double4>(scratch, s.xr_s), at<double2>(scratch, s.vw_s),
         at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
         at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
