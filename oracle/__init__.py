@@ -262,6 +262,9 @@ class Coupled:
     Lattice node i sits at origin + i*dx in DEM length units; the LBM time step
     is n_sub * dt.  F_sf, M_sf of the previous LBM step are held during the
     sub-steps; the last sub-step's corrector uses the new ones.
+    Pins (tests/test_oracle_coupled.py): the step does not depend on the units it is
+    posed in (dx, Dt, rho_f, origin: every conversion exponent), and the velocity after
+    two steps with n_sub = 4 is the closed form of "F_sf held, refreshed in the last kick".
     """
 
     def __init__(self, lbm, cpl, dem: Dem, f):

@@ -31,8 +31,11 @@
  * Pins (tests/test_oracle_dem.py): restitution closed form, elastic energy
  * and momentum conservation, Psi_out = Psi_in - 7 mu (Eq. 51), free fall,
  * static rest on the floor, Newton's third law, cell-walk pair list ==
- * O(N^2) pair list.  "parity unpinned": gamma_t (G5), the projection of
- * delta_t (G9), the choice of predictor (G11).
+ * O(N^2) pair list; walls: restitution = eps_w (linear and Hertz, pins
+ * m* = m_i and the wall's own zeta), elastic wall impact depth and duration
+ * (linear: k_n,w; Hertz: R* = R_i and Y* from the wall's material).
+ * "parity unpinned": gamma_t (G5), the projection of delta_t (G9), the
+ * choice of predictor (G11).
  */
 #include <math.h>
 #include <stdint.h>

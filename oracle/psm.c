@@ -23,7 +23,9 @@
  * Pins (tests/test_oracle_psm.py): no particle == lbm.c bit for bit; sum_i
  * Omega^s = 0 and sum_i Omega^s c_i = rho (u_k - u); B(0)=0, B(1)=1; momentum
  * budget of the fluid; co-moving sphere feels no force; torque sign on a
- * spinning sphere; sum of beta ~ sphere volume.  "parity unpinned": the
+ * spinning sphere; sum of beta ~ sphere volume; a third solid in a cell is
+ * dropped by id (the step equals the step without it, bit for bit).
+ * "parity unpinned": the
  * choice between the two readings of Eq. (34) beyond those identities (G21),
  * the truncation rule (G23).
  */

@@ -280,3 +280,75 @@ def test_hertz_normal_force_is_the_hertz_law_and_mindlin_ratio():
     kt = -Ft_y / (pd["dt"] * vt)
     Sn = 2.0 * Ystar * np.sqrt(Rstar * delta)                  # d F_n / d delta of the Hertz law
     assert abs(kt / Sn / (2 * (1 - nu) / (2 - nu)) - 1.0) < 1e-5
+
+
+# ---------------------------------------------------------------- walls (reading G13): m* = m_i, R* = R_i
+def wall_drop(eps_w, model=0, dt_frac=200.0, v0=0.1, R=0.5e-3, rho=2500.0, kn_w=2.0e4, E=1.0e7, nu=0.3, E_w=4.0e7, nu_w=0.2):
+    """One sphere hits the floor head-on, no gravity.  The particle-particle constants (k_n, restitution 1, E, nu)
+    differ from the wall's on purpose: using them for the wall contact fails the pins below."""
+    m = rho * 4.0 / 3.0 * np.pi * R ** 3
+    if model == 0:
+        tc = np.pi / np.sqrt(kn_w / m)                                   # m* = m_i: the wall has infinite mass
+        dmax = v0 * np.sqrt(m / kn_w)
+    else:
+        Ystar = 1.0 / ((1 - nu * nu) / E + (1 - nu_w * nu_w) / E_w)      # (A.6) with the wall's material
+        dmax = (15.0 * m * v0 ** 2 / (16.0 * Ystar * np.sqrt(R))) ** 0.4  # Hertz impact with m* = m_i, R* = R_i (A.8, R_j = inf)
+        tc = 2.9432 * dmax / v0
+    pd = W.dem_defaults(1, (0, 0, 0), (1, 1, 1), (1, 1, 1), cell=0.5, dt=tc / dt_frac, g=(0, 0, 0), density=rho,
+                        kn=1.0e4, restitution=1.0, mu=0.0, kn_w=kn_w, kt_w=kn_w * 2 / 7, restitution_w=eps_w, mu_w=0.0,
+                        model=model, young=E, poisson=nu, young_w=E_w, poisson_w=nu_w)
+    d = oracle.Dem(pd, [[0.5, 0.5, R * (1 + 1e-3)]], [[0, 0, -v0]], [[0, 0, 0]], [R], pairs_mode="brute")
+    return d, pd, dict(m=m, tc=tc, dmax=dmax, v0=v0, R=R)
+
+
+def bounce(d, R):
+    deepest, steps = 0.0, 0
+    for _ in range(100000):
+        d.step()
+        if len(d.pairs):
+            steps += 1
+            deepest = max(deepest, R - d.x[0, 2])
+        elif steps:
+            return deepest, steps
+    raise AssertionError("never separated")
+
+
+@pytest.mark.parametrize("eps_w", [0.5, 0.8])
+def test_wall_restitution_linear_is_epsilon_w(eps_w):
+    # G13 "wall restitution = eps": gamma_n = 2 zeta_w sqrt(k_n,w m*) with m* = m_i gives e = eps_w exactly in the
+    # limit dt -> 0 (same closed form as sphere-sphere, PAPER.md:982); m* = m_i/2 would give 0.616 for eps_w = 0.5
+    for frac in (50.0, 400.0):
+        d, pd, c = wall_drop(eps_w, dt_frac=frac)
+        bounce(d, c["R"])
+        e = d.v[0, 2] / c["v0"]
+        assert abs(e / eps_w - 1.0) < 1.0 / frac, (eps_w, frac, e)
+        assert d.pairs.shape == (0, 2) and abs(d.v[0, 0]) == 0.0
+
+
+def test_wall_elastic_linear_overlap_and_duration():
+    # elastic wall impact: half a period of the oscillator (m_i, k_n,w): delta_max = v sqrt(m/k), t_c = pi sqrt(m/k)
+    d, pd, c = wall_drop(1.0, dt_frac=400.0)
+    deepest, steps = bounce(d, c["R"])
+    assert abs(deepest / c["dmax"] - 1.0) < 2e-3
+    assert abs(steps * pd["dt"] / c["tc"] - 1.0) < 0.01
+    assert abs(d.v[0, 2] / c["v0"] - 1.0) < 1e-4
+
+
+def test_wall_hertz_impact_uses_the_sphere_radius_and_the_wall_material():
+    # Hertz impact on a plane: R* = R_i (A.8 with R_j = infinity), m* = m_i, Y* of (A.6) from both materials:
+    # delta_max = (15 m v^2 / (16 Y* sqrt(R)))^(2/5), duration 2.9432 delta_max / v.  R* = R_i/2 changes
+    # delta_max by 2^(1/5) = 15 %, the sphere's own modulus for the wall by 20 %.
+    d, pd, c = wall_drop(1.0, model=1, dt_frac=400.0)
+    deepest, steps = bounce(d, c["R"])
+    assert abs(deepest / c["dmax"] - 1.0) < 2e-3
+    assert abs(steps * pd["dt"] / c["tc"] - 1.0) < 0.01
+    assert abs(d.v[0, 2] / c["v0"] - 1.0) < 1e-3
+
+
+@pytest.mark.parametrize("eps_w", [0.5, 0.8])
+def test_wall_restitution_hertz_is_epsilon_w(eps_w):
+    # (A.2) with S_n of (A.3) and m* = m_i: restitution eps_w whatever the speed
+    for v0 in (0.05, 0.2):
+        d, pd, c = wall_drop(eps_w, model=1, dt_frac=400.0, v0=v0)
+        bounce(d, c["R"])
+        assert abs(d.v[0, 2] / v0 / eps_w - 1.0) < 0.01, (eps_w, v0)

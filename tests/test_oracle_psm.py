@@ -123,15 +123,51 @@ def test_torque_opposes_spin():
     assert ux[9, 14, 9] < -0.01 and ux[9, 5, 9] > 0.01
 
 
+def _cell_terms(shape, f, tau, xk, vk, wk, R):
+    """-B rho (u_k - u) per cell of one solid from the moments, in numpy (the identity of G21; pinned on its own by
+    test_force_identity_single_cell_sum) -> dF [3, N], beta [N]"""
+    nx, ny, nz = shape
+    rho_c, u_c = oracle.lbm_moments(shape, f)
+    z, y, x = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    d = np.stack([x.ravel() - xk[0], y.ravel() - xk[1], z.ravel() - xk[2]], 0)
+    beta = np.clip(((R + oracle.psm_rc()) - np.sqrt((d ** 2).sum(0))) / (2 * oracle.psm_rc()), 0, 1)
+    B = beta * (tau - 0.5) / ((1 - beta) + (tau - 0.5))
+    uk = np.asarray(vk)[:, None] + np.cross(wk, d.T).T
+    return -B * rho_c * (uk - u_c), beta
+
+
 def test_two_lowest_ids_kept_and_flag_raised():
-    # G24: three solids in one cell -> ids 0 and 1 are used, status bit 2 set, third feels no force from that cell
-    shape = (10, 10, 10)
-    f = oracle.lbm_equilibrium(shape)
-    xk = np.array([[4.9, 5.0, 5.0], [5.1, 5.0, 5.0], [5.0, 5.1, 5.0]])
-    f1, F, M, st = oracle.psm_step(shape, f, 0.6, (1, 1, 1), None, xk, [[0.01, 0, 0]] * 3, np.zeros((3, 3)), [1.0, 1.0, 1.0])
-    assert st & 2
-    f2, F2, M2, st2 = oracle.psm_step(shape, f, 0.6, (1, 1, 1), None, xk[:2], [[0.01, 0, 0]] * 2, np.zeros((2, 3)), [1.0, 1.0])
-    assert st2 == 0
+    # G24 (PAPER.md:515, n_s = 2): a cell cut by three solids keeps the two LOWEST ids and raises status bit 2.
+    # Solids 0 and 1 (R = 3) overlap around (8, 8, 8); solid 2 (R = 1.2) sits inside their intersection, so every
+    # cell it cuts is already taken by 0 and 1: it is dropped everywhere.  The step must then equal, bit for bit,
+    # the step without solid 2, and solid 2 feels nothing.  (Keeping the two highest ids instead gives F_2 != 0.)
+    shape = (16, 16, 16)
+    rho, u = W.random_flow(shape, 12, amp=0.01)
+    f = oracle.lbm_equilibrium(shape, rho, u)
+    xk = np.array([[7.0, 8.0, 8.0], [9.0, 8.0, 8.0], [8.0, 8.0, 8.0]])
+    vk = np.array([[0.01, 0.0, 0.0], [-0.01, 0.005, 0.0], [0.0, 0.02, -0.01]])
+    wk = np.array([[0.0, 0.0, 0.001], [0.002, 0.0, 0.0], [0.0, 0.003, 0.0]])
+    Rk = np.array([3.0, 3.0, 1.2])
+    f3, F3, M3, st3 = oracle.psm_step(shape, f, 0.6, (1, 1, 1), None, xk, vk, wk, Rk)
+    f2, F2, M2, st2 = oracle.psm_step(shape, f, 0.6, (1, 1, 1), None, xk[:2], vk[:2], wk[:2], Rk[:2])
+    assert st3 & 2 and st2 == 0
+    assert np.array_equal(f3, f2)
+    assert np.array_equal(F3[:2], F2) and np.array_equal(M3[:2], M2)
+    assert np.all(F3[2] == 0.0) and np.all(M3[2] == 0.0)
+    assert np.abs(F2).min() > 1e-6                              # the kept solids do exchange momentum
+    # the same three solids renumbered so that the small one has the lowest id: now it is kept (with the lower of
+    # the two large ones) and the highest id loses exactly the cells the small one cuts
+    perm = [2, 0, 1]
+    fp, Fp, Mp, stp = oracle.psm_step(shape, f, 0.6, (1, 1, 1), None, xk[perm], vk[perm], wk[perm], Rk[perm])
+    assert stp & 2
+    dF_small, beta_small = _cell_terms(shape, f, 0.6, xk[2], vk[2], wk[2], Rk[2])
+    dF_big, beta_big = _cell_terms(shape, f, 0.6, xk[1], vk[1], wk[1], Rk[1])
+    assert np.abs(Fp[0] - dF_small.sum(1)).max() < 1e-14                              # small one: all of its cells
+    assert np.abs(Fp[1] - F2[0]).max() == 0.0                                         # the lower large one: untouched
+    lost = beta_small > 0
+    assert lost.sum() >= 7
+    assert np.abs(Fp[2] - dF_big[:, ~lost].sum(1)).max() < 1e-14                      # the higher large one: minus those cells
+    assert np.abs(dF_big[:, lost].sum(1)).max() > 1e-5                                # (and they matter)
 
 
 def test_coupled_driver_buoyant_sphere_sinks_and_neutral_floats():
