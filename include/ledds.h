@@ -49,6 +49,10 @@ extern "C" {
 #define LEDDS_ST_SOLID_OVERFLOW 2   /* a fluid cell was cut by more than 2 solids        */
 #define LEDDS_ST_COINCIDENT 4       /* two sphere centres coincide (pair skipped)        */
 #define LEDDS_ST_NONFINITE 8        /* a non-finite force was produced                   */
+#define LEDDS_ST_RADIUS_RANGE 16    /* a radius is larger than the grids were sized for: 2 R > DEM cell width
+                                       (contacts beyond the 27-cell walk are missed) or R > r_max of the
+                                       coupling (the solid's cut cells are truncated)     */
+#define LEDDS_ST_OUT_OF_BOX 32      /* a sphere centre lies outside a walled box (its cell index was clamped) */
 
 typedef struct ledds_lbm ledds_lbm;
 typedef struct ledds_dem ledds_dem;
@@ -61,10 +65,10 @@ typedef struct {
     int bc[3];               /* per axis: 0 periodic, 1 walls (halfway bounce-back) on both sides */
     double u_wall[3][2][3];  /* wall velocity [axis][side: 0 low, 1 high][component], lattice units;
                                 velocity-modified bounce-back: f -= 6 t_i rho (c_i . u_wall)      */
-    int layout;              /* 0 = two-lattice (f holds 2 x 19 x N doubles).  1 (AA single array)
-                                is reserved: LEDDS_EINVAL in this version                         */
-    int variant;             /* kernel variant: 0 auto, 1 plain push, 2 row-rotate (aligned stores),
-                                3 plain push with 64-bit indices (the path lattices with 19 N >= 2^32 take) */
+    int layout;              /* must be 0: two-lattice streaming, f holds 2 x 19 x N doubles (PAPER.md:404:
+                                "two populations").  No other layout exists; anything else: LEDDS_EINVAL */
+    int variant;             /* index width of the kernel: 0 auto (32-bit when 19 N < 2^32, else 64-bit),
+                                1 = 0, 3 forces the 64-bit path (tests).  Anything else: LEDDS_EINVAL     */
     int collision;           /* 0 = BGK, Eq. (26).  1 = TRT, Eq. (29)-(30) with tau^+ = tau and tau^- of
                                 Eq. (31); also the Omega_i of the PSM collision Eq. (33)  */
 } ledds_lbm_params;
@@ -95,7 +99,7 @@ int ledds_lbm_destroy(ledds_lbm* h);
 /* Single-precision variant of the plain LBM calls above (the paper runs most of its validations and one
  * of its two performance curves in fp32).  Same operation, layout (two lattices of
  * 19 x N floats), boundaries and collision models; all arithmetic in fp32; rho, u and f_canonical are float
- * arrays.  variant 2 (row-rotate) does not exist in fp32: LEDDS_EINVAL.  A handle made by
+ * arrays.  A handle made by
  * ledds_lbm_init_f32 is accepted by the _f32 calls and ledds_lbm_destroy only, a handle made by
  * ledds_lbm_init by the fp64 calls only (LEDDS_EINVAL otherwise).  ledds_coupled_step_f32 below takes the
  * fp32 handle. */

@@ -18,7 +18,7 @@ if not os.path.exists(_LIB_PATH):
 _lib = C.CDLL(_LIB_PATH)
 
 LEDDS_OK, LEDDS_EINVAL, LEDDS_EALIGN, LEDDS_ECAPACITY, LEDDS_ECUDA = 0, -1, -2, -3, -4
-ST_CONTACT_OVERFLOW, ST_SOLID_OVERFLOW, ST_COINCIDENT, ST_NONFINITE = 1, 2, 4, 8
+ST_CONTACT_OVERFLOW, ST_SOLID_OVERFLOW, ST_COINCIDENT, ST_NONFINITE, ST_RADIUS_RANGE, ST_OUT_OF_BOX = 1, 2, 4, 8, 16, 32
 EXPORTS = ["ledds_lbm_workspace_bytes", "ledds_lbm_init", "ledds_lbm_import", "ledds_lbm_step", "ledds_lbm_export",
            "ledds_lbm_current", "ledds_lbm_destroy", "ledds_lbm_workspace_bytes_f32", "ledds_lbm_init_f32",
            "ledds_lbm_import_f32", "ledds_lbm_step_f32", "ledds_lbm_export_f32", "ledds_dem_workspace_bytes", "ledds_dem_init", "ledds_dem_step",

@@ -21,6 +21,8 @@ void ledds_prof_stop(int kernel_id, cudaStream_t st);
         if (cudaPeekAtLastError() != cudaSuccess) return LEDDS_ECUDA; \
     } while (0)
 
+int ledds_sm_count();   // multiprocessors of the current device (cached; prof.cu)
+
 static inline bool ledds_aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 // ---- D3Q19 tables (numbering of include/ledds.h); constexpr so unrolled loops fold them ----
@@ -73,6 +75,7 @@ struct DemDev {
     int nc[3];
     double inv_h[3];
     unsigned ncell;
+    double hmin;                   // smallest cell width of the grid: 2 R must not exceed it (LEDDS_ST_RADIUS_RANGE)
     double dt, g[3], density;
     double kn, kt, zeta, mu;
     double kn_w, kt_w, zeta_w, mu_w;

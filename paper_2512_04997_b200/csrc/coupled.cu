@@ -29,11 +29,12 @@ __global__ void cpl_solid_kernel(const CplDev C)
     double* o = C.sol + (size_t)k * 10;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        o[a] = (C.x[3 * k + a] - C.origin[a]) * C.inv_dx;
+        o[a] = (C.x[3 * k + a] - C.origin[a]) / C.dx;            // divisions, as PAPER.md:256 states the conversion
         o[4 + a] = C.vp[3 * k + a] * C.vscale;
         o[7 + a] = C.wp[3 * k + a] * C.wscale;
     }
-    o[3] = C.radius[k] * C.inv_dx;
+    o[3] = C.radius[k] / C.dx;
+    if (C.radius[k] > C.r_max) atomicOr(C.status, LEDDS_ST_RADIUS_RANGE);   // its box (H from r_max) would truncate it
 }
 
 // Eq. (38) in two kernels: every (solid, cell of its bounding box) is classified from its nearest and farthest
@@ -273,7 +274,8 @@ static int cpl_setup(const ledds_lbm* lbm, const ledds_dem* dem, const ledds_cpl
     C->n = dem->d.n;
     C->rc = rc;
     C->inv_2rc = 1.0 / (2.0 * rc);
-    C->inv_dx = 1.0 / c->dx;
+    C->dx = c->dx;
+    C->r_max = r_max;
     C->vscale = Dt / c->dx;
     C->wscale = Dt;
     C->fscale = c->rho_f * pow(c->dx, 4) / (Dt * Dt);
@@ -385,7 +387,7 @@ static int coupled_step_t(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params
             const unsigned rb = (unsigned)(((long long)C.n * C.S * C.S + 255) / 256);
             if (C.subdiv) {
                 cpl_beta_classify_kernel<<<(unsigned)(((long long)C.n * C.S * C.S * C.S + 255) / 256), 256, 0, st>>>(C);
-                cpl_beta_count_kernel<<<148 * 6, 256, 0, st>>>(C);
+                cpl_beta_count_kernel<<<ledds_sm_count() * 6, 256, 0, st>>>(C);
                 ledds_count_launch(2);
                 cpl_raster_kernel<true><<<rb, 256, 0, st>>>(d, C);
             }

@@ -58,7 +58,8 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
     const DemDev P, double* __restrict__ x, double* __restrict__ v, double* __restrict__ w, double* __restrict__ a,
     double* __restrict__ alpha, const double* __restrict__ radius, const double* __restrict__ ft,
     const double* __restrict__ f_ext, const double* __restrict__ m_ext, double* __restrict__ vp,
-    double* __restrict__ wp, double4* __restrict__ xr, uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift)
+    double* __restrict__ wp, double4* __restrict__ xr, uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift,
+    int32_t* __restrict__ status)
 {
     __shared__ double sx[3 * DRIFT_BLOCK];
     const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * P.n;
@@ -103,7 +104,14 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
     const int cx = dem_cell_coord(P, xn[0], 0), cy = dem_cell_coord(P, xn[1], 1), cz = dem_cell_coord(P, xn[2], 2);
     key[i] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
     idx[i] = (uint32_t)i;
-    xr[i] = make_double4(xn[0], xn[1], xn[2], radius[i]);          // one 32-byte sector per particle for the gather
+    const double R = radius[i];
+    xr[i] = make_double4(xn[0], xn[1], xn[2], R);                  // one 32-byte sector per particle for the gather
+    // input contract (include/ledds.h): 2 R <= cell width, centres inside a walled box
+    int st = 2.0 * R > P.hmin ? LEDDS_ST_RADIUS_RANGE : 0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+        if (P.bc[a] && !(xn[a] >= P.lo[a] && xn[a] <= P.hi[a])) st |= LEDDS_ST_OUT_OF_BOX;
+    if (st) atomicOr(status, st);
 }
 
 // ------------------------------------------------------------------------------ radix sort
@@ -791,6 +799,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     DemDev& d = h->d;
     d.n = p->n;
     double ncell = 1.0;
+    d.hmin = 1.0e300;
     for (int a = 0; a < 3; ++a) {
         if (!(p->hi[a] > p->lo[a]) || (p->bc[a] != 0 && p->bc[a] != 1)) return LEDDS_EINVAL;
         d.lo[a] = p->lo[a]; d.hi[a] = p->hi[a]; d.L[a] = p->hi[a] - p->lo[a]; d.bc[a] = p->bc[a];
@@ -800,6 +809,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
         if (!p->bc[a] && nc < 3) return LEDDS_EINVAL;          // a periodic axis needs >= 3 cells (27-cell walk)
         d.nc[a] = nc;
         d.inv_h[a] = (double)nc / d.L[a];
+        d.hmin = fmin(d.hmin, d.L[a] / (double)nc);
         d.g[a] = p->g[a];
         ncell *= nc;
         for (int s = 0; s < 2; ++s)
@@ -896,11 +906,11 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, do
         if (kick)
             dem_drift_key_kernel<true><<<grid, DRIFT_BLOCK, 0, st>>>(d, x, v, w, a, alpha, radius, ft, kick->f_ext, kick->m_ext,
                                                                       at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
-                                                                      at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
+                                                                      at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status);
         else
             dem_drift_key_kernel<false><<<grid, DRIFT_BLOCK, 0, st>>>(d, x, v, w, a, alpha, radius, ft, nullptr, nullptr,
                                                                        at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
-                                                                       at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0);
+                                                                       at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status);
     }
     ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
     LEDDS_CHECK_LAUNCH();
@@ -915,7 +925,7 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, do
     }
     ledds_prof_start(LEDDS_K_DEM_SORT, st);
     int hb = (n + SORT_THREADS * 8 - 1) / (SORT_THREADS * 8);
-    if (hb > 148 * 8) hb = 148 * 8;
+    if (hb > ledds_sm_count() * 8) hb = ledds_sm_count() * 8;
     dem_hist_kernel<<<hb, SORT_THREADS, 0, st>>>(at<uint32_t>(scratch, s.key[0]), n, h->passes,
                                                  at<uint32_t>(scratch, s.hist_digit));
     LEDDS_CHECK_LAUNCH();

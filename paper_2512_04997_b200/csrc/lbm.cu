@@ -2,10 +2,9 @@
 //
 // State = pre-collision populations in canonical layout f[q][z][y][x] (x fastest), two lattices.
 // One pass reads 19 doubles and writes 19 doubles per cell: 304 B/cell of algorithmic traffic.
-//   variant 1 "push":       one cell per thread, aligned coalesced loads, stores shifted by c_q.
-//   variant 2 "row-rotate": two cells per thread (16-B loads and stores); the +-1 shift along x is
-//                           done inside the row with warp shuffles (+ one smem word per warp and
-//                           direction), so every global store is aligned and full-sector too.
+// One kernel: one cell per thread, aligned coalesced loads, stores shifted by c_q ("push"); measured on B200 it
+// runs at the HBM copy rate, so no second variant is kept (a row-rotating kernel with aligned stores was measured
+// in round 1 and was not faster).
 #include <new>
 
 #include "lbm_kernels.cuh"
@@ -45,7 +44,7 @@ __global__ void lbm_export_kernel(const T* __restrict__ f, T* __restrict__ fc, T
     }
 }
 
-// ------------------------------------------------------------------------------------ variant 1
+// ------------------------------------------------------------------------------------ stream-collide
 // Block = 128 threads = BX cells along x times 128 / BX rows along y (BX = 128 unless the lattice is narrower,
 // so that narrow lattices do not run half-empty blocks); a warp always lies inside one row.
 template <typename T, typename I, int BX, bool TRT>
@@ -74,107 +73,6 @@ static void lbm_push_launch(const T* src, T* dst, const LbmDev& d, cudaStream_t 
     else lbm_push_kernel<T, I, 32, TRT><<<grid, block, 0, st>>>(src, dst, d);
 }
 
-// ------------------------------------------------------------------------------------ variant 2
-// blockDim = (nx/2, RY); thread (j, r) owns cells x = 2j, 2j+1 of row y = blockIdx.x*RY + r, z = blockIdx.y.
-// nx/2 is a multiple of 32, so a warp never straddles rows.
-#define LEDDS_ROT_MAX_THREADS 256
-
-__device__ __forceinline__ void st2(double* p, double a, double b)
-{
-    *reinterpret_cast<double2*>(p) = make_double2(a, b);
-}
-
-template <bool TRT>
-__global__ void __launch_bounds__(LEDDS_ROT_MAX_THREADS) lbm_rowrot_kernel(const double* __restrict__ fin,
-                                                                         double* __restrict__ fout, const LbmDev P)
-{
-    // edge[k][warp]: value crossing a warp boundary for the k-th direction with cx != 0
-    __shared__ double edge[10][LEDDS_ROT_MAX_THREADS / 32];
-    const int j = threadIdx.x, lane = threadIdx.x & 31;
-    const int wrow = threadIdx.x >> 5;                         // warp index inside the row
-    const int wpr = blockDim.x >> 5;                           // warps per row
-    const int wblk = threadIdx.y * wpr + wrow;                 // warp index inside the block
-    const int y = blockIdx.x * blockDim.y + threadIdx.y, z = blockIdx.y;
-    const int x0 = 2 * j;
-    const long long row = ((long long)z * P.ny + y) * P.nx;
-
-    double fa[LEDDS_Q], fb[LEDDS_Q];
-#pragma unroll
-    for (int q = 0; q < LEDDS_Q; ++q) {
-        const double2 v = __ldg(reinterpret_cast<const double2*>(fin + (long long)q * P.N + row) + j);
-        fa[q] = v.x; fb[q] = v.y;
-    }
-    double rhoa, rhob, ux, uy, uz;
-    lb_moments(fa, rhoa, ux, uy, uz);
-    lb_collide<TRT>(fa, P, rhoa, ux, uy, uz);
-    lb_moments(fb, rhob, ux, uy, uz);
-    lb_collide<TRT>(fb, P, rhob, ux, uy, uz);
-
-    // publish warp-edge values of the 10 x-moving directions
-    {
-        int k = 0;
-#pragma unroll
-        for (int q = 1; q < LEDDS_Q; ++q) {
-            if (lb_cx(q) == 1) { if (lane == 31) edge[k][wblk] = fb[q]; ++k; }
-            else if (lb_cx(q) == -1) { if (lane == 0) edge[k][wblk] = fa[q]; ++k; }
-        }
-    }
-    __syncthreads();
-
-    const bool xwall = P.bc[0] != 0;
-    const bool first = (j == 0), last = (j == (int)blockDim.x - 1);
-    int k = 0;
-#pragma unroll
-    for (int q = 0; q < LEDDS_Q; ++q) {
-        const int cx = lb_cx(q), cy = lb_cy(q), cz = lb_cz(q);
-        // row-level part of the link: target row and whether the whole row bounces off a y/z wall
-        bool rowb = false;
-        double cuw_row = 0.0;
-        const int ty = lb_axis_target<1>(P, q, cy, y, P.ny, rowb, cuw_row);
-        const int tz = lb_axis_target<2>(P, q, cz, z, P.nz, rowb, cuw_row);
-        const long long trow = ((long long)tz * P.ny + ty) * P.nx;
-        double* const dst = fout + (long long)q * P.N + trow;                 // streamed target (slot q)
-        double* const own = fout + (long long)lb_opp(q) * P.N + row;          // bounce target (slot opp q)
-        const double w6 = 6.0 * lb_w(q);
-
-        if (cx == 0) {
-            if (rowb) st2(own + x0, fa[q] - w6 * rhoa * cuw_row, fb[q] - w6 * rhob * cuw_row);
-            else st2(dst + x0, fa[q], fb[q]);
-            continue;
-        }
-        // x-wall crossing of the two edge cells of the row
-        double cuw_x = 0.0;
-        if (xwall && P.any_wall_velocity) {
-            const double* uw = P.uw + (cx > 0 ? 1 : 0) * 3;                   // axis 0, side hi for cx=+1
-            cuw_x = lb_cdot(q, uw[0], uw[1], uw[2]);
-        }
-        if (cx == 1) {
-            double lo = __shfl_up_sync(0xffffffffu, fb[q], 1);
-            if (lane == 0) lo = edge[k][threadIdx.y * wpr + (wrow == 0 ? wpr - 1 : wrow - 1)];
-            if (rowb) {
-                const double cb = cuw_row + ((xwall && last) ? cuw_x : 0.0);
-                st2(own + x0, fa[q] - w6 * rhoa * cuw_row, fb[q] - w6 * rhob * cb);
-            } else {
-                if (xwall && first) dst[x0 + 1] = fa[q];                      // x = 0 has no source
-                else st2(dst + x0, lo, fa[q]);
-                if (xwall && last) own[x0 + 1] = fb[q] - w6 * rhob * cuw_x;    // link leaves through x = nx-1/2
-            }
-        } else {
-            double hi = __shfl_down_sync(0xffffffffu, fa[q], 1);
-            if (lane == 31) hi = edge[k][threadIdx.y * wpr + (wrow == wpr - 1 ? 0 : wrow + 1)];
-            if (rowb) {
-                const double ca = cuw_row + ((xwall && first) ? cuw_x : 0.0);
-                st2(own + x0, fa[q] - w6 * rhoa * ca, fb[q] - w6 * rhob * cuw_row);
-            } else {
-                if (xwall && last) dst[x0] = fb[q];                           // x = nx-1 has no source
-                else st2(dst + x0, fb[q], hi);
-                if (xwall && first) own[x0] = fa[q] - w6 * rhoa * cuw_x;       // link leaves through x = -1/2
-            }
-        }
-        ++k;
-    }
-}
-
 // ------------------------------------------------------------------------------------ host API
 static int lbm_validate(const ledds_lbm_params* p)
 {
@@ -183,15 +81,13 @@ static int lbm_validate(const ledds_lbm_params* p)
     if ((long long)p->nx * p->ny * p->nz > (1ll << 31)) return LEDDS_EINVAL;
     if (!(p->tau > 0.5)) return LEDDS_EINVAL;
     if (p->layout != 0) return LEDDS_EINVAL;
-    if (p->variant < 0 || p->variant > 3) return LEDDS_EINVAL;
+    if (p->variant != 0 && p->variant != 1 && p->variant != 3) return LEDDS_EINVAL;
     if (p->collision != 0 && p->collision != 1) return LEDDS_EINVAL;
     for (int a = 0; a < 3; ++a)
         if (p->bc[a] != 0 && p->bc[a] != 1) return LEDDS_EINVAL;
     // a periodic axis of length 1 would stream a population onto itself: allowed (it is a no-op wrap)
     return LEDDS_OK;
 }
-
-static bool lbm_rowrot_ok(const ledds_lbm_params* p) { return p->nx % 64 == 0 && p->nx / 2 <= LEDDS_ROT_MAX_THREADS; }
 
 // ---- the calls are written once for both precisions; T = float is the _f32 set of entry points
 template <typename T>
@@ -200,7 +96,6 @@ static int lbm_workspace_bytes_t(const ledds_lbm_params* p, size_t* f_bytes)
     const int rc = lbm_validate(p);
     if (rc) return rc;
     if (!f_bytes) return LEDDS_EINVAL;
-    if (sizeof(T) == 4 && p->variant == 2) return LEDDS_EINVAL;
     *f_bytes = (size_t)2 * LEDDS_Q * p->nx * p->ny * p->nz * sizeof(T);
     return LEDDS_OK;
 }
@@ -212,7 +107,6 @@ static int lbm_init_t(ledds_lbm** out, const ledds_lbm_params* p, T* f, const T*
     if (rc) return rc;
     if (!out || !f) return LEDDS_EINVAL;
     if (!ledds_aligned16(f) || !ledds_aligned16(rho) || !ledds_aligned16(u)) return LEDDS_EALIGN;
-    if (p->variant == 2 && (sizeof(T) == 4 || !lbm_rowrot_ok(p))) return LEDDS_EINVAL;
     ledds_lbm* h = new (std::nothrow) ledds_lbm();
     if (!h) return LEDDS_EINVAL;
     h->p = *p;
@@ -259,10 +153,7 @@ static int lbm_import_t(ledds_lbm* h, T* f, const T* fc, void* stream)
 
 // one stream-collide launch src -> dst (used by ledds_lbm_step; coupled.cu has its own PSM launch)
 template <typename T>
-static int lbm_launch(const ledds_lbm* h, const T* src, T* dst, cudaStream_t st);
-
-template <typename T>
-static int lbm_launch_push(const ledds_lbm* h, const T* src, T* dst, cudaStream_t st)
+static int lbm_launch(const ledds_lbm* h, const T* src, T* dst, cudaStream_t st)
 {
     const LbmDev& d = h->d;
     if (d.ny > 65535 || d.nz > 65535) return LEDDS_EINVAL;
@@ -272,32 +163,6 @@ static int lbm_launch_push(const ledds_lbm* h, const T* src, T* dst, cudaStream_
     else if (u32) lbm_push_launch<T, unsigned, true>(src, dst, d, st);
     else if (!d.trt) lbm_push_launch<T, long long, false>(src, dst, d, st);
     else lbm_push_launch<T, long long, true>(src, dst, d, st);
-    ledds_prof_stop(LEDDS_K_LBM, st);
-    LEDDS_CHECK_LAUNCH();
-    return LEDDS_OK;
-}
-
-template <>
-int lbm_launch<float>(const ledds_lbm* h, const float* src, float* dst, cudaStream_t st)
-{
-    return lbm_launch_push<float>(h, src, dst, st);
-}
-
-template <>
-int lbm_launch<double>(const ledds_lbm* h, const double* src, double* dst, cudaStream_t st)
-{
-    const LbmDev& d = h->d;
-    // variant 0 (auto) = 1: measured on B200, the plain push kernel already runs at the HBM copy rate
-    if (h->p.variant != 2) return lbm_launch_push<double>(h, src, dst, st);
-    ledds_prof_start(LEDDS_K_LBM, st);
-    {
-        const int tx = d.nx / 2;
-        int ry = 1;
-        while (ry < 8 && tx * ry * 2 <= LEDDS_ROT_MAX_THREADS && d.ny % (ry * 2) == 0) ry *= 2;
-        dim3 block(tx, ry), grid(d.ny / ry, d.nz);
-        if (d.trt) lbm_rowrot_kernel<true><<<grid, block, 0, st>>>(src, dst, d);
-        else lbm_rowrot_kernel<false><<<grid, block, 0, st>>>(src, dst, d);
-    }
     ledds_prof_stop(LEDDS_K_LBM, st);
     LEDDS_CHECK_LAUNCH();
     return LEDDS_OK;

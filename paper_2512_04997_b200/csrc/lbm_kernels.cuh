@@ -87,28 +87,6 @@ __device__ __forceinline__ void lb_collide(T (&f)[LEDDS_Q], const LbmDev& P, T r
     else lb_collide_bgk(f, (T)P.omega, rho, ux, uy, uz);
 }
 
-// Where does the link q that starts at coordinate `r` on one axis end?  Returns the target
-// coordinate (wrapped on a periodic axis); sets `bounced` and adds c_q . u_wall of the crossed
-// wall when the axis is walled (halfway bounce-back).
-template <int AXIS, typename T>
-__device__ __forceinline__ int lb_axis_target(const LbmDev& P, int q, int c, int r, int n, bool& bounced, T& cuw)
-{
-    if (c == 0) return r;
-    int t = r + c;
-    if (t < 0 || t >= n) {
-        if (P.bc[AXIS]) {
-            bounced = true;
-            if (P.any_wall_velocity) {
-                const double* uw = P.uw + (AXIS * 2 + (t < 0 ? 0 : 1)) * 3;
-                cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]);
-            }
-        } else {
-            t = t < 0 ? t + n : t - n;
-        }
-    }
-    return t;
-}
-
 // cells along x covered by one 128-thread block (the rest of the block goes along y)
 static inline int lb_block_x(int nx) { return nx > 64 ? 128 : (nx > 32 ? 64 : 32); }
 

@@ -25,7 +25,8 @@
 struct CplDev {
     int n;
     double rc, inv_2rc;        // Eq. (40) in lattice units
-    double inv_dx, vscale, wscale, origin[3];
+    double dx, vscale, wscale, origin[3];
+    double r_max;              // largest radius the scratch and the raster boxes were sized for (DEM units)
     double fscale, mscale;     // lattice -> DEM units for force / torque
     int H, S;                  // half-width and width of the solid's bounding box in cells (raster)
     int subdiv;                // 0: distance-based solid fraction Eq. (39)-(40); else points per direction of Eq. (38)

@@ -54,8 +54,14 @@ def test_parameter_validation_without_gpu():
     assert L.ledds_lbm_workspace_bytes_f32(p) == 2 * 19 * 512 * 4
     p.variant = 2
     with pytest.raises(L.LeddsError):
-        L.ledds_lbm_workspace_bytes_f32(p)                     # no fp32 row-rotate kernel
+        L.ledds_lbm_workspace_bytes_f32(p)                     # no such kernel variant
+    with pytest.raises(L.LeddsError):
+        L.ledds_lbm_workspace_bytes(p)
     p.variant = 0
+    p.layout = 1
+    with pytest.raises(L.LeddsError):
+        L.ledds_lbm_workspace_bytes(p)                         # two-lattice is the only layout
+    p.layout = 0
     p.tau = 0.5
     with pytest.raises(L.LeddsError):
         L.ledds_lbm_workspace_bytes(p)

@@ -19,24 +19,36 @@ def both(lbm, cpl, pd, x, v, w, R, u=None):
     return o, g
 
 
-def compare(o, g, tol_f=1e-12, tol_F=1e-10):
+ACHIEVED = {}          # test name -> largest errors seen (printed by pytest -s; quoted in DESIGN.md section 11)
+
+
+def compare(o, g, tol_f=1e-12, tol_F=1e-10, name=None):
     """Populations 1e-12 of max |f|.  Forces: the momentum exchange of Eq. 41 is a sum of differences
     of O(1) populations, so its rounding floor is ~1e-17 per term whatever the size of the force:
-    tolerance = tol_F * max|F| + FLOOR (lattice units, set-ups here have dx = rho_f = Dt = 1), and
-    likewise for the velocities integrated from it."""
+    tolerance = tol_F * max|F| + FLOOR, FLOOR = 1e-13 lattice units converted to the units the problem is posed
+    in (rho_f dx^4 / Dt^2 for a force, one more dx for a torque, dx / Dt for a velocity, 1 / Dt for a spin)."""
+    dx, rho_f = o.cpl["dx"], o.cpl["rho_f"]
+    Dt = o.cpl["n_sub"] * o.dem.p.dt
     FLOOR = 1e-13
+    fF, fM = FLOOR * rho_f * dx ** 4 / Dt ** 2, FLOOR * rho_f * dx ** 5 / Dt ** 2
     f = g.lbm.export()
-    assert np.abs(f - o.f).max() <= tol_f * np.abs(o.f).max()
+    ef = np.abs(f - o.f).max() / np.abs(o.f).max()
+    assert ef <= tol_f
     F, M = g.f_hyd.cpu().numpy(), g.m_hyd.cpu().numpy()
-    Rm = float(o.dem.R.max())
-    assert np.abs(F - o.F_sf).max() <= tol_F * np.abs(o.F_sf).max() + FLOOR
-    assert np.abs(M - o.M_sf).max() <= tol_F * np.abs(o.M_sf).max() + FLOOR * Rm
+    Rm = float(o.dem.R.max()) / dx
+    eF = np.abs(F - o.F_sf).max() / max(np.abs(o.F_sf).max(), 1e-300)
+    assert np.abs(F - o.F_sf).max() <= tol_F * np.abs(o.F_sf).max() + fF
+    assert np.abs(M - o.M_sf).max() <= tol_F * np.abs(o.M_sf).max() + fM * Rm
     s = g.dem.state()
-    L = max(o.lbm["shape"])
-    assert np.abs(s["x"] - o.dem.x).max() <= 1e-9 * L
-    assert np.abs(s["v"] - o.dem.v).max() <= 1e-9 * np.abs(o.dem.v).max() + FLOOR
-    assert np.abs(s["w"] - o.dem.w).max() <= 1e-9 * np.abs(o.dem.w).max() + FLOOR
+    L = max(o.lbm["shape"]) * dx
+    ex = np.abs(s["x"] - o.dem.x).max() / L
+    assert ex <= 1e-9
+    assert np.abs(s["v"] - o.dem.v).max() <= 1e-9 * np.abs(o.dem.v).max() + FLOOR * dx / Dt
+    assert np.abs(s["w"] - o.dem.w).max() <= 1e-9 * np.abs(o.dem.w).max() + FLOOR / Dt
     assert int(g.dem.status[0].item()) == o.status
+    if name:
+        ACHIEVED[name] = (ef, eF, ex)
+        print(f"{name}: |df|/|f| = {ef:.1e}  |dF|/|F| = {eF:.1e}  |dx|/L = {ex:.1e}")
 
 
 def test_single_sphere_settling_small():
@@ -222,6 +234,70 @@ def test_paper_bed_workload_small():
     o, g = both(lbm, cpl, pd, x, v, w, R)
     o.step(2); g.step(2)
     compare(o, g)
+
+
+def posed_in_units(L, T, rho_f, origin, n_sub):
+    """The two-sphere settling problem of tests/test_oracle_coupled.py, posed in units of length L, time T, mass
+    rho_f L^3 with the lattice origin at `origin` of the DEM frame (the oracle's conversions are pinned there)."""
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(40, 24, 40), R=3.6, z0=22.0, g=2e-3)
+    x = np.array([[11.0, 10.0, 22.0], [15.3, 11.0, 26.3]]); R = np.array([3.6, 2.9])
+    v = np.tile(np.array([[0.004, -0.002, 0.0]]), (2, 1)); w = np.tile(np.array([[0.001, 0.002, -0.0015]]), (2, 1))
+    Mu = rho_f * L ** 3
+    org = np.asarray(origin, float)
+    pdB = dict(pd, n=2)
+    pdB.update(lo=tuple(org + L * np.asarray(pd["lo"])), hi=tuple(org + L * np.asarray(pd["hi"])), cell=pd["cell"] * L,
+               dt=T / n_sub, g=tuple(np.asarray(pd["g"]) * L / T ** 2), density=pd["density"] * Mu / L ** 3)
+    for k in ("kn", "kt", "kn_w", "kt_w"):
+        pdB[k] = pd[k] * Mu / T ** 2
+    cplB = dict(n_sub=n_sub, dx=L, rho_f=rho_f, origin=tuple(org))
+    return lbm, cplB, pdB, org + L * x, v * L / T, w / T, R * L
+
+
+@pytest.mark.parametrize("n_sub", [1, 4])
+@pytest.mark.parametrize("units", [(0.5, 0.25, 2.0, (3.0, -1.5, 0.25)), (3.0e-4, 7.0e-4, 998.2, (0.0123, -0.4, 1.7))])
+def test_units_and_origin_of_the_coupling(units, n_sub):
+    # ledds_cpl_params.dx, rho_f, origin and n_sub * dt != 1 (reading G32): x_k = (x - origin)/dx, v_k Dt/dx, w_k Dt,
+    # force scale rho_f dx^4/Dt^2, torque scale rho_f dx^5/Dt^2 on the CUDA path against the oracle
+    Lu, T, rho_f, org = units
+    lbm, cpl, pd, x, v, w, R = posed_in_units(Lu, T, rho_f, org, n_sub)
+    o, g = both(lbm, cpl, pd, x, v, w, R)
+    o.step(1); g.step(1)
+    compare(o, g)
+    o.step(9); g.step(9)
+    compare(o, g, name=f"units dx={Lu} n_sub={n_sub}")
+    assert np.abs(o.F_sf).max() > 1e-4 * rho_f * Lu ** 4 / T ** 2
+
+
+def test_radius_above_r_max_is_flagged():
+    import paper_2512_04997_b200 as L
+    from paper_2512_04997_b200 import Coupled, Dem, Lbm
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(32, 32, 32), R=4.0, z0=16.0, g=0.0)
+    g = Coupled(Lbm(lbm), Dem(pd, x, v, w, R), cpl, 3.5)       # the caller promised r_max = 3.5
+    g.step(1)
+    assert int(g.dem.status[0].item()) & L.ST_RADIUS_RANGE
+    g = Coupled(Lbm(lbm), Dem(pd, x, v, w, R), cpl, 4.0)
+    g.step(1)
+    assert int(g.dem.status[0].item()) == 0
+
+
+def test_full_size_config2_settling_20_steps():
+    # BASELINE configs[2] at full size (64 x 64 x 256, walls on all sides, tau = 0.55, one sphere R = 6, density ratio
+    # 1.5): 20 coupled steps in the launch configuration bench.py times (the BX = 64 instantiation), all populations
+    lbm, cpl, pd, x, v, w, R = W.cfg3_settling()
+    o, g = both(lbm, cpl, pd, x, v, w, R)
+    o.step(20); g.step(20)
+    compare(o, g, name="configs[2] full size, 20 steps")
+    assert o.dem.v[0, 2] < 0 and o.F_sf[0, 2] > 0
+
+
+def test_coupled_100_steps_small():
+    # drift between the two implementations shows late: 100 coupled steps of a sheared suspension with contacts,
+    # two-solid cells and periodic wrap
+    lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=11, n=48, n_part=40, R=4.0)
+    o, g = both(lbm, cpl, pd, x, v, w, R, u)
+    for _ in range(4):
+        o.step(25); g.step(25)
+        compare(o, g, name="48^3 shear, 100 steps")
 
 
 # ------------------------------------------------------------------------------------ fp32 lattice

@@ -182,3 +182,48 @@ def test_first_look_in_single_precision_never_hides_a_contact(bc):
     assert np.array_equal(q["pairs"], o.pairs), (len(q["pairs"]), len(o.pairs))
     touching = int((o.pairs[:, 1] < len(R)).sum())
     assert 400 < touching < npair - 400                        # both outcomes are well represented
+
+
+@pytest.mark.parametrize("model,eps_w", [(0, 0.5), (0, 0.8), (1, 0.5)])
+def test_wall_bounce_with_damping(model, eps_w):
+    # reading G13: wall contact with its own stiffness, restitution and material, m* = m_i, R* = R_i
+    # (pinned for the oracle by restitution = eps_w and the Hertz impact depth, tests/test_oracle_dem.py): a sphere
+    # thrown obliquely at the floor with spin, followed through the whole contact
+    R, rho = 0.5e-3, 2500.0
+    m = rho * 4.0 / 3.0 * np.pi * R ** 3
+    kn_w = 2.0e4
+    tc = np.pi / np.sqrt(kn_w / m)
+    pd = W.dem_defaults(1, (0, 0, 0), (1, 1, 1), (1, 1, 1), cell=0.5, dt=tc / 60.0, g=(0, 0, -9.81), density=rho, kn=1.0e4,
+                        restitution=1.0, mu=0.0, kn_w=kn_w, kt_w=kn_w * 2 / 7, restitution_w=eps_w, mu_w=0.4, model=model,
+                        young=1.0e7, poisson=0.3, young_w=4.0e7, poisson_w=0.2)
+    o, g = both(pd, [[0.5, 0.5, R * (1 + 1e-3)]], [[0.03, -0.01, -0.1]], [[5.0, -3.0, 2.0]], [R])
+    seen = 0
+    for _ in range(60):
+        o.step(10); g.step(10)
+        check_state(o, g, 0, 1.0)
+        seen += len(o.pairs)
+        if seen and not len(o.pairs):
+            break
+    assert seen >= 3 and len(o.pairs) == 0 and o.v[0, 2] > 0.3 * eps_w * 0.1
+
+
+def test_input_contract_violations_are_flagged():
+    # a sphere wider than a grid cell (contacts beyond the 27-cell walk would be missed) and a centre outside
+    # a walled box (cell index clamped) raise status bits instead of passing silently
+    import paper_2512_04997_b200 as L
+    from paper_2512_04997_b200 import Dem
+    pd = W.dem_defaults(3, (0, 0, 0), (4, 4, 4), (1, 1, 0), cell=1.0, dt=1e-4, g=(0, 0, 0), density=1000.0, kn=1e5,
+                        restitution=0.5, mu=0.3)
+    x = np.array([[1.0, 1.0, 1.0], [3.0, 3.0, 3.0], [2.0, 2.0, 2.0]])
+    z = np.zeros((3, 3))
+    g = Dem(pd, x, z, z, np.array([0.3, 0.5, 0.4]))
+    assert int(g.status[0].item()) == 0                        # 2 R = cell is allowed
+    g = Dem(pd, x, z, z, np.array([0.3, 0.51, 0.4]))
+    assert int(g.status[0].item()) == L.ST_RADIUS_RANGE
+    x[0, 1] = 4.2                                              # outside the walled y range
+    g = Dem(pd, x, z, z, np.array([0.3, 0.5, 0.4]))
+    assert int(g.status[0].item()) & L.ST_OUT_OF_BOX
+    x[0, 1] = 1.0; x[0, 2] = 4.2                               # z is periodic: wrapped by the drift, never out of the box
+    g = Dem(pd, x, z, z, np.array([0.3, 0.5, 0.4]))
+    g.step(1)
+    assert int(g.status[0].item()) == 0

@@ -28,7 +28,7 @@ MOVING = np.zeros((3, 2, 3))
 MOVING[2, 0, 0] = -0.05; MOVING[2, 1, 0] = 0.05; MOVING[1, 0, 2] = 0.02; MOVING[0, 1, 1] = -0.03
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("variant", [1, 3])
 @pytest.mark.parametrize("shape,bc,uw", [
     ((64, 12, 10), (0, 0, 0), None),
     ((64, 12, 10), (1, 1, 1), MOVING),
@@ -41,28 +41,26 @@ def test_populations_after_100_steps(variant, shape, bc, uw):
     assert np.abs(f - ref).max() <= TOL * np.abs(ref).max()
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 3])
 @pytest.mark.parametrize("shape,bc,uw", [((64, 12, 10), (0, 0, 0), None), ((64, 9, 10), (1, 0, 1), MOVING), ((37, 6, 5), (0, 1, 0), MOVING)])
 def test_trt_populations_after_100_steps(variant, shape, bc, uw):
     # PAPER.md:236-246, Eq. (29)-(31): the collision model the paper's results use
-    if variant == 2 and shape[0] % 64:
-        pytest.skip("row-rotate needs nx % 64 == 0")
     f, ref = run_pair(shape, 0.56, bc, uw, 100, variant, collision=1)
     assert np.abs(f - ref).max() <= TOL * np.abs(ref).max()
 
 
 @pytest.mark.parametrize("shape", [(37, 5, 3), (1, 1, 1), (130, 3, 2), (5, 1, 7)])
-def test_ragged_sizes_fall_back_to_push(shape):
-    # nx not a multiple of 64: auto variant must pick the plain push kernel; single cells and thin boxes work
+def test_ragged_sizes(shape):
+    # nx not a multiple of the block width; single cells and thin boxes work
     f, ref = run_pair(shape, 0.8, (0, 1, 0), MOVING, 20, 0)
     assert np.abs(f - ref).max() <= TOL * np.abs(ref).max()
 
 
-def test_pure_streaming_is_bit_exact():
-    # omega -> tiny is not exact; instead: both variants agree bit for bit with each other after 10 steps
+def test_index_widths_agree_bit_for_bit():
+    # the 32-bit and the 64-bit index instantiations are the same arithmetic: equal bit for bit after 10 steps
     import paper_2512_04997_b200  # noqa
     f1, _ = run_pair((64, 8, 8), 0.7, (1, 0, 1), MOVING, 10, 1)
-    f2, _ = run_pair((64, 8, 8), 0.7, (1, 0, 1), MOVING, 10, 2)
+    f2, _ = run_pair((64, 8, 8), 0.7, (1, 0, 1), MOVING, 10, 3)
     assert np.array_equal(f1, f2)
 
 
@@ -80,15 +78,35 @@ def test_mass_conserved_and_tgv_decay_config2_small():
     assert abs(np.log((u1 ** 2).sum() / (u2 ** 2).sum()) / 400 / rate - 1.0) < 0.005
 
 
-def test_full_size_config2_sampled_against_oracle():
-    # 128^3 (BASELINE configs[1]), bench launch configuration; oracle runs 10 steps on the same field
+def test_full_size_config2_100_steps_against_oracle():
+    # north_star: "lattice populations after 100 steps within 1e-12" at BASELINE configs[1] itself: 128^3 periodic
+    # Taylor-Green field, tau = 0.6, the launch configuration bench.py times; every population of every cell
     import oracle
     from paper_2512_04997_b200 import Lbm
     lbm, rho, u = W.cfg2_tgv(128)
     g = Lbm(lbm, rho, u)
-    g.step(10)
+    g.step(100)
     f = g.export()
-    ref = oracle.lbm_run(lbm["shape"], oracle.lbm_equilibrium(lbm["shape"], rho, u), lbm["tau"], 10)
+    ref = oracle.lbm_run(lbm["shape"], oracle.lbm_equilibrium(lbm["shape"], rho, u), lbm["tau"], 100)
+    err = np.abs(f - ref).max() / np.abs(ref).max()
+    print(f"configs[1] 128^3 x 100 steps: max |df| / max |f| = {err:.2e}")
+    assert err <= TOL
+
+
+TWO_AXES = np.zeros((3, 2, 3))
+TWO_AXES[1, 0] = (0.01, 0.0, 0.03); TWO_AXES[1, 1] = (-0.02, 0.0, -0.04)     # y walls slide along x and z
+TWO_AXES[2, 0] = (0.02, -0.05, 0.0); TWO_AXES[2, 1] = (0.0, 0.035, 0.0)      # z walls slide along x and y
+
+
+@pytest.mark.parametrize("collision", [0, 1])
+@pytest.mark.parametrize("shape,bc", [((64, 6, 5), (0, 1, 1)), ((37, 7, 6), (1, 1, 1))])
+def test_corner_links_crossing_two_moving_walls(shape, bc, collision):
+    # reading G19: a link that leaves through two walls takes the sum of c_i.u_w over both (pinned for the oracle by
+    # exact mass conservation, tests/test_oracle_lbm.py); here every edge and corner of the box has moving walls
+    uw = TWO_AXES.copy()
+    if bc[0]:
+        uw[0, 0] = (0.0, 0.02, -0.01); uw[0, 1] = (0.0, -0.03, 0.015)
+    f, ref = run_pair(shape, 0.7, bc, uw, 100, 1, seed=3, collision=collision)
     assert np.abs(f - ref).max() <= TOL * np.abs(ref).max()
 
 
@@ -100,7 +118,7 @@ def test_import_roundtrip_and_errors():
     g = Lbm(dict(shape=shape, tau=0.9, bc=(0, 0, 0), u_wall=None), f_canonical=f0)
     assert np.array_equal(g.export(), f0)
     with pytest.raises(L.LeddsError):
-        Lbm(dict(shape=(37, 4, 4), tau=0.9, bc=(0, 0, 0), u_wall=None, variant=2))
+        Lbm(dict(shape=(37, 4, 4), tau=0.9, bc=(0, 0, 0), u_wall=None, variant=2))      # no such kernel
     with pytest.raises(L.LeddsError):
         L.ledds_lbm_step(g.h, g.f[1:], 1)                    # misaligned pointer -> LEDDS_EALIGN
 
@@ -181,7 +199,7 @@ def test_f32_handles_and_fp64_calls_do_not_mix():
     with pytest.raises(L.LeddsError):
         L.ledds_lbm_step_f32(g64.h, g32.f, 1)
     with pytest.raises(L.LeddsError):
-        Lbm(dict(lbm, variant=2), precision="f32")           # no row-rotate kernel in fp32
+        Lbm(dict(lbm, variant=2), precision="f32")           # no such kernel
     f0 = (np.random.default_rng(1).random((19, 64 * 16)) + 0.5).astype(np.float32)
     g = Lbm(lbm, f_canonical=f0, precision="f32")
     assert np.array_equal(g.export(), f0)
