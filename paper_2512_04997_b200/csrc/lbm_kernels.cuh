@@ -108,44 +108,47 @@ __device__ __forceinline__ void lb_load(const T* __restrict__ fin, I N, I cell, 
 template <typename I>
 struct LbPush {
     int x, tx[3];                 // tx[0] / tx[2]: target x for c_x = -1 / +1
-    bool wx[2], wy[2], wz[2];     // link crosses the low / high wall of the axis
+    unsigned wmask;               // bit 2 a + s: a link towards side s (0 low, 1 high) of axis a leaves through a wall
     I N, rb[3][3];                // row offsets [c_z + 1][c_y + 1]
 
-    __device__ __forceinline__ LbPush(const LbmDev& P, int x_, int y, int z) : x(x_), N((I)P.N)
+    __device__ __forceinline__ LbPush(const LbmDev& P, int x_, int y, int z) : x(x_), wmask(0u), N((I)P.N)
     {
         int ty[3] = {y - 1, y, y + 1}, tz[3] = {z - 1, z, z + 1};
         tx[0] = x - 1; tx[1] = x; tx[2] = x + 1;
-        wx[0] = wx[1] = wy[0] = wy[1] = wz[0] = wz[1] = false;
-        if (x == 0) { if (P.bc[0]) wx[0] = true; else tx[0] = P.nx - 1; }
-        if (x == P.nx - 1) { if (P.bc[0]) wx[1] = true; else tx[2] = 0; }
-        if (y == 0) { if (P.bc[1]) wy[0] = true; else ty[0] = P.ny - 1; }
-        if (y == P.ny - 1) { if (P.bc[1]) wy[1] = true; else ty[2] = 0; }
-        if (z == 0) { if (P.bc[2]) wz[0] = true; else tz[0] = P.nz - 1; }
-        if (z == P.nz - 1) { if (P.bc[2]) wz[1] = true; else tz[2] = 0; }
+        if (x == 0) { if (P.bc[0]) wmask |= 1u; else tx[0] = P.nx - 1; }
+        if (x == P.nx - 1) { if (P.bc[0]) wmask |= 2u; else tx[2] = 0; }
+        if (y == 0) { if (P.bc[1]) wmask |= 4u; else ty[0] = P.ny - 1; }
+        if (y == P.ny - 1) { if (P.bc[1]) wmask |= 8u; else ty[2] = 0; }
+        if (z == 0) { if (P.bc[2]) wmask |= 16u; else tz[0] = P.nz - 1; }
+        if (z == P.nz - 1) { if (P.bc[2]) wmask |= 32u; else tz[2] = 0; }
 #pragma unroll
         for (int a = 0; a < 3; ++a)
 #pragma unroll
             for (int b = 0; b < 3; ++b) rb[a][b] = ((I)tz[a] * (I)P.ny + (I)ty[b]) * (I)P.nx;
     }
 
+    // walls a link of direction q can leave through (compile-time constant after unrolling)
+    static __device__ __forceinline__ constexpr unsigned link_mask(int q)
+    {
+        return (lb_cx(q) < 0 ? 1u : (lb_cx(q) > 0 ? 2u : 0u)) | (lb_cy(q) < 0 ? 4u : (lb_cy(q) > 0 ? 8u : 0u)) |
+               (lb_cz(q) < 0 ? 16u : (lb_cz(q) > 0 ? 32u : 0u));
+    }
+
     // post-collision population v of direction q (a compile-time constant after unrolling); rho = the cell's
-    // pre-collision density (moving-wall term, G19)
+    // pre-collision density (moving-wall term, G19).  A cell away from every wall (wmask == 0: all but the outermost
+    // layer of a walled axis) takes the first branch for all 19 directions: an index and a store.
     template <typename T>
     __device__ __forceinline__ void put(T* __restrict__ fout, const LbmDev& P, int q, T v, T rho) const
     {
         const int cx = lb_cx(q), cy = lb_cy(q), cz = lb_cz(q);
-        bool bounced = false;
-        if (cx != 0) bounced = bounced || wx[cx > 0];
-        if (cy != 0) bounced = bounced || wy[cy > 0];
-        if (cz != 0) bounced = bounced || wz[cz > 0];
-        if (!bounced) {
+        if ((wmask & link_mask(q)) == 0u) {
             fout[(I)((I)q * N + rb[cz + 1][cy + 1] + (I)tx[cx + 1])] = v;
         } else {
             T cuw = T(0);                                   // c_q . u_wall summed over the crossed walls
             if (P.any_wall_velocity) {
-                if (cx != 0 && wx[cx > 0]) { const double* uw = P.uw + (0 + (cx > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
-                if (cy != 0 && wy[cy > 0]) { const double* uw = P.uw + (2 + (cy > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
-                if (cz != 0 && wz[cz > 0]) { const double* uw = P.uw + (4 + (cz > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
+                if (cx != 0 && (wmask & (cx > 0 ? 2u : 1u))) { const double* uw = P.uw + (0 + (cx > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
+                if (cy != 0 && (wmask & (cy > 0 ? 8u : 4u))) { const double* uw = P.uw + (2 + (cy > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
+                if (cz != 0 && (wmask & (cz > 0 ? 32u : 16u))) { const double* uw = P.uw + (4 + (cz > 0)) * 3; cuw += lb_cdot(q, (T)uw[0], (T)uw[1], (T)uw[2]); }
             }
             fout[(I)((I)lb_opp(q) * N + rb[1][1] + (I)x)] = v - T(6.0 * lb_w(q)) * rho * cuw;
         }

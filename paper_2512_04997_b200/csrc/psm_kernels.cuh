@@ -198,10 +198,10 @@ __device__ __forceinline__ void psm_run_reduce(const CplDev& C, uint32_t id, int
     }
     if (id != PSM_EMPTY && ((starts >> lane) & 1u)) {
         unsigned long long* a = C.acc + (size_t)id * 12;
-        bool finite = true;
+        double big = fabs((double)v[0]);                                           // NaN-propagating: fmax would drop a NaN
 #pragma unroll
-        for (int c = 0; c < 6; ++c) finite = finite && fabs((double)v[c]) < 4.0e9;
-        if (!finite) { atomicOr(C.status, LEDDS_ST_NONFINITE); return; }
+        for (int c = 1; c < 6; ++c) big += fabs((double)v[c]);
+        if (!(big < 4.0e9)) { atomicOr(C.status, LEDDS_ST_NONFINITE); return; }
 #pragma unroll
         for (int c = 0; c < 6; ++c) {
             const double s = (double)v[c] * PSM_FIX_HI, h = rint(s), l = rint((s - h) * PSM_FIX_LO);   // s - h is exact
@@ -259,7 +259,15 @@ __device__ __forceinline__ void bgk_collide_stream(const T* sf, T omega, T rho, 
 }
 
 // PSM collision, Eq. (32)-(37), of a cell cut by the solid (B0, uk0) and, when the warp-uniform flag `two` is
-// set, by the second one parked in s2 (B = 0 there for the lanes that have none)
+// set, by the second one parked in s2 (B = 0 there for the lanes that have none).
+// For a pair of opposite directions (q, qbar) with a = f_q, b = f_qbar, E / O the even / odd part of f^eq(rho, u)
+// and Ek / Ok those of f^eq(rho, u_k), Eq. (34) reads
+//     Omega^s_q    = (b - (E - O)) - (a - (Ek + Ok)) = D + X,      D = Ek - E,  X = (Ok + O) - (a - b)
+//     Omega^s_qbar = (a - (E + O)) - (b - (Ek - Ok)) = D - X
+// and the fluid collision a - f^eq_q = Pp + Mm, b - f^eq_qbar = Pp - Mm with Pp = (a + b)/2 - E, Mm = (a - b)/2 - O,
+// so both outputs come from one even part U = sum_k B_k D_k - (1 - B_tot) w+ Pp and one odd part
+// V = sum_k B_k X_k - (1 - B_tot) w- Mm (w+ = w- for BGK): f*_q = a + (U + V), f*_qbar = b + (U - V).
+// D is formed as t_q rho [(k_k - k) + 4.5 (c.u_k - c.u)(c.u_k + c.u)]: no cancellation of the two equilibria.
 template <typename I, bool TRT, typename T>
 __device__ __forceinline__ void psm_collide_stream(const T* sf, T omega, T rho, T ux, T uy, T uz,
                                                    T B0, const T (&uk0)[3], bool two, const T* s2,
@@ -270,38 +278,35 @@ __device__ __forceinline__ void psm_collide_stream(const T* sf, T omega, T rho, 
     const T Bsum = B0 + (two ? s2[0] : T(0));
     const T keep = T(1) - (Bsum < T(1) ? Bsum : T(1));                              // 1 - B_tot, Eq. (37)
     const T komega = keep * omega;
+    const T komega_m = TRT ? keep * (T)P.omega_minus : komega;
+    const T dk0 = kk0 - k0;
+    T B1 = T(0), dk1 = T(0);
+    if (two) { B1 = s2[0]; dk1 = s2[PSM_BLOCK] - k0; }
     {   // rest population: its own opposite, Omega^s = feq(rho,u_k) - feq(rho,u)
         const T f0 = sf[0], wr = T(lb_w(0)) * rho, fe = wr * k0;
-        T acc = B0 * (wr * kk0 - fe);
-        if (two) acc += s2[0] * (wr * s2[PSM_BLOCK] - fe);
+        T acc = B0 * (wr * dk0);
+        if (two) acc += B1 * (wr * dk1);
         if (active) push.put(fout, P, 0, f0 + (acc - komega * (f0 - fe)), rho);
     }
 #pragma unroll
     for (int q = 1; q < LEDDS_Q; q += 2) {
         const T a = sf[q * PSM_BLOCK], b = sf[(q + 1) * PSM_BLOCK];
-        const T wr = T(lb_w(q)) * rho;
-        const T cu = lb_cdot(q, ux, uy, uz);
-        const T ev = wr * (k0 + T(4.5) * cu * cu), od = wr * T(3) * cu;
-        const T nq = a - (ev + od), no = b - (ev - od);                            // f - feq(rho,u), Eq. (28)
-        const T cuk = lb_cdot(q, uk0[0], uk0[1], uk0[2]);
-        const T evk = wr * (kk0 + T(4.5) * cuk * cuk), odk = wr * T(3) * cuk;
-        T acc_q = B0 * (no - (a - (evk + odk)));                                   // B Omega^s, Eq. (34), direction q
-        T acc_o = B0 * (nq - (b - (evk - odk)));                                   //                      its opposite
+        const T wr = T(lb_w(q)) * rho, wr3 = T(3) * wr;
+        const T cu = lb_cdot(q, ux, uy, uz), cuk = lb_cdot(q, uk0[0], uk0[1], uk0[2]);
+        const T s = a + b, d = a - b;
+        const T E = wr * (k0 + T(4.5) * cu * cu), O = wr3 * cu;
+        T U = B0 * (wr * (dk0 + T(4.5) * (cuk - cu) * (cuk + cu)));                // B D
+        T V = B0 * (wr3 * (cuk + cu) - d);                                          // B X
         if (two) {
-            const T B1 = s2[0], kk1 = s2[PSM_BLOCK];
             const T cu1 = lb_cdot(q, s2[2 * PSM_BLOCK], s2[3 * PSM_BLOCK], s2[4 * PSM_BLOCK]);
-            const T ev1 = wr * (kk1 + T(4.5) * cu1 * cu1), od1 = wr * T(3) * cu1;
-            acc_q += B1 * (no - (a - (ev1 + od1)));
-            acc_o += B1 * (nq - (b - (ev1 - od1)));
+            U += B1 * (wr * (dk1 + T(4.5) * (cu1 - cu) * (cu1 + cu)));
+            V += B1 * (wr3 * (cu1 + cu) - d);
         }
-        T oq = komega * nq, oo = komega * no;                                      // -(1 - B_tot) Omega_i, BGK
-        if (TRT) {                                                                      //                        TRT, Eq. (30)
-            const T rp = komega * (T(0.5) * (a + b) - ev), rm = keep * (T)P.omega_minus * (T(0.5) * (a - b) - od);
-            oq = rp + rm; oo = rp - rm;
-        }
+        U -= komega * (T(0.5) * s - E);                                             // Eq. (33): (1 - B_tot) Omega, BGK / TRT even part
+        V -= komega_m * (T(0.5) * d - O);                                           //                               odd part
         if (active) {
-            push.put(fout, P, q, a + (acc_q - oq), rho);                                // Eq. (32)-(33)
-            push.put(fout, P, q + 1, b + (acc_o - oo), rho);
+            push.put(fout, P, q, a + (U + V), rho);                                 // Eq. (32)
+            push.put(fout, P, q + 1, b + (U - V), rho);
         }
     }
 }
