@@ -84,25 +84,38 @@ struct DemDev {
 };
 
 // Layout of the caller-owned DEM scratch buffer (byte offsets, all 256-B aligned).
+// "home" order: the order the library keeps the particle state in between the steps of one call.  It is the
+// sorted order (by cell key, then id) of the last sort before the call began, so a particle's home index stays
+// close to its sorted position and every access "by particle" is nearly sequential.  The caller's arrays are
+// read once when a call begins (import) and written once when it ends (export).
 struct DemScratch {
-    size_t key[2], idx[2];         // ping-pong sort buffers (uint32 [n])
-    size_t hist_digit;             // global digit histograms (uint32 [4][256])
-    size_t tile_state;             // look-back descriptors (uint32 [tiles][256])
-    size_t tile_counter;           // dynamic tile ticket (uint32 [4])
-    size_t cell_range;             // uint2 [ncell]: [start, end) of the cell in the sorted order, 0,0 when empty
-    size_t xr, xr_s;               // (x, y, z, R) per particle, 32 B: particle order / sorted order
-    size_t xf_s;                   // (x - lo, R) in single precision, sorted order, 16 B (first look only)
+    size_t hist_digit;             // global digit histograms (uint32 [4][256])           } zeroed
+    size_t tile_counter;           // dynamic tile tickets of the sort passes and the scan } before
+    size_t tile_state;             // look-back descriptors of the sort (uint32 [4][tiles][256]) } every
+    size_t scan_state;             // look-back descriptors of the scan (uint32 [scan tiles])    } step
+    size_t cell_range;             // uint2 [ncell]: [start, end) of the cell in the sorted order, 0,0 when empty (zeroed too)
+    size_t key[2], idx[2];         // ping-pong sort buffers: cell key, home index (uint32 [n])
+    size_t hid;                    // uint32 [n]: caller's particle id of home slot h
+    size_t sid;                    // uint32 [n]: caller's particle id at sorted position s (last sort)
+    size_t sid_tmp;                // uint32 [n]: the same before the particles of a cell are put into id order
+    size_t hx;                     // double4 [n]: (x, y, z, R), home order
+    size_t hv, hw, ha, hal;        // double [n][3]: v, w, a, alpha, home order
+    size_t pvw;                    // double [n][6]: predictor (v^p, w^p), home order
+    size_t xr_s;                   // double4 [n]: (x, y, z, R), sorted order
+    size_t xf_s;                   // float4 [n]: (x - lo, R) in single precision, sorted order (first look only)
     size_t ncand, cand;            // contacts found per sorted position: uint32 [n], uint32 [maxc][n]
-    size_t vp, wp;                 // predictor velocities in particle order: double [n][3]
-    size_t vw_s;                   // (v^p, w^p) of the particles in contact, sorted order: double [n][6]
-    size_t pair_count, pair_off;   // query scratch (uint32 [n+1])
+    size_t off;                    // uint32 [n + 1]: first contact end of sorted position s (CSR offsets)
+    size_t end_s, end_t;           // uint32 [n maxc]: owner (sorted position) and partner (sorted position or wall code) per end
+    size_t pair_count, pair_off, pos_of_id;   // query scratch (uint32 [n+1])
     size_t total;
 };
 
+// Caller-owned DEM history buffer: what one force evaluation leaves for the next.
 struct DemHistory {
-    size_t ft[2];                  // per particle, 64 B: contact force[3], torque[3], number of contacts, history row
-    size_t id[2];                  // uint32 [n][maxc], rows in the sorted order of the step that wrote them
-    size_t dt[2];                  // double [n][maxc][3], same rows
+    size_t fm[2];                  // double [n][6]: contact force and torque per particle, home order (two copies: re-homing permutes)
+    size_t row[2];                 // uint2 [n]: (first end, number of ends) of the particle's contacts in hq / hdt, home order
+    size_t hq[2];                  // uint32 [n maxc]: partner id per contact end, two generations
+    size_t hdt[2];                 // double [n maxc][3]: delta_t per contact end as seen from its owner, two generations
     size_t total;
 };
 
@@ -111,9 +124,12 @@ struct ledds_dem {
     DemDev d;
     DemScratch s;
     DemHistory hs;
-    int cur;                       // which history buffer holds the latest contacts
-    int sorted_buf;                // which key/idx ping-pong buffer holds the sorted result
-    int key_bits, passes, tiles;
+    int cur;                       // which generation of hq / hdt holds the latest contacts
+    int rec;                       // which copy of fm / row is current
+    int sorted_buf;                // which key ping-pong buffer holds the sorted keys
+    int sh_buf;                    // which idx ping-pong buffer holds the home index of every sorted position
+    bool have_sort;                // sid / idx[sorted_buf] describe a sort of the current particle set
+    int key_bits, passes, tiles, scan_tiles;
     long long steps;
     // fork/join of the contact pipeline beside the lattice kernels of a coupled step (host resources, lazily made)
     cudaStream_t side = nullptr;
@@ -121,9 +137,13 @@ struct ledds_dem {
 };
 
 // entry points implemented in dem.cu and used by coupled.cu
-struct DemKick { const double* f_ext; const double* m_ext; };   // external force / torque of a kick, [n][3] or NULL
-int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha,
-                               const double* radius, void* history, void* scratch, int32_t* status, double dt_hist,
+struct DemKick { const double* f_ext; const double* m_ext; };   // external force / torque of a kick, [n][3] by caller id, or NULL
+// caller's arrays -> home order (begins a call); a / alpha may be NULL (zeros)
+int ledds_dem_import(ledds_dem* h, const double* x, const double* v, const double* w, const double* a, const double* alpha,
+                     const double* radius, void* history, void* scratch, cudaStream_t st);
+// home order -> caller's arrays (ends a call); any pointer may be NULL (not written)
+int ledds_dem_export(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha, const void* scratch, cudaStream_t st);
+// one force evaluation on the home state: [kick of the previous step] -> drift (optional) -> keys -> sort -> contacts
+int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32_t* status, double dt_hist,
                                bool drift, cudaStream_t st, bool fork = false, const DemKick* kick = nullptr);
-int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha, const double* radius,
-                   const double* f_ext, const double* m_ext, const void* history, int32_t* status, cudaStream_t st);
+int ledds_dem_kick(ledds_dem* h, const double* f_ext, const double* m_ext, const void* history, void* scratch, cudaStream_t st);

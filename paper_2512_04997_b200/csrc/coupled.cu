@@ -21,20 +21,23 @@
 
 #define RASTER_BATCH 6
 
-// sol[k] = the solid in lattice units (one thread per solid)
+// sol[k] = the solid in lattice units (one thread per home slot of the DEM state; k = the particle's id)
 __global__ void cpl_solid_kernel(const CplDev C)
 {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= C.n) return;
-    double* o = C.sol + (size_t)k * 10;
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= C.n) return;
+    const double4 r = C.hx[h];
+    const double xr[3] = {r.x, r.y, r.z};
+    const double* pv = C.pvw + 6 * (size_t)h;
+    double* o = C.sol + (size_t)C.hid[h] * 10;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        o[a] = (C.x[3 * k + a] - C.origin[a]) / C.dx;            // divisions, as PAPER.md:256 states the conversion
-        o[4 + a] = C.vp[3 * k + a] * C.vscale;
-        o[7 + a] = C.wp[3 * k + a] * C.wscale;
+        o[a] = (xr[a] - C.origin[a]) / C.dx;                     // divisions, as PAPER.md:256 states the conversion
+        o[4 + a] = pv[a] * C.vscale;
+        o[7 + a] = pv[3 + a] * C.wscale;
     }
-    o[3] = C.radius[k] / C.dx;
-    if (C.radius[k] > C.r_max) atomicOr(C.status, LEDDS_ST_RADIUS_RANGE);   // its box (H from r_max) would truncate it
+    o[3] = r.w / C.dx;
+    if (r.w > C.r_max) atomicOr(C.status, LEDDS_ST_RADIUS_RANGE);   // its box (H from r_max) would truncate it
 }
 
 // Eq. (38) in two kernels: every (solid, cell of its bounding box) is classified from its nearest and farthest
@@ -352,10 +355,9 @@ static int coupled_step_t(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params
     const DemScratch& s = dem->s;
     char* sc = static_cast<char*>(scratch);
     char* cs = static_cast<char*>(cpl_scratch);
-    C.x = x;
-    C.vp = reinterpret_cast<const double*>(sc + s.vp);
-    C.wp = reinterpret_cast<const double*>(sc + s.wp);
-    C.radius = radius;
+    C.hx = reinterpret_cast<const double4*>(sc + s.hx);
+    C.pvw = reinterpret_cast<const double*>(sc + s.pvw);
+    C.hid = reinterpret_cast<const uint32_t*>(sc + s.hid);
     C.slots = reinterpret_cast<uint2*>(cs + L.slots);
     C.sol = reinterpret_cast<double*>(cs + L.sol);
     C.acc = reinterpret_cast<unsigned long long*>(cs + L.acc);
@@ -370,12 +372,15 @@ static int coupled_step_t(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params
     // rides on the first drift of the next one; only the last step of the call kicks on its own.
     const DemKick hyd = {f_hyd, m_hyd};
     bool pending = false;
+    if (nsteps > 0) {                                                        // the DEM state in home order for the whole call
+        rc = ledds_dem_import(dem, x, v, w, a, alpha, radius, history, scratch, st);
+        if (rc) return rc;
+    }
     for (int step = 0; step < nsteps; ++step) {
         for (int sub = 0; sub < c->n_sub; ++sub) {
             // the contact pipeline of the last sub-step runs beside the lattice kernels: only the kick needs both
             const bool fork = sub == c->n_sub - 1 && dem->d.n > 0;
-            rc = ledds_dem_advance_contacts(dem, x, v, w, a, alpha, radius, history, scratch, status, dem->d.dt, true, st, fork,
-                                            pending ? &hyd : nullptr);
+            rc = ledds_dem_advance_contacts(dem, history, scratch, status, dem->d.dt, true, st, fork, pending ? &hyd : nullptr);
             if (rc) return rc;
             pending = sub < c->n_sub - 1;                                    // F_sf of the previous LBM step is held
             if (pending) dem->steps++;
@@ -417,7 +422,8 @@ static int coupled_step_t(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params
         dem->steps++;
         pending = step < nsteps - 1;
         if (!pending) {
-            rc = ledds_dem_kick(dem, v, w, a, alpha, radius, f_hyd, m_hyd, history, status, st);
+            rc = ledds_dem_kick(dem, f_hyd, m_hyd, history, scratch, st);
+            if (!rc) rc = ledds_dem_export(dem, x, v, w, a, alpha, scratch, st);
             if (rc) return rc;
         }
     }

@@ -1,16 +1,28 @@
 // DEM contact pipeline for spheres on sm_100a (Eq. 1-15, 158-192 Eq. 18-21, 431-511).
 //
-//   dem_drift_key_kernel   Eq. (18a) + predictor, cell key of every particle          (map N_part)
-//   dem_hist_kernel        digit histograms of all radix passes in one sweep          (smem histograms)
+// The particle state lives in the library's own "home" order between the steps of one call: the sorted order (cell
+// key, then id) of the last sort before the call began.  The caller's arrays are gathered once when a call begins
+// (dem_import_kernel) and scattered back once when it ends (dem_export_kernel); in between every per-particle access
+// is (nearly) sequential whatever order the caller numbers its particles in.
+//
+//   dem_drift_key_kernel   [kick of the previous step] + Eq. (18a) + predictor, cell key      (map N_part, home order)
+//   dem_hist_kernel        digit histograms of all radix passes in one sweep                  (smem histograms)
 //   dem_onesweep_kernel    one stable 8-bit radix pass: per-warp match ranking, chained scan with
-//                          decoupled look-back across tiles, scatter                    (x passes)
-//   dem_gather_kernel      sorted copies of x, v^p, w^p, R + cell start/end from key changes
-//   dem_contact_kernel     27-cell walk, Eq. (2)/(6) test, spring-dashpot + Coulomb + torque per pair,
-//                          history carried in per-particle slots, per-particle sums in registers
+//                          decoupled look-back across tiles, scatter                            (x passes)
+//   dem_ranges_kernel      cell start/end from the key changes
+//   dem_gather_kernel      ties of the sort put into id order; sorted copy of (x, R) + its single-precision copy, ids
+//   dem_detect_kernel      every pair of the 27-cell neighbourhood is tested ONCE, from the particle that comes first in
+//                          the sorted order (Eq. 2/6 in double after a first look in single precision); a contact is
+//                          entered into the lists of both partners (integer atomics on the list lengths)
+//   dem_scan_kernel        exclusive scan of the list lengths: the contact ends of all particles as one CSR array
+//   dem_fill_kernel        each particle orders its ends by partner id (the order of the paper's sorted pair list)
+//   dem_force_kernel       ONE THREAD PER CONTACT END: Eq. (7), (10)-(13), (5), (15), history carried per end; the
+//                          per-particle sums of Eq. (1) are taken by the particle's own thread from the block's shared
+//                          memory, in the order of the list: no floating-point atomics, bit-reproducible
 //   dem_kick_kernel        Eq. (18b-c), (19c-d) for spheres
 //
 // Compiled with -fmad=false: the discrete decisions (cell index, delta_n > 0) must not depend on
-// FMA contraction, and none of these kernels is ALU-bound.  No Thrust/CUB; no global fp atomics.
+// FMA contraction.  No Thrust/CUB; no global fp atomics.
 #include <math.h>
 
 #include <new>
@@ -20,12 +32,8 @@
 #define DEM_PI 3.14159265358979323846
 #define SORT_THREADS 256
 #define SORT_WARPS (SORT_THREADS / 32)
-#ifndef SORT_ITEMS
 #define SORT_ITEMS 12
-#endif
-#ifndef SORT_MIN_BLOCKS
 #define SORT_MIN_BLOCKS 4
-#endif
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define SORT_RADIX 256
 
@@ -34,9 +42,73 @@
 #define ST_VALUE_MASK 0x3fffffffu
 #define LOOKBACK 8
 
+#define SCAN_THREADS 256
+#define SCAN_ITEMS 8
+#define SCAN_TILE (SCAN_THREADS * SCAN_ITEMS)
+
+#define DEM_WALL 0xfffffff0u    // partner code of wall wl (0..5) in the contact lists: DEM_WALL + wl
+
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
 __device__ __forceinline__ double dem_mass(const DemDev& P, double R) { return P.density * (4.0 / 3.0) * DEM_PI * R * R * R; }
+
+// ------------------------------------------------------------------------------ import / export
+// Block = DRIFT_BLOCK particles; the [n][3] arrays are walked as flat arrays (element e = 3 h + k).
+#define DRIFT_BLOCK 128
+
+// hid_src: the caller id of every home slot of the NEW home order (NULL: identity).  perm: the OLD home index of the
+// particle in new slot h (NULL: identity); the per-particle records of the last force evaluation move with it.
+__global__ void __launch_bounds__(DRIFT_BLOCK) dem_import_kernel(
+    int n, const uint32_t* __restrict__ hid_src, const uint32_t* __restrict__ perm, const double* __restrict__ x,
+    const double* __restrict__ v, const double* __restrict__ w, const double* __restrict__ a, const double* __restrict__ alpha,
+    const double* __restrict__ radius, uint32_t* __restrict__ hid, double4* __restrict__ hx, double* __restrict__ hv,
+    double* __restrict__ hw, double* __restrict__ ha, double* __restrict__ hal, const double* __restrict__ fm_old,
+    const uint2* __restrict__ row_old, double* __restrict__ fm_new, uint2* __restrict__ row_new)
+{
+    const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * n;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const long long e = e0 + threadIdx.x + j * DRIFT_BLOCK;
+        if (e >= ne) break;
+        const int h = (int)(e / 3), k = (int)(e - 3ll * h);
+        const size_t src = 3 * (size_t)(hid_src ? hid_src[h] : (uint32_t)h) + k;
+        hv[e] = v[src]; hw[e] = w[src];
+        ha[e] = a ? a[src] : 0.0; hal[e] = alpha ? alpha[src] : 0.0;
+    }
+    const int h = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
+    if (h >= n) return;
+    const uint32_t i = hid_src ? hid_src[h] : (uint32_t)h;
+    hx[h] = make_double4(x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], radius[i]);
+    hid[h] = i;
+    const size_t o = perm ? perm[h] : (uint32_t)h;
+    row_new[h] = row_old[o];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) fm_new[6 * (size_t)h + c] = fm_old[6 * o + c];
+}
+
+__global__ void __launch_bounds__(DRIFT_BLOCK) dem_export_kernel(
+    int n, const uint32_t* __restrict__ hid, const double4* __restrict__ hx, const double* __restrict__ hv,
+    const double* __restrict__ hw, const double* __restrict__ ha, const double* __restrict__ hal, double* __restrict__ x,
+    double* __restrict__ v, double* __restrict__ w, double* __restrict__ a, double* __restrict__ alpha)
+{
+    const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * n;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const long long e = e0 + threadIdx.x + j * DRIFT_BLOCK;
+        if (e >= ne) break;
+        const int h = (int)(e / 3), k = (int)(e - 3ll * h);
+        const size_t dst = 3 * (size_t)hid[h] + k;
+        if (v) v[dst] = hv[e];
+        if (w) w[dst] = hw[e];
+        if (a) a[dst] = ha[e];
+        if (alpha) alpha[dst] = hal[e];
+    }
+    const int h = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
+    if (h >= n || !x) return;
+    const double4 r = hx[h];
+    const size_t i = hid[h];
+    x[3 * i] = r.x; x[3 * i + 1] = r.y; x[3 * i + 2] = r.z;
+}
 
 // ------------------------------------------------------------------------------ drift + key
 __device__ __forceinline__ int dem_cell_coord(const DemDev& P, double x, int a)
@@ -46,68 +118,68 @@ __device__ __forceinline__ int dem_cell_coord(const DemDev& P, double x, int a)
     return c > P.nc[a] - 1 ? P.nc[a] - 1 : c;
 }
 
-// Block = DRIFT_BLOCK particles.  The [n][3] arrays are walked as flat arrays (element e = 3 i + k), so every
-// load and store is fully coalesced; the new positions pass through shared memory to form the key and the
-// packed record per particle.
-// KICK = true: the kick of the previous step (Eq. 18b-c, 19c-d with the contact record ft and the external
-// force / torque) is applied first, in the same pass: between two steps of one call the state is read and
-// written once instead of twice.
-#define DRIFT_BLOCK 128
+// KICK = true: the kick of the previous step (Eq. 18b-c, 19c-d with the contact sums fm and the external force /
+// torque, which the caller indexes by particle id) is applied first, in the same pass: between two steps of one call
+// the state is read and written once instead of twice.  The new velocities and accelerations pass through shared
+// memory to the thread that owns the particle's packed (x, R) record.
 template <bool KICK>
 __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
-    const DemDev P, double* __restrict__ x, double* __restrict__ v, double* __restrict__ w, double* __restrict__ a,
-    double* __restrict__ alpha, const double* __restrict__ radius, const double* __restrict__ ft,
-    const double* __restrict__ f_ext, const double* __restrict__ m_ext, double* __restrict__ vp,
-    double* __restrict__ wp, double4* __restrict__ xr, uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift,
-    int32_t* __restrict__ status)
+    const DemDev P, double4* __restrict__ hx, double* __restrict__ hv, double* __restrict__ hw, double* __restrict__ ha,
+    double* __restrict__ hal, const uint32_t* __restrict__ hid, const double* __restrict__ fm,
+    const double* __restrict__ f_ext, const double* __restrict__ m_ext, double* __restrict__ pvw,
+    uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift, int32_t* __restrict__ status)
 {
-    __shared__ double sx[3 * DRIFT_BLOCK];
+    __shared__ double sv[3 * DRIFT_BLOCK], sa[3 * DRIFT_BLOCK];
     const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * P.n;
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
         const int le = threadIdx.x + j * DRIFT_BLOCK;
         const long long e = e0 + le;
         if (e >= ne) break;
-        const int k = le % 3;                                                 // e0 is a multiple of 3
-        double xv = x[e];
-        double vv = v[e], wv = w[e], av = a[e], alv = alpha[e];
+        const int h = (int)(e / 3), k = le % 3;                               // e0 is a multiple of 3
+        double vv = hv[e], wv = hw[e], av = ha[e], alv = hal[e];
         if (KICK) {                                                           // same expressions as dem_kick_kernel
-            const int i = (int)(e / 3);
-            const double R = radius[i];
+            const double R = reinterpret_cast<const double*>(hx)[4 * (size_t)h + 3];
             const double m = dem_mass(P, R), I = 0.4 * m * R * R;             // Eq. (21a)
-            const double Fq = ft[8 * (size_t)i + k] + (f_ext ? f_ext[e] : 0.0), Mq = ft[8 * (size_t)i + 3 + k] + (m_ext ? m_ext[e] : 0.0);
+            const size_t ie = (f_ext || m_ext) ? 3 * (size_t)hid[h] + k : 0;
+            const double Fq = fm[6 * (size_t)h + k] + (f_ext ? f_ext[ie] : 0.0), Mq = fm[6 * (size_t)h + 3 + k] + (m_ext ? m_ext[ie] : 0.0);
             const double an = Fq / m + P.g[k], aln = Mq / I;                  // Eq. (18b), (19c)
             vv = vv + (0.5 * P.dt) * (av + an);                               // Eq. (18c)
             wv = wv + (0.5 * P.dt) * (alv + aln);                             // Eq. (19d)
             av = an; alv = aln;
-            v[e] = vv; w[e] = wv; a[e] = av; alpha[e] = alv;
+            hv[e] = vv; hw[e] = wv; ha[e] = av; hal[e] = alv;
         }
         if (drift) {
-            xv = xv + P.dt * vv + (0.5 * P.dt * P.dt) * av;                   // Eq. (18a)
+            pvw[6 * (size_t)h + k] = vv + (0.5 * P.dt) * av;                  // predictor (G11)
+            pvw[6 * (size_t)h + 3 + k] = wv + (0.5 * P.dt) * alv;
+        } else {
+            pvw[6 * (size_t)h + k] = vv;
+            pvw[6 * (size_t)h + 3 + k] = wv;
+        }
+        sv[le] = vv; sa[le] = av;
+    }
+    __syncthreads();
+    const int h = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
+    if (h >= P.n) return;
+    const double4 r = hx[h];
+    double xn[3] = {r.x, r.y, r.z};
+    if (drift) {
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            double xv = xn[k] + P.dt * sv[3 * threadIdx.x + k] + (0.5 * P.dt * P.dt) * sa[3 * threadIdx.x + k];   // Eq. (18a)
             if (!P.bc[k]) {
                 if (xv >= P.hi[k]) xv -= P.L[k];
                 else if (xv < P.lo[k]) xv += P.L[k];
             }
-            x[e] = xv;
-            vp[e] = vv + (0.5 * P.dt) * av;                                   // predictor (G11)
-            wp[e] = wv + (0.5 * P.dt) * alv;
-        } else {
-            vp[e] = vv;
-            wp[e] = wv;
+            xn[k] = xv;
         }
-        sx[le] = xv;
+        hx[h] = make_double4(xn[0], xn[1], xn[2], r.w);
     }
-    __syncthreads();
-    const int i = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
-    if (i >= P.n) return;
-    const double xn[3] = {sx[3 * threadIdx.x], sx[3 * threadIdx.x + 1], sx[3 * threadIdx.x + 2]};
     const int cx = dem_cell_coord(P, xn[0], 0), cy = dem_cell_coord(P, xn[1], 1), cz = dem_cell_coord(P, xn[2], 2);
-    key[i] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
-    idx[i] = (uint32_t)i;
-    const double R = radius[i];
-    xr[i] = make_double4(xn[0], xn[1], xn[2], R);                  // one 32-byte sector per particle for the gather
+    key[h] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
+    idx[h] = (uint32_t)h;
     // input contract (include/ledds.h): 2 R <= cell width, centres inside a walled box
-    int st = 2.0 * R > P.hmin ? LEDDS_ST_RADIUS_RANGE : 0;
+    int st = 2.0 * r.w > P.hmin ? LEDDS_ST_RADIUS_RANGE : 0;
 #pragma unroll
     for (int a = 0; a < 3; ++a)
         if (P.bc[a] && !(xn[a] >= P.lo[a] && xn[a] <= P.hi[a])) st |= LEDDS_ST_OUT_OF_BOX;
@@ -115,16 +187,32 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
 }
 
 // ------------------------------------------------------------------------------ radix sort
-// All digit histograms in one pass over the keys (smem atomics, then one global add per bin).
+// All digit histograms in one pass over the keys (smem atomics, then one global add per bin).  The keys arrive in
+// home order, i.e. nearly sorted: the upper digits of a warp's 32 keys are usually all the same, and one lane then
+// adds 32 instead of 32 lanes queueing on one shared-memory word.
 __global__ void __launch_bounds__(SORT_THREADS) dem_hist_kernel(const uint32_t* __restrict__ key, int n, int passes,
                                                                uint32_t* __restrict__ ghist)
 {
     __shared__ uint32_t h[4][SORT_RADIX];
     for (int t = threadIdx.x; t < 4 * SORT_RADIX; t += blockDim.x) (&h[0][0])[t] = 0;
     __syncthreads();
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const uint32_t k = key[i];
-        for (int p = 0; p < passes; ++p) atomicAdd(&h[p][(k >> (8 * p)) & 255u], 1u);
+    const int lane = threadIdx.x & 31;
+    const int per = ((n + 31) / 32 + gridDim.x - 1) / gridDim.x * 32;             // a contiguous, warp-aligned piece per block
+    const int beg = blockIdx.x * per, end = min(n, beg + per);
+    for (int base = beg + (threadIdx.x & ~31); base < end; base += blockDim.x) {
+        const int i = base + lane;
+        const bool ok = i < end;
+        const uint32_t k = ok ? key[i] : 0u;
+        const unsigned live = __ballot_sync(0xffffffffu, ok);
+        for (int p = 0; p < passes; ++p) {
+            const uint32_t d = (k >> (8 * p)) & 255u;
+            const uint32_t d0 = __shfl_sync(0xffffffffu, d, __ffs(live) - 1);
+            if (__all_sync(0xffffffffu, !ok || d == d0)) {
+                if (lane == 0) atomicAdd(&h[p][d0], (uint32_t)__popc(live));
+            } else if (ok) {
+                atomicAdd(&h[p][d], 1u);
+            }
+        }
     }
     __syncthreads();
     for (int t = threadIdx.x; t < passes * SORT_RADIX; t += blockDim.x) {
@@ -279,26 +367,51 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS) dem_onesweep_ke
     }
 }
 
-// ------------------------------------------------------------------------------ gather + cell ranges
-__global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
-                                  const double4* __restrict__ xr, double4* __restrict__ xr_s,
-                                  float4* __restrict__ xf_s, uint2* __restrict__ cell_range)
+// ------------------------------------------------------------------------------ cell ranges + gather
+// The radix sort is stable with respect to its input order, the home order: inside a cell, particles that were there
+// before keep their relative (id) order, but one that has just moved in stands where its old home index puts it.  The
+// ordering the pipeline promises is (cell key, then ascending id) -- the stable sort of the ids, PAPER.md:388 -- so the
+// particles of a cell are ranked by id once more (cells hold a handful of particles).
+//   dem_ranges_kernel: [start, end) of every cell from the key changes (warp shuffle of neighbouring keys), and the id
+//                      of every particle in key-sorted order
+//   dem_gather_kernel: rank inside the cell by id -> final sorted position; sorted copies of (x, R), ids, home indices
+__global__ void dem_ranges_kernel(int n, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sh0,
+                                  const uint32_t* __restrict__ hid, uint32_t* __restrict__ sid_tmp, uint2* __restrict__ cell_range)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
-    const bool ok = s < P.n;
+    const bool ok = s < n;
     const uint32_t key = ok ? skey[s] : 0xffffffffu;
     // neighbours' keys inside the warp by shuffle, across warps by one extra load
     uint32_t prev = __shfl_up_sync(0xffffffffu, key, 1);
     uint32_t next = __shfl_down_sync(0xffffffffu, key, 1);
     if (!ok) return;
     if (lane == 0) prev = s > 0 ? skey[s - 1] : 0xffffffffu;
-    if (lane == 31 || s == P.n - 1) next = s < P.n - 1 ? skey[s + 1] : 0xffffffffu;
+    if (lane == 31 || s == n - 1) next = s < n - 1 ? skey[s + 1] : 0xffffffffu;
     if (s == 0 || prev != key) cell_range[key].x = (uint32_t)s;                    // [x, y) = the particles of the cell
-    if (s == P.n - 1 || next != key) cell_range[key].y = (uint32_t)s + 1u;
-    const double2* src = reinterpret_cast<const double2*>(xr + sidx[s]);
+    if (s == n - 1 || next != key) cell_range[key].y = (uint32_t)s + 1u;
+    sid_tmp[s] = hid[sh0[s]];
+}
+
+// sh0[s] = home index of the particle at key-sorted position s (a nearly sequential read of the home records)
+__global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sh0,
+                                  const uint32_t* __restrict__ sid_tmp, const uint2* __restrict__ cell_range,
+                                  const double4* __restrict__ hx, double4* __restrict__ xr_s, float4* __restrict__ xf_s,
+                                  uint32_t* __restrict__ sid, uint32_t* __restrict__ sh, uint32_t* __restrict__ ncand)
+{
+    const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s0 >= P.n) return;
+    const uint2 cr = cell_range[skey[s0]];
+    const uint32_t id = sid_tmp[s0];
+    uint32_t s = cr.x;
+    for (uint32_t t = cr.x; t < cr.y; ++t) s += sid_tmp[t] < id;                   // ids are distinct
+    const uint32_t h = sh0[s0];
+    const double2* src = reinterpret_cast<const double2*>(hx + h);
     const double2 a = __ldg(src), b = __ldg(src + 1);
     xr_s[s] = make_double4(a.x, a.y, b.x, b.y);
+    sid[s] = id;
+    sh[s] = h;
+    ncand[s] = 0u;
     // single-precision copy (x - lo, R) for the detect kernel's first look at a candidate (dem_near).  A particle
     // further than 2 L from the box corner (or not finite) gets NaN: it passes every first look.
     const double rx = a.x - P.lo[0], ry = a.y - P.lo[1], rz = b.x - P.lo[2];
@@ -308,8 +421,6 @@ __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ s
 }
 
 // ------------------------------------------------------------------------------ contact law
-struct Body { double x[3], v[3], w[3], R; };
-
 __device__ __forceinline__ void cross3(const double* a, const double* b, double* c)
 {
     c[0] = a[1] * b[2] - a[2] * b[1];
@@ -364,28 +475,12 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
     for (int a = 0; a < 3; ++a) F[a] = fn * en[a] + Ft[a];
 }
 
-// One thread per particle, in sorted order, two phases so that the lanes of a warp stay together:
-//   1. detect: walk the 9 runs of x-adjacent neighbour cells (they are contiguous in the sorted order), test
-//      Eq. (2)/(6) on the packed (x, R) records with squared distances (the square root only when the decision
-//      is within rounding) after a first look at the single-precision copy, and note the partners' sorted
-//      positions in a per-particle list in global memory;
-//   2. evaluate: all lanes work through their k-th contact together: Eq. (7), (10)-(13), (5), (15), history.
-// History slots: [sorted position of the step][slot] partner id + delta_t as seen from that particle (the partner
-// stores the negated vector).  Per-particle sums stay in registers: no atomics.
-// Tuning constants (overridable with -D for sweeps; the defaults are the measured best at 4 M spheres):
-#ifndef CONTACT_BLOCK
-#define CONTACT_BLOCK 128       // threads per block of both kernels (64 / 256: within 1 %)
-#endif
-#ifndef DETECT_NB
+// Tuning constants (the measured best at 4 M spheres)
+#define CONTACT_BLOCK 128       // threads per block of the detect and fill kernels
 #define DETECT_NB 3             // candidates in flight per iteration of the detect loop
-#endif
-#ifndef DETECT_MIN_BLOCKS
 #define DETECT_MIN_BLOCKS 8     // caps the detect kernel at 64 registers (8 blocks per SM)
-#endif
-#ifndef FORCE_MIN_BLOCKS
-#define FORCE_MIN_BLOCKS 1      // no register cap on the force kernel (caps spill and run slower)
-#endif
-#define DEM_IDLE 0xffffffffu   // ncand value of a particle the detect kernel has already finished
+#define FORCE_THREADS 256       // one thread per contact end ...
+#define FORCE_PB 512            // ... of the FORCE_PB particles of a block: ~6 full rounds of 256 ends in a dense bed
 
 // Stiffness and damping of one contact.  HERTZ = false: the linear spring-dashpot of the configs, gamma =
 // 2 zeta sqrt(k m*) (G5).  HERTZ = true: Hertz-Mindlin: (A.1) k_n = 4/3 Y* sqrt(R* d_n),
@@ -406,20 +501,6 @@ __device__ __forceinline__ void dem_coefficients(double kn0, double kt0, double 
         kn = kn0; kt = kt0;
         gn = 2.0 * zeta * sqrt(kn * mstar); gt = 2.0 * zeta * sqrt(kt * mstar);
     }
-}
-
-// one full 64-byte record per particle: contact force, torque, number of contacts and the row of the history
-// arrays that holds them (both exact in a double).  The history rows of a step are in that step's SORTED order
-// (row = sorted position): neighbouring threads write neighbouring rows, and because a particle's sorted
-// position changes little from one step to the next they also read nearly neighbouring rows.
-__device__ __forceinline__ void dem_store_ft(double* __restrict__ ft, uint32_t p, const double* F, const double* M, uint32_t count,
-                                             uint32_t row)
-{
-    double2* o = reinterpret_cast<double2*>(ft + 8 * (size_t)p);
-    o[0] = make_double2(F[0], F[1]);
-    o[1] = make_double2(F[2], M[0]);
-    o[2] = make_double2(M[1], M[2]);
-    o[3] = make_double2((double)count, (double)row);
 }
 
 // First look at a candidate on the 16-byte single-precision records: false only when the pair is certainly apart.
@@ -457,32 +538,34 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
     return sr - sqrt(d2) > 0.0;                                                       // Eq. (2), (6), strict (G7)
 }
 
-// cand[c][s] (c < ncand[s]) = sorted positions of the particles touching the particle at sorted position s
+// ------------------------------------------------------------------------------ detect
+// One thread per particle in sorted order.  The 9 runs of x-adjacent neighbour cells (contiguous in the sorted order;
+// a periodic row adds its one wrapped cell) are loaded up front and clipped to the positions AFTER the particle's own:
+// every unordered pair of the neighbourhood is looked at once, from the partner that comes first in the sorted order.
+// A contact is entered into both partners' lists: cand[c][s] (c < ncand[s]) = sorted positions of the particles that
+// touch the particle at sorted position s, or DEM_WALL + wall.  The order inside a list is the order of arrival (it
+// differs from run to run); dem_fill_kernel puts every list into the order of the partner ids.
 template <bool PERIODIC>
 __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_kernel(
-    const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sidx,
-    const double4* __restrict__ xr_s, const float4* __restrict__ xf_s, const uint2* __restrict__ cell_range,
-    const double* __restrict__ vp, const double* __restrict__ wp, double2* __restrict__ vw_s, uint32_t* __restrict__ ncand_g,
-    uint32_t* __restrict__ cand_g, double* __restrict__ ft_new, int32_t* __restrict__ status)
+    const DemDev P, const uint32_t* __restrict__ skey, const double4* __restrict__ xr_s, const float4* __restrict__ xf_s,
+    const uint2* __restrict__ cell_range, uint32_t* __restrict__ ncand, uint32_t* __restrict__ cand, int32_t* __restrict__ status)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
-    const int maxc = P.maxc;
+    const uint32_t maxc = (uint32_t)P.maxc;
     const uint32_t key = skey[s];
     const double4 mine = xr_s[s];
     const float4 minef = xf_s[s];
     int st = 0;
-    int ncand = 0;
 
     const int c0 = (int)(key % (uint32_t)P.nc[0]);
     const int c1 = (int)((key / (uint32_t)P.nc[0]) % (uint32_t)P.nc[1]);
     const int c2 = (int)(key / ((uint32_t)P.nc[0] * (uint32_t)P.nc[1]));
 
-    // ---- phase 1: detect
-    auto note = [&](uint32_t t) {
-        if (ncand < maxc) cand_g[(size_t)ncand * P.n + s] = t;
+    auto enter = [&](uint32_t owner, uint32_t partner) {
+        const uint32_t c = atomicAdd(ncand + owner, 1u);
+        if (c < maxc) cand[(size_t)c * P.n + owner] = partner;
         else st |= LEDDS_ST_CONTACT_OVERFLOW;
-        ncand += ncand < maxc;
     };
     // the 9 runs [t0, t1) of x-adjacent cells (c0-1 .. c0+1 inside the row): all 27 range loads are independent
     // and issued together; an empty cell holds (0, 0), so "first start, last end" needs no special case
@@ -502,7 +585,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
             if (c0 < P.nc[0] - 1) r2 = row[1];
         }
         const bool e0 = r0.y > r0.x, e1 = r1.y > r1.x, e2 = r2.y > r2.x;
-        t0[j] = e0 ? r0.x : (e1 ? r1.x : r2.x);
+        t0[j] = max(e0 ? r0.x : (e1 ? r1.x : r2.x), (uint32_t)s + 1u);               // only the positions after mine
         t1[j] = e2 ? r2.y : (e1 ? r1.y : r0.y);
     }
 #pragma unroll
@@ -518,13 +601,13 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
             }
 #pragma unroll
             for (int b = 0; b < DETECT_NB; ++b) {
-                nn[b] = dem_near<PERIODIC>(P, minef, fc[b]) & ((int)tt[b] != s) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
+                nn[b] = dem_near<PERIODIC>(P, minef, fc[b]) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
                 any |= nn[b];
             }
             if (any) {                                                             // Eq. (2) in double for the few that pass
 #pragma unroll
                 for (int b = 0; b < DETECT_NB; ++b)
-                    if (nn[b] && dem_touch<PERIODIC>(P, mine, xr_s[tt[b]])) note(tt[b]);
+                    if (nn[b] && dem_touch<PERIODIC>(P, mine, xr_s[tt[b]])) { enter((uint32_t)s, tt[b]); enter(tt[b], (uint32_t)s); }
             }
         }
     }
@@ -535,188 +618,313 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
             if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) continue; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
             if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) continue; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
             const uint2 r = cell_range[(size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + wc];
-            for (uint32_t t = r.x; t < r.y; ++t)
-                if ((int)t != s && dem_near<PERIODIC>(P, minef, xf_s[t]) && dem_touch<PERIODIC>(P, mine, xr_s[t])) note(t);
+            for (uint32_t t = max(r.x, (uint32_t)s + 1u); t < r.y; ++t)
+                if (dem_near<PERIODIC>(P, minef, xf_s[t]) && dem_touch<PERIODIC>(P, mine, xr_s[t])) { enter((uint32_t)s, t); enter(t, (uint32_t)s); }
         }
     }
-
-    // a particle that touches nothing and has no wall in reach is finished here (the usual case in a dilute
-    // state): zero record written, DEM_IDLE tells the force kernel to skip it
-    bool near_wall = false;
+    // walls: static infinite particles; overlap decided as the oracle does, R - distance > 0
     const double xm[3] = {mine.x, mine.y, mine.z};
 #pragma unroll
-    for (int a = 0; a < 3; ++a)
-        if (P.bc[a] && (xm[a] - P.lo[a] < mine.w || P.hi[a] - xm[a] < mine.w)) near_wall = true;
-    if (ncand == 0 && !near_wall) {
-        const double zero[3] = {0.0, 0.0, 0.0};
-        dem_store_ft(ft_new, sidx[s], zero, zero, 0u, 0u);
-        ncand_g[s] = DEM_IDLE;
-    } else {
-        // predictor velocities of the particles that take part in a contact, in sorted order: the force kernel
-        // reads its own and its partners' (v^p, w^p) from neighbouring records instead of by particle id
-        const size_t p3 = 3 * (size_t)sidx[s];
-        double2* o = vw_s + 3 * (size_t)s;
-        o[0] = make_double2(vp[p3], vp[p3 + 1]);
-        o[1] = make_double2(vp[p3 + 2], wp[p3]);
-        o[2] = make_double2(wp[p3 + 1], wp[p3 + 2]);
-        ncand_g[s] = (uint32_t)ncand;
+    for (int wl = 0; wl < 6; ++wl) {
+        const int ax = wl >> 1;
+        if (!P.bc[ax]) continue;
+        const double dist = (wl & 1) ? P.hi[ax] - xm[ax] : xm[ax] - P.lo[ax];
+        if (mine.w - dist > 0.0) enter((uint32_t)s, DEM_WALL + (uint32_t)wl);
     }
     if (st) atomicOr(status, st);
 }
 
-// ---- phase 2: evaluate
-template <bool HERTZ>
-__global__ void __launch_bounds__(CONTACT_BLOCK, FORCE_MIN_BLOCKS) dem_force_kernel(
-    const DemDev P, const uint32_t* __restrict__ sidx, const double4* __restrict__ xr_s,
-    const double2* __restrict__ vw_s, const uint32_t* __restrict__ ncand_g, const uint32_t* __restrict__ cand_g,
-    const double* __restrict__ ft_prev, const uint32_t* __restrict__ hid_prev, const double* __restrict__ hdt_prev,
-    double* __restrict__ ft_new, uint32_t* __restrict__ hid_new, double* __restrict__ hdt_new,
-    int32_t* __restrict__ status, double dt_hist)
+// ------------------------------------------------------------------------------ scan
+// off[s] = sum over s' < s of min(ncand[s'], maxc), off[n] = total: single pass, chained tiles with decoupled look-back
+// (tiles take tickets, as in the sort).
+__global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ cnt,
+                                                               uint32_t* __restrict__ off, uint32_t* __restrict__ state,
+                                                               uint32_t* __restrict__ ticket)
 {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= P.n) return;
-    const int maxc = P.maxc;
-    if (ncand_g[s] == DEM_IDLE) return;
-    const double4 mine = xr_s[s];
-    const int ncand = (int)ncand_g[s];
-    int st = 0;
-    const uint32_t p = sidx[s];
-    Body me;
-    me.x[0] = mine.x; me.x[1] = mine.y; me.x[2] = mine.z; me.R = mine.w;
-    {
-        const double2* r = vw_s + 3 * (size_t)s;
-        const double2 a = r[0], b = r[1], c = r[2];
-        me.v[0] = a.x; me.v[1] = a.y; me.v[2] = b.x; me.w[0] = b.y; me.w[1] = c.x; me.w[2] = c.y;
+    __shared__ uint32_t wsum[SCAN_THREADS / 32];
+    __shared__ uint32_t s_tile, s_excl;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const long long first = (long long)tile * SCAN_TILE + (long long)tid * SCAN_ITEMS;
+    uint32_t c[SCAN_ITEMS], sum = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) {
+        c[i] = first + i < n ? min(cnt[first + i], maxc) : 0u;
+        sum += c[i];
     }
-    const double m_me = dem_mass(P, me.R);
-    const double2 cr = *reinterpret_cast<const double2*>(ft_prev + 8 * (size_t)p + 6);   // (contacts, row) of the last step
-    const uint32_t nprev = (uint32_t)cr.x;
-    const size_t prow = (size_t)cr.y;
-    const uint32_t* pid = hid_prev + prow * maxc;
-    const double* pdt = hdt_prev + prow * maxc * 3;
-    uint32_t* nid = hid_new + (size_t)s * maxc;
-    double* ndt = hdt_new + (size_t)s * maxc * 3;
-    double Fs[3] = {0, 0, 0}, Ms[3] = {0, 0, 0};
-    uint32_t ncont = 0;
-
-    for (int c = 0; c < ncand; ++c) {
-        const uint32_t t = cand_g[(size_t)c * P.n + s];
-        const double4 o4 = xr_s[t];
-        const uint32_t q = sidx[t];
-        Body ot;
-        ot.x[0] = o4.x; ot.x[1] = o4.y; ot.x[2] = o4.z; ot.R = o4.w;
-        {
-            const double2* r = vw_s + 3 * (size_t)t;
-            const double2 a = r[0], b = r[1], c = r[2];
-            ot.v[0] = a.x; ot.v[1] = a.y; ot.v[2] = b.x; ot.w[0] = b.y; ot.w[1] = c.x; ot.w[2] = c.y;
-        }
-        const bool me_first = p < q;                                                   // canonical orientation i < j
-        const Body& bi = me_first ? me : ot;
-        const Body& bj = me_first ? ot : me;
-        double d[3];
-        dem_min_image(P, bi.x, bj.x, d);
-        const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-        const double dn = (bi.R + bj.R) - dist;                                        // Eq. (6)
-        if (dist == 0.0) { st |= LEDDS_ST_COINCIDENT; continue; }
-        double en[3] = {d[0] / dist, d[1] / dist, d[2] / dist};                        // Eq. (7)
-        const double mi = dem_mass(P, bi.R), mj = dem_mass(P, bj.R);
-        const double mstar = mi * mj / (mi + mj);                                      // (A.9)
-        const double sg = me_first ? 1.0 : -1.0;
-        double dt3[3] = {0, 0, 0};                                                     // previous delta_t, canonical
-        for (uint32_t h = 0; h < nprev; ++h)
-            if (pid[h] == q) {
-                dt3[0] = sg * pdt[3 * h]; dt3[1] = sg * pdt[3 * h + 1]; dt3[2] = sg * pdt[3 * h + 2];
-                break;
+    uint32_t incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    uint32_t before = 0, total = 0;
+#pragma unroll
+    for (int w2 = 0; w2 < SCAN_THREADS / 32; ++w2) {
+        if (w2 < warp) before += wsum[w2];
+        total += wsum[w2];
+    }
+    if (tid == 0) {
+        uint32_t excl = 0;
+        if (tile == 0) {
+            st_volatile(state, ST_FLAG_PRE | total);
+        } else {
+            st_volatile(state + tile, ST_FLAG_AGG | total);
+            long long t = (long long)tile - 1;
+            for (;;) {
+                uint32_t sb = ld_volatile(state + t);
+                while ((sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0) sb = ld_volatile(state + t);
+                excl += sb & ST_VALUE_MASK;
+                if (sb & ST_FLAG_PRE) break;
+                --t;
             }
-        double F[3], T[3];
-        double kn, kt, gn, gt;
-        dem_coefficients<HERTZ>(P.kn, P.kt, P.Ystar, P.Gstar, P.zeta, mstar, bi.R * bj.R / (bi.R + bj.R), dn, kn, kt, gn, gt);
-        dem_pair_force(en, dn, bi.v, bi.w, bi.R, bj.v, bj.w, bj.R, kn, kt, gn, gt, P.mu, dt_hist, dt3, F, T);
-#pragma unroll
-        for (int a = 0; a < 3; ++a) { Fs[a] += sg * F[a]; Ms[a] += me.R * (-T[a]); }
-        nid[ncont] = q;
-        ndt[3 * ncont] = sg * dt3[0]; ndt[3 * ncont + 1] = sg * dt3[1]; ndt[3 * ncont + 2] = sg * dt3[2];
-        ++ncont;
+            st_volatile(state + tile, ST_FLAG_PRE | (excl + total));
+        }
+        s_excl = excl;
     }
-    // walls: static infinite particles with a surface velocity
-    for (int wl = 0; wl < 6; ++wl) {
-        const int ax = wl >> 1, side = wl & 1;
-        if (!P.bc[ax]) continue;
-        const double dist = side ? P.hi[ax] - me.x[ax] : me.x[ax] - P.lo[ax];
-        const double dn = me.R - dist;
-        if (!(dn > 0.0)) continue;
-        double en[3] = {0, 0, 0};
-        en[ax] = side ? -1.0 : 1.0;
-        const uint32_t q = (uint32_t)P.n + (uint32_t)wl;
-        double dt3[3] = {0, 0, 0};
-        for (uint32_t h = 0; h < nprev; ++h)
-            if (pid[h] == q) { dt3[0] = pdt[3 * h]; dt3[1] = pdt[3 * h + 1]; dt3[2] = pdt[3 * h + 2]; break; }
-        const double vj[3] = {P.vw[wl * 3], P.vw[wl * 3 + 1], P.vw[wl * 3 + 2]}, wj[3] = {0, 0, 0};
-        double F[3], T[3];
-        double kn, kt, gn, gt;                                                        // the wall: R* = R_i, m* = m_i
-        dem_coefficients<HERTZ>(P.kn_w, P.kt_w, P.Ystar_w, P.Gstar_w, P.zeta_w, m_me, me.R, dn, kn, kt, gn, gt);
-        dem_pair_force(en, dn, me.v, me.w, me.R, vj, wj, 0.0, kn, kt, gn, gt, P.mu_w, dt_hist, dt3, F, T);
+    __syncthreads();
+    uint32_t run = s_excl + before + incl - sum;
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { Fs[a] += F[a]; Ms[a] += me.R * (-T[a]); }
-        if (ncont < (uint32_t)maxc) {
-            nid[ncont] = q;
-            ndt[3 * ncont] = dt3[0]; ndt[3 * ncont + 1] = dt3[1]; ndt[3 * ncont + 2] = dt3[2];
-            ++ncont;
-        } else st |= LEDDS_ST_CONTACT_OVERFLOW;
+    for (int i = 0; i < SCAN_ITEMS; ++i) {
+        if (first + i < n) off[first + i] = run;
+        run += c[i];
+        if (first + i == n - 1) off[n] = run;
     }
+}
+
+// ------------------------------------------------------------------------------ fill
+// One thread per particle: its list of partners, put into ascending order of the partner id (walls, id n + wall, last):
+// the order of the paper's lexicographically sorted pair list, which is also the order the oracle sums in.
+// end_s / end_t / hq are the CSR arrays of contact ends the force kernel works through.
+__global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ ncand,
+                                                                const uint32_t* __restrict__ cand, const uint32_t* __restrict__ sid,
+                                                                const uint32_t* __restrict__ off, uint32_t* __restrict__ end_s,
+                                                                uint32_t* __restrict__ end_t, uint32_t* __restrict__ hq)
+{
+    extern __shared__ uint2 tq[];                                                   // [maxc][CONTACT_BLOCK]: (partner code, partner id)
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const uint32_t cnt = min(ncand[s], maxc);
+    if (cnt == 0) return;
+    uint2* mine = tq + threadIdx.x;
+    for (uint32_t c = 0; c < cnt; ++c) {
+        const uint32_t t = cand[(size_t)c * n + s];
+        const uint32_t q = t >= DEM_WALL ? (uint32_t)n + (t - DEM_WALL) : sid[t];
+        uint32_t k = c;                                                             // insertion sort by q
+        while (k > 0 && mine[(k - 1) * CONTACT_BLOCK].y > q) { mine[k * CONTACT_BLOCK] = mine[(k - 1) * CONTACT_BLOCK]; --k; }
+        mine[k * CONTACT_BLOCK] = make_uint2(t, q);
+    }
+    const uint32_t o = off[s];
+    for (uint32_t c = 0; c < cnt; ++c) {
+        const uint2 e = mine[c * CONTACT_BLOCK];
+        end_s[o + c] = (uint32_t)s;
+        end_t[o + c] = e.x;
+        hq[o + c] = e.y;
+    }
+}
+
+// ------------------------------------------------------------------------------ force
+// A block owns FORCE_PB consecutive particles (sorted order) and all their contact ends, a contiguous piece
+// [off[s0], off[s0 + FORCE_PB]) of the CSR arrays.  It works through that piece FORCE_THREADS ends at a time, one end per
+// thread (all lanes busy whatever the contact counts of the particles are): both partners evaluate a contact in its
+// canonical orientation (i < j), so F_ij = -F_ji bit for bit; the end's force and torque go to shared memory, and the
+// thread that owns the particle adds up its ends in list order.  History: the previous delta_t of the end is looked up
+// in the particle's own row of last step's CSR arrays (row = (first, count), kept per particle in home order).
+template <bool HERTZ>
+__global__ void __launch_bounds__(FORCE_THREADS) dem_force_kernel(
+    const DemDev P, const uint32_t* __restrict__ sid, const uint32_t* __restrict__ sh, const double4* __restrict__ xr_s,
+    const double* __restrict__ pvw, const uint32_t* __restrict__ off, const uint32_t* __restrict__ end_s,
+    const uint32_t* __restrict__ end_t, const uint32_t* __restrict__ hq_new, uint2* __restrict__ row,
+    double* __restrict__ fm, const uint32_t* __restrict__ hq_prev, const double* __restrict__ hdt_prev,
+    double* __restrict__ hdt_new, int32_t* __restrict__ status, double dt_hist)
+{
+    __shared__ uint32_t s_off[FORCE_PB + 1];
+    __shared__ double stage[6][FORCE_THREADS];
+    const int tid = threadIdx.x;
+    const int s0 = blockIdx.x * FORCE_PB, np = min(FORCE_PB, P.n - s0);
+    for (int i = tid; i <= np; i += FORCE_THREADS) s_off[i] = off[s0 + i];
+    __syncthreads();
+    const uint32_t e_begin = s_off[0], e_end = s_off[np];
+    constexpr int OWN = FORCE_PB / FORCE_THREADS;
+    double acc[OWN][6];
 #pragma unroll
-    for (int a = 0; a < 3; ++a)
-        if (!isfinite(Fs[a]) || !isfinite(Ms[a])) st |= LEDDS_ST_NONFINITE;
-    dem_store_ft(ft_new, p, Fs, Ms, ncont, (uint32_t)s);
+    for (int j = 0; j < OWN; ++j)
+#pragma unroll
+        for (int c = 0; c < 6; ++c) acc[j][c] = 0.0;
+    int st = 0;
+
+    for (uint32_t chunk = e_begin; chunk < e_end; chunk += FORCE_THREADS) {
+        const uint32_t e = chunk + (uint32_t)tid;
+        double Fe[3] = {0, 0, 0}, Me[3] = {0, 0, 0};
+        if (e < e_end) {
+            const uint32_t s = end_s[e], t = end_t[e], q = hq_new[e];
+            const uint32_t p = sid[s], h = sh[s];
+            const double4 m4 = xr_s[s];
+            const double xm[3] = {m4.x, m4.y, m4.z}, Rm = m4.w;
+            double vm[3], wm[3];
+            {
+                const double2* r = reinterpret_cast<const double2*>(pvw + 6 * (size_t)h);
+                const double2 a = r[0], b = r[1], c = r[2];
+                vm[0] = a.x; vm[1] = a.y; vm[2] = b.x; wm[0] = b.y; wm[1] = c.x; wm[2] = c.y;
+            }
+            // previous delta_t of this end, as its owner stored it
+            double dt3[3] = {0, 0, 0};
+            {
+                const uint2 pr = row[h];
+                for (uint32_t k = 0; k < pr.y; ++k)
+                    if (hq_prev[pr.x + k] == q) {
+                        const double* d = hdt_prev + 3 * (size_t)(pr.x + k);
+                        dt3[0] = d[0]; dt3[1] = d[1]; dt3[2] = d[2];
+                        break;
+                    }
+            }
+            double F[3], T[3], kn, kt, gn, gt;
+            if (t < DEM_WALL) {
+                const double4 o4 = xr_s[t];
+                const double xo[3] = {o4.x, o4.y, o4.z}, Ro = o4.w;
+                double vo[3], wo[3];
+                {
+                    const double2* r = reinterpret_cast<const double2*>(pvw + 6 * (size_t)sh[t]);
+                    const double2 a = r[0], b = r[1], c = r[2];
+                    vo[0] = a.x; vo[1] = a.y; vo[2] = b.x; wo[0] = b.y; wo[1] = c.x; wo[2] = c.y;
+                }
+                const bool me_first = p < q;                                           // canonical orientation i < j
+                const double sg = me_first ? 1.0 : -1.0;
+                double xi[3], xj[3], vi[3], vj[3], wi[3], wj[3];
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    xi[a] = me_first ? xm[a] : xo[a]; xj[a] = me_first ? xo[a] : xm[a];
+                    vi[a] = me_first ? vm[a] : vo[a]; vj[a] = me_first ? vo[a] : vm[a];
+                    wi[a] = me_first ? wm[a] : wo[a]; wj[a] = me_first ? wo[a] : wm[a];
+                }
+                const double Ri = me_first ? Rm : Ro, Rj = me_first ? Ro : Rm;
+                double d[3];
+                dem_min_image(P, xi, xj, d);
+                const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+                const double dn = (Ri + Rj) - dist;                                    // Eq. (6)
+                if (dist == 0.0) {
+                    st |= LEDDS_ST_COINCIDENT;                                         // pair skipped, delta_t = 0 (as the oracle)
+                    dt3[0] = dt3[1] = dt3[2] = 0.0;
+                } else {
+                    const double en[3] = {d[0] / dist, d[1] / dist, d[2] / dist};      // Eq. (7)
+                    const double mi = dem_mass(P, Ri), mj = dem_mass(P, Rj);
+                    const double mstar = mi * mj / (mi + mj);                          // (A.9)
+                    dt3[0] *= sg; dt3[1] *= sg; dt3[2] *= sg;                          // canonical
+                    dem_coefficients<HERTZ>(P.kn, P.kt, P.Ystar, P.Gstar, P.zeta, mstar, Ri * Rj / (Ri + Rj), dn, kn, kt, gn, gt);
+                    dem_pair_force(en, dn, vi, wi, Ri, vj, wj, Rj, kn, kt, gn, gt, P.mu, dt_hist, dt3, F, T);
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) { Fe[a] = sg * F[a]; Me[a] = Rm * (-T[a]); dt3[a] *= sg; }
+                }
+            } else {                                                                   // a wall: R* = R_i, m* = m_i
+                const int wl = (int)(t - DEM_WALL), ax = wl >> 1, side = wl & 1;
+                const double xa = ax == 0 ? xm[0] : (ax == 1 ? xm[1] : xm[2]);          // selects: the arrays stay in registers
+                const double dist = side ? P.hi[ax] - xa : xa - P.lo[ax];
+                const double dn = Rm - dist;
+                const double sgn = side ? -1.0 : 1.0;
+                const double en[3] = {ax == 0 ? sgn : 0.0, ax == 1 ? sgn : 0.0, ax == 2 ? sgn : 0.0};
+                const double vj[3] = {P.vw[wl * 3], P.vw[wl * 3 + 1], P.vw[wl * 3 + 2]}, wj[3] = {0, 0, 0};
+                dem_coefficients<HERTZ>(P.kn_w, P.kt_w, P.Ystar_w, P.Gstar_w, P.zeta_w, dem_mass(P, Rm), Rm, dn, kn, kt, gn, gt);
+                dem_pair_force(en, dn, vm, wm, Rm, vj, wj, 0.0, kn, kt, gn, gt, P.mu_w, dt_hist, dt3, F, T);
+#pragma unroll
+                for (int a = 0; a < 3; ++a) { Fe[a] = F[a]; Me[a] = Rm * (-T[a]); }
+            }
+            double* nd = hdt_new + 3 * (size_t)e;
+            nd[0] = dt3[0]; nd[1] = dt3[1]; nd[2] = dt3[2];
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { stage[a][tid] = Fe[a]; stage[3 + a][tid] = Me[a]; }
+        __syncthreads();
+        // Eq. (1): every particle's thread adds up the ends of this round that are its own, in list order
+#pragma unroll
+        for (int j = 0; j < OWN; ++j) {
+            const int i = tid + j * FORCE_THREADS;
+            if (i < np) {
+                const uint32_t lo = max(s_off[i], chunk), hi = min(s_off[i + 1], chunk + (uint32_t)FORCE_THREADS);
+                for (uint32_t e2 = lo; e2 < hi; ++e2)
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) acc[j][c] += stage[c][e2 - chunk];
+            }
+        }
+        __syncthreads();
+    }
+    // the particle's record for the kick and for the next step's history look-up (home order)
+#pragma unroll
+    for (int j = 0; j < OWN; ++j) {
+        const int i = tid + j * FORCE_THREADS;
+        if (i >= np) continue;
+        const uint32_t h = sh[s0 + i];
+        const uint32_t cnt = s_off[i + 1] - s_off[i];
+        const uint2 old = row[h];
+        if (cnt == 0 && old.y == 0) continue;                  // no contact now, none before: the record is zero already
+        row[h] = make_uint2(s_off[i], cnt);
+        bool finite = true;
+#pragma unroll
+        for (int c = 0; c < 6; ++c) { fm[6 * (size_t)h + c] = acc[j][c]; finite = finite && isfinite(acc[j][c]); }
+        if (!finite) st |= LEDDS_ST_NONFINITE;
+    }
     if (st) atomicOr(status, st);
 }
 
 // ------------------------------------------------------------------------------ kick
-// One thread per vector component (element e = 3 i + k of the flat [n][3] arrays): coalesced.
-__global__ void dem_kick_kernel(const DemDev P, const double* __restrict__ radius, const double* __restrict__ ft,
-                                const double* __restrict__ f_ext, const double* __restrict__ m_ext, double* __restrict__ v,
-                                double* __restrict__ w, double* __restrict__ a, double* __restrict__ alpha, int only_accel)
+// One thread per vector component (element e = 3 h + k of the flat home arrays): coalesced.
+__global__ void dem_kick_kernel(const DemDev P, const double4* __restrict__ hx, const uint32_t* __restrict__ hid,
+                                const double* __restrict__ fm, const double* __restrict__ f_ext, const double* __restrict__ m_ext,
+                                double* __restrict__ hv, double* __restrict__ hw, double* __restrict__ ha, double* __restrict__ hal,
+                                int only_accel)
 {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= 3ll * P.n) return;
-    const int i = (int)(e / 3), k = (int)(e - 3ll * i);
-    const double R = radius[i];
+    const int h = (int)(e / 3), k = (int)(e - 3ll * h);
+    const double R = reinterpret_cast<const double*>(hx)[4 * (size_t)h + 3];
     const double m = dem_mass(P, R), I = 0.4 * m * R * R;                             // Eq. (21a)
-    const double Fq = ft[8 * (size_t)i + k] + (f_ext ? f_ext[e] : 0.0), Mq = ft[8 * (size_t)i + 3 + k] + (m_ext ? m_ext[e] : 0.0);
+    const size_t ie = (f_ext || m_ext) ? 3 * (size_t)hid[h] + k : 0;
+    const double Fq = fm[6 * (size_t)h + k] + (f_ext ? f_ext[ie] : 0.0), Mq = fm[6 * (size_t)h + 3 + k] + (m_ext ? m_ext[ie] : 0.0);
     const double an = Fq / m + P.g[k], aln = Mq / I;                                  // Eq. (18b), (19c)
     if (!only_accel) {
-        v[e] = v[e] + (0.5 * P.dt) * (a[e] + an);                                     // Eq. (18c)
-        w[e] = w[e] + (0.5 * P.dt) * (alpha[e] + aln);                                // Eq. (19d)
+        hv[e] = hv[e] + (0.5 * P.dt) * (ha[e] + an);                                  // Eq. (18c)
+        hw[e] = hw[e] + (0.5 * P.dt) * (hal[e] + aln);                                // Eq. (19d)
     }
-    a[e] = an;
-    alpha[e] = aln;
+    ha[e] = an;
+    hal[e] = aln;
 }
 
 // ------------------------------------------------------------------------------ query (parity only)
-__global__ void dem_pair_count_kernel(int n, int maxc, const double* __restrict__ ft,
-                                      const uint32_t* __restrict__ hid, uint32_t* __restrict__ cnt)
+__global__ void dem_query_pos_kernel(int n, const uint32_t* __restrict__ sid, uint32_t* __restrict__ pos_of_id)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s < n) pos_of_id[sid[s]] = (uint32_t)s;
+}
+
+// contact ends of particle id p with a partner of higher id: the pairs (p, q) of the canonical list
+__global__ void dem_pair_count_kernel(int n, const uint32_t* __restrict__ pos_of_id, const uint32_t* __restrict__ off,
+                                      const uint32_t* __restrict__ hq, uint32_t* __restrict__ cnt)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
+    const uint32_t s = pos_of_id[p];
     uint32_t c = 0;
-    const uint32_t hc = (uint32_t)ft[8 * (size_t)p + 6];
-    const size_t row = (size_t)ft[8 * (size_t)p + 7];
-    for (uint32_t h = 0; h < hc; ++h) c += hid[row * maxc + h] > (uint32_t)p;
+    for (uint32_t e = off[s]; e < off[s + 1]; ++e) c += hq[e] > (uint32_t)p;
     cnt[p] = c;
 }
 
-__global__ void dem_unpack_ft_kernel(int n, const double* __restrict__ ft, double* __restrict__ force, double* __restrict__ torque)
+__global__ void dem_unpack_fm_kernel(int n, const uint32_t* __restrict__ hid, const double* __restrict__ fm,
+                                     double* __restrict__ force, double* __restrict__ torque)
 {
-    const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n) return;
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n) return;
+    const size_t p = hid[h];
     for (int a = 0; a < 3; ++a) {
-        if (force) force[3 * p + a] = ft[8 * (size_t)p + a];
-        if (torque) torque[3 * p + a] = ft[8 * (size_t)p + 3 + a];
+        if (force) force[3 * p + a] = fm[6 * (size_t)h + a];
+        if (torque) torque[3 * p + a] = fm[6 * (size_t)h + 3 + a];
     }
 }
 
 // single-block exclusive scan of cnt[n] into off[n+1]
-__global__ void __launch_bounds__(1024) dem_scan_kernel(int n, const uint32_t* __restrict__ cnt, uint32_t* __restrict__ off)
+__global__ void __launch_bounds__(1024) dem_block_scan_kernel(int n, const uint32_t* __restrict__ cnt, uint32_t* __restrict__ off)
 {
     __shared__ uint32_t wsum[32];
     __shared__ uint32_t carry;
@@ -753,31 +961,25 @@ __global__ void __launch_bounds__(1024) dem_scan_kernel(int n, const uint32_t* _
     if (tid == 0) off[n] = carry;
 }
 
-__global__ void dem_pair_write_kernel(int n, int maxc, const double* __restrict__ ft,
-                                      const uint32_t* __restrict__ hid, const double* __restrict__ hdt,
-                                      const uint32_t* __restrict__ off, uint32_t cap, uint32_t* __restrict__ pairs,
+// the list of a particle is in ascending order of the partner id already (dem_fill_kernel)
+__global__ void dem_pair_write_kernel(int n, const uint32_t* __restrict__ pos_of_id, const uint32_t* __restrict__ off,
+                                      const uint32_t* __restrict__ hq, const double* __restrict__ hdt,
+                                      const uint32_t* __restrict__ pair_off, uint32_t cap, uint32_t* __restrict__ pairs,
                                       double* __restrict__ pair_dt, uint32_t* __restrict__ n_pairs)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p == 0 && n_pairs) *n_pairs = off[n];
+    if (p == 0 && n_pairs) *n_pairs = pair_off[n];
     if (p >= n) return;
-    uint32_t ids[32], slot[32];
-    int c = 0;
-    const uint32_t hc = (uint32_t)ft[8 * (size_t)p + 6];
-    const size_t row = (size_t)ft[8 * (size_t)p + 7];
-    for (uint32_t h = 0; h < hc; ++h) {
-        const uint32_t q = hid[row * maxc + h];
+    const uint32_t s = pos_of_id[p];
+    uint32_t o = pair_off[p];
+    for (uint32_t e = off[s]; e < off[s + 1]; ++e) {
+        const uint32_t q = hq[e];
         if (q <= (uint32_t)p) continue;
-        int k = c++;
-        while (k > 0 && ids[k - 1] > q) { ids[k] = ids[k - 1]; slot[k] = slot[k - 1]; --k; }   // insertion sort
-        ids[k] = q; slot[k] = h;
-    }
-    for (int k = 0; k < c; ++k) {
-        const uint32_t o = off[p] + k;
         if (o >= cap) break;
-        if (pairs) { pairs[2 * o] = (uint32_t)p; pairs[2 * o + 1] = ids[k]; }
+        if (pairs) { pairs[2 * (size_t)o] = (uint32_t)p; pairs[2 * (size_t)o + 1] = q; }
         if (pair_dt)
-            for (int a = 0; a < 3; ++a) pair_dt[3 * o + a] = hdt[(row * maxc + slot[k]) * 3 + a];
+            for (int a = 0; a < 3; ++a) pair_dt[3 * (size_t)o + a] = hdt[3 * (size_t)e + a];
+        ++o;
     }
 }
 
@@ -795,6 +997,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     if (!(p->cell > 0.0) || !(p->dt >= 0.0) || !(p->density > 0.0)) return LEDDS_EINVAL;
     if (p->model == 0 && (!(p->kn > 0.0) || !(p->kt > 0.0) || !(p->kn_w > 0.0) || !(p->kt_w > 0.0))) return LEDDS_EINVAL;
     if (!(p->restitution > 0.0) || !(p->restitution_w > 0.0) || p->mu < 0.0 || p->mu_w < 0.0) return LEDDS_EINVAL;
+    if ((unsigned long long)p->n * (unsigned long long)p->max_contacts >= (1ull << 30)) return LEDDS_EINVAL;   // scan descriptors: 30 bits
     h->p = *p;
     DemDev& d = h->d;
     d.n = p->n;
@@ -837,34 +1040,44 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     h->key_bits = bits;
     h->passes = (bits + 7) / 8;
     h->tiles = (p->n + SORT_TILE - 1) / SORT_TILE;
+    h->scan_tiles = (p->n + SCAN_TILE - 1) / SCAN_TILE;
 
-    const size_t n = (size_t)p->n;
+    const size_t n = (size_t)p->n, ecap = n * (size_t)d.maxc;
     size_t o = 0;
     DemScratch& s = h->s;
     auto take = [&](size_t bytes) { const size_t at = o; o += align_up(bytes); return at; };
-    // zeroed before every sort: histograms, tickets, tile states (kept contiguous)
+    // zeroed before every step: histograms, tickets, look-back descriptors, cell ranges (kept contiguous)
     s.hist_digit = take(4 * SORT_RADIX * 4);
-    s.tile_counter = take(4 * 4);
+    s.tile_counter = take(8 * 4);
     s.tile_state = take((size_t)4 * h->tiles * SORT_RADIX * 4);
-    // zeroed before every range build
+    s.scan_state = take(((size_t)h->scan_tiles + 1) * 4);
     s.cell_range = take((size_t)d.ncell * 8);
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
-    s.xr = take(n * 32); s.xr_s = take(n * 32); s.xf_s = take(n * 16);
-    s.ncand = take(n * 4); s.cand = take(n * d.maxc * 4);
-    s.vp = take(n * 24); s.wp = take(n * 24); s.vw_s = take(n * 48);
-    s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4);
+    s.hid = take(n * 4); s.sid = take(n * 4); s.sid_tmp = take(n * 4);
+    s.hx = take(n * 32);
+    s.hv = take(n * 24); s.hw = take(n * 24); s.ha = take(n * 24); s.hal = take(n * 24);
+    s.pvw = take(n * 48);
+    s.xr_s = take(n * 32); s.xf_s = take(n * 16);
+    s.ncand = take(n * 4); s.cand = take(ecap * 4);
+    s.off = take((n + 1) * 4);
+    s.end_s = take(ecap * 4); s.end_t = take(ecap * 4);
+    s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4); s.pos_of_id = take((n + 1) * 4);
     s.total = o;
 
     DemHistory& hs = h->hs;
     o = 0;
     for (int b = 0; b < 2; ++b) {
-        hs.ft[b] = take(n * 64);
-        hs.id[b] = take(n * d.maxc * 4);
-        hs.dt[b] = take(n * d.maxc * 24);
+        hs.fm[b] = take(n * 48);
+        hs.row[b] = take(n * 8);
+        hs.hq[b] = take(ecap * 4);
+        hs.hdt[b] = take(ecap * 24);
     }
     hs.total = o;
     h->cur = 0;
+    h->rec = 0;
     h->sorted_buf = 0;
+    h->sh_buf = 0;
+    h->have_sort = false;
     h->steps = 0;
     return LEDDS_OK;
 }
@@ -884,32 +1097,70 @@ static T* at(void* base, size_t off) { return reinterpret_cast<T*>(static_cast<c
 template <typename T>
 static const T* at(const void* base, size_t off) { return reinterpret_cast<const T*>(static_cast<const char*>(base) + off); }
 
-// drift (optional) -> keys -> sort -> gather/ranges -> contacts.  Leaves force/torque in scratch.
-int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha,
-                               const double* radius, void* history, void* scratch, int32_t* status, double dt_hist,
+// The caller's arrays in the home order of this call: the sorted order of the last sort (identity before the first).
+int ledds_dem_import(ledds_dem* h, const double* x, const double* v, const double* w, const double* a, const double* alpha,
+                     const double* radius, void* history, void* scratch, cudaStream_t st)
+{
+    const int n = h->d.n;
+    if (n == 0) return LEDDS_OK;
+    const DemScratch& s = h->s;
+    const DemHistory& hs = h->hs;
+    const int from = h->rec, to = 1 - h->rec;
+    const uint32_t* hid_src = h->have_sort ? at<uint32_t>(scratch, s.sid) : nullptr;
+    const uint32_t* perm = h->have_sort ? at<uint32_t>(scratch, s.idx[h->sh_buf]) : nullptr;
+    dem_import_kernel<<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(
+        n, hid_src, perm, x, v, w, a, alpha, radius, at<uint32_t>(scratch, s.hid), at<double4>(scratch, s.hx),
+        at<double>(scratch, s.hv), at<double>(scratch, s.hw), at<double>(scratch, s.ha), at<double>(scratch, s.hal),
+        at<double>(history, hs.fm[from]), at<uint2>(history, hs.row[from]), at<double>(history, hs.fm[to]),
+        at<uint2>(history, hs.row[to]));
+    LEDDS_CHECK_LAUNCH();
+    h->rec = to;
+    h->have_sort = false;                                      // idx[] no longer maps sorted positions to this home order
+    return LEDDS_OK;
+}
+
+int ledds_dem_export(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha, const void* scratch, cudaStream_t st)
+{
+    const int n = h->d.n;
+    if (n == 0) return LEDDS_OK;
+    const DemScratch& s = h->s;
+    dem_export_kernel<<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(
+        n, at<uint32_t>(scratch, s.hid), at<double4>(scratch, s.hx), at<double>(scratch, s.hv), at<double>(scratch, s.hw),
+        at<double>(scratch, s.ha), at<double>(scratch, s.hal), x, v, w, a, alpha);
+    LEDDS_CHECK_LAUNCH();
+    return LEDDS_OK;
+}
+
+// [kick] -> drift (optional) -> keys -> sort -> gather/ranges -> contacts, all on the home state.  Leaves the contact
+// sums of every particle in history (fm, row) and the contact ends in hq / hdt of the new generation.
+int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32_t* status, double dt_hist,
                                bool drift, cudaStream_t st, bool fork, const DemKick* kick)
 {
-    // kick != nullptr: the kick that closes the previous step (with the contact forces still in ft[cur] and the
+    // kick != nullptr: the kick that closes the previous step (with the contact sums still in fm and the
     // external force / torque of *kick) is fused into the drift kernel of this one.
     // fork = true: everything after the drift/key kernel is enqueued on the handle's side stream (ordered after
     // that kernel by an event); the caller joins by waiting on h->ev_join before it needs the contact forces.
     const DemDev& d = h->d;
     const DemScratch& s = h->s;
+    const DemHistory& hs = h->hs;
     const int n = d.n, tb = 128, nb = (n + tb - 1) / tb;
     if (n == 0) { h->cur = 1 - h->cur; return LEDDS_OK; }
-    // clear sort bookkeeping + cell ranges (one contiguous region)
+    // clear sort / scan bookkeeping + cell ranges (one contiguous region)
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
+    double* fm = at<double>(history, hs.fm[h->rec]);
+    uint2* row = at<uint2>(history, hs.row[h->rec]);
     ledds_prof_start(LEDDS_K_DEM_KEYS, st);
     {
         const dim3 grid((n + DRIFT_BLOCK - 1) / DRIFT_BLOCK);
-        const double* ft = at<double>(history, h->hs.ft[h->cur]);
         if (kick)
-            dem_drift_key_kernel<true><<<grid, DRIFT_BLOCK, 0, st>>>(d, x, v, w, a, alpha, radius, ft, kick->f_ext, kick->m_ext,
-                                                                      at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
+            dem_drift_key_kernel<true><<<grid, DRIFT_BLOCK, 0, st>>>(d, at<double4>(scratch, s.hx), at<double>(scratch, s.hv), at<double>(scratch, s.hw),
+                                                                      at<double>(scratch, s.ha), at<double>(scratch, s.hal), at<uint32_t>(scratch, s.hid), fm,
+                                                                      kick->f_ext, kick->m_ext, at<double>(scratch, s.pvw),
                                                                       at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status);
         else
-            dem_drift_key_kernel<false><<<grid, DRIFT_BLOCK, 0, st>>>(d, x, v, w, a, alpha, radius, ft, nullptr, nullptr,
-                                                                       at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double4>(scratch, s.xr),
+            dem_drift_key_kernel<false><<<grid, DRIFT_BLOCK, 0, st>>>(d, at<double4>(scratch, s.hx), at<double>(scratch, s.hv), at<double>(scratch, s.hw),
+                                                                       at<double>(scratch, s.ha), at<double>(scratch, s.hal), at<uint32_t>(scratch, s.hid), fm,
+                                                                       nullptr, nullptr, at<double>(scratch, s.pvw),
                                                                        at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status);
     }
     ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
@@ -940,32 +1191,44 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, do
     }
     ledds_prof_stop(LEDDS_K_DEM_SORT, st);
     h->sorted_buf = h->passes & 1;
+    h->sh_buf = 1 - h->sorted_buf;                             // the other idx buffer is free once the last pass is done
+    h->have_sort = true;
     const uint32_t* skey = at<uint32_t>(scratch, s.key[h->sorted_buf]);
-    const uint32_t* sidx = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
+    const uint32_t* sh0 = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
+    uint32_t* sh = at<uint32_t>(scratch, s.idx[h->sh_buf]);
+    uint32_t* sid = at<uint32_t>(scratch, s.sid);
+    uint32_t* ncand = at<uint32_t>(scratch, s.ncand);
+    uint32_t* off = at<uint32_t>(scratch, s.off);
     ledds_prof_start(LEDDS_K_DEM_GATHER, st);
-    dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr), at<double4>(scratch, s.xr_s),
-                                         at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range));
+    dem_ranges_kernel<<<nb, tb, 0, st>>>(n, skey, sh0, at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp),
+                                         at<uint2>(scratch, s.cell_range));
+    LEDDS_CHECK_LAUNCH();
+    dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sh0, at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range),
+                                         at<double4>(scratch, s.hx), at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+                                         sid, sh, ncand);
     ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
     LEDDS_CHECK_LAUNCH();
-    const DemHistory& hs = h->hs;
     const int prev = h->cur, nw = 1 - h->cur;
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
+    const int cb = (n + CONTACT_BLOCK - 1) / CONTACT_BLOCK;
     if (d.bc[0] && d.bc[1] && d.bc[2])
-        dem_detect_kernel<false><<<(n + CONTACT_BLOCK - 1) / CONTACT_BLOCK, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range),
-                                                               at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double2>(scratch, s.vw_s),
-                                                               at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
-                                                               at<double>(history, hs.ft[nw]), status);
+        dem_detect_kernel<false><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+                                                               at<uint2>(scratch, s.cell_range), ncand, at<uint32_t>(scratch, s.cand), status);
     else
-        dem_detect_kernel<true><<<(n + CONTACT_BLOCK - 1) / CONTACT_BLOCK, CONTACT_BLOCK, 0, st>>>(d, skey, sidx, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), at<uint2>(scratch, s.cell_range),
-                                                              at<double>(scratch, s.vp), at<double>(scratch, s.wp), at<double2>(scratch, s.vw_s),
-                                                              at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
-                                                              at<double>(history, hs.ft[nw]), status);
-    ledds_count_launch(1);
-    (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<(n + CONTACT_BLOCK - 1) / CONTACT_BLOCK, CONTACT_BLOCK, 0, st>>>(
-        d, sidx, at<double4>(scratch, s.xr_s), at<double2>(scratch, s.vw_s),
-        at<uint32_t>(scratch, s.ncand), at<uint32_t>(scratch, s.cand),
-        at<double>(history, hs.ft[prev]), at<uint32_t>(history, hs.id[prev]), at<double>(history, hs.dt[prev]),
-        at<double>(history, hs.ft[nw]), at<uint32_t>(history, hs.id[nw]), at<double>(history, hs.dt[nw]), status, dt_hist);
+        dem_detect_kernel<true><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+                                                              at<uint2>(scratch, s.cell_range), ncand, at<uint32_t>(scratch, s.cand), status);
+    LEDDS_CHECK_LAUNCH();
+    dem_scan_kernel<<<h->scan_tiles, SCAN_THREADS, 0, st>>>(n, (uint32_t)d.maxc, ncand, off, at<uint32_t>(scratch, s.scan_state),
+                                                            at<uint32_t>(scratch, s.tile_counter) + 4);
+    LEDDS_CHECK_LAUNCH();
+    dem_fill_kernel<<<cb, CONTACT_BLOCK, (size_t)d.maxc * CONTACT_BLOCK * sizeof(uint2), st>>>(
+        n, (uint32_t)d.maxc, ncand, at<uint32_t>(scratch, s.cand), sid, off, at<uint32_t>(scratch, s.end_s),
+        at<uint32_t>(scratch, s.end_t), at<uint32_t>(history, hs.hq[nw]));
+    LEDDS_CHECK_LAUNCH();
+    (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<(n + FORCE_PB - 1) / FORCE_PB, FORCE_THREADS, 0, st>>>(
+        d, sid, sh, at<double4>(scratch, s.xr_s), at<double>(scratch, s.pvw), off, at<uint32_t>(scratch, s.end_s),
+        at<uint32_t>(scratch, s.end_t), at<uint32_t>(history, hs.hq[nw]), row, fm, at<uint32_t>(history, hs.hq[prev]),
+        at<double>(history, hs.hdt[prev]), at<double>(history, hs.hdt[nw]), status, dt_hist);
     ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
     LEDDS_CHECK_LAUNCH();
     h->cur = nw;
@@ -973,14 +1236,16 @@ int ledds_dem_advance_contacts(ledds_dem* h, double* x, double* v, double* w, do
     return LEDDS_OK;
 }
 
-int ledds_dem_kick(ledds_dem* h, double* v, double* w, double* a, double* alpha, const double* radius,
-                   const double* f_ext, const double* m_ext, const void* history, int32_t* status, cudaStream_t st)
+int ledds_dem_kick(ledds_dem* h, const double* f_ext, const double* m_ext, const void* history, void* scratch, cudaStream_t st)
 {
-    (void)status;
     const int n = h->d.n;
     if (n == 0) return LEDDS_OK;
+    const DemScratch& s = h->s;
     ledds_prof_start(LEDDS_K_DEM_KICK, st);
-    dem_kick_kernel<<<(unsigned)((3ll * n + 255) / 256), 256, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), f_ext, m_ext, v, w, a, alpha, 0);
+    dem_kick_kernel<<<(unsigned)((3ll * n + 255) / 256), 256, 0, st>>>(h->d, at<double4>(scratch, s.hx), at<uint32_t>(scratch, s.hid),
+                                                                       at<double>(history, h->hs.fm[h->rec]), f_ext, m_ext,
+                                                                       at<double>(scratch, s.hv), at<double>(scratch, s.hw),
+                                                                       at<double>(scratch, s.ha), at<double>(scratch, s.hal), 0);
     ledds_prof_stop(LEDDS_K_DEM_KICK, st);
     LEDDS_CHECK_LAUNCH();
     return LEDDS_OK;
@@ -1005,40 +1270,58 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
         delete h;
         return LEDDS_ECUDA;
     }
-    // forces of the initial state: no drift, delta_t stays 0 (dt_hist = 0)
-    rc = ledds_dem_advance_contacts(h, const_cast<double*>(x), const_cast<double*>(v), const_cast<double*>(w), a, alpha, radius, history,
-                                    scratch, status, 0.0, false, st, false, nullptr);
+    // forces of the initial state: no drift, delta_t stays 0 (dt_hist = 0); a(0), alpha(0) back to the caller
+    rc = ledds_dem_import(h, x, v, w, nullptr, nullptr, radius, history, scratch, st);
+    if (!rc) rc = ledds_dem_advance_contacts(h, history, scratch, status, 0.0, false, st, false, nullptr);
     if (rc) { delete h; return rc; }
     if (h->d.n == 0) { *out = h; return LEDDS_OK; }
-    dem_kick_kernel<<<(unsigned)((3ll * h->d.n + 255) / 256), 256, 0, st>>>(h->d, radius, at<double>(history, h->hs.ft[h->cur]), nullptr,
-                                                                            nullptr, nullptr, nullptr, a, alpha, 1);
+    const DemScratch& s = h->s;
+    dem_kick_kernel<<<(unsigned)((3ll * h->d.n + 255) / 256), 256, 0, st>>>(h->d, at<double4>(scratch, s.hx), at<uint32_t>(scratch, s.hid),
+                                                                            at<double>(history, h->hs.fm[h->rec]), nullptr, nullptr,
+                                                                            at<double>(scratch, s.hv), at<double>(scratch, s.hw),
+                                                                            at<double>(scratch, s.ha), at<double>(scratch, s.hal), 1);
     ledds_count_launch(1);
     if (cudaPeekAtLastError() != cudaSuccess) { delete h; return LEDDS_ECUDA; }
+    rc = ledds_dem_export(h, nullptr, nullptr, nullptr, a, alpha, scratch, st);
+    if (rc) { delete h; return rc; }
     *out = h;
     return LEDDS_OK;
 }
+
+// steps between two re-homings inside one long call (the home order goes stale as particles change cells)
+#define DEM_REHOME_STEPS 256
 
 extern "C" int ledds_dem_step(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha,
                               const double* radius, const double* f_ext, const double* m_ext, void* history,
                               void* scratch, int32_t* status, int nsteps, void* stream)
 {
     if (!h || !status || nsteps < 0) return LEDDS_EINVAL;
-    if (h->d.n == 0) return LEDDS_OK;
+    if (h->d.n == 0 || nsteps == 0) return LEDDS_OK;
     if (!x || !v || !w || !a || !alpha || !radius || !history || !scratch) return LEDDS_EINVAL;
     const void* ptrs[] = {x, v, w, a, alpha, radius, f_ext, m_ext, history, scratch, status};
     for (const void* q : ptrs)
         if (!ledds_aligned16(q)) return LEDDS_EALIGN;
     cudaStream_t st = (cudaStream_t)stream;
     const DemKick kick = {f_ext, m_ext};
+    int rc = ledds_dem_import(h, x, v, w, a, alpha, radius, history, scratch, st);
+    if (rc) return rc;
     for (int s = 0; s < nsteps; ++s) {
-        // the kick of step s - 1 rides on the drift of step s; only the last step of the call kicks on its own
-        int rc = ledds_dem_advance_contacts(h, x, v, w, a, alpha, radius, history, scratch, status, h->d.dt, true, st, false,
-                                            s > 0 ? &kick : nullptr);
+        // the kick of step s - 1 rides on the drift of step s; only the last step of the call (and the one before
+        // a re-homing) kicks on its own
+        const bool rehome = s > 0 && s % DEM_REHOME_STEPS == 0;
+        if (rehome) {
+            rc = ledds_dem_kick(h, f_ext, m_ext, history, scratch, st);
+            if (!rc) rc = ledds_dem_export(h, x, v, w, a, alpha, scratch, st);
+            if (!rc) rc = ledds_dem_import(h, x, v, w, a, alpha, radius, history, scratch, st);
+            if (rc) return rc;
+        }
+        rc = ledds_dem_advance_contacts(h, history, scratch, status, h->d.dt, true, st, false, (s > 0 && !rehome) ? &kick : nullptr);
         if (rc) return rc;
         h->steps++;
     }
-    if (nsteps > 0) return ledds_dem_kick(h, v, w, a, alpha, radius, f_ext, m_ext, history, status, st);
-    return LEDDS_OK;
+    rc = ledds_dem_kick(h, f_ext, m_ext, history, scratch, st);
+    if (rc) return rc;
+    return ledds_dem_export(h, x, v, w, a, alpha, scratch, st);
 }
 
 extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* scratch, uint32_t* sorted_idx,
@@ -1054,29 +1337,31 @@ extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* sc
     }
     if (!history || !scratch) return LEDDS_EINVAL;
     const DemScratch& s = h->s;
+    const DemHistory& hs = h->hs;
     auto copy = [&](void* dst, const void* src, size_t bytes) {
         return !dst || cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st) == cudaSuccess;
     };
-    if (!copy(sorted_idx, at<char>(scratch, s.idx[h->sorted_buf]), n * 4) ||
+    if (!copy(sorted_idx, at<char>(scratch, s.sid), n * 4) ||
         !copy(sorted_key, at<char>(scratch, s.key[h->sorted_buf]), n * 4))
         return LEDDS_ECUDA;
+    const int tb = 128, nb = ((int)n + tb - 1) / tb;
     if (force || torque) {
-        dem_unpack_ft_kernel<<<((int)n + 127) / 128, 128, 0, st>>>((int)n, at<double>(history, h->hs.ft[h->cur]), force, torque);
+        dem_unpack_fm_kernel<<<nb, tb, 0, st>>>((int)n, at<uint32_t>(scratch, s.hid), at<double>(history, hs.fm[h->rec]), force, torque);
         LEDDS_CHECK_LAUNCH();
     }
     if (pairs || pair_dt || n_pairs) {
-        const DemHistory& hs = h->hs;
-        const int tb = 128, nb = ((int)n + tb - 1) / tb;
-        // scratch is logically const for the caller; the two query arrays are ours to overwrite
+        // scratch is logically const for the caller; the query arrays are ours to overwrite
         uint32_t* cnt = const_cast<uint32_t*>(at<uint32_t>(scratch, s.pair_count));
-        uint32_t* off = const_cast<uint32_t*>(at<uint32_t>(scratch, s.pair_off));
-        dem_pair_count_kernel<<<nb, tb, 0, st>>>((int)n, h->d.maxc, at<double>(history, hs.ft[h->cur]),
-                                                 at<uint32_t>(history, hs.id[h->cur]), cnt);
-        dem_scan_kernel<<<1, 1024, 0, st>>>((int)n, cnt, off);
-        dem_pair_write_kernel<<<nb, tb, 0, st>>>((int)n, h->d.maxc, at<double>(history, hs.ft[h->cur]),
-                                                 at<uint32_t>(history, hs.id[h->cur]), at<double>(history, hs.dt[h->cur]),
-                                                 off, pair_cap, pairs, pair_dt, n_pairs);
-        ledds_count_launch(2);
+        uint32_t* poff = const_cast<uint32_t*>(at<uint32_t>(scratch, s.pair_off));
+        uint32_t* pos = const_cast<uint32_t*>(at<uint32_t>(scratch, s.pos_of_id));
+        const uint32_t* off = at<uint32_t>(scratch, s.off);
+        const uint32_t* hq = at<uint32_t>(history, hs.hq[h->cur]);
+        dem_query_pos_kernel<<<nb, tb, 0, st>>>((int)n, at<uint32_t>(scratch, s.sid), pos);
+        dem_pair_count_kernel<<<nb, tb, 0, st>>>((int)n, pos, off, hq, cnt);
+        dem_block_scan_kernel<<<1, 1024, 0, st>>>((int)n, cnt, poff);
+        dem_pair_write_kernel<<<nb, tb, 0, st>>>((int)n, pos, off, hq, at<double>(history, hs.hdt[h->cur]), poff, pair_cap, pairs,
+                                                 pair_dt, n_pairs);
+        ledds_count_launch(3);
         LEDDS_CHECK_LAUNCH();
     }
     return LEDDS_OK;

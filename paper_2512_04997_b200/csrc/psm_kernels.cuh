@@ -32,7 +32,7 @@ struct CplDev {
     int subdiv;                // 0: distance-based solid fraction Eq. (39)-(40); else points per direction of Eq. (38)
     double* betabox;           // [n][S^3] solid fraction per (solid, cell of its box), subdivision method only
     uint32_t* blist;           // [0] = count, [1..]: box-cell indices k S^3 + e whose points have to be counted
-    const double* x; const double* vp; const double* wp; const double* radius;   // particle order, DEM units
+    const double4* hx; const double* pvw; const uint32_t* hid;   // DEM state in home order: (x, R), predictor (v^p, w^p), particle id
     uint2* slots;
     double* sol;
     unsigned long long* acc;
