@@ -106,6 +106,8 @@ struct DemScratch {
     size_t ncand, cand;            // contacts found per sorted position: uint32 [n], uint32 [maxc][n]
     size_t off;                    // uint32 [n + 1]: first contact end of sorted position s (CSR offsets)
     size_t end_s, end_t;           // uint32 [n maxc]: owner (sorted position) and partner (sorted position or wall code) per end
+    size_t end_hs, end_ht;         // uint32 [n maxc]: their home indices
+    size_t end_prev;               // uint32 [n maxc]: the end of last step this one continues (or none) + "owner is the first partner" bit
     size_t pair_count, pair_off, pos_of_id;   // query scratch (uint32 [n+1])
     size_t total;
 };

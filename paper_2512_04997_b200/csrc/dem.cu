@@ -478,9 +478,15 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // Tuning constants (the measured best at 4 M spheres)
 #define CONTACT_BLOCK 128       // threads per block of the detect and fill kernels
 #define DETECT_NB 3             // candidates in flight per iteration of the detect loop
-#define DETECT_MIN_BLOCKS 8     // caps the detect kernel at 64 registers (8 blocks per SM)
-#define FORCE_THREADS 256       // one thread per contact end ...
-#define FORCE_PB 512            // ... of the FORCE_PB particles of a block: ~6 full rounds of 256 ends in a dense bed
+#ifndef FORCE_THREADS
+#define FORCE_THREADS 128       // one thread per contact end ...
+#endif
+#ifndef FORCE_PB
+#define FORCE_PB 256            // ... of the FORCE_PB particles of a block: ~6 full rounds of ends in a dense bed
+#endif
+#ifndef FORCE_MIN_BLOCKS
+#define FORCE_MIN_BLOCKS 4
+#endif
 
 // Stiffness and damping of one contact.  HERTZ = false: the linear spring-dashpot of the configs, gamma =
 // 2 zeta sqrt(k m*) (G5).  HERTZ = true: Hertz-Mindlin: (A.1) k_n = 4/3 Y* sqrt(R* d_n),
@@ -539,97 +545,97 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
 }
 
 // ------------------------------------------------------------------------------ detect
-// One thread per particle in sorted order.  The 9 runs of x-adjacent neighbour cells (contiguous in the sorted order;
-// a periodic row adds its one wrapped cell) are loaded up front and clipped to the positions AFTER the particle's own:
-// every unordered pair of the neighbourhood is looked at once, from the partner that comes first in the sorted order.
+// One thread per (particle, row of neighbour cells): blockIdx.y = j selects the row (dy, dz) = (j % 3 - 1, j / 3 - 1) of
+// the 3 x 3 rows around the particle's cell; the three x-adjacent cells of a row are contiguous in the sorted order (a
+// periodic row adds its one wrapped cell).  The run is clipped to the positions AFTER the particle's own: every
+// unordered pair of the neighbourhood is looked at once, from the partner that comes first in the sorted order -- so
+// the four rows that lie before the particle's cell are dropped without a load unless a periodic wrap brought them
+// there.  Nine short, equally long pieces of work per particle instead of one long one: the lanes of a warp stay
+// together and nine times as many loads are in flight.
 // A contact is entered into both partners' lists: cand[c][s] (c < ncand[s]) = sorted positions of the particles that
 // touch the particle at sorted position s, or DEM_WALL + wall.  The order inside a list is the order of arrival (it
 // differs from run to run); dem_fill_kernel puts every list into the order of the partner ids.
 template <bool PERIODIC>
-__global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_kernel(
+__global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
     const DemDev P, const uint32_t* __restrict__ skey, const double4* __restrict__ xr_s, const float4* __restrict__ xf_s,
     const uint2* __restrict__ cell_range, uint32_t* __restrict__ ncand, uint32_t* __restrict__ cand, int32_t* __restrict__ status)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
+    const int j = blockIdx.y, dy = j % 3 - 1, dz = j / 3 - 1;
     const uint32_t maxc = (uint32_t)P.maxc;
     const uint32_t key = skey[s];
-    const double4 mine = xr_s[s];
-    const float4 minef = xf_s[s];
-    int st = 0;
-
     const int c0 = (int)(key % (uint32_t)P.nc[0]);
     const int c1 = (int)((key / (uint32_t)P.nc[0]) % (uint32_t)P.nc[1]);
     const int c2 = (int)(key / ((uint32_t)P.nc[0] * (uint32_t)P.nc[1]));
-
+    int qz = c2 + dz, qy = c1 + dy;
+    bool wrapped = false;
+    if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) return; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; wrapped = true; }
+    if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) return; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; wrapped = true; }
+    if (!wrapped && (dz < 0 || (dz == 0 && dy < 0))) return;          // the whole row comes before s in the sorted order
+    int st = 0;
     auto enter = [&](uint32_t owner, uint32_t partner) {
         const uint32_t c = atomicAdd(ncand + owner, 1u);
         if (c < maxc) cand[(size_t)c * P.n + owner] = partner;
         else st |= LEDDS_ST_CONTACT_OVERFLOW;
     };
-    // the 9 runs [t0, t1) of x-adjacent cells (c0-1 .. c0+1 inside the row): all 27 range loads are independent
-    // and issued together; an empty cell holds (0, 0), so "first start, last end" needs no special case
-    uint32_t t0[9], t1[9];
+    // the run [t0, t1) of the cells c0-1 .. c0+1 of the row: an empty cell holds (0, 0), so "first start, last end"
+    // needs no special case
+    const uint2* row = cell_range + (size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + c0;
+    const uint2 none = make_uint2(0u, 0u);
+    const uint2 r1 = row[0], r0 = c0 > 0 ? row[-1] : none, r2 = c0 < P.nc[0] - 1 ? row[1] : none;
+    uint2 rw = none;                                                                // the wrapped cell of a periodic row
+    if (PERIODIC && !P.bc[0] && (c0 == 0 || c0 == P.nc[0] - 1)) rw = row[c0 == 0 ? P.nc[0] - 1 : -c0];
+    const float4 minef = xf_s[s];
+    const bool e0 = r0.y > r0.x, e1 = r1.y > r1.x, e2 = r2.y > r2.x;
+    const uint32_t t0 = max(e0 ? r0.x : (e1 ? r1.x : r2.x), (uint32_t)s + 1u);      // only the positions after mine
+    const uint32_t t1 = e2 ? r2.y : (e1 ? r1.y : r0.y);
+    const double4 mine = xr_s[s];
+    for (uint32_t t = t0; t < t1; t += DETECT_NB) {                                // DETECT_NB candidates in flight
+        uint32_t tt[DETECT_NB];
+        float4 fc[DETECT_NB];
+        bool nn[DETECT_NB], any = false;
 #pragma unroll
-    for (int j = 0; j < 9; ++j) {
-        int qz = c2 + (j / 3 - 1), qy = c1 + (j % 3 - 1);
-        bool ok = true;
-        if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) ok = false; else qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
-        if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) ok = false; else qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
-        const uint2 none = make_uint2(0u, 0u);
-        uint2 r0 = none, r1 = none, r2 = none;
-        if (ok) {
-            const uint2* row = cell_range + (size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + c0;
-            r1 = row[0];
-            if (c0 > 0) r0 = row[-1];
-            if (c0 < P.nc[0] - 1) r2 = row[1];
+        for (int b = 0; b < DETECT_NB; ++b) {
+            tt[b] = min(t + (uint32_t)b, t1 - 1u);                                 // past the end: the last candidate again
+            fc[b] = xf_s[tt[b]];                                                   // first look in single precision (no branch),
         }
-        const bool e0 = r0.y > r0.x, e1 = r1.y > r1.x, e2 = r2.y > r2.x;
-        t0[j] = max(e0 ? r0.x : (e1 ? r1.x : r2.x), (uint32_t)s + 1u);               // only the positions after mine
-        t1[j] = e2 ? r2.y : (e1 ? r1.y : r0.y);
-    }
 #pragma unroll
-    for (int j = 0; j < 9; ++j) {
-        for (uint32_t t = t0[j]; t < t1[j]; t += DETECT_NB) {                      // DETECT_NB candidates in flight
-            uint32_t tt[DETECT_NB];
-            float4 fc[DETECT_NB];
-            bool nn[DETECT_NB], any = false;
+        for (int b = 0; b < DETECT_NB; ++b) {
+            nn[b] = dem_near<PERIODIC>(P, minef, fc[b]) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
+            any |= nn[b];
+        }
+        if (any) {                                                                 // Eq. (2) in double for the few that pass
 #pragma unroll
-            for (int b = 0; b < DETECT_NB; ++b) {
-                tt[b] = min(t + (uint32_t)b, t1[j] - 1u);                          // past the end: the last candidate again
-                fc[b] = xf_s[tt[b]];                                               // first look in single precision (no branch),
-            }
-#pragma unroll
-            for (int b = 0; b < DETECT_NB; ++b) {
-                nn[b] = dem_near<PERIODIC>(P, minef, fc[b]) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
-                any |= nn[b];
-            }
-            if (any) {                                                             // Eq. (2) in double for the few that pass
-#pragma unroll
-                for (int b = 0; b < DETECT_NB; ++b)
-                    if (nn[b] && dem_touch<PERIODIC>(P, mine, xr_s[tt[b]])) { enter((uint32_t)s, tt[b]); enter(tt[b], (uint32_t)s); }
-            }
+            for (int b = 0; b < DETECT_NB; ++b)
+                if (nn[b] && dem_touch<PERIODIC>(P, mine, xr_s[tt[b]])) { enter((uint32_t)s, tt[b]); enter(tt[b], (uint32_t)s); }
         }
     }
-    if (PERIODIC && !P.bc[0] && (c0 == 0 || c0 == P.nc[0] - 1)) {                  // the wrapped cell of a periodic row
-        const int wc = c0 == 0 ? P.nc[0] - 1 : 0;
-        for (int j = 0; j < 9; ++j) {
-            int qz = c2 + (j / 3 - 1), qy = c1 + (j % 3 - 1);
-            if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) continue; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
-            if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) continue; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
-            const uint2 r = cell_range[(size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + wc];
-            for (uint32_t t = max(r.x, (uint32_t)s + 1u); t < r.y; ++t)
-                if (dem_near<PERIODIC>(P, minef, xf_s[t]) && dem_touch<PERIODIC>(P, mine, xr_s[t])) { enter((uint32_t)s, t); enter(t, (uint32_t)s); }
-        }
+    if (PERIODIC) {
+        for (uint32_t t = max(rw.x, (uint32_t)s + 1u); t < rw.y; ++t)
+            if (dem_near<PERIODIC>(P, minef, xf_s[t])) {
+                    if (dem_touch<PERIODIC>(P, mine, xr_s[t])) { enter((uint32_t)s, t); enter(t, (uint32_t)s); }
+            }
     }
-    // walls: static infinite particles; overlap decided as the oracle does, R - distance > 0
-    const double xm[3] = {mine.x, mine.y, mine.z};
+    if (j == 4) {
+        // walls: static infinite particles; overlap decided as the oracle does, R - distance > 0.
+        // The single-precision record tells which particles can reach a wall at all.
+        bool maybe = !(minef.w == minef.w);                                        // a NaN record: look
 #pragma unroll
-    for (int wl = 0; wl < 6; ++wl) {
-        const int ax = wl >> 1;
-        if (!P.bc[ax]) continue;
-        const double dist = (wl & 1) ? P.hi[ax] - xm[ax] : xm[ax] - P.lo[ax];
-        if (mine.w - dist > 0.0) enter((uint32_t)s, DEM_WALL + (uint32_t)wl);
+        for (int a = 0; a < 3; ++a) {
+            const float xa = a == 0 ? minef.x : (a == 1 ? minef.y : minef.z);
+            if (P.bc[a] && (xa < minef.w + P.fmargin || P.Lf[a] - xa < minef.w + P.fmargin)) maybe = true;
+        }
+        if (maybe) {
+            const double xm[3] = {mine.x, mine.y, mine.z};
+#pragma unroll
+            for (int wl = 0; wl < 6; ++wl) {
+                const int ax = wl >> 1;
+                if (!P.bc[ax]) continue;
+                const double dist = (wl & 1) ? P.hi[ax] - xm[ax] : xm[ax] - P.lo[ax];
+                if (mine.w - dist > 0.0) enter((uint32_t)s, DEM_WALL + (uint32_t)wl);
+            }
+        }
     }
     if (st) atomicOr(status, st);
 }
@@ -668,23 +674,30 @@ __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t 
         if (w2 < warp) before += wsum[w2];
         total += wsum[w2];
     }
-    if (tid == 0) {
+    if (warp == 0) {                                                                // look back 32 predecessors at a time
         uint32_t excl = 0;
         if (tile == 0) {
-            st_volatile(state, ST_FLAG_PRE | total);
+            if (lane == 0) st_volatile(state, ST_FLAG_PRE | total);
         } else {
-            st_volatile(state + tile, ST_FLAG_AGG | total);
+            if (lane == 0) st_volatile(state + tile, ST_FLAG_AGG | total);
             long long t = (long long)tile - 1;
             for (;;) {
-                uint32_t sb = ld_volatile(state + t);
-                while ((sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0) sb = ld_volatile(state + t);
-                excl += sb & ST_VALUE_MASK;
-                if (sb & ST_FLAG_PRE) break;
-                --t;
+                const long long i = t - lane;
+                uint32_t sb = i >= 0 ? ld_volatile(state + i) : ST_FLAG_PRE;
+                while (__any_sync(0xffffffffu, (sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0))
+                    if ((sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0) sb = ld_volatile(state + i);
+                const unsigned pre = __ballot_sync(0xffffffffu, (sb & ST_FLAG_PRE) != 0);
+                const int last = pre ? __ffs(pre) - 1 : 31;                         // the nearest predecessor with a full prefix
+                uint32_t v = lane <= last ? (sb & ST_VALUE_MASK) : 0u;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                excl += v;
+                if (pre) break;
+                t -= 32;
             }
-            st_volatile(state + tile, ST_FLAG_PRE | (excl + total));
+            if (lane == 0) st_volatile(state + tile, ST_FLAG_PRE | (excl + total));
         }
-        s_excl = excl;
+        if (lane == 0) s_excl = excl;
     }
     __syncthreads();
     uint32_t run = s_excl + before + incl - sum;
@@ -698,18 +711,38 @@ __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t 
 
 // ------------------------------------------------------------------------------ fill
 // One thread per particle: its list of partners, put into ascending order of the partner id (walls, id n + wall, last):
-// the order of the paper's lexicographically sorted pair list, which is also the order the oracle sums in.
-// end_s / end_t / hq are the CSR arrays of contact ends the force kernel works through.
+// the order of the paper's lexicographically sorted pair list, which is also the order the oracle sums
+// in.  Last step's list of the particle is in the same order, so one merge finds for every end the end it continues
+// (PAPER.md:496 searches the previous sorted pair list instead).  Everything the force kernel needs to start an end comes
+// out as coalesced records: owner and partner (sorted position: the packed (x, R) records; home index: the predictor
+// velocities), where the previous delta_t is, and whether the owner is the contact's first partner (i < j).
+// The particle's row descriptor is renewed here; a particle that has just lost its last contact gets its sums zeroed.
+#define DEM_NO_PREV 0x7fffffffu
+#define DEM_ME_FIRST 0x80000000u
+struct DemEnds { uint32_t *s, *t, *hs, *ht, *prev; };   // per contact end, CSR order
+
 __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ ncand,
                                                                 const uint32_t* __restrict__ cand, const uint32_t* __restrict__ sid,
-                                                                const uint32_t* __restrict__ off, uint32_t* __restrict__ end_s,
-                                                                uint32_t* __restrict__ end_t, uint32_t* __restrict__ hq)
+                                                                const uint32_t* __restrict__ sh, const uint32_t* __restrict__ off,
+                                                                uint2* __restrict__ row, double* __restrict__ fm,
+                                                                const uint32_t* __restrict__ hq_prev, const DemEnds E,
+                                                                uint32_t* __restrict__ hq)
 {
     extern __shared__ uint2 tq[];                                                   // [maxc][CONTACT_BLOCK]: (partner code, partner id)
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
     const uint32_t cnt = min(ncand[s], maxc);
-    if (cnt == 0) return;
+    const uint32_t h = sh[s];
+    const uint2 old = row[h];
+    if (cnt == 0) {
+        if (old.y) {                                                                // the last contact has just ended
+            row[h] = make_uint2(0u, 0u);
+#pragma unroll
+            for (int c = 0; c < 6; ++c) fm[6 * (size_t)h + c] = 0.0;
+        }
+        return;
+    }
+    const uint32_t p = sid[s];
     uint2* mine = tq + threadIdx.x;
     for (uint32_t c = 0; c < cnt; ++c) {
         const uint32_t t = cand[(size_t)c * n + s];
@@ -719,12 +752,19 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
         mine[k * CONTACT_BLOCK] = make_uint2(t, q);
     }
     const uint32_t o = off[s];
+    uint32_t k = 0, qk = old.y ? hq_prev[old.x] : 0xffffffffu;
     for (uint32_t c = 0; c < cnt; ++c) {
         const uint2 e = mine[c * CONTACT_BLOCK];
-        end_s[o + c] = (uint32_t)s;
-        end_t[o + c] = e.x;
+        while (qk < e.y) { ++k; qk = k < old.y ? hq_prev[old.x + k] : 0xffffffffu; }
+        const uint32_t prev = qk == e.y ? old.x + k : DEM_NO_PREV;
+        E.s[o + c] = (uint32_t)s;
+        E.t[o + c] = e.x;
+        E.hs[o + c] = h;
+        E.ht[o + c] = e.x >= DEM_WALL ? 0u : sh[e.x];
+        E.prev[o + c] = prev | (p < e.y ? DEM_ME_FIRST : 0u);
         hq[o + c] = e.y;
     }
+    row[h] = make_uint2(o, cnt);
 }
 
 // ------------------------------------------------------------------------------ force
@@ -732,20 +772,19 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
 // [off[s0], off[s0 + FORCE_PB]) of the CSR arrays.  It works through that piece FORCE_THREADS ends at a time, one end per
 // thread (all lanes busy whatever the contact counts of the particles are): both partners evaluate a contact in its
 // canonical orientation (i < j), so F_ij = -F_ji bit for bit; the end's force and torque go to shared memory, and the
-// thread that owns the particle adds up its ends in list order.  History: the previous delta_t of the end is looked up
-// in the particle's own row of last step's CSR arrays (row = (first, count), kept per particle in home order).
+// thread that owns the particle adds up its ends in list order.  An end starts from the records dem_fill_kernel left:
+// one coalesced read, then every further load (both bodies, the previous delta_t) is independent of the others.
 template <bool HERTZ>
-__global__ void __launch_bounds__(FORCE_THREADS) dem_force_kernel(
-    const DemDev P, const uint32_t* __restrict__ sid, const uint32_t* __restrict__ sh, const double4* __restrict__ xr_s,
-    const double* __restrict__ pvw, const uint32_t* __restrict__ off, const uint32_t* __restrict__ end_s,
-    const uint32_t* __restrict__ end_t, const uint32_t* __restrict__ hq_new, uint2* __restrict__ row,
-    double* __restrict__ fm, const uint32_t* __restrict__ hq_prev, const double* __restrict__ hdt_prev,
+__global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_kernel(
+    const DemDev P, const double4* __restrict__ xr_s, const double* __restrict__ pvw, const uint32_t* __restrict__ off,
+    const DemEnds E, const uint32_t* __restrict__ sh, double* __restrict__ fm, const double* __restrict__ hdt_prev,
     double* __restrict__ hdt_new, int32_t* __restrict__ status, double dt_hist)
 {
     __shared__ uint32_t s_off[FORCE_PB + 1];
     __shared__ double stage[6][FORCE_THREADS];
     const int tid = threadIdx.x;
     const int s0 = blockIdx.x * FORCE_PB, np = min(FORCE_PB, P.n - s0);
+    if (off[s0] == off[s0 + np]) return;                                            // no contact in this block (block-uniform)
     for (int i = tid; i <= np; i += FORCE_THREADS) s_off[i] = off[s0 + i];
     __syncthreads();
     const uint32_t e_begin = s_off[0], e_end = s_off[np];
@@ -761,38 +800,28 @@ __global__ void __launch_bounds__(FORCE_THREADS) dem_force_kernel(
         const uint32_t e = chunk + (uint32_t)tid;
         double Fe[3] = {0, 0, 0}, Me[3] = {0, 0, 0};
         if (e < e_end) {
-            const uint32_t s = end_s[e], t = end_t[e], q = hq_new[e];
-            const uint32_t p = sid[s], h = sh[s];
+            const uint32_t s = E.s[e], t = E.t[e], hs = E.hs[e], ht = E.ht[e], pf = E.prev[e];
+            const bool wall = t >= DEM_WALL;
+            const uint32_t prev = pf & DEM_NO_PREV;
+            // all loads of the end, issued together
             const double4 m4 = xr_s[s];
+            const double2* rm = reinterpret_cast<const double2*>(pvw + 6 * (size_t)hs);
+            const double2 ma = rm[0], mb = rm[1], mc = rm[2];
+            const double4 o4 = xr_s[wall ? s : t];
+            const double2* ro = reinterpret_cast<const double2*>(pvw + 6 * (size_t)(wall ? hs : ht));
+            const double2 oa = ro[0], ob = ro[1], oc = ro[2];
+            double dt3[3] = {0, 0, 0};                                                 // previous delta_t of this end, as its owner stored it
+            if (prev != DEM_NO_PREV) {
+                const double* d = hdt_prev + 3 * (size_t)prev;
+                dt3[0] = d[0]; dt3[1] = d[1]; dt3[2] = d[2];
+            }
             const double xm[3] = {m4.x, m4.y, m4.z}, Rm = m4.w;
-            double vm[3], wm[3];
-            {
-                const double2* r = reinterpret_cast<const double2*>(pvw + 6 * (size_t)h);
-                const double2 a = r[0], b = r[1], c = r[2];
-                vm[0] = a.x; vm[1] = a.y; vm[2] = b.x; wm[0] = b.y; wm[1] = c.x; wm[2] = c.y;
-            }
-            // previous delta_t of this end, as its owner stored it
-            double dt3[3] = {0, 0, 0};
-            {
-                const uint2 pr = row[h];
-                for (uint32_t k = 0; k < pr.y; ++k)
-                    if (hq_prev[pr.x + k] == q) {
-                        const double* d = hdt_prev + 3 * (size_t)(pr.x + k);
-                        dt3[0] = d[0]; dt3[1] = d[1]; dt3[2] = d[2];
-                        break;
-                    }
-            }
+            const double vm[3] = {ma.x, ma.y, mb.x}, wm[3] = {mb.y, mc.x, mc.y};
             double F[3], T[3], kn, kt, gn, gt;
-            if (t < DEM_WALL) {
-                const double4 o4 = xr_s[t];
+            if (!wall) {
                 const double xo[3] = {o4.x, o4.y, o4.z}, Ro = o4.w;
-                double vo[3], wo[3];
-                {
-                    const double2* r = reinterpret_cast<const double2*>(pvw + 6 * (size_t)sh[t]);
-                    const double2 a = r[0], b = r[1], c = r[2];
-                    vo[0] = a.x; vo[1] = a.y; vo[2] = b.x; wo[0] = b.y; wo[1] = c.x; wo[2] = c.y;
-                }
-                const bool me_first = p < q;                                           // canonical orientation i < j
+                const double vo[3] = {oa.x, oa.y, ob.x}, wo[3] = {ob.y, oc.x, oc.y};
+                const bool me_first = (pf & DEM_ME_FIRST) != 0;                        // canonical orientation i < j
                 const double sg = me_first ? 1.0 : -1.0;
                 double xi[3], xj[3], vi[3], vj[3], wi[3], wj[3];
 #pragma unroll
@@ -851,16 +880,12 @@ __global__ void __launch_bounds__(FORCE_THREADS) dem_force_kernel(
         }
         __syncthreads();
     }
-    // the particle's record for the kick and for the next step's history look-up (home order)
+    // the sums of every particle that has a contact, for the kick (home order)
 #pragma unroll
     for (int j = 0; j < OWN; ++j) {
         const int i = tid + j * FORCE_THREADS;
-        if (i >= np) continue;
+        if (i >= np || s_off[i + 1] == s_off[i]) continue;
         const uint32_t h = sh[s0 + i];
-        const uint32_t cnt = s_off[i + 1] - s_off[i];
-        const uint2 old = row[h];
-        if (cnt == 0 && old.y == 0) continue;                  // no contact now, none before: the record is zero already
-        row[h] = make_uint2(s_off[i], cnt);
         bool finite = true;
 #pragma unroll
         for (int c = 0; c < 6; ++c) { fm[6 * (size_t)h + c] = acc[j][c]; finite = finite && isfinite(acc[j][c]); }
@@ -1060,7 +1085,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     s.xr_s = take(n * 32); s.xf_s = take(n * 16);
     s.ncand = take(n * 4); s.cand = take(ecap * 4);
     s.off = take((n + 1) * 4);
-    s.end_s = take(ecap * 4); s.end_t = take(ecap * 4);
+    s.end_s = take(ecap * 4); s.end_t = take(ecap * 4); s.end_hs = take(ecap * 4); s.end_ht = take(ecap * 4); s.end_prev = take(ecap * 4);
     s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4); s.pos_of_id = take((n + 1) * 4);
     s.total = o;
 
@@ -1212,23 +1237,24 @@ int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
     const int cb = (n + CONTACT_BLOCK - 1) / CONTACT_BLOCK;
     if (d.bc[0] && d.bc[1] && d.bc[2])
-        dem_detect_kernel<false><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
-                                                               at<uint2>(scratch, s.cell_range), ncand, at<uint32_t>(scratch, s.cand), status);
+        dem_detect_kernel<false><<<dim3(cb, 9), CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+                                                                        at<uint2>(scratch, s.cell_range), ncand, at<uint32_t>(scratch, s.cand), status);
     else
-        dem_detect_kernel<true><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
-                                                              at<uint2>(scratch, s.cell_range), ncand, at<uint32_t>(scratch, s.cand), status);
+        dem_detect_kernel<true><<<dim3(cb, 9), CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+                                                                       at<uint2>(scratch, s.cell_range), ncand, at<uint32_t>(scratch, s.cand), status);
     LEDDS_CHECK_LAUNCH();
     dem_scan_kernel<<<h->scan_tiles, SCAN_THREADS, 0, st>>>(n, (uint32_t)d.maxc, ncand, off, at<uint32_t>(scratch, s.scan_state),
                                                             at<uint32_t>(scratch, s.tile_counter) + 4);
     LEDDS_CHECK_LAUNCH();
+    const DemEnds E = {at<uint32_t>(scratch, s.end_s), at<uint32_t>(scratch, s.end_t), at<uint32_t>(scratch, s.end_hs),
+                       at<uint32_t>(scratch, s.end_ht), at<uint32_t>(scratch, s.end_prev)};
     dem_fill_kernel<<<cb, CONTACT_BLOCK, (size_t)d.maxc * CONTACT_BLOCK * sizeof(uint2), st>>>(
-        n, (uint32_t)d.maxc, ncand, at<uint32_t>(scratch, s.cand), sid, off, at<uint32_t>(scratch, s.end_s),
-        at<uint32_t>(scratch, s.end_t), at<uint32_t>(history, hs.hq[nw]));
+        n, (uint32_t)d.maxc, ncand, at<uint32_t>(scratch, s.cand), sid, sh, off, row, fm, at<uint32_t>(history, hs.hq[prev]), E,
+        at<uint32_t>(history, hs.hq[nw]));
     LEDDS_CHECK_LAUNCH();
     (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<(n + FORCE_PB - 1) / FORCE_PB, FORCE_THREADS, 0, st>>>(
-        d, sid, sh, at<double4>(scratch, s.xr_s), at<double>(scratch, s.pvw), off, at<uint32_t>(scratch, s.end_s),
-        at<uint32_t>(scratch, s.end_t), at<uint32_t>(history, hs.hq[nw]), row, fm, at<uint32_t>(history, hs.hq[prev]),
-        at<double>(history, hs.hdt[prev]), at<double>(history, hs.hdt[nw]), status, dt_hist);
+        d, at<double4>(scratch, s.xr_s), at<double>(scratch, s.pvw), off, E, sh, fm, at<double>(history, hs.hdt[prev]),
+        at<double>(history, hs.hdt[nw]), status, dt_hist);
     ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
     LEDDS_CHECK_LAUNCH();
     h->cur = nw;
