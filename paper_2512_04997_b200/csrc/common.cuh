@@ -74,7 +74,9 @@ struct DemDev {
     double vw[18];
     int nc[3];
     double inv_h[3];
-    unsigned ncell;
+    unsigned ncell, plane;         // cells in the grid, in one z-plane
+    unsigned long long magic_row, magic_plane;   // ceil(2^40 / nc[0]), ceil(2^40 / plane): key decode without divisions
+    int magic_ok;
     double hmin;                   // smallest cell width of the grid: 2 R must not exceed it (LEDDS_ST_RADIUS_RANGE)
     double dt, g[3], density;
     double kn, kt, zeta, mu;
@@ -103,11 +105,12 @@ struct DemScratch {
     size_t pvw;                    // double [n][6]: predictor (v^p, w^p), home order
     size_t xr_s;                   // double4 [n]: (x, y, z, R), sorted order
     size_t xf_s;                   // float4 [n]: (x - lo, R) in single precision, sorted order (first look only)
-    size_t ncand, cand;            // contacts found per sorted position: uint32 [n], uint32 [maxc][n]
+    size_t nfwd, nback;            // uint32 [n]: partners a particle found itself / partners that found it (sorted position)
+    size_t cand;                   // uint32 [maxc][n]: column s = its partners, found-by-itself from the top, found-by-others from the bottom
     size_t off;                    // uint32 [n + 1]: first contact end of sorted position s (CSR offsets)
     size_t end_s, end_t;           // uint32 [n maxc]: owner (sorted position) and partner (sorted position or wall code) per end
     size_t end_hs, end_ht;         // uint32 [n maxc]: their home indices
-    size_t end_prev;               // uint32 [n maxc]: the end of last step this one continues (or none) + "owner is the first partner" bit
+    size_t end_prev;               // uint32 [n maxc]: the end of last step this one continues (or none)
     size_t pair_count, pair_off, pos_of_id;   // query scratch (uint32 [n+1])
     size_t total;
 };

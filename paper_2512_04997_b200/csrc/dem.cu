@@ -186,6 +186,26 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
     if (st) atomicOr(status, st);
 }
 
+// key -> (cx, cy, cz).  The two divisions by run-time constants are multiplications by host-computed reciprocals:
+// floor(k m / 2^40) with m = ceil(2^40 / d) equals floor(k / d) whenever k d <= 2^40 (the host checks it for the
+// largest key and both divisors; else the plain divisions are used).
+__device__ __forceinline__ void dem_cell_of_key(const DemDev& P, uint32_t key, int& c0, int& c1, int& c2)
+{
+    uint32_t r, z;
+    if (P.magic_ok) {
+        z = (uint32_t)(((unsigned long long)key * P.magic_plane) >> 40);
+        const uint32_t rem = key - z * P.plane;
+        r = (uint32_t)(((unsigned long long)rem * P.magic_row) >> 40);
+        c0 = (int)(rem - r * (uint32_t)P.nc[0]);
+    } else {
+        z = key / P.plane;
+        const uint32_t rem = key - z * P.plane;
+        r = rem / (uint32_t)P.nc[0];
+        c0 = (int)(rem - r * (uint32_t)P.nc[0]);
+    }
+    c1 = (int)r; c2 = (int)z;
+}
+
 // ------------------------------------------------------------------------------ radix sort
 // All digit histograms in one pass over the keys (smem atomics, then one global add per bin).  The keys arrive in
 // home order, i.e. nearly sorted: the upper digits of a warp's 32 keys are usually all the same, and one lane then
@@ -197,20 +217,31 @@ __global__ void __launch_bounds__(SORT_THREADS) dem_hist_kernel(const uint32_t* 
     for (int t = threadIdx.x; t < 4 * SORT_RADIX; t += blockDim.x) (&h[0][0])[t] = 0;
     __syncthreads();
     const int lane = threadIdx.x & 31;
-    const int per = ((n + 31) / 32 + gridDim.x - 1) / gridDim.x * 32;             // a contiguous, warp-aligned piece per block
+    const int per = ((n + 127) / 128 + gridDim.x - 1) / gridDim.x * 128;          // a contiguous piece per block, 4 keys per lane and round
     const int beg = blockIdx.x * per, end = min(n, beg + per);
-    for (int base = beg + (threadIdx.x & ~31); base < end; base += blockDim.x) {
-        const int i = base + lane;
-        const bool ok = i < end;
-        const uint32_t k = ok ? key[i] : 0u;
-        const unsigned live = __ballot_sync(0xffffffffu, ok);
-        for (int p = 0; p < passes; ++p) {
-            const uint32_t d = (k >> (8 * p)) & 255u;
-            const uint32_t d0 = __shfl_sync(0xffffffffu, d, __ffs(live) - 1);
-            if (__all_sync(0xffffffffu, !ok || d == d0)) {
-                if (lane == 0) atomicAdd(&h[p][d0], (uint32_t)__popc(live));
-            } else if (ok) {
-                atomicAdd(&h[p][d], 1u);
+    for (int base = beg + (threadIdx.x & ~31) * 4; base < end; base += blockDim.x * 4) {
+        uint32_t k4[4];
+        bool ok4[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {                                             // four independent loads in flight
+            const int i = base + j * 32 + lane;
+            ok4[j] = i < end;
+            k4[j] = ok4[j] ? key[i] : 0u;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const bool ok = ok4[j];
+            const uint32_t k = k4[j];
+            const unsigned live = __ballot_sync(0xffffffffu, ok);
+            if (!live) continue;
+            for (int p = 0; p < passes; ++p) {
+                const uint32_t d = (k >> (8 * p)) & 255u;
+                const uint32_t d0 = __shfl_sync(0xffffffffu, d, __ffs(live) - 1);
+                if (__all_sync(0xffffffffu, !ok || d == d0)) {
+                    if (lane == 0) atomicAdd(&h[p][d0], (uint32_t)__popc(live));
+                } else if (ok) {
+                    atomicAdd(&h[p][d], 1u);
+                }
             }
         }
     }
@@ -397,7 +428,7 @@ __global__ void dem_ranges_kernel(int n, const uint32_t* __restrict__ skey, cons
 __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sh0,
                                   const uint32_t* __restrict__ sid_tmp, const uint2* __restrict__ cell_range,
                                   const double4* __restrict__ hx, double4* __restrict__ xr_s, float4* __restrict__ xf_s,
-                                  uint32_t* __restrict__ sid, uint32_t* __restrict__ sh, uint32_t* __restrict__ ncand)
+                                  uint32_t* __restrict__ sid, uint32_t* __restrict__ sh, uint32_t* __restrict__ nback)
 {
     const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
     if (s0 >= P.n) return;
@@ -411,7 +442,7 @@ __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ s
     xr_s[s] = make_double4(a.x, a.y, b.x, b.y);
     sid[s] = id;
     sh[s] = h;
-    ncand[s] = 0u;
+    nback[s] = 0u;
     // single-precision copy (x - lo, R) for the detect kernel's first look at a candidate (dem_near).  A particle
     // further than 2 L from the box corner (or not finite) gets NaN: it passes every first look.
     const double rx = a.x - P.lo[0], ry = a.y - P.lo[1], rz = b.x - P.lo[2];
@@ -478,14 +509,15 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // Tuning constants (the measured best at 4 M spheres)
 #define CONTACT_BLOCK 128       // threads per block of the detect and fill kernels
 #define DETECT_NB 3             // candidates in flight per iteration of the detect loop
-#ifndef FORCE_THREADS
+#define DETECT_MIN_BLOCKS 8     // caps the detect kernel at 64 registers (8 blocks per SM)
 #define FORCE_THREADS 128       // one thread per contact end ...
+#define FORCE_WARPS (FORCE_THREADS / 32)
+#ifndef FORCE_PW
+#define FORCE_PW 64             // ... of the FORCE_PW particles of a warp: ~7 rounds of 32 ends in a dense bed
 #endif
-#ifndef FORCE_PB
-#define FORCE_PB 256            // ... of the FORCE_PB particles of a block: ~6 full rounds of ends in a dense bed
-#endif
+#define FORCE_PB (FORCE_WARPS * FORCE_PW)
 #ifndef FORCE_MIN_BLOCKS
-#define FORCE_MIN_BLOCKS 4
+#define FORCE_MIN_BLOCKS 6
 #endif
 
 // Stiffness and damping of one contact.  HERTZ = false: the linear spring-dashpot of the configs, gamma =
@@ -545,107 +577,128 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
 }
 
 // ------------------------------------------------------------------------------ detect
-// One thread per (particle, row of neighbour cells): blockIdx.y = j selects the row (dy, dz) = (j % 3 - 1, j / 3 - 1) of
-// the 3 x 3 rows around the particle's cell; the three x-adjacent cells of a row are contiguous in the sorted order (a
-// periodic row adds its one wrapped cell).  The run is clipped to the positions AFTER the particle's own: every
-// unordered pair of the neighbourhood is looked at once, from the partner that comes first in the sorted order -- so
-// the four rows that lie before the particle's cell are dropped without a load unless a periodic wrap brought them
-// there.  Nine short, equally long pieces of work per particle instead of one long one: the lanes of a warp stay
-// together and nine times as many loads are in flight.
-// A contact is entered into both partners' lists: cand[c][s] (c < ncand[s]) = sorted positions of the particles that
-// touch the particle at sorted position s, or DEM_WALL + wall.  The order inside a list is the order of arrival (it
-// differs from run to run); dem_fill_kernel puts every list into the order of the partner ids.
+// One thread per particle in sorted order.  The 9 runs of x-adjacent neighbour cells (contiguous in the sorted order;
+// a periodic row adds its one wrapped cell) are loaded up front and clipped to the positions AFTER the particle's own:
+// every unordered pair of the neighbourhood is looked at once, from the partner that comes first in the sorted order.
+// A contact is entered into both partners' lists: column s of cand[maxc][n] holds, from the top, the partners found by
+// the particle itself (sorted positions > s, and DEM_WALL + wall) and, from the bottom, those that found it (arrival order,
+// which differs from run to run); dem_fill_kernel puts every list into the order of the partner ids.
+// (One thread per (particle, row) -- nine times the threads, a ninth of the work each -- was measured and is slower:
+// 0.61 against 0.52 ms in the dense 4 M state, 0.29 against 0.15 ms in the dilute one.)
 template <bool PERIODIC>
-__global__ void __launch_bounds__(CONTACT_BLOCK) dem_detect_kernel(
+__global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_kernel(
     const DemDev P, const uint32_t* __restrict__ skey, const double4* __restrict__ xr_s, const float4* __restrict__ xf_s,
-    const uint2* __restrict__ cell_range, uint32_t* __restrict__ ncand, uint32_t* __restrict__ cand, int32_t* __restrict__ status)
+    const uint2* __restrict__ cell_range, uint32_t* __restrict__ nfwd, uint32_t* __restrict__ nback, uint32_t* __restrict__ cand,
+    int32_t* __restrict__ status)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
-    const int j = blockIdx.y, dy = j % 3 - 1, dz = j / 3 - 1;
     const uint32_t maxc = (uint32_t)P.maxc;
     const uint32_t key = skey[s];
-    const int c0 = (int)(key % (uint32_t)P.nc[0]);
-    const int c1 = (int)((key / (uint32_t)P.nc[0]) % (uint32_t)P.nc[1]);
-    const int c2 = (int)(key / ((uint32_t)P.nc[0] * (uint32_t)P.nc[1]));
-    int qz = c2 + dz, qy = c1 + dy;
-    bool wrapped = false;
-    if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) return; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; wrapped = true; }
-    if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) return; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; wrapped = true; }
-    if (!wrapped && (dz < 0 || (dz == 0 && dy < 0))) return;          // the whole row comes before s in the sorted order
-    int st = 0;
-    auto enter = [&](uint32_t owner, uint32_t partner) {
-        const uint32_t c = atomicAdd(ncand + owner, 1u);
-        if (c < maxc) cand[(size_t)c * P.n + owner] = partner;
-        else st |= LEDDS_ST_CONTACT_OVERFLOW;
-    };
-    // the run [t0, t1) of the cells c0-1 .. c0+1 of the row: an empty cell holds (0, 0), so "first start, last end"
-    // needs no special case
-    const uint2* row = cell_range + (size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + c0;
-    const uint2 none = make_uint2(0u, 0u);
-    const uint2 r1 = row[0], r0 = c0 > 0 ? row[-1] : none, r2 = c0 < P.nc[0] - 1 ? row[1] : none;
-    uint2 rw = none;                                                                // the wrapped cell of a periodic row
-    if (PERIODIC && !P.bc[0] && (c0 == 0 || c0 == P.nc[0] - 1)) rw = row[c0 == 0 ? P.nc[0] - 1 : -c0];
-    const float4 minef = xf_s[s];
-    const bool e0 = r0.y > r0.x, e1 = r1.y > r1.x, e2 = r2.y > r2.x;
-    const uint32_t t0 = max(e0 ? r0.x : (e1 ? r1.x : r2.x), (uint32_t)s + 1u);      // only the positions after mine
-    const uint32_t t1 = e2 ? r2.y : (e1 ? r1.y : r0.y);
     const double4 mine = xr_s[s];
-    for (uint32_t t = t0; t < t1; t += DETECT_NB) {                                // DETECT_NB candidates in flight
-        uint32_t tt[DETECT_NB];
-        float4 fc[DETECT_NB];
-        bool nn[DETECT_NB], any = false;
-#pragma unroll
-        for (int b = 0; b < DETECT_NB; ++b) {
-            tt[b] = min(t + (uint32_t)b, t1 - 1u);                                 // past the end: the last candidate again
-            fc[b] = xf_s[tt[b]];                                                   // first look in single precision (no branch),
+    const float4 minef = xf_s[s];
+    int st = 0;
+
+    int c0, c1, c2;
+    dem_cell_of_key(P, key, c0, c1, c2);
+
+    // A contact (s, t), t > s, goes into two lists.  Mine: slots 0, 1, ... of my column, counted in a register (only this
+    // thread writes them).  The partner's: slots maxc-1, maxc-2, ... of its column, the slot taken with an atomic on
+    // nback[t]; the store that needs the atomic's result is put off until the next contact (or the end), so the
+    // round trip to L2 is covered by the tests in between.
+    uint32_t nf = 0, pend_c = 0, pend_t = 0xffffffffu;
+    auto flush = [&]() {
+        if (pend_t != 0xffffffffu) {
+            if (pend_c < maxc) cand[(size_t)(maxc - 1u - pend_c) * P.n + pend_t] = (uint32_t)s;
+            else st |= LEDDS_ST_CONTACT_OVERFLOW;
         }
+    };
+    auto own = [&](uint32_t partner) {
+        if (nf < maxc) cand[(size_t)nf * P.n + s] = partner;
+        else st |= LEDDS_ST_CONTACT_OVERFLOW;
+        ++nf;
+    };
+    auto enter = [&](uint32_t t) {
+        own(t);
+        flush();
+        pend_c = atomicAdd(nback + t, 1u);
+        pend_t = t;
+    };
+    // the 9 runs [t0, t1) of x-adjacent cells (c0-1 .. c0+1 inside the row): all 27 range loads are independent
+    // and issued together; an empty cell holds (0, 0), so "first start, last end" needs no special case
+    uint32_t t0[9], t1[9];
 #pragma unroll
-        for (int b = 0; b < DETECT_NB; ++b) {
-            nn[b] = dem_near<PERIODIC>(P, minef, fc[b]) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
-            any |= nn[b];
+    for (int j = 0; j < 9; ++j) {
+        int qz = c2 + (j / 3 - 1), qy = c1 + (j % 3 - 1);
+        bool ok = true;
+        if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) ok = false; else qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
+        if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) ok = false; else qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
+        const uint2 none = make_uint2(0u, 0u);
+        uint2 r0 = none, r1 = none, r2 = none;
+        if (ok) {
+            const uint2* row = cell_range + (size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + c0;
+            r1 = row[0];
+            if (c0 > 0) r0 = row[-1];
+            if (c0 < P.nc[0] - 1) r2 = row[1];
         }
-        if (any) {                                                                 // Eq. (2) in double for the few that pass
-#pragma unroll
-            for (int b = 0; b < DETECT_NB; ++b)
-                if (nn[b] && dem_touch<PERIODIC>(P, mine, xr_s[tt[b]])) { enter((uint32_t)s, tt[b]); enter(tt[b], (uint32_t)s); }
-        }
+        const bool e0 = r0.y > r0.x, e1 = r1.y > r1.x, e2 = r2.y > r2.x;
+        t0[j] = max(e0 ? r0.x : (e1 ? r1.x : r2.x), (uint32_t)s + 1u);               // only the positions after mine
+        t1[j] = e2 ? r2.y : (e1 ? r1.y : r0.y);
     }
-    if (PERIODIC) {
-        for (uint32_t t = max(rw.x, (uint32_t)s + 1u); t < rw.y; ++t)
-            if (dem_near<PERIODIC>(P, minef, xf_s[t])) {
-                    if (dem_touch<PERIODIC>(P, mine, xr_s[t])) { enter((uint32_t)s, t); enter(t, (uint32_t)s); }
+#pragma unroll
+    for (int j = 0; j < 9; ++j) {
+        for (uint32_t t = t0[j]; t < t1[j]; t += DETECT_NB) {                      // DETECT_NB candidates in flight
+            uint32_t tt[DETECT_NB];
+            float4 fc[DETECT_NB];
+            bool nn[DETECT_NB], any = false;
+#pragma unroll
+            for (int b = 0; b < DETECT_NB; ++b) {
+                tt[b] = min(t + (uint32_t)b, t1[j] - 1u);                          // past the end: the last candidate again
+                fc[b] = xf_s[tt[b]];                                               // first look in single precision (no branch),
             }
-    }
-    if (j == 4) {
-        // walls: static infinite particles; overlap decided as the oracle does, R - distance > 0.
-        // The single-precision record tells which particles can reach a wall at all.
-        bool maybe = !(minef.w == minef.w);                                        // a NaN record: look
 #pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            const float xa = a == 0 ? minef.x : (a == 1 ? minef.y : minef.z);
-            if (P.bc[a] && (xa < minef.w + P.fmargin || P.Lf[a] - xa < minef.w + P.fmargin)) maybe = true;
-        }
-        if (maybe) {
-            const double xm[3] = {mine.x, mine.y, mine.z};
+            for (int b = 0; b < DETECT_NB; ++b) {
+                nn[b] = dem_near<PERIODIC>(P, minef, fc[b]) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
+                any |= nn[b];
+            }
+            if (any) {                                                             // Eq. (2) in double for the few that pass
 #pragma unroll
-            for (int wl = 0; wl < 6; ++wl) {
-                const int ax = wl >> 1;
-                if (!P.bc[ax]) continue;
-                const double dist = (wl & 1) ? P.hi[ax] - xm[ax] : xm[ax] - P.lo[ax];
-                if (mine.w - dist > 0.0) enter((uint32_t)s, DEM_WALL + (uint32_t)wl);
+                for (int b = 0; b < DETECT_NB; ++b)
+                    if (nn[b] && dem_touch<PERIODIC>(P, mine, xr_s[tt[b]])) enter(tt[b]);
             }
         }
     }
+    if (PERIODIC && !P.bc[0] && (c0 == 0 || c0 == P.nc[0] - 1)) {                  // the wrapped cell of a periodic row
+        const int wc = c0 == 0 ? P.nc[0] - 1 : 0;
+        for (int j = 0; j < 9; ++j) {
+            int qz = c2 + (j / 3 - 1), qy = c1 + (j % 3 - 1);
+            if (qz < 0 || qz >= P.nc[2]) { if (P.bc[2]) continue; qz = qz < 0 ? qz + P.nc[2] : qz - P.nc[2]; }
+            if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) continue; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
+            const uint2 r = cell_range[(size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + wc];
+            for (uint32_t t = max(r.x, (uint32_t)s + 1u); t < r.y; ++t)
+                if (dem_near<PERIODIC>(P, minef, xf_s[t]) && dem_touch<PERIODIC>(P, mine, xr_s[t])) enter(t);
+        }
+    }
+    // walls: static infinite particles; overlap decided as the oracle does, R - distance > 0
+    const double xm[3] = {mine.x, mine.y, mine.z};
+#pragma unroll
+    for (int wl = 0; wl < 6; ++wl) {
+        const int ax = wl >> 1;
+        if (!P.bc[ax]) continue;
+        const double dist = (wl & 1) ? P.hi[ax] - xm[ax] : xm[ax] - P.lo[ax];
+        if (mine.w - dist > 0.0) own(DEM_WALL + (uint32_t)wl);
+    }
+    flush();
+    nfwd[s] = nf;
     if (st) atomicOr(status, st);
 }
 
 // ------------------------------------------------------------------------------ scan
-// off[s] = sum over s' < s of min(ncand[s'], maxc), off[n] = total: single pass, chained tiles with decoupled look-back
+// off[s] = sum over s' < s of min(nfwd[s'] + nback[s'], maxc), off[n] = total: single pass, chained tiles with decoupled look-back
 // (tiles take tickets, as in the sort).
 __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ cnt,
-                                                               uint32_t* __restrict__ off, uint32_t* __restrict__ state,
-                                                               uint32_t* __restrict__ ticket)
+                                                               const uint32_t* __restrict__ cnt2, uint32_t* __restrict__ off,
+                                                               uint32_t* __restrict__ state, uint32_t* __restrict__ ticket)
 {
     __shared__ uint32_t wsum[SCAN_THREADS / 32];
     __shared__ uint32_t s_tile, s_excl;
@@ -655,11 +708,18 @@ __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t 
     const uint32_t tile = s_tile;
     const long long first = (long long)tile * SCAN_TILE + (long long)tid * SCAN_ITEMS;
     uint32_t c[SCAN_ITEMS], sum = 0;
+    static_assert(SCAN_ITEMS == 8, "two 16-byte loads per thread");
+    if (first + SCAN_ITEMS <= n) {                                                  // cnt is 256-byte aligned and first a multiple of 8
+        const uint4 a = reinterpret_cast<const uint4*>(cnt + first)[0], b = reinterpret_cast<const uint4*>(cnt + first)[1];
+        const uint4 a2 = reinterpret_cast<const uint4*>(cnt2 + first)[0], b2 = reinterpret_cast<const uint4*>(cnt2 + first)[1];
+        c[0] = a.x + a2.x; c[1] = a.y + a2.y; c[2] = a.z + a2.z; c[3] = a.w + a2.w;
+        c[4] = b.x + b2.x; c[5] = b.y + b2.y; c[6] = b.z + b2.z; c[7] = b.w + b2.w;
+    } else {
 #pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) {
-        c[i] = first + i < n ? min(cnt[first + i], maxc) : 0u;
-        sum += c[i];
+        for (int i = 0; i < SCAN_ITEMS; ++i) c[i] = first + i < n ? cnt[first + i] + cnt2[first + i] : 0u;
     }
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { c[i] = min(c[i], maxc); sum += c[i]; }
     uint32_t incl = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -715,23 +775,24 @@ __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t 
 // in.  Last step's list of the particle is in the same order, so one merge finds for every end the end it continues
 // (PAPER.md:496 searches the previous sorted pair list instead).  Everything the force kernel needs to start an end comes
 // out as coalesced records: owner and partner (sorted position: the packed (x, R) records; home index: the predictor
-// velocities), where the previous delta_t is, and whether the owner is the contact's first partner (i < j).
+// velocities) and where the previous delta_t is.
 // The particle's row descriptor is renewed here; a particle that has just lost its last contact gets its sums zeroed.
-#define DEM_NO_PREV 0x7fffffffu
-#define DEM_ME_FIRST 0x80000000u
+#define DEM_NO_PREV 0xffffffffu
 struct DemEnds { uint32_t *s, *t, *hs, *ht, *prev; };   // per contact end, CSR order
 
-__global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ ncand,
-                                                                const uint32_t* __restrict__ cand, const uint32_t* __restrict__ sid,
-                                                                const uint32_t* __restrict__ sh, const uint32_t* __restrict__ off,
-                                                                uint2* __restrict__ row, double* __restrict__ fm,
-                                                                const uint32_t* __restrict__ hq_prev, const DemEnds E,
-                                                                uint32_t* __restrict__ hq)
+__global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ nfwd,
+                                                                const uint32_t* __restrict__ nback, const uint32_t* __restrict__ cand,
+                                                                const uint32_t* __restrict__ sid, const uint32_t* __restrict__ sh,
+                                                                const uint32_t* __restrict__ off, uint2* __restrict__ row,
+                                                                double* __restrict__ fm, const uint32_t* __restrict__ hq_prev,
+                                                                const DemEnds E, uint32_t* __restrict__ hq, int32_t* __restrict__ status)
 {
-    extern __shared__ uint2 tq[];                                                   // [maxc][CONTACT_BLOCK]: (partner code, partner id)
+    extern __shared__ uint2 tq[];                        // uint2 [maxc][CONTACT_BLOCK]: (partner code, partner id); then uint32 [maxc][CONTACT_BLOCK]
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
-    const uint32_t cnt = min(ncand[s], maxc);
+    const uint32_t nf = min(nfwd[s], maxc), nb = min(nback[s], maxc);
+    const uint32_t cnt = min(nf + nb, maxc);
+    if (nf + nb > maxc) atomicOr(status, LEDDS_ST_CONTACT_OVERFLOW);                // the two ends of the column met
     const uint32_t h = sh[s];
     const uint2 old = row[h];
     if (cnt == 0) {
@@ -742,67 +803,114 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
         }
         return;
     }
-    const uint32_t p = sid[s];
     uint2* mine = tq + threadIdx.x;
-    for (uint32_t c = 0; c < cnt; ++c) {
-        const uint32_t t = cand[(size_t)c * n + s];
-        const uint32_t q = t >= DEM_WALL ? (uint32_t)n + (t - DEM_WALL) : sid[t];
-        uint32_t k = c;                                                             // insertion sort by q
-        while (k > 0 && mine[(k - 1) * CONTACT_BLOCK].y > q) { mine[k * CONTACT_BLOCK] = mine[(k - 1) * CONTACT_BLOCK]; --k; }
-        mine[k * CONTACT_BLOCK] = make_uint2(t, q);
-    }
+    uint32_t* pq = reinterpret_cast<uint32_t*>(tq + (size_t)maxc * CONTACT_BLOCK) + threadIdx.x;   // last step's partner ids
     const uint32_t o = off[s];
-    uint32_t k = 0, qk = old.y ? hq_prev[old.x] : 0xffffffffu;
-    for (uint32_t c = 0; c < cnt; ++c) {
+    // every loop below keeps four independent loads in flight per thread: the partner codes, their ids, last step's
+    // ids of this particle; then the ordering runs in shared memory
+    for (uint32_t c0 = 0; c0 < cnt; c0 += 4) {
+        uint32_t t[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t c = c0 + j;
+            t[j] = c < cnt ? cand[(size_t)(c < nf ? c : maxc - 1u - (c - nf)) * n + s] : 0u;
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (c0 + j < cnt) mine[(c0 + j) * CONTACT_BLOCK].x = t[j];
+    }
+    for (uint32_t c0 = 0; c0 < old.y; c0 += 4) {
+        uint32_t q[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) q[j] = c0 + j < old.y ? hq_prev[old.x + c0 + j] : 0u;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (c0 + j < old.y) pq[(c0 + j) * CONTACT_BLOCK] = q[j];
+    }
+    for (uint32_t c0 = 0; c0 < cnt; c0 += 4) {
+        uint32_t q[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t t = c0 + j < cnt ? mine[(c0 + j) * CONTACT_BLOCK].x : DEM_WALL;
+            q[j] = t >= DEM_WALL ? (uint32_t)n + (t - DEM_WALL) : sid[t];
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (c0 + j < cnt) mine[(c0 + j) * CONTACT_BLOCK].y = q[j];
+    }
+    for (uint32_t c = 1; c < cnt; ++c) {                                            // insertion sort by id
         const uint2 e = mine[c * CONTACT_BLOCK];
-        while (qk < e.y) { ++k; qk = k < old.y ? hq_prev[old.x + k] : 0xffffffffu; }
-        const uint32_t prev = qk == e.y ? old.x + k : DEM_NO_PREV;
-        E.s[o + c] = (uint32_t)s;
-        E.t[o + c] = e.x;
-        E.hs[o + c] = h;
-        E.ht[o + c] = e.x >= DEM_WALL ? 0u : sh[e.x];
-        E.prev[o + c] = prev | (p < e.y ? DEM_ME_FIRST : 0u);
-        hq[o + c] = e.y;
+        uint32_t k = c;
+        while (k > 0 && mine[(k - 1) * CONTACT_BLOCK].y > e.y) { mine[k * CONTACT_BLOCK] = mine[(k - 1) * CONTACT_BLOCK]; --k; }
+        mine[k * CONTACT_BLOCK] = e;
+    }
+    uint32_t k = 0;
+    for (uint32_t c0 = 0; c0 < cnt; c0 += 4) {
+        uint2 e[4];
+        uint32_t ht[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            e[j] = c0 + j < cnt ? mine[(c0 + j) * CONTACT_BLOCK] : make_uint2(DEM_WALL, 0u);
+            ht[j] = e[j].x >= DEM_WALL ? 0u : sh[e[j].x];
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t c = c0 + j;
+            if (c >= cnt) break;
+            while (k < old.y && pq[k * CONTACT_BLOCK] < e[j].y) ++k;                 // both lists ascend in the partner id
+            E.s[o + c] = (uint32_t)s;
+            E.t[o + c] = e[j].x;
+            E.hs[o + c] = h;
+            E.ht[o + c] = ht[j];
+            E.prev[o + c] = (k < old.y && pq[k * CONTACT_BLOCK] == e[j].y) ? old.x + k : DEM_NO_PREV;
+            hq[o + c] = e[j].y;
+        }
     }
     row[h] = make_uint2(o, cnt);
 }
 
 // ------------------------------------------------------------------------------ force
-// A block owns FORCE_PB consecutive particles (sorted order) and all their contact ends, a contiguous piece
-// [off[s0], off[s0 + FORCE_PB]) of the CSR arrays.  It works through that piece FORCE_THREADS ends at a time, one end per
-// thread (all lanes busy whatever the contact counts of the particles are): both partners evaluate a contact in its
-// canonical orientation (i < j), so F_ij = -F_ji bit for bit; the end's force and torque go to shared memory, and the
-// thread that owns the particle adds up its ends in list order.  An end starts from the records dem_fill_kernel left:
-// one coalesced read, then every further load (both bodies, the previous delta_t) is independent of the others.
+// A warp owns FORCE_PW consecutive particles (sorted order) and all their contact ends, a contiguous piece
+// [off[s0], off[s0 + FORCE_PW]) of the CSR arrays.  It works through that piece 32 ends at a time, one end per lane
+// (all lanes busy whatever the contact counts of the particles are); the end's force and torque go to shared
+// memory, and the lane that owns the particle adds up its ends in list order (Eq. 1).  An end starts from the records
+// dem_fill_kernel left: one coalesced read, then every further load (both bodies, the previous delta_t) is independent
+// of the others.
+// Both partners evaluate their contact, each from its own side: e_n = (r_owner - r_partner)/|.|, v_rel, delta_t and the
+// forces all change sign exactly when the roles are swapped (every operation below is sign-symmetric in IEEE arithmetic
+// and the sums R_i w_i + R_j w_j, m_i m_j, m_i + m_j commute; no FMA contraction in this file), so F_ij = -F_ji and
+// M_i / R_i = M_j / R_j hold bit for bit, and what the owner with the higher id computes is exactly the negative of the
+// canonical (i < j) evaluation of the oracle.
 template <bool HERTZ>
 __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_kernel(
     const DemDev P, const double4* __restrict__ xr_s, const double* __restrict__ pvw, const uint32_t* __restrict__ off,
     const DemEnds E, const uint32_t* __restrict__ sh, double* __restrict__ fm, const double* __restrict__ hdt_prev,
     double* __restrict__ hdt_new, int32_t* __restrict__ status, double dt_hist)
 {
-    __shared__ uint32_t s_off[FORCE_PB + 1];
-    __shared__ double stage[6][FORCE_THREADS];
-    const int tid = threadIdx.x;
-    const int s0 = blockIdx.x * FORCE_PB, np = min(FORCE_PB, P.n - s0);
-    if (off[s0] == off[s0 + np]) return;                                            // no contact in this block (block-uniform)
-    for (int i = tid; i <= np; i += FORCE_THREADS) s_off[i] = off[s0 + i];
-    __syncthreads();
-    const uint32_t e_begin = s_off[0], e_end = s_off[np];
-    constexpr int OWN = FORCE_PB / FORCE_THREADS;
-    double acc[OWN][6];
-#pragma unroll
-    for (int j = 0; j < OWN; ++j)
-#pragma unroll
-        for (int c = 0; c < 6; ++c) acc[j][c] = 0.0;
+    // every warp works on its own FORCE_PW particles with its own piece of shared memory: no block-wide barrier
+    __shared__ uint32_t s_off_all[FORCE_WARPS][FORCE_PW + 1];
+    __shared__ double stage_all[FORCE_WARPS][6][32];
+    __shared__ double sacc_all[FORCE_WARPS][6][FORCE_PW];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int s0 = (blockIdx.x * FORCE_WARPS + warp) * FORCE_PW;
+    if (s0 >= P.n) return;
+    const int np = min(FORCE_PW, P.n - s0);
+    uint32_t* s_off = s_off_all[warp];
+    double (*stage)[32] = stage_all[warp];
+    double (*sacc)[FORCE_PW] = sacc_all[warp];
+    const uint32_t e_begin = off[s0], e_end = off[s0 + np];
+    if (e_begin == e_end) return;                                                   // no contact among these particles (warp-uniform)
+    for (int i = lane; i <= np; i += 32) s_off[i] = off[s0 + i];
+    for (int i = lane; i < 6 * FORCE_PW; i += 32) (&sacc[0][0])[i] = 0.0;
+    __syncwarp();
     int st = 0;
 
-    for (uint32_t chunk = e_begin; chunk < e_end; chunk += FORCE_THREADS) {
-        const uint32_t e = chunk + (uint32_t)tid;
+    for (uint32_t chunk = e_begin; chunk < e_end; chunk += 32) {
+        const uint32_t e = chunk + (uint32_t)lane;
         double Fe[3] = {0, 0, 0}, Me[3] = {0, 0, 0};
         if (e < e_end) {
-            const uint32_t s = E.s[e], t = E.t[e], hs = E.hs[e], ht = E.ht[e], pf = E.prev[e];
+            const uint32_t s = E.s[e], t = E.t[e], hs = E.hs[e], ht = E.ht[e], prev = E.prev[e];
             const bool wall = t >= DEM_WALL;
-            const uint32_t prev = pf & DEM_NO_PREV;
             // all loads of the end, issued together
             const double4 m4 = xr_s[s];
             const double2* rm = reinterpret_cast<const double2*>(pvw + 6 * (size_t)hs);
@@ -810,43 +918,30 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_ker
             const double4 o4 = xr_s[wall ? s : t];
             const double2* ro = reinterpret_cast<const double2*>(pvw + 6 * (size_t)(wall ? hs : ht));
             const double2 oa = ro[0], ob = ro[1], oc = ro[2];
-            double dt3[3] = {0, 0, 0};                                                 // previous delta_t of this end, as its owner stored it
+            double dt3[3] = {0, 0, 0};                                                 // previous delta_t of this end, seen from its owner
             if (prev != DEM_NO_PREV) {
                 const double* d = hdt_prev + 3 * (size_t)prev;
                 dt3[0] = d[0]; dt3[1] = d[1]; dt3[2] = d[2];
             }
             const double xm[3] = {m4.x, m4.y, m4.z}, Rm = m4.w;
             const double vm[3] = {ma.x, ma.y, mb.x}, wm[3] = {mb.y, mc.x, mc.y};
-            double F[3], T[3], kn, kt, gn, gt;
+            double F[3] = {0, 0, 0}, T[3] = {0, 0, 0}, kn, kt, gn, gt;
             if (!wall) {
                 const double xo[3] = {o4.x, o4.y, o4.z}, Ro = o4.w;
                 const double vo[3] = {oa.x, oa.y, ob.x}, wo[3] = {ob.y, oc.x, oc.y};
-                const bool me_first = (pf & DEM_ME_FIRST) != 0;                        // canonical orientation i < j
-                const double sg = me_first ? 1.0 : -1.0;
-                double xi[3], xj[3], vi[3], vj[3], wi[3], wj[3];
-#pragma unroll
-                for (int a = 0; a < 3; ++a) {
-                    xi[a] = me_first ? xm[a] : xo[a]; xj[a] = me_first ? xo[a] : xm[a];
-                    vi[a] = me_first ? vm[a] : vo[a]; vj[a] = me_first ? vo[a] : vm[a];
-                    wi[a] = me_first ? wm[a] : wo[a]; wj[a] = me_first ? wo[a] : wm[a];
-                }
-                const double Ri = me_first ? Rm : Ro, Rj = me_first ? Ro : Rm;
                 double d[3];
-                dem_min_image(P, xi, xj, d);
+                dem_min_image(P, xm, xo, d);
                 const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-                const double dn = (Ri + Rj) - dist;                                    // Eq. (6)
+                const double dn = (Rm + Ro) - dist;                                    // Eq. (6)
                 if (dist == 0.0) {
                     st |= LEDDS_ST_COINCIDENT;                                         // pair skipped, delta_t = 0 (as the oracle)
                     dt3[0] = dt3[1] = dt3[2] = 0.0;
                 } else {
                     const double en[3] = {d[0] / dist, d[1] / dist, d[2] / dist};      // Eq. (7)
-                    const double mi = dem_mass(P, Ri), mj = dem_mass(P, Rj);
+                    const double mi = dem_mass(P, Rm), mj = dem_mass(P, Ro);
                     const double mstar = mi * mj / (mi + mj);                          // (A.9)
-                    dt3[0] *= sg; dt3[1] *= sg; dt3[2] *= sg;                          // canonical
-                    dem_coefficients<HERTZ>(P.kn, P.kt, P.Ystar, P.Gstar, P.zeta, mstar, Ri * Rj / (Ri + Rj), dn, kn, kt, gn, gt);
-                    dem_pair_force(en, dn, vi, wi, Ri, vj, wj, Rj, kn, kt, gn, gt, P.mu, dt_hist, dt3, F, T);
-#pragma unroll
-                    for (int a = 0; a < 3; ++a) { Fe[a] = sg * F[a]; Me[a] = Rm * (-T[a]); dt3[a] *= sg; }
+                    dem_coefficients<HERTZ>(P.kn, P.kt, P.Ystar, P.Gstar, P.zeta, mstar, Rm * Ro / (Rm + Ro), dn, kn, kt, gn, gt);
+                    dem_pair_force(en, dn, vm, wm, Rm, vo, wo, Ro, kn, kt, gn, gt, P.mu, dt_hist, dt3, F, T);
                 }
             } else {                                                                   // a wall: R* = R_i, m* = m_i
                 const int wl = (int)(t - DEM_WALL), ax = wl >> 1, side = wl & 1;
@@ -858,37 +953,38 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_ker
                 const double vj[3] = {P.vw[wl * 3], P.vw[wl * 3 + 1], P.vw[wl * 3 + 2]}, wj[3] = {0, 0, 0};
                 dem_coefficients<HERTZ>(P.kn_w, P.kt_w, P.Ystar_w, P.Gstar_w, P.zeta_w, dem_mass(P, Rm), Rm, dn, kn, kt, gn, gt);
                 dem_pair_force(en, dn, vm, wm, Rm, vj, wj, 0.0, kn, kt, gn, gt, P.mu_w, dt_hist, dt3, F, T);
-#pragma unroll
-                for (int a = 0; a < 3; ++a) { Fe[a] = F[a]; Me[a] = Rm * (-T[a]); }
             }
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { Fe[a] = F[a]; Me[a] = Rm * (-T[a]); }         // Eq. (15)
             double* nd = hdt_new + 3 * (size_t)e;
             nd[0] = dt3[0]; nd[1] = dt3[1]; nd[2] = dt3[2];
         }
 #pragma unroll
-        for (int a = 0; a < 3; ++a) { stage[a][tid] = Fe[a]; stage[3 + a][tid] = Me[a]; }
-        __syncthreads();
-        // Eq. (1): every particle's thread adds up the ends of this round that are its own, in list order
+        for (int a = 0; a < 3; ++a) { stage[a][lane] = Fe[a]; stage[3 + a][lane] = Me[a]; }
+        __syncwarp();
+        // Eq. (1): the lane that owns a particle adds up the ends of this round that are the particle's, in list order
+        for (int i = lane; i < np; i += 32) {
+            const uint32_t lo = max(s_off[i], chunk), hi = min(s_off[i + 1], chunk + 32u);
+            if (lo < hi) {
+                double a6[6];
 #pragma unroll
-        for (int j = 0; j < OWN; ++j) {
-            const int i = tid + j * FORCE_THREADS;
-            if (i < np) {
-                const uint32_t lo = max(s_off[i], chunk), hi = min(s_off[i + 1], chunk + (uint32_t)FORCE_THREADS);
+                for (int c = 0; c < 6; ++c) a6[c] = sacc[c][i];
                 for (uint32_t e2 = lo; e2 < hi; ++e2)
 #pragma unroll
-                    for (int c = 0; c < 6; ++c) acc[j][c] += stage[c][e2 - chunk];
+                    for (int c = 0; c < 6; ++c) a6[c] += stage[c][e2 - chunk];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) sacc[c][i] = a6[c];
             }
         }
-        __syncthreads();
+        __syncwarp();
     }
     // the sums of every particle that has a contact, for the kick (home order)
-#pragma unroll
-    for (int j = 0; j < OWN; ++j) {
-        const int i = tid + j * FORCE_THREADS;
-        if (i >= np || s_off[i + 1] == s_off[i]) continue;
+    for (int i = lane; i < np; i += 32) {
+        if (s_off[i + 1] == s_off[i]) continue;
         const uint32_t h = sh[s0 + i];
         bool finite = true;
 #pragma unroll
-        for (int c = 0; c < 6; ++c) { fm[6 * (size_t)h + c] = acc[j][c]; finite = finite && isfinite(acc[j][c]); }
+        for (int c = 0; c < 6; ++c) { const double v = sacc[c][i]; fm[6 * (size_t)h + c] = v; finite = finite && isfinite(v); }
         if (!finite) st |= LEDDS_ST_NONFINITE;
     }
     if (st) atomicOr(status, st);
@@ -1045,6 +1141,11 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     }
     if (ncell > 4.0e9) return LEDDS_EINVAL;
     d.ncell = (unsigned)ncell;
+    d.plane = (unsigned)d.nc[0] * (unsigned)d.nc[1];
+    // floor(k m / 2^40) = floor(k / d) for m = ceil(2^40 / d) whenever k (m d - 2^40) < 2^40, which k d <= 2^40 ensures
+    d.magic_ok = ncell * (double)d.plane <= 1099511627776.0 && (double)d.plane * d.nc[0] <= 1099511627776.0;
+    d.magic_row = ((1ull << 40) + (unsigned)d.nc[0] - 1) / (unsigned)d.nc[0];
+    d.magic_plane = ((1ull << 40) + d.plane - 1) / d.plane;
     d.fmargin = (float)(fmax(d.L[0], fmax(d.L[1], d.L[2])) / 524288.0);              // 2^-19 max L (dem_near)
     d.dt = p->dt; d.density = p->density;
     d.kn = p->kn; d.kt = p->kt; d.zeta = dem_zeta_host(p->restitution); d.mu = p->mu;
@@ -1083,7 +1184,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     s.hv = take(n * 24); s.hw = take(n * 24); s.ha = take(n * 24); s.hal = take(n * 24);
     s.pvw = take(n * 48);
     s.xr_s = take(n * 32); s.xf_s = take(n * 16);
-    s.ncand = take(n * 4); s.cand = take(ecap * 4);
+    s.nfwd = take(n * 4); s.nback = take(n * 4); s.cand = take(ecap * 4);
     s.off = take((n + 1) * 4);
     s.end_s = take(ecap * 4); s.end_t = take(ecap * 4); s.end_hs = take(ecap * 4); s.end_ht = take(ecap * 4); s.end_prev = take(ecap * 4);
     s.pair_count = take((n + 1) * 4); s.pair_off = take((n + 1) * 4); s.pos_of_id = take((n + 1) * 4);
@@ -1222,7 +1323,8 @@ int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32
     const uint32_t* sh0 = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
     uint32_t* sh = at<uint32_t>(scratch, s.idx[h->sh_buf]);
     uint32_t* sid = at<uint32_t>(scratch, s.sid);
-    uint32_t* ncand = at<uint32_t>(scratch, s.ncand);
+    uint32_t* nfwd = at<uint32_t>(scratch, s.nfwd);
+    uint32_t* nback = at<uint32_t>(scratch, s.nback);
     uint32_t* off = at<uint32_t>(scratch, s.off);
     ledds_prof_start(LEDDS_K_DEM_GATHER, st);
     dem_ranges_kernel<<<nb, tb, 0, st>>>(n, skey, sh0, at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp),
@@ -1230,27 +1332,27 @@ int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32
     LEDDS_CHECK_LAUNCH();
     dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sh0, at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range),
                                          at<double4>(scratch, s.hx), at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
-                                         sid, sh, ncand);
+                                         sid, sh, nback);
     ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
     LEDDS_CHECK_LAUNCH();
     const int prev = h->cur, nw = 1 - h->cur;
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
     const int cb = (n + CONTACT_BLOCK - 1) / CONTACT_BLOCK;
     if (d.bc[0] && d.bc[1] && d.bc[2])
-        dem_detect_kernel<false><<<dim3(cb, 9), CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
-                                                                        at<uint2>(scratch, s.cell_range), ncand, at<uint32_t>(scratch, s.cand), status);
+        dem_detect_kernel<false><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+                                                                        at<uint2>(scratch, s.cell_range), nfwd, nback, at<uint32_t>(scratch, s.cand), status);
     else
-        dem_detect_kernel<true><<<dim3(cb, 9), CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
-                                                                       at<uint2>(scratch, s.cell_range), ncand, at<uint32_t>(scratch, s.cand), status);
+        dem_detect_kernel<true><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+                                                                       at<uint2>(scratch, s.cell_range), nfwd, nback, at<uint32_t>(scratch, s.cand), status);
     LEDDS_CHECK_LAUNCH();
-    dem_scan_kernel<<<h->scan_tiles, SCAN_THREADS, 0, st>>>(n, (uint32_t)d.maxc, ncand, off, at<uint32_t>(scratch, s.scan_state),
+    dem_scan_kernel<<<h->scan_tiles, SCAN_THREADS, 0, st>>>(n, (uint32_t)d.maxc, nfwd, nback, off, at<uint32_t>(scratch, s.scan_state),
                                                             at<uint32_t>(scratch, s.tile_counter) + 4);
     LEDDS_CHECK_LAUNCH();
     const DemEnds E = {at<uint32_t>(scratch, s.end_s), at<uint32_t>(scratch, s.end_t), at<uint32_t>(scratch, s.end_hs),
                        at<uint32_t>(scratch, s.end_ht), at<uint32_t>(scratch, s.end_prev)};
-    dem_fill_kernel<<<cb, CONTACT_BLOCK, (size_t)d.maxc * CONTACT_BLOCK * sizeof(uint2), st>>>(
-        n, (uint32_t)d.maxc, ncand, at<uint32_t>(scratch, s.cand), sid, sh, off, row, fm, at<uint32_t>(history, hs.hq[prev]), E,
-        at<uint32_t>(history, hs.hq[nw]));
+    dem_fill_kernel<<<cb, CONTACT_BLOCK, (size_t)d.maxc * CONTACT_BLOCK * 12, st>>>(
+        n, (uint32_t)d.maxc, nfwd, nback, at<uint32_t>(scratch, s.cand), sid, sh, off, row, fm, at<uint32_t>(history, hs.hq[prev]), E,
+        at<uint32_t>(history, hs.hq[nw]), status);
     LEDDS_CHECK_LAUNCH();
     (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<(n + FORCE_PB - 1) / FORCE_PB, FORCE_THREADS, 0, st>>>(
         d, at<double4>(scratch, s.xr_s), at<double>(scratch, s.pvw), off, E, sh, fm, at<double>(history, hs.hdt[prev]),
