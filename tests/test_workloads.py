@@ -24,6 +24,13 @@ def test_paper_bed_spheres_do_not_overlap_and_reach_the_fraction():
         assert x[:, 2].min() - R[0] > -0.5 and x[:, 2].max() + R[0] < 799.5
         assert cpl["n_sub"] == 10 and lbm["collision"] == 1
     assert len(W.paper_bed(0.0)[6]) == 0
+    # the packed variant bench.py times: columns of touching spheres, nothing overlaps by more than 0.5 % of a diameter
+    for phi, expect in ((0.15, 2866), (0.45, 8596)):
+        lbm, cpl, pd, x, v, w, R = W.paper_bed(phi, contacts=True)
+        assert abs(len(R) / expect - 1.0) < 0.03
+        gap = _min_gap(x, R, (500.0, 200.0, 800.0), (True, True, False))
+        assert -0.1 < gap < 0.0
+        assert x[:, 2].min() - R[0] > -0.6 and x[:, 2].max() + R[0] < 799.5
 
 
 def test_config_generators_are_seeded_and_shaped():

@@ -233,13 +233,15 @@ def dem_random(seed, n, box=(10.0, 10.0, 10.0), bc=(1, 1, 1), rmin=0.4, rmax=0.6
     return pd, x, v, w, radius
 
 
-def paper_bed(phi, shape=(500, 200, 800), D=20.0, seed=6, n_sub=10):
+def paper_bed(phi, shape=(500, 200, 800), D=20.0, seed=6, n_sub=10, contacts=False):
     """the paper's performance workload: a 500 x 200 x 800 lattice,
     spheres of diameter 20 cells at solid fraction phi (0 / 0.15 / 0.30 / 0.45 -> 0 / 2 866 / 5 731 / 8 596 spheres
     in the paper), density ratio 1.1, 10 DEM sub-steps per LBM step, TRT collision.  The paper's inlet / outlet
     are not part of the hot path: here the box is periodic in x, y with walls in z, fluid at rest, gravity on
     the spheres.  Placement: seeded jittered simple-cubic lattice at the spacing that gives phi (RSA cannot
-    reach 0.45), filled from the bottom."""
+    reach 0.45), filled from the bottom.  contacts=True: the same number of spheres stacked in vertical columns
+    whose neighbours overlap by 0.4 % of a diameter (the lowest one rests on the floor), so that the bed has
+    about one contact per sphere from the first step on and the DEM contact path is loaded."""
     nx, ny, nz = shape
     R = 0.5 * D
     lbm = dict(shape=shape, tau=0.6, bc=(0, 0, 1), u_wall=np.zeros(18), collision=1)
@@ -248,7 +250,25 @@ def paper_bed(phi, shape=(500, 200, 800), D=20.0, seed=6, n_sub=10):
     vol = (4.0 / 3.0) * PI * R ** 3
     n_part = int(round(phi * nx * ny * nz / vol))
     g = _rng(seed)
-    if n_part > 0:
+    if n_part > 0 and contacts:
+        szc = 2.0 * R * 0.996
+        best = None
+        for mx in range(max(1, int(nx // (2 * R)) - 8), int(nx // (2 * R)) + 1):
+            for my in range(max(1, int(ny // (2 * R)) - 4), int(ny // (2 * R)) + 1):
+                sx, sy = nx / mx, ny / my
+                layers = -(-n_part // (mx * my))
+                if min(sx, sy) <= 2.0 * R + 0.2 or layers * szc + 2.0 > nz:
+                    continue
+                if best is None or min(sx, sy) > best[0]:
+                    best = (min(sx, sy), mx, my, sx, sy)
+        assert best is not None, "bed does not fit at this fraction"
+        _, mx, my, sx, sy = best
+        sites = np.arange(n_part)
+        i, j, k = sites % mx, (sites // mx) % my, sites // (mx * my)
+        x = np.stack([(i + 0.5) * sx - 0.5, (j + 0.5) * sy - 0.5, -0.5 + 0.996 * R + k * szc], -1)
+        x[:, :2] += g.uniform(-0.05, 0.05, (n_part, 2))
+        x = x[g.permutation(n_part)]
+    elif n_part > 0:
         # lattice spacing for the target fraction, snapped so that whole cells fit the periodic directions
         s = (vol / phi) ** (1.0 / 3.0)
         best = None
