@@ -422,9 +422,10 @@ def run_ours(args, rank, world):
                                                "note": "159 MB per lattice: close to L2 size, so MLUPS may exceed the HBM bound"}
             del g3, gl3, gd3
         # configs[4]: DEM-only, 4 M polydisperse spheres (jittered-lattice placement), + supplementary dense state
-        for name, dense in (("cfg5_dem_pour_4M", False), ("cfg5_dense_supplement_4M", True)):
+        for name, dense, prec in (("cfg5_dem_pour_4M", False, "f64"), ("cfg5_dense_supplement_4M", True, "f64"),
+                                  ("cfg5_dem_pour_4M_f32", False, "f32"), ("cfg5_dense_supplement_4M_f32", True, "f32")):
             pd5, x5, v5, w5, R5 = W.cfg5_pour(n_side=160 if not small else 40, n_part=4_000_000 if not small else 64000, dense=dense)
-            gd = Dem(pd5, x5, v5, w5, R5)
+            gd = Dem(pd5, x5, v5, w5, R5, precision=prec)
             gd.step(5); torch.cuda.synchronize()
             L.ledds_profile(True)
             kd = 50
@@ -432,7 +433,7 @@ def run_ours(args, rank, world):
             pr = {nm: round(L.ledds_profile_read(i)[0] / kd, 5) for i, nm in enumerate(L.KERNEL_GROUPS) if nm.startswith("dem")}
             L.ledds_profile(False)
             q = torch.zeros(4, dtype=torch.int32, device="cuda")
-            L.ledds_dem_query(gd.h, gd.history, gd.scratch, None, None, None, None, 0, q, None, None)
+            (L.ledds_dem_query_f32 if prec == "f32" else L.ledds_dem_query)(gd.h, gd.history, gd.scratch, None, None, None, None, 0, q, None, None)
             contacts = int(q[0].item())
             ncell = 1
             for a in range(3):
@@ -441,6 +442,13 @@ def run_ours(args, rank, world):
             bytes_k, bpp, bpe = dem_bytes((max(1, int(np.ceil(np.log2(ncell)))) + 7) // 8, len(R5), ends)
             gbs = {nm: fracs(bytes_k[nm] / (pr[nm] * 1e-3) / 1e9, peak) for nm in bytes_k if pr.get(nm, 0) > 0}
             total_bytes = sum(bytes_k.values())
+            if prec == "f32":                                            # the fp64 byte model does not apply: times only
+                sub[name] = {"particle_updates_per_s": round(len(R5) * 1e3 / ms5, 1), "ms_per_step": round(ms5, 5), "steps": kd,
+                             "particles": len(R5), "contacts": contacts, "kernel_ms_per_step": pr, "dtype": "f32",
+                             "status_word": int(gd.status[0].item())}
+                del gd
+                torch.cuda.empty_cache()
+                continue
             sub[name] = {"particle_updates_per_s": round(len(R5) * 1e3 / ms5, 1), "ms_per_step": round(ms5, 5), "steps": kd,
                          "particles": len(R5), "contacts": contacts, "kernel_ms_per_step": pr,
                          "algorithmic_bytes_per_particle": bpp, "algorithmic_bytes_per_contact_end": bpe, "kernel_hbm": gbs,

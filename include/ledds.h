@@ -139,6 +139,10 @@ typedef struct {
     double young_w, poisson_w;     /* ... of the walls                                            */
 } ledds_dem_params;
 
+/* scratch and history are caller-owned but belong to the handle between calls: the library keeps the particle state
+ * there in its own ("home") order while a call runs, and the last sort, the contact lists and the tangential history
+ * between calls.  The caller's arrays x, v, w, a, alpha are read when a call begins and written when it ends; they may
+ * be changed by the caller between calls (the next call picks the changes up), scratch and history may not. */
 int ledds_dem_workspace_bytes(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes);
 
 /* Creates the handle, clears history/scratch, evaluates the contacts of the initial state with
@@ -164,6 +168,26 @@ int ledds_dem_query(ledds_dem* h, const void* history, const void* scratch, uint
                     double* force, double* torque, void* stream);
 
 int ledds_dem_destroy(ledds_dem* h);
+
+/* Single-precision variant of the DEM calls (the paper runs most of its DEM validations in single precision and shows
+ * fp32 next to fp64 energy curves, Appendix B).  Same pipeline and arguments on float
+ * arrays; the particle state, the sorted records, the predictor velocities, the contact history and every operation
+ * of the step are fp32.  Rules for the discrete decisions: the cell of a particle is floor((x - lo) * inv_h) in fp32
+ * with inv_h = (float)(n_cells / L); a pair is in contact when (R_i + R_j) - sqrt(d.d) > 0 in fp32, d the fp32
+ * difference of the fp32 positions (nearest image), summed as (dx dx + dy dy) + dz dz; a wall when R - distance > 0
+ * in fp32.  Ordering (cell key, then id) and the canonical pair list are defined as for fp64, on those decisions.
+ * A handle made by ledds_dem_init_f32 is accepted by the _f32 calls and ledds_dem_destroy only, and not by
+ * ledds_coupled_step (LEDDS_EINVAL). */
+int ledds_dem_workspace_bytes_f32(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes);
+int ledds_dem_init_f32(ledds_dem** h, const ledds_dem_params* p, const float* x, const float* v, const float* w,
+                       const float* radius, float* a, float* alpha, void* history, void* scratch, int32_t* status,
+                       void* stream);
+int ledds_dem_step_f32(ledds_dem* h, float* x, float* v, float* w, float* a, float* alpha, const float* radius,
+                       const float* f_ext, const float* m_ext, void* history, void* scratch, int32_t* status, int nsteps,
+                       void* stream);
+int ledds_dem_query_f32(ledds_dem* h, const void* history, const void* scratch, uint32_t* sorted_idx,
+                        uint32_t* sorted_key, uint32_t* pairs, float* pair_dt, uint32_t pair_cap, uint32_t* n_pairs,
+                        float* force, float* torque, void* stream);
 
 /* -------------------------------------------------------------------------------- coupling
  * Partially saturated cells: solid fraction Eq. (39)-(40), weights Eq. (36)-(37),

@@ -22,7 +22,8 @@ ST_CONTACT_OVERFLOW, ST_SOLID_OVERFLOW, ST_COINCIDENT, ST_NONFINITE, ST_RADIUS_R
 EXPORTS = ["ledds_lbm_workspace_bytes", "ledds_lbm_init", "ledds_lbm_import", "ledds_lbm_step", "ledds_lbm_export",
            "ledds_lbm_current", "ledds_lbm_destroy", "ledds_lbm_workspace_bytes_f32", "ledds_lbm_init_f32",
            "ledds_lbm_import_f32", "ledds_lbm_step_f32", "ledds_lbm_export_f32", "ledds_dem_workspace_bytes", "ledds_dem_init", "ledds_dem_step",
-           "ledds_dem_query", "ledds_dem_destroy", "ledds_cpl_workspace_bytes", "ledds_cpl_init", "ledds_coupled_step",
+           "ledds_dem_query", "ledds_dem_destroy", "ledds_dem_workspace_bytes_f32", "ledds_dem_init_f32", "ledds_dem_step_f32",
+           "ledds_dem_query_f32", "ledds_cpl_workspace_bytes", "ledds_cpl_init", "ledds_coupled_step",
            "ledds_coupled_step_f32", "ledds_version",
            "ledds_profile", "ledds_profile_read", "ledds_launch_count"]
 
@@ -222,6 +223,31 @@ def ledds_dem_query(h, history, scratch, sorted_idx=None, sorted_key=None, pairs
 
 def ledds_dem_destroy(h):
     _lib.ledds_dem_destroy(h)
+
+
+# fp32 set: same calls on float arrays (include/ledds.h)
+def ledds_dem_workspace_bytes_f32(p: DemParams):
+    a, b = C.c_size_t(0), C.c_size_t(0)
+    _check(_lib.ledds_dem_workspace_bytes_f32(C.byref(p), C.byref(a), C.byref(b)), "ledds_dem_workspace_bytes_f32")
+    return a.value, b.value
+
+
+def ledds_dem_init_f32(p: DemParams, x, v, w, radius, a, alpha, history, scratch, status):
+    h = C.c_void_p(0)
+    _check(_lib.ledds_dem_init_f32(C.byref(h), C.byref(p), _p(x), _p(v), _p(w), _p(radius), _p(a), _p(alpha), _p(history),
+                                   _p(scratch), _p(status), _stream()), "ledds_dem_init_f32")
+    return h
+
+
+def ledds_dem_step_f32(h, x, v, w, a, alpha, radius, f_ext, m_ext, history, scratch, status, nsteps=1):
+    _check(_lib.ledds_dem_step_f32(h, _p(x), _p(v), _p(w), _p(a), _p(alpha), _p(radius), _p(f_ext), _p(m_ext), _p(history),
+                                   _p(scratch), _p(status), C.c_int(nsteps), _stream()), "ledds_dem_step_f32")
+
+
+def ledds_dem_query_f32(h, history, scratch, sorted_idx=None, sorted_key=None, pairs=None, pair_dt=None, pair_cap=0,
+                        n_pairs=None, force=None, torque=None):
+    _check(_lib.ledds_dem_query_f32(h, _p(history), _p(scratch), _p(sorted_idx), _p(sorted_key), _p(pairs), _p(pair_dt),
+                                    C.c_uint32(pair_cap), _p(n_pairs), _p(force), _p(torque), _stream()), "ledds_dem_query_f32")
 
 
 # ------------------------------------------------------------------------------------ coupled

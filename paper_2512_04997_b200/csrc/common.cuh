@@ -65,25 +65,41 @@ struct ledds_lbm {
     bool f32;              // populations are float (ledds_lbm_*_f32 calls); the coupled step takes fp64 handles only
 };
 
-// Kernel-side DEM parameters.
-struct DemDev {
+// Real type of the DEM path: double on the path of the configs; float = the ledds_dem_*_f32 calls (state, records,
+// history and all arithmetic of the step in single precision).
+template <typename T> struct Real;
+template <> struct Real<double> {
+    typedef double4 v4; typedef double2 v2;
+    static __host__ __device__ __forceinline__ v4 make4(double a, double b, double c, double d) { return make_double4(a, b, c, d); }
+    static __host__ __device__ constexpr double touch_eps() { return 1e-14; }   // |d^2 / (R_i + R_j)^2 - 1| below which Eq. (2) takes the square root
+};
+template <> struct Real<float> {
+    typedef float4 v4; typedef float2 v2;
+    static __host__ __device__ __forceinline__ v4 make4(float a, float b, float c, float d) { return make_float4(a, b, c, d); }
+    static __host__ __device__ constexpr float touch_eps() { return 1e-6f; }
+};
+
+// Kernel-side DEM parameters (passed by value), in the real type of the kernels.
+template <typename T>
+struct DemDevT {
     int n;
-    double lo[3], hi[3], L[3];
+    T lo[3], hi[3], L[3];
     float Lf[3], fmargin;          // single-precision first look of the detect kernel: (float)L, 2^-19 max L
     int bc[3];
-    double vw[18];
+    T vw[18];
     int nc[3];
-    double inv_h[3];
+    T inv_h[3];
     unsigned ncell, plane;         // cells in the grid, in one z-plane
     unsigned long long magic_row, magic_plane;   // ceil(2^40 / nc[0]), ceil(2^40 / plane): key decode without divisions
     int magic_ok;
-    double hmin;                   // smallest cell width of the grid: 2 R must not exceed it (LEDDS_ST_RADIUS_RANGE)
-    double dt, g[3], density;
-    double kn, kt, zeta, mu;
-    double kn_w, kt_w, zeta_w, mu_w;
-    double Ystar, Gstar, Ystar_w, Gstar_w;   // Hertz-Mindlin (A.6), (A.7): sphere-sphere / sphere-wall
+    T hmin;                        // smallest cell width of the grid: 2 R must not exceed it (LEDDS_ST_RADIUS_RANGE)
+    T dt, g[3], density;
+    T kn, kt, zeta, mu;
+    T kn_w, kt_w, zeta_w, mu_w;
+    T Ystar, Gstar, Ystar_w, Gstar_w;   // Hertz-Mindlin (A.6), (A.7): sphere-sphere / sphere-wall
     int maxc;
 };
+typedef DemDevT<double> DemDev;
 
 // Layout of the caller-owned DEM scratch buffer (byte offsets, all 256-B aligned).
 // "home" order: the order the library keeps the particle state in between the steps of one call.  It is the
@@ -126,7 +142,9 @@ struct DemHistory {
 
 struct ledds_dem {
     ledds_dem_params p;
-    DemDev d;
+    DemDev d;                      // parameters in double (host logic reads these whatever the precision)
+    DemDevT<float> df;             // the same in float, for the kernels of an fp32 handle
+    bool f32;                      // the handle's real type: ledds_dem_*_f32 calls only / fp64 calls only
     DemScratch s;
     DemHistory hs;
     int cur;                       // which generation of hq / hdt holds the latest contacts
@@ -142,7 +160,8 @@ struct ledds_dem {
 };
 
 // entry points implemented in dem.cu and used by coupled.cu
-struct DemKick { const double* f_ext; const double* m_ext; };   // external force / torque of a kick, [n][3] by caller id, or NULL
+template <typename T> struct DemKickT { const T* f_ext; const T* m_ext; };   // external force / torque of a kick, [n][3] by caller id, or NULL
+typedef DemKickT<double> DemKick;
 // caller's arrays -> home order (begins a call); a / alpha may be NULL (zeros)
 int ledds_dem_import(ledds_dem* h, const double* x, const double* v, const double* w, const double* a, const double* alpha,
                      const double* radius, void* history, void* scratch, cudaStream_t st);

@@ -342,6 +342,7 @@ static int coupled_step_t(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params
 {
     if (!lbm || !dem || !f || !cpl_scratch || !status || nsteps < 0) return LEDDS_EINVAL;
     if (lbm->f32 != (sizeof(T) == 4)) return LEDDS_EINVAL;                    // the handle fixes the population type
+    if (dem->f32) return LEDDS_EINVAL;                                        // the coupled step drives the fp64 DEM
     if (dem->d.n != 0 && (!x || !v || !w || !a || !alpha || !radius || !f_hyd || !m_hyd || !history || !scratch))
         return LEDDS_EINVAL;                                                 // an empty particle system needs none of them
     const void* ptrs[] = {f, x, v, w, a, alpha, radius, f_hyd, m_hyd, history, scratch, cpl_scratch, status};

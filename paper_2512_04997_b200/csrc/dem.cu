@@ -50,7 +50,8 @@
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
-__device__ __forceinline__ double dem_mass(const DemDev& P, double R) { return P.density * (4.0 / 3.0) * DEM_PI * R * R * R; }
+template <typename T>
+__device__ __forceinline__ T dem_mass(const DemDevT<T>& P, T R) { return P.density * (T(4.0) / T(3.0)) * T(DEM_PI) * R * R * R; }
 
 // ------------------------------------------------------------------------------ import / export
 // Block = DRIFT_BLOCK particles; the [n][3] arrays are walked as flat arrays (element e = 3 h + k).
@@ -58,12 +59,13 @@ __device__ __forceinline__ double dem_mass(const DemDev& P, double R) { return P
 
 // hid_src: the caller id of every home slot of the NEW home order (NULL: identity).  perm: the OLD home index of the
 // particle in new slot h (NULL: identity); the per-particle records of the last force evaluation move with it.
+template <typename T>
 __global__ void __launch_bounds__(DRIFT_BLOCK) dem_import_kernel(
-    int n, const uint32_t* __restrict__ hid_src, const uint32_t* __restrict__ perm, const double* __restrict__ x,
-    const double* __restrict__ v, const double* __restrict__ w, const double* __restrict__ a, const double* __restrict__ alpha,
-    const double* __restrict__ radius, uint32_t* __restrict__ hid, double4* __restrict__ hx, double* __restrict__ hv,
-    double* __restrict__ hw, double* __restrict__ ha, double* __restrict__ hal, const double* __restrict__ fm_old,
-    const uint2* __restrict__ row_old, double* __restrict__ fm_new, uint2* __restrict__ row_new)
+    int n, const uint32_t* __restrict__ hid_src, const uint32_t* __restrict__ perm, const T* __restrict__ x,
+    const T* __restrict__ v, const T* __restrict__ w, const T* __restrict__ a, const T* __restrict__ alpha,
+    const T* __restrict__ radius, uint32_t* __restrict__ hid, typename Real<T>::v4* __restrict__ hx, T* __restrict__ hv,
+    T* __restrict__ hw, T* __restrict__ ha, T* __restrict__ hal, const T* __restrict__ fm_old,
+    const uint2* __restrict__ row_old, T* __restrict__ fm_new, uint2* __restrict__ row_new)
 {
     const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * n;
 #pragma unroll
@@ -73,12 +75,12 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_import_kernel(
         const int h = (int)(e / 3), k = (int)(e - 3ll * h);
         const size_t src = 3 * (size_t)(hid_src ? hid_src[h] : (uint32_t)h) + k;
         hv[e] = v[src]; hw[e] = w[src];
-        ha[e] = a ? a[src] : 0.0; hal[e] = alpha ? alpha[src] : 0.0;
+        ha[e] = a ? a[src] : T(0.0); hal[e] = alpha ? alpha[src] : T(0.0);
     }
     const int h = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
     if (h >= n) return;
     const uint32_t i = hid_src ? hid_src[h] : (uint32_t)h;
-    hx[h] = make_double4(x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], radius[i]);
+    hx[h] = Real<T>::make4(x[3 * (size_t)i], x[3 * (size_t)i + 1], x[3 * (size_t)i + 2], radius[i]);
     hid[h] = i;
     const size_t o = perm ? perm[h] : (uint32_t)h;
     row_new[h] = row_old[o];
@@ -86,10 +88,11 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_import_kernel(
     for (int c = 0; c < 6; ++c) fm_new[6 * (size_t)h + c] = fm_old[6 * o + c];
 }
 
+template <typename T>
 __global__ void __launch_bounds__(DRIFT_BLOCK) dem_export_kernel(
-    int n, const uint32_t* __restrict__ hid, const double4* __restrict__ hx, const double* __restrict__ hv,
-    const double* __restrict__ hw, const double* __restrict__ ha, const double* __restrict__ hal, double* __restrict__ x,
-    double* __restrict__ v, double* __restrict__ w, double* __restrict__ a, double* __restrict__ alpha)
+    int n, const uint32_t* __restrict__ hid, const typename Real<T>::v4* __restrict__ hx, const T* __restrict__ hv,
+    const T* __restrict__ hw, const T* __restrict__ ha, const T* __restrict__ hal, T* __restrict__ x,
+    T* __restrict__ v, T* __restrict__ w, T* __restrict__ a, T* __restrict__ alpha)
 {
     const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * n;
 #pragma unroll
@@ -105,13 +108,14 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_export_kernel(
     }
     const int h = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
     if (h >= n || !x) return;
-    const double4 r = hx[h];
+    const typename Real<T>::v4 r = hx[h];
     const size_t i = hid[h];
     x[3 * i] = r.x; x[3 * i + 1] = r.y; x[3 * i + 2] = r.z;
 }
 
 // ------------------------------------------------------------------------------ drift + key
-__device__ __forceinline__ int dem_cell_coord(const DemDev& P, double x, int a)
+template <typename T>
+__device__ __forceinline__ int dem_cell_coord(const DemDevT<T>& P, T x, int a)
 {
     int c = (int)floor((x - P.lo[a]) * P.inv_h[a]);
     c = c < 0 ? 0 : c;
@@ -122,14 +126,14 @@ __device__ __forceinline__ int dem_cell_coord(const DemDev& P, double x, int a)
 // torque, which the caller indexes by particle id) is applied first, in the same pass: between two steps of one call
 // the state is read and written once instead of twice.  The new velocities and accelerations pass through shared
 // memory to the thread that owns the particle's packed (x, R) record.
-template <bool KICK>
+template <typename T, bool KICK>
 __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
-    const DemDev P, double4* __restrict__ hx, double* __restrict__ hv, double* __restrict__ hw, double* __restrict__ ha,
-    double* __restrict__ hal, const uint32_t* __restrict__ hid, const double* __restrict__ fm,
-    const double* __restrict__ f_ext, const double* __restrict__ m_ext, double* __restrict__ pvw,
+    const DemDevT<T> P, typename Real<T>::v4* __restrict__ hx, T* __restrict__ hv, T* __restrict__ hw, T* __restrict__ ha,
+    T* __restrict__ hal, const uint32_t* __restrict__ hid, const T* __restrict__ fm,
+    const T* __restrict__ f_ext, const T* __restrict__ m_ext, T* __restrict__ pvw,
     uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift, int32_t* __restrict__ status)
 {
-    __shared__ double sv[3 * DRIFT_BLOCK], sa[3 * DRIFT_BLOCK];
+    __shared__ T sv[3 * DRIFT_BLOCK], sa[3 * DRIFT_BLOCK];
     const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * P.n;
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
@@ -137,21 +141,21 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
         const long long e = e0 + le;
         if (e >= ne) break;
         const int h = (int)(e / 3), k = le % 3;                               // e0 is a multiple of 3
-        double vv = hv[e], wv = hw[e], av = ha[e], alv = hal[e];
+        T vv = hv[e], wv = hw[e], av = ha[e], alv = hal[e];
         if (KICK) {                                                           // same expressions as dem_kick_kernel
-            const double R = reinterpret_cast<const double*>(hx)[4 * (size_t)h + 3];
-            const double m = dem_mass(P, R), I = 0.4 * m * R * R;             // Eq. (21a)
+            const T R = reinterpret_cast<const T*>(hx)[4 * (size_t)h + 3];
+            const T m = dem_mass(P, R), I = T(0.4) * m * R * R;             // Eq. (21a)
             const size_t ie = (f_ext || m_ext) ? 3 * (size_t)hid[h] + k : 0;
-            const double Fq = fm[6 * (size_t)h + k] + (f_ext ? f_ext[ie] : 0.0), Mq = fm[6 * (size_t)h + 3 + k] + (m_ext ? m_ext[ie] : 0.0);
-            const double an = Fq / m + P.g[k], aln = Mq / I;                  // Eq. (18b), (19c)
-            vv = vv + (0.5 * P.dt) * (av + an);                               // Eq. (18c)
-            wv = wv + (0.5 * P.dt) * (alv + aln);                             // Eq. (19d)
+            const T Fq = fm[6 * (size_t)h + k] + (f_ext ? f_ext[ie] : T(0.0)), Mq = fm[6 * (size_t)h + 3 + k] + (m_ext ? m_ext[ie] : T(0.0));
+            const T an = Fq / m + P.g[k], aln = Mq / I;                  // Eq. (18b), (19c)
+            vv = vv + (T(0.5) * P.dt) * (av + an);                               // Eq. (18c)
+            wv = wv + (T(0.5) * P.dt) * (alv + aln);                             // Eq. (19d)
             av = an; alv = aln;
             hv[e] = vv; hw[e] = wv; ha[e] = av; hal[e] = alv;
         }
         if (drift) {
-            pvw[6 * (size_t)h + k] = vv + (0.5 * P.dt) * av;                  // predictor (G11)
-            pvw[6 * (size_t)h + 3 + k] = wv + (0.5 * P.dt) * alv;
+            pvw[6 * (size_t)h + k] = vv + (T(0.5) * P.dt) * av;                  // predictor (G11)
+            pvw[6 * (size_t)h + 3 + k] = wv + (T(0.5) * P.dt) * alv;
         } else {
             pvw[6 * (size_t)h + k] = vv;
             pvw[6 * (size_t)h + 3 + k] = wv;
@@ -161,25 +165,25 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
     __syncthreads();
     const int h = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
     if (h >= P.n) return;
-    const double4 r = hx[h];
-    double xn[3] = {r.x, r.y, r.z};
+    const typename Real<T>::v4 r = hx[h];
+    T xn[3] = {r.x, r.y, r.z};
     if (drift) {
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            double xv = xn[k] + P.dt * sv[3 * threadIdx.x + k] + (0.5 * P.dt * P.dt) * sa[3 * threadIdx.x + k];   // Eq. (18a)
+            T xv = xn[k] + P.dt * sv[3 * threadIdx.x + k] + (T(0.5) * P.dt * P.dt) * sa[3 * threadIdx.x + k];   // Eq. (18a)
             if (!P.bc[k]) {
                 if (xv >= P.hi[k]) xv -= P.L[k];
                 else if (xv < P.lo[k]) xv += P.L[k];
             }
             xn[k] = xv;
         }
-        hx[h] = make_double4(xn[0], xn[1], xn[2], r.w);
+        hx[h] = Real<T>::make4(xn[0], xn[1], xn[2], r.w);
     }
     const int cx = dem_cell_coord(P, xn[0], 0), cy = dem_cell_coord(P, xn[1], 1), cz = dem_cell_coord(P, xn[2], 2);
     key[h] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
     idx[h] = (uint32_t)h;
     // input contract (include/ledds.h): 2 R <= cell width, centres inside a walled box
-    int st = 2.0 * r.w > P.hmin ? LEDDS_ST_RADIUS_RANGE : 0;
+    int st = T(2.0) * r.w > P.hmin ? LEDDS_ST_RADIUS_RANGE : 0;
 #pragma unroll
     for (int a = 0; a < 3; ++a)
         if (P.bc[a] && !(xn[a] >= P.lo[a] && xn[a] <= P.hi[a])) st |= LEDDS_ST_OUT_OF_BOX;
@@ -189,7 +193,8 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
 // key -> (cx, cy, cz).  The two divisions by run-time constants are multiplications by host-computed reciprocals:
 // floor(k m / 2^40) with m = ceil(2^40 / d) equals floor(k / d) whenever k d <= 2^40 (the host checks it for the
 // largest key and both divisors; else the plain divisions are used).
-__device__ __forceinline__ void dem_cell_of_key(const DemDev& P, uint32_t key, int& c0, int& c1, int& c2)
+template <typename T>
+__device__ __forceinline__ void dem_cell_of_key(const DemDevT<T>& P, uint32_t key, int& c0, int& c1, int& c2)
 {
     uint32_t r, z;
     if (P.magic_ok) {
@@ -425,9 +430,10 @@ __global__ void dem_ranges_kernel(int n, const uint32_t* __restrict__ skey, cons
 }
 
 // sh0[s] = home index of the particle at key-sorted position s (a nearly sequential read of the home records)
-__global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sh0,
+template <typename T>
+__global__ void dem_gather_kernel(const DemDevT<T> P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sh0,
                                   const uint32_t* __restrict__ sid_tmp, const uint2* __restrict__ cell_range,
-                                  const double4* __restrict__ hx, double4* __restrict__ xr_s, float4* __restrict__ xf_s,
+                                  const typename Real<T>::v4* __restrict__ hx, typename Real<T>::v4* __restrict__ xr_s, float4* __restrict__ xf_s,
                                   uint32_t* __restrict__ sid, uint32_t* __restrict__ sh, uint32_t* __restrict__ nback)
 {
     const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
@@ -437,22 +443,23 @@ __global__ void dem_gather_kernel(const DemDev P, const uint32_t* __restrict__ s
     uint32_t s = cr.x;
     for (uint32_t t = cr.x; t < cr.y; ++t) s += sid_tmp[t] < id;                   // ids are distinct
     const uint32_t h = sh0[s0];
-    const double2* src = reinterpret_cast<const double2*>(hx + h);
-    const double2 a = __ldg(src), b = __ldg(src + 1);
-    xr_s[s] = make_double4(a.x, a.y, b.x, b.y);
+    const typename Real<T>::v2* src = reinterpret_cast<const typename Real<T>::v2*>(hx + h);
+    const typename Real<T>::v2 a = __ldg(src), b = __ldg(src + 1);
+    xr_s[s] = Real<T>::make4(a.x, a.y, b.x, b.y);
     sid[s] = id;
     sh[s] = h;
     nback[s] = 0u;
     // single-precision copy (x - lo, R) for the detect kernel's first look at a candidate (dem_near).  A particle
     // further than 2 L from the box corner (or not finite) gets NaN: it passes every first look.
-    const double rx = a.x - P.lo[0], ry = a.y - P.lo[1], rz = b.x - P.lo[2];
-    const bool sane = fabs(rx) <= 2.0 * P.L[0] && fabs(ry) <= 2.0 * P.L[1] && fabs(rz) <= 2.0 * P.L[2];
+    const T rx = a.x - P.lo[0], ry = a.y - P.lo[1], rz = b.x - P.lo[2];
+    const bool sane = fabs(rx) <= T(2.0) * P.L[0] && fabs(ry) <= T(2.0) * P.L[1] && fabs(rz) <= T(2.0) * P.L[2];
     const float qnan = __int_as_float(0x7fc00000);
     xf_s[s] = sane ? make_float4((float)rx, (float)ry, (float)rz, (float)b.y) : make_float4(qnan, qnan, qnan, qnan);
 }
 
 // ------------------------------------------------------------------------------ contact law
-__device__ __forceinline__ void cross3(const double* a, const double* b, double* c)
+template <typename T>
+__device__ __forceinline__ void cross3(const T* a, const T* b, T* c)
 {
     c[0] = a[1] * b[2] - a[2] * b[1];
     c[1] = a[2] * b[0] - a[0] * b[2];
@@ -460,14 +467,15 @@ __device__ __forceinline__ void cross3(const double* a, const double* b, double*
 }
 
 // r_i - r_j with the nearest image on periodic axes
-__device__ __forceinline__ void dem_min_image(const DemDev& P, const double* xi, const double* xj, double* d)
+template <typename T>
+__device__ __forceinline__ void dem_min_image(const DemDevT<T>& P, const T* xi, const T* xj, T* d)
 {
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         d[a] = xi[a] - xj[a];
         if (!P.bc[a]) {
-            if (d[a] > 0.5 * P.L[a]) d[a] -= P.L[a];
-            else if (d[a] < -0.5 * P.L[a]) d[a] += P.L[a];
+            if (d[a] > T(0.5) * P.L[a]) d[a] -= P.L[a];
+            else if (d[a] < -T(0.5) * P.L[a]) d[a] += P.L[a];
         }
     }
 }
@@ -475,33 +483,34 @@ __device__ __forceinline__ void dem_min_image(const DemDev& P, const double* xi,
 // Force of one contact in its canonical orientation (i < j, or j = wall), Eq. (4)-(15).
 // en, dn: unit normal from j to i and overlap.  dt3: in = previous delta_t, out = new delta_t.
 // F = force on i; T = e_n x F_t (torque on a body of radius R is -R T, Eq. 15).
-__device__ __forceinline__ void dem_pair_force(const double* en, double dn, const double* vi, const double* wi,
-                                               double Ri, const double* vj, const double* wj, double Rj,
-                                               double kn, double kt, double gn, double gt, double mu,
-                                               double dt_hist, double* dt3, double* F, double* T)
+template <typename T>
+__device__ __forceinline__ void dem_pair_force(const T* en, T dn, const T* vi, const T* wi,
+                                               T Ri, const T* vj, const T* wj, T Rj,
+                                               T kn, T kt, T gn, T gt, T mu,
+                                               T dt_hist, T* dt3, T* F, T* Tq)
 {
-    double rw[3], rwxe[3], vrel[3], vt[3], Ft[3];
+    T rw[3], rwxe[3], vrel[3], vt[3], Ft[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) rw[a] = Ri * wi[a] + Rj * wj[a];
     cross3(rw, en, rwxe);
 #pragma unroll
     for (int a = 0; a < 3; ++a) vrel[a] = (vi[a] - vj[a]) - rwxe[a];                  // Eq. (11)
-    const double vn = vrel[0] * en[0] + vrel[1] * en[1] + vrel[2] * en[2];
+    const T vn = vrel[0] * en[0] + vrel[1] * en[1] + vrel[2] * en[2];
 #pragma unroll
     for (int a = 0; a < 3; ++a) vt[a] = vrel[a] - vn * en[a];                         // Eq. (12)
-    const double fn = kn * dn - gn * vn;                                              // Eq. (10)
-    const double dte = dt3[0] * en[0] + dt3[1] * en[1] + dt3[2] * en[2];
+    const T fn = kn * dn - gn * vn;                                              // Eq. (10)
+    const T dte = dt3[0] * en[0] + dt3[1] * en[1] + dt3[2] * en[2];
 #pragma unroll
     for (int a = 0; a < 3; ++a) dt3[a] = (dt3[a] - dte * en[a]) + dt_hist * vt[a];    // Eq. (13)
 #pragma unroll
     for (int a = 0; a < 3; ++a) Ft[a] = -kt * dt3[a] - gt * vt[a];                    // Eq. (4)
-    const double ft = sqrt(Ft[0] * Ft[0] + Ft[1] * Ft[1] + Ft[2] * Ft[2]), fmax = mu * fabs(fn);
+    const T ft = sqrt(Ft[0] * Ft[0] + Ft[1] * Ft[1] + Ft[2] * Ft[2]), fmax = mu * fabs(fn);
     if (ft > fmax) {                                                                  // Eq. (5)
-        const double s = fmax / ft;
+        const T s = fmax / ft;
 #pragma unroll
         for (int a = 0; a < 3; ++a) { Ft[a] *= s; dt3[a] = -(Ft[a] + gt * vt[a]) / kt; }
     }
-    cross3(en, Ft, T);
+    cross3(en, Ft, Tq);
 #pragma unroll
     for (int a = 0; a < 3; ++a) F[a] = fn * en[a] + Ft[a];
 }
@@ -524,20 +533,20 @@ __device__ __forceinline__ void dem_pair_force(const double* en, double dn, cons
 // 2 zeta sqrt(k m*) (G5).  HERTZ = true: Hertz-Mindlin: (A.1) k_n = 4/3 Y* sqrt(R* d_n),
 // k_t = 8 G* sqrt(R* d_n); (A.3)-(A.4) S_n = 2 Y* sqrt(R* d_n), S_t = 8 G* sqrt(R* d_n); (A.2) gamma =
 // 2 sqrt(5/6) zeta sqrt(S m*), zeta = -beta of (A.5).  Y*, G* of (A.6)-(A.7) come from the host (one material).
-template <bool HERTZ>
-__device__ __forceinline__ void dem_coefficients(double kn0, double kt0, double Ystar, double Gstar, double zeta, double mstar,
-                                                 double Rstar, double dn, double& kn, double& kt, double& gn, double& gt)
+template <typename T, bool HERTZ>
+__device__ __forceinline__ void dem_coefficients(T kn0, T kt0, T Ystar, T Gstar, T zeta, T mstar,
+                                                 T Rstar, T dn, T& kn, T& kt, T& gn, T& gt)
 {
     if (HERTZ) {
-        const double sq = sqrt(Rstar * dn);
-        kn = (4.0 / 3.0) * Ystar * sq;
-        kt = 8.0 * Gstar * sq;
-        const double Sn = 2.0 * Ystar * sq, St = 8.0 * Gstar * sq;
-        gn = 2.0 * sqrt(5.0 / 6.0) * zeta * sqrt(Sn * mstar);
-        gt = 2.0 * sqrt(5.0 / 6.0) * zeta * sqrt(St * mstar);
+        const T sq = sqrt(Rstar * dn);
+        kn = (T(4.0) / T(3.0)) * Ystar * sq;
+        kt = T(8.0) * Gstar * sq;
+        const T Sn = T(2.0) * Ystar * sq, St = T(8.0) * Gstar * sq;
+        gn = T(2.0) * sqrt(T(5.0) / T(6.0)) * zeta * sqrt(Sn * mstar);
+        gt = T(2.0) * sqrt(T(5.0) / T(6.0)) * zeta * sqrt(St * mstar);
     } else {
         kn = kn0; kt = kt0;
-        gn = 2.0 * zeta * sqrt(kn * mstar); gt = 2.0 * zeta * sqrt(kt * mstar);
+        gn = T(2.0) * zeta * sqrt(kn * mstar); gt = T(2.0) * zeta * sqrt(kt * mstar);
     }
 }
 
@@ -545,8 +554,8 @@ __device__ __forceinline__ void dem_coefficients(double kn0, double kt0, double 
 // Stored coordinates are within 2 L of the origin, so each is off by <= L 2^-23, a difference by <= L 2^-22 (+ the
 // rounding of L itself on a wrapped axis) and the distance by < 5e-7 L; fmargin = 2^-19 max L = 1.9e-6 L covers
 // that four times over and the factor 1.00001 the roundings of the squares.  NaN records compare as "maybe".
-template <bool PERIODIC>
-__device__ __forceinline__ bool dem_near(const DemDev& P, const float4& a, const float4& b)
+template <typename T, bool PERIODIC>
+__device__ __forceinline__ bool dem_near(const DemDevT<T>& P, const float4& a, const float4& b)
 {
     float d[3] = {a.x - b.x, a.y - b.y, a.z - b.z};
     if (PERIODIC) {
@@ -563,17 +572,17 @@ __device__ __forceinline__ bool dem_near(const DemDev& P, const float4& a, const
 }
 
 // PERIODIC = false: no axis is periodic, the nearest image is the particle itself
-template <bool PERIODIC>
-__device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, const double4& b)
+template <typename T, bool PERIODIC>
+__device__ __forceinline__ bool dem_touch(const DemDevT<T>& P, const typename Real<T>::v4& a, const typename Real<T>::v4& b)
 {
-    const double xa[3] = {a.x, a.y, a.z}, xb[3] = {b.x, b.y, b.z};
-    double d[3] = {xa[0] - xb[0], xa[1] - xb[1], xa[2] - xb[2]};
+    const T xa[3] = {a.x, a.y, a.z}, xb[3] = {b.x, b.y, b.z};
+    T d[3] = {xa[0] - xb[0], xa[1] - xb[1], xa[2] - xb[2]};
     if (PERIODIC) dem_min_image(P, xa, xb, d);
-    const double d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
-    const double sr = a.w + b.w, s2 = sr * sr;
-    if (d2 > s2 * (1.0 + 1e-14)) return false;
-    if (d2 < s2 * (1.0 - 1e-14)) return true;
-    return sr - sqrt(d2) > 0.0;                                                       // Eq. (2), (6), strict (G7)
+    const T d2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+    const T sr = a.w + b.w, s2 = sr * sr;
+    if (d2 > s2 * (T(1.0) + Real<T>::touch_eps())) return false;
+    if (d2 < s2 * (T(1.0) - Real<T>::touch_eps())) return true;
+    return sr - sqrt(d2) > T(0.0);                                                       // Eq. (2), (6), strict (G7)
 }
 
 // ------------------------------------------------------------------------------ detect
@@ -585,9 +594,9 @@ __device__ __forceinline__ bool dem_touch(const DemDev& P, const double4& a, con
 // which differs from run to run); dem_fill_kernel puts every list into the order of the partner ids.
 // (One thread per (particle, row) -- nine times the threads, a ninth of the work each -- was measured and is slower:
 // 0.61 against 0.52 ms in the dense 4 M state, 0.29 against 0.15 ms in the dilute one.)
-template <bool PERIODIC>
+template <typename T, bool PERIODIC>
 __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_kernel(
-    const DemDev P, const uint32_t* __restrict__ skey, const double4* __restrict__ xr_s, const float4* __restrict__ xf_s,
+    const DemDevT<T> P, const uint32_t* __restrict__ skey, const typename Real<T>::v4* __restrict__ xr_s, const float4* __restrict__ xf_s,
     const uint2* __restrict__ cell_range, uint32_t* __restrict__ nfwd, uint32_t* __restrict__ nback, uint32_t* __restrict__ cand,
     int32_t* __restrict__ status)
 {
@@ -595,7 +604,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
     if (s >= P.n) return;
     const uint32_t maxc = (uint32_t)P.maxc;
     const uint32_t key = skey[s];
-    const double4 mine = xr_s[s];
+    const typename Real<T>::v4 mine = xr_s[s];
     const float4 minef = xf_s[s];
     int st = 0;
 
@@ -658,13 +667,13 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
             }
 #pragma unroll
             for (int b = 0; b < DETECT_NB; ++b) {
-                nn[b] = dem_near<PERIODIC>(P, minef, fc[b]) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
+                nn[b] = dem_near<T, PERIODIC>(P, minef, fc[b]) & (b == 0 || tt[b] != tt[b > 0 ? b - 1 : 0]);
                 any |= nn[b];
             }
-            if (any) {                                                             // Eq. (2) in double for the few that pass
+            if (any) {                                                             // Eq. (2) in T for the few that pass
 #pragma unroll
                 for (int b = 0; b < DETECT_NB; ++b)
-                    if (nn[b] && dem_touch<PERIODIC>(P, mine, xr_s[tt[b]])) enter(tt[b]);
+                    if (nn[b] && dem_touch<T, PERIODIC>(P, mine, xr_s[tt[b]])) enter(tt[b]);
             }
         }
     }
@@ -676,17 +685,17 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
             if (qy < 0 || qy >= P.nc[1]) { if (P.bc[1]) continue; qy = qy < 0 ? qy + P.nc[1] : qy - P.nc[1]; }
             const uint2 r = cell_range[(size_t)P.nc[0] * (size_t)(qy + P.nc[1] * qz) + wc];
             for (uint32_t t = max(r.x, (uint32_t)s + 1u); t < r.y; ++t)
-                if (dem_near<PERIODIC>(P, minef, xf_s[t]) && dem_touch<PERIODIC>(P, mine, xr_s[t])) enter(t);
+                if (dem_near<T, PERIODIC>(P, minef, xf_s[t]) && dem_touch<T, PERIODIC>(P, mine, xr_s[t])) enter(t);
         }
     }
     // walls: static infinite particles; overlap decided as the oracle does, R - distance > 0
-    const double xm[3] = {mine.x, mine.y, mine.z};
+    const T xm[3] = {mine.x, mine.y, mine.z};
 #pragma unroll
     for (int wl = 0; wl < 6; ++wl) {
         const int ax = wl >> 1;
         if (!P.bc[ax]) continue;
-        const double dist = (wl & 1) ? P.hi[ax] - xm[ax] : xm[ax] - P.lo[ax];
-        if (mine.w - dist > 0.0) own(DEM_WALL + (uint32_t)wl);
+        const T dist = (wl & 1) ? P.hi[ax] - xm[ax] : xm[ax] - P.lo[ax];
+        if (mine.w - dist > T(0.0)) own(DEM_WALL + (uint32_t)wl);
     }
     flush();
     nfwd[s] = nf;
@@ -780,11 +789,12 @@ __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t 
 #define DEM_NO_PREV 0xffffffffu
 struct DemEnds { uint32_t *s, *t, *hs, *ht, *prev; };   // per contact end, CSR order
 
+template <typename T>
 __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ nfwd,
                                                                 const uint32_t* __restrict__ nback, const uint32_t* __restrict__ cand,
                                                                 const uint32_t* __restrict__ sid, const uint32_t* __restrict__ sh,
                                                                 const uint32_t* __restrict__ off, uint2* __restrict__ row,
-                                                                double* __restrict__ fm, const uint32_t* __restrict__ hq_prev,
+                                                                T* __restrict__ fm, const uint32_t* __restrict__ hq_prev,
                                                                 const DemEnds E, uint32_t* __restrict__ hq, int32_t* __restrict__ status)
 {
     extern __shared__ uint2 tq[];                        // uint2 [maxc][CONTACT_BLOCK]: (partner code, partner id); then uint32 [maxc][CONTACT_BLOCK]
@@ -799,7 +809,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
         if (old.y) {                                                                // the last contact has just ended
             row[h] = make_uint2(0u, 0u);
 #pragma unroll
-            for (int c = 0; c < 6; ++c) fm[6 * (size_t)h + c] = 0.0;
+            for (int c = 0; c < 6; ++c) fm[6 * (size_t)h + c] = T(0.0);
         }
         return;
     }
@@ -881,82 +891,82 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
 // and the sums R_i w_i + R_j w_j, m_i m_j, m_i + m_j commute; no FMA contraction in this file), so F_ij = -F_ji and
 // M_i / R_i = M_j / R_j hold bit for bit, and what the owner with the higher id computes is exactly the negative of the
 // canonical (i < j) evaluation of the oracle.
-template <bool HERTZ>
+template <typename T, bool HERTZ>
 __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_kernel(
-    const DemDev P, const double4* __restrict__ xr_s, const double* __restrict__ pvw, const uint32_t* __restrict__ off,
-    const DemEnds E, const uint32_t* __restrict__ sh, double* __restrict__ fm, const double* __restrict__ hdt_prev,
-    double* __restrict__ hdt_new, int32_t* __restrict__ status, double dt_hist)
+    const DemDevT<T> P, const typename Real<T>::v4* __restrict__ xr_s, const T* __restrict__ pvw, const uint32_t* __restrict__ off,
+    const DemEnds E, const uint32_t* __restrict__ sh, T* __restrict__ fm, const T* __restrict__ hdt_prev,
+    T* __restrict__ hdt_new, int32_t* __restrict__ status, T dt_hist)
 {
     // every warp works on its own FORCE_PW particles with its own piece of shared memory: no block-wide barrier
     __shared__ uint32_t s_off_all[FORCE_WARPS][FORCE_PW + 1];
-    __shared__ double stage_all[FORCE_WARPS][6][32];
-    __shared__ double sacc_all[FORCE_WARPS][6][FORCE_PW];
+    __shared__ T stage_all[FORCE_WARPS][6][32];
+    __shared__ T sacc_all[FORCE_WARPS][6][FORCE_PW];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int s0 = (blockIdx.x * FORCE_WARPS + warp) * FORCE_PW;
     if (s0 >= P.n) return;
     const int np = min(FORCE_PW, P.n - s0);
     uint32_t* s_off = s_off_all[warp];
-    double (*stage)[32] = stage_all[warp];
-    double (*sacc)[FORCE_PW] = sacc_all[warp];
+    T (*stage)[32] = stage_all[warp];
+    T (*sacc)[FORCE_PW] = sacc_all[warp];
     const uint32_t e_begin = off[s0], e_end = off[s0 + np];
     if (e_begin == e_end) return;                                                   // no contact among these particles (warp-uniform)
     for (int i = lane; i <= np; i += 32) s_off[i] = off[s0 + i];
-    for (int i = lane; i < 6 * FORCE_PW; i += 32) (&sacc[0][0])[i] = 0.0;
+    for (int i = lane; i < 6 * FORCE_PW; i += 32) (&sacc[0][0])[i] = T(0.0);
     __syncwarp();
     int st = 0;
 
     for (uint32_t chunk = e_begin; chunk < e_end; chunk += 32) {
         const uint32_t e = chunk + (uint32_t)lane;
-        double Fe[3] = {0, 0, 0}, Me[3] = {0, 0, 0};
+        T Fe[3] = {0, 0, 0}, Me[3] = {0, 0, 0};
         if (e < e_end) {
             const uint32_t s = E.s[e], t = E.t[e], hs = E.hs[e], ht = E.ht[e], prev = E.prev[e];
             const bool wall = t >= DEM_WALL;
             // all loads of the end, issued together
-            const double4 m4 = xr_s[s];
-            const double2* rm = reinterpret_cast<const double2*>(pvw + 6 * (size_t)hs);
-            const double2 ma = rm[0], mb = rm[1], mc = rm[2];
-            const double4 o4 = xr_s[wall ? s : t];
-            const double2* ro = reinterpret_cast<const double2*>(pvw + 6 * (size_t)(wall ? hs : ht));
-            const double2 oa = ro[0], ob = ro[1], oc = ro[2];
-            double dt3[3] = {0, 0, 0};                                                 // previous delta_t of this end, seen from its owner
+            const typename Real<T>::v4 m4 = xr_s[s];
+            const typename Real<T>::v2* rm = reinterpret_cast<const typename Real<T>::v2*>(pvw + 6 * (size_t)hs);
+            const typename Real<T>::v2 ma = rm[0], mb = rm[1], mc = rm[2];
+            const typename Real<T>::v4 o4 = xr_s[wall ? s : t];
+            const typename Real<T>::v2* ro = reinterpret_cast<const typename Real<T>::v2*>(pvw + 6 * (size_t)(wall ? hs : ht));
+            const typename Real<T>::v2 oa = ro[0], ob = ro[1], oc = ro[2];
+            T dt3[3] = {0, 0, 0};                                                 // previous delta_t of this end, seen from its owner
             if (prev != DEM_NO_PREV) {
-                const double* d = hdt_prev + 3 * (size_t)prev;
+                const T* d = hdt_prev + 3 * (size_t)prev;
                 dt3[0] = d[0]; dt3[1] = d[1]; dt3[2] = d[2];
             }
-            const double xm[3] = {m4.x, m4.y, m4.z}, Rm = m4.w;
-            const double vm[3] = {ma.x, ma.y, mb.x}, wm[3] = {mb.y, mc.x, mc.y};
-            double F[3] = {0, 0, 0}, T[3] = {0, 0, 0}, kn, kt, gn, gt;
+            const T xm[3] = {m4.x, m4.y, m4.z}, Rm = m4.w;
+            const T vm[3] = {ma.x, ma.y, mb.x}, wm[3] = {mb.y, mc.x, mc.y};
+            T F[3] = {0, 0, 0}, Tq[3] = {0, 0, 0}, kn, kt, gn, gt;
             if (!wall) {
-                const double xo[3] = {o4.x, o4.y, o4.z}, Ro = o4.w;
-                const double vo[3] = {oa.x, oa.y, ob.x}, wo[3] = {ob.y, oc.x, oc.y};
-                double d[3];
+                const T xo[3] = {o4.x, o4.y, o4.z}, Ro = o4.w;
+                const T vo[3] = {oa.x, oa.y, ob.x}, wo[3] = {ob.y, oc.x, oc.y};
+                T d[3];
                 dem_min_image(P, xm, xo, d);
-                const double dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-                const double dn = (Rm + Ro) - dist;                                    // Eq. (6)
-                if (dist == 0.0) {
+                const T dist = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+                const T dn = (Rm + Ro) - dist;                                    // Eq. (6)
+                if (dist == T(0.0)) {
                     st |= LEDDS_ST_COINCIDENT;                                         // pair skipped, delta_t = 0 (as the oracle)
-                    dt3[0] = dt3[1] = dt3[2] = 0.0;
+                    dt3[0] = dt3[1] = dt3[2] = T(0.0);
                 } else {
-                    const double en[3] = {d[0] / dist, d[1] / dist, d[2] / dist};      // Eq. (7)
-                    const double mi = dem_mass(P, Rm), mj = dem_mass(P, Ro);
-                    const double mstar = mi * mj / (mi + mj);                          // (A.9)
-                    dem_coefficients<HERTZ>(P.kn, P.kt, P.Ystar, P.Gstar, P.zeta, mstar, Rm * Ro / (Rm + Ro), dn, kn, kt, gn, gt);
-                    dem_pair_force(en, dn, vm, wm, Rm, vo, wo, Ro, kn, kt, gn, gt, P.mu, dt_hist, dt3, F, T);
+                    const T en[3] = {d[0] / dist, d[1] / dist, d[2] / dist};      // Eq. (7)
+                    const T mi = dem_mass(P, Rm), mj = dem_mass(P, Ro);
+                    const T mstar = mi * mj / (mi + mj);                          // (A.9)
+                    dem_coefficients<T, HERTZ>(P.kn, P.kt, P.Ystar, P.Gstar, P.zeta, mstar, Rm * Ro / (Rm + Ro), dn, kn, kt, gn, gt);
+                    dem_pair_force(en, dn, vm, wm, Rm, vo, wo, Ro, kn, kt, gn, gt, P.mu, dt_hist, dt3, F, Tq);
                 }
             } else {                                                                   // a wall: R* = R_i, m* = m_i
                 const int wl = (int)(t - DEM_WALL), ax = wl >> 1, side = wl & 1;
-                const double xa = ax == 0 ? xm[0] : (ax == 1 ? xm[1] : xm[2]);          // selects: the arrays stay in registers
-                const double dist = side ? P.hi[ax] - xa : xa - P.lo[ax];
-                const double dn = Rm - dist;
-                const double sgn = side ? -1.0 : 1.0;
-                const double en[3] = {ax == 0 ? sgn : 0.0, ax == 1 ? sgn : 0.0, ax == 2 ? sgn : 0.0};
-                const double vj[3] = {P.vw[wl * 3], P.vw[wl * 3 + 1], P.vw[wl * 3 + 2]}, wj[3] = {0, 0, 0};
-                dem_coefficients<HERTZ>(P.kn_w, P.kt_w, P.Ystar_w, P.Gstar_w, P.zeta_w, dem_mass(P, Rm), Rm, dn, kn, kt, gn, gt);
-                dem_pair_force(en, dn, vm, wm, Rm, vj, wj, 0.0, kn, kt, gn, gt, P.mu_w, dt_hist, dt3, F, T);
+                const T xa = ax == 0 ? xm[0] : (ax == 1 ? xm[1] : xm[2]);          // selects: the arrays stay in registers
+                const T dist = side ? P.hi[ax] - xa : xa - P.lo[ax];
+                const T dn = Rm - dist;
+                const T sgn = side ? -T(1.0) : T(1.0);
+                const T en[3] = {ax == 0 ? sgn : T(0.0), ax == 1 ? sgn : T(0.0), ax == 2 ? sgn : T(0.0)};
+                const T vj[3] = {P.vw[wl * 3], P.vw[wl * 3 + 1], P.vw[wl * 3 + 2]}, wj[3] = {0, 0, 0};
+                dem_coefficients<T, HERTZ>(P.kn_w, P.kt_w, P.Ystar_w, P.Gstar_w, P.zeta_w, dem_mass(P, Rm), Rm, dn, kn, kt, gn, gt);
+                dem_pair_force(en, dn, vm, wm, Rm, vj, wj, T(0.0), kn, kt, gn, gt, P.mu_w, dt_hist, dt3, F, Tq);
             }
 #pragma unroll
-            for (int a = 0; a < 3; ++a) { Fe[a] = F[a]; Me[a] = Rm * (-T[a]); }         // Eq. (15)
-            double* nd = hdt_new + 3 * (size_t)e;
+            for (int a = 0; a < 3; ++a) { Fe[a] = F[a]; Me[a] = Rm * (-Tq[a]); }         // Eq. (15)
+            T* nd = hdt_new + 3 * (size_t)e;
             nd[0] = dt3[0]; nd[1] = dt3[1]; nd[2] = dt3[2];
         }
 #pragma unroll
@@ -966,7 +976,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_ker
         for (int i = lane; i < np; i += 32) {
             const uint32_t lo = max(s_off[i], chunk), hi = min(s_off[i + 1], chunk + 32u);
             if (lo < hi) {
-                double a6[6];
+                T a6[6];
 #pragma unroll
                 for (int c = 0; c < 6; ++c) a6[c] = sacc[c][i];
                 for (uint32_t e2 = lo; e2 < hi; ++e2)
@@ -984,7 +994,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_ker
         const uint32_t h = sh[s0 + i];
         bool finite = true;
 #pragma unroll
-        for (int c = 0; c < 6; ++c) { const double v = sacc[c][i]; fm[6 * (size_t)h + c] = v; finite = finite && isfinite(v); }
+        for (int c = 0; c < 6; ++c) { const T v = sacc[c][i]; fm[6 * (size_t)h + c] = v; finite = finite && isfinite(v); }
         if (!finite) st |= LEDDS_ST_NONFINITE;
     }
     if (st) atomicOr(status, st);
@@ -992,22 +1002,23 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_ker
 
 // ------------------------------------------------------------------------------ kick
 // One thread per vector component (element e = 3 h + k of the flat home arrays): coalesced.
-__global__ void dem_kick_kernel(const DemDev P, const double4* __restrict__ hx, const uint32_t* __restrict__ hid,
-                                const double* __restrict__ fm, const double* __restrict__ f_ext, const double* __restrict__ m_ext,
-                                double* __restrict__ hv, double* __restrict__ hw, double* __restrict__ ha, double* __restrict__ hal,
+template <typename T>
+__global__ void dem_kick_kernel(const DemDevT<T> P, const typename Real<T>::v4* __restrict__ hx, const uint32_t* __restrict__ hid,
+                                const T* __restrict__ fm, const T* __restrict__ f_ext, const T* __restrict__ m_ext,
+                                T* __restrict__ hv, T* __restrict__ hw, T* __restrict__ ha, T* __restrict__ hal,
                                 int only_accel)
 {
     const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= 3ll * P.n) return;
     const int h = (int)(e / 3), k = (int)(e - 3ll * h);
-    const double R = reinterpret_cast<const double*>(hx)[4 * (size_t)h + 3];
-    const double m = dem_mass(P, R), I = 0.4 * m * R * R;                             // Eq. (21a)
+    const T R = reinterpret_cast<const T*>(hx)[4 * (size_t)h + 3];
+    const T m = dem_mass(P, R), I = T(0.4) * m * R * R;                             // Eq. (21a)
     const size_t ie = (f_ext || m_ext) ? 3 * (size_t)hid[h] + k : 0;
-    const double Fq = fm[6 * (size_t)h + k] + (f_ext ? f_ext[ie] : 0.0), Mq = fm[6 * (size_t)h + 3 + k] + (m_ext ? m_ext[ie] : 0.0);
-    const double an = Fq / m + P.g[k], aln = Mq / I;                                  // Eq. (18b), (19c)
+    const T Fq = fm[6 * (size_t)h + k] + (f_ext ? f_ext[ie] : T(0.0)), Mq = fm[6 * (size_t)h + 3 + k] + (m_ext ? m_ext[ie] : T(0.0));
+    const T an = Fq / m + P.g[k], aln = Mq / I;                                  // Eq. (18b), (19c)
     if (!only_accel) {
-        hv[e] = hv[e] + (0.5 * P.dt) * (ha[e] + an);                                  // Eq. (18c)
-        hw[e] = hw[e] + (0.5 * P.dt) * (hal[e] + aln);                                // Eq. (19d)
+        hv[e] = hv[e] + (T(0.5) * P.dt) * (ha[e] + an);                                  // Eq. (18c)
+        hw[e] = hw[e] + (T(0.5) * P.dt) * (hal[e] + aln);                                // Eq. (19d)
     }
     ha[e] = an;
     hal[e] = aln;
@@ -1032,8 +1043,9 @@ __global__ void dem_pair_count_kernel(int n, const uint32_t* __restrict__ pos_of
     cnt[p] = c;
 }
 
-__global__ void dem_unpack_fm_kernel(int n, const uint32_t* __restrict__ hid, const double* __restrict__ fm,
-                                     double* __restrict__ force, double* __restrict__ torque)
+template <typename T>
+__global__ void dem_unpack_fm_kernel(int n, const uint32_t* __restrict__ hid, const T* __restrict__ fm,
+                                     T* __restrict__ force, T* __restrict__ torque)
 {
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     if (h >= n) return;
@@ -1083,10 +1095,11 @@ __global__ void __launch_bounds__(1024) dem_block_scan_kernel(int n, const uint3
 }
 
 // the list of a particle is in ascending order of the partner id already (dem_fill_kernel)
+template <typename T>
 __global__ void dem_pair_write_kernel(int n, const uint32_t* __restrict__ pos_of_id, const uint32_t* __restrict__ off,
-                                      const uint32_t* __restrict__ hq, const double* __restrict__ hdt,
+                                      const uint32_t* __restrict__ hq, const T* __restrict__ hdt,
                                       const uint32_t* __restrict__ pair_off, uint32_t cap, uint32_t* __restrict__ pairs,
-                                      double* __restrict__ pair_dt, uint32_t* __restrict__ n_pairs)
+                                      T* __restrict__ pair_dt, uint32_t* __restrict__ n_pairs)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p == 0 && n_pairs) *n_pairs = pair_off[n];
@@ -1112,7 +1125,8 @@ static double dem_zeta_host(double eps)
     return -l / sqrt(l * l + DEM_PI * DEM_PI);                                        // -beta of (A.5)
 }
 
-static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
+// es = bytes of the handle's real type (8: fp64 calls, 4: the _f32 calls)
+static int dem_setup(const ledds_dem_params* p, ledds_dem* h, size_t es)
 {
     if (!p || p->n < 0 || p->max_contacts < 1 || p->max_contacts > 32) return LEDDS_EINVAL;   // n = 0: a valid, empty system
     if (!(p->cell > 0.0) || !(p->dt >= 0.0) || !(p->density > 0.0)) return LEDDS_EINVAL;
@@ -1180,10 +1194,10 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     s.cell_range = take((size_t)d.ncell * 8);
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
     s.hid = take(n * 4); s.sid = take(n * 4); s.sid_tmp = take(n * 4);
-    s.hx = take(n * 32);
-    s.hv = take(n * 24); s.hw = take(n * 24); s.ha = take(n * 24); s.hal = take(n * 24);
-    s.pvw = take(n * 48);
-    s.xr_s = take(n * 32); s.xf_s = take(n * 16);
+    s.hx = take(n * 4 * es);
+    s.hv = take(n * 3 * es); s.hw = take(n * 3 * es); s.ha = take(n * 3 * es); s.hal = take(n * 3 * es);
+    s.pvw = take(n * 6 * es);
+    s.xr_s = take(n * 4 * es); s.xf_s = take(n * 16);
     s.nfwd = take(n * 4); s.nback = take(n * 4); s.cand = take(ecap * 4);
     s.off = take((n + 1) * 4);
     s.end_s = take(ecap * 4); s.end_t = take(ecap * 4); s.end_hs = take(ecap * 4); s.end_ht = take(ecap * 4); s.end_prev = take(ecap * 4);
@@ -1193,12 +1207,27 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     DemHistory& hs = h->hs;
     o = 0;
     for (int b = 0; b < 2; ++b) {
-        hs.fm[b] = take(n * 48);
+        hs.fm[b] = take(n * 6 * es);
         hs.row[b] = take(n * 8);
         hs.hq[b] = take(ecap * 4);
-        hs.hdt[b] = take(ecap * 24);
+        hs.hdt[b] = take(ecap * 3 * es);
     }
     hs.total = o;
+    h->f32 = es == 4;
+    {   // the same parameters in float for the kernels of an fp32 handle
+        DemDevT<float>& f = h->df;
+        f.n = d.n; f.fmargin = d.fmargin; f.ncell = d.ncell; f.plane = d.plane; f.magic_row = d.magic_row;
+        f.magic_plane = d.magic_plane; f.magic_ok = d.magic_ok; f.hmin = (float)d.hmin; f.dt = (float)d.dt;
+        f.density = (float)d.density; f.maxc = d.maxc;
+        f.kn = (float)d.kn; f.kt = (float)d.kt; f.zeta = (float)d.zeta; f.mu = (float)d.mu;
+        f.kn_w = (float)d.kn_w; f.kt_w = (float)d.kt_w; f.zeta_w = (float)d.zeta_w; f.mu_w = (float)d.mu_w;
+        f.Ystar = (float)d.Ystar; f.Gstar = (float)d.Gstar; f.Ystar_w = (float)d.Ystar_w; f.Gstar_w = (float)d.Gstar_w;
+        for (int a = 0; a < 3; ++a) {
+            f.lo[a] = (float)d.lo[a]; f.hi[a] = (float)d.hi[a]; f.L[a] = (float)d.L[a]; f.Lf[a] = d.Lf[a]; f.bc[a] = d.bc[a];
+            f.nc[a] = d.nc[a]; f.inv_h[a] = (float)d.inv_h[a]; f.g[a] = (float)d.g[a];
+        }
+        for (int k = 0; k < 18; ++k) f.vw[k] = (float)d.vw[k];
+    }
     h->cur = 0;
     h->rec = 0;
     h->sorted_buf = 0;
@@ -1208,15 +1237,28 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h)
     return LEDDS_OK;
 }
 
-extern "C" int ledds_dem_workspace_bytes(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes)
+static int dem_workspace_bytes(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes, size_t es)
 {
     ledds_dem tmp;
-    const int rc = dem_setup(p, &tmp);
+    const int rc = dem_setup(p, &tmp, es);
     if (rc) return rc;
     if (scratch_bytes) *scratch_bytes = tmp.s.total;
     if (history_bytes) *history_bytes = tmp.hs.total;
     return LEDDS_OK;
 }
+extern "C" int ledds_dem_workspace_bytes(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes)
+{
+    return dem_workspace_bytes(p, scratch_bytes, history_bytes, 8);
+}
+extern "C" int ledds_dem_workspace_bytes_f32(const ledds_dem_params* p, size_t* scratch_bytes, size_t* history_bytes)
+{
+    return dem_workspace_bytes(p, scratch_bytes, history_bytes, 4);
+}
+
+// the kernel-side parameters of a handle in the real type T
+template <typename T> static const DemDevT<T>& dem_dev(const ledds_dem* h);
+template <> const DemDevT<double>& dem_dev<double>(const ledds_dem* h) { return h->d; }
+template <> const DemDevT<float>& dem_dev<float>(const ledds_dem* h) { return h->df; }
 
 template <typename T>
 static T* at(void* base, size_t off) { return reinterpret_cast<T*>(static_cast<char*>(base) + off); }
@@ -1224,8 +1266,9 @@ template <typename T>
 static const T* at(const void* base, size_t off) { return reinterpret_cast<const T*>(static_cast<const char*>(base) + off); }
 
 // The caller's arrays in the home order of this call: the sorted order of the last sort (identity before the first).
-int ledds_dem_import(ledds_dem* h, const double* x, const double* v, const double* w, const double* a, const double* alpha,
-                     const double* radius, void* history, void* scratch, cudaStream_t st)
+template <typename T>
+static int dem_import_t(ledds_dem* h, const T* x, const T* v, const T* w, const T* a, const T* alpha,
+                     const T* radius, void* history, void* scratch, cudaStream_t st)
 {
     const int n = h->d.n;
     if (n == 0) return LEDDS_OK;
@@ -1234,10 +1277,10 @@ int ledds_dem_import(ledds_dem* h, const double* x, const double* v, const doubl
     const int from = h->rec, to = 1 - h->rec;
     const uint32_t* hid_src = h->have_sort ? at<uint32_t>(scratch, s.sid) : nullptr;
     const uint32_t* perm = h->have_sort ? at<uint32_t>(scratch, s.idx[h->sh_buf]) : nullptr;
-    dem_import_kernel<<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(
-        n, hid_src, perm, x, v, w, a, alpha, radius, at<uint32_t>(scratch, s.hid), at<double4>(scratch, s.hx),
-        at<double>(scratch, s.hv), at<double>(scratch, s.hw), at<double>(scratch, s.ha), at<double>(scratch, s.hal),
-        at<double>(history, hs.fm[from]), at<uint2>(history, hs.row[from]), at<double>(history, hs.fm[to]),
+    dem_import_kernel<T><<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(
+        n, hid_src, perm, x, v, w, a, alpha, radius, at<uint32_t>(scratch, s.hid), at<typename Real<T>::v4>(scratch, s.hx),
+        at<T>(scratch, s.hv), at<T>(scratch, s.hw), at<T>(scratch, s.ha), at<T>(scratch, s.hal),
+        at<T>(history, hs.fm[from]), at<uint2>(history, hs.row[from]), at<T>(history, hs.fm[to]),
         at<uint2>(history, hs.row[to]));
     LEDDS_CHECK_LAUNCH();
     h->rec = to;
@@ -1245,48 +1288,50 @@ int ledds_dem_import(ledds_dem* h, const double* x, const double* v, const doubl
     return LEDDS_OK;
 }
 
-int ledds_dem_export(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha, const void* scratch, cudaStream_t st)
+template <typename T>
+static int dem_export_t(ledds_dem* h, T* x, T* v, T* w, T* a, T* alpha, const void* scratch, cudaStream_t st)
 {
     const int n = h->d.n;
     if (n == 0) return LEDDS_OK;
     const DemScratch& s = h->s;
-    dem_export_kernel<<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(
-        n, at<uint32_t>(scratch, s.hid), at<double4>(scratch, s.hx), at<double>(scratch, s.hv), at<double>(scratch, s.hw),
-        at<double>(scratch, s.ha), at<double>(scratch, s.hal), x, v, w, a, alpha);
+    dem_export_kernel<T><<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(
+        n, at<uint32_t>(scratch, s.hid), at<typename Real<T>::v4>(scratch, s.hx), at<T>(scratch, s.hv), at<T>(scratch, s.hw),
+        at<T>(scratch, s.ha), at<T>(scratch, s.hal), x, v, w, a, alpha);
     LEDDS_CHECK_LAUNCH();
     return LEDDS_OK;
 }
 
 // [kick] -> drift (optional) -> keys -> sort -> gather/ranges -> contacts, all on the home state.  Leaves the contact
 // sums of every particle in history (fm, row) and the contact ends in hq / hdt of the new generation.
-int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32_t* status, double dt_hist,
-                               bool drift, cudaStream_t st, bool fork, const DemKick* kick)
+template <typename T>
+static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* status, double dt_hist,
+                               bool drift, cudaStream_t st, bool fork, const DemKickT<T>* kick)
 {
     // kick != nullptr: the kick that closes the previous step (with the contact sums still in fm and the
     // external force / torque of *kick) is fused into the drift kernel of this one.
     // fork = true: everything after the drift/key kernel is enqueued on the handle's side stream (ordered after
     // that kernel by an event); the caller joins by waiting on h->ev_join before it needs the contact forces.
-    const DemDev& d = h->d;
+    const DemDevT<T>& d = dem_dev<T>(h);
     const DemScratch& s = h->s;
     const DemHistory& hs = h->hs;
     const int n = d.n, tb = 128, nb = (n + tb - 1) / tb;
     if (n == 0) { h->cur = 1 - h->cur; return LEDDS_OK; }
     // clear sort / scan bookkeeping + cell ranges (one contiguous region)
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
-    double* fm = at<double>(history, hs.fm[h->rec]);
+    T* fm = at<T>(history, hs.fm[h->rec]);
     uint2* row = at<uint2>(history, hs.row[h->rec]);
     ledds_prof_start(LEDDS_K_DEM_KEYS, st);
     {
         const dim3 grid((n + DRIFT_BLOCK - 1) / DRIFT_BLOCK);
         if (kick)
-            dem_drift_key_kernel<true><<<grid, DRIFT_BLOCK, 0, st>>>(d, at<double4>(scratch, s.hx), at<double>(scratch, s.hv), at<double>(scratch, s.hw),
-                                                                      at<double>(scratch, s.ha), at<double>(scratch, s.hal), at<uint32_t>(scratch, s.hid), fm,
-                                                                      kick->f_ext, kick->m_ext, at<double>(scratch, s.pvw),
+            dem_drift_key_kernel<T, true><<<grid, DRIFT_BLOCK, 0, st>>>(d, at<typename Real<T>::v4>(scratch, s.hx), at<T>(scratch, s.hv), at<T>(scratch, s.hw),
+                                                                      at<T>(scratch, s.ha), at<T>(scratch, s.hal), at<uint32_t>(scratch, s.hid), fm,
+                                                                      kick->f_ext, kick->m_ext, at<T>(scratch, s.pvw),
                                                                       at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status);
         else
-            dem_drift_key_kernel<false><<<grid, DRIFT_BLOCK, 0, st>>>(d, at<double4>(scratch, s.hx), at<double>(scratch, s.hv), at<double>(scratch, s.hw),
-                                                                       at<double>(scratch, s.ha), at<double>(scratch, s.hal), at<uint32_t>(scratch, s.hid), fm,
-                                                                       nullptr, nullptr, at<double>(scratch, s.pvw),
+            dem_drift_key_kernel<T, false><<<grid, DRIFT_BLOCK, 0, st>>>(d, at<typename Real<T>::v4>(scratch, s.hx), at<T>(scratch, s.hv), at<T>(scratch, s.hw),
+                                                                       at<T>(scratch, s.ha), at<T>(scratch, s.hal), at<uint32_t>(scratch, s.hid), fm,
+                                                                       nullptr, nullptr, at<T>(scratch, s.pvw),
                                                                        at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status);
     }
     ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
@@ -1330,8 +1375,8 @@ int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32
     dem_ranges_kernel<<<nb, tb, 0, st>>>(n, skey, sh0, at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp),
                                          at<uint2>(scratch, s.cell_range));
     LEDDS_CHECK_LAUNCH();
-    dem_gather_kernel<<<nb, tb, 0, st>>>(d, skey, sh0, at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range),
-                                         at<double4>(scratch, s.hx), at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+    dem_gather_kernel<T><<<nb, tb, 0, st>>>(d, skey, sh0, at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range),
+                                         at<typename Real<T>::v4>(scratch, s.hx), at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
                                          sid, sh, nback);
     ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
     LEDDS_CHECK_LAUNCH();
@@ -1339,10 +1384,10 @@ int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
     const int cb = (n + CONTACT_BLOCK - 1) / CONTACT_BLOCK;
     if (d.bc[0] && d.bc[1] && d.bc[2])
-        dem_detect_kernel<false><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+        dem_detect_kernel<T, false><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
                                                                         at<uint2>(scratch, s.cell_range), nfwd, nback, at<uint32_t>(scratch, s.cand), status);
     else
-        dem_detect_kernel<true><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<double4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+        dem_detect_kernel<T, true><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
                                                                        at<uint2>(scratch, s.cell_range), nfwd, nback, at<uint32_t>(scratch, s.cand), status);
     LEDDS_CHECK_LAUNCH();
     dem_scan_kernel<<<h->scan_tiles, SCAN_THREADS, 0, st>>>(n, (uint32_t)d.maxc, nfwd, nback, off, at<uint32_t>(scratch, s.scan_state),
@@ -1354,9 +1399,9 @@ int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32
         n, (uint32_t)d.maxc, nfwd, nback, at<uint32_t>(scratch, s.cand), sid, sh, off, row, fm, at<uint32_t>(history, hs.hq[prev]), E,
         at<uint32_t>(history, hs.hq[nw]), status);
     LEDDS_CHECK_LAUNCH();
-    (h->p.model == 1 ? dem_force_kernel<true> : dem_force_kernel<false>)<<<(n + FORCE_PB - 1) / FORCE_PB, FORCE_THREADS, 0, st>>>(
-        d, at<double4>(scratch, s.xr_s), at<double>(scratch, s.pvw), off, E, sh, fm, at<double>(history, hs.hdt[prev]),
-        at<double>(history, hs.hdt[nw]), status, dt_hist);
+    (h->p.model == 1 ? dem_force_kernel<T, true> : dem_force_kernel<T, false>)<<<(n + FORCE_PB - 1) / FORCE_PB, FORCE_THREADS, 0, st>>>(
+        d, at<typename Real<T>::v4>(scratch, s.xr_s), at<T>(scratch, s.pvw), off, E, sh, fm, at<T>(history, hs.hdt[prev]),
+        at<T>(history, hs.hdt[nw]), status, (T)dt_hist);
     ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
     LEDDS_CHECK_LAUNCH();
     h->cur = nw;
@@ -1364,23 +1409,25 @@ int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32
     return LEDDS_OK;
 }
 
-int ledds_dem_kick(ledds_dem* h, const double* f_ext, const double* m_ext, const void* history, void* scratch, cudaStream_t st)
+template <typename T>
+static int dem_kick_t(ledds_dem* h, const T* f_ext, const T* m_ext, const void* history, void* scratch, cudaStream_t st)
 {
     const int n = h->d.n;
     if (n == 0) return LEDDS_OK;
     const DemScratch& s = h->s;
     ledds_prof_start(LEDDS_K_DEM_KICK, st);
-    dem_kick_kernel<<<(unsigned)((3ll * n + 255) / 256), 256, 0, st>>>(h->d, at<double4>(scratch, s.hx), at<uint32_t>(scratch, s.hid),
-                                                                       at<double>(history, h->hs.fm[h->rec]), f_ext, m_ext,
-                                                                       at<double>(scratch, s.hv), at<double>(scratch, s.hw),
-                                                                       at<double>(scratch, s.ha), at<double>(scratch, s.hal), 0);
+    dem_kick_kernel<T><<<(unsigned)((3ll * n + 255) / 256), 256, 0, st>>>(dem_dev<T>(h), at<typename Real<T>::v4>(scratch, s.hx), at<uint32_t>(scratch, s.hid),
+                                                                       at<T>(history, h->hs.fm[h->rec]), f_ext, m_ext,
+                                                                       at<T>(scratch, s.hv), at<T>(scratch, s.hw),
+                                                                       at<T>(scratch, s.ha), at<T>(scratch, s.hal), 0);
     ledds_prof_stop(LEDDS_K_DEM_KICK, st);
     LEDDS_CHECK_LAUNCH();
     return LEDDS_OK;
 }
 
-extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const double* x, const double* v,
-                              const double* w, const double* radius, double* a, double* alpha, void* history,
+template <typename T>
+static int dem_init_t(ledds_dem** out, const ledds_dem_params* p, const T* x, const T* v,
+                              const T* w, const T* radius, T* a, T* alpha, void* history,
                               void* scratch, int32_t* status, void* stream)
 {
     if (!out || !p || !status) return LEDDS_EINVAL;
@@ -1390,7 +1437,7 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
         if (!ledds_aligned16(q)) return LEDDS_EALIGN;
     ledds_dem* h = new (std::nothrow) ledds_dem();
     if (!h) return LEDDS_EINVAL;
-    int rc = dem_setup(p, h);
+    int rc = dem_setup(p, h, sizeof(T));
     if (rc) { delete h; return rc; }
     cudaStream_t st = (cudaStream_t)stream;
     if ((h->hs.total && cudaMemsetAsync(history, 0, h->hs.total, st) != cudaSuccess) ||
@@ -1399,18 +1446,18 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
         return LEDDS_ECUDA;
     }
     // forces of the initial state: no drift, delta_t stays 0 (dt_hist = 0); a(0), alpha(0) back to the caller
-    rc = ledds_dem_import(h, x, v, w, nullptr, nullptr, radius, history, scratch, st);
-    if (!rc) rc = ledds_dem_advance_contacts(h, history, scratch, status, 0.0, false, st, false, nullptr);
+    rc = dem_import_t<T>(h, x, v, w, (const T*)nullptr, (const T*)nullptr, radius, history, scratch, st);
+    if (!rc) rc = dem_advance_t<T>(h, history, scratch, status, 0.0, false, st, false, nullptr);
     if (rc) { delete h; return rc; }
     if (h->d.n == 0) { *out = h; return LEDDS_OK; }
     const DemScratch& s = h->s;
-    dem_kick_kernel<<<(unsigned)((3ll * h->d.n + 255) / 256), 256, 0, st>>>(h->d, at<double4>(scratch, s.hx), at<uint32_t>(scratch, s.hid),
-                                                                            at<double>(history, h->hs.fm[h->rec]), nullptr, nullptr,
-                                                                            at<double>(scratch, s.hv), at<double>(scratch, s.hw),
-                                                                            at<double>(scratch, s.ha), at<double>(scratch, s.hal), 1);
+    dem_kick_kernel<T><<<(unsigned)((3ll * h->d.n + 255) / 256), 256, 0, st>>>(dem_dev<T>(h), at<typename Real<T>::v4>(scratch, s.hx), at<uint32_t>(scratch, s.hid),
+                                                                            at<T>(history, h->hs.fm[h->rec]), (const T*)nullptr, (const T*)nullptr,
+                                                                            at<T>(scratch, s.hv), at<T>(scratch, s.hw),
+                                                                            at<T>(scratch, s.ha), at<T>(scratch, s.hal), 1);
     ledds_count_launch(1);
     if (cudaPeekAtLastError() != cudaSuccess) { delete h; return LEDDS_ECUDA; }
-    rc = ledds_dem_export(h, nullptr, nullptr, nullptr, a, alpha, scratch, st);
+    rc = dem_export_t<T>(h, (T*)nullptr, (T*)nullptr, (T*)nullptr, a, alpha, scratch, st);
     if (rc) { delete h; return rc; }
     *out = h;
     return LEDDS_OK;
@@ -1419,44 +1466,46 @@ extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const 
 // steps between two re-homings inside one long call (the home order goes stale as particles change cells)
 #define DEM_REHOME_STEPS 256
 
-extern "C" int ledds_dem_step(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha,
-                              const double* radius, const double* f_ext, const double* m_ext, void* history,
+template <typename T>
+static int dem_step_t(ledds_dem* h, T* x, T* v, T* w, T* a, T* alpha,
+                              const T* radius, const T* f_ext, const T* m_ext, void* history,
                               void* scratch, int32_t* status, int nsteps, void* stream)
 {
-    if (!h || !status || nsteps < 0) return LEDDS_EINVAL;
+    if (!h || !status || nsteps < 0 || h->f32 != (sizeof(T) == 4)) return LEDDS_EINVAL;   // the handle fixes the real type
     if (h->d.n == 0 || nsteps == 0) return LEDDS_OK;
     if (!x || !v || !w || !a || !alpha || !radius || !history || !scratch) return LEDDS_EINVAL;
     const void* ptrs[] = {x, v, w, a, alpha, radius, f_ext, m_ext, history, scratch, status};
     for (const void* q : ptrs)
         if (!ledds_aligned16(q)) return LEDDS_EALIGN;
     cudaStream_t st = (cudaStream_t)stream;
-    const DemKick kick = {f_ext, m_ext};
-    int rc = ledds_dem_import(h, x, v, w, a, alpha, radius, history, scratch, st);
+    const DemKickT<T> kick = {f_ext, m_ext};
+    int rc = dem_import_t<T>(h, x, v, w, a, alpha, radius, history, scratch, st);
     if (rc) return rc;
     for (int s = 0; s < nsteps; ++s) {
         // the kick of step s - 1 rides on the drift of step s; only the last step of the call (and the one before
         // a re-homing) kicks on its own
         const bool rehome = s > 0 && s % DEM_REHOME_STEPS == 0;
         if (rehome) {
-            rc = ledds_dem_kick(h, f_ext, m_ext, history, scratch, st);
-            if (!rc) rc = ledds_dem_export(h, x, v, w, a, alpha, scratch, st);
-            if (!rc) rc = ledds_dem_import(h, x, v, w, a, alpha, radius, history, scratch, st);
+            rc = dem_kick_t<T>(h, f_ext, m_ext, history, scratch, st);
+            if (!rc) rc = dem_export_t<T>(h, x, v, w, a, alpha, scratch, st);
+            if (!rc) rc = dem_import_t<T>(h, x, v, w, a, alpha, radius, history, scratch, st);
             if (rc) return rc;
         }
-        rc = ledds_dem_advance_contacts(h, history, scratch, status, h->d.dt, true, st, false, (s > 0 && !rehome) ? &kick : nullptr);
+        rc = dem_advance_t<T>(h, history, scratch, status, h->d.dt, true, st, false, (s > 0 && !rehome) ? &kick : nullptr);
         if (rc) return rc;
         h->steps++;
     }
-    rc = ledds_dem_kick(h, f_ext, m_ext, history, scratch, st);
+    rc = dem_kick_t<T>(h, f_ext, m_ext, history, scratch, st);
     if (rc) return rc;
-    return ledds_dem_export(h, x, v, w, a, alpha, scratch, st);
+    return dem_export_t<T>(h, x, v, w, a, alpha, scratch, st);
 }
 
-extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* scratch, uint32_t* sorted_idx,
-                               uint32_t* sorted_key, uint32_t* pairs, double* pair_dt, uint32_t pair_cap,
-                               uint32_t* n_pairs, double* force, double* torque, void* stream)
+template <typename T>
+static int dem_query_t(ledds_dem* h, const void* history, const void* scratch, uint32_t* sorted_idx,
+                               uint32_t* sorted_key, uint32_t* pairs, T* pair_dt, uint32_t pair_cap,
+                               uint32_t* n_pairs, T* force, T* torque, void* stream)
 {
-    if (!h) return LEDDS_EINVAL;
+    if (!h || h->f32 != (sizeof(T) == 4)) return LEDDS_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t n = (size_t)h->d.n;
     if (n == 0) {
@@ -1474,7 +1523,7 @@ extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* sc
         return LEDDS_ECUDA;
     const int tb = 128, nb = ((int)n + tb - 1) / tb;
     if (force || torque) {
-        dem_unpack_fm_kernel<<<nb, tb, 0, st>>>((int)n, at<uint32_t>(scratch, s.hid), at<double>(history, hs.fm[h->rec]), force, torque);
+        dem_unpack_fm_kernel<T><<<nb, tb, 0, st>>>((int)n, at<uint32_t>(scratch, s.hid), at<T>(history, hs.fm[h->rec]), force, torque);
         LEDDS_CHECK_LAUNCH();
     }
     if (pairs || pair_dt || n_pairs) {
@@ -1487,12 +1536,69 @@ extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* sc
         dem_query_pos_kernel<<<nb, tb, 0, st>>>((int)n, at<uint32_t>(scratch, s.sid), pos);
         dem_pair_count_kernel<<<nb, tb, 0, st>>>((int)n, pos, off, hq, cnt);
         dem_block_scan_kernel<<<1, 1024, 0, st>>>((int)n, cnt, poff);
-        dem_pair_write_kernel<<<nb, tb, 0, st>>>((int)n, pos, off, hq, at<double>(history, hs.hdt[h->cur]), poff, pair_cap, pairs,
+        dem_pair_write_kernel<T><<<nb, tb, 0, st>>>((int)n, pos, off, hq, at<T>(history, hs.hdt[h->cur]), poff, pair_cap, pairs,
                                                  pair_dt, n_pairs);
         ledds_count_launch(3);
         LEDDS_CHECK_LAUNCH();
     }
     return LEDDS_OK;
+}
+
+// ---- entry points: the fp64 set, the fp32 set (include/ledds.h), and the fp64 pieces coupled.cu drives
+extern "C" int ledds_dem_init(ledds_dem** out, const ledds_dem_params* p, const double* x, const double* v, const double* w,
+                              const double* radius, double* a, double* alpha, void* history, void* scratch, int32_t* status,
+                              void* stream)
+{
+    return dem_init_t<double>(out, p, x, v, w, radius, a, alpha, history, scratch, status, stream);
+}
+extern "C" int ledds_dem_init_f32(ledds_dem** out, const ledds_dem_params* p, const float* x, const float* v, const float* w,
+                                  const float* radius, float* a, float* alpha, void* history, void* scratch, int32_t* status,
+                                  void* stream)
+{
+    return dem_init_t<float>(out, p, x, v, w, radius, a, alpha, history, scratch, status, stream);
+}
+extern "C" int ledds_dem_step(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha, const double* radius,
+                              const double* f_ext, const double* m_ext, void* history, void* scratch, int32_t* status,
+                              int nsteps, void* stream)
+{
+    return dem_step_t<double>(h, x, v, w, a, alpha, radius, f_ext, m_ext, history, scratch, status, nsteps, stream);
+}
+extern "C" int ledds_dem_step_f32(ledds_dem* h, float* x, float* v, float* w, float* a, float* alpha, const float* radius,
+                                  const float* f_ext, const float* m_ext, void* history, void* scratch, int32_t* status,
+                                  int nsteps, void* stream)
+{
+    return dem_step_t<float>(h, x, v, w, a, alpha, radius, f_ext, m_ext, history, scratch, status, nsteps, stream);
+}
+extern "C" int ledds_dem_query(ledds_dem* h, const void* history, const void* scratch, uint32_t* sorted_idx,
+                               uint32_t* sorted_key, uint32_t* pairs, double* pair_dt, uint32_t pair_cap, uint32_t* n_pairs,
+                               double* force, double* torque, void* stream)
+{
+    return dem_query_t<double>(h, history, scratch, sorted_idx, sorted_key, pairs, pair_dt, pair_cap, n_pairs, force, torque, stream);
+}
+extern "C" int ledds_dem_query_f32(ledds_dem* h, const void* history, const void* scratch, uint32_t* sorted_idx,
+                                   uint32_t* sorted_key, uint32_t* pairs, float* pair_dt, uint32_t pair_cap, uint32_t* n_pairs,
+                                   float* force, float* torque, void* stream)
+{
+    return dem_query_t<float>(h, history, scratch, sorted_idx, sorted_key, pairs, pair_dt, pair_cap, n_pairs, force, torque, stream);
+}
+
+int ledds_dem_import(ledds_dem* h, const double* x, const double* v, const double* w, const double* a, const double* alpha,
+                     const double* radius, void* history, void* scratch, cudaStream_t st)
+{
+    return h->f32 ? LEDDS_EINVAL : dem_import_t<double>(h, x, v, w, a, alpha, radius, history, scratch, st);
+}
+int ledds_dem_export(ledds_dem* h, double* x, double* v, double* w, double* a, double* alpha, const void* scratch, cudaStream_t st)
+{
+    return dem_export_t<double>(h, x, v, w, a, alpha, scratch, st);
+}
+int ledds_dem_advance_contacts(ledds_dem* h, void* history, void* scratch, int32_t* status, double dt_hist, bool drift,
+                               cudaStream_t st, bool fork, const DemKick* kick)
+{
+    return dem_advance_t<double>(h, history, scratch, status, dt_hist, drift, st, fork, kick);
+}
+int ledds_dem_kick(ledds_dem* h, const double* f_ext, const double* m_ext, const void* history, void* scratch, cudaStream_t st)
+{
+    return dem_kick_t<double>(h, f_ext, m_ext, history, scratch, st);
 }
 
 extern "C" int ledds_dem_destroy(ledds_dem* h)

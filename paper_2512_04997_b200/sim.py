@@ -61,36 +61,44 @@ class Lbm:
 
 
 class Dem:
-    """Sphere DEM on the GPU (ledds_dem_*).  State tensors are [n,3] in particle order."""
+    """Sphere DEM on the GPU (ledds_dem_*; precision="f32" -> the ledds_dem_*_f32 calls on float arrays).
+    State tensors are [n,3] in particle order."""
 
-    def __init__(self, pd: dict, x, v, w, radius):
+    def __init__(self, pd: dict, x, v, w, radius, precision="f64"):
+        if precision not in ("f64", "f32"):
+            raise ValueError(precision)
         self.pd = dict(pd)
         self.p = L.dem_params(pd)
+        self.f32 = precision == "f32"
+        dt = self.dtype = torch.float32 if self.f32 else torch.float64
+        self._bytes, self._init, self._step, self._query = (
+            (L.ledds_dem_workspace_bytes_f32, L.ledds_dem_init_f32, L.ledds_dem_step_f32, L.ledds_dem_query_f32) if self.f32 else
+            (L.ledds_dem_workspace_bytes, L.ledds_dem_init, L.ledds_dem_step, L.ledds_dem_query))
         n = self.n = self.p.n
-        self.x, self.v, self.w = _dev(x).reshape(n, 3), _dev(v).reshape(n, 3), _dev(w).reshape(n, 3)
-        self.radius = _dev(radius).reshape(n)
-        self.a = torch.zeros(n, 3, dtype=torch.float64, device="cuda")
-        self.alpha = torch.zeros(n, 3, dtype=torch.float64, device="cuda")
-        sb, hb = L.ledds_dem_workspace_bytes(self.p)
+        self.x, self.v, self.w = _dev(x, dt).reshape(n, 3), _dev(v, dt).reshape(n, 3), _dev(w, dt).reshape(n, 3)
+        self.radius = _dev(radius, dt).reshape(n)
+        self.a = torch.zeros(n, 3, dtype=dt, device="cuda")
+        self.alpha = torch.zeros(n, 3, dtype=dt, device="cuda")
+        sb, hb = self._bytes(self.p)
         self.scratch = torch.empty(sb, dtype=torch.uint8, device="cuda")
         self.history = torch.empty(hb, dtype=torch.uint8, device="cuda")
         self.status = torch.zeros(4, dtype=torch.int32, device="cuda")
-        self.h = L.ledds_dem_init(self.p, self.x, self.v, self.w, self.radius, self.a, self.alpha, self.history,
-                                  self.scratch, self.status)
+        self.h = self._init(self.p, self.x, self.v, self.w, self.radius, self.a, self.alpha, self.history,
+                            self.scratch, self.status)
 
     def step(self, nsteps=1, f_ext=None, m_ext=None):
-        L.ledds_dem_step(self.h, self.x, self.v, self.w, self.a, self.alpha, self.radius, f_ext, m_ext, self.history,
-                         self.scratch, self.status, nsteps)
+        self._step(self.h, self.x, self.v, self.w, self.a, self.alpha, self.radius, f_ext, m_ext, self.history,
+                   self.scratch, self.status, nsteps)
 
     def query(self, pair_cap=None):
         n = self.n
         cap = pair_cap if pair_cap is not None else 16 * n + 64
         idx = torch.empty(n, dtype=torch.int32, device="cuda"); key = torch.empty(n, dtype=torch.int32, device="cuda")
         pairs = torch.zeros(cap, 2, dtype=torch.int32, device="cuda")
-        pdt = torch.zeros(cap, 3, dtype=torch.float64, device="cuda")
+        pdt = torch.zeros(cap, 3, dtype=self.dtype, device="cuda")
         npairs = torch.zeros(4, dtype=torch.int32, device="cuda")
-        F = torch.empty(n, 3, dtype=torch.float64, device="cuda"); M = torch.empty(n, 3, dtype=torch.float64, device="cuda")
-        L.ledds_dem_query(self.h, self.history, self.scratch, idx, key, pairs, pdt, cap, npairs, F, M)
+        F = torch.empty(n, 3, dtype=self.dtype, device="cuda"); M = torch.empty(n, 3, dtype=self.dtype, device="cuda")
+        self._query(self.h, self.history, self.scratch, idx, key, pairs, pdt, cap, npairs, F, M)
         k = int(npairs[0].item())
         if k > cap:
             raise L.LeddsError("pair_cap too small")
