@@ -40,9 +40,10 @@ __global__ void cpl_solid_kernel(const CplDev C)
     if (r.w > C.r_max) atomicOr(C.status, LEDDS_ST_RADIUS_RANGE);   // its box (H from r_max) would truncate it
 }
 
-// Eq. (38) in two kernels: every (solid, cell of its bounding box) is classified from its nearest and farthest
-// sample point (all inside: 1, all outside: 0); the cells the surface crosses go to a list, and the second kernel
-// counts their 10^3 points with one thread per listed cell, so that its warps hold only cells that need it.
+// Eq. (38) in two kernels: every (solid, cell of its bounding box) is classified -- by the distance of its centre where
+// that settles it, else from its nearest and farthest sample point (all inside: 1, all outside: 0); the cells the
+// surface crosses go to a list, and the second kernel counts their 10^3 points with one thread per listed cell, so
+// that its warps hold only cells that need it.
 __device__ __forceinline__ void cpl_box_cell(const CplDev& C, long long t, double* d, double& Rk)
 {
     const int S = C.S, S3 = S * S * S;
@@ -55,32 +56,55 @@ __device__ __forceinline__ void cpl_box_cell(const CplDev& C, long long t, doubl
     Rk = o[3];
 }
 
+// one thread per (solid, row of its box): the row's cells one after the other (the index arithmetic, the solid's record
+// and the y, z parts of the distances once per row)
 __global__ void __launch_bounds__(256) cpl_beta_classify_kernel(const CplDev C)
 {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool in = t < (long long)C.n * C.S * C.S * C.S;
-    double beta = 0.0;
-    if (in) {
-        double d[3], Rk;
-        cpl_box_cell(C, t, d, Rk);
-        SubdivPoints p;
-        cpl_subdiv_points(d, Rk, p);
-        beta = cpl_beta_classify(p);
-        C.betabox[t] = beta;
-    }
-    const bool todo = in && beta < 0.0;
-    const unsigned m = __ballot_sync(0xffffffffu, todo);                            // one list append per warp
-    if (m) {
-        const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
-        uint32_t base = 0;
-        if (lane == leader) base = atomicAdd(C.blist, (uint32_t)__popc(m));
-        base = __shfl_sync(0xffffffffu, base, leader);
-        if (todo) C.blist[1 + base + __popc(m & ((1u << lane) - 1u))] = (uint32_t)t;
+    const int S = C.S, S2 = S * S;
+    const bool in = t < (long long)C.n * S2;
+    const int k = in ? (int)(t / S2) : 0;
+    const int r = (int)(t - (long long)k * S2), lz = r / S, ly = r - lz * S;
+    const double* o = C.sol + (size_t)k * 10;
+    const double Rk = o[3], ro = Rk + 0.78, ri = Rk - 0.78;
+    const int fx = (int)floor(o[0]);
+    const double dy = (double)((int)floor(o[1]) + ly - C.H) - o[1], dz = (double)((int)floor(o[2]) + lz - C.H) - o[2];
+    const double dyz2 = dy * dy + dz * dz;
+    const int lane = threadIdx.x & 31;
+    for (int lx = 0; lx < S; ++lx) {
+        const long long cell = t * S + lx;                                         // = (k S^2 + r) S + lx
+        double beta = 0.0;
+        if (in) {
+            const double dx = (double)(fx + lx - C.H) - o[0];
+            // every sample point lies within 0.45 sqrt(3) = 0.7795 of the cell centre: a centre further than R + 0.78 from
+            // the solid's (nearer than R - 0.78) has all its points outside (inside) whatever the rounding of the point
+            // tests (the slack, 6e-4, is twelve orders above it); only the shell in between is looked at point by point
+            const double d2 = dx * dx + dyz2;
+            if (d2 > ro * ro) beta = 0.0;
+            else if (ri > 0.0 && d2 < ri * ri) beta = 1.0;
+            else {
+                const double d[3] = {dx, dy, dz};
+                SubdivPoints p;
+                cpl_subdiv_points(d, Rk, p);
+                beta = cpl_beta_classify(p);
+            }
+            C.betabox[cell] = beta;
+        }
+        const bool todo = in && beta < 0.0;
+        const unsigned m = __ballot_sync(0xffffffffu, todo);                        // one list append per warp
+        if (m) {
+            const int leader = __ffs(m) - 1;
+            uint32_t base = 0;
+            if (lane == leader) base = atomicAdd(C.blist, (uint32_t)__popc(m));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            if (todo) C.blist[1 + base + __popc(m & ((1u << lane) - 1u))] = (uint32_t)cell;
+        }
     }
 }
 
 __global__ void __launch_bounds__(256, 3) cpl_beta_count_kernel(const CplDev C)
 {
+    __shared__ double zs[PSM_NSUB][256];
     const uint32_t count = C.blist[0];
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < count; i += gridDim.x * blockDim.x) {
         const long long t = C.blist[1 + i];
@@ -88,7 +112,7 @@ __global__ void __launch_bounds__(256, 3) cpl_beta_count_kernel(const CplDev C)
         cpl_box_cell(C, t, d, Rk);
         SubdivPoints p;
         cpl_subdiv_points(d, Rk, p);
-        C.betabox[t] = cpl_beta_count(p);
+        C.betabox[t] = cpl_beta_count(p, &zs[0][threadIdx.x], 256);
     }
 }
 
@@ -392,7 +416,7 @@ static int coupled_step_t(ledds_lbm* lbm, ledds_dem* dem, const ledds_cpl_params
             ledds_count_launch(1);
             const unsigned rb = (unsigned)(((long long)C.n * C.S * C.S + 255) / 256);
             if (C.subdiv) {
-                cpl_beta_classify_kernel<<<(unsigned)(((long long)C.n * C.S * C.S * C.S + 255) / 256), 256, 0, st>>>(C);
+                cpl_beta_classify_kernel<<<(unsigned)(((long long)C.n * C.S * C.S + 255) / 256), 256, 0, st>>>(C);
                 cpl_beta_count_kernel<<<ledds_sm_count() * 6, 256, 0, st>>>(C);
                 ledds_count_launch(2);
                 cpl_raster_kernel<true><<<rb, 256, 0, st>>>(d, C);

@@ -100,16 +100,44 @@ __device__ __forceinline__ double cpl_beta_classify(const SubdivPoints& p)
     return -1.0;
 }
 
-__device__ __forceinline__ double cpl_beta_count(const SubdivPoints& p)
+// Number of the NSUB^3 points inside, exactly as the oracle counts them -- (sx^2 + sy^2) + sz^2 < R^2 with every operation
+// rounded -- but without testing every point: rounding is monotone, so with the ten squares of the z offsets put in
+// ascending order the points of a column (x, y) that pass are a prefix of them, and its length comes from a 4-step
+// search instead of 10 tests (the 100 searches are independent: no loop-carried chain).  zs = this thread's column of
+// shared memory (stride `zstride` doubles) for the sorted z squares, which the search indexes.
+__device__ __forceinline__ void cpl_sort10(double (&v)[PSM_NSUB])
 {
+#pragma unroll
+    for (int r = 0; r < PSM_NSUB; ++r)                                               // odd-even transposition network
+#pragma unroll
+        for (int i = r & 1; i + 1 < PSM_NSUB; i += 2) {
+            const double lo = fmin(v[i], v[i + 1]), hi = fmax(v[i], v[i + 1]);
+            v[i] = lo; v[i + 1] = hi;
+        }
+}
+
+__device__ __forceinline__ double cpl_beta_count(const SubdivPoints& p, double* zs, int zstride)
+{
+    double z[PSM_NSUB];
+#pragma unroll
+    for (int i = 0; i < PSM_NSUB; ++i) z[i] = p.s2[2][i];
+    cpl_sort10(z);
+#pragma unroll
+    for (int i = 0; i < PSM_NSUB; ++i) zs[i * zstride] = z[i];
     int count = 0;
 #pragma unroll
     for (int a = 0; a < PSM_NSUB; ++a)
 #pragma unroll
         for (int b = 0; b < PSM_NSUB; ++b) {
             const double sxy = __dadd_rn(p.s2[0][a], p.s2[1][b]);                   // (sx^2 + sy^2) + sz^2, as the oracle sums
+            int pos = 0;                                                             // z squares 0 .. pos-1 pass
 #pragma unroll
-            for (int c = 0; c < PSM_NSUB; ++c) count += __dadd_rn(sxy, p.s2[2][c]) < p.R2;
+            for (int step = 8; step > 0; step >>= 1) {
+                const int q = pos + step;
+                const bool ok = q <= PSM_NSUB && __dadd_rn(sxy, zs[(min(q, PSM_NSUB) - 1) * zstride]) < p.R2;
+                pos = ok ? q : pos;
+            }
+            count += pos;
         }
     return (double)count / (double)(PSM_NSUB * PSM_NSUB * PSM_NSUB);
 }
