@@ -7,7 +7,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libledds.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("LEDDS_NVCC_FLAGS", "").split()
+COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 # dem.cu: no FMA contraction (cell index and delta_n > 0 must not depend on it); lbm/coupled keep FMA
 UNITS = [("lbm.cu", []), ("dem.cu", ["-fmad=false"]), ("coupled.cu", []), ("prof.cu", [])]
 HEADERS = ["common.cuh", "lbm_kernels.cuh", "psm_kernels.cuh", os.path.join("..", "..", "include", "ledds.h")]

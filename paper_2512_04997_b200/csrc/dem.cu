@@ -521,13 +521,9 @@ __device__ __forceinline__ void dem_pair_force(const T* en, T dn, const T* vi, c
 #define DETECT_MIN_BLOCKS 8     // caps the detect kernel at 64 registers (8 blocks per SM)
 #define FORCE_THREADS 128       // one thread per contact end ...
 #define FORCE_WARPS (FORCE_THREADS / 32)
-#ifndef FORCE_PW
 #define FORCE_PW 64             // ... of the FORCE_PW particles of a warp: ~7 rounds of 32 ends in a dense bed
-#endif
 #define FORCE_PB (FORCE_WARPS * FORCE_PW)
-#ifndef FORCE_MIN_BLOCKS
 #define FORCE_MIN_BLOCKS 6
-#endif
 
 // Stiffness and damping of one contact.  HERTZ = false: the linear spring-dashpot of the configs, gamma =
 // 2 zeta sqrt(k m*) (G5).  HERTZ = true: Hertz-Mindlin: (A.1) k_n = 4/3 Y* sqrt(R* d_n),

@@ -3,12 +3,8 @@
 #include "lbm_kernels.cuh"
 
 #define PSM_BLOCK 128
-#ifndef PSM_MIN_BLOCKS
 #define PSM_MIN_BLOCKS 5      // resident blocks per SM the collide kernel is compiled for (<= 102 registers)
-#endif
-#ifndef PSM_MIN_BLOCKS_F32
 #define PSM_MIN_BLOCKS_F32 8  // the same for float populations (<= 64 registers)
-#endif
 #define PSM_EMPTY 0xffffffffu
 
 // Layout of the caller-owned coupling scratch (ledds_cpl_workspace_bytes):
