@@ -50,6 +50,34 @@
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
+// Programmatic dependent launch: the kernels of a step form one dependent chain of short launches (for a few thousand
+// particles each runs a few microseconds).  Every kernel of the chain lets its successor be launched as soon as all of
+// its own blocks have started, and waits for its predecessor's results before it touches them: the launch latency of
+// kernel k + 1 is hidden behind kernel k.  Used for systems of up to DEM_PDL_MAX_N particles: with millions of particles
+// the early-launched blocks only take resident slots from the kernel they wait for (4 M spheres: + 3 %).
+#define DEM_PDL_MAX_N 262144
+#define DEM_PDL_ENTER(n)                                                \
+    do {                                                                \
+        if ((n) <= DEM_PDL_MAX_N) {                                     \
+            asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); \
+            asm volatile("griddepcontrol.wait;" ::: "memory");           \
+        }                                                               \
+    } while (0)
+
+static thread_local bool g_pdl = false;   // set by dem_advance_t for the launches of one step
+
+template <typename... KArgs, typename... Args>
+static void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = g_pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 template <typename T>
 __device__ __forceinline__ T dem_mass(const DemDevT<T>& P, T R) { return P.density * (T(4.0) / T(3.0)) * T(DEM_PI) * R * R * R; }
 
@@ -218,6 +246,7 @@ __device__ __forceinline__ void dem_cell_of_key(const DemDevT<T>& P, uint32_t ke
 __global__ void __launch_bounds__(SORT_THREADS) dem_hist_kernel(const uint32_t* __restrict__ key, int n, int passes,
                                                                uint32_t* __restrict__ ghist)
 {
+    DEM_PDL_ENTER(n);
     __shared__ uint32_t h[4][SORT_RADIX];
     for (int t = threadIdx.x; t < 4 * SORT_RADIX; t += blockDim.x) (&h[0][0])[t] = 0;
     __syncthreads();
@@ -268,6 +297,7 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS) dem_onesweep_ke
     uint32_t* __restrict__ val_out, int n, int shift, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
     uint32_t* __restrict__ tile_state /*[tiles][256] of this pass*/, uint32_t* __restrict__ ticket)
 {
+    DEM_PDL_ENTER(n);
     __shared__ uint32_t warp_hist[SORT_WARPS][SORT_RADIX];
     __shared__ uint32_t bin_base[SORT_RADIX];
     __shared__ uint32_t tile_start[SORT_RADIX];
@@ -414,6 +444,7 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS) dem_onesweep_ke
 __global__ void dem_ranges_kernel(int n, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sh0,
                                   const uint32_t* __restrict__ hid, uint32_t* __restrict__ sid_tmp, uint2* __restrict__ cell_range)
 {
+    DEM_PDL_ENTER(n);
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const bool ok = s < n;
@@ -436,6 +467,7 @@ __global__ void dem_gather_kernel(const DemDevT<T> P, const uint32_t* __restrict
                                   const typename Real<T>::v4* __restrict__ hx, typename Real<T>::v4* __restrict__ xr_s, float4* __restrict__ xf_s,
                                   uint32_t* __restrict__ sid, uint32_t* __restrict__ sh, uint32_t* __restrict__ nback)
 {
+    DEM_PDL_ENTER(P.n);
     const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
     if (s0 >= P.n) return;
     const uint2 cr = cell_range[skey[s0]];
@@ -596,6 +628,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
     const uint2* __restrict__ cell_range, uint32_t* __restrict__ nfwd, uint32_t* __restrict__ nback, uint32_t* __restrict__ cand,
     int32_t* __restrict__ status)
 {
+    DEM_PDL_ENTER(P.n);
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.n) return;
     const uint32_t maxc = (uint32_t)P.maxc;
@@ -705,6 +738,7 @@ __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t 
                                                                const uint32_t* __restrict__ cnt2, uint32_t* __restrict__ off,
                                                                uint32_t* __restrict__ state, uint32_t* __restrict__ ticket)
 {
+    DEM_PDL_ENTER(n);
     __shared__ uint32_t wsum[SCAN_THREADS / 32];
     __shared__ uint32_t s_tile, s_excl;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -793,6 +827,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
                                                                 T* __restrict__ fm, const uint32_t* __restrict__ hq_prev,
                                                                 const DemEnds E, uint32_t* __restrict__ hq, int32_t* __restrict__ status)
 {
+    DEM_PDL_ENTER(n);
     extern __shared__ uint2 tq[];                        // uint2 [maxc][CONTACT_BLOCK]: (partner code, partner id); then uint32 [maxc][CONTACT_BLOCK]
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n) return;
@@ -893,6 +928,7 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_ker
     const DemEnds E, const uint32_t* __restrict__ sh, T* __restrict__ fm, const T* __restrict__ hdt_prev,
     T* __restrict__ hdt_new, int32_t* __restrict__ status, T dt_hist)
 {
+    DEM_PDL_ENTER(P.n);
     // every warp works on its own FORCE_PW particles with its own piece of shared memory: no block-wide barrier
     __shared__ uint32_t s_off_all[FORCE_WARPS][FORCE_PW + 1];
     __shared__ T stage_all[FORCE_WARPS][6][32];
@@ -1312,6 +1348,7 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     const DemHistory& hs = h->hs;
     const int n = d.n, tb = 128, nb = (n + tb - 1) / tb;
     if (n == 0) { h->cur = 1 - h->cur; return LEDDS_OK; }
+    g_pdl = n <= DEM_PDL_MAX_N;
     // clear sort / scan bookkeeping + cell ranges (one contiguous region)
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
     T* fm = at<T>(history, hs.fm[h->rec]);
@@ -1344,12 +1381,12 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     ledds_prof_start(LEDDS_K_DEM_SORT, st);
     int hb = (n + SORT_THREADS * 8 - 1) / (SORT_THREADS * 8);
     if (hb > ledds_sm_count() * 8) hb = ledds_sm_count() * 8;
-    dem_hist_kernel<<<hb, SORT_THREADS, 0, st>>>(at<uint32_t>(scratch, s.key[0]), n, h->passes,
+    launch_pdl(dem_hist_kernel, dim3(hb), dim3(SORT_THREADS), 0, st, at<uint32_t>(scratch, s.key[0]), n, h->passes,
                                                  at<uint32_t>(scratch, s.hist_digit));
     LEDDS_CHECK_LAUNCH();
     for (int p = 0; p < h->passes; ++p) {
         const int in = p & 1, out = in ^ 1;
-        dem_onesweep_kernel<<<h->tiles, SORT_THREADS, 0, st>>>(
+        launch_pdl(dem_onesweep_kernel, dim3(h->tiles), dim3(SORT_THREADS), 0, st, 
             at<uint32_t>(scratch, s.key[in]), at<uint32_t>(scratch, s.idx[in]), at<uint32_t>(scratch, s.key[out]),
             at<uint32_t>(scratch, s.idx[out]), n, 8 * p, at<uint32_t>(scratch, s.hist_digit) + p * SORT_RADIX,
             at<uint32_t>(scratch, s.tile_state) + (size_t)p * h->tiles * SORT_RADIX,
@@ -1368,10 +1405,10 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     uint32_t* nback = at<uint32_t>(scratch, s.nback);
     uint32_t* off = at<uint32_t>(scratch, s.off);
     ledds_prof_start(LEDDS_K_DEM_GATHER, st);
-    dem_ranges_kernel<<<nb, tb, 0, st>>>(n, skey, sh0, at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp),
+    launch_pdl(dem_ranges_kernel, dim3(nb), dim3(tb), 0, st, n, skey, sh0, at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp),
                                          at<uint2>(scratch, s.cell_range));
     LEDDS_CHECK_LAUNCH();
-    dem_gather_kernel<T><<<nb, tb, 0, st>>>(d, skey, sh0, at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range),
+    launch_pdl(dem_gather_kernel<T>, dim3(nb), dim3(tb), 0, st, d, skey, sh0, at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range),
                                          at<typename Real<T>::v4>(scratch, s.hx), at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
                                          sid, sh, nback);
     ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
@@ -1380,22 +1417,24 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
     const int cb = (n + CONTACT_BLOCK - 1) / CONTACT_BLOCK;
     if (d.bc[0] && d.bc[1] && d.bc[2])
-        dem_detect_kernel<T, false><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+        launch_pdl(dem_detect_kernel<T, false>, dim3(cb), dim3(CONTACT_BLOCK), 0, st, d, skey, at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
                                                                         at<uint2>(scratch, s.cell_range), nfwd, nback, at<uint32_t>(scratch, s.cand), status);
     else
-        dem_detect_kernel<T, true><<<cb, CONTACT_BLOCK, 0, st>>>(d, skey, at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
+        launch_pdl(dem_detect_kernel<T, true>, dim3(cb), dim3(CONTACT_BLOCK), 0, st, d, skey, at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
                                                                        at<uint2>(scratch, s.cell_range), nfwd, nback, at<uint32_t>(scratch, s.cand), status);
     LEDDS_CHECK_LAUNCH();
-    dem_scan_kernel<<<h->scan_tiles, SCAN_THREADS, 0, st>>>(n, (uint32_t)d.maxc, nfwd, nback, off, at<uint32_t>(scratch, s.scan_state),
+    launch_pdl(dem_scan_kernel, dim3(h->scan_tiles), dim3(SCAN_THREADS), 0, st, n, (uint32_t)d.maxc, nfwd, nback, off, at<uint32_t>(scratch, s.scan_state),
                                                             at<uint32_t>(scratch, s.tile_counter) + 4);
     LEDDS_CHECK_LAUNCH();
     const DemEnds E = {at<uint32_t>(scratch, s.end_s), at<uint32_t>(scratch, s.end_t), at<uint32_t>(scratch, s.end_hs),
                        at<uint32_t>(scratch, s.end_ht), at<uint32_t>(scratch, s.end_prev)};
-    dem_fill_kernel<<<cb, CONTACT_BLOCK, (size_t)d.maxc * CONTACT_BLOCK * 12, st>>>(
+    launch_pdl(dem_fill_kernel<T>, dim3(cb), dim3(CONTACT_BLOCK), (size_t)d.maxc * CONTACT_BLOCK * 12, st, 
         n, (uint32_t)d.maxc, nfwd, nback, at<uint32_t>(scratch, s.cand), sid, sh, off, row, fm, at<uint32_t>(history, hs.hq[prev]), E,
         at<uint32_t>(history, hs.hq[nw]), status);
     LEDDS_CHECK_LAUNCH();
-    (h->p.model == 1 ? dem_force_kernel<T, true> : dem_force_kernel<T, false>)<<<(n + FORCE_PB - 1) / FORCE_PB, FORCE_THREADS, 0, st>>>(
+    void (*force_kernel)(const DemDevT<T>, const typename Real<T>::v4*, const T*, const uint32_t*, const DemEnds, const uint32_t*, T*, const T*, T*,
+                         int32_t*, T) = h->p.model == 1 ? dem_force_kernel<T, true> : dem_force_kernel<T, false>;
+    launch_pdl(force_kernel, dim3((n + FORCE_PB - 1) / FORCE_PB), dim3(FORCE_THREADS), 0, st, 
         d, at<typename Real<T>::v4>(scratch, s.xr_s), at<T>(scratch, s.pvw), off, E, sh, fm, at<T>(history, hs.hdt[prev]),
         at<T>(history, hs.hdt[nw]), status, (T)dt_hist);
     ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
