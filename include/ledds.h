@@ -137,6 +137,9 @@ typedef struct {
                                       PAPER.md:968-1001 (A.1)-(A.8); kn, kt are then ignored          */
     double young, poisson;         /* Young's modulus and Poisson ratio of the spheres (model 1)  */
     double young_w, poisson_w;     /* ... of the walls                                            */
+    int sort_every_step;           /* 0: the radix passes of a step are skipped when the cell keys are still in
+                                      order (the sort would be the identity; the result is the same);
+                                      1: always run them (measurement)                             */
 } ledds_dem_params;
 
 /* scratch and history are caller-owned but belong to the handle between calls: the library keeps the particle state

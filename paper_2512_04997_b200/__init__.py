@@ -39,7 +39,7 @@ class DemParams(C.Structure):
                 ("density", C.c_double), ("kn", C.c_double), ("kt", C.c_double), ("restitution", C.c_double),
                 ("mu", C.c_double), ("kn_w", C.c_double), ("kt_w", C.c_double), ("restitution_w", C.c_double),
                 ("mu_w", C.c_double), ("max_contacts", C.c_int), ("model", C.c_int), ("young", C.c_double),
-                ("poisson", C.c_double), ("young_w", C.c_double), ("poisson_w", C.c_double)]
+                ("poisson", C.c_double), ("young_w", C.c_double), ("poisson_w", C.c_double), ("sort_every_step", C.c_int)]
 
 
 class CplParams(C.Structure):
@@ -107,6 +107,7 @@ def dem_params(d) -> DemParams:
     p.model = int(d.get("model", 0))
     p.young = float(d.get("young", 0.0)); p.poisson = float(d.get("poisson", 0.0))
     p.young_w = float(d.get("young_w", p.young)); p.poisson_w = float(d.get("poisson_w", p.poisson))
+    p.sort_every_step = int(d.get("sort_every_step", 0))
     return p
 
 

@@ -116,6 +116,7 @@ struct DemScratch {
     size_t hid;                    // uint32 [n]: caller's particle id of home slot h
     size_t sid;                    // uint32 [n]: caller's particle id at sorted position s (last sort)
     size_t sid_tmp;                // uint32 [n]: the same before the particles of a cell are put into id order
+    size_t skey_f;                 // uint32 [n]: the sorted keys (from the radix passes, or the home keys when those were skipped)
     size_t hx;                     // double4 [n]: (x, y, z, R), home order
     size_t hv, hw, ha, hal;        // double [n][3]: v, w, a, alpha, home order
     size_t pvw;                    // double [n][6]: predictor (v^p, w^p), home order

@@ -242,9 +242,13 @@ __device__ __forceinline__ void dem_cell_of_key(const DemDevT<T>& P, uint32_t ke
 // ------------------------------------------------------------------------------ radix sort
 // All digit histograms in one pass over the keys (smem atomics, then one global add per bin).  The keys arrive in
 // home order, i.e. nearly sorted: the upper digits of a warp's 32 keys are usually all the same, and one lane then
-// adds 32 instead of 32 lanes queueing on one shared-memory word.
+// adds 32 instead of 32 lanes queueing on one shared-memory word.  The same sweep checks whether the keys are still in
+// non-descending order: then this step's sort is the identity (ties inside a cell are put into id order by
+// dem_gather_kernel in any case) and the radix passes return at once -- the rule in a settled bed, where a particle
+// changes its cell once in thousands of steps (the paper's own cell lists are updated incrementally on the same
+// grounds).  ledds_dem_params.sort_every_step = 1 switches that off (measurement).
 __global__ void __launch_bounds__(SORT_THREADS) dem_hist_kernel(const uint32_t* __restrict__ key, int n, int passes,
-                                                               uint32_t* __restrict__ ghist)
+                                                               uint32_t* __restrict__ ghist, uint32_t* __restrict__ unsorted)
 {
     DEM_PDL_ENTER(n);
     __shared__ uint32_t h[4][SORT_RADIX];
@@ -268,6 +272,12 @@ __global__ void __launch_bounds__(SORT_THREADS) dem_hist_kernel(const uint32_t* 
             const uint32_t k = k4[j];
             const unsigned live = __ballot_sync(0xffffffffu, ok);
             if (!live) continue;
+            {   // are the keys still in order (home order = last sorted order)?  Then the sort of this step is the identity.
+                const int i = base + j * 32 + lane;
+                uint32_t pk = __shfl_up_sync(0xffffffffu, k, 1);
+                if (lane == 0) pk = i > 0 ? key[i - 1] : 0u;
+                if (ok && k < pk) *unsorted = 1u;
+            }
             for (int p = 0; p < passes; ++p) {
                 const uint32_t d = (k >> (8 * p)) & 255u;
                 const uint32_t d0 = __shfl_sync(0xffffffffu, d, __ffs(live) - 1);
@@ -295,9 +305,11 @@ __device__ __forceinline__ void st_volatile(uint32_t* p, uint32_t v) { *reinterp
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS) dem_onesweep_kernel(
     const uint32_t* __restrict__ key_in, const uint32_t* __restrict__ val_in, uint32_t* __restrict__ key_out,
     uint32_t* __restrict__ val_out, int n, int shift, const uint32_t* __restrict__ ghist /*[256] of this pass*/,
-    uint32_t* __restrict__ tile_state /*[tiles][256] of this pass*/, uint32_t* __restrict__ ticket)
+    uint32_t* __restrict__ tile_state /*[tiles][256] of this pass*/, uint32_t* __restrict__ ticket,
+    const uint32_t* __restrict__ unsorted, int always)
 {
     DEM_PDL_ENTER(n);
+    if (!always && *unsorted == 0u) return;                     // the keys are in order already (block-uniform)
     __shared__ uint32_t warp_hist[SORT_WARPS][SORT_RADIX];
     __shared__ uint32_t bin_base[SORT_RADIX];
     __shared__ uint32_t tile_start[SORT_RADIX];
@@ -441,10 +453,13 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS) dem_onesweep_ke
 //   dem_ranges_kernel: [start, end) of every cell from the key changes (warp shuffle of neighbouring keys), and the id
 //                      of every particle in key-sorted order
 //   dem_gather_kernel: rank inside the cell by id -> final sorted position; sorted copies of (x, R), ids, home indices
-__global__ void dem_ranges_kernel(int n, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sh0,
+__global__ void dem_ranges_kernel(int n, const uint32_t* __restrict__ key_home, const uint32_t* __restrict__ key_sorted,
+                                  const uint32_t* __restrict__ idx_sorted, const uint32_t* __restrict__ unsorted, int always,
                                   const uint32_t* __restrict__ hid, uint32_t* __restrict__ sid_tmp, uint2* __restrict__ cell_range)
 {
     DEM_PDL_ENTER(n);
+    const bool sorted = always || *unsorted != 0u;              // did the radix passes run?  Else sorted order = home order
+    const uint32_t* skey = sorted ? key_sorted : key_home;
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const bool ok = s < n;
@@ -457,24 +472,28 @@ __global__ void dem_ranges_kernel(int n, const uint32_t* __restrict__ skey, cons
     if (lane == 31 || s == n - 1) next = s < n - 1 ? skey[s + 1] : 0xffffffffu;
     if (s == 0 || prev != key) cell_range[key].x = (uint32_t)s;                    // [x, y) = the particles of the cell
     if (s == n - 1 || next != key) cell_range[key].y = (uint32_t)s + 1u;
-    sid_tmp[s] = hid[sh0[s]];
+    sid_tmp[s] = hid[sorted ? idx_sorted[s] : (uint32_t)s];
 }
 
-// sh0[s] = home index of the particle at key-sorted position s (a nearly sequential read of the home records)
+// idx_sorted[s] = home index of the particle at key-sorted position s (a nearly sequential read of the home records)
 template <typename T>
-__global__ void dem_gather_kernel(const DemDevT<T> P, const uint32_t* __restrict__ skey, const uint32_t* __restrict__ sh0,
-                                  const uint32_t* __restrict__ sid_tmp, const uint2* __restrict__ cell_range,
+__global__ void dem_gather_kernel(const DemDevT<T> P, const uint32_t* __restrict__ key_home, const uint32_t* __restrict__ key_sorted,
+                                  const uint32_t* __restrict__ idx_sorted, const uint32_t* __restrict__ unsorted, int always,
+                                  uint32_t* __restrict__ skey_f, const uint32_t* __restrict__ sid_tmp, const uint2* __restrict__ cell_range,
                                   const typename Real<T>::v4* __restrict__ hx, typename Real<T>::v4* __restrict__ xr_s, float4* __restrict__ xf_s,
                                   uint32_t* __restrict__ sid, uint32_t* __restrict__ sh, uint32_t* __restrict__ nback)
 {
     DEM_PDL_ENTER(P.n);
     const int s0 = blockIdx.x * blockDim.x + threadIdx.x;
     if (s0 >= P.n) return;
-    const uint2 cr = cell_range[skey[s0]];
+    const bool sorted = always || *unsorted != 0u;
+    const uint32_t key = sorted ? key_sorted[s0] : key_home[s0];
+    const uint2 cr = cell_range[key];
     const uint32_t id = sid_tmp[s0];
     uint32_t s = cr.x;
     for (uint32_t t = cr.x; t < cr.y; ++t) s += sid_tmp[t] < id;                   // ids are distinct
-    const uint32_t h = sh0[s0];
+    const uint32_t h = sorted ? idx_sorted[s0] : (uint32_t)s0;
+    skey_f[s] = key;                                                               // the sorted keys, whichever way they came
     const typename Real<T>::v2* src = reinterpret_cast<const typename Real<T>::v2*>(hx + h);
     const typename Real<T>::v2 a = __ldg(src), b = __ldg(src + 1);
     xr_s[s] = Real<T>::make4(a.x, a.y, b.x, b.y);
@@ -1225,7 +1244,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h, size_t es)
     s.scan_state = take(((size_t)h->scan_tiles + 1) * 4);
     s.cell_range = take((size_t)d.ncell * 8);
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
-    s.hid = take(n * 4); s.sid = take(n * 4); s.sid_tmp = take(n * 4);
+    s.hid = take(n * 4); s.sid = take(n * 4); s.sid_tmp = take(n * 4); s.skey_f = take(n * 4);
     s.hx = take(n * 4 * es);
     s.hv = take(n * 3 * es); s.hw = take(n * 3 * es); s.ha = take(n * 3 * es); s.hal = take(n * 3 * es);
     s.pvw = take(n * 6 * es);
@@ -1381,8 +1400,10 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     ledds_prof_start(LEDDS_K_DEM_SORT, st);
     int hb = (n + SORT_THREADS * 8 - 1) / (SORT_THREADS * 8);
     if (hb > ledds_sm_count() * 8) hb = ledds_sm_count() * 8;
+    uint32_t* unsorted = at<uint32_t>(scratch, s.tile_counter) + 7;          // zeroed with the tickets
+    const int always = h->p.sort_every_step ? 1 : 0;
     launch_pdl(dem_hist_kernel, dim3(hb), dim3(SORT_THREADS), 0, st, at<uint32_t>(scratch, s.key[0]), n, h->passes,
-                                                 at<uint32_t>(scratch, s.hist_digit));
+                                                 at<uint32_t>(scratch, s.hist_digit), unsorted);
     LEDDS_CHECK_LAUNCH();
     for (int p = 0; p < h->passes; ++p) {
         const int in = p & 1, out = in ^ 1;
@@ -1390,27 +1411,29 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
             at<uint32_t>(scratch, s.key[in]), at<uint32_t>(scratch, s.idx[in]), at<uint32_t>(scratch, s.key[out]),
             at<uint32_t>(scratch, s.idx[out]), n, 8 * p, at<uint32_t>(scratch, s.hist_digit) + p * SORT_RADIX,
             at<uint32_t>(scratch, s.tile_state) + (size_t)p * h->tiles * SORT_RADIX,
-            at<uint32_t>(scratch, s.tile_counter) + p);
+            at<uint32_t>(scratch, s.tile_counter) + p, unsorted, always);
         LEDDS_CHECK_LAUNCH();
     }
     ledds_prof_stop(LEDDS_K_DEM_SORT, st);
     h->sorted_buf = h->passes & 1;
     h->sh_buf = 1 - h->sorted_buf;                             // the other idx buffer is free once the last pass is done
     h->have_sort = true;
-    const uint32_t* skey = at<uint32_t>(scratch, s.key[h->sorted_buf]);
-    const uint32_t* sh0 = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
+    const uint32_t* key_home = at<uint32_t>(scratch, s.key[0]);
+    const uint32_t* key_sorted = at<uint32_t>(scratch, s.key[h->sorted_buf]);
+    const uint32_t* idx_sorted = at<uint32_t>(scratch, s.idx[h->sorted_buf]);
+    uint32_t* skey = at<uint32_t>(scratch, s.skey_f);
     uint32_t* sh = at<uint32_t>(scratch, s.idx[h->sh_buf]);
     uint32_t* sid = at<uint32_t>(scratch, s.sid);
     uint32_t* nfwd = at<uint32_t>(scratch, s.nfwd);
     uint32_t* nback = at<uint32_t>(scratch, s.nback);
     uint32_t* off = at<uint32_t>(scratch, s.off);
     ledds_prof_start(LEDDS_K_DEM_GATHER, st);
-    launch_pdl(dem_ranges_kernel, dim3(nb), dim3(tb), 0, st, n, skey, sh0, at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp),
-                                         at<uint2>(scratch, s.cell_range));
+    launch_pdl(dem_ranges_kernel, dim3(nb), dim3(tb), 0, st, n, key_home, key_sorted, idx_sorted, unsorted, always,
+               at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range));
     LEDDS_CHECK_LAUNCH();
-    launch_pdl(dem_gather_kernel<T>, dim3(nb), dim3(tb), 0, st, d, skey, sh0, at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range),
-                                         at<typename Real<T>::v4>(scratch, s.hx), at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s),
-                                         sid, sh, nback);
+    launch_pdl(dem_gather_kernel<T>, dim3(nb), dim3(tb), 0, st, d, key_home, key_sorted, idx_sorted, unsorted, always, skey,
+               at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range), at<typename Real<T>::v4>(scratch, s.hx),
+               at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), sid, sh, nback);
     ledds_prof_stop(LEDDS_K_DEM_GATHER, st);
     LEDDS_CHECK_LAUNCH();
     const int prev = h->cur, nw = 1 - h->cur;
@@ -1554,7 +1577,7 @@ static int dem_query_t(ledds_dem* h, const void* history, const void* scratch, u
         return !dst || cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, st) == cudaSuccess;
     };
     if (!copy(sorted_idx, at<char>(scratch, s.sid), n * 4) ||
-        !copy(sorted_key, at<char>(scratch, s.key[h->sorted_buf]), n * 4))
+        !copy(sorted_key, at<char>(scratch, s.skey_f), n * 4))
         return LEDDS_ECUDA;
     const int tb = 128, nb = ((int)n + tb - 1) / tb;
     if (force || torque) {
