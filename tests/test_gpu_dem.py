@@ -227,3 +227,30 @@ def test_input_contract_violations_are_flagged():
     g = Dem(pd, x, z, z, np.array([0.3, 0.5, 0.4]))
     g.step(1)
     assert int(g.status[0].item()) == 0
+
+
+def test_sort_is_skipped_only_when_it_is_the_identity():
+    # the radix passes of a step return at once when the keys are still in order (ledds.h: sort_every_step).  Fast
+    # particles (a few change their cell every step) and a frozen state, each with the skip and with the passes forced:
+    # ordering, pair list and state must be the oracle's / bit-identical between the two settings
+    from paper_2512_04997_b200 import Dem
+    import oracle
+    pd, x, v, w, R = W.dem_random(21, 2000, box=(14.0, 11.0, 9.0), bc=(0, 1, 0))
+    pd["max_contacts"] = 32
+    for scale in (40.0, 0.0):
+        vv = v * scale
+        o = oracle.Dem(pd, x, vv, w, R)
+        g0, g1 = Dem(pd, x, vv, w, R), Dem(dict(pd, sort_every_step=1), x, vv, w, R)
+        crossed = 0
+        for _ in range(8):
+            key_before = o.key.copy()
+            o.step(); g0.step(); g1.step()
+            crossed += int((o.key != key_before).sum())
+            q0, q1 = g0.query(), g1.query()
+            assert np.array_equal(q0["idx"], o.idx) and np.array_equal(q0["key"], o.key[o.idx])
+            assert np.array_equal(q0["pairs"], o.pairs)
+            for k in ("idx", "key", "pairs", "pair_dt", "F", "M"):
+                assert np.array_equal(q0[k], q1[k]), k
+            s0, s1 = g0.state(), g1.state()
+            assert all(np.array_equal(s0[k], s1[k]) for k in s0)
+        assert (crossed > 20) if scale else (crossed < 20)
