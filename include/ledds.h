@@ -172,6 +172,24 @@ int ledds_dem_query(ledds_dem* h, const void* history, const void* scratch, uint
 
 int ledds_dem_destroy(ledds_dem* h);
 
+/* The cell order of a particle set -- the linear cell index of every particle and the stable radix sort of the ids
+ * by it, PAPER.md:388, 431-439 -- for callers that can neither allocate nor bring a scratch buffer (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  No handle, no workspace: the sort's scratch
+ * is a static device array inside the library (about 4.4 MiB, held by every GPU that loads the library until the
+ * process exits), so n is limited to LEDDS_CELL_ORDER_STATIC_MAX_N; a larger p->n returns LEDDS_ECAPACITY and
+ * nothing is launched.  The call allocates no host or device memory and creates no stream or event.
+ *   p: as for ledds_dem_init (validated in the same way); n, lo, hi, bc and cell decide the result;
+ *   x[3n]: in, device, positions by particle id (a position outside the box takes the nearest cell, as in a step);
+ *   sorted_idx[n], sorted_key[n]: out, device: particle ids ordered by (cell key, id) and their keys -- the same
+ *   arrays ledds_dem_query returns after ledds_dem_init on these positions, bit for bit.
+ * All calls on one device share the static array: calls that overlap on the GPU (different streams, or different
+ * host threads without ordering between their streams) race and give undefined results; calls on one stream, or
+ * ordered by events, are safe.  Works on the current device. */
+#define LEDDS_CELL_ORDER_STATIC_MAX_N 262144
+int ledds_dem_cell_order_static(const ledds_dem_params* p, const double* x, uint32_t* sorted_idx, uint32_t* sorted_key,
+                                void* stream);
+int ledds_dem_cell_order_static_max_n(void);   /* LEDDS_CELL_ORDER_STATIC_MAX_N of the loaded library */
+
 /* Single-precision variant of the DEM calls (the paper runs most of its DEM validations in single precision and shows
  * fp32 next to fp64 energy curves, Appendix B).  Same pipeline and arguments on float
  * arrays; the particle state, the sorted records, the predictor velocities, the contact history and every operation

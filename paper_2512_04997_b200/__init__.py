@@ -22,7 +22,8 @@ ST_CONTACT_OVERFLOW, ST_SOLID_OVERFLOW, ST_COINCIDENT, ST_NONFINITE, ST_RADIUS_R
 EXPORTS = ["ledds_lbm_workspace_bytes", "ledds_lbm_init", "ledds_lbm_import", "ledds_lbm_step", "ledds_lbm_export",
            "ledds_lbm_current", "ledds_lbm_destroy", "ledds_lbm_workspace_bytes_f32", "ledds_lbm_init_f32",
            "ledds_lbm_import_f32", "ledds_lbm_step_f32", "ledds_lbm_export_f32", "ledds_dem_workspace_bytes", "ledds_dem_init", "ledds_dem_step",
-           "ledds_dem_query", "ledds_dem_destroy", "ledds_dem_workspace_bytes_f32", "ledds_dem_init_f32", "ledds_dem_step_f32",
+           "ledds_dem_query", "ledds_dem_destroy", "ledds_dem_cell_order_static", "ledds_dem_cell_order_static_max_n",
+           "ledds_dem_workspace_bytes_f32", "ledds_dem_init_f32", "ledds_dem_step_f32",
            "ledds_dem_query_f32", "ledds_cpl_workspace_bytes", "ledds_cpl_init", "ledds_coupled_step",
            "ledds_coupled_step_f32", "ledds_version",
            "ledds_profile", "ledds_profile_read", "ledds_launch_count"]
@@ -224,6 +225,20 @@ def ledds_dem_query(h, history, scratch, sorted_idx=None, sorted_key=None, pairs
 
 def ledds_dem_destroy(h):
     _lib.ledds_dem_destroy(h)
+
+
+def ledds_dem_cell_order_static_max_n() -> int:
+    return int(_lib.ledds_dem_cell_order_static_max_n())
+
+
+def ledds_dem_cell_order_static(p: DemParams, x, sorted_idx, sorted_key):
+    """(cell key, id) order of the particles at x with the library's static scratch: no workspace, no allocation
+    (include/ledds.h).  Calls that overlap on the GPU race."""
+    rc = _lib.ledds_dem_cell_order_static(C.byref(p), _p(x), _p(sorted_idx), _p(sorted_key), _stream())
+    if rc == -3:
+        raise LeddsError(f"ledds_dem_cell_order_static: n = {p.n} particles exceed the static scratch of the library "
+                         f"({ledds_dem_cell_order_static_max_n()} particles): LEDDS_ECAPACITY")
+    _check(rc, "ledds_dem_cell_order_static")
 
 
 # fp32 set: same calls on float arrays (include/ledds.h)

@@ -1669,3 +1669,100 @@ extern "C" int ledds_dem_destroy(ledds_dem* h)
     delete h;
     return LEDDS_OK;
 }
+
+// ------------------------------------------------------------------------------ cell order without any allocation
+// ledds_dem_cell_order_static (include/ledds.h): the key + radix-sort stage of the pipeline above for callers that can
+// neither allocate nor bring a scratch buffer (graph capture, serving loops).  Its scratch -- digit histograms, tile
+// tickets, look-back descriptors and the ping-pong key / index buffers -- is this file-scope device array; every GPU
+// that loads the library holds its STATIC_SCRATCH_BYTES (about 4.4 MiB) until the process exits.  All calls on a device
+// share it: calls that overlap on the GPU race (see the header).
+#include <mutex>
+
+#define STATIC_MAX_N LEDDS_CELL_ORDER_STATIC_MAX_N
+#define STATIC_MAX_TILES ((STATIC_MAX_N + SORT_TILE - 1) / SORT_TILE)
+#define STATIC_OFF_HIST 0                                                         /* uint32 [4][256]             */
+#define STATIC_OFF_TICKET (STATIC_OFF_HIST + 4 * SORT_RADIX * 4)                  /* uint32 [8] (+ padding)      */
+#define STATIC_OFF_STATE (STATIC_OFF_TICKET + 256)                                /* uint32 [4][max tiles][256]  */
+#define STATIC_OFF_KEY (STATIC_OFF_STATE + 4 * STATIC_MAX_TILES * SORT_RADIX * 4) /* uint32 [2][max n]           */
+#define STATIC_OFF_IDX (STATIC_OFF_KEY + 2 * STATIC_MAX_N * 4)                    /* uint32 [2][max n]           */
+#define STATIC_SCRATCH_BYTES (STATIC_OFF_IDX + 2 * STATIC_MAX_N * 4)
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_SCRATCH_BYTES];
+
+// In host code g_static_scratch is only a stand-in for the symbol: its device address is asked for once per device,
+// with that device current, and kept here.
+#define STATIC_MAX_DEVICES 64
+static unsigned char* g_static_ptr[STATIC_MAX_DEVICES];
+static std::mutex g_static_mutex;
+
+static int dem_static_scratch(unsigned char** out)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return LEDDS_ECUDA;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return LEDDS_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_static_scratch) != cudaSuccess || !p) return LEDDS_ECUDA;
+        g_static_ptr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = g_static_ptr[dev];
+    return LEDDS_OK;
+}
+
+// cell key of every particle from the caller's positions (same expressions as dem_drift_key_kernel), value = id
+__global__ void __launch_bounds__(DRIFT_BLOCK) dem_key_of_x_kernel(const DemDev P, const double* __restrict__ x,
+                                                                   uint32_t* __restrict__ key, uint32_t* __restrict__ idx)
+{
+    const int i = blockIdx.x * DRIFT_BLOCK + threadIdx.x;
+    if (i >= P.n) return;
+    const int cx = dem_cell_coord(P, x[3 * (size_t)i], 0), cy = dem_cell_coord(P, x[3 * (size_t)i + 1], 1),
+              cz = dem_cell_coord(P, x[3 * (size_t)i + 2], 2);
+    key[i] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
+    idx[i] = (uint32_t)i;
+}
+
+extern "C" int ledds_dem_cell_order_static_max_n(void) { return STATIC_MAX_N; }
+
+extern "C" int ledds_dem_cell_order_static(const ledds_dem_params* p, const double* x, uint32_t* sorted_idx,
+                                           uint32_t* sorted_key, void* stream)
+{
+    if (!p) return LEDDS_EINVAL;
+    if (p->n > STATIC_MAX_N) return LEDDS_ECAPACITY;           // the static scratch holds STATIC_MAX_N particles, no more
+    ledds_dem tmp;
+    const int rc = dem_setup(p, &tmp, 8);
+    if (rc) return rc;
+    const int n = p->n;
+    if (n == 0) return LEDDS_OK;
+    if (!x || !sorted_idx || !sorted_key) return LEDDS_EINVAL;
+    if (((uintptr_t)x | (uintptr_t)sorted_idx | (uintptr_t)sorted_key) & 15) return LEDDS_EALIGN;
+    unsigned char* base = nullptr;
+    const int rs = dem_static_scratch(&base);
+    if (rs) return rs;
+    cudaStream_t st = (cudaStream_t)stream;
+    uint32_t* hist = reinterpret_cast<uint32_t*>(base + STATIC_OFF_HIST);
+    uint32_t* ticket = reinterpret_cast<uint32_t*>(base + STATIC_OFF_TICKET);
+    uint32_t* state = reinterpret_cast<uint32_t*>(base + STATIC_OFF_STATE);
+    uint32_t* key[2] = {reinterpret_cast<uint32_t*>(base + STATIC_OFF_KEY), reinterpret_cast<uint32_t*>(base + STATIC_OFF_KEY) + STATIC_MAX_N};
+    uint32_t* idx[2] = {reinterpret_cast<uint32_t*>(base + STATIC_OFF_IDX), reinterpret_cast<uint32_t*>(base + STATIC_OFF_IDX) + STATIC_MAX_N};
+    // the array keeps what the last call left: histograms, tickets and descriptors must start at zero
+    if (cudaMemsetAsync(base + STATIC_OFF_HIST, 0, STATIC_OFF_STATE + (size_t)4 * tmp.tiles * SORT_RADIX * 4, st) != cudaSuccess)
+        return LEDDS_ECUDA;
+    dem_key_of_x_kernel<<<(n + DRIFT_BLOCK - 1) / DRIFT_BLOCK, DRIFT_BLOCK, 0, st>>>(tmp.d, x, key[0], idx[0]);
+    LEDDS_CHECK_LAUNCH();
+    int hb = (n + SORT_THREADS * 8 - 1) / (SORT_THREADS * 8);
+    if (hb > ledds_sm_count() * 8) hb = ledds_sm_count() * 8;
+    uint32_t* unsorted = ticket + 7;
+    dem_hist_kernel<<<hb, SORT_THREADS, 0, st>>>(key[0], n, tmp.passes, hist, unsorted);
+    LEDDS_CHECK_LAUNCH();
+    // the input is in id order and every pass is stable: the result is ordered by (cell key, id) as it stands.  The
+    // last pass writes into the caller's arrays.
+    for (int q = 0; q < tmp.passes; ++q) {
+        const int in = q & 1, out = in ^ 1;
+        const bool last = q == tmp.passes - 1;
+        dem_onesweep_kernel<<<tmp.tiles, SORT_THREADS, 0, st>>>(key[in], idx[in], last ? sorted_key : key[out],
+                                                                last ? sorted_idx : idx[out], n, 8 * q, hist + q * SORT_RADIX,
+                                                                state + (size_t)q * tmp.tiles * SORT_RADIX, ticket + q, unsorted, 1);
+        LEDDS_CHECK_LAUNCH();
+    }
+    return LEDDS_OK;
+}
