@@ -411,8 +411,14 @@ def run_ours(args, rank, world):
             sub["cfg1_dem_gas_2048"] = {"steps_per_s": round(1e3 / ms1, 1), "particle_updates_per_s": round(len(R1) * 1e3 / ms1, 1),
                                          "cuda_graph_steps_per_s": round(1e3 / ms1g, 1),
                                          "cuda_graph_particle_updates_per_s": round(len(R1) * 1e3 / ms1g, 1),
-                                         "status_word": int(g1.status[0].item()), "note": "launch-latency bound: 9 launches + 1 memset per step"}
+                                         "status_word": int(g1.status[0].item()),
+                                         "note": "one launch per step: a cluster of 8 blocks does the whole step (n <= 4096)"}
             del g1
+            g1c = Dem(dict(pd1, no_single_block=1), x1, v1, w1, R1)     # the chain of kernels larger systems take, for comparison
+            g1c.step(50); torch.cuda.synchronize()
+            ms1c = timed(g1c.step, 1000) / 1000
+            sub["cfg1_dem_gas_2048"]["kernel_chain_steps_per_s"] = round(1e3 / ms1c, 1)
+            del g1c
             lb3, cp3, pd3, x3, v3, w3, R3 = W.cfg3_settling()
             gl3 = Lbm(lb3); gd3 = Dem(pd3, x3, v3, w3, R3); g3 = Coupled(gl3, gd3, cp3, float(R3.max()))
             g3.step(20); torch.cuda.synchronize()

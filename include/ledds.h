@@ -140,6 +140,11 @@ typedef struct {
     int sort_every_step;           /* 0: the radix passes of a step are skipped when the cell keys are still in
                                       order (the sort would be the identity; the result is the same);
                                       1: always run them (measurement)                             */
+    int no_single_block;           /* 0: a system of up to 4 096 particles on a grid of up to 32 768 cells is
+                                      stepped by ONE launch per step (a cluster of 8 thread blocks with cluster
+                                      barriers between the phases) instead of twelve dependent launches; same
+                                      results: the order and the lists are unique, the arithmetic is the same;
+                                      1: always the chain of kernels (measurement, tests)          */
 } ledds_dem_params;
 
 /* scratch and history are caller-owned but belong to the handle between calls: the library keeps the particle state

@@ -155,6 +155,7 @@ struct ledds_dem {
     bool have_sort;                // sid / idx[sorted_buf] describe a sort of the current particle set
     int key_bits, passes, tiles, scan_tiles;
     long long steps;
+    bool small_cells_clear;        // single-launch step: cell_range is all-empty (every step leaves it so)
     // fork/join of the contact pipeline beside the lattice kernels of a coupled step (host resources, lazily made)
     cudaStream_t side = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;

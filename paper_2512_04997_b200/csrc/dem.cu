@@ -641,20 +641,18 @@ __device__ __forceinline__ bool dem_touch(const DemDevT<T>& P, const typename Re
 // which differs from run to run); dem_fill_kernel puts every list into the order of the partner ids.
 // (One thread per (particle, row) -- nine times the threads, a ninth of the work each -- was measured and is slower:
 // 0.61 against 0.52 ms in the dense 4 M state, 0.29 against 0.15 ms in the dilute one.)
+// The walk of the particle at sorted position s; returns the number of partners it found itself (nfwd[s]), status bits
+// are or-ed into st.  nback may be global or shared memory (the single-block step keeps it in shared memory).
 template <typename T, bool PERIODIC>
-__global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_kernel(
-    const DemDevT<T> P, const uint32_t* __restrict__ skey, const typename Real<T>::v4* __restrict__ xr_s, const float4* __restrict__ xf_s,
-    const uint2* __restrict__ cell_range, uint32_t* __restrict__ nfwd, uint32_t* __restrict__ nback, uint32_t* __restrict__ cand,
-    int32_t* __restrict__ status)
+__device__ __forceinline__ uint32_t dem_detect_one(
+    const DemDevT<T>& P, const int s, const uint32_t* __restrict__ skey, const typename Real<T>::v4* __restrict__ xr_s,
+    const float4* __restrict__ xf_s, const uint2* __restrict__ cell_range, uint32_t* __restrict__ nback,
+    uint32_t* __restrict__ cand, int& st)
 {
-    DEM_PDL_ENTER(P.n);
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= P.n) return;
     const uint32_t maxc = (uint32_t)P.maxc;
     const uint32_t key = skey[s];
     const typename Real<T>::v4 mine = xr_s[s];
     const float4 minef = xf_s[s];
-    int st = 0;
 
     int c0, c1, c2;
     dem_cell_of_key(P, key, c0, c1, c2);
@@ -746,7 +744,20 @@ __global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_k
         if (mine.w - dist > T(0.0)) own(DEM_WALL + (uint32_t)wl);
     }
     flush();
-    nfwd[s] = nf;
+    return nf;
+}
+
+template <typename T, bool PERIODIC>
+__global__ void __launch_bounds__(CONTACT_BLOCK, DETECT_MIN_BLOCKS) dem_detect_kernel(
+    const DemDevT<T> P, const uint32_t* __restrict__ skey, const typename Real<T>::v4* __restrict__ xr_s, const float4* __restrict__ xf_s,
+    const uint2* __restrict__ cell_range, uint32_t* __restrict__ nfwd, uint32_t* __restrict__ nback, uint32_t* __restrict__ cand,
+    int32_t* __restrict__ status)
+{
+    DEM_PDL_ENTER(P.n);
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.n) return;
+    int st = 0;
+    nfwd[s] = dem_detect_one<T, PERIODIC>(P, s, skey, xr_s, xf_s, cell_range, nback, cand, st);
     if (st) atomicOr(status, st);
 }
 
@@ -838,18 +849,16 @@ __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t 
 #define DEM_NO_PREV 0xffffffffu
 struct DemEnds { uint32_t *s, *t, *hs, *ht, *prev; };   // per contact end, CSR order
 
-template <typename T>
-__global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ nfwd,
-                                                                const uint32_t* __restrict__ nback, const uint32_t* __restrict__ cand,
-                                                                const uint32_t* __restrict__ sid, const uint32_t* __restrict__ sh,
-                                                                const uint32_t* __restrict__ off, uint2* __restrict__ row,
-                                                                T* __restrict__ fm, const uint32_t* __restrict__ hq_prev,
-                                                                const DemEnds E, uint32_t* __restrict__ hq, int32_t* __restrict__ status)
+// The list of the particle at sorted position s.  tq = shared memory, uint2 [maxc][STRIDE] (partner code, partner id)
+// followed by uint32 [maxc][STRIDE] (last step's partner ids); the calling thread owns column `col` of both.
+template <typename T, int STRIDE>
+__device__ __forceinline__ void dem_fill_one(const int n, const uint32_t maxc, const int s, const int col, uint2* tq,
+                                             const uint32_t* __restrict__ nfwd, const uint32_t* __restrict__ nback,
+                                             const uint32_t* __restrict__ cand, const uint32_t* __restrict__ sid,
+                                             const uint32_t* __restrict__ sh, const uint32_t* __restrict__ off,
+                                             uint2* __restrict__ row, T* __restrict__ fm, const uint32_t* __restrict__ hq_prev,
+                                             const DemEnds& E, uint32_t* __restrict__ hq, int32_t* __restrict__ status)
 {
-    DEM_PDL_ENTER(n);
-    extern __shared__ uint2 tq[];                        // uint2 [maxc][CONTACT_BLOCK]: (partner code, partner id); then uint32 [maxc][CONTACT_BLOCK]
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= n) return;
     const uint32_t nf = min(nfwd[s], maxc), nb = min(nback[s], maxc);
     const uint32_t cnt = min(nf + nb, maxc);
     if (nf + nb > maxc) atomicOr(status, LEDDS_ST_CONTACT_OVERFLOW);                // the two ends of the column met
@@ -863,8 +872,8 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
         }
         return;
     }
-    uint2* mine = tq + threadIdx.x;
-    uint32_t* pq = reinterpret_cast<uint32_t*>(tq + (size_t)maxc * CONTACT_BLOCK) + threadIdx.x;   // last step's partner ids
+    uint2* mine = tq + col;
+    uint32_t* pq = reinterpret_cast<uint32_t*>(tq + (size_t)maxc * STRIDE) + col;   // last step's partner ids
     const uint32_t o = off[s];
     // every loop below keeps four independent loads in flight per thread: the partner codes, their ids, last step's
     // ids of this particle; then the ordering runs in shared memory
@@ -877,7 +886,7 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-            if (c0 + j < cnt) mine[(c0 + j) * CONTACT_BLOCK].x = t[j];
+            if (c0 + j < cnt) mine[(c0 + j) * STRIDE].x = t[j];
     }
     for (uint32_t c0 = 0; c0 < old.y; c0 += 4) {
         uint32_t q[4];
@@ -885,24 +894,24 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
         for (int j = 0; j < 4; ++j) q[j] = c0 + j < old.y ? hq_prev[old.x + c0 + j] : 0u;
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-            if (c0 + j < old.y) pq[(c0 + j) * CONTACT_BLOCK] = q[j];
+            if (c0 + j < old.y) pq[(c0 + j) * STRIDE] = q[j];
     }
     for (uint32_t c0 = 0; c0 < cnt; c0 += 4) {
         uint32_t q[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            const uint32_t t = c0 + j < cnt ? mine[(c0 + j) * CONTACT_BLOCK].x : DEM_WALL;
+            const uint32_t t = c0 + j < cnt ? mine[(c0 + j) * STRIDE].x : DEM_WALL;
             q[j] = t >= DEM_WALL ? (uint32_t)n + (t - DEM_WALL) : sid[t];
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j)
-            if (c0 + j < cnt) mine[(c0 + j) * CONTACT_BLOCK].y = q[j];
+            if (c0 + j < cnt) mine[(c0 + j) * STRIDE].y = q[j];
     }
     for (uint32_t c = 1; c < cnt; ++c) {                                            // insertion sort by id
-        const uint2 e = mine[c * CONTACT_BLOCK];
+        const uint2 e = mine[c * STRIDE];
         uint32_t k = c;
-        while (k > 0 && mine[(k - 1) * CONTACT_BLOCK].y > e.y) { mine[k * CONTACT_BLOCK] = mine[(k - 1) * CONTACT_BLOCK]; --k; }
-        mine[k * CONTACT_BLOCK] = e;
+        while (k > 0 && mine[(k - 1) * STRIDE].y > e.y) { mine[k * STRIDE] = mine[(k - 1) * STRIDE]; --k; }
+        mine[k * STRIDE] = e;
     }
     uint32_t k = 0;
     for (uint32_t c0 = 0; c0 < cnt; c0 += 4) {
@@ -910,23 +919,38 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
         uint32_t ht[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
-            e[j] = c0 + j < cnt ? mine[(c0 + j) * CONTACT_BLOCK] : make_uint2(DEM_WALL, 0u);
+            e[j] = c0 + j < cnt ? mine[(c0 + j) * STRIDE] : make_uint2(DEM_WALL, 0u);
             ht[j] = e[j].x >= DEM_WALL ? 0u : sh[e[j].x];
         }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const uint32_t c = c0 + j;
             if (c >= cnt) break;
-            while (k < old.y && pq[k * CONTACT_BLOCK] < e[j].y) ++k;                 // both lists ascend in the partner id
+            while (k < old.y && pq[k * STRIDE] < e[j].y) ++k;                 // both lists ascend in the partner id
             E.s[o + c] = (uint32_t)s;
             E.t[o + c] = e[j].x;
             E.hs[o + c] = h;
             E.ht[o + c] = ht[j];
-            E.prev[o + c] = (k < old.y && pq[k * CONTACT_BLOCK] == e[j].y) ? old.x + k : DEM_NO_PREV;
+            E.prev[o + c] = (k < old.y && pq[k * STRIDE] == e[j].y) ? old.x + k : DEM_NO_PREV;
             hq[o + c] = e[j].y;
         }
     }
     row[h] = make_uint2(o, cnt);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t maxc, const uint32_t* __restrict__ nfwd,
+                                                                const uint32_t* __restrict__ nback, const uint32_t* __restrict__ cand,
+                                                                const uint32_t* __restrict__ sid, const uint32_t* __restrict__ sh,
+                                                                const uint32_t* __restrict__ off, uint2* __restrict__ row,
+                                                                T* __restrict__ fm, const uint32_t* __restrict__ hq_prev,
+                                                                const DemEnds E, uint32_t* __restrict__ hq, int32_t* __restrict__ status)
+{
+    DEM_PDL_ENTER(n);
+    extern __shared__ uint2 tq[];                        // uint2 [maxc][CONTACT_BLOCK] + uint32 [maxc][CONTACT_BLOCK]
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    dem_fill_one<T, CONTACT_BLOCK>(n, maxc, s, (int)threadIdx.x, tq, nfwd, nback, cand, sid, sh, off, row, fm, hq_prev, E, hq, status);
 }
 
 // ------------------------------------------------------------------------------ force
@@ -941,24 +965,15 @@ __global__ void __launch_bounds__(CONTACT_BLOCK) dem_fill_kernel(int n, uint32_t
 // and the sums R_i w_i + R_j w_j, m_i m_j, m_i + m_j commute; no FMA contraction in this file), so F_ij = -F_ji and
 // M_i / R_i = M_j / R_j hold bit for bit, and what the owner with the higher id computes is exactly the negative of the
 // canonical (i < j) evaluation of the oracle.
+// The FORCE_PW particles from sorted position s0 on, by one warp with its own piece of shared memory (s_off, stage, sacc).
 template <typename T, bool HERTZ>
-__global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_kernel(
-    const DemDevT<T> P, const typename Real<T>::v4* __restrict__ xr_s, const T* __restrict__ pvw, const uint32_t* __restrict__ off,
-    const DemEnds E, const uint32_t* __restrict__ sh, T* __restrict__ fm, const T* __restrict__ hdt_prev,
-    T* __restrict__ hdt_new, int32_t* __restrict__ status, T dt_hist)
+__device__ __forceinline__ void dem_force_warp(
+    const DemDevT<T>& P, const int s0, const int lane, uint32_t* s_off, T (*stage)[32], T (*sacc)[FORCE_PW],
+    const typename Real<T>::v4* __restrict__ xr_s, const T* __restrict__ pvw, const uint32_t* __restrict__ off,
+    const DemEnds& E, const uint32_t* __restrict__ sh, T* __restrict__ fm, const T* __restrict__ hdt_prev,
+    T* __restrict__ hdt_new, int32_t* __restrict__ status, const T dt_hist)
 {
-    DEM_PDL_ENTER(P.n);
-    // every warp works on its own FORCE_PW particles with its own piece of shared memory: no block-wide barrier
-    __shared__ uint32_t s_off_all[FORCE_WARPS][FORCE_PW + 1];
-    __shared__ T stage_all[FORCE_WARPS][6][32];
-    __shared__ T sacc_all[FORCE_WARPS][6][FORCE_PW];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int s0 = (blockIdx.x * FORCE_WARPS + warp) * FORCE_PW;
-    if (s0 >= P.n) return;
     const int np = min(FORCE_PW, P.n - s0);
-    uint32_t* s_off = s_off_all[warp];
-    T (*stage)[32] = stage_all[warp];
-    T (*sacc)[FORCE_PW] = sacc_all[warp];
     const uint32_t e_begin = off[s0], e_end = off[s0 + np];
     if (e_begin == e_end) return;                                                   // no contact among these particles (warp-uniform)
     for (int i = lane; i <= np; i += 32) s_off[i] = off[s0 + i];
@@ -1049,6 +1064,265 @@ __global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_ker
         if (!finite) st |= LEDDS_ST_NONFINITE;
     }
     if (st) atomicOr(status, st);
+}
+
+template <typename T, bool HERTZ>
+__global__ void __launch_bounds__(FORCE_THREADS, FORCE_MIN_BLOCKS) dem_force_kernel(
+    const DemDevT<T> P, const typename Real<T>::v4* __restrict__ xr_s, const T* __restrict__ pvw, const uint32_t* __restrict__ off,
+    const DemEnds E, const uint32_t* __restrict__ sh, T* __restrict__ fm, const T* __restrict__ hdt_prev,
+    T* __restrict__ hdt_new, int32_t* __restrict__ status, T dt_hist)
+{
+    DEM_PDL_ENTER(P.n);
+    // every warp works on its own FORCE_PW particles with its own piece of shared memory: no block-wide barrier
+    __shared__ uint32_t s_off_all[FORCE_WARPS][FORCE_PW + 1];
+    __shared__ T stage_all[FORCE_WARPS][6][32];
+    __shared__ T sacc_all[FORCE_WARPS][6][FORCE_PW];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int s0 = (blockIdx.x * FORCE_WARPS + warp) * FORCE_PW;
+    if (s0 >= P.n) return;
+    dem_force_warp<T, HERTZ>(P, s0, lane, s_off_all[warp], stage_all[warp], sacc_all[warp], xr_s, pvw, off, E, sh, fm, hdt_prev,
+                             hdt_new, status, dt_hist);
+}
+
+// ------------------------------------------------------------------------------ small systems: the step in one launch
+// For a few thousand particles every kernel of the chain above runs a few microseconds and the step is bound by its
+// twelve dependent launches (PAPER.md:682-712 has workloads of this size; BASELINE configs[0]: 2 048 spheres).  Here ONE
+// thread-block cluster of SMALL_CTAS blocks (one per SM, 256 or 512 threads each) does the whole step -- [kick] -> drift ->
+// keys -> order -> sorted copies -> detect -> scan -> fill -> force -- on the same arrays of the scratch and history
+// buffers, with cluster barriers (release / acquire: ~0.2 us, the L1 caches are invalidated) where the chain has kernel
+// boundaries, so import / export / query / re-homing and the coupled step see no difference.  (A single block was
+// measured first: 80 us per step for 2 048 spheres, bound by what one SM can move to and from L2.)
+// The order (cell key, id) is reached by a counting sort: particles count themselves into their cells (integer
+// atomics), the cell counts are scanned by the cluster, and the particles of a cell are ranked by id (the ranking of
+// dem_gather_kernel): a unique result, equal to that of the radix passes bit for bit.  Detection, list ordering /
+// history merge and the force evaluation are the device functions of the kernels above (dem_detect_one,
+// dem_fill_one, dem_force_warp), called with the cluster's threads / warps in place of a grid.
+// Used when n <= SMALL_MAX_N and the grid has <= SMALL_MAX_CELLS cells (ledds_dem_params.no_single_block = 0).
+#define SMALL_CTAS 8                          // portable cluster size
+#define SMALL_THREADS 512                     // the most threads a block is launched with (256 for n <= 2 048: all 8 SMs busy)
+#define SMALL_WARPS (SMALL_THREADS / 32)
+#define SMALL_MAX_N 4096                      // measured: 1.2 x the chain of kernels at 4 096 spheres, 1.5 x at 2 048, equal at ~6 000
+#define SMALL_MAX_CELLS 32768
+
+template <typename T>
+struct DemSmallArgs {
+    DemDevT<T> P;
+    typename Real<T>::v4* hx;                // home state
+    T *hv, *hw, *ha, *hal, *pvw;
+    const uint32_t* hid;
+    T* fm;                                   // contact sums of the last evaluation (read by the kick, renewed by fill / force)
+    uint2* row;
+    const T *f_ext, *m_ext;
+    uint32_t *key, *slot;                    // by home index: cell key; arrival number inside the cell
+    uint32_t *htmp, *sid_tmp;                // by position before the ranking inside a cell: home index; id
+    uint2* cell_range;
+    uint32_t *skey, *sid, *sh;               // sorted order: key, id, home index
+    typename Real<T>::v4* xr_s;
+    float4* xf_s;
+    uint32_t *nfwd, *nback, *cand, *off;
+    uint32_t* csum;                          // 2 x SMALL_CTAS words: block totals of the two cluster-wide scans
+    DemEnds E;
+    const uint32_t* hq_prev;
+    uint32_t* hq;
+    const T* hdt_prev;
+    T* hdt_new;
+    int32_t* status;
+    T dt_hist;
+    int kick, drift;
+    int part;                                // bit 0: kick / drift / keys / cell counts; bit 1: everything after
+};
+
+// all threads of the cluster; what they wrote before is visible to all of them after
+__device__ __forceinline__ void small_sync()
+{
+    asm volatile("barrier.cluster.arrive.release;\n\tbarrier.cluster.wait.acquire;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t small_rank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+
+// exclusive prefix of v over the threads of the cluster in the order (block rank, thread), and the total.
+// wsum: SMALL_WARPS words of shared memory; csum: SMALL_CTAS words of global memory, used once per launch.
+__device__ __forceinline__ uint32_t small_cluster_scan(uint32_t v, uint32_t* wsum, uint32_t* csum, uint32_t rank, uint32_t& total)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (int)(blockDim.x >> 5);
+    uint32_t incl = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    __syncthreads();                                          // wsum may still be read from the last scan
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    uint32_t before = 0, btotal = 0;
+    for (int w2 = 0; w2 < nw; ++w2) {
+        const uint32_t c = wsum[w2];
+        if (w2 < warp) before += c;
+        btotal += c;
+    }
+    if (threadIdx.x == 0) csum[rank] = btotal;
+    small_sync();
+    total = 0;
+#pragma unroll
+    for (uint32_t r = 0; r < SMALL_CTAS; ++r) {
+        const uint32_t c = __ldcg(csum + r);
+        if (r < rank) before += c;
+        total += c;
+    }
+    return before + incl - v;
+}
+
+template <typename T, bool HERTZ, bool PERIODIC>
+__global__ void __launch_bounds__(SMALL_THREADS, 1) dem_small_step_kernel(const __grid_constant__ DemSmallArgs<T> A)
+{
+    extern __shared__ __align__(16) unsigned char small_dyn[];
+    __shared__ uint32_t wsum[SMALL_WARPS];
+    const DemDevT<T>& P = A.P;
+    const uint32_t rank = small_rank();
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, n = P.n, ncell = (int)P.ncell;
+    const int nt = (int)blockDim.x, SMALL_TOTAL = SMALL_CTAS * nt, nw = nt >> 5;   // 256 or SMALL_THREADS threads per block
+    const int gtid = (int)rank * nt + tid;
+    const uint32_t maxc = (uint32_t)P.maxc;
+    int st = 0;
+    if (A.part & 1) {
+        // [kick] + drift + predictor + key: the expressions of dem_drift_key_kernel, one thread per particle
+        for (int h = gtid; h < n; h += SMALL_TOTAL) {
+            const typename Real<T>::v4 r = A.hx[h];
+            T xn[3] = {r.x, r.y, r.z};
+            const T R = r.w;
+            const T m = dem_mass(P, R), I = T(0.4) * m * R * R;               // Eq. (21a)
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const size_t e = 3 * (size_t)h + k;
+                T vv = A.hv[e], wv = A.hw[e], av = A.ha[e], alv = A.hal[e];
+                if (A.kick) {
+                    const size_t ie = (A.f_ext || A.m_ext) ? 3 * (size_t)A.hid[h] + k : 0;
+                    const T Fq = A.fm[6 * (size_t)h + k] + (A.f_ext ? A.f_ext[ie] : T(0.0)), Mq = A.fm[6 * (size_t)h + 3 + k] + (A.m_ext ? A.m_ext[ie] : T(0.0));
+                    const T an = Fq / m + P.g[k], aln = Mq / I;                  // Eq. (18b), (19c)
+                    vv = vv + (T(0.5) * P.dt) * (av + an);                               // Eq. (18c)
+                    wv = wv + (T(0.5) * P.dt) * (alv + aln);                             // Eq. (19d)
+                    av = an; alv = aln;
+                    A.hv[e] = vv; A.hw[e] = wv; A.ha[e] = av; A.hal[e] = alv;
+                }
+                if (A.drift) {
+                    A.pvw[6 * (size_t)h + k] = vv + (T(0.5) * P.dt) * av;                // predictor (G11)
+                    A.pvw[6 * (size_t)h + 3 + k] = wv + (T(0.5) * P.dt) * alv;
+                    T xv = xn[k] + P.dt * vv + (T(0.5) * P.dt * P.dt) * av;              // Eq. (18a)
+                    if (!P.bc[k]) {
+                        if (xv >= P.hi[k]) xv -= P.L[k];
+                        else if (xv < P.lo[k]) xv += P.L[k];
+                    }
+                    xn[k] = xv;
+                } else {
+                    A.pvw[6 * (size_t)h + k] = vv;
+                    A.pvw[6 * (size_t)h + 3 + k] = wv;
+                }
+            }
+            if (A.drift) A.hx[h] = Real<T>::make4(xn[0], xn[1], xn[2], r.w);
+            const int cx = dem_cell_coord(P, xn[0], 0), cy = dem_cell_coord(P, xn[1], 1), cz = dem_cell_coord(P, xn[2], 2);
+            const uint32_t key = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
+            A.key[h] = key;
+            A.slot[h] = atomicAdd(&A.cell_range[key].y, 1u);                  // the particle's number among those of its cell
+            if (T(2.0) * r.w > P.hmin) st |= LEDDS_ST_RADIUS_RANGE;          // input contract (include/ledds.h)
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                if (P.bc[a] && !(xn[a] >= P.lo[a] && xn[a] <= P.hi[a])) st |= LEDDS_ST_OUT_OF_BOX;
+        }
+    }
+    if (A.part == 3) small_sync();
+    if (A.part & 2) {
+        // cell counts -> [start, end): every thread sums a contiguous piece of the cells, the cluster scans the sums.
+        // The counts were made by atomics (in L2): they are read past the L1 cache.
+        {
+            const int per = (ncell + SMALL_TOTAL - 1) / SMALL_TOTAL;
+            const int c0 = min(ncell, gtid * per), c1 = min(ncell, c0 + per);
+            uint32_t sum = 0;
+            for (int c = c0; c < c1; ++c) sum += __ldcg(&A.cell_range[c].y);
+            uint32_t total;
+            uint32_t run = small_cluster_scan(sum, wsum, A.csum, rank, total);
+            for (int c = c0; c < c1; ++c) {
+                const uint32_t k = __ldcg(&A.cell_range[c].y);
+                if (k) A.cell_range[c] = make_uint2(run, run + k);
+                run += k;
+            }
+        }
+        small_sync();
+        for (int h = gtid; h < n; h += SMALL_TOTAL) {                         // into the cell, in arrival order
+            const uint32_t p = A.cell_range[A.key[h]].x + A.slot[h];
+            A.sid_tmp[p] = A.hid[h];
+            A.htmp[p] = (uint32_t)h;
+        }
+        small_sync();
+        for (int p = gtid; p < n; p += SMALL_TOTAL) {                         // rank by id inside the cell, sorted copies
+            const uint32_t h = A.htmp[p], key = A.key[h], id = A.sid_tmp[p];
+            const uint2 cr = A.cell_range[key];
+            uint32_t s = cr.x;
+            for (uint32_t t = cr.x; t < cr.y; ++t) s += A.sid_tmp[t] < id;   // ids are distinct
+            A.skey[s] = key;
+            const typename Real<T>::v4 r = A.hx[h];
+            A.xr_s[s] = r;
+            A.sid[s] = id;
+            A.sh[s] = h;
+            A.nback[s] = 0u;
+            const T rx = r.x - P.lo[0], ry = r.y - P.lo[1], rz = r.z - P.lo[2];   // as dem_gather_kernel
+            const bool sane = fabs(rx) <= T(2.0) * P.L[0] && fabs(ry) <= T(2.0) * P.L[1] && fabs(rz) <= T(2.0) * P.L[2];
+            const float qnan = __int_as_float(0x7fc00000);
+            A.xf_s[s] = sane ? make_float4((float)rx, (float)ry, (float)rz, (float)r.w) : make_float4(qnan, qnan, qnan, qnan);
+        }
+        small_sync();
+        for (int s = gtid; s < n; s += SMALL_TOTAL)
+            A.nfwd[s] = dem_detect_one<T, PERIODIC>(P, s, A.skey, A.xr_s, A.xf_s, A.cell_range, A.nback, A.cand, st);
+        small_sync();
+        // the cell ranges have done their work: all cells empty again for the next step's counts (the first step of a
+        // handle finds them cleared by the host)
+        for (int c = gtid; c < ncell; c += SMALL_TOTAL) A.cell_range[c] = make_uint2(0u, 0u);
+        {   // off[s] = sum over s' < s of min(nfwd + nback, maxc), off[n] = total (nback was counted by atomics)
+            const int per = (n + SMALL_TOTAL - 1) / SMALL_TOTAL;
+            const int i0 = min(n, gtid * per), i1 = min(n, i0 + per);
+            uint32_t sum = 0;
+            for (int i = i0; i < i1; ++i) sum += min(A.nfwd[i] + __ldcg(A.nback + i), maxc);
+            uint32_t total;
+            uint32_t run = small_cluster_scan(sum, wsum, A.csum + SMALL_CTAS, rank, total);
+            for (int i = i0; i < i1; ++i) {
+                A.off[i] = run;
+                run += min(A.nfwd[i] + __ldcg(A.nback + i), maxc);
+            }
+            if (gtid == 0) A.off[n] = total;
+        }
+        small_sync();
+        {
+            uint2* tq = reinterpret_cast<uint2*>(small_dyn);
+            for (int s = gtid; s < n; s += SMALL_TOTAL)
+                dem_fill_one<T, SMALL_THREADS>(n, maxc, s, tid, tq, A.nfwd, A.nback, A.cand, A.sid, A.sh, A.off, A.row, A.fm,
+                                               A.hq_prev, A.E, A.hq, A.status);
+        }
+        small_sync();
+        {   // a warp's piece of shared memory: s_off (FORCE_PW + 1 words, padded), stage [6][32], sacc [6][FORCE_PW]
+            constexpr size_t per_warp = 272 + (6 * 32 + 6 * FORCE_PW) * sizeof(T);
+            unsigned char* mine = small_dyn + (size_t)warp * per_warp;
+            uint32_t* s_off = reinterpret_cast<uint32_t*>(mine);
+            T (*stage)[32] = reinterpret_cast<T (*)[32]>(mine + 272);
+            T (*sacc)[FORCE_PW] = reinterpret_cast<T (*)[FORCE_PW]>(mine + 272 + 6 * 32 * sizeof(T));
+            for (int s0 = ((int)rank * nw + warp) * FORCE_PW; s0 < n; s0 += SMALL_CTAS * nw * FORCE_PW) {
+                dem_force_warp<T, HERTZ>(P, s0, lane, s_off, stage, sacc, A.xr_s, A.pvw, A.off, A.E, A.sh, A.fm, A.hdt_prev,
+                                         A.hdt_new, A.status, A.dt_hist);
+                __syncwarp();
+            }
+        }
+    }
+    if (st) atomicOr(A.status, st);
+}
+
+// shared memory a block is launched with: the larger of the fill phase's and the force phase's needs
+template <typename T>
+static size_t dem_small_smem(int maxc)
+{
+    const size_t fill = (size_t)maxc * SMALL_THREADS * 12, force = (size_t)SMALL_WARPS * (272 + (6 * 32 + 6 * FORCE_PW) * sizeof(T));
+    return fill > force ? fill : force;
 }
 
 // ------------------------------------------------------------------------------ kick
@@ -1285,6 +1559,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h, size_t es)
     h->sh_buf = 0;
     h->have_sort = false;
     h->steps = 0;
+    h->small_cells_clear = false;
     return LEDDS_OK;
 }
 
@@ -1352,6 +1627,111 @@ static int dem_export_t(ledds_dem* h, T* x, T* v, T* w, T* a, T* alpha, const vo
     return LEDDS_OK;
 }
 
+// The single-block step (dem_small_step_kernel) in place of the chain of launches below.
+static bool dem_small_ok(const ledds_dem* h)
+{
+    return !h->p.no_single_block && h->d.n <= SMALL_MAX_N && h->d.ncell <= SMALL_MAX_CELLS;
+}
+
+template <typename T, bool HERTZ, bool PERIODIC>
+static int dem_small_launch(const DemSmallArgs<T>& A, cudaStream_t st)
+{
+    static bool sized[64];                                     // per device: the opt-in to > 48 KB of dynamic shared memory
+    const size_t smem = dem_small_smem<T>(A.P.maxc);
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return LEDDS_ECUDA;
+    if (dev < 0 || dev >= 64 || !sized[dev]) {
+        if (cudaFuncSetAttribute(dem_small_step_kernel<T, HERTZ, PERIODIC>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)dem_small_smem<T>(32)) != cudaSuccess)
+            return LEDDS_ECUDA;
+        if (dev >= 0 && dev < 64) sized[dev] = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(SMALL_CTAS); cfg.blockDim = dim3(A.P.n <= SMALL_CTAS * 256 ? 256 : SMALL_THREADS); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = SMALL_CTAS; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, dem_small_step_kernel<T, HERTZ, PERIODIC>, A) != cudaSuccess) return LEDDS_ECUDA;
+    LEDDS_CHECK_LAUNCH();
+    return LEDDS_OK;
+}
+
+template <typename T>
+static int dem_small_advance(ledds_dem* h, void* history, void* scratch, int32_t* status, double dt_hist, bool drift,
+                             cudaStream_t st, bool fork, const DemKickT<T>* kick)
+{
+    const DemScratch& s = h->s;
+    const DemHistory& hs = h->hs;
+    const int prev = h->cur, nw = 1 - h->cur;
+    DemSmallArgs<T> A;
+    A.P = dem_dev<T>(h);
+    A.hx = at<typename Real<T>::v4>(scratch, s.hx);
+    A.hv = at<T>(scratch, s.hv); A.hw = at<T>(scratch, s.hw); A.ha = at<T>(scratch, s.ha); A.hal = at<T>(scratch, s.hal);
+    A.pvw = at<T>(scratch, s.pvw);
+    A.hid = at<uint32_t>(scratch, s.hid);
+    A.fm = at<T>(history, hs.fm[h->rec]);
+    A.row = at<uint2>(history, hs.row[h->rec]);
+    A.f_ext = kick ? kick->f_ext : nullptr;
+    A.m_ext = kick ? kick->m_ext : nullptr;
+    A.key = at<uint32_t>(scratch, s.key[0]); A.slot = at<uint32_t>(scratch, s.idx[0]);
+    A.htmp = at<uint32_t>(scratch, s.key[1]); A.sid_tmp = at<uint32_t>(scratch, s.sid_tmp);
+    A.cell_range = at<uint2>(scratch, s.cell_range);
+    A.skey = at<uint32_t>(scratch, s.skey_f); A.sid = at<uint32_t>(scratch, s.sid); A.sh = at<uint32_t>(scratch, s.idx[1]);
+    A.xr_s = at<typename Real<T>::v4>(scratch, s.xr_s);
+    A.xf_s = at<float4>(scratch, s.xf_s);
+    A.nfwd = at<uint32_t>(scratch, s.nfwd); A.nback = at<uint32_t>(scratch, s.nback);
+    A.cand = at<uint32_t>(scratch, s.cand); A.off = at<uint32_t>(scratch, s.off);
+    A.csum = at<uint32_t>(scratch, s.hist_digit);            // the radix histograms are not used on this path
+    A.E = {at<uint32_t>(scratch, s.end_s), at<uint32_t>(scratch, s.end_t), at<uint32_t>(scratch, s.end_hs),
+           at<uint32_t>(scratch, s.end_ht), at<uint32_t>(scratch, s.end_prev)};
+    A.hq_prev = at<uint32_t>(history, hs.hq[prev]); A.hq = at<uint32_t>(history, hs.hq[nw]);
+    A.hdt_prev = at<T>(history, hs.hdt[prev]); A.hdt_new = at<T>(history, hs.hdt[nw]);
+    A.status = status;
+    A.dt_hist = (T)dt_hist;
+    A.kick = kick ? 1 : 0;
+    A.drift = drift ? 1 : 0;
+    const bool hertz = h->p.model == 1, periodic = !(A.P.bc[0] && A.P.bc[1] && A.P.bc[2]);
+    auto launch = [&](int part, cudaStream_t on) {
+        A.part = part;
+        if (hertz) return periodic ? dem_small_launch<T, true, true>(A, on) : dem_small_launch<T, true, false>(A, on);
+        return periodic ? dem_small_launch<T, false, true>(A, on) : dem_small_launch<T, false, false>(A, on);
+    };
+    if (!h->small_cells_clear) {
+        if (cudaMemsetAsync(A.cell_range, 0, (size_t)A.P.ncell * sizeof(uint2), st) != cudaSuccess) return LEDDS_ECUDA;
+        h->small_cells_clear = true;
+    }
+    int rc;
+    if (!fork) {
+        ledds_prof_start(LEDDS_K_DEM_CONTACT, st);
+        rc = launch(3, st);
+        ledds_prof_stop(LEDDS_K_DEM_CONTACT, st);
+        if (rc) return rc;
+    } else {
+        // drift and keys on the caller's stream (the raster of a coupled step needs the new positions), the rest beside it
+        ledds_prof_start(LEDDS_K_DEM_KEYS, st);
+        rc = launch(1, st);
+        ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
+        if (rc) return rc;
+        if (!h->side && (cudaStreamCreateWithFlags(&h->side, cudaStreamNonBlocking) != cudaSuccess ||
+                         cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+                         cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess))
+            return LEDDS_ECUDA;
+        if (cudaEventRecord(h->ev_fork, st) != cudaSuccess || cudaStreamWaitEvent(h->side, h->ev_fork, 0) != cudaSuccess)
+            return LEDDS_ECUDA;
+        ledds_prof_start(LEDDS_K_DEM_CONTACT, h->side);
+        rc = launch(2, h->side);
+        ledds_prof_stop(LEDDS_K_DEM_CONTACT, h->side);
+        if (rc) return rc;
+        if (cudaEventRecord(h->ev_join, h->side) != cudaSuccess) return LEDDS_ECUDA;
+    }
+    h->sorted_buf = 1;
+    h->sh_buf = 1;                                             // idx[1] = home index of every sorted position
+    h->have_sort = true;
+    h->cur = nw;
+    return LEDDS_OK;
+}
+
 // [kick] -> drift (optional) -> keys -> sort -> gather/ranges -> contacts, all on the home state.  Leaves the contact
 // sums of every particle in history (fm, row) and the contact ends in hq / hdt of the new generation.
 template <typename T>
@@ -1367,6 +1747,7 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     const DemHistory& hs = h->hs;
     const int n = d.n, tb = 128, nb = (n + tb - 1) / tb;
     if (n == 0) { h->cur = 1 - h->cur; return LEDDS_OK; }
+    if (dem_small_ok(h)) return dem_small_advance<T>(h, history, scratch, status, dt_hist, drift, st, fork, kick);
     g_pdl = n <= DEM_PDL_MAX_N;
     // clear sort / scan bookkeeping + cell ranges (one contiguous region)
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;

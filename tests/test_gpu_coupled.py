@@ -7,6 +7,17 @@ import workloads as W
 pytestmark = pytest.mark.gpu
 
 
+@pytest.fixture(params=["one_launch", "kernel_chain"])
+def dem_path(request):
+    """The DEM sub-steps of a small system by the single-launch cluster kernel (drift on the caller's stream, the rest
+    forked beside the lattice kernels) and by the chain of kernels (ledds_dem_params.no_single_block)."""
+    from paper_2512_04997_b200 import Dem
+    old = Dem.NO_SINGLE_BLOCK
+    Dem.NO_SINGLE_BLOCK = 1 if request.param == "kernel_chain" else 0
+    yield request.param
+    Dem.NO_SINGLE_BLOCK = old
+
+
 def both(lbm, cpl, pd, x, v, w, R, u=None):
     import oracle
     from paper_2512_04997_b200 import Coupled, Dem, Lbm
@@ -81,6 +92,7 @@ def test_zero_reach_particle_is_plain_lbm_bit_exact():
     assert np.all(g.f_hyd.cpu().numpy() == 0)
 
 
+@pytest.mark.usefixtures("dem_path")
 def test_shear_suspension_small_with_contacts_and_periodic_wrap():
     # config-4 shaped: periodic x,y, moving z walls, spheres placed by RSA, some across the periodic seam
     lbm, cpl, pd, x, v, w, R, u = W.cfg4_shear(seed=2, n=64, n_part=60, R=4.0)
@@ -102,6 +114,7 @@ def test_shear_suspension_small_with_contacts_and_periodic_wrap():
     assert np.abs(o.F_sf).max() > 0
 
 
+@pytest.mark.usefixtures("dem_path")
 def test_substepping():
     lbm, cpl, pd, x, v, w, R = W.cfg3_settling(shape=(32, 32, 48), R=4.0, z0=5.0, g=2e-3)
     cpl = dict(cpl, n_sub=4); pd = dict(pd, dt=0.25)
@@ -253,6 +266,7 @@ def posed_in_units(L, T, rho_f, origin, n_sub):
     return lbm, cplB, pdB, org + L * x, v * L / T, w / T, R * L
 
 
+@pytest.mark.usefixtures("dem_path")
 @pytest.mark.parametrize("n_sub", [1, 4])
 @pytest.mark.parametrize("units", [(0.5, 0.25, 2.0, (3.0, -1.5, 0.25)), (3.0e-4, 7.0e-4, 998.2, (0.0123, -0.4, 1.7))])
 def test_units_and_origin_of_the_coupling(units, n_sub):
@@ -290,6 +304,7 @@ def test_full_size_config2_settling_20_steps():
     assert o.dem.v[0, 2] < 0 and o.F_sf[0, 2] > 0
 
 
+@pytest.mark.usefixtures("dem_path")
 def test_coupled_100_steps_small():
     # drift between the two implementations shows late: 100 coupled steps of a sheared suspension with contacts,
     # two-solid cells and periodic wrap

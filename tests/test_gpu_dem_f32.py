@@ -15,6 +15,17 @@ import pytest
 import workloads as W
 
 pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True, params=["one_launch", "kernel_chain"])
+def dem_path(request):
+    """Every test of this file runs twice: small systems (n <= 3 072) stepped by the single-launch cluster kernel, and
+    by the chain of kernels that larger systems always take (ledds_dem_params.no_single_block)."""
+    from paper_2512_04997_b200 import Dem
+    old = Dem.NO_SINGLE_BLOCK
+    Dem.NO_SINGLE_BLOCK = 1 if request.param == "kernel_chain" else 0
+    yield request.param
+    Dem.NO_SINGLE_BLOCK = old
 EPS32 = 2.0 ** -24
 f32 = np.float32
 
