@@ -25,6 +25,7 @@
 // FMA contraction.  No Thrust/CUB; no global fp atomics.
 #include <math.h>
 
+#include <algorithm>
 #include <new>
 
 #include "common.cuh"
@@ -1128,8 +1129,9 @@ struct DemSmallArgs {
     T* hdt_new;
     int32_t* status;
     T dt_hist;
-    int kick, drift;
+    int kick, drift;                         // kick: the first step begins with the kick of the step before the launch
     int part;                                // bit 0: kick / drift / keys / cell counts; bit 1: everything after
+    int nsteps;                              // steps in this launch (> 1 only with part = 3 and drift = 1)
 };
 
 // all threads of the cluster; what they wrote before is visible to all of them after
@@ -1188,6 +1190,15 @@ __global__ void __launch_bounds__(SMALL_THREADS, 1) dem_small_step_kernel(const 
     const int gtid = (int)rank * nt + tid;
     const uint32_t maxc = (uint32_t)P.maxc;
     int st = 0;
+    // nsteps > 1 (part = 3 only): that many steps in this one launch; the contact lists and delta_t of a step are the
+    // "previous" ones of the next (the two generations change roles), and every step after the first begins with
+    // the kick that closes the one before it
+    const uint32_t* hq_prev = A.hq_prev;
+    uint32_t* hq = A.hq;
+    const T* hdt_prev = A.hdt_prev;
+    T* hdt_new = A.hdt_new;
+    for (int it = 0; it < A.nsteps; ++it) {
+    const bool kick = it > 0 || A.kick;
     if (A.part & 1) {
         // [kick] + drift + predictor + key: the expressions of dem_drift_key_kernel, one thread per particle
         for (int h = gtid; h < n; h += SMALL_TOTAL) {
@@ -1199,7 +1210,7 @@ __global__ void __launch_bounds__(SMALL_THREADS, 1) dem_small_step_kernel(const 
             for (int k = 0; k < 3; ++k) {
                 const size_t e = 3 * (size_t)h + k;
                 T vv = A.hv[e], wv = A.hw[e], av = A.ha[e], alv = A.hal[e];
-                if (A.kick) {
+                if (kick) {
                     const size_t ie = (A.f_ext || A.m_ext) ? 3 * (size_t)A.hid[h] + k : 0;
                     const T Fq = A.fm[6 * (size_t)h + k] + (A.f_ext ? A.f_ext[ie] : T(0.0)), Mq = A.fm[6 * (size_t)h + 3 + k] + (A.m_ext ? A.m_ext[ie] : T(0.0));
                     const T an = Fq / m + P.g[k], aln = Mq / I;                  // Eq. (18b), (19c)
@@ -1298,7 +1309,7 @@ __global__ void __launch_bounds__(SMALL_THREADS, 1) dem_small_step_kernel(const 
             uint2* tq = reinterpret_cast<uint2*>(small_dyn);
             for (int s = gtid; s < n; s += SMALL_TOTAL)
                 dem_fill_one<T, SMALL_THREADS>(n, maxc, s, tid, tq, A.nfwd, A.nback, A.cand, A.sid, A.sh, A.off, A.row, A.fm,
-                                               A.hq_prev, A.E, A.hq, A.status);
+                                               hq_prev, A.E, hq, A.status);
         }
         small_sync();
         {   // a warp's piece of shared memory: s_off (FORCE_PW + 1 words, padded), stage [6][32], sacc [6][FORCE_PW]
@@ -1308,11 +1319,17 @@ __global__ void __launch_bounds__(SMALL_THREADS, 1) dem_small_step_kernel(const 
             T (*stage)[32] = reinterpret_cast<T (*)[32]>(mine + 272);
             T (*sacc)[FORCE_PW] = reinterpret_cast<T (*)[FORCE_PW]>(mine + 272 + 6 * 32 * sizeof(T));
             for (int s0 = ((int)rank * nw + warp) * FORCE_PW; s0 < n; s0 += SMALL_CTAS * nw * FORCE_PW) {
-                dem_force_warp<T, HERTZ>(P, s0, lane, s_off, stage, sacc, A.xr_s, A.pvw, A.off, A.E, A.sh, A.fm, A.hdt_prev,
-                                         A.hdt_new, A.status, A.dt_hist);
+                dem_force_warp<T, HERTZ>(P, s0, lane, s_off, stage, sacc, A.xr_s, A.pvw, A.off, A.E, A.sh, A.fm, hdt_prev,
+                                         hdt_new, A.status, A.dt_hist);
                 __syncwarp();
             }
         }
+    }
+    if (it + 1 < A.nsteps) {
+        small_sync();                                          // the sums and lists of this step before the next one's kick
+        const uint32_t* q = hq_prev; hq_prev = hq; hq = const_cast<uint32_t*>(q);
+        const T* d = hdt_prev; hdt_prev = hdt_new; hdt_new = const_cast<T*>(d);
+    }
     }
     if (st) atomicOr(A.status, st);
 }
@@ -1657,10 +1674,14 @@ static int dem_small_launch(const DemSmallArgs<T>& A, cudaStream_t st)
     return LEDDS_OK;
 }
 
+// nsteps > 1: that many steps in one launch (no fork); ext = the external force / torque of every kick after the first
 template <typename T>
 static int dem_small_advance(ledds_dem* h, void* history, void* scratch, int32_t* status, double dt_hist, bool drift,
-                             cudaStream_t st, bool fork, const DemKickT<T>* kick)
+                             cudaStream_t st, bool fork, const DemKickT<T>* kick, int nsteps = 1,
+                             const DemKickT<T>* ext = nullptr)
 {
+    if (nsteps > 1 && (fork || !drift)) return LEDDS_EINVAL;
+    if (!ext) ext = kick;
     const DemScratch& s = h->s;
     const DemHistory& hs = h->hs;
     const int prev = h->cur, nw = 1 - h->cur;
@@ -1672,8 +1693,9 @@ static int dem_small_advance(ledds_dem* h, void* history, void* scratch, int32_t
     A.hid = at<uint32_t>(scratch, s.hid);
     A.fm = at<T>(history, hs.fm[h->rec]);
     A.row = at<uint2>(history, hs.row[h->rec]);
-    A.f_ext = kick ? kick->f_ext : nullptr;
-    A.m_ext = kick ? kick->m_ext : nullptr;
+    A.f_ext = ext ? ext->f_ext : nullptr;
+    A.m_ext = ext ? ext->m_ext : nullptr;
+    A.nsteps = nsteps;
     A.key = at<uint32_t>(scratch, s.key[0]); A.slot = at<uint32_t>(scratch, s.idx[0]);
     A.htmp = at<uint32_t>(scratch, s.key[1]); A.sid_tmp = at<uint32_t>(scratch, s.sid_tmp);
     A.cell_range = at<uint2>(scratch, s.cell_range);
@@ -1728,7 +1750,7 @@ static int dem_small_advance(ledds_dem* h, void* history, void* scratch, int32_t
     h->sorted_buf = 1;
     h->sh_buf = 1;                                             // idx[1] = home index of every sorted position
     h->have_sort = true;
-    h->cur = nw;
+    h->cur = (nsteps & 1) ? nw : prev;
     return LEDDS_OK;
 }
 
@@ -1930,9 +1952,14 @@ static int dem_step_t(ledds_dem* h, T* x, T* v, T* w, T* a, T* alpha,
             if (!rc) rc = dem_import_t<T>(h, x, v, w, a, alpha, radius, history, scratch, st);
             if (rc) return rc;
         }
-        rc = dem_advance_t<T>(h, history, scratch, status, h->d.dt, true, st, false, (s > 0 && !rehome) ? &kick : nullptr);
+        const DemKickT<T>* first = (s > 0 && !rehome) ? &kick : nullptr;
+        int batch = 1;                                         // small systems: all steps up to the next re-homing in one launch
+        if (dem_small_ok(h)) batch = std::min(nsteps - s, DEM_REHOME_STEPS - s % DEM_REHOME_STEPS);
+        if (batch > 1) rc = dem_small_advance<T>(h, history, scratch, status, h->d.dt, true, st, false, first, batch, &kick);
+        else rc = dem_advance_t<T>(h, history, scratch, status, h->d.dt, true, st, false, first);
         if (rc) return rc;
-        h->steps++;
+        h->steps += batch;
+        s += batch - 1;
     }
     rc = dem_kick_t<T>(h, f_ext, m_ext, history, scratch, st);
     if (rc) return rc;
