@@ -145,6 +145,10 @@ typedef struct {
                                       barriers between the phases) instead of twelve dependent launches; same
                                       results: the order and the lists are unique, the arithmetic is the same;
                                       1: always the chain of kernels (measurement, tests)          */
+    int cell_order;                /* how the chain of kernels orders the particles by cell: 0 = counting sort over
+                                      the cells when the grid has at most 4 n cells, radix passes over the keys
+                                      otherwise; 1 = always the radix passes; 2 = always the counting sort.  The
+                                      order (cell key, then id) is the same either way, bit for bit  */
 } ledds_dem_params;
 
 /* scratch and history are caller-owned but belong to the handle between calls: the library keeps the particle state

@@ -41,7 +41,7 @@ class DemParams(C.Structure):
                 ("mu", C.c_double), ("kn_w", C.c_double), ("kt_w", C.c_double), ("restitution_w", C.c_double),
                 ("mu_w", C.c_double), ("max_contacts", C.c_int), ("model", C.c_int), ("young", C.c_double),
                 ("poisson", C.c_double), ("young_w", C.c_double), ("poisson_w", C.c_double), ("sort_every_step", C.c_int),
-                ("no_single_block", C.c_int)]
+                ("no_single_block", C.c_int), ("cell_order", C.c_int)]
 
 
 class CplParams(C.Structure):
@@ -111,6 +111,7 @@ def dem_params(d) -> DemParams:
     p.young_w = float(d.get("young_w", p.young)); p.poisson_w = float(d.get("poisson_w", p.poisson))
     p.sort_every_step = int(d.get("sort_every_step", 0))
     p.no_single_block = int(d.get("no_single_block", 0))
+    p.cell_order = int(d.get("cell_order", 0))
     return p
 
 

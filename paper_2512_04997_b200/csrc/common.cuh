@@ -111,6 +111,7 @@ struct DemScratch {
     size_t tile_counter;           // dynamic tile tickets of the sort passes and the scan } before
     size_t tile_state;             // look-back descriptors of the sort (uint32 [4][tiles][256]) } every
     size_t scan_state;             // look-back descriptors of the scan (uint32 [scan tiles])    } step
+    size_t cell_scan_state;        // look-back descriptors of the scan over the cells (counting sort; zeroed too)
     size_t cell_range;             // uint2 [ncell]: [start, end) of the cell in the sorted order, 0,0 when empty (zeroed too)
     size_t key[2], idx[2];         // ping-pong sort buffers: cell key, home index (uint32 [n])
     size_t hid;                    // uint32 [n]: caller's particle id of home slot h
@@ -153,7 +154,8 @@ struct ledds_dem {
     int sorted_buf;                // which key ping-pong buffer holds the sorted keys
     int sh_buf;                    // which idx ping-pong buffer holds the home index of every sorted position
     bool have_sort;                // sid / idx[sorted_buf] describe a sort of the current particle set
-    int key_bits, passes, tiles, scan_tiles;
+    int key_bits, passes, tiles, scan_tiles, cell_tiles;
+    bool counting;                 // order by cell from counting (ncell <= 4 n) instead of radix passes
     long long steps;
     bool small_cells_clear;        // single-launch step: cell_range is all-empty (every step leaves it so)
     // fork/join of the contact pipeline beside the lattice kernels of a coupled step (host resources, lazily made)

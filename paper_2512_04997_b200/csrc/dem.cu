@@ -44,7 +44,7 @@
 #define LOOKBACK 8
 
 #define SCAN_THREADS 256
-#define SCAN_ITEMS 8
+#define SCAN_ITEMS 16            // per thread: 4 096 values per tile, staged in shared memory so that loads and stores are coalesced
 #define SCAN_TILE (SCAN_THREADS * SCAN_ITEMS)
 
 #define DEM_WALL 0xfffffff0u    // partner code of wall wl (0..5) in the contact lists: DEM_WALL + wl
@@ -160,7 +160,8 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
     const DemDevT<T> P, typename Real<T>::v4* __restrict__ hx, T* __restrict__ hv, T* __restrict__ hw, T* __restrict__ ha,
     T* __restrict__ hal, const uint32_t* __restrict__ hid, const T* __restrict__ fm,
     const T* __restrict__ f_ext, const T* __restrict__ m_ext, T* __restrict__ pvw,
-    uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift, int32_t* __restrict__ status)
+    uint32_t* __restrict__ key, uint32_t* __restrict__ idx, int drift, int32_t* __restrict__ status,
+    uint2* __restrict__ cells /* counting sort: .y of a cell counts its particles (NULL: radix sort, idx = home index) */)
 {
     __shared__ T sv[3 * DRIFT_BLOCK], sa[3 * DRIFT_BLOCK];
     const long long e0 = (long long)blockIdx.x * (3 * DRIFT_BLOCK), ne = 3ll * P.n;
@@ -209,8 +210,9 @@ __global__ void __launch_bounds__(DRIFT_BLOCK) dem_drift_key_kernel(
         hx[h] = Real<T>::make4(xn[0], xn[1], xn[2], r.w);
     }
     const int cx = dem_cell_coord(P, xn[0], 0), cy = dem_cell_coord(P, xn[1], 1), cz = dem_cell_coord(P, xn[2], 2);
-    key[h] = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
-    idx[h] = (uint32_t)h;
+    const uint32_t ck = (uint32_t)(cx + P.nc[0] * (cy + P.nc[1] * cz));
+    key[h] = ck;
+    idx[h] = cells ? atomicAdd(&cells[ck].y, 1u) : (uint32_t)h;                  // its number among the particles of its cell
     // input contract (include/ledds.h): 2 R <= cell width, centres inside a walled box
     int st = T(2.0) * r.w > P.hmin ? LEDDS_ST_RADIUS_RANGE : 0;
 #pragma unroll
@@ -444,6 +446,117 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MIN_BLOCKS) dem_onesweep_ke
         key_out[dst] = kk;
         val_out[dst] = stage_val[i];
     }
+}
+
+// ------------------------------------------------------------------------------ counting sort
+// When the grid has about as many cells as there are particles (a packed bed, a pour: ncell <= 4 n) the order by cell
+// comes cheaper from counting than from radix passes over the keys: every particle has counted itself into its cell
+// in the drift kernel (integer atomic, the returned value is its number inside the cell), one chained scan over the
+// CELLS turns the counts into [start, end) -- which is the cell-range table itself, no pass over sorted keys needed
+// -- and one scatter puts (key, home index, id) at start + number.  The order inside a cell is the order of arrival
+// here; dem_gather_kernel ranks the particles of a cell by id as it does after the radix sort, so the final order
+// (cell key, id) is the same, bit for bit.  Same tile / ticket / look-back scheme as dem_scan_kernel below.
+// Chained exclusive scan of one tile of SCAN_TILE values, common to dem_cell_scan_kernel and dem_scan_kernel.  The
+// values were put into sc[] (padded index scan_pad(x), so that a thread's SCAN_ITEMS consecutive values and a warp's
+// 32 consecutive values are both conflict-free); on return sc[scan_pad(x)] = global exclusive prefix of value x and the
+// function's value = global prefix at the end of the tile.  Tiles take tickets (every tile a block waits for is resident
+// or done); a tile publishes its sum at once and the first warp looks back over 32 predecessors per round trip.
+__device__ __forceinline__ int scan_pad(int x) { return x + (x >> 5); }
+#define SCAN_SMEM (SCAN_TILE + SCAN_TILE / 32)
+
+__device__ __forceinline__ uint32_t scan_tile_chained(uint32_t* sc, uint32_t tile, uint32_t* __restrict__ state)
+{
+    __shared__ uint32_t wsum[SCAN_THREADS / 32];
+    __shared__ uint32_t s_excl;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    uint32_t c[SCAN_ITEMS], sum = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { c[i] = sc[scan_pad(tid * SCAN_ITEMS + i)]; sum += c[i]; }
+    uint32_t incl = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    uint32_t before = 0, total = 0;
+#pragma unroll
+    for (int w2 = 0; w2 < SCAN_THREADS / 32; ++w2) {
+        if (w2 < warp) before += wsum[w2];
+        total += wsum[w2];
+    }
+    if (warp == 0) {
+        uint32_t excl = 0;
+        if (tile == 0) {
+            if (lane == 0) st_volatile(state, ST_FLAG_PRE | total);
+        } else {
+            if (lane == 0) st_volatile(state + tile, ST_FLAG_AGG | total);
+            long long t = (long long)tile - 1;
+            for (;;) {
+                const long long i = t - lane;
+                uint32_t sb = i >= 0 ? ld_volatile(state + i) : ST_FLAG_PRE;
+                while (__any_sync(0xffffffffu, (sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0))
+                    if ((sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0) sb = ld_volatile(state + i);
+                const unsigned pre = __ballot_sync(0xffffffffu, (sb & ST_FLAG_PRE) != 0);
+                const int last = pre ? __ffs(pre) - 1 : 31;                         // the nearest predecessor with a full prefix
+                uint32_t v = lane <= last ? (sb & ST_VALUE_MASK) : 0u;
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                excl += v;
+                if (pre) break;
+                t -= 32;
+            }
+            if (lane == 0) st_volatile(state + tile, ST_FLAG_PRE | (excl + total));
+        }
+        if (lane == 0) s_excl = excl;
+    }
+    __syncthreads();
+    uint32_t run = s_excl + before + incl - sum;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) { sc[scan_pad(tid * SCAN_ITEMS + i)] = run; run += c[i]; }
+    __syncthreads();
+    return s_excl + total;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) dem_cell_scan_kernel(int n, uint32_t ncell, uint2* __restrict__ cells,
+                                                                    uint32_t* __restrict__ state, uint32_t* __restrict__ ticket)
+{
+    DEM_PDL_ENTER(n);
+    __shared__ uint32_t sc[SCAN_SMEM];
+    __shared__ uint32_t s_tile;
+    const int tid = threadIdx.x;
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const long long base = (long long)tile * SCAN_TILE;
+#pragma unroll
+    for (int j = 0; j < SCAN_ITEMS; ++j) {                                          // coalesced: a warp reads 32 consecutive cells
+        const int x = j * SCAN_THREADS + tid;
+        sc[scan_pad(x)] = base + x < (long long)ncell ? cells[base + x].y : 0u;
+    }
+    __syncthreads();
+    const uint32_t end = scan_tile_chained(sc, tile, state);
+#pragma unroll
+    for (int j = 0; j < SCAN_ITEMS; ++j) {
+        const int x = j * SCAN_THREADS + tid;
+        const uint32_t start = sc[scan_pad(x)], stop = x + 1 < SCAN_TILE ? sc[scan_pad(x + 1)] : end;
+        if (stop > start) cells[base + x] = make_uint2(start, stop);                // an empty cell stays (0, 0)
+    }
+}
+
+__global__ void dem_scatter_kernel(int n, const uint32_t* __restrict__ key, const uint32_t* __restrict__ slot,
+                                   const uint2* __restrict__ cells, const uint32_t* __restrict__ hid,
+                                   uint32_t* __restrict__ key_sorted, uint32_t* __restrict__ idx_sorted, uint32_t* __restrict__ sid_tmp)
+{
+    DEM_PDL_ENTER(n);
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n) return;
+    const uint32_t k = key[h];
+    const uint32_t p = cells[k].x + slot[h];
+    key_sorted[p] = k;
+    idx_sorted[p] = (uint32_t)h;
+    sid_tmp[p] = hid[h];
 }
 
 // ------------------------------------------------------------------------------ cell ranges + gather
@@ -770,73 +883,26 @@ __global__ void __launch_bounds__(SCAN_THREADS) dem_scan_kernel(int n, uint32_t 
                                                                uint32_t* __restrict__ state, uint32_t* __restrict__ ticket)
 {
     DEM_PDL_ENTER(n);
-    __shared__ uint32_t wsum[SCAN_THREADS / 32];
-    __shared__ uint32_t s_tile, s_excl;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    __shared__ uint32_t sc[SCAN_SMEM];
+    __shared__ uint32_t s_tile;
+    const int tid = threadIdx.x;
     if (tid == 0) s_tile = atomicAdd(ticket, 1u);
     __syncthreads();
     const uint32_t tile = s_tile;
-    const long long first = (long long)tile * SCAN_TILE + (long long)tid * SCAN_ITEMS;
-    uint32_t c[SCAN_ITEMS], sum = 0;
-    static_assert(SCAN_ITEMS == 8, "two 16-byte loads per thread");
-    if (first + SCAN_ITEMS <= n) {                                                  // cnt is 256-byte aligned and first a multiple of 8
-        const uint4 a = reinterpret_cast<const uint4*>(cnt + first)[0], b = reinterpret_cast<const uint4*>(cnt + first)[1];
-        const uint4 a2 = reinterpret_cast<const uint4*>(cnt2 + first)[0], b2 = reinterpret_cast<const uint4*>(cnt2 + first)[1];
-        c[0] = a.x + a2.x; c[1] = a.y + a2.y; c[2] = a.z + a2.z; c[3] = a.w + a2.w;
-        c[4] = b.x + b2.x; c[5] = b.y + b2.y; c[6] = b.z + b2.z; c[7] = b.w + b2.w;
-    } else {
+    const long long base = (long long)tile * SCAN_TILE;
 #pragma unroll
-        for (int i = 0; i < SCAN_ITEMS; ++i) c[i] = first + i < n ? cnt[first + i] + cnt2[first + i] : 0u;
-    }
-#pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) { c[i] = min(c[i], maxc); sum += c[i]; }
-    uint32_t incl = sum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
-    }
-    if (lane == 31) wsum[warp] = incl;
-    __syncthreads();
-    uint32_t before = 0, total = 0;
-#pragma unroll
-    for (int w2 = 0; w2 < SCAN_THREADS / 32; ++w2) {
-        if (w2 < warp) before += wsum[w2];
-        total += wsum[w2];
-    }
-    if (warp == 0) {                                                                // look back 32 predecessors at a time
-        uint32_t excl = 0;
-        if (tile == 0) {
-            if (lane == 0) st_volatile(state, ST_FLAG_PRE | total);
-        } else {
-            if (lane == 0) st_volatile(state + tile, ST_FLAG_AGG | total);
-            long long t = (long long)tile - 1;
-            for (;;) {
-                const long long i = t - lane;
-                uint32_t sb = i >= 0 ? ld_volatile(state + i) : ST_FLAG_PRE;
-                while (__any_sync(0xffffffffu, (sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0))
-                    if ((sb & (ST_FLAG_AGG | ST_FLAG_PRE)) == 0) sb = ld_volatile(state + i);
-                const unsigned pre = __ballot_sync(0xffffffffu, (sb & ST_FLAG_PRE) != 0);
-                const int last = pre ? __ffs(pre) - 1 : 31;                         // the nearest predecessor with a full prefix
-                uint32_t v = lane <= last ? (sb & ST_VALUE_MASK) : 0u;
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-                excl += v;
-                if (pre) break;
-                t -= 32;
-            }
-            if (lane == 0) st_volatile(state + tile, ST_FLAG_PRE | (excl + total));
-        }
-        if (lane == 0) s_excl = excl;
+    for (int j = 0; j < SCAN_ITEMS; ++j) {
+        const int x = j * SCAN_THREADS + tid;
+        sc[scan_pad(x)] = base + x < n ? min(cnt[base + x] + cnt2[base + x], maxc) : 0u;
     }
     __syncthreads();
-    uint32_t run = s_excl + before + incl - sum;
+    const uint32_t end = scan_tile_chained(sc, tile, state);
 #pragma unroll
-    for (int i = 0; i < SCAN_ITEMS; ++i) {
-        if (first + i < n) off[first + i] = run;
-        run += c[i];
-        if (first + i == n - 1) off[n] = run;
+    for (int j = 0; j < SCAN_ITEMS; ++j) {
+        const int x = j * SCAN_THREADS + tid;
+        if (base + x < n) off[base + x] = sc[scan_pad(x)];
     }
+    if (tid == 0 && base + SCAN_TILE >= n) off[n] = end;                            // the last tile
 }
 
 // ------------------------------------------------------------------------------ fill
@@ -1523,6 +1589,9 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h, size_t es)
     h->passes = (bits + 7) / 8;
     h->tiles = (p->n + SORT_TILE - 1) / SORT_TILE;
     h->scan_tiles = (p->n + SCAN_TILE - 1) / SCAN_TILE;
+    h->cell_tiles = (int)((d.ncell + SCAN_TILE - 1) / SCAN_TILE);
+    if (p->cell_order < 0 || p->cell_order > 2) return LEDDS_EINVAL;
+    h->counting = p->cell_order == 2 || (p->cell_order == 0 && (double)d.ncell <= 4.0 * (double)p->n);
 
     const size_t n = (size_t)p->n, ecap = n * (size_t)d.maxc;
     size_t o = 0;
@@ -1533,6 +1602,7 @@ static int dem_setup(const ledds_dem_params* p, ledds_dem* h, size_t es)
     s.tile_counter = take(8 * 4);
     s.tile_state = take((size_t)4 * h->tiles * SORT_RADIX * 4);
     s.scan_state = take(((size_t)h->scan_tiles + 1) * 4);
+    s.cell_scan_state = take(((size_t)h->cell_tiles + 1) * 4);
     s.cell_range = take((size_t)d.ncell * 8);
     for (int b = 0; b < 2; ++b) { s.key[b] = take(n * 4); s.idx[b] = take(n * 4); }
     s.hid = take(n * 4); s.sid = take(n * 4); s.sid_tmp = take(n * 4); s.skey_f = take(n * 4);
@@ -1775,6 +1845,7 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     if (cudaMemsetAsync(at<char>(scratch, s.hist_digit), 0, s.key[0] - s.hist_digit, st) != cudaSuccess) return LEDDS_ECUDA;
     T* fm = at<T>(history, hs.fm[h->rec]);
     uint2* row = at<uint2>(history, hs.row[h->rec]);
+    uint2* const cells = h->counting ? at<uint2>(scratch, s.cell_range) : nullptr;
     ledds_prof_start(LEDDS_K_DEM_KEYS, st);
     {
         const dim3 grid((n + DRIFT_BLOCK - 1) / DRIFT_BLOCK);
@@ -1782,12 +1853,12 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
             dem_drift_key_kernel<T, true><<<grid, DRIFT_BLOCK, 0, st>>>(d, at<typename Real<T>::v4>(scratch, s.hx), at<T>(scratch, s.hv), at<T>(scratch, s.hw),
                                                                       at<T>(scratch, s.ha), at<T>(scratch, s.hal), at<uint32_t>(scratch, s.hid), fm,
                                                                       kick->f_ext, kick->m_ext, at<T>(scratch, s.pvw),
-                                                                      at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status);
+                                                                      at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status, cells);
         else
             dem_drift_key_kernel<T, false><<<grid, DRIFT_BLOCK, 0, st>>>(d, at<typename Real<T>::v4>(scratch, s.hx), at<T>(scratch, s.hv), at<T>(scratch, s.hw),
                                                                        at<T>(scratch, s.ha), at<T>(scratch, s.hal), at<uint32_t>(scratch, s.hid), fm,
                                                                        nullptr, nullptr, at<T>(scratch, s.pvw),
-                                                                       at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status);
+                                                                       at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]), drift ? 1 : 0, status, cells);
     }
     ledds_prof_stop(LEDDS_K_DEM_KEYS, st);
     LEDDS_CHECK_LAUNCH();
@@ -1804,7 +1875,17 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     int hb = (n + SORT_THREADS * 8 - 1) / (SORT_THREADS * 8);
     if (hb > ledds_sm_count() * 8) hb = ledds_sm_count() * 8;
     uint32_t* unsorted = at<uint32_t>(scratch, s.tile_counter) + 7;          // zeroed with the tickets
-    const int always = h->p.sort_every_step ? 1 : 0;
+    const int always = (h->p.sort_every_step || h->counting) ? 1 : 0;
+    if (h->counting) {
+        // counting sort: the drift kernel has counted; cell counts -> cell ranges, then every particle to start + its number
+        launch_pdl(dem_cell_scan_kernel, dim3(h->cell_tiles), dim3(SCAN_THREADS), 0, st, n, (uint32_t)d.ncell, cells,
+                   at<uint32_t>(scratch, s.cell_scan_state), at<uint32_t>(scratch, s.tile_counter) + 5);
+        LEDDS_CHECK_LAUNCH();
+        launch_pdl(dem_scatter_kernel, dim3(nb), dim3(tb), 0, st, n, at<uint32_t>(scratch, s.key[0]), at<uint32_t>(scratch, s.idx[0]),
+                   cells, at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.key[1]), at<uint32_t>(scratch, s.idx[1]),
+                   at<uint32_t>(scratch, s.sid_tmp));
+        LEDDS_CHECK_LAUNCH();
+    } else {
     launch_pdl(dem_hist_kernel, dim3(hb), dim3(SORT_THREADS), 0, st, at<uint32_t>(scratch, s.key[0]), n, h->passes,
                                                  at<uint32_t>(scratch, s.hist_digit), unsorted);
     LEDDS_CHECK_LAUNCH();
@@ -1817,9 +1898,10 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
             at<uint32_t>(scratch, s.tile_counter) + p, unsorted, always);
         LEDDS_CHECK_LAUNCH();
     }
+    }
     ledds_prof_stop(LEDDS_K_DEM_SORT, st);
-    h->sorted_buf = h->passes & 1;
-    h->sh_buf = 1 - h->sorted_buf;                             // the other idx buffer is free once the last pass is done
+    h->sorted_buf = h->counting ? 1 : (h->passes & 1);
+    h->sh_buf = 1 - h->sorted_buf;                             // the other idx buffer is free once the last pass / the scatter is done
     h->have_sort = true;
     const uint32_t* key_home = at<uint32_t>(scratch, s.key[0]);
     const uint32_t* key_sorted = at<uint32_t>(scratch, s.key[h->sorted_buf]);
@@ -1831,9 +1913,11 @@ static int dem_advance_t(ledds_dem* h, void* history, void* scratch, int32_t* st
     uint32_t* nback = at<uint32_t>(scratch, s.nback);
     uint32_t* off = at<uint32_t>(scratch, s.off);
     ledds_prof_start(LEDDS_K_DEM_GATHER, st);
-    launch_pdl(dem_ranges_kernel, dim3(nb), dim3(tb), 0, st, n, key_home, key_sorted, idx_sorted, unsorted, always,
-               at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range));
-    LEDDS_CHECK_LAUNCH();
+    if (!h->counting) {                                        // (the counting sort has made the cell ranges and sid_tmp itself)
+        launch_pdl(dem_ranges_kernel, dim3(nb), dim3(tb), 0, st, n, key_home, key_sorted, idx_sorted, unsorted, always,
+                   at<uint32_t>(scratch, s.hid), at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range));
+        LEDDS_CHECK_LAUNCH();
+    }
     launch_pdl(dem_gather_kernel<T>, dim3(nb), dim3(tb), 0, st, d, key_home, key_sorted, idx_sorted, unsorted, always, skey,
                at<uint32_t>(scratch, s.sid_tmp), at<uint2>(scratch, s.cell_range), at<typename Real<T>::v4>(scratch, s.hx),
                at<typename Real<T>::v4>(scratch, s.xr_s), at<float4>(scratch, s.xf_s), sid, sh, nback);

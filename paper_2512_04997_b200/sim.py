@@ -64,13 +64,14 @@ class Dem:
     """Sphere DEM on the GPU (ledds_dem_*; precision="f32" -> the ledds_dem_*_f32 calls on float arrays).
     State tensors are [n,3] in particle order."""
 
-    NO_SINGLE_BLOCK = 0   # default of ledds_dem_params.no_single_block for parameter dicts that do not name it (tests run both paths)
+    DEFAULTS = {}   # ledds_dem_params switches (no_single_block, cell_order, ...) for parameter dicts that do not name them: tests run every path
 
     def __init__(self, pd: dict, x, v, w, radius, precision="f64"):
         if precision not in ("f64", "f32"):
             raise ValueError(precision)
         self.pd = dict(pd)
-        self.pd.setdefault("no_single_block", Dem.NO_SINGLE_BLOCK)
+        for key, val in Dem.DEFAULTS.items():
+            self.pd.setdefault(key, val)
         self.p = L.dem_params(self.pd)
         self.f32 = precision == "f32"
         dt = self.dtype = torch.float32 if self.f32 else torch.float64

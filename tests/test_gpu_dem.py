@@ -9,15 +9,20 @@ import workloads as W
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(autouse=True, params=["one_launch", "kernel_chain"])
+PATHS = {"one_launch": {}, "chain_radix": {"no_single_block": 1, "cell_order": 1},
+         "chain_counting": {"no_single_block": 1, "cell_order": 2}}
+
+
+@pytest.fixture(autouse=True, params=list(PATHS))
 def dem_path(request):
-    """Every test of this file runs twice: small systems (n <= 3 072) stepped by the single-launch cluster kernel, and
-    by the chain of kernels that larger systems always take (ledds_dem_params.no_single_block)."""
+    """Every test of this file runs on every path of the step: small systems (n <= 4 096) by the single-launch cluster
+    kernel, and the chain of kernels that larger systems take with the order by cell from the radix passes and from
+    the counting sort (ledds_dem_params.no_single_block, cell_order)."""
     from paper_2512_04997_b200 import Dem
-    old = Dem.NO_SINGLE_BLOCK
-    Dem.NO_SINGLE_BLOCK = 1 if request.param == "kernel_chain" else 0
+    old = Dem.DEFAULTS
+    Dem.DEFAULTS = PATHS[request.param]
     yield request.param
-    Dem.NO_SINGLE_BLOCK = old
+    Dem.DEFAULTS = old
 
 
 def both(pd, x, v, w, R):
