@@ -81,3 +81,32 @@ def test_parameter_validation_without_gpu():
     d["n"] = -1
     with pytest.raises(L.LeddsError):
         L.ledds_dem_workspace_bytes(L.dem_params(d))
+
+
+def test_no_load_is_hoisted_above_the_dependent_launch_wait():
+    """The kernels of a DEM step are chained by programmatic dependent launch: a kernel may start while its
+    predecessor still runs and must not read what that one writes before `griddepcontrol.wait` (ACQBULK in SASS).  The
+    compiler is free to hoist loads through `const __restrict__` pointers (LDG.E.CONSTANT) above the wait -- it did so
+    once, for a block-uniform load, and the kernel read a word its predecessor had not written yet.  This checks the
+    machine code of every kernel that waits: no global / generic load, atomic or reduction before the wait."""
+    import shutil, subprocess
+    _lib()
+    obj = os.path.join(ROOT, "paper_2512_04997_b200", "csrc", "dem.o")
+    tool = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    sass = subprocess.run([tool, "-sass", obj], capture_output=True, text=True, check=True).stdout
+    waits, fn, seen, early = 0, None, False, {}
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            fn, seen = m.group(1), False
+            continue
+        if fn is None:
+            continue
+        if "ACQBULK" in line:
+            waits += not seen
+            seen = True
+        elif not seen and re.search(r"\b(LDG|LD\.E|ATOMG|ATOM\.|REDG|RED\.)", line):
+            early.setdefault(fn, []).append(line.strip())
+    assert waits >= 10                                        # the chain: hist, passes, scans, scatter, ranges, gather, detect, fill, force ...
+    hoisted = {f: v for f, v in early.items() if "ACQBULK" in sass.split("Function : " + f, 1)[1].split("Function : ", 1)[0]}
+    assert not hoisted, hoisted
