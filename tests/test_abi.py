@@ -110,3 +110,12 @@ def test_no_load_is_hoisted_above_the_dependent_launch_wait():
     assert waits >= 10                                        # the chain: hist, passes, scans, scatter, ranges, gather, detect, fill, force ...
     hoisted = {f: v for f, v in early.items() if "ACQBULK" in sass.split("Function : " + f, 1)[1].split("Function : ", 1)[0]}
     assert not hoisted, hoisted
+    # the single-launch step exchanges data between its phases through global memory, with cluster barriers in between:
+    # none of its loads may be of the non-coherent kind (which the compiler may move across a barrier and the L1 may
+    # serve from a stale line)
+    clusters = 0
+    for body in sass.split("Function : ")[1:]:
+        if "UCGABAR" in body:
+            clusters += 1
+            assert ".CONSTANT" not in body, body.split("\n", 1)[0]
+    assert clusters >= 8                                      # T x HERTZ x PERIODIC
