@@ -71,26 +71,35 @@ __global__ void __launch_bounds__(256) cpl_beta_classify_kernel(const CplDev C)
     const double dy = (double)((int)floor(o[1]) + ly - C.H) - o[1], dz = (double)((int)floor(o[2]) + lz - C.H) - o[2];
     const double dyz2 = dy * dy + dz * dz;
     const int lane = threadIdx.x & 31;
-    for (int lx = 0; lx < S; ++lx) {
+    // First the whole row by the distance of the cell centres: every sample point lies within 0.45 sqrt(3) = 0.7795 of
+    // its cell's centre, so a centre further than R + 0.78 from the solid's (nearer than R - 0.78) has all its points
+    // outside (inside) whatever the rounding of the point tests (the slack, 6e-4, is twelve orders above it).  The cells
+    // of the shell in between -- two to four of a row -- are remembered in a bit mask and looked at point by point in a
+    // second loop, which runs as often as the lane with the most shell cells needs, not once per cell of the row.
+    for (int lx0 = 0; lx0 < S; lx0 += 64) {                                        // 64 cells of the row at a time (one mask)
+    unsigned long long shell = 0ull;
+    for (int lx = lx0; lx < min(S, lx0 + 64); ++lx) {
+        if (!in) break;
+        const double dx = (double)(fx + lx - C.H) - o[0];
+        const double d2 = dx * dx + dyz2;
+        if (d2 > ro * ro) C.betabox[t * S + lx] = 0.0;
+        else if (ri > 0.0 && d2 < ri * ri) C.betabox[t * S + lx] = 1.0;
+        else shell |= 1ull << (lx - lx0);
+    }
+    while (__any_sync(0xffffffffu, shell != 0ull)) {
+        const bool has = shell != 0ull;
+        const int lx = lx0 + (has ? __ffsll((long long)shell) - 1 : 0);
+        shell &= shell - 1ull;
         const long long cell = t * S + lx;                                         // = (k S^2 + r) S + lx
         double beta = 0.0;
-        if (in) {
-            const double dx = (double)(fx + lx - C.H) - o[0];
-            // every sample point lies within 0.45 sqrt(3) = 0.7795 of the cell centre: a centre further than R + 0.78 from
-            // the solid's (nearer than R - 0.78) has all its points outside (inside) whatever the rounding of the point
-            // tests (the slack, 6e-4, is twelve orders above it); only the shell in between is looked at point by point
-            const double d2 = dx * dx + dyz2;
-            if (d2 > ro * ro) beta = 0.0;
-            else if (ri > 0.0 && d2 < ri * ri) beta = 1.0;
-            else {
-                const double d[3] = {dx, dy, dz};
-                SubdivPoints p;
-                cpl_subdiv_points(d, Rk, p);
-                beta = cpl_beta_classify(p);
-            }
+        if (has) {
+            const double d[3] = {(double)(fx + lx - C.H) - o[0], dy, dz};
+            SubdivPoints p;
+            cpl_subdiv_points(d, Rk, p);
+            beta = cpl_beta_classify(p);
             C.betabox[cell] = beta;
         }
-        const bool todo = in && beta < 0.0;
+        const bool todo = has && beta < 0.0;
         const unsigned m = __ballot_sync(0xffffffffu, todo);                        // one list append per warp
         if (m) {
             const int leader = __ffs(m) - 1;
@@ -99,6 +108,7 @@ __global__ void __launch_bounds__(256) cpl_beta_classify_kernel(const CplDev C)
             base = __shfl_sync(0xffffffffu, base, leader);
             if (todo) C.blist[1 + base + __popc(m & ((1u << lane) - 1u))] = (uint32_t)cell;
         }
+    }
     }
 }
 
