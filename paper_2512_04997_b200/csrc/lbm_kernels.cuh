@@ -137,11 +137,12 @@ struct LbPush {
     // post-collision population v of direction q (a compile-time constant after unrolling); rho = the cell's
     // pre-collision density (moving-wall term, G19).  A cell away from every wall (wmask == 0: all but the outermost
     // layer of a walled axis) takes the first branch for all 19 directions: an index and a store.
-    template <typename T>
+    // NOWALL: the caller has found wmask == 0 for every lane of the warp: no test
+    template <typename T, bool NOWALL = false>
     __device__ __forceinline__ void put(T* __restrict__ fout, const LbmDev& P, int q, T v, T rho) const
     {
         const int cx = lb_cx(q), cy = lb_cy(q), cz = lb_cz(q);
-        if ((wmask & link_mask(q)) == 0u) {
+        if (NOWALL || (wmask & link_mask(q)) == 0u) {
             fout[(I)((I)q * N + rb[cz + 1][cy + 1] + (I)tx[cx + 1])] = v;
         } else {
             T cuw = T(0);                                   // c_q . u_wall summed over the crossed walls

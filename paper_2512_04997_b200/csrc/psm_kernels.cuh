@@ -3,7 +3,7 @@
 #include "lbm_kernels.cuh"
 
 #define PSM_BLOCK 128
-#define PSM_MIN_BLOCKS 5      // resident blocks per SM the collide kernel is compiled for (<= 102 registers)
+#define PSM_MIN_BLOCKS 6      // resident blocks per SM the collide kernel is compiled for (<= 85 registers)
 #define PSM_MIN_BLOCKS_F32 8  // the same for float populations (<= 64 registers)
 #define PSM_EMPTY 0xffffffffu
 
@@ -292,7 +292,7 @@ __device__ __forceinline__ void bgk_collide_stream(const T* sf, T omega, T rho, 
 // so both outputs come from one even part U = sum_k B_k D_k - (1 - B_tot) w+ Pp and one odd part
 // V = sum_k B_k X_k - (1 - B_tot) w- Mm (w+ = w- for BGK): f*_q = a + (U + V), f*_qbar = b + (U - V).
 // D is formed as t_q rho [(k_k - k) + 4.5 (c.u_k - c.u)(c.u_k + c.u)]: no cancellation of the two equilibria.
-template <typename I, bool TRT, typename T>
+template <typename I, bool TRT, bool FAST, typename T>
 __device__ __forceinline__ void psm_collide_stream(const T* sf, T omega, T rho, T ux, T uy, T uz,
                                                    T B0, const T (&uk0)[3], bool two, const T* s2,
                                                    const LbPush<I>& push, T* __restrict__ fout, const LbmDev& P, bool active)
@@ -310,7 +310,7 @@ __device__ __forceinline__ void psm_collide_stream(const T* sf, T omega, T rho, 
         const T f0 = sf[0], wr = T(lb_w(0)) * rho, fe = wr * k0;
         T acc = B0 * (wr * dk0);
         if (two) acc += B1 * (wr * dk1);
-        if (active) push.put(fout, P, 0, f0 + (acc - komega * (f0 - fe)), rho);
+        if (FAST || active) push.template put<T, FAST>(fout, P, 0, f0 + (acc - komega * (f0 - fe)), rho);
     }
 #pragma unroll
     for (int q = 1; q < LEDDS_Q; q += 2) {
@@ -328,9 +328,9 @@ __device__ __forceinline__ void psm_collide_stream(const T* sf, T omega, T rho, 
         }
         U -= komega * (T(0.5) * s - E);                                             // Eq. (33): (1 - B_tot) Omega, BGK / TRT even part
         V -= komega_m * (T(0.5) * d - O);                                           //                               odd part
-        if (active) {
-            push.put(fout, P, q, a + (U + V), rho);                                 // Eq. (32)
-            push.put(fout, P, q + 1, b + (U - V), rho);
+        if (FAST || active) {
+            push.template put<T, FAST>(fout, P, q, a + (U + V), rho);               // Eq. (32)
+            push.template put<T, FAST>(fout, P, q + 1, b + (U - V), rho);
         }
     }
 }
