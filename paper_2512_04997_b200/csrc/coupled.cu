@@ -262,10 +262,11 @@ __global__ void __launch_bounds__(PSM_BLOCK, sizeof(T) == 4 ? PSM_MIN_BLOCKS_F32
         psm_run_reduce(C, id0, ent, rec);
     }
     // a warp all of whose cells are inside the lattice and away from every wall pushes without the per-link wall tests
-    if (__all_sync(0xffffffffu, active && push.wmask == 0u))
-        psm_collide_stream<I, TRT, true>(sf, (T)P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
-    else
-        psm_collide_stream<I, TRT, false>(sf, (T)P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
+    if (__all_sync(0xffffffffu, active && push.wmask == 0u)) {
+        if (!two) psm_collide_stream<I, TRT, true, true>(sf, (T)P.omega, rho, ux, uy, uz, B0, uk0, false, s2col, push, fout, P, active);
+        else psm_collide_stream<I, TRT, true, false>(sf, (T)P.omega, rho, ux, uy, uz, B0, uk0, true, s2col, push, fout, P, active);
+    } else
+        psm_collide_stream<I, TRT, false, false>(sf, (T)P.omega, rho, ux, uy, uz, B0, uk0, two, s2col, push, fout, P, active);
 }
 
 template <typename T, typename I, bool TRT, bool SUBDIV>

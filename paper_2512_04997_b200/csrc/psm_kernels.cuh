@@ -292,11 +292,12 @@ __device__ __forceinline__ void bgk_collide_stream(const T* sf, T omega, T rho, 
 // so both outputs come from one even part U = sum_k B_k D_k - (1 - B_tot) w+ Pp and one odd part
 // V = sum_k B_k X_k - (1 - B_tot) w- Mm (w+ = w- for BGK): f*_q = a + (U + V), f*_qbar = b + (U - V).
 // D is formed as t_q rho [(k_k - k) + 4.5 (c.u_k - c.u)(c.u_k + c.u)]: no cancellation of the two equilibria.
-template <typename I, bool TRT, bool FAST, typename T>
+template <typename I, bool TRT, bool FAST, bool ONE, typename T>
 __device__ __forceinline__ void psm_collide_stream(const T* sf, T omega, T rho, T ux, T uy, T uz,
-                                                   T B0, const T (&uk0)[3], bool two, const T* s2,
+                                                   T B0, const T (&uk0)[3], bool two_, const T* s2,
                                                    const LbPush<I>& push, T* __restrict__ fout, const LbmDev& P, bool active)
 {
+    const bool two = !ONE && two_;                                                  // ONE: the caller knows that no lane has a second solid
     const T k0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
     const T kk0 = T(1) - T(1.5) * (uk0[0] * uk0[0] + uk0[1] * uk0[1] + uk0[2] * uk0[2]);
     const T Bsum = B0 + (two ? s2[0] : T(0));
