@@ -229,6 +229,7 @@ __global__ void __launch_bounds__(PSM_BLOCK, sizeof(T) == 4 ? PSM_MIN_BLOCKS_F32
         const uint2 slot = C.slots[cell];
         id0 = slot.x; id1 = slot.y;
     }
+    const LbPush<I> push(P, x, y, z);                                                 // index work while the populations are in flight
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     T rho, ux, uy, uz;
     {
@@ -237,7 +238,6 @@ __global__ void __launch_bounds__(PSM_BLOCK, sizeof(T) == 4 ? PSM_MIN_BLOCKS_F32
         for (int q = 0; q < LEDDS_Q; ++q) f[q] = sf[q * PSM_BLOCK];
         lb_moments(f, rho, ux, uy, uz);
     }
-    const LbPush<I> push(P, x, y, z);
     if (!__any_sync(0xffffffffu, id0 != PSM_EMPTY)) {
         bgk_collide_stream<I, TRT>(sf, (T)P.omega, rho, ux, uy, uz, push, fout, P, active);
         return;
