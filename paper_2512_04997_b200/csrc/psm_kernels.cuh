@@ -176,7 +176,13 @@ __device__ __forceinline__ void psm_solid_terms(const LbmDev& P, const CplDev& C
         beta = (has && beta > R(0)) ? beta : R(0);
     }
     const R tm = (R)(P.tau - 0.5);
-    B = beta * tm / ((R(1) - beta) + tm);                                            // Eq. (36)
+    {   // Eq. (36).  A lane without a solid (beta = 0) divides a stand-in value instead of 0: a zero numerator sends the
+        // whole warp through the slow path of the division; the lanes with a solid compute exactly beta tm / (1 - beta + tm)
+        const bool on = beta > R(0);
+        const R bb = on ? beta : R(0.5);
+        const R q = bb * tm / ((R(1) - bb) + tm);
+        B = on ? q : R(0);
+    }
     uk[0] = vk[0] + (wk[1] * d[2] - wk[2] * d[1]);                                   // Eq. (35)
     uk[1] = vk[1] + (wk[2] * d[0] - wk[0] * d[2]);
     uk[2] = vk[2] + (wk[0] * d[1] - wk[1] * d[0]);
